@@ -1,0 +1,151 @@
+/* ltv_scan.h - C ABI of the B200-native LTV-scan library (libltvscan.so).
+ *
+ * The data-parallel hot path of CORD-SLS (arxiv 2606.14188): the scan over the planning horizon of a
+ * batched linear time-varying system
+ *
+ *     x_{t+1} = A_t x_t + B_t u_t + c_t ,   t = 0 .. T-1
+ *
+ * "linearizations of the dynamics ... about the nominal trajectory" (Sec. 4.2); "Both (13)
+ * and (14) require dense matrix multiplications serially through the planning horizon.  As such, we use
+ * parallel associative scans on the GPU"; "forward parallel associative scan"
+ * (PAPER.md:177).  Three operations:
+ *
+ *   ltv_scan_rollout               x_1 .. x_T                       PAPER.md:53 eq.(2), :139 eq.(12b)
+ *   ltv_scan_system_response_tube  Phi(t,s) = A_{t-1} ... A_s, s<t  PAPER.md:142 eq.(12c), Z of :150,
+ *                                  (strictly-lower blocks of          recursion shape of :159 eq.(14)
+ *                                  (I - Z A)^{-1}) fused with
+ *                                  r_t = sum_{s<t} |Phi(t,s)| w_s   PAPER.md:147 eq.(12e), box form
+ *   ltv_scan_adjoint               lam_t = A_t^T lam_{t+1} + g_t,   PAPER.md:106-110 eq.(10) chained
+ *                                  dL/du_t = B_t^T lam_{t+1}          over the horizon
+ *
+ * Conventions common to all entry points
+ *   - fp32, dense, contiguous, row-major, batch outermost.  A[b,t,i,j] = d x_{t+1,i} / d x_{t,j}.
+ *   - Pointers documented "device" are CUDA device pointers of the current device, 16-byte aligned.
+ *     Pointers documented "host" are ordinary host pointers (pinned memory recommended).
+ *   - Ownership: the caller owns every buffer (inputs, outputs, workspace).  The library allocates no
+ *     device memory, keeps no state across calls besides cached function attributes, enqueues its work on
+ *     `cuda_stream` (a cudaStream_t passed as void*, NULL = legacy default stream) and returns WITHOUT
+ *     synchronising.  Inputs are never modified; outputs and workspace must not alias inputs or each other.
+ *   - Errors: every entry point returns an ltv_status.  Arguments are validated on the host before
+ *     anything is enqueued (so a failed call has no side effects); nothing throws or aborts.  There is no
+ *     CPU fallback: without an sm_100 device the calls return LTV_ERR_ARCH / LTV_ERR_CUDA.
+ *   - Shape limits: batch, T, n >= 1; m >= 0; n % 4 == 0 (16-byte rows: TMA / 128-bit access); n <= 8192.
+ *     Anything else is LTV_ERR_BAD_DIM (non-positive) or LTV_ERR_UNSUPPORTED_SHAPE.
+ */
+#ifndef LTV_SCAN_H_
+#define LTV_SCAN_H_
+
+#include <stddef.h>
+
+#if defined(__GNUC__)
+#define LTV_API __attribute__((visibility("default")))
+#else
+#define LTV_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  LTV_OK = 0,
+  LTV_ERR_NULL_PTR = 1,            /* a required pointer is NULL                                     */
+  LTV_ERR_BAD_DIM = 2,             /* batch, T, n < 1 or m < 0, or an unknown enum / flag value       */
+  LTV_ERR_UNSUPPORTED_SHAPE = 3,   /* n % 4 != 0, n > 8192, index space overflow                      */
+  LTV_ERR_ALIGNMENT = 4,           /* a device pointer is not 16-byte aligned                         */
+  LTV_ERR_WORKSPACE_TOO_SMALL = 5, /* workspace_bytes < ltv_scan_workspace_bytes(...)                 */
+  LTV_ERR_ARCH = 6,                /* current device is not compute capability 10.x                   */
+  LTV_ERR_CUDA = 7                 /* a CUDA runtime / driver call failed: see ltv_last_cuda_error()  */
+} ltv_status;
+
+/* `op` argument of ltv_scan_workspace_bytes */
+enum { LTV_OP_ROLLOUT = 0, LTV_OP_SYSTEM_RESPONSE_TUBE = 1, LTV_OP_ADJOINT = 2, LTV_OP_PIPELINE_HOST = 3 };
+
+/* `phi_layout` argument.  COLUMN_PACKED (the only layout of this version): the P = T(T-1)/2 blocks of one
+ * item are stored column by column of the block-lower-triangular operator; block (t,s), 0 <= s < t <= T-1,
+ * sits at block index  q(t,s) = s(T-1) - s(s-1)/2 + (t-s-1)  in phi_out[batch, P, n, n].  All blocks with
+ * the same s are therefore one contiguous tall (T-1-s)n x n row-major matrix, which is what lets the
+ * divide-and-conquer combine  Phi(t,s) = Phi(t,mid) Phi(mid,s)  stream its left operand as one matrix. */
+enum { LTV_PHI_COLUMN_PACKED = 0 };
+
+/* Block index q(t,s) of the COLUMN_PACKED layout; -1 if not 0 <= s < t <= T-1.  Pure host arithmetic. */
+LTV_API long long ltv_phi_block_index(int T, int t, int s);
+
+/* Bytes of device workspace the given op needs for these sizes (0 is a valid answer; a NULL workspace is
+ * then accepted).  Returns 0 for invalid arguments.  For LTV_OP_PIPELINE_HOST the figure covers device
+ * staging copies of every input and output of ltv_scan_pipeline_host (including Phi). */
+LTV_API size_t ltv_scan_workspace_bytes(int op, int batch, int T, int n, int m);
+
+/* Rollout  x_{t+1} = A_t x_t + B_t u_t + c_t  (north_star (i)).
+ *   A      device [batch,T,n,n]       required
+ *   B      device [batch,T,n,m]       may be NULL (then u is ignored; the term is zero); also if m == 0
+ *   c      device [batch,T,n]         may be NULL (zero)
+ *   x0     device [batch,n]           required
+ *   u      device [batch,T,m]         may be NULL (zero)
+ *   x_out  device [batch,T,n]         x_out[b,t] = x_{t+1}
+ * One thread-block cluster per item streams A_t through a shared-memory ring (HBM-bound GEMV chain);
+ * the affine term b_t = B_t u_t + c_t is formed on the fly and never written. */
+LTV_API int ltv_scan_rollout(const float* A, const float* B, const float* c, const float* x0, const float* u,
+                     float* x_out, int batch, int T, int n, int m,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* System response + reachable tube (north_star (ii); eq.(12c), :147 eq.(12e)).
+ *   A        device [batch,T,n,n]     required; only A_0 .. A_{T-2} are read
+ *   w        device [batch,T,n]       required; w_s >= 0, only s <= T-2 read
+ *   phi_out  device [batch,P,n,n]     P = T(T-1)/2, layout `phi_layout`; Phi(t,t) = I is not stored
+ *   r_out    device [batch,T,n]       r_0 = 0, r_t = sum_{s<t} |Phi(t,s)| w_s  (element-wise abs)
+ *   flags    must be 0
+ * T == 1 is valid: no blocks, r zero-filled.  Time-parallel schedule: level 0 copies the sub-diagonal
+ * blocks Phi(s+1,s) = A_s; level l = 1..ceil(log2(T-1)) forms, for every aligned segment of 2^l steps with
+ * midpoint mid, all Phi(t,s) = Phi(t,mid) Phi(mid,s), s < mid < t, as one stacked GEMM (3xTF32 on tcgen05
+ * tensor cores for n >= 96, fp32 FMA below) whose epilogue also accumulates |Phi| w_s, so Phi is never
+ * re-read for the tube.  The tube reduction is deterministic (fixed-order partial sums, no atomics). */
+LTV_API int ltv_scan_system_response_tube(const float* A, const float* w, float* phi_out, float* r_out,
+                                  int batch, int T, int n, int phi_layout, unsigned flags,
+                                  void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Adjoint scan (north_star (iii); eq.(10) chained over the horizon) for
+ * L = sum_{t=1}^{T} l_t(x_t), g_t = dl_t/dx_t, lam_{T+1} = 0:
+ *     lam_T = g_T;  lam_t = A_t^T lam_{t+1} + g_t (t = T-1 .. 1);  grad_u[t] = B_t^T lam_{t+1} (t = 0 .. T-1);
+ *     grad_x0 = A_0^T lam_1.
+ *   A            device [batch,T,n,n]   required (A_0 is read only if grad_x0_out != NULL)
+ *   B            device [batch,T,n,m]   required iff grad_u_out != NULL
+ *   g            device [batch,T,n]     required; g[b,t-1] = g_t
+ *   lambda_out   device [batch,T,n]     lambda_out[b,t-1] = lam_t
+ *   grad_u_out   device [batch,T,m]     may be NULL
+ *   grad_x0_out  device [batch,n]       may be NULL */
+LTV_API int ltv_scan_adjoint(const float* A, const float* B, const float* g,
+                     float* lambda_out, float* grad_u_out, float* grad_x0_out,
+                     int batch, int T, int n, int m,
+                     void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* One pass of the whole hot path from HOST buffers: copies A, B, c, x0, u, w, g host->device into
+ * `workspace` (device, >= ltv_scan_workspace_bytes(LTV_OP_PIPELINE_HOST, ...)), runs the three calls above
+ * on `cuda_stream`, copies x, r, lambda, grad_u, grad_x0 device->host and synchronises the stream before
+ * returning.  Phi (11 GB at the benchmark sizes) stays in the workspace on the device, where its consumer
+ * (the tube / constraint tightening) lives, unless phi_host != NULL, in which case it is copied back too.
+ * All *_host pointers are host memory; B, c, u may be NULL as in ltv_scan_rollout; grad_x0_host and
+ * phi_host may be NULL.  *phi_device_out (if not NULL) receives the device address of Phi inside workspace. */
+LTV_API int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float* c_host,
+                           const float* x0_host, const float* u_host, const float* w_host,
+                           const float* g_host,
+                           float* x_host, float* phi_host, float* r_host, float* lambda_host,
+                           float* grad_u_host, float* grad_x0_host,
+                           int batch, int T, int n, int m,
+                           void* workspace, size_t workspace_bytes, void* cuda_stream,
+                           float** phi_device_out);
+
+/* Human-readable name of a status code (static storage). */
+LTV_API const char* ltv_status_string(int status);
+/* cudaError_t (as int) of the last failing CUDA call made by this library in this thread, 0 if none. */
+LTV_API int ltv_last_cuda_error(void);
+/* Library version, major*10000 + minor*100 + patch. */
+LTV_API int ltv_version(void);
+/* Number of kernel launches the library has enqueued since load (all threads); used by bench.py to report
+ * `gpu_launches`. */
+LTV_API unsigned long long ltv_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LTV_SCAN_H_ */

@@ -1,0 +1,171 @@
+"""ctypes binding of libltvscan.so (include/ltv_scan.h).  Argument marshalling ONLY: every step of the path
+runs in the library's CUDA kernels.  torch is used for device memory and the current stream.  There is no
+CPU fallback: if the shared library is missing this module raises at import."""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libltvscan.so")
+
+LTV_OK = 0
+STATUS_NAMES = {
+    0: "LTV_OK", 1: "LTV_ERR_NULL_PTR", 2: "LTV_ERR_BAD_DIM", 3: "LTV_ERR_UNSUPPORTED_SHAPE",
+    4: "LTV_ERR_ALIGNMENT", 5: "LTV_ERR_WORKSPACE_TOO_SMALL", 6: "LTV_ERR_ARCH", 7: "LTV_ERR_CUDA",
+}
+LTV_OP_ROLLOUT, LTV_OP_SYSTEM_RESPONSE_TUBE, LTV_OP_ADJOINT, LTV_OP_PIPELINE_HOST = 0, 1, 2, 3
+LTV_PHI_COLUMN_PACKED = 0
+
+EXPORTS = (
+    "ltv_phi_block_index", "ltv_scan_workspace_bytes", "ltv_scan_rollout", "ltv_scan_system_response_tube",
+    "ltv_scan_adjoint", "ltv_scan_pipeline_host", "ltv_status_string", "ltv_last_cuda_error", "ltv_version",
+    "ltv_launch_count",
+)
+
+
+class LtvError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {STATUS_NAMES.get(status, status)} (cuda error {lib.ltv_last_cuda_error()})")
+
+
+def _load() -> ctypes.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2606_14188_b200.build` "
+            "(nvcc, sm_100a).  There is no CPU fallback.")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, sz, i, fp = ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int, ctypes.c_void_p
+    L.ltv_phi_block_index.restype = ctypes.c_longlong
+    L.ltv_phi_block_index.argtypes = [i, i, i]
+    L.ltv_scan_workspace_bytes.restype = sz
+    L.ltv_scan_workspace_bytes.argtypes = [i, i, i, i, i]
+    L.ltv_scan_rollout.restype = i
+    L.ltv_scan_rollout.argtypes = [fp] * 6 + [i] * 4 + [vp, sz, vp]
+    L.ltv_scan_system_response_tube.restype = i
+    L.ltv_scan_system_response_tube.argtypes = [fp] * 4 + [i] * 4 + [ctypes.c_uint, vp, sz, vp]
+    L.ltv_scan_adjoint.restype = i
+    L.ltv_scan_adjoint.argtypes = [fp] * 6 + [i] * 4 + [vp, sz, vp]
+    L.ltv_scan_pipeline_host.restype = i
+    L.ltv_scan_pipeline_host.argtypes = [fp] * 13 + [i] * 4 + [vp, sz, vp, ctypes.POINTER(ctypes.c_void_p)]
+    L.ltv_status_string.restype = ctypes.c_char_p
+    L.ltv_status_string.argtypes = [i]
+    L.ltv_last_cuda_error.restype = i
+    L.ltv_version.restype = i
+    L.ltv_launch_count.restype = ctypes.c_ulonglong
+    return L
+
+
+lib = _load()
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _dev(t, name, shape):
+    if t is None:
+        return None
+    if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise ValueError(f"{name}: need a contiguous fp32 CUDA tensor")
+    if tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: shape {tuple(t.shape)} != {tuple(shape)}")
+    return t
+
+
+def _stream():
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def ltv_phi_block_index(T: int, t: int, s: int) -> int:
+    return int(lib.ltv_phi_block_index(T, t, s))
+
+
+def ltv_scan_workspace_bytes(op: int, batch: int, T: int, n: int, m: int) -> int:
+    return int(lib.ltv_scan_workspace_bytes(op, batch, T, n, m))
+
+
+def ltv_launch_count() -> int:
+    return int(lib.ltv_launch_count())
+
+
+def ltv_scan_rollout(A, B, c, x0, u, x_out=None):
+    """x_out[b,t] = x_{t+1};  A[batch,T,n,n], B[batch,T,n,m]|None, c[batch,T,n]|None, x0[batch,n], u[batch,T,m]|None."""
+    batch, T, n, _ = A.shape
+    m = 0 if B is None else B.shape[-1]
+    _dev(A, "A", (batch, T, n, n)); _dev(B, "B", (batch, T, n, m)); _dev(c, "c", (batch, T, n))
+    _dev(x0, "x0", (batch, n)); _dev(u, "u", (batch, T, m))
+    if x_out is None:
+        x_out = torch.empty((batch, T, n), device=A.device, dtype=torch.float32)
+    _dev(x_out, "x_out", (batch, T, n))
+    st = lib.ltv_scan_rollout(_ptr(A), _ptr(B), _ptr(c), _ptr(x0), _ptr(u), _ptr(x_out), batch, T, n, m,
+                              None, 0, _stream())
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_rollout")
+    return x_out
+
+
+def ltv_scan_system_response_tube(A, w, phi_out=None, r_out=None, workspace=None):
+    """Returns (phi[batch,P,n,n] COLUMN_PACKED, r[batch,T,n]).  `workspace`: optional uint8 CUDA tensor."""
+    batch, T, n, _ = A.shape
+    P = T * (T - 1) // 2
+    _dev(A, "A", (batch, T, n, n)); _dev(w, "w", (batch, T, n))
+    if phi_out is None:
+        phi_out = torch.empty((batch, P, n, n), device=A.device, dtype=torch.float32)
+    if r_out is None:
+        r_out = torch.empty((batch, T, n), device=A.device, dtype=torch.float32)
+    _dev(phi_out, "phi_out", (batch, P, n, n)); _dev(r_out, "r_out", (batch, T, n))
+    need = ltv_scan_workspace_bytes(LTV_OP_SYSTEM_RESPONSE_TUBE, batch, T, n, 0)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), device=A.device, dtype=torch.uint8)
+    st = lib.ltv_scan_system_response_tube(_ptr(A), _ptr(w), _ptr(phi_out), _ptr(r_out), batch, T, n,
+                                           LTV_PHI_COLUMN_PACKED, 0, _ptr(workspace), workspace.numel(), _stream())
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_system_response_tube")
+    return phi_out, r_out
+
+
+def ltv_scan_adjoint(A, B, g, want_grad_x0=True, lambda_out=None, grad_u_out=None, grad_x0_out=None):
+    """Returns (lam[batch,T,n] with lam[b,t-1] = lam_t, grad_u[batch,T,m]|None, grad_x0[batch,n]|None)."""
+    batch, T, n, _ = A.shape
+    m = 0 if B is None else B.shape[-1]
+    _dev(A, "A", (batch, T, n, n)); _dev(B, "B", (batch, T, n, m)); _dev(g, "g", (batch, T, n))
+    if lambda_out is None:
+        lambda_out = torch.empty((batch, T, n), device=A.device, dtype=torch.float32)
+    if grad_u_out is None and B is not None and m > 0:
+        grad_u_out = torch.empty((batch, T, m), device=A.device, dtype=torch.float32)
+    if grad_x0_out is None and want_grad_x0:
+        grad_x0_out = torch.empty((batch, n), device=A.device, dtype=torch.float32)
+    st = lib.ltv_scan_adjoint(_ptr(A), _ptr(B), _ptr(g), _ptr(lambda_out), _ptr(grad_u_out), _ptr(grad_x0_out),
+                              batch, T, n, m, None, 0, _stream())
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_adjoint")
+    return lambda_out, grad_u_out, grad_x0_out
+
+
+def ltv_scan_pipeline_host(A, B, c, x0, u, w, g, workspace, want_grad_x0=True, phi_host=None, outs=None):
+    """Whole path from HOST (CPU, ideally pinned) fp32 tensors; returns dict of host outputs and the device
+    address of Phi inside `workspace` (a uint8 CUDA tensor of >= workspace_bytes(LTV_OP_PIPELINE_HOST))."""
+    batch, T, n, _ = A.shape
+    m = 0 if B is None else B.shape[-1]
+    for name, t in (("A", A), ("B", B), ("c", c), ("x0", x0), ("u", u), ("w", w), ("g", g), ("phi_host", phi_host)):
+        if t is not None and (t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous()):
+            raise ValueError(f"{name}: need a contiguous fp32 host tensor")
+    if outs is None:
+        pin = torch.cuda.is_available()
+        mk = lambda *s: torch.empty(s, dtype=torch.float32, pin_memory=pin)
+        outs = dict(x=mk(batch, T, n), r=mk(batch, T, n), lam=mk(batch, T, n),
+                    grad_u=mk(batch, T, m) if (B is not None and m > 0) else None,
+                    grad_x0=mk(batch, n) if want_grad_x0 else None)
+    phi_dev = ctypes.c_void_p(0)
+    st = lib.ltv_scan_pipeline_host(_ptr(A), _ptr(B), _ptr(c), _ptr(x0), _ptr(u), _ptr(w), _ptr(g),
+                                    _ptr(outs["x"]), _ptr(phi_host), _ptr(outs["r"]), _ptr(outs["lam"]),
+                                    _ptr(outs["grad_u"]), _ptr(outs["grad_x0"]), batch, T, n, m,
+                                    _ptr(workspace), workspace.numel(), _stream(), ctypes.byref(phi_dev))
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_pipeline_host")
+    outs["phi_device_ptr"] = phi_dev.value
+    return outs

@@ -1,0 +1,280 @@
+// ltv_scan_adjoint: lam_T = g_T; lam_t = A_t^T lam_{t+1} + g_t; grad_u[t] = B_t^T lam_{t+1}; grad_x0 = A_0^T lam_1
+// (eq.(10) chained over the horizon).
+//
+// HBM-bound transposed-GEMV chain.  One cluster per batch item; CTA `rank` owns a band of COLUMNS of every
+// A_t (so that its slice of A_t^T lam needs no cross-CTA reduction).  The band is streamed as
+// [rows x <=256 columns] boxes by 2-D tensor TMA into a shared-memory ring, in reverse time order, by a
+// producer thread that runs ahead of the consumers.  A consumer thread owns four adjacent columns and one
+// residue class of rows, so the inner loop is one 128-bit shared load + one broadcast load + 4 FMA; the
+// row classes are combined through shared memory once per (step, column slab).  The new costate is
+// written into every CTA of the cluster through DSMEM (st.async + mbarrier byte count), as in the rollout.
+#include <cuda.h>
+
+#include "ltv_internal.h"
+#include "ptx.cuh"
+
+namespace ltv {
+
+namespace {
+
+constexpr int kAdjConsThreads = 256;
+constexpr int kAdjThreads = kAdjConsThreads + 64;  // + producer warp + helper warp
+constexpr int kAdjMaxStages = 8;
+
+struct AdjPlan {
+  int bw;      // box width (columns), multiple of 4, <= 256
+  int rcb;     // box rows
+  int stages;
+  int qt, rg;  // quad-threads per row, row groups
+  uint32_t stage_bytes, off_lam, off_red, off_bar, total;
+};
+
+struct AdjParams {
+  const float *A, *B, *g;
+  float *lam_out, *gu_out, *gx0_out;
+  int batch, T, n, m;
+  AdjPlan ap;
+};
+
+__host__ __device__ inline void col_band(int n, int C, int rank, int& j0, int& j1) {
+  const int nq = n >> 2;
+  j0 = 4 * static_cast<int>((static_cast<long long>(nq) * rank) / C);
+  j1 = 4 * static_cast<int>((static_cast<long long>(nq) * (rank + 1)) / C);
+}
+
+__device__ __forceinline__ uint32_t lam_parity(int k) { return static_cast<uint32_t>(k / 3 - (k % 3 == 0 ? 1 : 0)) & 1u; }
+
+__global__ void __launch_bounds__(kAdjThreads, 1)
+adjoint_kernel(const AdjParams p, const __grid_constant__ CUtensorMap tmapA) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  const int C = static_cast<int>(cluster_nctarank());
+  const int rank = static_cast<int>(cluster_ctarank());
+  const int item = blockIdx.x / C;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n = p.n, T = p.T, m = p.m;
+  const AdjPlan& ap = p.ap;
+  int j0, j1;
+  col_band(n, C, rank, j0, j1);
+  const int W = j1 - j0;
+  const int nslab = (W + ap.bw - 1) / ap.bw;
+  const int nrb = (n + ap.rcb - 1) / ap.rcb;
+  const int nstep = (T - 1) + (p.gx0_out ? 1 : 0);  // GEMV steps: A_{T-1} .. A_1 (, A_0)
+
+  float* lambuf = reinterpret_cast<float*>(smem + ap.off_lam);  // [3][n] (three: the helper may lag a step)
+  float* red = reinterpret_cast<float*>(smem + ap.off_red);     // [rg][bw]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + ap.off_bar);
+  uint64_t* full = bars;
+  uint64_t* empty = bars + kAdjMaxStages;   // kAdjConsThreads/32 arrivals
+  uint64_t* lfull = bars + 2 * kAdjMaxStages;  // [3] input costate of step k complete in lambuf[k%3]
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < ap.stages; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], kAdjConsThreads / 32);
+    }
+    mbar_init(&lfull[0], 1);
+    mbar_init(&lfull[1], 1);
+    mbar_init(&lfull[2], 1);
+    fence_mbar_init();
+    tma_prefetch_desc(&tmapA);
+  }
+  // lambuf[0] = lam_T = g_T
+  const float* gT = p.g + (static_cast<size_t>(item) * T + (T - 1)) * n;
+  for (int j = threadIdx.x; j < n; j += kAdjThreads) lambuf[j] = gT[j];
+  __syncthreads();
+  cluster_sync_all();
+
+  // step k = 0 .. nstep-1 multiplies by A_t^T with t = T-1-k; its input costate lam_{t+1} is lambuf[k%3];
+  // barrier lfull[k%3] is used for k = j, j+3, .. except k = 0 (local init): phase index k/3 - (k%3==0)
+  if (warp == kAdjConsThreads / 32) {
+    // ------------------------------------------------------------------ producer
+    if (lane == 0 && W > 0) {
+      const uint64_t pol = l2_policy_evict_first();
+      uint32_t it = 0;
+      for (int k = 0; k < nstep; ++k) {
+        const int t = T - 1 - k;
+        const int row_base = (item * T + t) * n;  // validated on the host to fit in int
+        for (int sl = 0; sl < nslab; ++sl) {
+          for (int rb = 0; rb < nrb; ++rb, ++it) {
+            const int st = it % ap.stages;
+            const uint32_t use = it / ap.stages;
+            if (use > 0) mbar_wait(&empty[st], (use - 1) & 1);
+            mbar_arrive_expect_tx(&full[st], static_cast<uint32_t>(ap.bw) * ap.rcb * 4u);
+            tma_load_2d(smem + static_cast<size_t>(st) * ap.stage_bytes, &tmapA, j0 + sl * ap.bw,
+                        row_base + rb * ap.rcb, &full[st], pol);
+          }
+        }
+      }
+    }
+  } else if (warp == kAdjConsThreads / 32 + 1) {
+    // ------------------------------------------------------------------ helper: outputs + grad_u
+    // at step k (t = T-1-k): wait lam_{t+1}, arm the barrier of lam_t, write lam_{t+1} (own column band),
+    // grad_u[t][l] for l = rank, rank + C, ...
+    for (int k = 0; k < T; ++k) {
+      const int t = T - 1 - k;
+      if (k >= 1) mbar_wait_cluster(&lfull[k % 3], lam_parity(k));
+      if (k + 1 < T && lane == 0) mbar_arrive_expect_tx(&lfull[(k + 1) % 3], static_cast<uint32_t>(n) * 4u);
+      const float* lam = lambuf + (k % 3) * n;
+      float* dst = p.lam_out + (static_cast<size_t>(item) * T + t) * n;  // lam_out[t] = lam_{t+1}
+      for (int j = j0 + lane; j < j1; j += 32) dst[j] = lam[j];
+      if (p.gu_out) {
+        const float* Bt = p.B + (static_cast<size_t>(item) * T + t) * n * m;
+        for (int l = rank; l < m; l += C) {
+          float acc = 0.f;
+          for (int i = lane; i < n; i += 32) acc = fmaf(__ldg(Bt + static_cast<size_t>(i) * m + l), lam[i], acc);
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+          if (lane == 0) p.gu_out[(static_cast<size_t>(item) * T + t) * m + l] = acc;
+        }
+      }
+    }
+  } else {
+    // ------------------------------------------------------------------ consumers
+    const int tid = threadIdx.x;
+    const int q = tid % ap.qt, rgi = tid / ap.qt;
+    const bool active = rgi < ap.rg;
+    uint32_t it = 0;
+    for (int k = 0; k < nstep; ++k) {
+      const int t = T - 1 - k;
+      if (k >= 1) mbar_wait_cluster(&lfull[k % 3], lam_parity(k));
+      const float* lam = lambuf + (k % 3) * n;
+      float* lnext = lambuf + ((k + 1) % 3) * n;
+      uint64_t* lbar = &lfull[(k + 1) % 3];
+      const float* gt = (t >= 1) ? p.g + (static_cast<size_t>(item) * T + (t - 1)) * n : nullptr;
+      for (int sl = 0; sl < nslab; ++sl) {
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int rb = 0; rb < nrb; ++rb, ++it) {
+          const int st = it % ap.stages;
+          mbar_wait(&full[st], (it / ap.stages) & 1);
+          const float* tile = reinterpret_cast<const float*>(smem + static_cast<size_t>(st) * ap.stage_bytes);
+          const int i0 = rb * ap.rcb;
+          const int rk = min(ap.rcb, n - i0);
+          if (active) {
+#pragma unroll 4
+            for (int i = rgi; i < rk; i += ap.rg) {
+              const float4 a = *reinterpret_cast<const float4*>(tile + static_cast<size_t>(i) * ap.bw + 4 * q);
+              const float l = lam[i0 + i];
+              acc.x = fmaf(a.x, l, acc.x);
+              acc.y = fmaf(a.y, l, acc.y);
+              acc.z = fmaf(a.z, l, acc.z);
+              acc.w = fmaf(a.w, l, acc.w);
+            }
+          }
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&empty[st]);
+        }
+        // combine the row classes (fixed order => deterministic) and publish this slab of the costate
+        if (active) *reinterpret_cast<float4*>(red + static_cast<size_t>(rgi) * ap.bw + 4 * q) = acc;
+        named_bar_sync(1, kAdjConsThreads);
+        for (int jj = tid; jj < ap.bw; jj += kAdjConsThreads) {
+          const int col = j0 + sl * ap.bw + jj;
+          if (col < j1) {
+            float v = 0.f;
+            for (int r = 0; r < ap.rg; ++r) v += red[static_cast<size_t>(r) * ap.bw + jj];
+            if (t >= 1) {
+              v += gt[col];
+              for (int cta = 0; cta < C; ++cta) st_async_remote_f32(lnext + col, v, lbar, cta);
+            } else {
+              p.gx0_out[static_cast<size_t>(item) * n + col] = v;
+            }
+          }
+        }
+        named_bar_sync(1, kAdjConsThreads);
+      }
+    }
+  }
+  __syncthreads();
+  cluster_sync_all();
+}
+
+AdjPlan plan_adjoint(int n, int C) {
+  AdjPlan ap{};
+  const int nq = n >> 2;
+  const int wmax = 4 * ((nq + C - 1) / C);
+  ap.bw = wmax < 256 ? wmax : 256;
+  if (ap.bw < 4) ap.bw = 4;
+  ap.qt = ap.bw / 4;
+  ap.rg = kAdjConsThreads / ap.qt;
+  if (ap.rg > 32) ap.rg = 32;
+  int rcb = (32 * 1024) / (ap.bw * 4);
+  if (rcb > 256) rcb = 256;
+  if (rcb > n) rcb = n;
+  if (rcb < 1) rcb = 1;
+  ap.rcb = rcb;
+  ap.stage_bytes = static_cast<uint32_t>(align_up(static_cast<size_t>(ap.bw) * rcb * 4, 128));
+  const uint32_t lam_bytes = static_cast<uint32_t>(align_up(3u * n * 4u, 128));
+  const uint32_t red_bytes = static_cast<uint32_t>(align_up(static_cast<size_t>(ap.rg) * ap.bw * 4, 128));
+  const uint32_t budget = 227u * 1024u - lam_bytes - red_bytes - 256u;
+  int st = static_cast<int>(budget / ap.stage_bytes);
+  if (st > kAdjMaxStages) st = kAdjMaxStages;
+  ap.stages = st;
+  ap.off_lam = ap.stage_bytes * st;
+  ap.off_red = ap.off_lam + lam_bytes;
+  ap.off_bar = ap.off_red + red_bytes;
+  ap.total = ap.off_bar + (2 * kAdjMaxStages + 3) * 8;
+  return ap;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+}  // namespace
+
+// shared with phi.cu
+void* get_encode_tiled() {
+  static void* fn = nullptr;
+  if (!fn) {
+    cudaDriverEntryPointQueryResult q;
+    void* f = nullptr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = f;
+  }
+  return fn;
+}
+
+cudaError_t launch_adjoint(const AdjointArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches) {
+  AdjParams p{};
+  p.A = a.A; p.B = a.B; p.g = a.g;
+  p.lam_out = a.lambda_out; p.gu_out = (a.m > 0) ? a.grad_u_out : nullptr; p.gx0_out = a.grad_x0_out;
+  p.batch = a.batch; p.T = a.T; p.n = a.n; p.m = a.m;
+  p.ap = plan_adjoint(a.n, cluster);
+  if (p.ap.stages < 2) return cudaErrorInvalidConfiguration;
+
+  EncodeTiledFn enc = reinterpret_cast<EncodeTiledFn>(get_encode_tiled());
+  if (!enc) return cudaErrorNotSupported;
+  CUtensorMap tmap;
+  const cuuint64_t dims[2] = {static_cast<cuuint64_t>(a.n), static_cast<cuuint64_t>(a.batch) * a.T * a.n};
+  const cuuint64_t strides[1] = {static_cast<cuuint64_t>(a.n) * 4};
+  const cuuint32_t box[2] = {static_cast<cuuint32_t>(p.ap.bw), static_cast<cuuint32_t>(p.ap.rcb)};
+  const cuuint32_t estr[2] = {1, 1};
+  CUresult r = enc(&tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(a.A), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+
+  cudaError_t e = cudaFuncSetAttribute(adjoint_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, p.ap.total);
+  if (e != cudaSuccess) return e;
+  if (cluster > 8) {
+    e = cudaFuncSetAttribute(adjoint_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    if (e != cudaSuccess) return e;
+  }
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(static_cast<unsigned>(a.batch) * cluster);
+  cfg.blockDim = dim3(kAdjThreads);
+  cfg.dynamicSmemBytes = p.ap.total;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = cluster;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  e = cudaLaunchKernelEx(&cfg, adjoint_kernel, p, tmap);
+  if (e == cudaSuccess) ++*launches;
+  return e;
+}
+
+}  // namespace ltv

@@ -1,0 +1,275 @@
+// extern "C" boundary of libltvscan.so (include/ltv_scan.h): argument validation, workspace sizing,
+// device check, dispatch to the launchers.  No torch types, no exceptions across the ABI.
+#include <atomic>
+#include <cstdlib>
+#include <cstring>
+
+#include "../../include/ltv_scan.h"
+#include "ltv_internal.h"
+#include "phi_geom.cuh"
+
+namespace ltv {
+
+static thread_local int g_last_cuda_error = 0;
+static std::atomic<unsigned long long> g_launches{0};
+
+int env_int(const char* name, int dflt) {
+  char key[64] = "LTV_SCAN_";
+  std::strncat(key, name, sizeof(key) - std::strlen(key) - 1);
+  const char* v = std::getenv(key);
+  return (v && *v) ? std::atoi(v) : dflt;
+}
+
+int pick_cluster(int batch, int n, int num_sms) {
+  const int forced = env_int("CLUSTER", 0);
+  if (forced == 1 || forced == 2 || forced == 4 || forced == 8 || forced == 16) return forced;
+  int c = 1;
+  while (c < 16 && static_cast<long long>(batch) * (2 * c) <= num_sms && n / (2 * c) >= 32) c *= 2;
+  return c;
+}
+
+static int fail_cuda(cudaError_t e) {
+  g_last_cuda_error = static_cast<int>(e);
+  cudaGetLastError();  // clear the sticky-free error state of the runtime
+  return LTV_ERR_CUDA;
+}
+
+static bool misaligned(const void* p) { return p && (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+static int check_dims(int batch, int T, int n, int m) {
+  if (batch < 1 || T < 1 || n < 1 || m < 0) return LTV_ERR_BAD_DIM;
+  if (n % 4 != 0 || n > 8192) return LTV_ERR_UNSUPPORTED_SHAPE;
+  // TMA row coordinates and block indices are 32-bit
+  if (static_cast<long long>(batch) * T * n >= (1ll << 31)) return LTV_ERR_UNSUPPORTED_SHAPE;
+  if (static_cast<long long>(batch) * T * (T - 1) / 2 * n >= (1ll << 31)) return LTV_ERR_UNSUPPORTED_SHAPE;
+  return LTV_OK;
+}
+
+// current device must be sm_100-class; returns the SM count through *sms
+static int check_device(int* sms) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return fail_cuda(e);
+  int major = 0;
+  e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (e != cudaSuccess) return fail_cuda(e);
+  if (major != 10) return LTV_ERR_ARCH;
+  e = cudaDeviceGetAttribute(sms, cudaDevAttrMultiProcessorCount, dev);
+  if (e != cudaSuccess) return fail_cuda(e);
+  return LTV_OK;
+}
+
+}  // namespace ltv
+
+using namespace ltv;
+
+extern "C" {
+
+long long ltv_phi_block_index(int T, int t, int s) {
+  if (T < 1 || s < 0 || t <= s || t > T - 1) return -1;
+  return phi_colbase(T, s) + (t - s - 1);
+}
+
+size_t ltv_scan_workspace_bytes(int op, int batch, int T, int n, int m) {
+  if (check_dims(batch, T, n, m) != LTV_OK) return 0;
+  switch (op) {
+    case LTV_OP_ROLLOUT:
+    case LTV_OP_ADJOINT:
+      return 0;
+    case LTV_OP_SYSTEM_RESPONSE_TUBE:
+      return phi_workspace_bytes(batch, T, n);
+    case LTV_OP_PIPELINE_HOST: {
+      const size_t b = batch, t = T, nn = n, mm = m;
+      const size_t P = t * (t - 1) / 2;
+      size_t tot = 0;
+      auto add = [&](size_t floats) { tot += align_up(floats * 4 + 16, 256); };
+      add(b * t * nn * nn);  // A
+      add(b * t * nn * mm);  // B
+      add(b * t * nn);       // c
+      add(b * nn);           // x0
+      add(b * t * mm);       // u
+      add(b * t * nn);       // w
+      add(b * t * nn);       // g
+      add(b * t * nn);       // x
+      add(b * P * nn * nn);  // phi
+      add(b * t * nn);       // r
+      add(b * t * nn);       // lambda
+      add(b * t * mm);       // grad_u
+      add(b * nn);           // grad_x0
+      tot += phi_workspace_bytes(batch, T, n);
+      return tot;
+    }
+    default:
+      return 0;
+  }
+}
+
+int ltv_scan_rollout(const float* A, const float* B, const float* c, const float* x0, const float* u, float* x_out,
+                     int batch, int T, int n, int m, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  (void)workspace; (void)workspace_bytes;
+  if (!A || !x0 || !x_out) return LTV_ERR_NULL_PTR;
+  int st = check_dims(batch, T, n, m);
+  if (st != LTV_OK) return st;
+  if (misaligned(A) || misaligned(B) || misaligned(c) || misaligned(x0) || misaligned(u) || misaligned(x_out))
+    return LTV_ERR_ALIGNMENT;
+  int sms = 0;
+  st = check_device(&sms);
+  if (st != LTV_OK) return st;
+  RolloutArgs a{A, B, c, x0, u, x_out, batch, T, n, m};
+  unsigned long long l = 0;
+  cudaError_t e = cudaErrorUnknown;
+  for (int cl = pick_cluster(batch, n, sms); cl >= 1; cl /= 2) {  // a 16-CTA cluster may not be placeable
+    e = launch_rollout(a, cl, static_cast<cudaStream_t>(cuda_stream), &l);
+    if (e == cudaSuccess) break;
+    cudaGetLastError();
+  }
+  g_launches += l;
+  return e == cudaSuccess ? LTV_OK : fail_cuda(e);
+}
+
+int ltv_scan_adjoint(const float* A, const float* B, const float* g, float* lambda_out, float* grad_u_out,
+                     float* grad_x0_out, int batch, int T, int n, int m, void* workspace, size_t workspace_bytes,
+                     void* cuda_stream) {
+  (void)workspace; (void)workspace_bytes;
+  if (!A || !g || !lambda_out) return LTV_ERR_NULL_PTR;
+  if (grad_u_out && m > 0 && !B) return LTV_ERR_NULL_PTR;
+  int st = check_dims(batch, T, n, m);
+  if (st != LTV_OK) return st;
+  if (misaligned(A) || misaligned(B) || misaligned(g) || misaligned(lambda_out) || misaligned(grad_u_out) ||
+      misaligned(grad_x0_out))
+    return LTV_ERR_ALIGNMENT;
+  int sms = 0;
+  st = check_device(&sms);
+  if (st != LTV_OK) return st;
+  AdjointArgs a{A, B, g, lambda_out, grad_u_out, grad_x0_out, batch, T, n, m};
+  unsigned long long l = 0;
+  cudaError_t e = cudaErrorUnknown;
+  for (int cl = pick_cluster(batch, n, sms); cl >= 1; cl /= 2) {
+    e = launch_adjoint(a, cl, static_cast<cudaStream_t>(cuda_stream), &l);
+    if (e == cudaSuccess) break;
+    cudaGetLastError();
+  }
+  g_launches += l;
+  return e == cudaSuccess ? LTV_OK : fail_cuda(e);
+}
+
+int ltv_scan_system_response_tube(const float* A, const float* w, float* phi_out, float* r_out, int batch, int T,
+                                  int n, int phi_layout, unsigned flags, void* workspace, size_t workspace_bytes,
+                                  void* cuda_stream) {
+  if (!A || !w || !r_out) return LTV_ERR_NULL_PTR;
+  if (T > 1 && !phi_out) return LTV_ERR_NULL_PTR;
+  int st = check_dims(batch, T, n, 0);
+  if (st != LTV_OK) return st;
+  if (phi_layout != LTV_PHI_COLUMN_PACKED || flags != 0) return LTV_ERR_BAD_DIM;
+  if (misaligned(A) || misaligned(w) || misaligned(phi_out) || misaligned(r_out) || misaligned(workspace))
+    return LTV_ERR_ALIGNMENT;
+  const size_t need = phi_workspace_bytes(batch, T, n);
+  if (!workspace) return LTV_ERR_NULL_PTR;
+  if (workspace_bytes < need) return LTV_ERR_WORKSPACE_TOO_SMALL;
+  int sms = 0;
+  st = check_device(&sms);
+  if (st != LTV_OK) return st;
+  PhiArgs a{A, w, phi_out, r_out, static_cast<float*>(workspace), batch, T, n};
+  unsigned long long l = 0;
+  cudaError_t e = launch_phi_tube(a, static_cast<cudaStream_t>(cuda_stream), &l);
+  g_launches += l;
+  return e == cudaSuccess ? LTV_OK : fail_cuda(e);
+}
+
+int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float* c_host, const float* x0_host,
+                           const float* u_host, const float* w_host, const float* g_host, float* x_host,
+                           float* phi_host, float* r_host, float* lambda_host, float* grad_u_host,
+                           float* grad_x0_host, int batch, int T, int n, int m, void* workspace,
+                           size_t workspace_bytes, void* cuda_stream, float** phi_device_out) {
+  if (!A_host || !x0_host || !w_host || !g_host || !x_host || !r_host || !lambda_host || !workspace)
+    return LTV_ERR_NULL_PTR;
+  if (grad_u_host && m > 0 && !B_host) return LTV_ERR_NULL_PTR;
+  int st = check_dims(batch, T, n, m);
+  if (st != LTV_OK) return st;
+  if (misaligned(workspace)) return LTV_ERR_ALIGNMENT;
+  if (workspace_bytes < ltv_scan_workspace_bytes(LTV_OP_PIPELINE_HOST, batch, T, n, m))
+    return LTV_ERR_WORKSPACE_TOO_SMALL;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  const size_t b = batch, t = T, nn = n, mm = m, P = t * (t - 1) / 2;
+  char* cur = static_cast<char*>(workspace);
+  auto carve = [&](size_t floats) {
+    float* p = reinterpret_cast<float*>(cur);
+    cur += align_up(floats * 4 + 16, 256);
+    return p;
+  };
+  float* dA = carve(b * t * nn * nn);
+  float* dB = carve(b * t * nn * mm);
+  float* dc = carve(b * t * nn);
+  float* dx0 = carve(b * nn);
+  float* du = carve(b * t * mm);
+  float* dw = carve(b * t * nn);
+  float* dg = carve(b * t * nn);
+  float* dx = carve(b * t * nn);
+  float* dphi = carve(b * P * nn * nn);
+  float* dr = carve(b * t * nn);
+  float* dl = carve(b * t * nn);
+  float* dgu = carve(b * t * mm);
+  float* dgx = carve(b * nn);
+  void* phi_ws = cur;
+  const size_t phi_ws_bytes = phi_workspace_bytes(batch, T, n);
+  if (phi_device_out) *phi_device_out = dphi;
+
+  cudaError_t e;
+#define LTV_H2D(dst, src, floats)                                                                   \
+  if ((src) && (floats) > 0) {                                                                      \
+    e = cudaMemcpyAsync((dst), (src), (floats) * sizeof(float), cudaMemcpyHostToDevice, s);         \
+    if (e != cudaSuccess) return fail_cuda(e);                                                      \
+  }
+#define LTV_D2H(dst, src, floats)                                                                   \
+  if ((dst) && (floats) > 0) {                                                                      \
+    e = cudaMemcpyAsync((dst), (src), (floats) * sizeof(float), cudaMemcpyDeviceToHost, s);         \
+    if (e != cudaSuccess) return fail_cuda(e);                                                      \
+  }
+  LTV_H2D(dA, A_host, b * t * nn * nn);
+  LTV_H2D(dB, B_host, b * t * nn * mm);
+  LTV_H2D(dc, c_host, b * t * nn);
+  LTV_H2D(dx0, x0_host, b * nn);
+  LTV_H2D(du, u_host, b * t * mm);
+  LTV_H2D(dw, w_host, b * t * nn);
+  LTV_H2D(dg, g_host, b * t * nn);
+  st = ltv_scan_rollout(dA, B_host ? dB : nullptr, c_host ? dc : nullptr, dx0, u_host ? du : nullptr, dx, batch, T, n,
+                        m, nullptr, 0, cuda_stream);
+  if (st != LTV_OK) return st;
+  st = ltv_scan_system_response_tube(dA, dw, dphi, dr, batch, T, n, LTV_PHI_COLUMN_PACKED, 0, phi_ws, phi_ws_bytes,
+                                     cuda_stream);
+  if (st != LTV_OK) return st;
+  st = ltv_scan_adjoint(dA, B_host ? dB : nullptr, dg, dl, (grad_u_host && B_host) ? dgu : nullptr,
+                        grad_x0_host ? dgx : nullptr, batch, T, n, m, nullptr, 0, cuda_stream);
+  if (st != LTV_OK) return st;
+  LTV_D2H(x_host, dx, b * t * nn);
+  LTV_D2H(r_host, dr, b * t * nn);
+  LTV_D2H(lambda_host, dl, b * t * nn);
+  if (B_host) LTV_D2H(grad_u_host, dgu, b * t * mm);
+  LTV_D2H(grad_x0_host, dgx, b * nn);
+  LTV_D2H(phi_host, dphi, b * P * nn * nn);
+#undef LTV_H2D
+#undef LTV_D2H
+  e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) return fail_cuda(e);
+  return LTV_OK;
+}
+
+const char* ltv_status_string(int status) {
+  switch (status) {
+    case LTV_OK: return "LTV_OK";
+    case LTV_ERR_NULL_PTR: return "LTV_ERR_NULL_PTR";
+    case LTV_ERR_BAD_DIM: return "LTV_ERR_BAD_DIM";
+    case LTV_ERR_UNSUPPORTED_SHAPE: return "LTV_ERR_UNSUPPORTED_SHAPE";
+    case LTV_ERR_ALIGNMENT: return "LTV_ERR_ALIGNMENT";
+    case LTV_ERR_WORKSPACE_TOO_SMALL: return "LTV_ERR_WORKSPACE_TOO_SMALL";
+    case LTV_ERR_ARCH: return "LTV_ERR_ARCH";
+    case LTV_ERR_CUDA: return "LTV_ERR_CUDA";
+    default: return "LTV_ERR_UNKNOWN";
+  }
+}
+
+int ltv_last_cuda_error(void) { return g_last_cuda_error; }
+int ltv_version(void) { return 100; }
+unsigned long long ltv_launch_count(void) { return g_launches.load(); }
+
+}  // extern "C"

@@ -1,0 +1,45 @@
+// Internal host-side declarations shared by the translation units of libltvscan.so.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace ltv {
+
+// Every launcher enqueues on `stream`, never synchronises, and returns the cudaError_t of the launch.
+// `launches` is incremented by the number of kernels enqueued.
+
+struct RolloutArgs {
+  const float *A, *B, *c, *x0, *u;
+  float* x_out;
+  int batch, T, n, m;
+};
+cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches);
+
+struct AdjointArgs {
+  const float *A, *B, *g;
+  float *lambda_out, *grad_u_out, *grad_x0_out;
+  int batch, T, n, m;
+};
+cudaError_t launch_adjoint(const AdjointArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches);
+
+struct PhiArgs {
+  const float *A, *w;
+  float *phi, *r;
+  float* part;  // workspace: [batch, P, NT, n] per-(block, n-tile) tube partial sums
+  int batch, T, n;
+};
+// n-tile width the Phi path uses for this n (decides the size of `part`) and whether it is the tcgen05 path
+int phi_tile_n(int n);
+bool phi_uses_tensor_cores(int n);
+size_t phi_workspace_bytes(int batch, int T, int n);
+cudaError_t launch_phi_tube(const PhiArgs& a, cudaStream_t stream, unsigned long long* launches);
+
+// cluster-size heuristic shared by rollout and adjoint (power of two, 1..16)
+int pick_cluster(int batch, int n, int num_sms);
+// environment override for experiments: LTV_SCAN_<name>=<int>; returns `dflt` if unset
+int env_int(const char* name, int dflt);
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+}  // namespace ltv

@@ -1,0 +1,72 @@
+// ltv_scan_system_response_tube orchestration: level 0, ceil(log2(T-1)) combine levels, tube finalise.
+// All launches go to one stream in level order; no host synchronisation.
+#include <cuda.h>
+
+#include "ltv_internal.h"
+#include "phi_geom.cuh"
+#include "phi_kernels.h"
+
+namespace ltv {
+
+bool phi_uses_tensor_cores(int n) { return n >= 96 && env_int("PHI_SIMT", 0) == 0; }
+
+// n-tile width: the multiple of 32 in [64, 256] with the least padding, ties to the wider tile
+static int pick_nch(int n) {
+  int forced = env_int("PHI_NCH", 0);
+  if (forced >= 2 && forced <= 8) return forced;
+  int best = 2;
+  long long best_pad = -1;
+  for (int nch = 2; nch <= 8; ++nch) {
+    const int nt = 32 * nch;
+    const long long padded = static_cast<long long>((n + nt - 1) / nt) * nt;
+    if (best_pad < 0 || padded <= best_pad) {
+      best_pad = padded;
+      best = nch;
+    }
+  }
+  return best;
+}
+
+int phi_tile_n(int n) { return phi_uses_tensor_cores(n) ? 32 * pick_nch(n) : 64; }
+
+size_t phi_workspace_bytes(int batch, int T, int n) {
+  const int tn = phi_tile_n(n);
+  const size_t NT = (n + tn - 1) / tn;
+  const size_t P = static_cast<size_t>(T) * (T - 1) / 2;
+  size_t bytes = static_cast<size_t>(batch) * P * NT * n * sizeof(float);
+  if (bytes == 0) bytes = 16;
+  return align_up(bytes, 256);
+}
+
+cudaError_t launch_phi_tube(const PhiArgs& a, cudaStream_t stream, unsigned long long* launches) {
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int tn = phi_tile_n(a.n);
+  const int NT = (a.n + tn - 1) / tn;
+  cudaError_t e;
+  const int NS = a.T - 1;
+  if (NS >= 1) {
+    e = launch_phi_level0(a, NT, sms, stream);
+    if (e != cudaSuccess) return e;
+    ++*launches;
+    const bool tc = phi_uses_tensor_cores(a.n);
+    alignas(64) unsigned char maps[512];
+    if (tc && NS >= 2) {
+      if (phi_tc_maps_size() > sizeof(maps)) return cudaErrorInvalidValue;
+      e = phi_tc_make_maps(a, tn / 32, maps);
+      if (e != cudaSuccess) return e;
+    }
+    for (int level = 1; (1 << (level - 1)) < NS; ++level) {
+      e = tc ? launch_phi_combine_tc(a, level, tn / 32, maps, sms, stream)
+             : launch_phi_combine_simt(a, level, sms, stream);
+      if (e != cudaSuccess) return e;
+      ++*launches;
+    }
+  }
+  e = launch_phi_finalize(a, NT, stream);
+  if (e == cudaSuccess) ++*launches;
+  return e;
+}
+
+}  // namespace ltv

@@ -1,0 +1,165 @@
+// Phi path, non-tensor-core kernels: level 0 (copy + tube), the fp32 FMA combine used for small n, and the
+// deterministic tube finalise.  (eq.(12c), :147 eq.(12e).)
+#include "ltv_internal.h"
+#include "phi_geom.cuh"
+#include "phi_kernels.h"
+#include "ptx.cuh"
+
+namespace ltv {
+
+// ------------------------------------------------------------------------------------------ level 0
+// Phi(s+1,s) = A_s, part[b][q(s+1,s)][0][i] = sum_j |A_s[i,j]| w_s[j]; part slots 1..NT-1 are zeroed.
+// HBM-bound: one warp per matrix row, 128-bit loads/stores.
+__global__ void __launch_bounds__(256) phi_level0_kernel(const float* __restrict__ A, const float* __restrict__ w,
+                                                         float* __restrict__ phi, float* __restrict__ part,
+                                                         int batch, int T, int n, int NT) {
+  const int P = T * (T - 1) / 2;
+  const long long nrows = static_cast<long long>(batch) * (T - 1) * n;
+  const int lane = threadIdx.x & 31;
+  const int n4 = n >> 2;
+  for (long long row = static_cast<long long>(blockIdx.x) * 8 + (threadIdx.x >> 5); row < nrows;
+       row += static_cast<long long>(gridDim.x) * 8) {
+    const int i = static_cast<int>(row % n);
+    const long long bs = row / n;
+    const int s = static_cast<int>(bs % (T - 1));
+    const int b = static_cast<int>(bs / (T - 1));
+    const float4* src = reinterpret_cast<const float4*>(A + ((static_cast<size_t>(b) * T + s) * n + i) * n);
+    const float4* wv = reinterpret_cast<const float4*>(w + (static_cast<size_t>(b) * T + s) * n);
+    const size_t q = static_cast<size_t>(b) * P + phi_colbase(T, s);
+    float* dst = phi + (q * n + i) * n;
+    float acc = 0.f;
+    for (int c = lane; c < n4; c += 32) {
+      const float4 a = __ldcs(src + c);
+      const float4 ww = __ldg(wv + c);
+      st_global_f4_na(dst + 4 * c, a);
+      acc = fmaf(fabsf(a.x), ww.x, fmaf(fabsf(a.y), ww.y, fmaf(fabsf(a.z), ww.z, fmaf(fabsf(a.w), ww.w, acc))));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) part[(q * NT) * n + i] = acc;
+    if (lane > 0 && lane < NT) part[(q * NT + lane) * n + i] = 0.f;
+    for (int e = 32; e < NT; e += 32)
+      if (e + lane < NT) part[(q * NT + e + lane) * n + i] = 0.f;
+  }
+}
+
+// ------------------------------------------------------------------------------------------ SIMT combine
+// 64 x 64 output tile, 256 threads, 4 x 4 register micro-tile, K blocked by 16 through shared memory.
+constexpr int kST = 64, kSK = 16;
+__global__ void __launch_bounds__(256) phi_combine_simt_kernel(float* phi, const float* __restrict__ w,
+                                                               float* __restrict__ part, PhiGeom g) {
+  __shared__ float As[kSK][kST + 4];  // [k][m]
+  __shared__ float Bs[kSK][kST + 4];  // [k][j]
+  __shared__ float ws[kST];
+  __shared__ float tube[kST][17];
+  const int n = g.n;
+  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+  for (long long idx = blockIdx.x; idx < g.total; idx += gridDim.x) {
+    const PhiTile t = phi_decode(g, idx);
+    const size_t item = static_cast<size_t>(t.b) * g.P;
+    const float* Aop = phi + (item + phi_colbase(g.T, t.mid)) * n * n;                       // rows (t,i)
+    const float* Bop = phi + (item + phi_colbase(g.T, t.s) + (t.mid - t.s - 1)) * n * n;    // Phi(mid,s)
+    float* Out = phi + (item + phi_colbase(g.T, t.s) + (t.mid - t.s)) * n * n;             // rows (t,i), col s
+    const int Mrows = t.cnt_t * n;
+    const int m0 = t.m_tile * kST, j0 = t.n_tile * kST;
+    if (threadIdx.x < kST) {
+      const int j = j0 + threadIdx.x;
+      ws[threadIdx.x] = (j < n) ? w[(static_cast<size_t>(t.b) * g.T + t.s) * n + j] : 0.f;
+    }
+    float acc[4][4] = {};
+    for (int k0 = 0; k0 < n; k0 += kSK) {
+      for (int e = threadIdx.x; e < kST * kSK; e += 256) {
+        const int kk = e % kSK, mm = e / kSK;
+        const int r = m0 + mm, k = k0 + kk;
+        As[kk][mm] = (r < Mrows && k < n) ? Aop[static_cast<size_t>(r) * n + k] : 0.f;
+      }
+      for (int e = threadIdx.x; e < kST * kSK; e += 256) {
+        const int jj = e % kST, kk = e / kST;
+        const int j = j0 + jj, k = k0 + kk;
+        Bs[kk][jj] = (j < n && k < n) ? Bop[static_cast<size_t>(k) * n + j] : 0.f;
+      }
+      __syncthreads();
+#pragma unroll
+      for (int kk = 0; kk < kSK; ++kk) {
+        float a[4], bb[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) a[r] = As[kk][ty * 4 + r];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) bb[c] = Bs[kk][tx * 4 + c];
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+          for (int c = 0; c < 4; ++c) acc[r][c] = fmaf(a[r], bb[c], acc[r][c]);
+      }
+      __syncthreads();
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      const int row = m0 + ty * 4 + r;
+      float tb = 0.f;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        const int j = j0 + tx * 4 + c;
+        tb = fmaf(fabsf(acc[r][c]), ws[tx * 4 + c], tb);
+        if (row < Mrows && j < n) Out[static_cast<size_t>(row) * n + j] = acc[r][c];
+      }
+      tube[ty * 4 + r][tx] = tb;
+    }
+    __syncthreads();
+    if (threadIdx.x < kST) {
+      const int row = m0 + threadIdx.x;
+      if (row < Mrows) {
+        float v = 0.f;
+#pragma unroll
+        for (int c = 0; c < 16; ++c) v += tube[threadIdx.x][c];
+        const size_t q = item + phi_colbase(g.T, t.s) + (t.mid - t.s) + row / n;
+        part[(q * g.NT + t.n_tile) * n + row % n] = v;
+      }
+    }
+    __syncthreads();
+  }
+}
+
+// ------------------------------------------------------------------------------------------ finalise
+// r[b][t][i] = sum_{s<t} sum_{nt} part[b][q(t,s)][nt][i], fixed order; r[b][0][:] = 0.
+__global__ void __launch_bounds__(128) phi_tube_finalize_kernel(const float* __restrict__ part, float* __restrict__ r,
+                                                                int batch, int T, int n, int NT) {
+  const int P = T * (T - 1) / 2;
+  const int t = blockIdx.x % T, b = blockIdx.x / T;
+  for (int i = blockIdx.y * blockDim.x + threadIdx.x; i < n; i += gridDim.y * blockDim.x) {
+    float acc = 0.f;
+    for (int s = 0; s < t; ++s) {
+      const size_t q = static_cast<size_t>(b) * P + phi_colbase(T, s) + (t - s - 1);
+      for (int nt = 0; nt < NT; ++nt) acc += part[(q * NT + nt) * n + i];
+    }
+    r[(static_cast<size_t>(b) * T + t) * n + i] = acc;
+  }
+}
+
+cudaError_t launch_phi_level0(const PhiArgs& a, int NT, int num_sms, cudaStream_t stream) {
+  const long long nrows = static_cast<long long>(a.batch) * (a.T - 1) * a.n;
+  long long blocks = (nrows + 7) / 8;
+  const long long cap = static_cast<long long>(num_sms) * 16;
+  if (blocks > cap) blocks = cap;
+  phi_level0_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(a.A, a.w, a.phi, a.part, a.batch, a.T, a.n, NT);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_phi_combine_simt(const PhiArgs& a, int level, int num_sms, cudaStream_t stream) {
+  const PhiGeom g = phi_geom(a.batch, a.T, a.n, level, kST, kST);
+  if (g.total == 0) return cudaSuccess;
+  long long blocks = g.total;
+  const long long cap = static_cast<long long>(num_sms) * 8;
+  if (blocks > cap) blocks = cap;
+  phi_combine_simt_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(a.phi, a.w, a.part, g);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_phi_finalize(const PhiArgs& a, int NT, cudaStream_t stream) {
+  dim3 grid(static_cast<unsigned>(a.batch) * a.T, static_cast<unsigned>((a.n + 127) / 128));
+  if (grid.y > 64) grid.y = 64;
+  phi_tube_finalize_kernel<<<grid, 128, 0, stream>>>(a.part, a.r, a.batch, a.T, a.n, NT);
+  return cudaGetLastError();
+}
+
+}  // namespace ltv

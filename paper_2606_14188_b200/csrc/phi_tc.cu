@@ -1,0 +1,324 @@
+// Phi path, levels >= 1, n >= 96: the divide-and-conquer combine Phi(t,s) = Phi(t,mid) Phi(mid,s) as a
+// persistent, warp-specialised tcgen05 GEMM with 3xTF32 operand splitting and the tube reduction
+// r_t += |Phi(t,s)| w_s fused into the TMEM epilogue (eq.(12c), :147 eq.(12e), :166, :177).
+//
+//   D[(t,i), j] = sum_k  L[(t,i), k] * R[k, j],   L = stacked Phi(t,mid) (K-major), R = Phi(mid,s) (N-major)
+//
+// Per CTA tile: 128 rows x NT = 32*NCH columns, K = n in blocks of 32.
+//   warp 0      TMA producer: fp32 tiles of L (one 128x32 box, SWIZZLE_128B) and R (NCH boxes of 32x32,
+//               SWIZZLE_128B_ATOM_32B: the only MN-major layout kind::tf32 accepts)
+//   warps 8-11  split: lo = rna_tf32(a - trunc_tf32(a)) written to a second buffer with the SAME byte layout
+//               (position-preserving, so no knowledge of the swizzle is needed); the raw buffer serves as
+//               the hi operand (kind::tf32 reads the top 19 bits of each 32-bit word)
+//   warp 1      one thread issues, per 8-deep k-step: D += Llo*Rhi, D += Lhi*Rlo, D += Lhi*Rhi (small first)
+//   warps 4-7   epilogue: TMEM -> registers -> global (row per thread) + per-row |D| w partial sum
+// The accumulator is double-buffered in TMEM (2 * NT <= 512 columns) so the epilogue of tile i overlaps the
+// MMAs of tile i+1.
+#include <cuda.h>
+
+#include "ltv_internal.h"
+#include "phi_geom.cuh"
+#include "phi_kernels.h"
+#include "ptx.cuh"
+
+namespace ltv {
+
+namespace {
+
+constexpr int kTcThreads = 384;
+constexpr int kTM = 128;
+constexpr int kKB = 32;  // k-block = one 128-byte swizzle row of fp32
+constexpr uint32_t kABytes = kTM * kKB * 4;  // 16 KB
+constexpr int kTcMaxStages = 4;
+
+struct TcParams {
+  float* phi;
+  const float* w;
+  float* part;
+  PhiGeom g;
+  int stages;
+  int hi_inplace;
+};
+
+struct TcMaps {
+  CUtensorMap L;  // 2-D [batch*P*n rows][n]           box 32 x 128
+  CUtensorMap R;  // 3-D [batch*P blocks][n][n]        box 32 x 32 x 1
+};
+
+__device__ __forceinline__ float tf32_lo(float a, float& hi) {
+  hi = __uint_as_float(__float_as_uint(a) & 0xffffe000u);
+  const float d = a - hi;
+  uint32_t r;
+  asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(d));
+  return __uint_as_float(r);
+}
+
+template <bool kHiInplace>
+__device__ __forceinline__ void split_f4(float4* raw, float4* lo, int i) {
+  float4 a = raw[i], h, l;
+  l.x = tf32_lo(a.x, h.x);
+  l.y = tf32_lo(a.y, h.y);
+  l.z = tf32_lo(a.z, h.z);
+  l.w = tf32_lo(a.w, h.w);
+  lo[i] = l;
+  if (kHiInplace) raw[i] = h;
+}
+
+template <int NCH>
+__global__ void __launch_bounds__(kTcThreads, 1)
+phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL,
+                      const __grid_constant__ CUtensorMap mapR) {
+  constexpr int NT = 32 * NCH;
+  constexpr uint32_t kBBytes = NCH * 4096u;
+  constexpr uint32_t kStageBytes = 2 * kABytes + 2 * kBBytes;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const PhiGeom& g = p.g;
+  const int n = g.n;
+  const int stages = p.stages;
+  const int nkb = (n + kKB - 1) / kKB;
+  const int ks_last = ((n - (nkb - 1) * kKB) + 7) / 8;  // k-steps of the last k-block that hold data
+
+  uint8_t* misc = smem + static_cast<size_t>(stages) * kStageBytes;
+  float* wbuf = reinterpret_cast<float*>(misc);  // [2][NT]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(misc + 2 * NT * 4);
+  uint64_t* full = bars;                        // TMA bytes landed
+  uint64_t* conv = bars + kTcMaxStages;         // lo planes written (4 warp arrivals)
+  uint64_t* empty = bars + 2 * kTcMaxStages;    // MMAs that read the stage have completed
+  uint64_t* tfull = bars + 3 * kTcMaxStages;    // [2] accumulator ready
+  uint64_t* tempty = tfull + 2;                 // [2] accumulator drained (4 warp arrivals)
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < stages; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&conv[s], 4);
+      mbar_init(&empty[s], 1);
+    }
+    for (int a = 0; a < 2; ++a) {
+      mbar_init(&tfull[a], 1);
+      mbar_init(&tempty[a], 4);
+    }
+    fence_mbar_init();
+    tma_prefetch_desc(&mapL);
+    tma_prefetch_desc(&mapR);
+  }
+  if (warp == 2) tmem_alloc<512>(tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    // ---------------------------------------------------------------------------------- TMA producer
+    if (lane == 0) {
+      const uint64_t pol = l2_policy_evict_last();  // operands are re-read by many tiles: keep them in L2
+      uint32_t it = 0;
+      for (long long idx = blockIdx.x; idx < g.total; idx += gridDim.x) {
+        const PhiTile t = phi_decode(g, idx);
+        const long long item = static_cast<long long>(t.b) * g.P;
+        const int rowL = static_cast<int>((item + phi_colbase(g.T, t.mid)) * n) + t.m_tile * kTM;
+        const int blkR = static_cast<int>(item + phi_colbase(g.T, t.s) + (t.mid - t.s - 1));
+        const int j0 = t.n_tile * NT;
+        for (int kb = 0; kb < nkb; ++kb, ++it) {
+          const int st = it % stages;
+          const uint32_t use = it / stages;
+          if (use > 0) mbar_wait(&empty[st], (use - 1) & 1);
+          uint8_t* sp = smem + static_cast<size_t>(st) * kStageBytes;
+          mbar_arrive_expect_tx(&full[st], kABytes + kBBytes);
+          tma_load_2d(sp, &mapL, kb * kKB, rowL, &full[st], pol);
+#pragma unroll
+          for (int c = 0; c < NCH; ++c)
+            tma_load_3d(sp + 2 * kABytes + c * 4096, &mapR, j0 + 32 * c, kb * kKB, blkR, &full[st], pol);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ---------------------------------------------------------------------------------- MMA issuer
+    if (lane == 0) {
+      constexpr uint32_t idesc = umma_idesc_tf32(kTM, NT, 0, 1);
+      uint32_t it = 0, lt = 0;
+      for (long long idx = blockIdx.x; idx < g.total; idx += gridDim.x, ++lt) {
+        const uint32_t acc = lt & 1;
+        if (lt >= 2) mbar_wait(&tempty[acc], ((lt >> 1) - 1) & 1);
+        tc_fence_after();
+        const uint32_t d_tmem = tmem_base + acc * NT;
+        for (int kb = 0; kb < nkb; ++kb, ++it) {
+          const int st = it % stages;
+          mbar_wait(&conv[st], (it / stages) & 1);
+          tc_fence_after();
+          const uint32_t sa = smem_u32(smem + static_cast<size_t>(st) * kStageBytes);
+          const uint32_t sb = sa + 2 * kABytes;
+          const int nks = (kb == nkb - 1) ? ks_last : 4;
+          for (int ks = 0; ks < nks; ++ks) {
+            const uint64_t a_hi = umma_smem_desc(sa + ks * 32, 16, 1024, kUmmaSw128);
+            const uint64_t a_lo = umma_smem_desc(sa + kABytes + ks * 32, 16, 1024, kUmmaSw128);
+            const uint64_t b_hi = umma_smem_desc(sb + ks * 1024, 4096, 512, kUmmaSw128Base32);
+            const uint64_t b_lo = umma_smem_desc(sb + kBBytes + ks * 1024, 4096, 512, kUmmaSw128Base32);
+            umma_tf32_ss(d_tmem, a_lo, b_hi, idesc, (kb | ks) != 0);
+            umma_tf32_ss(d_tmem, a_hi, b_lo, idesc, 1);
+            umma_tf32_ss(d_tmem, a_hi, b_hi, idesc, 1);
+          }
+          umma_commit(&empty[st]);
+        }
+        umma_commit(&tfull[acc]);
+      }
+    }
+  } else if (warp >= 8) {
+    // ---------------------------------------------------------------------------------- operand split
+    const int tid = threadIdx.x - 256;
+    uint32_t it = 0;
+    for (long long idx = blockIdx.x; idx < g.total; idx += gridDim.x) {
+      for (int kb = 0; kb < nkb; ++kb, ++it) {
+        const int st = it % stages;
+        mbar_wait(&full[st], (it / stages) & 1);
+        uint8_t* sp = smem + static_cast<size_t>(st) * kStageBytes;
+        float4* ar = reinterpret_cast<float4*>(sp);
+        float4* al = reinterpret_cast<float4*>(sp + kABytes);
+        float4* br = reinterpret_cast<float4*>(sp + 2 * kABytes);
+        float4* bl = reinterpret_cast<float4*>(sp + 2 * kABytes + kBBytes);
+        if (p.hi_inplace) {
+#pragma unroll
+          for (int i = tid; i < static_cast<int>(kABytes / 16); i += 128) split_f4<true>(ar, al, i);
+#pragma unroll
+          for (int i = tid; i < static_cast<int>(kBBytes / 16); i += 128) split_f4<true>(br, bl, i);
+        } else {
+#pragma unroll
+          for (int i = tid; i < static_cast<int>(kABytes / 16); i += 128) split_f4<false>(ar, al, i);
+#pragma unroll
+          for (int i = tid; i < static_cast<int>(kBBytes / 16); i += 128) split_f4<false>(br, bl, i);
+        }
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&conv[st]);
+      }
+    }
+  } else if (warp >= 4) {
+    // ---------------------------------------------------------------------------------- epilogue
+    const int wq = warp - 4;            // == warp % 4: the TMEM lane quarter this warp may read
+    const int etid = threadIdx.x - 128;
+    uint32_t lt = 0;
+    for (long long idx = blockIdx.x; idx < g.total; idx += gridDim.x, ++lt) {
+      const PhiTile t = phi_decode(g, idx);
+      const uint32_t acc = lt & 1;
+      const int j0 = t.n_tile * NT;
+      float* wb = wbuf + acc * NT;
+      for (int j = etid; j < NT; j += 128)
+        wb[j] = (j0 + j < n) ? __ldg(p.w + (static_cast<size_t>(t.b) * g.T + t.s) * n + j0 + j) : 0.f;
+      named_bar_sync(1, 128);
+      const size_t item = static_cast<size_t>(t.b) * g.P;
+      const size_t qcol = item + phi_colbase(g.T, t.s) + (t.mid - t.s);  // block (mid+1, s)
+      const int rho = t.m_tile * kTM + wq * 32 + lane;
+      const bool valid = rho < t.cnt_t * n;
+      float* out = p.phi + (qcol * n + rho) * n + j0;
+      mbar_wait(&tfull[acc], (lt >> 1) & 1);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + (static_cast<uint32_t>(wq * 32) << 16) + acc * NT;
+      float tube = 0.f;
+#pragma unroll
+      for (int cc = 0; cc < NCH; ++cc) {
+        uint32_t v[32];
+        tmem_ld_32x32(taddr + cc * 32, v);
+        tmem_ld_wait();
+#pragma unroll
+        for (int e = 0; e < 32; ++e) tube = fmaf(fabsf(__uint_as_float(v[e])), wb[cc * 32 + e], tube);
+        if (valid) {
+#pragma unroll
+          for (int e = 0; e < 8; ++e) {
+            if (j0 + cc * 32 + 4 * e < n)
+              st_global_f4_na(out + cc * 32 + 4 * e,
+                              make_float4(__uint_as_float(v[4 * e]), __uint_as_float(v[4 * e + 1]),
+                                          __uint_as_float(v[4 * e + 2]), __uint_as_float(v[4 * e + 3])));
+          }
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&tempty[acc]);
+      if (valid) p.part[((qcol + rho / n) * g.NT + t.n_tile) * n + rho % n] = tube;
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) {
+    tc_fence_after();
+    tmem_dealloc<512>(tmem_base);
+  }
+}
+
+template <int NCH>
+cudaError_t launch_tc(const TcParams& p, const TcMaps& maps, int num_sms, cudaStream_t stream) {
+  constexpr uint32_t kStageBytes = 2 * kABytes + 2 * NCH * 4096u;
+  const uint32_t misc = 2 * 32 * NCH * 4 + (3 * kTcMaxStages + 4) * 8 + 16;
+  TcParams q = p;
+  int st = static_cast<int>((227u * 1024u - 1024u - misc) / kStageBytes);
+  if (st > kTcMaxStages) st = kTcMaxStages;
+  if (st < 2) return cudaErrorInvalidConfiguration;
+  q.stages = st;
+  const uint32_t smem = 1024u + st * kStageBytes + misc;
+  cudaError_t e = cudaFuncSetAttribute(phi_combine_tc_kernel<NCH>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e != cudaSuccess) return e;
+  long long blocks = q.g.total < num_sms ? q.g.total : num_sms;
+  phi_combine_tc_kernel<NCH><<<static_cast<unsigned>(blocks), kTcThreads, smem, stream>>>(q, maps.L, maps.R);
+  return cudaGetLastError();
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+}  // namespace
+
+size_t phi_tc_maps_size() { return sizeof(TcMaps); }
+
+cudaError_t phi_tc_make_maps(const PhiArgs& a, int nch, void* maps_out) {
+  (void)nch;
+  EncodeTiledFn enc = reinterpret_cast<EncodeTiledFn>(get_encode_tiled());
+  if (!enc) return cudaErrorNotSupported;
+  TcMaps* m = static_cast<TcMaps*>(maps_out);
+  const cuuint64_t P = static_cast<cuuint64_t>(a.T) * (a.T - 1) / 2;
+  const cuuint64_t n = a.n;
+  const cuuint32_t estr[3] = {1, 1, 1};
+  {
+    const cuuint64_t dims[2] = {n, static_cast<cuuint64_t>(a.batch) * P * n};
+    const cuuint64_t strides[1] = {n * 4};
+    const cuuint32_t box[2] = {kKB, kTM};
+    if (enc(&m->L, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, a.phi, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+  }
+  {
+    const cuuint64_t dims[3] = {n, n, static_cast<cuuint64_t>(a.batch) * P};
+    const cuuint64_t strides[2] = {n * 4, n * n * 4};
+    const cuuint32_t box[3] = {32, kKB, 1};
+    if (enc(&m->R, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, a.phi, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+  }
+  return cudaSuccess;
+}
+
+cudaError_t launch_phi_combine_tc(const PhiArgs& a, int level, int nch, const void* maps, int num_sms,
+                                  cudaStream_t stream) {
+  TcParams p{};
+  p.phi = a.phi; p.w = a.w; p.part = a.part;
+  p.g = phi_geom(a.batch, a.T, a.n, level, kTM, 32 * nch);
+  p.hi_inplace = env_int("HI_INPLACE", 0);
+  if (p.g.total == 0) return cudaSuccess;
+  const TcMaps& m = *static_cast<const TcMaps*>(maps);
+  switch (nch) {
+    case 2: return launch_tc<2>(p, m, num_sms, stream);
+    case 3: return launch_tc<3>(p, m, num_sms, stream);
+    case 4: return launch_tc<4>(p, m, num_sms, stream);
+    case 5: return launch_tc<5>(p, m, num_sms, stream);
+    case 6: return launch_tc<6>(p, m, num_sms, stream);
+    case 7: return launch_tc<7>(p, m, num_sms, stream);
+    case 8: return launch_tc<8>(p, m, num_sms, stream);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+}  // namespace ltv

@@ -1,0 +1,88 @@
+"""The C-ABI library loads, exports every symbol include/ltv_scan.h declares, and validates its arguments on
+the host before touching the GPU (no compute calls here: runs without a GPU)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    import __graft_entry__ as G
+
+    G.build()
+    import paper_2606_14188_b200 as lib
+
+    return lib
+
+
+def test_exports_match_header(L):
+    hdr = open(os.path.join(ROOT, "include", "ltv_scan.h")).read()
+    declared = set(re.findall(r"LTV_API[^;(]*?\b(ltv_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(L.EXPORTS)
+    raw = ctypes.CDLL(L.LIB_PATH)
+    for name in declared:
+        assert hasattr(raw, name), name
+
+
+def test_status_strings_and_version(L):
+    assert L.lib.ltv_status_string(0) == b"LTV_OK"
+    assert L.lib.ltv_status_string(5) == b"LTV_ERR_WORKSPACE_TOO_SMALL"
+    assert L.lib.ltv_version() >= 100
+
+
+def test_block_index_is_column_packed(L):
+    T = 7
+    seen = []
+    for s in range(T - 1):
+        for t in range(s + 1, T):
+            seen.append(L.ltv_phi_block_index(T, t, s))
+    assert seen == list(range(T * (T - 1) // 2))
+    assert L.ltv_phi_block_index(T, 3, 3) == -1 and L.ltv_phi_block_index(T, T, 0) == -1
+
+
+def test_workspace_sizes(L):
+    assert L.ltv_scan_workspace_bytes(L.LTV_OP_ROLLOUT, 4, 8, 48, 6) == 0
+    n, T, b = 300, 32, 64
+    need = L.ltv_scan_workspace_bytes(L.LTV_OP_SYSTEM_RESPONSE_TUBE, b, T, n, 0)
+    assert need >= b * (T * (T - 1) // 2) * 2 * n * 4          # two n-tiles of 160 columns
+    assert L.ltv_scan_workspace_bytes(L.LTV_OP_SYSTEM_RESPONSE_TUBE, b, T, 301, 0) == 0
+    big = L.ltv_scan_workspace_bytes(L.LTV_OP_PIPELINE_HOST, b, T, n, 6)
+    assert big > b * (T * (T - 1) // 2) * n * n * 4 + b * T * n * n * 4
+
+
+def test_host_side_validation_needs_no_gpu(L):
+    f = ctypes.c_void_p
+    buf = (ctypes.c_float * 64)()
+    p = ctypes.cast(buf, f)
+    odd = f(ctypes.addressof(buf) + 4)
+    r = L.lib.ltv_scan_rollout
+    assert r(None, None, None, p, None, p, 1, 1, 4, 0, None, 0, None) == 1          # NULL A
+    assert r(p, None, None, p, None, p, 0, 1, 4, 0, None, 0, None) == 2             # batch 0
+    assert r(p, None, None, p, None, p, 1, 1, 6, 0, None, 0, None) == 3             # n % 4
+    assert r(p, None, None, p, None, p, 1, 1, 8196, 0, None, 0, None) == 3          # n too large
+    assert r(odd, None, None, p, None, p, 1, 1, 4, 0, None, 0, None) == 4           # alignment
+    s = L.lib.ltv_scan_system_response_tube
+    assert s(p, p, p, None, 1, 2, 4, 0, 0, p, 1 << 20, None) == 1                   # NULL r_out
+    assert s(p, p, p, p, 1, 2, 4, 1, 0, p, 1 << 20, None) == 2                      # unknown layout
+    assert s(p, p, p, p, 1, 2, 4, 0, 1, p, 1 << 20, None) == 2                      # unknown flag
+    assert s(p, p, p, p, 1, 2, 4, 0, 0, p, 8, None) == 5                            # workspace too small
+    a = L.lib.ltv_scan_adjoint
+    assert a(p, None, p, p, p, None, 1, 2, 4, 2, None, 0, None) == 1                # grad_u wanted, B NULL
+    assert a(p, p, None, p, None, None, 1, 2, 4, 2, None, 0, None) == 1             # NULL g
+
+
+def test_valid_call_without_gpu_fails_loudly(L):
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    f = ctypes.c_void_p
+    buf = (ctypes.c_float * 64)()
+    base = (ctypes.addressof(buf) + 15) & ~15
+    p = f(base)
+    st = L.lib.ltv_scan_rollout(p, None, None, p, None, p, 1, 1, 4, 0, None, 0, None)
+    assert st in (6, 7)                                                            # ARCH or CUDA, never OK

@@ -1,0 +1,196 @@
+"""Parity of the CUDA path (through the C-ABI binding) against the fp64 oracle, element by element, on the
+same seeded inputs.  Tolerance: north_star's max|err| / max|ref| <= 1e-4 per output tensor (fp32 / 3xTF32);
+integer-valued inputs must be reproduced EXACTLY (all partial sums < 2^24)."""
+import numpy as np
+import pytest
+
+from oracle import ltv_oracle as O
+from workloads import config, dense_random, generate, small_integer
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def L():
+    import torch
+
+    assert torch.cuda.is_available(), "GPU tests need a GPU (no CPU fallback)"
+    import __graft_entry__ as G
+
+    G.build()
+    import paper_2606_14188_b200 as lib
+
+    return lib
+
+
+def _dev(W):
+    import torch
+
+    return {k: torch.from_numpy(getattr(W, k)).cuda() for k in ("A", "B", "c", "x0", "u", "w", "g")}
+
+
+def _col_perm(T):
+    """oracle row-packed index of every block, in COLUMN_PACKED order"""
+    return [O.packed_index(t, s) for s in range(T - 1) for t in range(s + 1, T)]
+
+
+def _run_all(L, W, phi=True):
+    import torch
+
+    d = _dev(W)
+    out = {}
+    out["x"] = L.ltv_scan_rollout(d["A"], d["B"], d["c"], d["x0"], d["u"])
+    if phi:
+        out["phi"], out["r"] = L.ltv_scan_system_response_tube(d["A"], d["w"])
+    out["lam"], out["grad_u"], out["grad_x0"] = L.ltv_scan_adjoint(d["A"], d["B"], d["g"])
+    torch.cuda.synchronize()
+    return {k: (None if v is None else v.cpu().numpy()) for k, v in out.items()}
+
+
+def _ref_all(W, phi=True):
+    ref = {"x": O.rollout(W.A, W.B, W.c, W.x0, W.u)}
+    if phi:
+        T = W.A.shape[1]
+        perm = _col_perm(T)
+        pr = [O.system_response_tube_item(W.A[b], W.w[b]) for b in range(W.A.shape[0])]
+        ref["phi"] = np.stack([p[0][perm] for p in pr]) if perm else np.zeros((W.A.shape[0], 0) + W.A.shape[2:])
+        ref["r"] = np.stack([p[1] for p in pr])
+    ref["lam"], ref["grad_u"], ref["grad_x0"] = O.adjoint(W.A, W.B, W.g)
+    return ref
+
+
+def _check(got, ref, exact=False):
+    errs = {}
+    for k, r in ref.items():
+        if r is None:
+            continue
+        assert got[k].shape == r.shape, k
+        assert np.all(np.isfinite(got[k])), k
+        if exact:
+            assert np.array_equal(got[k].astype(np.float64), r), k
+        errs[k] = O.rel_err(got[k], r)
+        assert errs[k] <= TOL, (k, errs)
+    return errs
+
+
+# ------------------------------------------------------------------ the five configs (C2-C5 at reduced batch / T
+# so the oracle finishes in seconds; full sizes are sampled in test_gpu_full_size.py)
+@pytest.mark.parametrize("k,over", [
+    (0, {}),                                   # C1 exactly: n=48 (fp32-FMA Phi path), T=16, batch 1
+    (1, dict(batch=3, T=9)),                   # C2 shape: n=300 -> two 160-wide n-tiles, ragged m-tiles
+    (1, dict(batch=2, T=32)),                  # C2 full horizon (5 levels)
+    (2, dict(batch=2, T=6)),                   # C3: n=600
+    (4, dict(batch=5, T=64)),                  # C5: n=180, long horizon
+])
+def test_configs(L, k, over):
+    W = generate(config(k, **over))
+    errs = _check(_run_all(L, W), _ref_all(W))
+    print(config(k, **over)["name"], errs)
+
+
+def test_config4_large_cloth_small_T(L):
+    W = generate(config(3, batch=1, T=4))      # n=2400, m=12
+    _check(_run_all(L, W), _ref_all(W))
+
+
+@pytest.mark.parametrize("n,T,batch,m", [(128, 5, 2, 3), (256, 16, 2, 4), (96, 3, 1, 0), (100, 7, 3, 2),
+                                         (32, 12, 4, 5), (4, 3, 2, 1), (420, 4, 1, 7)])
+def test_dense_random(L, n, T, batch, m):
+    """Dense Jacobians (PAPER.md:166 'dense matrix multiplications'): no kernel may rely on sparsity."""
+    W = dense_random(batch, T, n, max(m, 1), seed=100 + n)
+    if m == 0:
+        W.B = None
+        W.u = None
+        d = _dev_partial(W)
+        import torch
+
+        x = L.ltv_scan_rollout(d["A"], None, d["c"], d["x0"], None)
+        lam, gu, gx0 = L.ltv_scan_adjoint(d["A"], None, d["g"])
+        phi, r = L.ltv_scan_system_response_tube(d["A"], d["w"])
+        torch.cuda.synchronize()
+        assert gu is None
+        assert O.rel_err(x.cpu().numpy(), O.rollout(W.A, None, W.c, W.x0, None)) <= TOL
+        rl, _, rgx = O.adjoint(W.A, None, W.g)
+        assert O.rel_err(lam.cpu().numpy(), rl) <= TOL and O.rel_err(gx0.cpu().numpy(), rgx) <= TOL
+        assert O.rel_err(r.cpu().numpy(), O.tube(W.A, W.w)) <= TOL
+        return
+    _check(_run_all(L, W), _ref_all(W))
+
+
+def _dev_partial(W):
+    import torch
+
+    return {k: torch.from_numpy(getattr(W, k)).cuda() for k in ("A", "c", "x0", "w", "g")}
+
+
+@pytest.mark.parametrize("n,T", [(64, 9), (160, 9), (288, 6)])
+def test_integer_inputs_are_exact(L, n, T):
+    """SURVEY 8c pin (vii): with small-integer data every product and partial sum is exactly representable, so
+    fp32 FMA and the 3xTF32 split (hi carries everything, lo = 0) must match the fp64 oracle bit for bit."""
+    W = small_integer(2, T, n, 3, seed=n + T)
+    ref = _ref_all(W)
+    assert max(np.abs(v).max() for v in ref.values()) < 2 ** 22
+    _check(_run_all(L, W), ref, exact=True)
+
+
+def test_edge_T1_and_T2(L):
+    for T in (1, 2):
+        W = dense_random(2, T, 128, 2, seed=T)
+        got = _run_all(L, W)
+        ref = _ref_all(W)
+        _check(got, ref)
+        assert np.all(got["r"][:, 0] == 0)
+
+
+def test_null_optional_outputs_and_determinism(L):
+    import torch
+
+    W = dense_random(3, 10, 192, 4, seed=9)
+    d = _dev(W)
+    lam, gu, gx0 = L.ltv_scan_adjoint(d["A"], d["B"], d["g"], want_grad_x0=False)
+    assert gx0 is None
+    rl, rgu, _ = O.adjoint(W.A, W.B, W.g)
+    assert O.rel_err(lam.cpu().numpy(), rl) <= TOL and O.rel_err(gu.cpu().numpy(), rgu) <= TOL
+    p1, r1 = L.ltv_scan_system_response_tube(d["A"], d["w"])
+    p2, r2 = L.ltv_scan_system_response_tube(d["A"], d["w"])
+    torch.cuda.synchronize()
+    assert torch.equal(p1, p2) and torch.equal(r1, r2)          # fixed-order tube reduction, no atomics
+
+
+def test_inputs_not_modified_and_no_overrun(L):
+    import torch
+
+    W = dense_random(2, 6, 132, 3, seed=11)
+    d = _dev(W)
+    keep = {k: v.clone() for k, v in d.items()}
+    batch, T, n, m = W.shape
+    P = T * (T - 1) // 2
+    guard = 1024
+    phi = torch.full((batch * P * n * n + guard,), 7.0, device="cuda")
+    r = torch.full((batch * T * n + guard,), 7.0, device="cuda")
+    L.ltv_scan_system_response_tube(d["A"], d["w"], phi[:batch * P * n * n].view(batch, P, n, n),
+                                    r[:batch * T * n].view(batch, T, n))
+    L.ltv_scan_rollout(d["A"], d["B"], d["c"], d["x0"], d["u"])
+    L.ltv_scan_adjoint(d["A"], d["B"], d["g"])
+    torch.cuda.synchronize()
+    assert torch.all(phi[-guard:] == 7.0) and torch.all(r[-guard:] == 7.0)
+    for k in d:
+        assert torch.equal(d[k], keep[k]), k
+
+
+def test_pipeline_host_matches_device_calls(L):
+    import torch
+
+    W = generate(config(1, batch=2, T=6))
+    batch, T, n, m = W.shape
+    need = L.ltv_scan_workspace_bytes(L.LTV_OP_PIPELINE_HOST, batch, T, n, m)
+    ws = torch.empty(need, dtype=torch.uint8, device="cuda")
+    h = {k: torch.from_numpy(getattr(W, k)).pin_memory() for k in ("A", "B", "c", "x0", "u", "w", "g")}
+    P = T * (T - 1) // 2
+    phi_host = torch.empty((batch, P, n, n), dtype=torch.float32).pin_memory()
+    outs = L.ltv_scan_pipeline_host(h["A"], h["B"], h["c"], h["x0"], h["u"], h["w"], h["g"], ws, phi_host=phi_host)
+    got = dict(x=outs["x"].numpy(), r=outs["r"].numpy(), lam=outs["lam"].numpy(), grad_u=outs["grad_u"].numpy(),
+               grad_x0=outs["grad_x0"].numpy(), phi=phi_host.numpy())
+    _check(got, _ref_all(W))
+    assert outs["phi_device_ptr"] != 0
