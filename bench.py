@@ -1,0 +1,310 @@
+#!/usr/bin/env python
+"""bench.py - one JSON line for the LTV-scan hot path (rollout + Phi/tube + adjoint) on N B200s.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl ours|reference]
+  python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A "step" is one pass of the whole hot path over one batch of the workload (default: BASELINE.json
+configs[1], rope N=50: n=300, m=6, T=32, batch 64 per GPU; seeded synthetic mass-spring Jacobians, see
+DESIGN.md).  `value` = Phi blocks per second over the whole step, inputs resident in HBM, CUDA-event timed,
+max over ranks; `e2e` = the same through ltv_scan_pipeline_host with pinned HOST buffers (H2D of every input
+and D2H of x, r, lambda, grad_u, grad_x0 inside the timed region; Phi stays device-resident).
+`--impl reference` times the fp64 CPU oracle on a bounded sample (rank 0 only)."""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "LTV scan rollouts/s + SLS Phi blocks/s; % of B200 tensor/HBM roofline"
+UNIT = "Phi blocks/s (whole step: rollout + Phi/tube + adjoint)"
+NOMINAL_TF32_OVER_BF16 = 0.5          # dense tensor peaks, B200_PROFILING.md: tf32 1.1 vs bf16 2.25 PFLOP/s
+FALLBACK_BF16_TFLOPS = 1590.0         # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
+FALLBACK_BF16_SUSTAINED = 1400.0
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=40)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (0..4)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-items", type=int, default=0, help="items in the CPU-oracle sample (0 = auto)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(source="measured", hbm_gbs=p["hbm_gbs"], bf16=p["bf16_tflops"],
+                    bf16_sustained=p.get("bf16_tflops_sustained", p["bf16_tflops"]))
+    return dict(source="fallback", hbm_gbs=6650.0, bf16=FALLBACK_BF16_TFLOPS, bf16_sustained=FALLBACK_BF16_SUSTAINED)
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML during the timed region."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.stop_flag, self.max_mhz = index, [], set(), False, None
+
+    def run(self):
+        try:
+            import pynvml as N
+
+            N.nvmlInit()
+            h = N.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = N.nvmlDeviceGetMaxClockInfo(h, N.NVML_CLOCK_SM)
+            names = {
+                N.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                N.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                N.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                N.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+            }
+            while not self.stop_flag:
+                self.samples.append(N.nvmlDeviceGetClockInfo(h, N.NVML_CLOCK_SM))
+                r = N.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+                time.sleep(0.02)
+        except Exception as e:  # NVML missing: report that, never fail the bench
+            self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+
+    def result(self):
+        s = sorted(self.samples)
+        return dict(sm_mhz=(s[len(s) // 2] if s else None), sm_max_mhz=self.max_mhz, reasons=sorted(self.reasons),
+                    samples=len(s))
+
+
+def workload(cfg_index, rank, world, batch_override=None):
+    """Per-rank inputs: rank r gets its own `batch` items (weak scaling: seed offset by rank)."""
+    from workloads import config, generate
+
+    over = {}
+    if batch_override:
+        over["batch"] = batch_override
+    cfg = config(cfg_index, **over)
+    cfg["seed"] = cfg["seed"] + 1000 * rank
+    return cfg, generate(cfg)
+
+
+def cpu_oracle_step(W, items):
+    """One pass of the whole path by the fp64 oracle over `items` batch items; returns seconds."""
+    from oracle import ltv_oracle as O
+
+    t0 = time.perf_counter()
+    for b in range(items):
+        O.rollout_item(W.A[b], W.B[b], W.c[b], W.x0[b], W.u[b])
+        O.system_response_tube_item(W.A[b], W.w[b])
+        O.adjoint_item(W.A[b], W.B[b], W.g[b])
+    return time.perf_counter() - t0
+
+
+def blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+
+        return max([p.get("num_threads", 1) for p in threadpool_info()] or [os.cpu_count() or 1])
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    cfg, W = workload(args.config, 0, 1, batch_override=max(1, args.cpu_items or 2))
+    items = W.A.shape[0]
+    T, n = cfg["T"], cfg["n"]
+    P = T * (T - 1) // 2
+    for _ in range(min(args.warmup, 1)):
+        cpu_oracle_step(W, 1)
+    times = [cpu_oracle_step(W, items) for _ in range(args.steps)]
+    sec = sum(times) / len(times)
+    val = items * P / sec
+    cores = blas_threads()
+    line = dict(metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=sec * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+                data="synthetic", impl="reference",
+                config=dict(workload=f"{cfg['name']}: n={n} m={cfg['m']} T={T}, {items}-item sample per step "
+                                     f"(full batch {64 if args.config == 1 else cfg['batch']})", l2="n/a (CPU)"),
+                cpu_baseline=dict(value=val, unit=UNIT, cores=cores, kind="oracle",
+                                  sample=f"{items} items of {cfg['name']} per step, whole path in fp64 numpy"),
+                e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                gpu_launches=0)
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    assert torch.cuda.is_available(), "bench.py needs a GPU (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import __graft_entry__ as G
+
+    G.build()
+    import paper_2606_14188_b200 as L
+
+    cfg, W = workload(args.config, rank, world)
+    batch, T, n, m = W.shape
+    P = T * (T - 1) // 2
+    phi_on = args.config != 4
+    dev = torch.device("cuda", local)
+    d = {k: torch.from_numpy(getattr(W, k)).to(dev) for k in ("A", "B", "c", "x0", "u", "w", "g")}
+    x = torch.empty((batch, T, n), device=dev)
+    lam = torch.empty((batch, T, n), device=dev)
+    gu = torch.empty((batch, T, m), device=dev)
+    gx0 = torch.empty((batch, n), device=dev)
+    if phi_on:
+        phi = torch.empty((batch, P, n, n), device=dev)
+        r = torch.empty((batch, T, n), device=dev)
+        ws = torch.empty(max(16, L.ltv_scan_workspace_bytes(L.LTV_OP_SYSTEM_RESPONSE_TUBE, batch, T, n, 0)),
+                         dtype=torch.uint8, device=dev)
+
+    def step():
+        L.ltv_scan_rollout(d["A"], d["B"], d["c"], d["x0"], d["u"], x_out=x)
+        if phi_on:
+            L.ltv_scan_system_response_tube(d["A"], d["w"], phi_out=phi, r_out=r, workspace=ws)
+        L.ltv_scan_adjoint(d["A"], d["B"], d["g"], lambda_out=lam, grad_u_out=gu, grad_x0_out=gx0)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    L.ltv_profile_enable(True)
+    l0 = L.ltv_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    launches = L.ltv_launch_count() - l0
+    prof = L.ltv_profile_collect()
+    L.ltv_profile_enable(False)
+    sampler.stop_flag = True
+    sampler.join(timeout=2)
+    ms_total = e0.elapsed_time(e1)
+    if world > 1:
+        tt = torch.tensor([ms_total], device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms_total = float(tt.item())
+    ms_step = ms_total / args.steps
+    units = (P if phi_on else 1) * batch * world            # Phi blocks (or rollouts at config 5) per step
+    value = units / (ms_step * 1e-3)
+
+    # ---- roofline of the dominant kernel
+    pk = peaks()
+    k_ms = {k: (v[0] / max(v[1], 1), v[1]) for k, v in prof.items()}       # avg ms per launch, launches
+    if phi_on and prof["phi_combine_tc"][1] > 0:
+        G_blocks = (T - 1) * (T - 2) // 2                                   # GEMM blocks per item
+        flops_issued = 3.0 * 2.0 * n ** 3 * G_blocks * batch                # 3xTF32, per step (all levels)
+        ms_kernel = prof["phi_combine_tc"][0] / args.steps                  # all level launches of one step
+        ach = flops_issued / (ms_kernel * 1e-3) / 1e12
+        peak = pk["bf16_sustained"] * NOMINAL_TF32_OVER_BF16
+        roof = dict(bound="tensor", kernel="phi_combine_tc_kernel (3xTF32 tcgen05, all levels of one step)",
+                    achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak, traffic=None,
+                    peak_source=f"{pk['source']} bf16 sustained x {NOMINAL_TF32_OVER_BF16} (nominal tf32/bf16)",
+                    logical_fp32_tflops=ach / 3.0, kernel_ms_per_step=ms_kernel,
+                    launches_per_step=prof["phi_combine_tc"][1] / args.steps)
+    else:
+        bytes_roll = batch * (T * (n * n + n * m + n + m) + n + T * n) * 4.0
+        ms_kernel = prof["rollout"][0] / max(prof["rollout"][1], 1)
+        ach = bytes_roll / (ms_kernel * 1e-3) / 1e9
+        roof = dict(bound="hbm", kernel="rollout_kernel", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s",
+                    frac=ach / pk["hbm_gbs"], traffic=None, peak_source=pk["source"], kernel_ms_per_step=ms_kernel)
+    share = {k: round(v[0] / args.steps, 4) for k, v in prof.items() if v[1]}
+
+    # ---- secondary HBM rooflines (rollout / adjoint), reported beside the headline
+    bytes_roll = batch * (T * (n * n + n * m + n + m) + n + T * n) * 4.0
+    extra = {}
+    for k in ("rollout", "adjoint"):
+        if prof[k][1]:
+            ms = prof[k][0] / prof[k][1]
+            extra[k] = dict(per_s=batch * world / (ms * 1e-3), ms=ms, hbm_gbs=bytes_roll / (ms * 1e-3) / 1e9,
+                            hbm_frac=bytes_roll / (ms * 1e-3) / 1e9 / pk["hbm_gbs"])
+
+    # ---- end to end through the C-ABI with host buffers
+    e2e = None
+    if not args.no_e2e:
+        if phi_on:
+            del phi, ws
+        torch.cuda.empty_cache()
+        need = L.ltv_scan_workspace_bytes(L.LTV_OP_PIPELINE_HOST, batch, T, n, m)
+        wsh = torch.empty(need, dtype=torch.uint8, device=dev)
+        h = {k: torch.from_numpy(getattr(W, k)).pin_memory() for k in ("A", "B", "c", "x0", "u", "w", "g")}
+        outs = None
+        h2d = sum(v.numel() * 4 for v in h.values())
+        for i in range(1 + args.e2e_steps):
+            if i == 1:
+                barrier()
+                t0 = time.perf_counter()
+            outs = L.ltv_scan_pipeline_host(h["A"], h["B"], h["c"], h["x0"], h["u"], h["w"], h["g"], wsh, outs=outs)
+        barrier()
+        sec = (time.perf_counter() - t0) / args.e2e_steps
+        if world > 1:
+            tt = torch.tensor([sec], device=dev)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            sec = float(tt.item())
+        d2h = sum(outs[k].numel() * 4 for k in ("x", "r", "lam", "grad_u", "grad_x0") if outs[k] is not None)
+        e2e = dict(value=units / sec, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
+                   ms_per_step=sec * 1e3, note="ltv_scan_pipeline_host, pinned host buffers; Phi stays in HBM")
+
+    # ---- CPU oracle beside it (rank 0, N = 1 only)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        items = args.cpu_items or (2 if n <= 600 else 1)
+        sec = cpu_oracle_step(W, items)
+        cpu = dict(value=items * (P if phi_on else 1) / sec, unit=UNIT, cores=blas_threads(), kind="oracle",
+                   sample=f"{items} of {batch} items of {cfg['name']}, whole path, fp64 numpy, {sec:.1f} s")
+
+    if rank == 0:
+        line = dict(metric=METRIC, value=value, unit=UNIT if phi_on else "rollout+adjoint pairs/s", n_gpus=world,
+                    steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms_step, higher_is_better=True,
+                    scaling="weak", vs_baseline=None, dtype="tf32x3/f32", data="synthetic",
+                    config=dict(workload=f"{cfg['name']}: n={n} m={m} T={T} batch={batch} per GPU, "
+                                         f"{P if phi_on else 0} Phi blocks/item (BASELINE.json configs[{args.config}])",
+                                l2="inputs (A 0.74 GB) and outputs (Phi 11.4 GB) larger than the 126 MB L2; no flush",
+                                phi_layout="column-packed"),
+                    clocks=sampler.result(), e2e=e2e, gpu_launches=int(launches), roofline=roof,
+                    cpu_baseline=cpu, kernel_ms_per_step=share, vector_scans=extra,
+                    rollouts_per_s=extra.get("rollout", {}).get("per_s"),
+                    adjoints_per_s=extra.get("adjoint", {}).get("per_s"))
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

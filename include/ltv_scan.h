@@ -145,6 +145,16 @@ LTV_API int ltv_version(void);
  * `gpu_launches`. */
 LTV_API unsigned long long ltv_launch_count(void);
 
+/* Optional per-kernel timing for benchmarks.  While enabled, every kernel the library enqueues is bracketed by
+ * CUDA events recorded on the launch stream (no synchronisation, no change to the kernels).
+ * ltv_profile_collect waits for the recorded events, adds their elapsed times (milliseconds) and launch counts
+ * per kernel class into the two caller arrays of LTV_PROFILE_CLASSES entries (host memory), and clears the
+ * record.  Classes: 0 rollout, 1 adjoint, 2 Phi level 0 (copy + tube), 3 Phi combine (tcgen05 3xTF32),
+ * 4 Phi combine (fp32 FMA, small n), 5 tube finalise. */
+#define LTV_PROFILE_CLASSES 6
+LTV_API int ltv_profile_enable(int on);
+LTV_API int ltv_profile_collect(double* ms_by_class, unsigned long long* launches_by_class);
+
 #ifdef __cplusplus
 }
 #endif

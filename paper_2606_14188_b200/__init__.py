@@ -1,20 +1,23 @@
 """B200-native LTV-scan hot path of CORD-SLS (arxiv 2606.14188): rollout, system response + tube, adjoint.
-Thin ctypes binding over the C-ABI library built from csrc/ (see include/ltv_scan.h)."""
-from .binding import (  # noqa: F401
-    EXPORTS,
-    LIB_PATH,
-    LTV_OP_ADJOINT,
-    LTV_OP_PIPELINE_HOST,
-    LTV_OP_ROLLOUT,
-    LTV_OP_SYSTEM_RESPONSE_TUBE,
-    LTV_PHI_COLUMN_PACKED,
-    LtvError,
-    lib,
-    ltv_launch_count,
-    ltv_phi_block_index,
-    ltv_scan_adjoint,
-    ltv_scan_pipeline_host,
-    ltv_scan_rollout,
-    ltv_scan_system_response_tube,
-    ltv_scan_workspace_bytes,
+Thin ctypes binding over the C-ABI library built from csrc/ (see include/ltv_scan.h).
+
+The binding (and with it libltvscan.so) is loaded on first attribute access, so that
+`paper_2606_14188_b200.build` can be imported to compile the library before it exists.  There is no CPU
+fallback: touching any API name without the built library raises ImportError."""
+import importlib
+
+_API = (
+    "EXPORTS", "LIB_PATH", "LTV_OP_ADJOINT", "LTV_OP_PIPELINE_HOST", "LTV_OP_ROLLOUT",
+    "LTV_OP_SYSTEM_RESPONSE_TUBE", "LTV_PHI_COLUMN_PACKED", "PROFILE_CLASSES", "LtvError", "lib",
+    "ltv_launch_count", "ltv_phi_block_index", "ltv_profile_collect", "ltv_profile_enable",
+    "ltv_scan_adjoint", "ltv_scan_pipeline_host", "ltv_scan_rollout", "ltv_scan_system_response_tube",
+    "ltv_scan_workspace_bytes",
 )
+__all__ = list(_API)
+
+
+def __getattr__(name):
+    if name in _API:
+        binding = importlib.import_module(".binding", __name__)
+        return getattr(binding, name)
+    raise AttributeError(f"module {__name__!r} has no attribute {name!r}")

@@ -22,7 +22,7 @@ LTV_PHI_COLUMN_PACKED = 0
 EXPORTS = (
     "ltv_phi_block_index", "ltv_scan_workspace_bytes", "ltv_scan_rollout", "ltv_scan_system_response_tube",
     "ltv_scan_adjoint", "ltv_scan_pipeline_host", "ltv_status_string", "ltv_last_cuda_error", "ltv_version",
-    "ltv_launch_count",
+    "ltv_launch_count", "ltv_profile_enable", "ltv_profile_collect",
 )
 
 
@@ -56,6 +56,10 @@ def _load() -> ctypes.CDLL:
     L.ltv_last_cuda_error.restype = i
     L.ltv_version.restype = i
     L.ltv_launch_count.restype = ctypes.c_ulonglong
+    L.ltv_profile_enable.restype = i
+    L.ltv_profile_enable.argtypes = [i]
+    L.ltv_profile_collect.restype = i
+    L.ltv_profile_collect.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_ulonglong)]
     return L
 
 
@@ -90,6 +94,23 @@ def ltv_scan_workspace_bytes(op: int, batch: int, T: int, n: int, m: int) -> int
 
 def ltv_launch_count() -> int:
     return int(lib.ltv_launch_count())
+
+
+PROFILE_CLASSES = ("rollout", "adjoint", "phi_level0", "phi_combine_tc", "phi_combine_simt", "phi_finalize")
+
+
+def ltv_profile_enable(on: bool) -> None:
+    lib.ltv_profile_enable(1 if on else 0)
+
+
+def ltv_profile_collect() -> dict:
+    """{class: (total ms, launches)} of the kernels enqueued since the last collect / enable."""
+    ms = (ctypes.c_double * len(PROFILE_CLASSES))()
+    cnt = (ctypes.c_ulonglong * len(PROFILE_CLASSES))()
+    st = lib.ltv_profile_collect(ms, cnt)
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_profile_collect")
+    return {k: (float(ms[i]), int(cnt[i])) for i, k in enumerate(PROFILE_CLASSES)}
 
 
 def ltv_scan_rollout(A, B, c, x0, u, x_out=None):

@@ -272,7 +272,10 @@ cudaError_t launch_adjoint(const AdjointArgs& a, int cluster, cudaStream_t strea
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  e = cudaLaunchKernelEx(&cfg, adjoint_kernel, p, tmap);
+  {
+    ProfScope prof(kProfAdjoint, stream);
+    e = cudaLaunchKernelEx(&cfg, adjoint_kernel, p, tmap);
+  }
   if (e == cudaSuccess) ++*launches;
   return e;
 }

@@ -3,6 +3,8 @@
 #include <atomic>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
+#include <vector>
 
 #include "../../include/ltv_scan.h"
 #include "ltv_internal.h"
@@ -26,6 +28,40 @@ int pick_cluster(int batch, int n, int num_sms) {
   int c = 1;
   while (c < 16 && static_cast<long long>(batch) * (2 * c) <= num_sms && n / (2 * c) >= 32) c *= 2;
   return c;
+}
+
+// ---- optional kernel timing --------------------------------------------------------------------------
+namespace {
+struct ProfState {
+  std::mutex mu;
+  bool on = false;
+  std::vector<cudaEvent_t> beg, end;
+  std::vector<int> cls;
+  size_t used = 0;
+};
+ProfState& prof() {
+  static ProfState p;
+  return p;
+}
+}  // namespace
+
+ProfScope::ProfScope(int cls_, cudaStream_t s) : slot(-1), stream(s) {
+  ProfState& p = prof();
+  if (!p.on) return;
+  std::lock_guard<std::mutex> lk(p.mu);
+  if (p.used == p.beg.size()) {
+    cudaEvent_t a, b;
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
+    p.beg.push_back(a);
+    p.end.push_back(b);
+    p.cls.push_back(0);
+  }
+  slot = static_cast<int>(p.used++);
+  p.cls[slot] = cls_;
+  cudaEventRecord(p.beg[slot], stream);
+}
+ProfScope::~ProfScope() {
+  if (slot >= 0) cudaEventRecord(prof().end[slot], stream);
 }
 
 static int fail_cuda(cudaError_t e) {
@@ -266,6 +302,35 @@ const char* ltv_status_string(int status) {
     case LTV_ERR_CUDA: return "LTV_ERR_CUDA";
     default: return "LTV_ERR_UNKNOWN";
   }
+}
+
+int ltv_profile_enable(int on) {
+  ProfState& p = prof();
+  std::lock_guard<std::mutex> lk(p.mu);
+  p.on = on != 0;
+  p.used = 0;
+  return LTV_OK;
+}
+
+int ltv_profile_collect(double* ms_by_class, unsigned long long* launches_by_class) {
+  if (!ms_by_class || !launches_by_class) return LTV_ERR_NULL_PTR;
+  ProfState& p = prof();
+  std::lock_guard<std::mutex> lk(p.mu);
+  for (int c = 0; c < LTV_PROFILE_CLASSES; ++c) {
+    ms_by_class[c] = 0.0;
+    launches_by_class[c] = 0;
+  }
+  for (size_t i = 0; i < p.used; ++i) {
+    cudaError_t e = cudaEventSynchronize(p.end[i]);
+    if (e != cudaSuccess) return fail_cuda(e);
+    float ms = 0.f;
+    e = cudaEventElapsedTime(&ms, p.beg[i], p.end[i]);
+    if (e != cudaSuccess) return fail_cuda(e);
+    ms_by_class[p.cls[i]] += ms;
+    launches_by_class[p.cls[i]] += 1;
+  }
+  p.used = 0;
+  return LTV_OK;
 }
 
 int ltv_last_cuda_error(void) { return g_last_cuda_error; }

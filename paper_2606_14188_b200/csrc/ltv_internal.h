@@ -40,6 +40,16 @@ int pick_cluster(int batch, int n, int num_sms);
 // environment override for experiments: LTV_SCAN_<name>=<int>; returns `dflt` if unset
 int env_int(const char* name, int dflt);
 
+// optional per-kernel timing (ltv_profile_enable): CUDA events recorded on the launch stream around a kernel
+enum ProfClass { kProfRollout = 0, kProfAdjoint, kProfPhiLevel0, kProfPhiCombineTc, kProfPhiCombineSimt,
+                 kProfPhiFinalize, kProfNumClasses };
+struct ProfScope {
+  ProfScope(int cls, cudaStream_t s);
+  ~ProfScope();
+  int slot;
+  cudaStream_t stream;
+};
+
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 }  // namespace ltv

@@ -10,13 +10,14 @@ namespace ltv {
 
 bool phi_uses_tensor_cores(int n) { return n >= 96 && env_int("PHI_SIMT", 0) == 0; }
 
-// n-tile width: the multiple of 32 in [64, 256] with the least padding, ties to the wider tile
+// n-tile width: the multiple of 32 in [64, 160] with the least padding, ties to the wider tile
+// (2 * NT accumulator columns + 192 columns of L-operand ring must fit the 512 TMEM columns)
 static int pick_nch(int n) {
   int forced = env_int("PHI_NCH", 0);
-  if (forced >= 2 && forced <= 8) return forced;
+  if (forced >= 2 && forced <= 5) return forced;
   int best = 2;
   long long best_pad = -1;
-  for (int nch = 2; nch <= 8; ++nch) {
+  for (int nch = 2; nch <= 5; ++nch) {
     const int nt = 32 * nch;
     const long long padded = static_cast<long long>((n + nt - 1) / nt) * nt;
     if (best_pad < 0 || padded <= best_pad) {

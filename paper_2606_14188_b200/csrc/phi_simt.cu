@@ -141,6 +141,7 @@ cudaError_t launch_phi_level0(const PhiArgs& a, int NT, int num_sms, cudaStream_
   long long blocks = (nrows + 7) / 8;
   const long long cap = static_cast<long long>(num_sms) * 16;
   if (blocks > cap) blocks = cap;
+  ProfScope prof(kProfPhiLevel0, stream);
   phi_level0_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(a.A, a.w, a.phi, a.part, a.batch, a.T, a.n, NT);
   return cudaGetLastError();
 }
@@ -151,6 +152,7 @@ cudaError_t launch_phi_combine_simt(const PhiArgs& a, int level, int num_sms, cu
   long long blocks = g.total;
   const long long cap = static_cast<long long>(num_sms) * 8;
   if (blocks > cap) blocks = cap;
+  ProfScope prof(kProfPhiCombineSimt, stream);
   phi_combine_simt_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(a.phi, a.w, a.part, g);
   return cudaGetLastError();
 }
@@ -158,6 +160,7 @@ cudaError_t launch_phi_combine_simt(const PhiArgs& a, int level, int num_sms, cu
 cudaError_t launch_phi_finalize(const PhiArgs& a, int NT, cudaStream_t stream) {
   dim3 grid(static_cast<unsigned>(a.batch) * a.T, static_cast<unsigned>((a.n + 127) / 128));
   if (grid.y > 64) grid.y = 64;
+  ProfScope prof(kProfPhiFinalize, stream);
   phi_tube_finalize_kernel<<<grid, 128, 0, stream>>>(a.part, a.r, a.batch, a.T, a.n, NT);
   return cudaGetLastError();
 }

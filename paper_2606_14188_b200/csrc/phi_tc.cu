@@ -4,16 +4,21 @@
 //
 //   D[(t,i), j] = sum_k  L[(t,i), k] * R[k, j],   L = stacked Phi(t,mid) (K-major), R = Phi(mid,s) (N-major)
 //
-// Per CTA tile: 128 rows x NT = 32*NCH columns, K = n in blocks of 32.
-//   warp 0      TMA producer: fp32 tiles of L (one 128x32 box, SWIZZLE_128B) and R (NCH boxes of 32x32,
-//               SWIZZLE_128B_ATOM_32B: the only MN-major layout kind::tf32 accepts)
-//   warps 8-11  split: lo = rna_tf32(a - trunc_tf32(a)) written to a second buffer with the SAME byte layout
-//               (position-preserving, so no knowledge of the swizzle is needed); the raw buffer serves as
-//               the hi operand (kind::tf32 reads the top 19 bits of each 32-bit word)
-//   warp 1      one thread issues, per 8-deep k-step: D += Llo*Rhi, D += Lhi*Rlo, D += Lhi*Rhi (small first)
-//   warps 4-7   epilogue: TMEM -> registers -> global (row per thread) + per-row |D| w partial sum
-// The accumulator is double-buffered in TMEM (2 * NT <= 512 columns) so the epilogue of tile i overlaps the
-// MMAs of tile i+1.
+// Per CTA tile: 128 rows x NT = 32*NCH columns (NCH <= 5), K = n in blocks of 32.
+//   warp 0       TMA producer: fp32 tiles of L (one 128x32 box, SWIZZLE_128B) and R (NCH boxes of 32x32,
+//                SWIZZLE_128B_ATOM_32B: the only MN-major layout kind::tf32 accepts) into a ring of R stages
+//   warps 8-15   split (lo = rna_tf32(a - trunc_tf32(a))): the L tile goes from shared memory into TMEM as two
+//                128-lane x 32-column operands (raw bits = hi, since kind::tf32 reads only the top 19 bits, and
+//                lo); the lo plane of R is written to shared memory at the same byte offsets as the raw tile
+//                (position-preserving, so no knowledge of the swizzle is needed).  Ring of 3.
+//   warp 1       one thread issues, per 8-deep k-step: D += Llo*Rhi, D += Lhi*Rlo, D += Lhi*Rhi (small first),
+//                L from TMEM, R from shared memory
+//   warps 4-7    epilogue: TMEM -> registers -> global (row per thread) + per-row |D| w partial sum
+// Why L goes through TMEM: with both operands in shared memory a k-block moves 216 KB through the 128 B/clk
+// shared-memory port against 960 cycles of MMA issue (measured 47 % tensor-pipe activity, profiles/r1_v1_*);
+// L in TMEM removes 48 KB of MMA operand reads and 16 KB of split writes per k-block.
+// The accumulator is double-buffered in TMEM (2 * NT columns) so the epilogue of tile i overlaps the MMAs of
+// tile i+1; TMEM columns: [0, 2NT) accumulators, [2NT, 2NT + 192) L-operand ring.
 #include <cuda.h>
 
 #include "ltv_internal.h"
@@ -25,11 +30,13 @@ namespace ltv {
 
 namespace {
 
-constexpr int kTcThreads = 384;
+constexpr int kTcThreads = 512;
+constexpr int kConvWarps = 8;
+constexpr int kConvStages = 3;  // ring of split operands: L (hi, lo) in TMEM, R lo plane in shared memory
 constexpr int kTM = 128;
 constexpr int kKB = 32;  // k-block = one 128-byte swizzle row of fp32
 constexpr uint32_t kABytes = kTM * kKB * 4;  // 16 KB
-constexpr int kTcMaxStages = 4;
+constexpr int kTcMaxStages = 6;
 
 struct TcParams {
   float* phi;
@@ -37,7 +44,6 @@ struct TcParams {
   float* part;
   PhiGeom g;
   int stages;
-  int hi_inplace;
 };
 
 struct TcMaps {
@@ -53,48 +59,44 @@ __device__ __forceinline__ float tf32_lo(float a, float& hi) {
   return __uint_as_float(r);
 }
 
-template <bool kHiInplace>
-__device__ __forceinline__ void split_f4(float4* raw, float4* lo, int i) {
-  float4 a = raw[i], h, l;
-  l.x = tf32_lo(a.x, h.x);
-  l.y = tf32_lo(a.y, h.y);
-  l.z = tf32_lo(a.z, h.z);
-  l.w = tf32_lo(a.w, h.w);
-  lo[i] = l;
-  if (kHiInplace) raw[i] = h;
-}
-
 template <int NCH>
 __global__ void __launch_bounds__(kTcThreads, 1)
 phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL,
                       const __grid_constant__ CUtensorMap mapR) {
   constexpr int NT = 32 * NCH;
   constexpr uint32_t kBBytes = NCH * 4096u;
-  constexpr uint32_t kStageBytes = 2 * kABytes + 2 * kBBytes;
+  constexpr uint32_t kRawBytes = kABytes + kBBytes;       // one TMA stage: L tile + R tile, fp32
+  constexpr uint32_t kTmemA = 2 * NT;                      // first TMEM column of the L-operand ring
+  static_assert(2 * NT + kConvStages * 64 <= 512, "TMEM budget");
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const PhiGeom& g = p.g;
   const int n = g.n;
-  const int stages = p.stages;
+  const int R = p.stages;
   const int nkb = (n + kKB - 1) / kKB;
   const int ks_last = ((n - (nkb - 1) * kKB) + 7) / 8;  // k-steps of the last k-block that hold data
 
-  uint8_t* misc = smem + static_cast<size_t>(stages) * kStageBytes;
+  uint8_t* lo_ring = smem + static_cast<size_t>(R) * kRawBytes;               // [kConvStages][kBBytes]
+  uint8_t* misc = lo_ring + kConvStages * kBBytes;
   float* wbuf = reinterpret_cast<float*>(misc);  // [2][NT]
   uint64_t* bars = reinterpret_cast<uint64_t*>(misc + 2 * NT * 4);
-  uint64_t* full = bars;                        // TMA bytes landed
-  uint64_t* conv = bars + kTcMaxStages;         // lo planes written (4 warp arrivals)
-  uint64_t* empty = bars + 2 * kTcMaxStages;    // MMAs that read the stage have completed
-  uint64_t* tfull = bars + 3 * kTcMaxStages;    // [2] accumulator ready
-  uint64_t* tempty = tfull + 2;                 // [2] accumulator drained (4 warp arrivals)
+  uint64_t* full = bars;                            // [R] TMA bytes landed
+  uint64_t* rempty = bars + kTcMaxStages;           // [R] MMAs reading the raw stage have completed
+  uint64_t* conv = bars + 2 * kTcMaxStages;         // [kConvStages] split operands ready (8 warp arrivals)
+  uint64_t* cempty = conv + kConvStages;            // [kConvStages] MMAs reading them have completed
+  uint64_t* tfull = cempty + kConvStages;           // [2] accumulator ready
+  uint64_t* tempty = tfull + 2;                     // [2] accumulator drained (4 warp arrivals)
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + 2);
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < stages; ++s) {
+    for (int s = 0; s < R; ++s) {
       mbar_init(&full[s], 1);
-      mbar_init(&conv[s], 4);
-      mbar_init(&empty[s], 1);
+      mbar_init(&rempty[s], 1);
+    }
+    for (int s = 0; s < kConvStages; ++s) {
+      mbar_init(&conv[s], kConvWarps);
+      mbar_init(&cempty[s], 1);
     }
     for (int a = 0; a < 2; ++a) {
       mbar_init(&tfull[a], 1);
@@ -122,15 +124,15 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
         const int blkR = static_cast<int>(item + phi_colbase(g.T, t.s) + (t.mid - t.s - 1));
         const int j0 = t.n_tile * NT;
         for (int kb = 0; kb < nkb; ++kb, ++it) {
-          const int st = it % stages;
-          const uint32_t use = it / stages;
-          if (use > 0) mbar_wait(&empty[st], (use - 1) & 1);
-          uint8_t* sp = smem + static_cast<size_t>(st) * kStageBytes;
-          mbar_arrive_expect_tx(&full[st], kABytes + kBBytes);
-          tma_load_2d(sp, &mapL, kb * kKB, rowL, &full[st], pol);
+          const int rs = it % R;
+          const uint32_t use = it / R;
+          if (use > 0) mbar_wait(&rempty[rs], (use - 1) & 1);
+          uint8_t* sp = smem + static_cast<size_t>(rs) * kRawBytes;
+          mbar_arrive_expect_tx(&full[rs], kRawBytes);
+          tma_load_2d(sp, &mapL, kb * kKB, rowL, &full[rs], pol);
 #pragma unroll
           for (int c = 0; c < NCH; ++c)
-            tma_load_3d(sp + 2 * kABytes + c * 4096, &mapR, j0 + 32 * c, kb * kKB, blkR, &full[st], pol);
+            tma_load_3d(sp + kABytes + c * 4096, &mapR, j0 + 32 * c, kb * kKB, blkR, &full[rs], pol);
         }
       }
     }
@@ -145,53 +147,73 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + acc * NT;
         for (int kb = 0; kb < nkb; ++kb, ++it) {
-          const int st = it % stages;
-          mbar_wait(&conv[st], (it / stages) & 1);
+          const int rs = it % R, cs = it % kConvStages;
+          mbar_wait(&conv[cs], (it / kConvStages) & 1);
           tc_fence_after();
-          const uint32_t sa = smem_u32(smem + static_cast<size_t>(st) * kStageBytes);
-          const uint32_t sb = sa + 2 * kABytes;
+          const uint32_t sb_hi = smem_u32(smem + static_cast<size_t>(rs) * kRawBytes + kABytes);
+          const uint32_t sb_lo = smem_u32(lo_ring + static_cast<size_t>(cs) * kBBytes);
+          const uint32_t a_hi = tmem_base + kTmemA + cs * 64;   // raw fp32 bits: the MMA keeps the top 19
+          const uint32_t a_lo = a_hi + 32;
           const int nks = (kb == nkb - 1) ? ks_last : 4;
           for (int ks = 0; ks < nks; ++ks) {
-            const uint64_t a_hi = umma_smem_desc(sa + ks * 32, 16, 1024, kUmmaSw128);
-            const uint64_t a_lo = umma_smem_desc(sa + kABytes + ks * 32, 16, 1024, kUmmaSw128);
-            const uint64_t b_hi = umma_smem_desc(sb + ks * 1024, 4096, 512, kUmmaSw128Base32);
-            const uint64_t b_lo = umma_smem_desc(sb + kBBytes + ks * 1024, 4096, 512, kUmmaSw128Base32);
-            umma_tf32_ss(d_tmem, a_lo, b_hi, idesc, (kb | ks) != 0);
-            umma_tf32_ss(d_tmem, a_hi, b_lo, idesc, 1);
-            umma_tf32_ss(d_tmem, a_hi, b_hi, idesc, 1);
+            const uint64_t b_hi = umma_smem_desc(sb_hi + ks * 1024, 4096, 512, kUmmaSw128Base32);
+            const uint64_t b_lo = umma_smem_desc(sb_lo + ks * 1024, 4096, 512, kUmmaSw128Base32);
+            umma_tf32_ts(d_tmem, a_lo + ks * 8, b_hi, idesc, (kb | ks) != 0);
+            umma_tf32_ts(d_tmem, a_hi + ks * 8, b_lo, idesc, 1);
+            umma_tf32_ts(d_tmem, a_hi + ks * 8, b_hi, idesc, 1);
           }
-          umma_commit(&empty[st]);
+          umma_commit(&rempty[rs]);
+          umma_commit(&cempty[cs]);
         }
         umma_commit(&tfull[acc]);
       }
     }
   } else if (warp >= 8) {
     // ---------------------------------------------------------------------------------- operand split
-    const int tid = threadIdx.x - 256;
+    // L: warp (q, h) moves rows 32q..32q+31, k-columns 16h..16h+15 of the swizzled landing tile into TMEM
+    // (raw bits = hi, and lo); R: lo plane written to shared memory at the same byte offsets as the raw tile.
+    const int ctid = threadIdx.x - 256;
+    const int q = warp & 3, h = (warp - 8) >> 2;
+    const int row = q * 32 + lane;
     uint32_t it = 0;
     for (long long idx = blockIdx.x; idx < g.total; idx += gridDim.x) {
       for (int kb = 0; kb < nkb; ++kb, ++it) {
-        const int st = it % stages;
-        mbar_wait(&full[st], (it / stages) & 1);
-        uint8_t* sp = smem + static_cast<size_t>(st) * kStageBytes;
-        float4* ar = reinterpret_cast<float4*>(sp);
-        float4* al = reinterpret_cast<float4*>(sp + kABytes);
-        float4* br = reinterpret_cast<float4*>(sp + 2 * kABytes);
-        float4* bl = reinterpret_cast<float4*>(sp + 2 * kABytes + kBBytes);
-        if (p.hi_inplace) {
-#pragma unroll
-          for (int i = tid; i < static_cast<int>(kABytes / 16); i += 128) split_f4<true>(ar, al, i);
-#pragma unroll
-          for (int i = tid; i < static_cast<int>(kBBytes / 16); i += 128) split_f4<true>(br, bl, i);
-        } else {
-#pragma unroll
-          for (int i = tid; i < static_cast<int>(kABytes / 16); i += 128) split_f4<false>(ar, al, i);
-#pragma unroll
-          for (int i = tid; i < static_cast<int>(kBBytes / 16); i += 128) split_f4<false>(br, bl, i);
+        const int rs = it % R, cs = it % kConvStages;
+        const uint32_t cuse = it / kConvStages;
+        mbar_wait(&full[rs], (it / R) & 1);
+        if (cuse > 0) {
+          mbar_wait(&cempty[cs], (cuse - 1) & 1);
+          tc_fence_after();
         }
+        const uint8_t* sp = smem + static_cast<size_t>(rs) * kRawBytes;
+        uint32_t vh[16], vl[16];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          const float4 f = *reinterpret_cast<const float4*>(sp + row * 128 + (((4 * h + c) ^ (row & 7)) << 4));
+          float hh;
+          vh[4 * c + 0] = __float_as_uint(f.x); vl[4 * c + 0] = __float_as_uint(tf32_lo(f.x, hh));
+          vh[4 * c + 1] = __float_as_uint(f.y); vl[4 * c + 1] = __float_as_uint(tf32_lo(f.y, hh));
+          vh[4 * c + 2] = __float_as_uint(f.z); vl[4 * c + 2] = __float_as_uint(tf32_lo(f.z, hh));
+          vh[4 * c + 3] = __float_as_uint(f.w); vl[4 * c + 3] = __float_as_uint(tf32_lo(f.w, hh));
+        }
+        const uint32_t ta = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + kTmemA + cs * 64 + h * 16;
+        tmem_st_32x16(ta, vh);
+        tmem_st_32x16(ta + 32, vl);
+        const float4* br = reinterpret_cast<const float4*>(sp + kABytes);
+        float4* bl = reinterpret_cast<float4*>(lo_ring + static_cast<size_t>(cs) * kBBytes);
+#pragma unroll
+        for (int i = ctid; i < static_cast<int>(kBBytes / 16); i += 32 * kConvWarps) {
+          const float4 a = br[i];
+          float4 l;
+          float hh;
+          l.x = tf32_lo(a.x, hh); l.y = tf32_lo(a.y, hh); l.z = tf32_lo(a.z, hh); l.w = tf32_lo(a.w, hh);
+          bl[i] = l;
+        }
+        tmem_st_wait();
         fence_proxy_async_smem();
+        tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(&conv[st]);
+        if (lane == 0) mbar_arrive(&conv[cs]);
       }
     }
   } else if (warp >= 4) {
@@ -249,17 +271,19 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
 
 template <int NCH>
 cudaError_t launch_tc(const TcParams& p, const TcMaps& maps, int num_sms, cudaStream_t stream) {
-  constexpr uint32_t kStageBytes = 2 * kABytes + 2 * NCH * 4096u;
-  const uint32_t misc = 2 * 32 * NCH * 4 + (3 * kTcMaxStages + 4) * 8 + 16;
+  constexpr uint32_t kBBytes = NCH * 4096u;
+  constexpr uint32_t kRawBytes = kABytes + kBBytes;
+  const uint32_t misc = 2 * 32 * NCH * 4 + (2 * kTcMaxStages + 2 * kConvStages + 4) * 8 + 16;
   TcParams q = p;
-  int st = static_cast<int>((227u * 1024u - 1024u - misc) / kStageBytes);
+  int st = static_cast<int>((227u * 1024u - 1024u - misc - kConvStages * kBBytes) / kRawBytes);
   if (st > kTcMaxStages) st = kTcMaxStages;
   if (st < 2) return cudaErrorInvalidConfiguration;
   q.stages = st;
-  const uint32_t smem = 1024u + st * kStageBytes + misc;
+  const uint32_t smem = 1024u + st * kRawBytes + kConvStages * kBBytes + misc;
   cudaError_t e = cudaFuncSetAttribute(phi_combine_tc_kernel<NCH>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e != cudaSuccess) return e;
   long long blocks = q.g.total < num_sms ? q.g.total : num_sms;
+  ProfScope prof(kProfPhiCombineTc, stream);
   phi_combine_tc_kernel<NCH><<<static_cast<unsigned>(blocks), kTcThreads, smem, stream>>>(q, maps.L, maps.R);
   return cudaGetLastError();
 }
@@ -306,7 +330,6 @@ cudaError_t launch_phi_combine_tc(const PhiArgs& a, int level, int nch, const vo
   TcParams p{};
   p.phi = a.phi; p.w = a.w; p.part = a.part;
   p.g = phi_geom(a.batch, a.T, a.n, level, kTM, 32 * nch);
-  p.hi_inplace = env_int("HI_INPLACE", 0);
   if (p.g.total == 0) return cudaSuccess;
   const TcMaps& m = *static_cast<const TcMaps*>(maps);
   switch (nch) {
@@ -314,9 +337,6 @@ cudaError_t launch_phi_combine_tc(const PhiArgs& a, int level, int nch, const vo
     case 3: return launch_tc<3>(p, m, num_sms, stream);
     case 4: return launch_tc<4>(p, m, num_sms, stream);
     case 5: return launch_tc<5>(p, m, num_sms, stream);
-    case 6: return launch_tc<6>(p, m, num_sms, stream);
-    case 7: return launch_tc<7>(p, m, num_sms, stream);
-    case 8: return launch_tc<8>(p, m, num_sms, stream);
     default: return cudaErrorInvalidValue;
   }
 }

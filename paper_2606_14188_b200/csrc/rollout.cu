@@ -234,7 +234,10 @@ cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t strea
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  e = cudaLaunchKernelEx(&cfg, rollout_kernel, p);
+  {
+    ProfScope prof(kProfRollout, stream);
+    e = cudaLaunchKernelEx(&cfg, rollout_kernel, p);
+  }
   if (e == cudaSuccess) ++*launches;
   return e;
 }
