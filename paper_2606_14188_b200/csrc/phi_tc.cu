@@ -44,11 +44,13 @@ struct TcParams {
   float* part;
   PhiGeom g;
   int stages;
+  int dbg;  // experiment knock-outs (LTV_SCAN_TC_DBG): 1 = no stores, 2 = no R split, 4 = no L split, 8 = no TMA store
 };
 
 struct TcMaps {
   CUtensorMap L;  // 2-D [batch*P*n rows][n]           box 32 x 128
   CUtensorMap R;  // 3-D [batch*P blocks][n][n]        box 32 x 32 x 1
+  CUtensorMap O;  // 2-D [batch*P*n rows][n]           box 32 x 32 (epilogue stores)
 };
 
 __device__ __forceinline__ float tf32_lo(float a, float& hi) {
@@ -62,7 +64,7 @@ __device__ __forceinline__ float tf32_lo(float a, float& hi) {
 template <int NCH>
 __global__ void __launch_bounds__(kTcThreads, 1)
 phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL,
-                      const __grid_constant__ CUtensorMap mapR) {
+                      const __grid_constant__ CUtensorMap mapR, const __grid_constant__ CUtensorMap mapO) {
   constexpr int NT = 32 * NCH;
   constexpr uint32_t kBBytes = NCH * 4096u;
   constexpr uint32_t kRawBytes = kABytes + kBBytes;       // one TMA stage: L tile + R tile, fp32
@@ -78,7 +80,8 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
   const int ks_last = ((n - (nkb - 1) * kKB) + 7) / 8;  // k-steps of the last k-block that hold data
 
   uint8_t* lo_ring = smem + static_cast<size_t>(R) * kRawBytes;               // [kConvStages][kBBytes]
-  uint8_t* misc = lo_ring + kConvStages * kBBytes;
+  uint8_t* stage_out = lo_ring + kConvStages * kBBytes;                        // [4 warps][32 rows x 128 B]
+  uint8_t* misc = stage_out + 4 * 4096;
   float* wbuf = reinterpret_cast<float*>(misc);  // [2][NT]
   uint64_t* bars = reinterpret_cast<uint64_t*>(misc + 2 * NT * 4);
   uint64_t* full = bars;                            // [R] TMA bytes landed
@@ -105,6 +108,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
     fence_mbar_init();
     tma_prefetch_desc(&mapL);
     tma_prefetch_desc(&mapR);
+    tma_prefetch_desc(&mapO);
   }
   if (warp == 2) tmem_alloc<512>(tmem_slot);
   tc_fence_before();
@@ -187,6 +191,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
         }
         const uint8_t* sp = smem + static_cast<size_t>(rs) * kRawBytes;
         uint32_t vh[16], vl[16];
+        if (!(p.dbg & 4))
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           const float4 f = *reinterpret_cast<const float4*>(sp + row * 128 + (((4 * h + c) ^ (row & 7)) << 4));
@@ -201,6 +206,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
         tmem_st_32x16(ta + 32, vl);
         const float4* br = reinterpret_cast<const float4*>(sp + kABytes);
         float4* bl = reinterpret_cast<float4*>(lo_ring + static_cast<size_t>(cs) * kBBytes);
+        if (!(p.dbg & 2))
 #pragma unroll
         for (int i = ctid; i < static_cast<int>(kBBytes / 16); i += 32 * kConvWarps) {
           const float4 a = br[i];
@@ -237,6 +243,11 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
       mbar_wait(&tfull[acc], (lt >> 1) & 1);
       tc_fence_after();
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(wq * 32) << 16) + acc * NT;
+      // all 32 rows of this warp inside the interval: swizzled shared-memory box + TMA store (coalesced, off the
+      // LSU); otherwise (ragged last m-tile) masked row-per-thread stores
+      const bool box_ok = (t.m_tile * kTM + wq * 32 + 31) < t.cnt_t * n && !(p.dbg & 8);
+      const int row0 = static_cast<int>(qcol * n) + t.m_tile * kTM + wq * 32;
+      uint8_t* sbox = stage_out + wq * 4096;
       float tube = 0.f;
 #pragma unroll
       for (int cc = 0; cc < NCH; ++cc) {
@@ -245,7 +256,23 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
         tmem_ld_wait();
 #pragma unroll
         for (int e = 0; e < 32; ++e) tube = fmaf(fabsf(__uint_as_float(v[e])), wb[cc * 32 + e], tube);
-        if (valid) {
+        if (p.dbg & 1) continue;
+        if (box_ok) {
+          if (j0 + cc * 32 < n) {
+            if (lane == 0) tma_store_wait_read<0>();   // the previous box of this warp has been read out
+            __syncwarp();
+#pragma unroll
+            for (int e = 0; e < 8; ++e)
+              *reinterpret_cast<uint4*>(sbox + lane * 128 + ((e ^ (lane & 7)) << 4)) =
+                  make_uint4(v[4 * e], v[4 * e + 1], v[4 * e + 2], v[4 * e + 3]);
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) {
+              tma_store_2d(&mapO, j0 + cc * 32, row0, sbox);
+              tma_store_commit();
+            }
+          }
+        } else if (valid) {
 #pragma unroll
           for (int e = 0; e < 8; ++e) {
             if (j0 + cc * 32 + 4 * e < n)
@@ -260,6 +287,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
       if (lane == 0) mbar_arrive(&tempty[acc]);
       if (valid) p.part[((qcol + rho / n) * g.NT + t.n_tile) * n + rho % n] = tube;
     }
+    if (lane == 0) tma_store_wait_all<0>();   // shared memory must outlive the last bulk store
   }
   tc_fence_before();
   __syncthreads();
@@ -273,7 +301,7 @@ template <int NCH>
 cudaError_t launch_tc(const TcParams& p, const TcMaps& maps, int num_sms, cudaStream_t stream) {
   constexpr uint32_t kBBytes = NCH * 4096u;
   constexpr uint32_t kRawBytes = kABytes + kBBytes;
-  const uint32_t misc = 2 * 32 * NCH * 4 + (2 * kTcMaxStages + 2 * kConvStages + 4) * 8 + 16;
+  const uint32_t misc = 4 * 4096 + 2 * 32 * NCH * 4 + (2 * kTcMaxStages + 2 * kConvStages + 4) * 8 + 16;
   TcParams q = p;
   int st = static_cast<int>((227u * 1024u - 1024u - misc - kConvStages * kBBytes) / kRawBytes);
   if (st > kTcMaxStages) st = kTcMaxStages;
@@ -284,7 +312,7 @@ cudaError_t launch_tc(const TcParams& p, const TcMaps& maps, int num_sms, cudaSt
   if (e != cudaSuccess) return e;
   long long blocks = q.g.total < num_sms ? q.g.total : num_sms;
   ProfScope prof(kProfPhiCombineTc, stream);
-  phi_combine_tc_kernel<NCH><<<static_cast<unsigned>(blocks), kTcThreads, smem, stream>>>(q, maps.L, maps.R);
+  phi_combine_tc_kernel<NCH><<<static_cast<unsigned>(blocks), kTcThreads, smem, stream>>>(q, maps.L, maps.R, maps.O);
   return cudaGetLastError();
 }
 
@@ -322,6 +350,15 @@ cudaError_t phi_tc_make_maps(const PhiArgs& a, int nch, void* maps_out) {
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return cudaErrorInvalidValue;
   }
+  {
+    const cuuint64_t dims[2] = {n, static_cast<cuuint64_t>(a.batch) * P * n};
+    const cuuint64_t strides[1] = {n * 4};
+    const cuuint32_t box[2] = {32, 32};
+    if (enc(&m->O, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, a.phi, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+  }
   return cudaSuccess;
 }
 
@@ -330,6 +367,7 @@ cudaError_t launch_phi_combine_tc(const PhiArgs& a, int level, int nch, const vo
   TcParams p{};
   p.phi = a.phi; p.w = a.w; p.part = a.part;
   p.g = phi_geom(a.batch, a.T, a.n, level, kTM, 32 * nch);
+  p.dbg = env_int("TC_DBG", 0);
   if (p.g.total == 0) return cudaSuccess;
   const TcMaps& m = *static_cast<const TcMaps*>(maps);
   switch (nch) {
