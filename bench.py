@@ -90,15 +90,19 @@ class ClockSampler(threading.Thread):
 
 
 def workload(cfg_index, rank, world, batch_override=None):
-    """Per-rank inputs: rank r gets its own `batch` items (weak scaling: seed offset by rank)."""
+    """Per-rank inputs.  Weak scaling: the global batch is `batch * world` items of the same seeded workload and
+    rank r owns the contiguous shard `shard_range(global, r, world)` (no data-path collective: items are
+    independent); at world = 1 this is exactly BASELINE.json's config."""
+    from paper_2606_14188_b200.sharding import shard_range
     from workloads import config, generate
 
-    over = {}
-    if batch_override:
-        over["batch"] = batch_override
-    cfg = config(cfg_index, **over)
-    cfg["seed"] = cfg["seed"] + 1000 * rank
-    return cfg, generate(cfg)
+    base = config(cfg_index)
+    per_gpu = batch_override or base["batch"]
+    cfg = config(cfg_index, batch=per_gpu * world)
+    b0, b1 = shard_range(cfg["batch"], rank, world)
+    W = generate(cfg, item_range=(b0, b1))
+    cfg["batch"] = per_gpu
+    return cfg, W
 
 
 def cpu_oracle_step(W, items):

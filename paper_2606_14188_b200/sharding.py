@@ -1,0 +1,35 @@
+"""Batch sharding for N > 1 GPUs: the LTV path has no data-path collective (items are independent), so a
+rank just owns a contiguous range of batch items; timing is reduced with a MAX over ranks."""
+from __future__ import annotations
+
+
+def shard_range(global_batch: int, rank: int, world: int) -> tuple[int, int]:
+    """Contiguous, balanced [b0, b1) of `global_batch` items for `rank` of `world` (sizes differ by <= 1)."""
+    if not (0 <= rank < world) or global_batch < 0:
+        raise ValueError("bad rank/world/batch")
+    base, rem = divmod(global_batch, world)
+    b0 = rank * base + min(rank, rem)
+    return b0, b0 + base + (1 if rank < rem else 0)
+
+
+def reduce_max(value: float, device=None) -> float:
+    """max over ranks of a python float (identity when torch.distributed is not initialised)."""
+    import torch
+    import torch.distributed as dist
+
+    if not (dist.is_available() and dist.is_initialized()):
+        return float(value)
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def reduce_sum(value: float, device=None) -> float:
+    import torch
+    import torch.distributed as dist
+
+    if not (dist.is_available() and dist.is_initialized()):
+        return float(value)
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())

@@ -1,0 +1,136 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (same binding calls, same
+batch, default cluster / tile choices).  The oracle cannot produce 11 GB of Phi in seconds, so outputs are
+SAMPLED: whole items for the vector outputs and the tube, single blocks Phi(t,s) (oracle/phi_block: the plain
+ordered product) for the system response, plus properties that hold at any size (semigroup identity, r_0 = 0,
+translation fixed point of the mass-spring generator).  Tolerance 1e-4 (north_star), per sampled tensor."""
+import numpy as np
+import pytest
+
+from oracle import ltv_oracle as O
+from workloads import config, generate
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def L():
+    import torch
+
+    assert torch.cuda.is_available()
+    import __graft_entry__ as G
+
+    G.build()
+    import paper_2606_14188_b200 as lib
+
+    return lib
+
+
+def _dev(W, keys=("A", "B", "c", "x0", "u", "w", "g")):
+    import torch
+
+    return {k: torch.from_numpy(getattr(W, k)).cuda() for k in keys}
+
+
+def _vector_outputs(L, W, d, items):
+    import torch
+
+    x = L.ltv_scan_rollout(d["A"], d["B"], d["c"], d["x0"], d["u"])
+    lam, gu, gx0 = L.ltv_scan_adjoint(d["A"], d["B"], d["g"])
+    torch.cuda.synchronize()
+    for b in items:
+        assert O.rel_err(x[b].cpu().numpy(), O.rollout_item(W.A[b], W.B[b], W.c[b], W.x0[b], W.u[b])) <= TOL
+        rl, rgu, rgx = O.adjoint_item(W.A[b], W.B[b], W.g[b])
+        assert O.rel_err(lam[b].cpu().numpy(), rl) <= TOL
+        assert O.rel_err(gu[b].cpu().numpy(), rgu) <= TOL
+        assert O.rel_err(gx0[b].cpu().numpy(), rgx) <= TOL
+    assert bool(torch.isfinite(x).all()) and bool(torch.isfinite(lam).all())
+
+
+def _phi_samples(L, W, phi, samples):
+    T = W.A.shape[1]
+    worst = 0.0
+    for b, t, s in samples:
+        ref = O.phi_block(W.A[b], t, s)
+        got = phi[b, L.ltv_phi_block_index(T, t, s)].cpu().numpy()
+        worst = max(worst, O.rel_err(got, ref))
+    assert worst <= TOL, worst
+    return worst
+
+
+def _semigroup(L, phi, b, t, k, s, T):
+    """Phi(t,s) = Phi(t,k) Phi(k,s): checked on the GPU's own blocks in fp64 (a property, not the oracle)."""
+    q = lambda tt, ss: phi[b, L.ltv_phi_block_index(T, tt, ss)].double()
+    lhs = q(t, s)
+    rhs = q(t, k) @ q(k, s)
+    err = float((lhs - rhs).abs().max() / rhs.abs().max())
+    assert err <= TOL, err
+
+
+def test_c2_full(L):
+    import torch
+
+    W = generate(config(1))                               # n=300, T=32, batch=64: the bench workload
+    batch, T, n, m = W.shape
+    d = _dev(W)
+    _vector_outputs(L, W, d, items=[0, 31, 63])
+    phi, r = L.ltv_scan_system_response_tube(d["A"], d["w"])
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(r).all()) and bool((r[:, 0] == 0).all())
+    # whole tube + every block of two items (the oracle needs ~1 s per item here)
+    for b in (0, 63):
+        ref_phi, ref_r = O.system_response_tube_item(W.A[b], W.w[b])
+        perm = [O.packed_index(t, s) for s in range(T - 1) for t in range(s + 1, T)]
+        assert O.rel_err(phi[b].cpu().numpy(), ref_phi[perm]) <= TOL
+        assert O.rel_err(r[b].cpu().numpy(), ref_r) <= TOL
+    _phi_samples(L, W, phi, [(17, 31, 0), (40, 16, 15), (5, 24, 7), (62, 2, 0), (33, 31, 30)])
+    _semigroup(L, phi, 21, 31, 16, 0, T)
+    # translation fixed point (L 1 = 0): Phi(t,s) tau = tau for every block of an item
+    N = n // 6
+    tau = torch.zeros(n, device="cuda")
+    tau[0:3 * N:3] = 1.0
+    assert float((phi[7] @ tau - tau).abs().max()) < 1e-3
+
+
+def test_c3_full(L):
+    import torch
+
+    W = generate(config(2))                               # n=600, T=32, batch=16
+    batch, T, n, m = W.shape
+    d = _dev(W)
+    _vector_outputs(L, W, d, items=[0, 15])
+    phi, r = L.ltv_scan_system_response_tube(d["A"], d["w"])
+    torch.cuda.synchronize()
+    ref_phi, ref_r = O.system_response_tube_item(W.A[3], W.w[3])
+    perm = [O.packed_index(t, s) for s in range(T - 1) for t in range(s + 1, T)]
+    assert O.rel_err(phi[3].cpu().numpy(), ref_phi[perm]) <= TOL
+    assert O.rel_err(r[3].cpu().numpy(), ref_r) <= TOL
+    _phi_samples(L, W, phi, [(0, 31, 0), (15, 20, 3), (9, 1, 0)])
+    _semigroup(L, phi, 12, 30, 8, 1, T)
+
+
+def test_c4_full(L):
+    import torch
+
+    W = generate(config(3))                               # n=2400, T=16, batch=4, m=12
+    batch, T, n, m = W.shape
+    d = _dev(W)
+    _vector_outputs(L, W, d, items=[0, 3])
+    phi, r = L.ltv_scan_system_response_tube(d["A"], d["w"])
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(r).all()) and bool((r[:, 0] == 0).all())
+    _phi_samples(L, W, phi, [(0, 2, 0), (3, 15, 12), (1, 9, 4), (2, 15, 0)])
+    _semigroup(L, phi, 1, 15, 8, 0, T)
+    # r_1 and r_2 of one item from the definition (|A_0| w_0; |A_1 A_0| w_0 + |A_1| w_1)
+    A = W.A[2].astype(np.float64)
+    w = W.w[2].astype(np.float64)
+    r1 = np.abs(A[0]) @ w[0]
+    r2 = np.abs(A[1] @ A[0]) @ w[0] + np.abs(A[1]) @ w[1]
+    assert O.rel_err(r[2, 1].cpu().numpy(), r1) <= TOL and O.rel_err(r[2, 2].cpu().numpy(), r2) <= TOL
+
+
+@pytest.mark.parametrize("batch", [64, 256, 1024])
+def test_c5_sweep(L, batch):
+    W = generate(config(4, batch=batch))                  # n=180, T=64: rollout + adjoint only
+    d = _dev(W, keys=("A", "B", "c", "x0", "u", "g"))
+    _vector_outputs(L, W, d, items=[0, batch // 2, batch - 1])

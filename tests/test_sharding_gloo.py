@@ -1,0 +1,69 @@
+"""N > 1 host logic on CPU: world_size-2 gloo.  Shards partition the batch, every rank generates exactly the
+items of the unsharded workload it owns, the oracle on the shards equals the oracle on the whole batch (no
+collective is needed on the data path), and the timing reduction is a max over ranks."""
+import os
+import socket
+
+import numpy as np
+import torch.multiprocessing as mp
+
+from paper_2606_14188_b200.sharding import shard_range
+
+
+def test_shard_range_partitions():
+    for gb in (0, 1, 5, 64, 1023):
+        for world in (1, 2, 3, 8):
+            r = [shard_range(gb, k, world) for k in range(world)]
+            assert r[0][0] == 0 and r[-1][1] == gb
+            assert all(r[k][1] == r[k + 1][0] for k in range(world - 1))
+            sizes = [b - a for a, b in r]
+            assert max(sizes) - min(sizes) <= 1
+
+
+def _worker(rank, world, port, q):
+    import torch.distributed as dist
+
+    from oracle import ltv_oracle as O
+    from paper_2606_14188_b200.sharding import reduce_max, reduce_sum
+    from workloads import config, generate
+
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    cfg = config(0, batch=5, T=6)
+    b0, b1 = shard_range(cfg["batch"], rank, world)
+    W = generate(cfg, item_range=(b0, b1))
+    X = O.rollout(W.A, W.B, W.c, W.x0, W.u)
+    r = O.tube(W.A, W.w)
+    t_max = reduce_max(1.0 + rank)              # "time" of this rank
+    units = reduce_sum(float(b1 - b0))
+    q.put((rank, b0, b1, X, r, t_max, units))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_batch_sharding_gloo():
+    from oracle import ltv_oracle as O
+    from workloads import config, generate
+
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    world = 2
+    procs = [ctx.Process(target=_worker, args=(k, world, port, q)) for k in range(world)]
+    for p in procs:
+        p.start()
+    got = sorted([q.get(timeout=120) for _ in range(world)], key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    W = generate(config(0, batch=5, T=6))
+    X = O.rollout(W.A, W.B, W.c, W.x0, W.u)
+    r = O.tube(W.A, W.w)
+    assert np.array_equal(np.concatenate([g[3] for g in got]), X)
+    assert np.array_equal(np.concatenate([g[4] for g in got]), r)
+    assert all(g[5] == 2.0 for g in got)        # max over ranks
+    assert all(g[6] == 5.0 for g in got)        # units of all ranks
