@@ -116,60 +116,74 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
+  // NOTE on the two single-thread roles: the whole warp runs the loops and the mbarrier waits (warp-uniform
+  // control flow) and one lane is picked with elect.sync only around the TMA / MMA instructions.  Those
+  // instructions live on the uniform datapath; issued from a divergent `lane == 0` branch the compiler wraps
+  // every one of them in an election loop, which made the MMA warp issue-bound (measured: ~110 instead of 80
+  // cycles per MMA).
   if (warp == 0) {
     // ---------------------------------------------------------------------------------- TMA producer
-    if (lane == 0) {
-      const uint64_t pol = l2_policy_evict_last();  // operands are re-read by many tiles: keep them in L2
-      uint32_t it = 0;
-      for (long long idx = blockIdx.x; idx < g.total; idx += gridDim.x) {
-        const PhiTile t = phi_decode(g, idx);
-        const long long item = static_cast<long long>(t.b) * g.P;
-        const int rowL = static_cast<int>((item + phi_colbase(g.T, t.mid)) * n) + t.m_tile * kTM;
-        const int blkR = static_cast<int>(item + phi_colbase(g.T, t.s) + (t.mid - t.s - 1));
-        const int j0 = t.n_tile * NT;
-        for (int kb = 0; kb < nkb; ++kb, ++it) {
-          const int rs = it % R;
-          const uint32_t use = it / R;
-          if (use > 0) mbar_wait(&rempty[rs], (use - 1) & 1);
-          uint8_t* sp = smem + static_cast<size_t>(rs) * kRawBytes;
-          mbar_arrive_expect_tx(&full[rs], kRawBytes);
-          tma_load_2d(sp, &mapL, kb * kKB, rowL, &full[rs], pol);
+    const uint64_t pol = l2_policy_evict_last();  // operands are re-read by many tiles: keep them in L2
+    uint32_t it = 0;
+    for (long long idx = blockIdx.x; idx < g.total; idx += gridDim.x) {
+      const PhiTile t = phi_decode(g, idx);
+      const long long item = static_cast<long long>(t.b) * g.P;
+      const int rowL = static_cast<int>((item + phi_colbase(g.T, t.mid)) * n) + t.m_tile * kTM;
+      const int blkR = static_cast<int>(item + phi_colbase(g.T, t.s) + (t.mid - t.s - 1));
+      const int j0 = t.n_tile * NT;
+      for (int kb = 0; kb < nkb; ++kb, ++it) {
+        const int rs = it % R;
+        const uint32_t use = it / R;
+        if (use > 0) mbar_wait(&rempty[rs], (use - 1) & 1);
+        uint8_t* sp = smem + static_cast<size_t>(rs) * kRawBytes;
+        if (elect_one()) {
+          mbar_arrive_expect_tx(&full[rs], ((p.dbg & 32) ? 0u : kABytes) + ((p.dbg & 64) ? 0u : kBBytes));
+          if (!(p.dbg & 32)) tma_load_2d(sp, &mapL, kb * kKB, rowL, &full[rs], pol);
+          if (!(p.dbg & 64)) {
 #pragma unroll
-          for (int c = 0; c < NCH; ++c)
-            tma_load_3d(sp + kABytes + c * 4096, &mapR, j0 + 32 * c, kb * kKB, blkR, &full[rs], pol);
+            for (int c = 0; c < NCH; ++c)
+              tma_load_3d(sp + kABytes + c * 4096, &mapR, j0 + 32 * c, kb * kKB, blkR, &full[rs], pol);
+          }
         }
+        __syncwarp();
       }
     }
   } else if (warp == 1) {
     // ---------------------------------------------------------------------------------- MMA issuer
-    if (lane == 0) {
-      constexpr uint32_t idesc = umma_idesc_tf32(kTM, NT, 0, 1);
-      uint32_t it = 0, lt = 0;
-      for (long long idx = blockIdx.x; idx < g.total; idx += gridDim.x, ++lt) {
-        const uint32_t acc = lt & 1;
-        if (lt >= 2) mbar_wait(&tempty[acc], ((lt >> 1) - 1) & 1);
+    constexpr uint32_t idesc = umma_idesc_tf32(kTM, NT, 0, 1);
+    uint32_t it = 0, lt = 0;
+    for (long long idx = blockIdx.x; idx < g.total; idx += gridDim.x, ++lt) {
+      const uint32_t acc = lt & 1;
+      if (lt >= 2) mbar_wait(&tempty[acc], ((lt >> 1) - 1) & 1);
+      tc_fence_after();
+      const uint32_t d_tmem = tmem_base + acc * NT;
+      for (int kb = 0; kb < nkb; ++kb, ++it) {
+        const int rs = it % R, cs = it % kConvStages;
+        if (!(p.dbg & 256)) mbar_wait(&conv[cs], (it / kConvStages) & 1);
         tc_fence_after();
-        const uint32_t d_tmem = tmem_base + acc * NT;
-        for (int kb = 0; kb < nkb; ++kb, ++it) {
-          const int rs = it % R, cs = it % kConvStages;
-          mbar_wait(&conv[cs], (it / kConvStages) & 1);
-          tc_fence_after();
-          const uint32_t sb_hi = smem_u32(smem + static_cast<size_t>(rs) * kRawBytes + kABytes);
-          const uint32_t sb_lo = smem_u32(lo_ring + static_cast<size_t>(cs) * kBBytes);
-          const uint32_t a_hi = tmem_base + kTmemA + cs * 64;   // raw fp32 bits: the MMA keeps the top 19
-          const uint32_t a_lo = a_hi + 32;
-          const int nks = (kb == nkb - 1) ? ks_last : 4;
-          for (int ks = 0; ks < nks; ++ks) {
-            const uint64_t b_hi = umma_smem_desc(sb_hi + ks * 1024, 4096, 512, kUmmaSw128Base32);
-            const uint64_t b_lo = umma_smem_desc(sb_lo + ks * 1024, 4096, 512, kUmmaSw128Base32);
-            umma_tf32_ts(d_tmem, a_lo + ks * 8, b_hi, idesc, (kb | ks) != 0);
-            umma_tf32_ts(d_tmem, a_hi + ks * 8, b_lo, idesc, 1);
-            umma_tf32_ts(d_tmem, a_hi + ks * 8, b_hi, idesc, 1);
+        const uint32_t sb_hi = smem_u32(smem + static_cast<size_t>(rs) * kRawBytes + kABytes);
+        const uint32_t sb_lo = smem_u32(lo_ring + static_cast<size_t>(cs) * kBBytes);
+        const uint32_t a_hi = tmem_base + kTmemA + cs * 64;   // raw fp32 bits: the MMA keeps the top 19
+        const uint32_t a_lo = a_hi + 32;
+        const int nks = (kb == nkb - 1) ? ks_last : 4;
+        if (elect_one()) {
+#pragma unroll
+          for (int ks = 0; ks < 4; ++ks) {
+            if (ks < nks) {
+              const uint64_t b_hi = umma_smem_desc(sb_hi + ks * 1024, 4096, 512, kUmmaSw128Base32);
+              const uint64_t b_lo = umma_smem_desc(sb_lo + ks * 1024, 4096, 512, kUmmaSw128Base32);
+              if (!(p.dbg & 16)) {
+                umma_tf32_ts(d_tmem, a_lo + ks * 8, b_hi, idesc, (kb | ks) != 0);
+                umma_tf32_ts(d_tmem, a_hi + ks * 8, b_lo, idesc, 1);
+              }
+              umma_tf32_ts(d_tmem, a_hi + ks * 8, b_hi, idesc, (p.dbg & 16) ? ((kb | ks) != 0) : 1);
+            }
           }
           umma_commit(&rempty[rs]);
           umma_commit(&cempty[cs]);
+          if (kb == nkb - 1) umma_commit(&tfull[acc]);
         }
-        umma_commit(&tfull[acc]);
+        __syncwarp();
       }
     }
   } else if (warp >= 8) {
@@ -202,8 +216,10 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
           vh[4 * c + 3] = __float_as_uint(f.w); vl[4 * c + 3] = __float_as_uint(tf32_lo(f.w, hh));
         }
         const uint32_t ta = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + kTmemA + cs * 64 + h * 16;
-        tmem_st_32x16(ta, vh);
-        tmem_st_32x16(ta + 32, vl);
+        if (!(p.dbg & 128)) {
+          tmem_st_32x16(ta, vh);
+          tmem_st_32x16(ta + 32, vl);
+        }
         const float4* br = reinterpret_cast<const float4*>(sp + kABytes);
         float4* bl = reinterpret_cast<float4*>(lo_ring + static_cast<size_t>(cs) * kBBytes);
         if (!(p.dbg & 2))
@@ -215,9 +231,11 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
           l.x = tf32_lo(a.x, hh); l.y = tf32_lo(a.y, hh); l.z = tf32_lo(a.z, hh); l.w = tf32_lo(a.w, hh);
           bl[i] = l;
         }
-        tmem_st_wait();
-        fence_proxy_async_smem();
-        tc_fence_before();
+        if (!(p.dbg & 128)) {
+          tmem_st_wait();
+          fence_proxy_async_smem();
+          tc_fence_before();
+        }
         __syncwarp();
         if (lane == 0) mbar_arrive(&conv[cs]);
       }
