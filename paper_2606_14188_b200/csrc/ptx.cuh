@@ -39,6 +39,18 @@ __device__ __forceinline__ void mbar_arrive_remote(uint64_t* bar, uint32_t cta_r
       ::"r"(smem_u32(bar)), "r"(cta_rank)
       : "memory");
 }
+// same, default (.release.cta) semantics: what CUTLASS's ClusterBarrier::arrive(cta_id) emits.  Used where the
+// data being published is consumed by the async proxy / tensor core (made visible by tcgen05.wait::st,
+// fence.proxy.async and tcgen05.fence::before_thread_sync), not by generic loads of the waiting thread: a
+// cluster-scope release costs a full memory barrier per arrival.
+__device__ __forceinline__ void mbar_arrive_remote_relaxed(uint64_t* bar, uint32_t cta_rank) {
+  asm volatile(
+      "{\n\t.reg .b32 ra;\n\t"
+      "mapa.shared::cluster.u32 ra, %0, %1;\n\t"
+      "mbarrier.arrive.shared::cluster.b64 _, [ra];\n\t}"
+      ::"r"(smem_u32(bar)), "r"(cta_rank)
+      : "memory");
+}
 __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
   uint32_t ok;
   asm volatile(
