@@ -30,6 +30,20 @@ int pick_cluster(int batch, int n, int num_sms) {
   return c;
 }
 
+// The HBM stream needs (nearly) every SM pulling: one SM sustains ~48 GB/s (measured), so take the smallest
+// power-of-two cluster that puts CTAs on at least three quarters of the SMs.  `occ` (CTAs per SM) stays 1: the
+// 18-warp CTA needs most of an SM's registers and shared memory.
+void pick_rollout_shape(int batch, int n, int num_sms, int* cluster, int* occ) {
+  int c = 1;
+  while (c < 16 && static_cast<long long>(batch) * c * 4 < 3ll * num_sms && n / (2 * c) >= 32) c *= 2;
+  int o = 1;
+  const int fc = env_int("CLUSTER", 0), fo = env_int("OCC", 0);
+  if (fc == 1 || fc == 2 || fc == 4 || fc == 8 || fc == 16) c = fc;
+  if (fo == 1 || fo == 2) o = fo;
+  *cluster = c;
+  *occ = o;
+}
+
 // ---- optional kernel timing --------------------------------------------------------------------------
 namespace {
 struct ProfState {
@@ -154,8 +168,14 @@ int ltv_scan_rollout(const float* A, const float* B, const float* c, const float
   RolloutArgs a{A, B, c, x0, u, x_out, batch, T, n, m};
   unsigned long long l = 0;
   cudaError_t e = cudaErrorUnknown;
-  for (int cl = pick_cluster(batch, n, sms); cl >= 1; cl /= 2) {  // a 16-CTA cluster may not be placeable
-    e = launch_rollout(a, cl, static_cast<cudaStream_t>(cuda_stream), &l);
+  int cl = 1, occ = 1;
+  pick_rollout_shape(batch, n, sms, &cl, &occ);
+  for (; cl >= 1; cl /= 2) {  // a 16-CTA cluster may not be placeable
+    e = launch_rollout(a, cl, occ, sms, static_cast<cudaStream_t>(cuda_stream), &l);
+    if (e != cudaSuccess && occ > 1) {
+      cudaGetLastError();
+      e = launch_rollout(a, cl, 1, sms, static_cast<cudaStream_t>(cuda_stream), &l);
+    }
     if (e == cudaSuccess) break;
     cudaGetLastError();
   }

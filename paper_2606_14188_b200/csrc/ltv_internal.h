@@ -14,7 +14,8 @@ struct RolloutArgs {
   float* x_out;
   int batch, T, n, m;
 };
-cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches);
+cudaError_t launch_rollout(const RolloutArgs& a, int cluster, int occ, int num_sms, cudaStream_t stream,
+                           unsigned long long* launches);
 
 struct AdjointArgs {
   const float *A, *B, *g;
@@ -35,8 +36,10 @@ bool phi_uses_tensor_cores(int n);
 size_t phi_workspace_bytes(int batch, int T, int n);
 cudaError_t launch_phi_tube(const PhiArgs& a, cudaStream_t stream, unsigned long long* launches);
 
-// cluster-size heuristic shared by rollout and adjoint (power of two, 1..16)
+// cluster-size heuristic of the adjoint (power of two, 1..16)
 int pick_cluster(int batch, int n, int num_sms);
+// rollout: CTAs per item (power of two, 1..16) and CTAs per SM (1 or 2) so that every SM streams
+void pick_rollout_shape(int batch, int n, int num_sms, int* cluster, int* occ);
 // environment override for experiments: LTV_SCAN_<name>=<int>; returns `dflt` if unset
 int env_int(const char* name, int dflt);
 

@@ -21,17 +21,31 @@
 #include "ltv_internal.h"
 #include "ptx.cuh"
 
-#ifndef LTV_ROLL_DBG
-#define LTV_ROLL_DBG 0
-#endif
-
 namespace ltv {
+
+#ifdef LTV_ROLL_TRACE
+static unsigned long long* g_roll_trace = nullptr;
+static int g_roll_trace_cap = 0;
+extern "C" __attribute__((visibility("default"))) void ltv_debug_set_roll_trace(void* ptr, int cap) {
+  g_roll_trace = static_cast<unsigned long long*>(ptr);
+  g_roll_trace_cap = cap;
+}
+#define LTV_RT(role, idx, ev)                                                                      \
+  if (p.trace && blockIdx.x == 0 && lane == 0 && static_cast<int>(idx) < p.trace_cap)              \
+    p.trace[(static_cast<size_t>(role) * p.trace_cap + (idx)) * 4 + (ev)] = clock64();
+#else
+#define LTV_RT(role, idx, ev)
+#endif
 
 namespace {
 
-constexpr int kConsWarps = 8;
-constexpr int kRollThreads = (kConsWarps + 2) * 32;  // + producer warp + affine warp
+constexpr int kConsWarps = 8;    // warps of one consumer group
+constexpr int kGroups = 2;       // consumer groups; group g takes the ring chunks with index % kGroups == g
+constexpr int kAllCons = kConsWarps * kGroups;
+constexpr int kRollThreads = (kAllCons + 2) * 32;  // + producer warp + affine warp
 constexpr int kMaxStages = 8;
+constexpr int kBStages = 4;     // affine terms formed ahead of the consumers
+constexpr int kStageVecs = 384; // float4 of the B band the affine warp stages in shared memory (6 KB)
 constexpr int kModeAMaxN = 640;
 
 struct RollSmemPlan {
@@ -40,13 +54,16 @@ struct RollSmemPlan {
   int wide;            // 0 = mode A, 1 = mode B
   int stages;
   uint32_t stage_bytes;
-  uint32_t off_x, off_b, off_part, off_bar, total;
+  uint32_t off_x, off_b, off_part, off_stage, off_bar, total;
   int rows_max;        // max rows owned by one CTA
 };
 
+// rows [r0, r1) of CTA `rank`: multiples of 4 rows (n % 4 == 0), so that the bands of A, B and c start on
+// 16-byte boundaries
 __host__ __device__ inline void band(int n, int C, int rank, int& r0, int& r1) {
-  r0 = static_cast<int>((static_cast<long long>(n) * rank) / C);
-  r1 = static_cast<int>((static_cast<long long>(n) * (rank + 1)) / C);
+  const long long nq = n >> 2;
+  r0 = 4 * static_cast<int>((nq * rank) / C);
+  r1 = 4 * static_cast<int>((nq * (rank + 1)) / C);
 }
 
 struct RollParams {
@@ -54,6 +71,8 @@ struct RollParams {
   float* x_out;
   int batch, T, n, m;
   RollSmemPlan sp;
+  unsigned long long* trace;   // experiments only (LTV_ROLL_TRACE)
+  int trace_cap;
 };
 
 // Four per-lane partial sums (one per row) -> every lane of lane group g = lane / 8 holds the complete sum of
@@ -76,24 +95,31 @@ __device__ __forceinline__ float dot4(const float4 a, const float4 x, float acc)
   return fmaf(a.x, x.x, fmaf(a.y, x.y, fmaf(a.z, x.z, fmaf(a.w, x.w, acc))));
 }
 
-// acc[r] += sum_j A[row_r][q0 + 32 j] . xq[j] for four rows of a shared-memory tile (row stride n floats);
-// quads at or beyond q_end are skipped, rows flagged invalid contribute nothing (their address is clamped by
-// the caller so that the loads stay inside the stage)
-template <int QLMAX>
-__device__ __forceinline__ void rows4_dot(const float* tile, int n, const int (&rowi)[4], int q0, int q_end, int ql,
-                                          const float4 (&xq)[QLMAX], float (&acc)[4]) {
+// acc[r] += sum_j A[row0 + r][q0 + 32 j] . xq[j] for NR consecutive rows of a shared-memory tile (row stride n
+// floats); quads at or beyond q_end are skipped.  All NR x ql loads of a pass are independent.
+template <int QLMAX, int NR>
+__device__ __forceinline__ void rows_dot(const float* tile, int n, int row0, int q0, int q_end, int ql,
+                                         const float4 (&xq)[QLMAX], float (&acc)[4]) {
+  const float* base = tile + static_cast<size_t>(row0) * n + 4 * q0;
 #pragma unroll
   for (int j = 0; j < QLMAX; ++j) {
-    if (j < ql) {
-      const int q = q0 + 32 * j;
-      if (q < q_end) {
+    if (j < ql && q0 + 32 * j < q_end) {
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
-          const float4 a = *reinterpret_cast<const float4*>(tile + static_cast<size_t>(rowi[r]) * n + 4 * q);
-          acc[r] = dot4(a, xq[j], acc[r]);
-        }
+      for (int r = 0; r < NR; ++r) {
+        const float4 a = *reinterpret_cast<const float4*>(base + static_cast<size_t>(r) * n + 128 * j);
+        acc[r] = dot4(a, xq[j], acc[r]);
       }
     }
+  }
+}
+template <int QLMAX>
+__device__ __forceinline__ void rows_dot_n(int nr, const float* tile, int n, int row0, int q0, int q_end, int ql,
+                                           const float4 (&xq)[QLMAX], float (&acc)[4]) {
+  switch (nr) {   // warp-uniform
+    case 4: rows_dot<QLMAX, 4>(tile, n, row0, q0, q_end, ql, xq, acc); break;
+    case 3: rows_dot<QLMAX, 3>(tile, n, row0, q0, q_end, ql, xq, acc); break;
+    case 2: rows_dot<QLMAX, 2>(tile, n, row0, q0, q_end, ql, xq, acc); break;
+    default: rows_dot<QLMAX, 1>(tile, n, row0, q0, q_end, ql, xq, acc); break;
   }
 }
 
@@ -103,7 +129,7 @@ __global__ void __launch_bounds__(kRollThreads, 1) rollout_kernel(const RollPara
   extern __shared__ __align__(128) uint8_t smem[];
   const int C = static_cast<int>(cluster_nctarank());
   const int rank = static_cast<int>(cluster_ctarank());
-  const int item = blockIdx.x / C;
+  const int cl = blockIdx.x / C, ncl = gridDim.x / C;   // this cluster, clusters in the grid
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int n = p.n, T = p.T, m = p.m;
   int r0, r1;
@@ -113,168 +139,249 @@ __global__ void __launch_bounds__(kRollThreads, 1) rollout_kernel(const RollPara
   const int nchunks = (rows + rc - 1) / rc;
 
   float* ring = reinterpret_cast<float*>(smem);
-  float* xbuf = reinterpret_cast<float*>(smem + p.sp.off_x);   // [2][n]
-  float* bvec = reinterpret_cast<float*>(smem + p.sp.off_b);   // [2][rows_max]
-  float* part = reinterpret_cast<float*>(smem + p.sp.off_part);  // mode B: [2][kConsWarps][4]
+  float* xbuf = reinterpret_cast<float*>(smem + p.sp.off_x);   // [3][n]
+  float* bvec = reinterpret_cast<float*>(smem + p.sp.off_b);   // [kBStages][rows_max]
+  float* part = reinterpret_cast<float*>(smem + p.sp.off_part);  // mode B: [kGroups][2][kConsWarps][4]
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + p.sp.off_bar);
   uint64_t* full = bars;                    // [stages]  producer -> consumers (tx bytes)
   uint64_t* empty = bars + kMaxStages;      // [stages]  consumers -> producer (kConsWarps arrivals)
-  uint64_t* xfull = bars + 2 * kMaxStages;  // [2]       x_{t} complete in xbuf[t&1] (n*4 tx bytes + 1 arrival)
-  uint64_t* bfull = xfull + 2;              // [2]       b_t complete in bvec[t&1]
+  uint64_t* xfull = bars + 2 * kMaxStages;  // [3]       state number g complete in xbuf[g % 3]
+  uint64_t* bfull = xfull + 3;              // [kBStages] affine term number h complete in bvec[h % kBStages]
+  uint64_t* bempty = bfull + kBStages;      // [kBStages] consumers are done with it (kAllCons arrivals)
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < stages; ++s) {
       mbar_init(&full[s], 1);
       mbar_init(&empty[s], kConsWarps);
     }
-    mbar_init(&xfull[0], 1);
-    mbar_init(&xfull[1], 1);
-    mbar_init(&bfull[0], 1);
-    mbar_init(&bfull[1], 1);
+    for (int s = 0; s < 3; ++s) mbar_init(&xfull[s], 1);
+    for (int s = 0; s < kBStages; ++s) {
+      mbar_init(&bfull[s], 1);
+      mbar_init(&bempty[s], kAllCons);
+    }
     fence_mbar_init();
   }
-  for (int j = threadIdx.x; j < n; j += kRollThreads) xbuf[j] = p.x0[static_cast<size_t>(item) * n + j];
   __syncthreads();
   cluster_sync_all();  // every CTA's barriers are initialised before any remote st.async can target them
 
-  const size_t itemA = static_cast<size_t>(item) * T * n * n;
-
-  if (warp == kConsWarps) {
+  // Persistent over items: cluster `cl` takes items cl, cl + ncl, ...  Steps are numbered h = j T + t over the
+  // item rounds j.  x_0 is read from global memory by the consumers themselves; x_{t+1}, t + 1 < T, is
+  // exchanged through xbuf[(h+1) % 3] behind xfull[(h+1) % 3] (armed by consumer thread 0 at the start of
+  // step t); the affine term b_t lives in bvec[h % kBStages] behind bfull / bempty, formed up to kBStages
+  // steps ahead by a warp that depends on nothing but those buffers.  The producer streams A straight
+  // through item boundaries.
+  if (warp == kAllCons) {
     // ------------------------------------------------------------------ producer (one thread)
     if (lane == 0 && rows > 0) {
       const uint64_t pol = l2_policy_evict_first();
       int st = 0;
       uint32_t eph = 1;   // parity of empty[st] to wait for (the first pass over the ring does not block)
-      for (int t = 0; t < T; ++t) {
-        const float* At = p.A + itemA + (static_cast<size_t>(t) * n + r0) * n;
-        for (int k = 0; k < nchunks; ++k) {
-          mbar_wait(&empty[st], eph);
-          const int rk = min(rc, rows - k * rc);
-          const uint32_t bytes = static_cast<uint32_t>(rk) * n * 4u;
-          mbar_arrive_expect_tx(&full[st], bytes);
-          bulk_g2s(reinterpret_cast<uint8_t*>(ring) + static_cast<size_t>(st) * p.sp.stage_bytes,
-                   At + static_cast<size_t>(k) * rc * n, bytes, &full[st], pol);
-          if (++st == stages) { st = 0; eph ^= 1; }
+      uint32_t pit = 0;
+      (void)pit;
+      for (int item = cl; item < p.batch; item += ncl) {
+        const size_t itemA = static_cast<size_t>(item) * T * n * n;
+        for (int t = 0; t < T; ++t) {
+          const float* At = p.A + itemA + (static_cast<size_t>(t) * n + r0) * n;
+          for (int k = 0; k < nchunks; ++k) {
+            LTV_RT(0, pit, 0)
+            mbar_wait(&empty[st], eph);
+            LTV_RT(0, pit, 1)
+            const int rk = min(rc, rows - k * rc);
+            const uint32_t bytes = static_cast<uint32_t>(rk) * n * 4u;
+            mbar_arrive_expect_tx(&full[st], bytes);
+            bulk_g2s(reinterpret_cast<uint8_t*>(ring) + static_cast<size_t>(st) * p.sp.stage_bytes,
+                     At + static_cast<size_t>(k) * rc * n, bytes, &full[st], pol);
+            if (++st == stages) { st = 0; eph ^= 1; }
+            ++pit;
+          }
         }
       }
     }
-  } else if (warp == kConsWarps + 1) {
-    // ------------------------------------------------------------------ affine / output warp
-    // step t: wait x_t, arm the barrier of x_{t+1}, write x_t to global, form b_{t+1}
-    auto form_b = [&](int t) {
-      float* bv = bvec + (t & 1) * p.sp.rows_max;
-      const size_t bt = static_cast<size_t>(item) * T + t;
-      for (int i = lane; i < rows; i += 32) {
-        float acc = p.c ? p.c[bt * n + r0 + i] : 0.f;
-        if (p.B && p.u) {
-          const float* Brow = p.B + (bt * n + r0 + i) * m;
-          const float* ut = p.u + bt * m;
-          for (int l = 0; l < m; ++l) acc = fmaf(__ldg(Brow + l), __ldg(ut + l), acc);
+  } else if (warp == kAllCons + 1) {
+    // ------------------------------------------------------------------ affine warp: b_t = B_t u_t + c_t
+    // The bands of B_t and c_t are contiguous: all of their 128-bit loads (and u_t) are issued before the first
+    // use, so a step costs one memory latency however many rows the band has; B_t is staged in shared memory
+    // and reduced lane-per-row.  (Row-at-a-time loads made this warp the bottleneck at batch 1024, where B no
+    // longer sits in L2.)
+    float4* stB = reinterpret_cast<float4*>(smem + p.sp.off_stage);
+    const bool has_bu = p.B && p.u && m > 0;
+    const int nvB = has_bu ? (rows * m) >> 2 : 0, nvC = p.c ? rows >> 2 : 0;
+    const bool staged = nvB <= kStageVecs;
+    int bs = 0;
+    uint32_t bph = 1;   // parity of bempty[bs] (the first pass over the buffers does not block)
+    for (int item = cl; item < p.batch; item += ncl) {
+      for (int t = 0; t < T; ++t) {
+        float* bv = bvec + bs * p.sp.rows_max;
+        const size_t bt = static_cast<size_t>(item) * T + t;
+        const float ul = (has_bu && lane < m) ? __ldg(p.u + bt * m + lane) : 0.f;
+        const float4* gB = has_bu ? reinterpret_cast<const float4*>(p.B + (bt * n + r0) * m) : nullptr;
+        const float4* gC = p.c ? reinterpret_cast<const float4*>(p.c + bt * n + r0) : nullptr;
+        constexpr int kVB = kStageVecs / 32, kVC = 2;
+        float4 vb[kVB], vc[kVC];
+        if (staged) {
+#pragma unroll
+          for (int j = 0; j < kVB; ++j) vb[j] = (lane + 32 * j < nvB) ? __ldg(gB + lane + 32 * j) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
-        bv[i] = acc;
-      }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&bfull[t & 1]);
-    };
-    form_b(0);
-    for (int t = 0; t <= T; ++t) {
-      if (t >= 1) {
-        mbar_wait_cluster(&xfull[t & 1], (((t + 1) >> 1) - 1) & 1);
-        const float* xt = xbuf + (t & 1) * n;
-        float* dst = p.x_out + (static_cast<size_t>(item) * T + (t - 1)) * n;
-        for (int i = r0 + lane; i < r1; i += 32) dst[i] = xt[i];
-      }
-      if (t < T) {
-        if (lane == 0) mbar_arrive_expect_tx(&xfull[(t + 1) & 1], static_cast<uint32_t>(n) * 4u);
-        if (t + 1 < T) form_b(t + 1);
+#pragma unroll
+        for (int j = 0; j < kVC; ++j) vc[j] = (lane + 32 * j < nvC) ? __ldg(gC + lane + 32 * j) : make_float4(0.f, 0.f, 0.f, 0.f);
+        mbar_wait(&bempty[bs], bph);
+        float4* bv4 = reinterpret_cast<float4*>(bv);
+#pragma unroll
+        for (int j = 0; j < kVC; ++j)
+          if (lane + 32 * j < (rows >> 2)) bv4[lane + 32 * j] = vc[j];
+        for (int v = lane + 32 * kVC; v < (rows >> 2); v += 32) bv4[v] = gC ? __ldg(gC + v) : make_float4(0.f, 0.f, 0.f, 0.f);
+        if (has_bu) {
+          if (staged) {
+#pragma unroll
+            for (int j = 0; j < kVB; ++j)
+              if (lane + 32 * j < nvB) stB[lane + 32 * j] = vb[j];
+          }
+          __syncwarp();
+          const float* sB = reinterpret_cast<const float*>(stB);
+          for (int i = lane; i < rows; i += 32) {
+            float acc = bv[i];
+            if (m <= 32) {
+              for (int l = 0; l < m; ++l) {
+                const float bl = staged ? sB[i * m + l] : __ldg(p.B + (bt * n + r0 + i) * m + l);
+                acc = fmaf(bl, __shfl_sync(__activemask(), ul, l), acc);
+              }
+            } else {
+              for (int l = 0; l < m; ++l)
+                acc = fmaf(staged ? sB[i * m + l] : __ldg(p.B + (bt * n + r0 + i) * m + l), __ldg(p.u + bt * m + l), acc);
+            }
+            bv[i] = acc;
+          }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bfull[bs]);
+        if (++bs == kBStages) { bs = 0; bph ^= 1; }
       }
     }
   } else {
     // ------------------------------------------------------------------ consumers: shared-memory GEMV
+    // Two groups take alternate chunks: a pass is a chain of latencies (shared loads, 6 shuffles, remote stores:
+    // ~1500 cycles measured with clock traces) in which shared memory is busy for a quarter of the time, so
+    // one group's loads run under the other group's reduction.
+    const int grpid = warp / kConsWarps, gw = warp % kConsWarps;   // consumer group, warp within it
     const int n4 = n >> 2;
     const int sl = WIDE ? (n4 + kConsWarps - 1) / kConsWarps : n4;   // quads in this warp's column slice
-    const int q0 = (WIDE ? warp * sl : 0) + lane;
-    const int q_end = WIDE ? min(n4, (warp + 1) * sl) : n4;
+    const int q0 = (WIDE ? gw * sl : 0) + lane;
+    const int q_end = WIDE ? min(n4, (gw + 1) * sl) : n4;
     const int ql = (sl + 31) / 32;
     const int rpw = p.sp.rpw;
     const int grp = lane >> 3, sub = lane & 7;   // after reduce4_rows lane group `grp` holds row `grp` of the pass
     int st = 0;
     uint32_t fph = 0, cidx = 0;
+    int bs = 0;
+    uint32_t bph = 0;   // parity of bfull[bs]
+    uint32_t xph = 0;   // bit s: parity of the next phase of xfull[s] (x_0 of an item never uses its slot)
+    uint32_t h = 0;
+    for (int item = cl; item < p.batch; item += ncl, h += T)
     for (int t = 0; t < T; ++t) {
-      if (t >= 1 && !(LTV_ROLL_DBG & 2)) mbar_wait_cluster(&xfull[t & 1], (((t + 1) >> 1) - 1) & 1);
-      const float4* x4 = reinterpret_cast<const float4*>(xbuf + (t & 1) * n);
+      const uint32_t ht = h + t;
+      const bool exch = t + 1 < T;   // x_T only goes to global memory
+      if (warp == 0) { LTV_RT(1, ht, 0) }
       float4 xq[QLMAX];
+      if (t == 0) {
+        const float4* x4 = reinterpret_cast<const float4*>(p.x0 + static_cast<size_t>(item) * n);
 #pragma unroll
-      for (int j = 0; j < QLMAX; ++j) {
-        const int q = q0 + 32 * j;
-        xq[j] = (j < ql && q < q_end) ? x4[q] : make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int j = 0; j < QLMAX; ++j) {
+          const int q = q0 + 32 * j;
+          xq[j] = (j < ql && q < q_end) ? __ldg(x4 + q) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+      } else {
+        mbar_wait_cluster(&xfull[ht % 3], (xph >> (ht % 3)) & 1u);
+        xph ^= 1u << (ht % 3);
+        const float4* x4 = reinterpret_cast<const float4*>(xbuf + (ht % 3) * n);
+#pragma unroll
+        for (int j = 0; j < QLMAX; ++j) {
+          const int q = q0 + 32 * j;
+          xq[j] = (j < ql && q < q_end) ? x4[q] : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
       }
-      mbar_wait(&bfull[t & 1], (t >> 1) & 1);
-      float* xn = xbuf + ((t + 1) & 1) * n;
-      const float* bv = bvec + (t & 1) * p.sp.rows_max;
-      uint64_t* xbar = &xfull[(t + 1) & 1];
+      // every warp of every CTA has finished step t-1, so nobody reads xbuf[(ht+1) % 3] (= x_{t-2}) any more
+      if (exch && threadIdx.x == 0) mbar_arrive_expect_tx(&xfull[(ht + 1) % 3], static_cast<uint32_t>(n) * 4u);
+      if (warp == 0) { LTV_RT(1, ht, 1) }
+      mbar_wait(&bfull[bs], bph);
+      if (warp == 0) { LTV_RT(1, ht, 2) }
+      float* xn = xbuf + ((ht + 1) % 3) * n;
+      const float* bv = bvec + bs * p.sp.rows_max;
+      uint64_t* xbar = &xfull[(ht + 1) % 3];
+      float* xg = p.x_out + (static_cast<size_t>(item) * T + t) * n + r0;   // x_{t+1}, this CTA's rows
       for (int k = 0; k < nchunks; ++k, ++cidx) {
+        if (static_cast<int>(cidx % kGroups) == grpid) {
+        if (warp == 0) { LTV_RT(2, cidx, 0) }
         mbar_wait(&full[st], fph);
+        if (warp == 0) { LTV_RT(2, cidx, 1) }
         const float* tile = reinterpret_cast<const float*>(reinterpret_cast<uint8_t*>(ring) +
                                                             static_cast<size_t>(st) * p.sp.stage_bytes);
         const int rk = min(rc, rows - k * rc);
         if (!WIDE) {
-          // warp w: rows [w rpw, (w+1) rpw) of the chunk, four per pass
+          // warp gw: rows [gw rpw, (gw+1) rpw) of the chunk, four per pass
           for (int b0 = 0; b0 < rpw; b0 += 4) {
-            const int base = warp * rpw + b0;
+            const int base = gw * rpw + b0;
             if (base >= rk) break;
-            int rowi[4];
             const int nval = min(min(4, rpw - b0), rk - base);
-#pragma unroll
-            for (int r = 0; r < 4; ++r) rowi[r] = base + (r < nval ? r : 0);
             float acc[4] = {0.f, 0.f, 0.f, 0.f};
-            if (!(LTV_ROLL_DBG & 1)) rows4_dot<QLMAX>(tile, n, rowi, q0, q_end, ql, xq, acc);
-            const float v = (LTV_ROLL_DBG & 4) ? acc[0] : reduce4_rows(acc, lane);
+            rows_dot_n<QLMAX>(nval, tile, n, base, q0, q_end, ql, xq, acc);
+            if (warp == 0 && b0 == 0) { LTV_RT(3, cidx, 0) }
+            const float v = reduce4_rows(acc, lane);
+            if (warp == 0 && b0 == 0) { LTV_RT(3, cidx, 1) }
             if (grp < nval) {
               const int li = k * rc + base + grp;
               const float y = v + bv[li];
-              for (int cta = sub; cta < C; cta += 8) st_async_remote_f32(xn + r0 + li, y, xbar, cta);
+              if (exch)
+                for (int cta = sub; cta < C; cta += 8) st_async_remote_f32(xn + r0 + li, y, xbar, cta);
+              if (sub == 0) xg[li] = y;
             }
+            if (warp == 0 && b0 == 0) { LTV_RT(3, cidx, 2) }
           }
         } else {
-          // warp w: its eighth of the columns of all (<= 4) rows of the chunk; partial sums meet in shared memory
-          int rowi[4];
-#pragma unroll
-          for (int r = 0; r < 4; ++r) rowi[r] = r < rk ? r : 0;
+          // warp gw: its eighth of the columns of all (<= 4) rows of the chunk; partial sums meet in shared memory
           float acc[4] = {0.f, 0.f, 0.f, 0.f};
-          rows4_dot<QLMAX>(tile, n, rowi, q0, q_end, ql, xq, acc);
+          rows_dot_n<QLMAX>(rk, tile, n, 0, q0, q_end, ql, xq, acc);
           const float v = reduce4_rows(acc, lane);
-          float* pb = part + (cidx & 1) * (kConsWarps * 4);
-          if (sub == 0) pb[warp * 4 + grp] = v;
-          named_bar_sync(1, kConsWarps * 32);
-          const int tid = threadIdx.x;   // consumers are threads 0 .. 255
+          float* pb = part + (grpid * 2 + ((cidx / kGroups) & 1)) * (kConsWarps * 4);
+          if (sub == 0) pb[gw * 4 + grp] = v;
+          named_bar_sync(1 + grpid, kConsWarps * 32);
+          const int tid = gw * 32 + lane;
           if (tid < rk * C) {
             const int row = tid / C, cta = tid - row * C;
             float y = bv[k * rc + row];
 #pragma unroll
             for (int w = 0; w < kConsWarps; ++w) y += pb[w * 4 + row];
-            st_async_remote_f32(xn + r0 + k * rc + row, y, xbar, cta);
+            if (exch) st_async_remote_f32(xn + r0 + k * rc + row, y, xbar, cta);
+            if (cta == 0) xg[k * rc + row] = y;
           }
         }
         __syncwarp();
+        if (warp == 0) { LTV_RT(2, cidx, 2) }
         if (lane == 0) mbar_arrive(&empty[st]);
+        }
         if (++st == stages) { st = 0; fph ^= 1; }
       }
+      __syncwarp();
+      if (warp == 0) { LTV_RT(1, ht, 3) }
+      if (lane == 0) mbar_arrive(&bempty[bs]);
+      if (++bs == kBStages) { bs = 0; bph ^= 1; }
     }
   }
   __syncthreads();
   cluster_sync_all();  // no CTA may exit while a peer can still write into its shared memory
 }
 
-RollSmemPlan plan_rollout(int n, int C) {
+RollSmemPlan plan_rollout(int n, int C, int occ) {
   RollSmemPlan sp{};
-  sp.rows_max = (n + C - 1) / C + 1;
+  sp.rows_max = 4 * (((n >> 2) + C - 1) / C) + 4;   // bands are multiples of 4 rows
   sp.wide = n > kModeAMaxN ? 1 : 0;
   const uint32_t row_bytes = static_cast<uint32_t>(n) * 4u;
-  const uint32_t vec_bytes = static_cast<uint32_t>(align_up(2 * row_bytes, 128) + align_up(2u * sp.rows_max * 4u, 128)) +
-                             256u /* part */;
-  const uint32_t budget = 227u * 1024u - vec_bytes - 256u;
-  const uint32_t target = 32u * 1024u;
+  const uint32_t vec_bytes = static_cast<uint32_t>(align_up(3 * row_bytes, 128) + align_up(kBStages * sp.rows_max * 4u, 128)) +
+                             512u /* part */ + kStageVecs * 16u;
+  // occ CTAs share the 228 KB of an SM (1 KB of each is reserved by the system)
+  const uint32_t cta_bytes = occ > 1 ? (228u * 1024u) / occ - 1024u : 227u * 1024u;
+  if (cta_bytes < vec_bytes + 512u) return sp;   // stages = 0: caller falls back
+  const uint32_t budget = cta_bytes - vec_bytes - 256u;
+  const uint32_t target = budget / 6u < 32u * 1024u ? budget / 6u : 32u * 1024u;
   int rc;
   if (sp.wide) {
     rc = static_cast<int>(target / row_bytes);
@@ -286,7 +393,7 @@ RollSmemPlan plan_rollout(int n, int C) {
     rc = static_cast<int>((target + row_bytes * 4) / (row_bytes * 8)) * 8;
     if (rc < 8) rc = 8;
     if (rc > 64) rc = 64;
-    const int need = (sp.rows_max - 1 + 7) / 8 * 8;
+    const int need = (sp.rows_max - 4 + 7) / 8 * 8;
     if (rc > need) rc = need;
     sp.rpw = rc / 8;
   }
@@ -296,20 +403,28 @@ RollSmemPlan plan_rollout(int n, int C) {
   if (st > kMaxStages) st = kMaxStages;
   sp.stages = st;
   sp.off_x = sp.stage_bytes * st;
-  sp.off_b = sp.off_x + static_cast<uint32_t>(align_up(2 * row_bytes, 128));
-  sp.off_part = sp.off_b + static_cast<uint32_t>(align_up(2u * sp.rows_max * 4u, 128));
-  sp.off_bar = sp.off_part + 256u;
-  sp.total = sp.off_bar + (2 * kMaxStages + 4) * 8;
+  sp.off_b = sp.off_x + static_cast<uint32_t>(align_up(3 * row_bytes, 128));
+  sp.off_part = sp.off_b + static_cast<uint32_t>(align_up(kBStages * sp.rows_max * 4u, 128));
+  sp.off_stage = sp.off_part + 512u;
+  sp.off_bar = sp.off_stage + kStageVecs * 16u;
+  sp.total = sp.off_bar + (2 * kMaxStages + 3 + 2 * kBStages) * 8;
   return sp;
 }
 
 }  // namespace
 
-cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches) {
+// `cluster` CTAs per item, `occ` CTAs per SM the shared-memory plan leaves room for; the grid is as many
+// clusters as fit on the device at that occupancy (at most one per item), each looping over items
+cudaError_t launch_rollout(const RolloutArgs& a, int cluster, int occ, int num_sms, cudaStream_t stream,
+                           unsigned long long* launches) {
   RollParams p{};
   p.A = a.A; p.B = (a.m > 0) ? a.B : nullptr; p.c = a.c; p.x0 = a.x0; p.u = a.u; p.x_out = a.x_out;
   p.batch = a.batch; p.T = a.T; p.n = a.n; p.m = a.m;
-  p.sp = plan_rollout(a.n, cluster);
+  p.sp = plan_rollout(a.n, cluster, occ);
+#ifdef LTV_ROLL_TRACE
+  p.trace = g_roll_trace;
+  p.trace_cap = g_roll_trace_cap;
+#endif
   if (p.sp.stages < 2) return cudaErrorInvalidConfiguration;
 
   auto kern = p.sp.wide ? rollout_kernel<true> : rollout_kernel<false>;
@@ -320,7 +435,10 @@ cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t strea
     if (e != cudaSuccess) return e;
   }
   cudaLaunchConfig_t cfg{};
-  cfg.gridDim = dim3(static_cast<unsigned>(a.batch) * cluster);
+  int ncl = (num_sms * occ) / cluster;
+  if (ncl > a.batch) ncl = a.batch;
+  if (ncl < 1) ncl = 1;
+  cfg.gridDim = dim3(static_cast<unsigned>(ncl) * cluster);
   cfg.blockDim = dim3(kRollThreads);
   cfg.dynamicSmemBytes = p.sp.total;
   cfg.stream = stream;
