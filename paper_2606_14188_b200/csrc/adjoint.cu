@@ -17,16 +17,20 @@ namespace ltv {
 
 namespace {
 
-constexpr int kAdjConsThreads = 256;
-constexpr int kAdjThreads = kAdjConsThreads + 64;  // + producer warp + helper warp
+constexpr int kAdjConsThreads = 256;   // threads of one consumer group
+constexpr int kAdjGroups = 2;          // consumer groups; group g takes the ring boxes with index % kAdjGroups == g
+constexpr int kAdjAllCons = kAdjConsThreads * kAdjGroups;
+constexpr int kAdjThreads = kAdjAllCons + 64;  // + producer warp + helper warp
 constexpr int kAdjMaxStages = 8;
+constexpr int kStageVecs = 384;  // float4 of B_t the helper warp stages in shared memory per tile (6 KB)
+constexpr int kMaxL = 8;         // columns of grad_u one CTA reduces on the fast path
 
 struct AdjPlan {
   int bw;      // box width (columns), multiple of 4, <= 256
   int rcb;     // box rows
   int stages;
   int qt, rg;  // quad-threads per row, row groups
-  uint32_t stage_bytes, off_lam, off_red, off_bar, total;
+  uint32_t stage_bytes, off_lam, off_red, off_stage, off_bar, total;
 };
 
 struct AdjParams {
@@ -80,45 +84,93 @@ adjoint_kernel(const AdjParams p, const __grid_constant__ CUtensorMap tmapA) {
   }
   // lambuf[0] = lam_T = g_T
   const float* gT = p.g + (static_cast<size_t>(item) * T + (T - 1)) * n;
-  for (int j = threadIdx.x; j < n; j += kAdjThreads) lambuf[j] = gT[j];
+  for (int j = threadIdx.x; j < n; j += kAdjThreads) {
+    const float v = gT[j];
+    lambuf[j] = v;
+    if (j >= j0 && j < j1) p.lam_out[(static_cast<size_t>(item) * T + (T - 1)) * n + j] = v;   // lam_out[T-1] = lam_T
+  }
   __syncthreads();
   cluster_sync_all();
 
   // step k = 0 .. nstep-1 multiplies by A_t^T with t = T-1-k; its input costate lam_{t+1} is lambuf[k%3];
   // barrier lfull[k%3] is used for k = j, j+3, .. except k = 0 (local init): phase index k/3 - (k%3==0)
-  if (warp == kAdjConsThreads / 32) {
+  if (warp == kAdjAllCons / 32) {
     // ------------------------------------------------------------------ producer
     if (lane == 0 && W > 0) {
       const uint64_t pol = l2_policy_evict_first();
-      uint32_t it = 0;
+      int st = 0;
+      uint32_t eph = 1;   // parity of empty[st] (the first pass over the ring does not block)
       for (int k = 0; k < nstep; ++k) {
         const int t = T - 1 - k;
         const int row_base = (item * T + t) * n;  // validated on the host to fit in int
         for (int sl = 0; sl < nslab; ++sl) {
-          for (int rb = 0; rb < nrb; ++rb, ++it) {
-            const int st = it % ap.stages;
-            const uint32_t use = it / ap.stages;
-            if (use > 0) mbar_wait(&empty[st], (use - 1) & 1);
+          for (int rb = 0; rb < nrb; ++rb) {
+            mbar_wait(&empty[st], eph);
             mbar_arrive_expect_tx(&full[st], static_cast<uint32_t>(ap.bw) * ap.rcb * 4u);
             tma_load_2d(smem + static_cast<size_t>(st) * ap.stage_bytes, &tmapA, j0 + sl * ap.bw,
                         row_base + rb * ap.rcb, &full[st], pol);
+            if (++st == ap.stages) { st = 0; eph ^= 1; }
           }
         }
       }
     }
-  } else if (warp == kAdjConsThreads / 32 + 1) {
-    // ------------------------------------------------------------------ helper: outputs + grad_u
-    // at step k (t = T-1-k): wait lam_{t+1}, arm the barrier of lam_t, write lam_{t+1} (own column band),
-    // grad_u[t][l] for l = rank, rank + C, ...
+  } else if (warp == kAdjAllCons / 32 + 1) {
+    // ------------------------------------------------------------------ helper: barrier arming + grad_u
+    // at step k (t = T-1-k): wait lam_{t+1}, arm the barrier of lam_t, grad_u[t][l] = sum_i B_t[i][l] lam_{t+1}[i]
+    // for the columns l = rank, rank + C, ...  B_t is contiguous: it is read with 128-bit loads, a tile of
+    // kStageVecs float4 at a time (all loads of a tile in flight together, the next tile's issued before this
+    // one is reduced), staged in shared memory and reduced lane-per-row.
+    float4* stB = reinterpret_cast<float4*>(smem + ap.off_stage);
+    const int ncol = (p.gu_out && rank < m) ? (m - rank + C - 1) / C : 0;   // columns of grad_u this CTA owns
+    const bool fast = ncol > 0 && ncol <= kMaxL && 4 * m <= kStageVecs * 4;
+    const int rows_tile = fast ? ((kStageVecs * 4) / m) & ~3 : 0;           // rows of B per tile (multiple of 4: 16-byte tiles)
+    const int ntile = fast ? (n + rows_tile - 1) / rows_tile : 0;
+    constexpr int kVB = kStageVecs / 32;
     for (int k = 0; k < T; ++k) {
       const int t = T - 1 - k;
+      const float* Bt = p.B + (static_cast<size_t>(item) * T + t) * n * m;
+      float4 vb[kVB];
+      auto issue = [&](int tile) {
+        const float4* src = reinterpret_cast<const float4*>(Bt + static_cast<size_t>(tile) * rows_tile * m);
+        const int nv = (min(rows_tile, n - tile * rows_tile) * m) >> 2;   // n % 4 == 0: whole float4
+#pragma unroll
+        for (int j = 0; j < kVB; ++j) vb[j] = (lane + 32 * j < nv) ? __ldg(src + lane + 32 * j) : make_float4(0.f, 0.f, 0.f, 0.f);
+      };
+      if (fast) issue(0);
       if (k >= 1) mbar_wait_cluster(&lfull[k % 3], lam_parity(k));
       if (k + 1 < T && lane == 0) mbar_arrive_expect_tx(&lfull[(k + 1) % 3], static_cast<uint32_t>(n) * 4u);
       const float* lam = lambuf + (k % 3) * n;
-      float* dst = p.lam_out + (static_cast<size_t>(item) * T + t) * n;  // lam_out[t] = lam_{t+1}
-      for (int j = j0 + lane; j < j1; j += 32) dst[j] = lam[j];
-      if (p.gu_out) {
-        const float* Bt = p.B + (static_cast<size_t>(item) * T + t) * n * m;
+      if (fast) {
+        float acc[kMaxL];
+#pragma unroll
+        for (int c = 0; c < kMaxL; ++c) acc[c] = 0.f;
+        for (int tile = 0; tile < ntile; ++tile) {
+          const int rt = min(rows_tile, n - tile * rows_tile);
+          const int nv = (rt * m) >> 2;
+          __syncwarp();   // the previous tile has been reduced
+#pragma unroll
+          for (int j = 0; j < kVB; ++j)
+            if (lane + 32 * j < nv) stB[lane + 32 * j] = vb[j];
+          __syncwarp();
+          if (tile + 1 < ntile) issue(tile + 1);
+          const float* sB = reinterpret_cast<const float*>(stB);
+          for (int i = lane; i < rt; i += 32) {
+            const float li = lam[tile * rows_tile + i];
+#pragma unroll
+            for (int c = 0; c < kMaxL; ++c)
+              if (c < ncol) acc[c] = fmaf(sB[i * m + rank + c * C], li, acc[c]);
+          }
+        }
+#pragma unroll
+        for (int c = 0; c < kMaxL; ++c) {
+          if (c < ncol) {
+            float a = acc[c];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+            if (lane == 0) p.gu_out[(static_cast<size_t>(item) * T + t) * m + rank + c * C] = a;
+          }
+        }
+      } else if (p.gu_out) {
         for (int l = rank; l < m; l += C) {
           float acc = 0.f;
           for (int i = lane; i < n; i += 32) acc = fmaf(__ldg(Bt + static_cast<size_t>(i) * m + l), lam[i], acc);
@@ -130,10 +182,16 @@ adjoint_kernel(const AdjParams p, const __grid_constant__ CUtensorMap tmapA) {
     }
   } else {
     // ------------------------------------------------------------------ consumers
-    const int tid = threadIdx.x;
+    // Two groups of 256 threads take alternate ring boxes (one group's shared loads run under the other
+    // group's barrier waits and loop overheads); a thread keeps one accumulator quad per slab over its group's
+    // boxes, and the row classes of BOTH groups are combined in fixed order at the end of the slab.
+    const int grp = threadIdx.x / kAdjConsThreads;
+    const int tid = threadIdx.x % kAdjConsThreads;
     const int q = tid % ap.qt, rgi = tid / ap.qt;
     const bool active = rgi < ap.rg;
     uint32_t it = 0;
+    int st = 0;
+    uint32_t fph = 0;
     for (int k = 0; k < nstep; ++k) {
       const int t = T - 1 - k;
       if (k >= 1) mbar_wait_cluster(&lfull[k % 3], lam_parity(k));
@@ -144,42 +202,45 @@ adjoint_kernel(const AdjParams p, const __grid_constant__ CUtensorMap tmapA) {
       for (int sl = 0; sl < nslab; ++sl) {
         float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
         for (int rb = 0; rb < nrb; ++rb, ++it) {
-          const int st = it % ap.stages;
-          mbar_wait(&full[st], (it / ap.stages) & 1);
-          const float* tile = reinterpret_cast<const float*>(smem + static_cast<size_t>(st) * ap.stage_bytes);
-          const int i0 = rb * ap.rcb;
-          const int rk = min(ap.rcb, n - i0);
-          if (active) {
-#pragma unroll 4
-            for (int i = rgi; i < rk; i += ap.rg) {
-              const float4 a = *reinterpret_cast<const float4*>(tile + static_cast<size_t>(i) * ap.bw + 4 * q);
-              const float l = lam[i0 + i];
-              acc.x = fmaf(a.x, l, acc.x);
-              acc.y = fmaf(a.y, l, acc.y);
-              acc.z = fmaf(a.z, l, acc.z);
-              acc.w = fmaf(a.w, l, acc.w);
+          if (static_cast<int>(it % kAdjGroups) == grp) {
+            mbar_wait(&full[st], fph);
+            const float* tile = reinterpret_cast<const float*>(smem + static_cast<size_t>(st) * ap.stage_bytes);
+            const int i0 = rb * ap.rcb;
+            const int rk = min(ap.rcb, n - i0);
+            if (active) {
+#pragma unroll 8
+              for (int i = rgi; i < rk; i += ap.rg) {
+                const float4 a = *reinterpret_cast<const float4*>(tile + static_cast<size_t>(i) * ap.bw + 4 * q);
+                const float l = lam[i0 + i];
+                acc.x = fmaf(a.x, l, acc.x);
+                acc.y = fmaf(a.y, l, acc.y);
+                acc.z = fmaf(a.z, l, acc.z);
+                acc.w = fmaf(a.w, l, acc.w);
+              }
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[st]);
           }
-          __syncwarp();
-          if (lane == 0) mbar_arrive(&empty[st]);
+          if (++st == ap.stages) { st = 0; fph ^= 1; }
         }
         // combine the row classes (fixed order => deterministic) and publish this slab of the costate
-        if (active) *reinterpret_cast<float4*>(red + static_cast<size_t>(rgi) * ap.bw + 4 * q) = acc;
-        named_bar_sync(1, kAdjConsThreads);
-        for (int jj = tid; jj < ap.bw; jj += kAdjConsThreads) {
+        if (active) *reinterpret_cast<float4*>(red + static_cast<size_t>(grp * ap.rg + rgi) * ap.bw + 4 * q) = acc;
+        named_bar_sync(1, kAdjAllCons);
+        for (int jj = threadIdx.x; jj < ap.bw; jj += kAdjAllCons) {
           const int col = j0 + sl * ap.bw + jj;
           if (col < j1) {
             float v = 0.f;
-            for (int r = 0; r < ap.rg; ++r) v += red[static_cast<size_t>(r) * ap.bw + jj];
+            for (int r = 0; r < kAdjGroups * ap.rg; ++r) v += red[static_cast<size_t>(r) * ap.bw + jj];
             if (t >= 1) {
               v += gt[col];
               for (int cta = 0; cta < C; ++cta) st_async_remote_f32(lnext + col, v, lbar, cta);
+              p.lam_out[(static_cast<size_t>(item) * T + (t - 1)) * n + col] = v;   // lam_out[t-1] = lam_t
             } else {
               p.gx0_out[static_cast<size_t>(item) * n + col] = v;
             }
           }
         }
-        named_bar_sync(1, kAdjConsThreads);
+        named_bar_sync(1, kAdjAllCons);
       }
     }
   }
@@ -203,14 +264,15 @@ AdjPlan plan_adjoint(int n, int C) {
   ap.rcb = rcb;
   ap.stage_bytes = static_cast<uint32_t>(align_up(static_cast<size_t>(ap.bw) * rcb * 4, 128));
   const uint32_t lam_bytes = static_cast<uint32_t>(align_up(3u * n * 4u, 128));
-  const uint32_t red_bytes = static_cast<uint32_t>(align_up(static_cast<size_t>(ap.rg) * ap.bw * 4, 128));
-  const uint32_t budget = 227u * 1024u - lam_bytes - red_bytes - 256u;
+  const uint32_t red_bytes = static_cast<uint32_t>(align_up(static_cast<size_t>(kAdjGroups) * ap.rg * ap.bw * 4, 128));
+  const uint32_t budget = 227u * 1024u - lam_bytes - red_bytes - kStageVecs * 16u - 256u;
   int st = static_cast<int>(budget / ap.stage_bytes);
   if (st > kAdjMaxStages) st = kAdjMaxStages;
   ap.stages = st;
   ap.off_lam = ap.stage_bytes * st;
   ap.off_red = ap.off_lam + lam_bytes;
-  ap.off_bar = ap.off_red + red_bytes;
+  ap.off_stage = ap.off_red + red_bytes;
+  ap.off_bar = ap.off_stage + kStageVecs * 16u;
   ap.total = ap.off_bar + (2 * kAdjMaxStages + 3) * 8;
   return ap;
 }
