@@ -42,7 +42,8 @@ namespace {
 constexpr int kConsWarps = 8;    // warps of one consumer group
 constexpr int kGroups = 2;       // consumer groups; group g takes the ring chunks with index % kGroups == g
 constexpr int kAllCons = kConsWarps * kGroups;
-constexpr int kRollThreads = (kAllCons + 2) * 32;  // + producer warp + affine warp
+constexpr int kAffWarps = 2;      // affine warps; warp a forms the terms of the steps with number % kAffWarps == a
+constexpr int kRollThreads = (kAllCons + 1 + kAffWarps) * 32;  // + producer warp + affine warps
 constexpr int kMaxStages = 8;
 constexpr int kBStages = 4;     // affine terms formed ahead of the consumers
 constexpr int kStageVecs = 384; // float4 of the B band the affine warp stages in shared memory (6 KB)
@@ -197,7 +198,7 @@ __global__ void __launch_bounds__(kRollThreads, 1) rollout_kernel(const RollPara
         }
       }
     }
-  } else if (warp == kAllCons + 1) {
+  } else if (warp > kAllCons) {
     // ------------------------------------------------------------------ affine warp: b_t = B_t u_t + c_t
     // The bands of B_t and c_t are contiguous: all of their 128-bit loads (and u_t) are issued before the first
     // use, so a step costs one memory latency however many rows the band has; B_t is staged in shared memory
@@ -207,10 +208,17 @@ __global__ void __launch_bounds__(kRollThreads, 1) rollout_kernel(const RollPara
     const bool has_bu = p.B && p.u && m > 0;
     const int nvB = has_bu ? (rows * m) >> 2 : 0, nvC = p.c ? rows >> 2 : 0;
     const bool staged = nvB <= kStageVecs;
+    const int aw = warp - kAllCons - 1;
+    stB += aw * kStageVecs;
     int bs = 0;
     uint32_t bph = 1;   // parity of bempty[bs] (the first pass over the buffers does not block)
+    uint32_t sn = 0;    // step number over all items of this cluster
     for (int item = cl; item < p.batch; item += ncl) {
-      for (int t = 0; t < T; ++t) {
+      for (int t = 0; t < T; ++t, ++sn) {
+        if (static_cast<int>(sn % kAffWarps) != aw) {
+          if (++bs == kBStages) { bs = 0; bph ^= 1; }
+          continue;
+        }
         float* bv = bvec + bs * p.sp.rows_max;
         const size_t bt = static_cast<size_t>(item) * T + t;
         const float ul = (has_bu && lane < m) ? __ldg(p.u + bt * m + lane) : 0.f;
@@ -376,7 +384,7 @@ RollSmemPlan plan_rollout(int n, int C, int occ) {
   sp.wide = n > kModeAMaxN ? 1 : 0;
   const uint32_t row_bytes = static_cast<uint32_t>(n) * 4u;
   const uint32_t vec_bytes = static_cast<uint32_t>(align_up(3 * row_bytes, 128) + align_up(kBStages * sp.rows_max * 4u, 128)) +
-                             512u /* part */ + kStageVecs * 16u;
+                             512u /* part */ + kAffWarps * kStageVecs * 16u;
   // occ CTAs share the 228 KB of an SM (1 KB of each is reserved by the system)
   const uint32_t cta_bytes = occ > 1 ? (228u * 1024u) / occ - 1024u : 227u * 1024u;
   if (cta_bytes < vec_bytes + 512u) return sp;   // stages = 0: caller falls back
@@ -406,7 +414,7 @@ RollSmemPlan plan_rollout(int n, int C, int occ) {
   sp.off_b = sp.off_x + static_cast<uint32_t>(align_up(3 * row_bytes, 128));
   sp.off_part = sp.off_b + static_cast<uint32_t>(align_up(kBStages * sp.rows_max * 4u, 128));
   sp.off_stage = sp.off_part + 512u;
-  sp.off_bar = sp.off_stage + kStageVecs * 16u;
+  sp.off_bar = sp.off_stage + kAffWarps * kStageVecs * 16u;
   sp.total = sp.off_bar + (2 * kMaxStages + 3 + 2 * kBStages) * 8;
   return sp;
 }
