@@ -25,6 +25,7 @@ if ROOT not in sys.path:
 
 METRIC = "LTV scan rollouts/s + SLS Phi blocks/s; % of B200 tensor/HBM roofline"
 UNIT = "Phi blocks/s (whole step: rollout + Phi/tube + adjoint)"
+UNIT_C5 = "rollout+adjoint pairs/s"
 NOMINAL_TF32_OVER_BF16 = 0.5          # dense tensor peaks, B200_PROFILING.md: tf32 1.1 vs bf16 2.25 PFLOP/s
 FALLBACK_BF16_TFLOPS = 1590.0         # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 FALLBACK_BF16_SUSTAINED = 1400.0
@@ -36,12 +37,26 @@ def parse():
     ap.add_argument("--steps", type=int, default=40)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (0..4)")
+    ap.add_argument("--batch", type=int, default=0, help="items per GPU (0 = the config's own; config 4 sweeps 64/256/1024)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-items", type=int, default=0, help="items in the CPU-oracle sample (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
+
+
+def ncu_traffic(cfg_index, kernel):
+    """dram bytes per step of `kernel` from the committed ncu capture (profiles/r1_v4_traffic.csv), or None."""
+    path = os.path.join(ROOT, "profiles", "r1_v4_traffic.csv")
+    try:
+        for ln in open(path).read().splitlines()[1:]:
+            c, k, b = ln.split(",")[:3]
+            if int(c) == cfg_index and k == kernel:
+                return float(b)
+    except Exception:
+        pass
+    return None
 
 
 def peaks():
@@ -173,7 +188,7 @@ def main():
     G.build()
     import paper_2606_14188_b200 as L
 
-    cfg, W = workload(args.config, rank, world)
+    cfg, W = workload(args.config, rank, world, batch_override=args.batch or None)
     batch, T, n, m = W.shape
     P = T * (T - 1) // 2
     phi_on = args.config != 4
@@ -237,8 +252,14 @@ def main():
         ms_kernel = prof["phi_combine_tc"][0] / args.steps                  # all level launches of one step
         ach = flops_issued / (ms_kernel * 1e-3) / 1e12
         peak = pk["bf16_sustained"] * NOMINAL_TF32_OVER_BF16
+        clk = sampler.result()["sm_mhz"] or 1965
+        ceiling = 148 * 4096 * clk * 1e6 / 1e12            # 4096 dense tf32 flop / clk / SM at the sampled SM clock
         roof = dict(bound="tensor", kernel="phi_combine_tc_kernel (3xTF32 tcgen05, all levels of one step)",
-                    achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak, traffic=None,
+                    achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak,
+                    traffic=ncu_traffic(args.config, "phi_combine_tc"),
+                    algorithmic="issued tf32 flop = 3 x 2 n^3 x (T-1)(T-2)/2 x batch per step (no padding, no split work)",
+                    frac_of_unit_ceiling=ach / ceiling,
+                    unit_ceiling=f"{ceiling:.0f} TFLOP/s = 148 SM x 4096 flop/clk x {clk} MHz (median SM clock sampled during the run)",
                     peak_source=f"{pk['source']} bf16 sustained x {NOMINAL_TF32_OVER_BF16} (nominal tf32/bf16)",
                     logical_fp32_tflops=ach / 3.0, kernel_ms_per_step=ms_kernel,
                     launches_per_step=prof["phi_combine_tc"][1] / args.steps)
@@ -247,7 +268,9 @@ def main():
         ms_kernel = prof["rollout"][0] / max(prof["rollout"][1], 1)
         ach = bytes_roll / (ms_kernel * 1e-3) / 1e9
         roof = dict(bound="hbm", kernel="rollout_kernel", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s",
-                    frac=ach / pk["hbm_gbs"], traffic=None, peak_source=pk["source"], kernel_ms_per_step=ms_kernel)
+                    frac=ach / pk["hbm_gbs"], traffic=ncu_traffic(args.config, "rollout"),
+                    algorithmic="bytes = batch x (T(n^2 + nm + n + m) + n + Tn) x 4 per launch",
+                    peak_source=pk["source"] + " copy bandwidth", kernel_ms_per_step=ms_kernel)
     share = {k: round(v[0] / args.steps, 4) for k, v in prof.items() if v[1]}
 
     # ---- secondary HBM rooflines (rollout / adjoint), reported beside the headline
@@ -265,16 +288,19 @@ def main():
         if phi_on:
             del phi, ws
         torch.cuda.empty_cache()
-        need = L.ltv_scan_workspace_bytes(L.LTV_OP_PIPELINE_HOST, batch, T, n, m)
+        need = L.ltv_scan_workspace_bytes(L.LTV_OP_PIPELINE_HOST if phi_on else L.LTV_OP_PIPELINE_HOST_NO_PHI, batch, T, n, m)
         wsh = torch.empty(need, dtype=torch.uint8, device=dev)
         h = {k: torch.from_numpy(getattr(W, k)).pin_memory() for k in ("A", "B", "c", "x0", "u", "w", "g")}
+        if not phi_on:
+            h.pop("w")
         outs = None
         h2d = sum(v.numel() * 4 for v in h.values())
         for i in range(1 + args.e2e_steps):
             if i == 1:
                 barrier()
                 t0 = time.perf_counter()
-            outs = L.ltv_scan_pipeline_host(h["A"], h["B"], h["c"], h["x0"], h["u"], h["w"], h["g"], wsh, outs=outs)
+            outs = L.ltv_scan_pipeline_host(h["A"], h["B"], h["c"], h["x0"], h["u"], h["w"] if phi_on else None, h["g"],
+                                            wsh, outs=outs)
         barrier()
         sec = (time.perf_counter() - t0) / args.e2e_steps
         if world > 1:
@@ -282,24 +308,29 @@ def main():
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
             sec = float(tt.item())
         d2h = sum(outs[k].numel() * 4 for k in ("x", "r", "lam", "grad_u", "grad_x0") if outs[k] is not None)
-        e2e = dict(value=units / sec, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
-                   ms_per_step=sec * 1e3, note="ltv_scan_pipeline_host, pinned host buffers; Phi stays in HBM")
+        e2e = dict(value=units / sec, unit=UNIT if phi_on else UNIT_C5, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
+                   ms_per_step=sec * 1e3, note="ltv_scan_pipeline_host, pinned host buffers, upload of chunk i+1 overlapped with the compute of chunk i" +
+                        ("; Phi stays in HBM" if phi_on else "; rollout + adjoint only"))
 
     # ---- CPU oracle beside it (rank 0, N = 1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        items = args.cpu_items or (2 if n <= 600 else 1)
+        items = min(batch, args.cpu_items or (2 if n <= 600 else 1))
         sec = cpu_oracle_step(W, items)
-        cpu = dict(value=items * (P if phi_on else 1) / sec, unit=UNIT, cores=blas_threads(), kind="oracle",
+        cpu = dict(value=items * (P if phi_on else 1) / sec, unit=UNIT if phi_on else UNIT_C5, cores=blas_threads(), kind="oracle",
                    sample=f"{items} of {batch} items of {cfg['name']}, whole path, fp64 numpy, {sec:.1f} s")
 
     if rank == 0:
-        line = dict(metric=METRIC, value=value, unit=UNIT if phi_on else "rollout+adjoint pairs/s", n_gpus=world,
+        a_gb = batch * T * n * n * 4 / 1e9
+        phi_gb = batch * P * n * n * 4 / 1e9 if phi_on else 0.0
+        line = dict(metric=METRIC, value=value, unit=UNIT if phi_on else UNIT_C5, n_gpus=world,
                     steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms_step, higher_is_better=True,
                     scaling="weak", vs_baseline=None, dtype="tf32x3/f32", data="synthetic",
                     config=dict(workload=f"{cfg['name']}: n={n} m={m} T={T} batch={batch} per GPU, "
                                          f"{P if phi_on else 0} Phi blocks/item (BASELINE.json configs[{args.config}])",
-                                l2="inputs (A 0.74 GB) and outputs (Phi 11.4 GB) larger than the 126 MB L2; no flush",
+                                l2=(f"inputs (A {a_gb:.2f} GB) and outputs (Phi {phi_gb:.1f} GB) larger than the 126 MB L2; "
+                                    "no flush" if a_gb > 0.3 else
+                                    f"working set (A {a_gb * 1e3:.2f} MB) fits L2: warm-cache, latency-bound case"),
                                 phi_layout="column-packed"),
                     clocks=sampler.result(), e2e=e2e, gpu_launches=int(launches), roofline=roof,
                     cpu_baseline=cpu, kernel_ms_per_step=share, vector_scans=extra,

@@ -59,7 +59,8 @@ typedef enum {
 } ltv_status;
 
 /* `op` argument of ltv_scan_workspace_bytes */
-enum { LTV_OP_ROLLOUT = 0, LTV_OP_SYSTEM_RESPONSE_TUBE = 1, LTV_OP_ADJOINT = 2, LTV_OP_PIPELINE_HOST = 3 };
+enum { LTV_OP_ROLLOUT = 0, LTV_OP_SYSTEM_RESPONSE_TUBE = 1, LTV_OP_ADJOINT = 2, LTV_OP_PIPELINE_HOST = 3,
+       LTV_OP_PIPELINE_HOST_NO_PHI = 4 /* ltv_scan_pipeline_host with w_host == NULL: rollout + adjoint only */ };
 
 /* `phi_layout` argument.  COLUMN_PACKED (the only layout of this version): the P = T(T-1)/2 blocks of one
  * item are stored column by column of the block-lower-triangular operator; block (t,s), 0 <= s < t <= T-1,
@@ -125,7 +126,12 @@ LTV_API int ltv_scan_adjoint(const float* A, const float* B, const float* g,
  * returning.  Phi (11 GB at the benchmark sizes) stays in the workspace on the device, where its consumer
  * (the tube / constraint tightening) lives, unless phi_host != NULL, in which case it is copied back too.
  * All *_host pointers are host memory; B, c, u may be NULL as in ltv_scan_rollout; grad_x0_host and
- * phi_host may be NULL.  *phi_device_out (if not NULL) receives the device address of Phi inside workspace. */
+ * phi_host may be NULL.  *phi_device_out (if not NULL) receives the device address of Phi inside workspace.
+ * w_host == NULL skips the system-response / tube stage (rollout + adjoint only, BASELINE.json configs[4]): r_host
+ * is then not written and may be NULL, and the workspace need is LTV_OP_PIPELINE_HOST_NO_PHI.
+ * The batch is processed in up to four chunks (multiples of 4 items): an internal non-blocking copy stream,
+ * created and destroyed inside the call, uploads chunk i+1 while chunk i is computed on `cuda_stream` (items
+ * are independent, so this changes no result); host buffers should be pinned for the copies to overlap. */
 LTV_API int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float* c_host,
                            const float* x0_host, const float* u_host, const float* w_host,
                            const float* g_host,

@@ -17,6 +17,7 @@ STATUS_NAMES = {
     4: "LTV_ERR_ALIGNMENT", 5: "LTV_ERR_WORKSPACE_TOO_SMALL", 6: "LTV_ERR_ARCH", 7: "LTV_ERR_CUDA",
 }
 LTV_OP_ROLLOUT, LTV_OP_SYSTEM_RESPONSE_TUBE, LTV_OP_ADJOINT, LTV_OP_PIPELINE_HOST = 0, 1, 2, 3
+LTV_OP_PIPELINE_HOST_NO_PHI = 4
 LTV_PHI_COLUMN_PACKED = 0
 
 EXPORTS = (
@@ -169,7 +170,8 @@ def ltv_scan_adjoint(A, B, g, want_grad_x0=True, lambda_out=None, grad_u_out=Non
 
 def ltv_scan_pipeline_host(A, B, c, x0, u, w, g, workspace, want_grad_x0=True, phi_host=None, outs=None):
     """Whole path from HOST (CPU, ideally pinned) fp32 tensors; returns dict of host outputs and the device
-    address of Phi inside `workspace` (a uint8 CUDA tensor of >= workspace_bytes(LTV_OP_PIPELINE_HOST))."""
+    address of Phi inside `workspace` (a uint8 CUDA tensor of >= workspace_bytes(LTV_OP_PIPELINE_HOST)).
+    w=None skips the Phi / tube stage (workspace need: LTV_OP_PIPELINE_HOST_NO_PHI)."""
     batch, T, n, _ = A.shape
     m = 0 if B is None else B.shape[-1]
     for name, t in (("A", A), ("B", B), ("c", c), ("x0", x0), ("u", u), ("w", w), ("g", g), ("phi_host", phi_host)):
@@ -178,7 +180,7 @@ def ltv_scan_pipeline_host(A, B, c, x0, u, w, g, workspace, want_grad_x0=True, p
     if outs is None:
         pin = torch.cuda.is_available()
         mk = lambda *s: torch.empty(s, dtype=torch.float32, pin_memory=pin)
-        outs = dict(x=mk(batch, T, n), r=mk(batch, T, n), lam=mk(batch, T, n),
+        outs = dict(x=mk(batch, T, n), r=mk(batch, T, n) if w is not None else None, lam=mk(batch, T, n),
                     grad_u=mk(batch, T, m) if (B is not None and m > 0) else None,
                     grad_x0=mk(batch, n) if want_grad_x0 else None)
     phi_dev = ctypes.c_void_p(0)

@@ -226,17 +226,25 @@ adjoint_kernel(const AdjParams p, const __grid_constant__ CUtensorMap tmapA) {
         // combine the row classes (fixed order => deterministic) and publish this slab of the costate
         if (active) *reinterpret_cast<float4*>(red + static_cast<size_t>(grp * ap.rg + rgi) * ap.bw + 4 * q) = acc;
         named_bar_sync(1, kAdjAllCons);
-        for (int jj = threadIdx.x; jj < ap.bw; jj += kAdjAllCons) {
-          const int col = j0 + sl * ap.bw + jj;
-          if (col < j1) {
-            float v = 0.f;
-            for (int r = 0; r < kAdjGroups * ap.rg; ++r) v += red[static_cast<size_t>(r) * ap.bw + jj];
+        // thread (column quad, destination CTA): one 16-byte remote store per pair instead of 4 x C 4-byte ones
+        const int nquad = ap.bw >> 2;
+        for (int idx = threadIdx.x; idx < nquad * C; idx += kAdjAllCons) {
+          const int jq = idx / C, cta = idx - jq * C;
+          const int col = j0 + sl * ap.bw + 4 * jq;
+          if (col < j1) {   // bands and boxes are whole quads
+            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int r = 0; r < kAdjGroups * ap.rg; ++r) {
+              const float4 pr = *reinterpret_cast<const float4*>(red + static_cast<size_t>(r) * ap.bw + 4 * jq);
+              v.x += pr.x; v.y += pr.y; v.z += pr.z; v.w += pr.w;
+            }
             if (t >= 1) {
-              v += gt[col];
-              for (int cta = 0; cta < C; ++cta) st_async_remote_f32(lnext + col, v, lbar, cta);
-              p.lam_out[(static_cast<size_t>(item) * T + (t - 1)) * n + col] = v;   // lam_out[t-1] = lam_t
-            } else {
-              p.gx0_out[static_cast<size_t>(item) * n + col] = v;
+              const float4 gq = __ldg(reinterpret_cast<const float4*>(gt + col));
+              v.x += gq.x; v.y += gq.y; v.z += gq.z; v.w += gq.w;
+              st_async_remote_f32x4(lnext + col, v, lbar, cta);
+              if (cta == 0)   // lam_out[t-1] = lam_t
+                *reinterpret_cast<float4*>(p.lam_out + (static_cast<size_t>(item) * T + (t - 1)) * n + col) = v;
+            } else if (cta == 0) {
+              *reinterpret_cast<float4*>(p.gx0_out + static_cast<size_t>(item) * n + col) = v;
             }
           }
         }
@@ -301,6 +309,13 @@ cudaError_t launch_adjoint(const AdjointArgs& a, int cluster, cudaStream_t strea
   p.A = a.A; p.B = a.B; p.g = a.g;
   p.lam_out = a.lambda_out; p.gu_out = (a.m > 0) ? a.grad_u_out : nullptr; p.gx0_out = a.grad_x0_out;
   p.batch = a.batch; p.T = a.T; p.n = a.n; p.m = a.m;
+  static int max_active[17];
+  static bool have = false;
+  if (!have) {
+    query_max_active_clusters(reinterpret_cast<const void*>(adjoint_kernel), kAdjThreads, 200 * 1024, max_active);
+    have = true;
+  }
+  if (cluster <= 0) cluster = pick_cluster_model(a.batch, a.n, max_active);
   p.ap = plan_adjoint(a.n, cluster);
   if (p.ap.stages < 2) return cudaErrorInvalidConfiguration;
 

@@ -22,26 +22,54 @@ int env_int(const char* name, int dflt) {
   return (v && *v) ? std::atoi(v) : dflt;
 }
 
-int pick_cluster(int batch, int n, int num_sms) {
+int pick_cluster_model(int batch, int n, const int* max_active) {
   const int forced = env_int("CLUSTER", 0);
-  if (forced == 1 || forced == 2 || forced == 4 || forced == 8 || forced == 16) return forced;
-  int c = 1;
-  while (c < 16 && static_cast<long long>(batch) * (2 * c) <= num_sms && n / (2 * c) >= 32) c *= 2;
-  return c;
+  if (forced >= 1 && forced <= 16 && max_active[forced] > 0) return forced;
+  const double sm_gbs = 70.0, dev_gbs = 6500.0;
+  int best = 1;
+  double best_t = 1e300;
+  for (int c = 1; c <= 16; ++c) {
+    if (max_active[c] <= 0) continue;
+    if (c > 1 && (n / c < 32 || (n >> 2) < c)) continue;   // keep at least ~32 rows / columns per CTA
+    double t = 0.0;
+    for (int rem = batch; rem > 0;) {
+      const int w = rem < max_active[c] ? rem : max_active[c];
+      const double rate = (w * c * sm_gbs < dev_gbs) ? w * c * sm_gbs : dev_gbs;
+      t += w / rate;
+      rem -= w;
+    }
+    t *= 1.0 + 0.01 * c;   // ties go to the smaller cluster (less exchange per step)
+    if (t < best_t) {
+      best_t = t;
+      best = c;
+    }
+  }
+  return best;
 }
 
-// The HBM stream needs (nearly) every SM pulling: one SM sustains ~48 GB/s (measured), so take the smallest
-// power-of-two cluster that puts CTAs on at least three quarters of the SMs.  `occ` (CTAs per SM) stays 1: the
-// 18-warp CTA needs most of an SM's registers and shared memory.
-void pick_rollout_shape(int batch, int n, int num_sms, int* cluster, int* occ) {
-  int c = 1;
-  while (c < 16 && static_cast<long long>(batch) * c * 4 < 3ll * num_sms && n / (2 * c) >= 32) c *= 2;
-  int o = 1;
-  const int fc = env_int("CLUSTER", 0), fo = env_int("OCC", 0);
-  if (fc == 1 || fc == 2 || fc == 4 || fc == 8 || fc == 16) c = fc;
-  if (fo == 1 || fo == 2) o = fo;
-  *cluster = c;
-  *occ = o;
+void query_max_active_clusters(const void* kernel, int threads, size_t smem, int* max_active) {
+  cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+  cudaFuncSetAttribute(kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+  max_active[0] = 0;
+  for (int c = 1; c <= 16; ++c) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3(c * 64);
+    cfg.blockDim = dim3(threads);
+    cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = c;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    int nact = 0;
+    if (cudaOccupancyMaxActiveClusters(&nact, kernel, &cfg) != cudaSuccess) {
+      cudaGetLastError();
+      nact = 0;
+    }
+    max_active[c] = nact;
+  }
 }
 
 // ---- optional kernel timing --------------------------------------------------------------------------
@@ -128,7 +156,9 @@ size_t ltv_scan_workspace_bytes(int op, int batch, int T, int n, int m) {
       return 0;
     case LTV_OP_SYSTEM_RESPONSE_TUBE:
       return phi_workspace_bytes(batch, T, n);
-    case LTV_OP_PIPELINE_HOST: {
+    case LTV_OP_PIPELINE_HOST:
+    case LTV_OP_PIPELINE_HOST_NO_PHI: {
+      const bool with_phi = op == LTV_OP_PIPELINE_HOST;
       const size_t b = batch, t = T, nn = n, mm = m;
       const size_t P = t * (t - 1) / 2;
       size_t tot = 0;
@@ -141,12 +171,12 @@ size_t ltv_scan_workspace_bytes(int op, int batch, int T, int n, int m) {
       add(b * t * nn);       // w
       add(b * t * nn);       // g
       add(b * t * nn);       // x
-      add(b * P * nn * nn);  // phi
+      add(with_phi ? b * P * nn * nn : 0);  // phi
       add(b * t * nn);       // r
       add(b * t * nn);       // lambda
       add(b * t * mm);       // grad_u
       add(b * nn);           // grad_x0
-      tot += phi_workspace_bytes(batch, T, n);
+      if (with_phi) tot += phi_workspace_bytes(batch, T, n);
       return tot;
     }
     default:
@@ -168,16 +198,10 @@ int ltv_scan_rollout(const float* A, const float* B, const float* c, const float
   RolloutArgs a{A, B, c, x0, u, x_out, batch, T, n, m};
   unsigned long long l = 0;
   cudaError_t e = cudaErrorUnknown;
-  int cl = 1, occ = 1;
-  pick_rollout_shape(batch, n, sms, &cl, &occ);
-  for (; cl >= 1; cl /= 2) {  // a 16-CTA cluster may not be placeable
-    e = launch_rollout(a, cl, occ, sms, static_cast<cudaStream_t>(cuda_stream), &l);
-    if (e != cudaSuccess && occ > 1) {
-      cudaGetLastError();
-      e = launch_rollout(a, cl, 1, sms, static_cast<cudaStream_t>(cuda_stream), &l);
-    }
-    if (e == cudaSuccess) break;
+  e = launch_rollout(a, 0, static_cast<cudaStream_t>(cuda_stream), &l);
+  if (e != cudaSuccess) {   // the modelled cluster could not be placed: one CTA per item always can
     cudaGetLastError();
+    e = launch_rollout(a, 1, static_cast<cudaStream_t>(cuda_stream), &l);
   }
   g_launches += l;
   return e == cudaSuccess ? LTV_OK : fail_cuda(e);
@@ -200,10 +224,10 @@ int ltv_scan_adjoint(const float* A, const float* B, const float* g, float* lamb
   AdjointArgs a{A, B, g, lambda_out, grad_u_out, grad_x0_out, batch, T, n, m};
   unsigned long long l = 0;
   cudaError_t e = cudaErrorUnknown;
-  for (int cl = pick_cluster(batch, n, sms); cl >= 1; cl /= 2) {
-    e = launch_adjoint(a, cl, static_cast<cudaStream_t>(cuda_stream), &l);
-    if (e == cudaSuccess) break;
+  e = launch_adjoint(a, 0, static_cast<cudaStream_t>(cuda_stream), &l);
+  if (e != cudaSuccess) {
     cudaGetLastError();
+    e = launch_adjoint(a, 1, static_cast<cudaStream_t>(cuda_stream), &l);
   }
   g_launches += l;
   return e == cudaSuccess ? LTV_OK : fail_cuda(e);
@@ -237,13 +261,14 @@ int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float
                            float* phi_host, float* r_host, float* lambda_host, float* grad_u_host,
                            float* grad_x0_host, int batch, int T, int n, int m, void* workspace,
                            size_t workspace_bytes, void* cuda_stream, float** phi_device_out) {
-  if (!A_host || !x0_host || !w_host || !g_host || !x_host || !r_host || !lambda_host || !workspace)
-    return LTV_ERR_NULL_PTR;
+  const bool with_phi = w_host != nullptr;
+  if (!A_host || !x0_host || !g_host || !x_host || !lambda_host || !workspace) return LTV_ERR_NULL_PTR;
+  if (with_phi && !r_host) return LTV_ERR_NULL_PTR;
   if (grad_u_host && m > 0 && !B_host) return LTV_ERR_NULL_PTR;
   int st = check_dims(batch, T, n, m);
   if (st != LTV_OK) return st;
   if (misaligned(workspace)) return LTV_ERR_ALIGNMENT;
-  if (workspace_bytes < ltv_scan_workspace_bytes(LTV_OP_PIPELINE_HOST, batch, T, n, m))
+  if (workspace_bytes < ltv_scan_workspace_bytes(with_phi ? LTV_OP_PIPELINE_HOST : LTV_OP_PIPELINE_HOST_NO_PHI, batch, T, n, m))
     return LTV_ERR_WORKSPACE_TOO_SMALL;
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
   const size_t b = batch, t = T, nn = n, mm = m, P = t * (t - 1) / 2;
@@ -261,14 +286,14 @@ int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float
   float* dw = carve(b * t * nn);
   float* dg = carve(b * t * nn);
   float* dx = carve(b * t * nn);
-  float* dphi = carve(b * P * nn * nn);
+  float* dphi = carve(with_phi ? b * P * nn * nn : 0);
   float* dr = carve(b * t * nn);
   float* dl = carve(b * t * nn);
   float* dgu = carve(b * t * mm);
   float* dgx = carve(b * nn);
   void* phi_ws = cur;
-  const size_t phi_ws_bytes = phi_workspace_bytes(batch, T, n);
-  if (phi_device_out) *phi_device_out = dphi;
+  const size_t phi_ws_bytes = with_phi ? phi_workspace_bytes(batch, T, n) : 0;
+  if (phi_device_out) *phi_device_out = with_phi ? dphi : nullptr;
 
   cudaError_t e;
 #define LTV_H2D(dst, src, floats)                                                                   \
@@ -281,33 +306,85 @@ int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float
     e = cudaMemcpyAsync((dst), (src), (floats) * sizeof(float), cudaMemcpyDeviceToHost, s);         \
     if (e != cudaSuccess) return fail_cuda(e);                                                      \
   }
-  LTV_H2D(dA, A_host, b * t * nn * nn);
-  LTV_H2D(dB, B_host, b * t * nn * mm);
-  LTV_H2D(dc, c_host, b * t * nn);
-  LTV_H2D(dx0, x0_host, b * nn);
-  LTV_H2D(du, u_host, b * t * mm);
-  LTV_H2D(dw, w_host, b * t * nn);
-  LTV_H2D(dg, g_host, b * t * nn);
-  st = ltv_scan_rollout(dA, B_host ? dB : nullptr, c_host ? dc : nullptr, dx0, u_host ? du : nullptr, dx, batch, T, n,
-                        m, nullptr, 0, cuda_stream);
-  if (st != LTV_OK) return st;
-  st = ltv_scan_system_response_tube(dA, dw, dphi, dr, batch, T, n, LTV_PHI_COLUMN_PACKED, 0, phi_ws, phi_ws_bytes,
-                                     cuda_stream);
-  if (st != LTV_OK) return st;
-  st = ltv_scan_adjoint(dA, B_host ? dB : nullptr, dg, dl, (grad_u_host && B_host) ? dgu : nullptr,
-                        grad_x0_host ? dgx : nullptr, batch, T, n, m, nullptr, 0, cuda_stream);
-  if (st != LTV_OK) return st;
+  // Chunks of the batch are pipelined: an internal copy stream uploads chunk i+1 while chunk i is computed on
+  // the caller's stream (items are independent; the upload, 97 % of it A, is the longer leg at PCIe rates).
+  // Chunks are multiples of 4 items so that every slice stays 16-byte aligned.
+  int cb = batch;
+  if (batch >= 8 && env_int("E2E_CHUNKS", 4) > 1) {
+    const int want = env_int("E2E_CHUNKS", 4);
+    cb = ((batch + want - 1) / want + 3) & ~3;
+  }
+  const int nchunk = (batch + cb - 1) / cb;
+  cudaStream_t cs = nullptr;
+  cudaEvent_t ev_start = nullptr, ev_up[16] = {};
+  if (nchunk > 16) return LTV_ERR_BAD_DIM;
+  auto cleanup = [&]() {
+    for (int i = 0; i < 16; ++i)
+      if (ev_up[i]) cudaEventDestroy(ev_up[i]);
+    if (ev_start) cudaEventDestroy(ev_start);
+    if (cs) cudaStreamDestroy(cs);
+  };
+#define LTV_TRY(call)                     \
+  if ((e = (call)) != cudaSuccess) {      \
+    cleanup();                            \
+    return fail_cuda(e);                  \
+  }
+  LTV_TRY(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+  LTV_TRY(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+  LTV_TRY(cudaEventRecord(ev_start, s));        // earlier work on the caller's stream may still use the workspace
+  LTV_TRY(cudaStreamWaitEvent(cs, ev_start, 0));
+  auto up = [&](float* dst, const float* src, size_t per_item, int c0, int cn) -> cudaError_t {
+    if (!src || per_item == 0) return cudaSuccess;
+    return cudaMemcpyAsync(dst + per_item * c0, src + per_item * c0, per_item * cn * sizeof(float),
+                           cudaMemcpyHostToDevice, cs);
+  };
+  for (int ci = 0; ci < nchunk; ++ci) {
+    const int c0 = ci * cb, cn = (c0 + cb <= batch) ? cb : batch - c0;
+    LTV_TRY(up(dA, A_host, t * nn * nn, c0, cn));
+    LTV_TRY(up(dB, B_host, t * nn * mm, c0, cn));
+    LTV_TRY(up(dc, c_host, t * nn, c0, cn));
+    LTV_TRY(up(dx0, x0_host, nn, c0, cn));
+    LTV_TRY(up(du, u_host, t * mm, c0, cn));
+    LTV_TRY(up(dw, w_host, t * nn, c0, cn));
+    LTV_TRY(up(dg, g_host, t * nn, c0, cn));
+    LTV_TRY(cudaEventCreateWithFlags(&ev_up[ci], cudaEventDisableTiming));
+    LTV_TRY(cudaEventRecord(ev_up[ci], cs));
+  }
+  for (int ci = 0; ci < nchunk; ++ci) {
+    const size_t c0 = static_cast<size_t>(ci) * cb;
+    const int cn = (c0 + cb <= b) ? cb : static_cast<int>(b - c0);
+    LTV_TRY(cudaStreamWaitEvent(s, ev_up[ci], 0));
+    st = ltv_scan_rollout(dA + c0 * t * nn * nn, B_host ? dB + c0 * t * nn * mm : nullptr,
+                          c_host ? dc + c0 * t * nn : nullptr, dx0 + c0 * nn, u_host ? du + c0 * t * mm : nullptr,
+                          dx + c0 * t * nn, cn, T, n, m, nullptr, 0, cuda_stream);
+    if (st == LTV_OK && with_phi)
+      st = ltv_scan_system_response_tube(dA + c0 * t * nn * nn, dw + c0 * t * nn, dphi + c0 * P * nn * nn,
+                                         dr + c0 * t * nn, cn, T, n, LTV_PHI_COLUMN_PACKED, 0, phi_ws, phi_ws_bytes,
+                                         cuda_stream);
+    if (st == LTV_OK)
+      st = ltv_scan_adjoint(dA + c0 * t * nn * nn, B_host ? dB + c0 * t * nn * mm : nullptr, dg + c0 * t * nn,
+                            dl + c0 * t * nn, (grad_u_host && B_host) ? dgu + c0 * t * mm : nullptr,
+                            grad_x0_host ? dgx + c0 * nn : nullptr, cn, T, n, m, nullptr, 0, cuda_stream);
+    if (st != LTV_OK) {
+      cudaStreamSynchronize(cs);
+      cleanup();
+      return st;
+    }
+  }
   LTV_D2H(x_host, dx, b * t * nn);
-  LTV_D2H(r_host, dr, b * t * nn);
+  if (with_phi) LTV_D2H(r_host, dr, b * t * nn);
   LTV_D2H(lambda_host, dl, b * t * nn);
   if (B_host) LTV_D2H(grad_u_host, dgu, b * t * mm);
   LTV_D2H(grad_x0_host, dgx, b * nn);
-  LTV_D2H(phi_host, dphi, b * P * nn * nn);
-#undef LTV_H2D
-#undef LTV_D2H
+  if (with_phi) LTV_D2H(phi_host, dphi, b * P * nn * nn);
   e = cudaStreamSynchronize(s);
+  cudaStreamSynchronize(cs);
+  cleanup();
   if (e != cudaSuccess) return fail_cuda(e);
   return LTV_OK;
+#undef LTV_TRY
+#undef LTV_H2D
+#undef LTV_D2H
 }
 
 const char* ltv_status_string(int status) {

@@ -14,8 +14,8 @@ struct RolloutArgs {
   float* x_out;
   int batch, T, n, m;
 };
-cudaError_t launch_rollout(const RolloutArgs& a, int cluster, int occ, int num_sms, cudaStream_t stream,
-                           unsigned long long* launches);
+// cluster = 0: chosen by pick_cluster_model
+cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches);
 
 struct AdjointArgs {
   const float *A, *B, *g;
@@ -36,10 +36,12 @@ bool phi_uses_tensor_cores(int n);
 size_t phi_workspace_bytes(int batch, int T, int n);
 cudaError_t launch_phi_tube(const PhiArgs& a, cudaStream_t stream, unsigned long long* launches);
 
-// cluster-size heuristic of the adjoint (power of two, 1..16)
-int pick_cluster(int batch, int n, int num_sms);
-// rollout: CTAs per item (power of two, 1..16) and CTAs per SM (1 or 2) so that every SM streams
-void pick_rollout_shape(int batch, int n, int num_sms, int* cluster, int* occ);
+// Cluster size (CTAs per item, 1..16, any integer) for the two vector kernels.  max_active[C] = clusters of C CTAs
+// that can be resident at once (cudaOccupancyMaxActiveClusters; 0 = not launchable).  Minimises a simple
+// time model over the waves of clusters: an SM streams ~70 GB/s, the device ~6.5 TB/s (both measured).
+int pick_cluster_model(int batch, int n, const int* max_active);
+// fills max_active[1..16] for `kernel` (any __global__ function pointer) at the given block size / dynamic smem
+void query_max_active_clusters(const void* kernel, int threads, size_t smem, int* max_active);
 // environment override for experiments: LTV_SCAN_<name>=<int>; returns `dflt` if unset
 int env_int(const char* name, int dflt);
 

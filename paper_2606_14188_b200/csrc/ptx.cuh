@@ -117,6 +117,19 @@ __device__ __forceinline__ void st_async_remote_f32(float* dst_local_addr, float
       : "memory");
 }
 
+// 16-byte variant (dst 16-byte aligned): one packet on the SM-to-SM network instead of four
+__device__ __forceinline__ void st_async_remote_f32x4(float* dst_local_addr, float4 v, uint64_t* bar_local_addr,
+                                                      uint32_t cta_rank) {
+  asm volatile(
+      "{\n\t.reg .b32 rd, rb;\n\t"
+      "mapa.shared::cluster.u32 rd, %0, %6;\n\t"
+      "mapa.shared::cluster.u32 rb, %5, %6;\n\t"
+      "st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.b32 [rd], {%1, %2, %3, %4}, [rb];\n\t}"
+      ::"r"(smem_u32(dst_local_addr)), "r"(__float_as_uint(v.x)), "r"(__float_as_uint(v.y)), "r"(__float_as_uint(v.z)),
+        "r"(__float_as_uint(v.w)), "r"(smem_u32(bar_local_addr)), "r"(cta_rank)
+      : "memory");
+}
+
 // ---------------------------------------------------------------------------------------- TMA
 __device__ __forceinline__ uint64_t l2_policy_evict_first() {
   uint64_t p;

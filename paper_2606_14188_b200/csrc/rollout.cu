@@ -246,18 +246,22 @@ __global__ void __launch_bounds__(kRollThreads, 1) rollout_kernel(const RollPara
           }
           __syncwarp();
           const float* sB = reinterpret_cast<const float*>(stB);
-          for (int i = lane; i < rows; i += 32) {
-            float acc = bv[i];
+          for (int i0 = 0; i0 < rows; i0 += 32) {   // warp-uniform trip count: the shuffles need every lane
+            const int i = i0 + lane;
+            const bool ok = i < rows;
+            float acc = ok ? bv[i] : 0.f;
             if (m <= 32) {
               for (int l = 0; l < m; ++l) {
-                const float bl = staged ? sB[i * m + l] : __ldg(p.B + (bt * n + r0 + i) * m + l);
-                acc = fmaf(bl, __shfl_sync(__activemask(), ul, l), acc);
+                const float bl = !ok ? 0.f : staged ? sB[i * m + l] : __ldg(p.B + (bt * n + r0 + i) * m + l);
+                acc = fmaf(bl, __shfl_sync(0xffffffffu, ul, l), acc);
               }
             } else {
-              for (int l = 0; l < m; ++l)
-                acc = fmaf(staged ? sB[i * m + l] : __ldg(p.B + (bt * n + r0 + i) * m + l), __ldg(p.u + bt * m + l), acc);
+              for (int l = 0; l < m; ++l) {
+                const float bl = !ok ? 0.f : staged ? sB[i * m + l] : __ldg(p.B + (bt * n + r0 + i) * m + l);
+                acc = fmaf(bl, __ldg(p.u + bt * m + l), acc);
+              }
             }
-            bv[i] = acc;
+            if (ok) bv[i] = acc;
           }
         }
         __syncwarp();
@@ -325,24 +329,34 @@ __global__ void __launch_bounds__(kRollThreads, 1) rollout_kernel(const RollPara
                                                             static_cast<size_t>(st) * p.sp.stage_bytes);
         const int rk = min(rc, rows - k * rc);
         if (!WIDE) {
-          // warp gw: rows [gw rpw, (gw+1) rpw) of the chunk, four per pass
-          for (int b0 = 0; b0 < rpw; b0 += 4) {
-            const int base = gw * rpw + b0;
-            if (base >= rk) break;
-            const int nval = min(min(4, rpw - b0), rk - base);
+          // units of 4 consecutive rows are dealt round-robin to the warps of the group, one unit per pass
+          const int nu = (rk + 3) >> 2;
+          for (int un = gw; un < nu; un += kConsWarps) {
+            const int base = 4 * un;
+            const int nval = min(4, rk - base);
             float acc[4] = {0.f, 0.f, 0.f, 0.f};
             rows_dot_n<QLMAX>(nval, tile, n, base, q0, q_end, ql, xq, acc);
-            if (warp == 0 && b0 == 0) { LTV_RT(3, cidx, 0) }
+            if (warp == 0 && un == 0) { LTV_RT(3, cidx, 0) }
             const float v = reduce4_rows(acc, lane);
-            if (warp == 0 && b0 == 0) { LTV_RT(3, cidx, 1) }
-            if (grp < nval) {
-              const int li = k * rc + base + grp;
+            if (warp == 0 && un == 0) { LTV_RT(3, cidx, 1) }
+            const int li0 = k * rc + base;
+            if (nval == 4) {
+              // all four sums into every lane: one 16-byte remote store per destination CTA, one 16-byte global store
+              float4 y;
+              y.x = __shfl_sync(0xffffffffu, v, 0) + bv[li0];
+              y.y = __shfl_sync(0xffffffffu, v, 8) + bv[li0 + 1];
+              y.z = __shfl_sync(0xffffffffu, v, 16) + bv[li0 + 2];
+              y.w = __shfl_sync(0xffffffffu, v, 24) + bv[li0 + 3];
+              if (exch && lane < C) st_async_remote_f32x4(xn + r0 + li0, y, xbar, lane);
+              if (lane == 31) *reinterpret_cast<float4*>(xg + li0) = y;
+            } else if (grp < nval) {
+              const int li = li0 + grp;
               const float y = v + bv[li];
               if (exch)
                 for (int cta = sub; cta < C; cta += 8) st_async_remote_f32(xn + r0 + li, y, xbar, cta);
               if (sub == 0) xg[li] = y;
             }
-            if (warp == 0 && b0 == 0) { LTV_RT(3, cidx, 2) }
+            if (warp == 0 && un == 0) { LTV_RT(3, cidx, 2) }
           }
         } else {
           // warp gw: its eighth of the columns of all (<= 4) rows of the chunk; partial sums meet in shared memory
@@ -353,7 +367,18 @@ __global__ void __launch_bounds__(kRollThreads, 1) rollout_kernel(const RollPara
           if (sub == 0) pb[gw * 4 + grp] = v;
           named_bar_sync(1 + grpid, kConsWarps * 32);
           const int tid = gw * 32 + lane;
-          if (tid < rk * C) {
+          if (rk == 4) {
+            if (tid < C) {
+              float4 y = *reinterpret_cast<const float4*>(bv + k * rc);
+#pragma unroll
+              for (int w = 0; w < kConsWarps; ++w) {
+                const float4 pw = *reinterpret_cast<const float4*>(pb + w * 4);
+                y.x += pw.x; y.y += pw.y; y.z += pw.z; y.w += pw.w;
+              }
+              if (exch) st_async_remote_f32x4(xn + r0 + k * rc, y, xbar, tid);
+              if (tid == 0) *reinterpret_cast<float4*>(xg + k * rc) = y;
+            }
+          } else if (tid < rk * C) {
             const int row = tid / C, cta = tid - row * C;
             float y = bv[k * rc + row];
 #pragma unroll
@@ -394,7 +419,7 @@ RollSmemPlan plan_rollout(int n, int C, int occ) {
   if (sp.wide) {
     rc = static_cast<int>(target / row_bytes);
     if (rc < 1) rc = 1;
-    if (rc > 4) rc = 4;
+    if (rc > 4 || 4u * row_bytes <= 48u * 1024u) rc = 4;   // 4-row chunks: 16-byte state exchange
     sp.rpw = 0;
   } else {
     // a multiple of 8 rows near the 32 KB target, at most 64 (8 per warp) and no more than the band needs
@@ -421,14 +446,23 @@ RollSmemPlan plan_rollout(int n, int C, int occ) {
 
 }  // namespace
 
-// `cluster` CTAs per item, `occ` CTAs per SM the shared-memory plan leaves room for; the grid is as many
-// clusters as fit on the device at that occupancy (at most one per item), each looping over items
-cudaError_t launch_rollout(const RolloutArgs& a, int cluster, int occ, int num_sms, cudaStream_t stream,
-                           unsigned long long* launches) {
+// `cluster` CTAs per item (0 = modelled); the grid is as many clusters as can be resident at once (at most one
+// per item), each looping over items
+cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches) {
+  static int max_active[2][17];
+  static bool have[2] = {false, false};
+  const int wide = a.n > kModeAMaxN ? 1 : 0;
+  if (!have[wide]) {
+    query_max_active_clusters(wide ? reinterpret_cast<const void*>(rollout_kernel<true>)
+                                   : reinterpret_cast<const void*>(rollout_kernel<false>),
+                              kRollThreads, 200 * 1024, max_active[wide]);
+    have[wide] = true;
+  }
+  if (cluster <= 0) cluster = pick_cluster_model(a.batch, a.n, max_active[wide]);
   RollParams p{};
   p.A = a.A; p.B = (a.m > 0) ? a.B : nullptr; p.c = a.c; p.x0 = a.x0; p.u = a.u; p.x_out = a.x_out;
   p.batch = a.batch; p.T = a.T; p.n = a.n; p.m = a.m;
-  p.sp = plan_rollout(a.n, cluster, occ);
+  p.sp = plan_rollout(a.n, cluster, 1);
 #ifdef LTV_ROLL_TRACE
   p.trace = g_roll_trace;
   p.trace_cap = g_roll_trace_cap;
@@ -443,7 +477,7 @@ cudaError_t launch_rollout(const RolloutArgs& a, int cluster, int occ, int num_s
     if (e != cudaSuccess) return e;
   }
   cudaLaunchConfig_t cfg{};
-  int ncl = (num_sms * occ) / cluster;
+  int ncl = max_active[wide][cluster];
   if (ncl > a.batch) ncl = a.batch;
   if (ncl < 1) ncl = 1;
   cfg.gridDim = dim3(static_cast<unsigned>(ncl) * cluster);

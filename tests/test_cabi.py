@@ -52,6 +52,8 @@ def test_workspace_sizes(L):
     assert L.ltv_scan_workspace_bytes(L.LTV_OP_SYSTEM_RESPONSE_TUBE, b, T, 301, 0) == 0
     big = L.ltv_scan_workspace_bytes(L.LTV_OP_PIPELINE_HOST, b, T, n, 6)
     assert big > b * (T * (T - 1) // 2) * n * n * 4 + b * T * n * n * 4
+    small = L.ltv_scan_workspace_bytes(L.LTV_OP_PIPELINE_HOST_NO_PHI, b, T, n, 6)
+    assert b * T * n * n * 4 < small < big - b * (T * (T - 1) // 2) * n * n * 4
 
 
 def test_host_side_validation_needs_no_gpu(L):

@@ -194,3 +194,44 @@ def test_pipeline_host_matches_device_calls(L):
                grad_x0=outs["grad_x0"].numpy(), phi=phi_host.numpy())
     _check(got, _ref_all(W))
     assert outs["phi_device_ptr"] != 0
+
+
+@pytest.mark.gpu
+def test_pipeline_host_chunked_and_without_phi(L):
+    """batch 12 is uploaded and computed in chunks (4 + 4 + 4); w=None runs rollout + adjoint only."""
+    import torch
+
+    W = generate(config(0, batch=12, T=5))
+    batch, T, n, m = W.shape
+    ref = _ref_all(W)
+    h = {k: torch.from_numpy(getattr(W, k)).pin_memory() for k in ("A", "B", "c", "x0", "u", "w", "g")}
+    ws = torch.empty(L.ltv_scan_workspace_bytes(L.LTV_OP_PIPELINE_HOST, batch, T, n, m), dtype=torch.uint8, device="cuda")
+    P = T * (T - 1) // 2
+    phi_host = torch.empty((batch, P, n, n), dtype=torch.float32).pin_memory()
+    outs = L.ltv_scan_pipeline_host(h["A"], h["B"], h["c"], h["x0"], h["u"], h["w"], h["g"], ws, phi_host=phi_host)
+    _check(dict(x=outs["x"].numpy(), r=outs["r"].numpy(), lam=outs["lam"].numpy(), grad_u=outs["grad_u"].numpy(),
+                grad_x0=outs["grad_x0"].numpy(), phi=phi_host.numpy()), ref)
+    need = L.ltv_scan_workspace_bytes(L.LTV_OP_PIPELINE_HOST_NO_PHI, batch, T, n, m)
+    assert 0 < need < ws.numel()
+    ws2 = torch.empty(need, dtype=torch.uint8, device="cuda")
+    o2 = L.ltv_scan_pipeline_host(h["A"], h["B"], h["c"], h["x0"], h["u"], None, h["g"], ws2)
+    assert o2["r"] is None and o2["phi_device_ptr"] in (0, None)
+    _check(dict(x=o2["x"].numpy(), lam=o2["lam"].numpy(), grad_u=o2["grad_u"].numpy(), grad_x0=o2["grad_x0"].numpy()),
+           {k: ref[k] for k in ("x", "lam", "grad_u", "grad_x0")})
+
+
+@pytest.mark.parametrize("cluster", [1, 2, 3, 5, 6, 7, 9, 10, 16])
+def test_vector_scans_any_cluster_size(L, cluster, monkeypatch):
+    """Rollout and adjoint give the same answer for every cluster size the model may pick (LTV_SCAN_CLUSTER
+    forces it): bands of 4-row multiples, last band blocks with fewer rows than m, clusters wider than 8."""
+    import torch
+
+    W = dense_random(2, 7, 640 if cluster == 16 else 300, 6, seed=40 + cluster)
+    d = {k: torch.from_numpy(getattr(W, k)).cuda() for k in ("A", "B", "c", "x0", "u", "g")}
+    monkeypatch.setenv("LTV_SCAN_CLUSTER", str(cluster))
+    x = L.ltv_scan_rollout(d["A"], d["B"], d["c"], d["x0"], d["u"])
+    lam, gu, gx0 = L.ltv_scan_adjoint(d["A"], d["B"], d["g"])
+    torch.cuda.synchronize()
+    rl, rgu, rgx = O.adjoint(W.A, W.B, W.g)
+    _check(dict(x=x.cpu().numpy(), lam=lam.cpu().numpy(), grad_u=gu.cpu().numpy(), grad_x0=gx0.cpu().numpy()),
+           dict(x=O.rollout(W.A, W.B, W.c, W.x0, W.u), lam=rl, grad_u=rgu, grad_x0=rgx))
