@@ -9,37 +9,66 @@ namespace ltv {
 
 // ------------------------------------------------------------------------------------------ level 0
 // Phi(s+1,s) = A_s, part[b][q(s+1,s)][0][i] = sum_j |A_s[i,j]| w_s[j]; part slots 1..NT-1 are zeroed.
-// HBM-bound: one warp per matrix row, 128-bit loads/stores.
+// HBM-bound copy.  A warp takes FOUR consecutive rows (never straddling a block: n % 4 == 0) and, per pass,
+// four column quads per lane: 16 independent 128-bit loads in flight per lane, w_s read once for the four rows,
+// and the four row sums finished with one transpose-reduce (6 shuffles) instead of four 5-level trees.
+__device__ __forceinline__ float level0_reduce4(const float (&a)[4], int lane) {
+  const bool hi16 = (lane & 16) != 0;
+  const float b0 = (hi16 ? a[2] : a[0]) + __shfl_xor_sync(0xffffffffu, hi16 ? a[0] : a[2], 16);
+  const float b1 = (hi16 ? a[3] : a[1]) + __shfl_xor_sync(0xffffffffu, hi16 ? a[1] : a[3], 16);
+  const bool hi8 = (lane & 8) != 0;
+  float v = (hi8 ? b1 : b0) + __shfl_xor_sync(0xffffffffu, hi8 ? b0 : b1, 8);
+  v += __shfl_xor_sync(0xffffffffu, v, 4);
+  v += __shfl_xor_sync(0xffffffffu, v, 2);
+  v += __shfl_xor_sync(0xffffffffu, v, 1);
+  return v;   // lanes 8g .. 8g+7 hold the sum of row g
+}
+
 __global__ void __launch_bounds__(256) phi_level0_kernel(const float* __restrict__ A, const float* __restrict__ w,
                                                          float* __restrict__ phi, float* __restrict__ part,
                                                          int batch, int T, int n, int NT) {
   const int P = T * (T - 1) / 2;
-  const long long nrows = static_cast<long long>(batch) * (T - 1) * n;
+  const long long nunits = static_cast<long long>(batch) * (T - 1) * (n >> 2);
   const int lane = threadIdx.x & 31;
   const int n4 = n >> 2;
-  for (long long row = static_cast<long long>(blockIdx.x) * 8 + (threadIdx.x >> 5); row < nrows;
-       row += static_cast<long long>(gridDim.x) * 8) {
-    const int i = static_cast<int>(row % n);
-    const long long bs = row / n;
+  for (long long un = static_cast<long long>(blockIdx.x) * 8 + (threadIdx.x >> 5); un < nunits;
+       un += static_cast<long long>(gridDim.x) * 8) {
+    const int i = 4 * static_cast<int>(un % n4);
+    const long long bs = un / n4;
     const int s = static_cast<int>(bs % (T - 1));
     const int b = static_cast<int>(bs / (T - 1));
     const float4* src = reinterpret_cast<const float4*>(A + ((static_cast<size_t>(b) * T + s) * n + i) * n);
     const float4* wv = reinterpret_cast<const float4*>(w + (static_cast<size_t>(b) * T + s) * n);
     const size_t q = static_cast<size_t>(b) * P + phi_colbase(T, s);
     float* dst = phi + (q * n + i) * n;
-    float acc = 0.f;
-    for (int c = lane; c < n4; c += 32) {
-      const float4 a = __ldcs(src + c);
-      const float4 ww = __ldg(wv + c);
-      st_global_f4_na(dst + 4 * c, a);
-      acc = fmaf(fabsf(a.x), ww.x, fmaf(fabsf(a.y), ww.y, fmaf(fabsf(a.z), ww.z, fmaf(fabsf(a.w), ww.w, acc))));
-    }
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int c0 = 0; c0 < n4; c0 += 128) {
+      float4 a[4][4], ww[4];
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if (lane == 0) part[(q * NT) * n + i] = acc;
-    if (lane > 0 && lane < NT) part[(q * NT + lane) * n + i] = 0.f;
-    for (int e = 32; e < NT; e += 32)
-      if (e + lane < NT) part[(q * NT + e + lane) * n + i] = 0.f;
+      for (int j = 0; j < 4; ++j) {
+        const int c = c0 + lane + 32 * j;
+        const bool ok = c < n4;
+        ww[j] = ok ? __ldg(wv + c) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) a[r][j] = ok ? __ldcs(src + static_cast<size_t>(r) * n4 + c) : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int c = c0 + lane + 32 * j;
+        if (c < n4) {
+#pragma unroll
+          for (int r = 0; r < 4; ++r) {
+            st_global_f4_na(dst + static_cast<size_t>(r) * n + 4 * c, a[r][j]);
+            acc[r] = fmaf(fabsf(a[r][j].x), ww[j].x, fmaf(fabsf(a[r][j].y), ww[j].y,
+                     fmaf(fabsf(a[r][j].z), ww[j].z, fmaf(fabsf(a[r][j].w), ww[j].w, acc[r]))));
+          }
+        }
+      }
+    }
+    const float v = level0_reduce4(acc, lane);
+    const int g = lane >> 3, sub = lane & 7;
+    // lane (g, sub): row i + g, tube slots sub, sub + 8, ... (slot 0 = the sum, the others zero)
+    for (int e = sub; e < NT; e += 8) part[(q * NT + e) * n + i + g] = (e == 0) ? v : 0.f;
   }
 }
 
@@ -137,9 +166,9 @@ __global__ void __launch_bounds__(128) phi_tube_finalize_kernel(const float* __r
 }
 
 cudaError_t launch_phi_level0(const PhiArgs& a, int NT, int num_sms, cudaStream_t stream) {
-  const long long nrows = static_cast<long long>(a.batch) * (a.T - 1) * a.n;
-  long long blocks = (nrows + 7) / 8;
-  const long long cap = static_cast<long long>(num_sms) * 16;
+  const long long nunits = static_cast<long long>(a.batch) * (a.T - 1) * (a.n >> 2);   // 4-row units, one per warp
+  long long blocks = (nunits + 7) / 8;
+  const long long cap = static_cast<long long>(num_sms) * 8;
   if (blocks > cap) blocks = cap;
   ProfScope prof(kProfPhiLevel0, stream);
   phi_level0_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(a.A, a.w, a.phi, a.part, a.batch, a.T, a.n, NT);
