@@ -120,14 +120,15 @@ def workload(cfg_index, rank, world, batch_override=None):
     return cfg, W
 
 
-def cpu_oracle_step(W, items):
+def cpu_oracle_step(W, items, phi_on=True):
     """One pass of the whole path by the fp64 oracle over `items` batch items; returns seconds."""
     from oracle import ltv_oracle as O
 
     t0 = time.perf_counter()
     for b in range(items):
         O.rollout_item(W.A[b], W.B[b], W.c[b], W.x0[b], W.u[b])
-        O.system_response_tube_item(W.A[b], W.w[b])
+        if phi_on:
+            O.system_response_tube_item(W.A[b], W.w[b])
         O.adjoint_item(W.A[b], W.B[b], W.g[b])
     return time.perf_counter() - t0
 
@@ -144,24 +145,29 @@ def blas_threads():
 def run_reference(args, rank, world):
     if rank != 0:
         return
-    cfg, W = workload(args.config, 0, 1, batch_override=max(1, args.cpu_items or 2))
+    cfg, W = workload(args.config, 0, 1, batch_override=max(1, args.cpu_items or (8 if args.config in (1, 2) else
+                                                                                  2 if args.config == 3 else 32)))
     items = W.A.shape[0]
+    from workloads import config as _config
+    config_batch = _config(args.config)["batch"]
     T, n = cfg["T"], cfg["n"]
     P = T * (T - 1) // 2
+    phi_on = args.config != 4
+    unit = UNIT if phi_on else UNIT_C5
     for _ in range(min(args.warmup, 1)):
-        cpu_oracle_step(W, 1)
-    times = [cpu_oracle_step(W, items) for _ in range(args.steps)]
+        cpu_oracle_step(W, 1, phi_on)
+    times = [cpu_oracle_step(W, items, phi_on) for _ in range(args.steps)]
     sec = sum(times) / len(times)
-    val = items * P / sec
+    val = items * (P if phi_on else 1) / sec
     cores = blas_threads()
-    line = dict(metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+    line = dict(metric=METRIC, value=val, unit=unit, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
                 ms_per_step=sec * 1e3, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
                 data="synthetic", impl="reference",
                 config=dict(workload=f"{cfg['name']}: n={n} m={cfg['m']} T={T}, {items}-item sample per step "
-                                     f"(full batch {64 if args.config == 1 else cfg['batch']})", l2="n/a (CPU)"),
-                cpu_baseline=dict(value=val, unit=UNIT, cores=cores, kind="oracle",
+                                     f"(full batch {config_batch})", l2="n/a (CPU)"),
+                cpu_baseline=dict(value=val, unit=unit, cores=cores, kind="oracle",
                                   sample=f"{items} items of {cfg['name']} per step, whole path in fp64 numpy"),
-                e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                e2e=dict(value=val, unit=unit, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
                 gpu_launches=0)
     print(json.dumps(line), flush=True)
 
@@ -315,8 +321,12 @@ def main():
     # ---- CPU oracle beside it (rank 0, N = 1 only)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        items = min(batch, args.cpu_items or (2 if n <= 600 else 1))
-        sec = cpu_oracle_step(W, items)
+        if args.cpu_items:
+            items = min(batch, args.cpu_items)
+        else:                                   # about 10-20 s of oracle work: calibrate on one item
+            t1 = cpu_oracle_step(W, 1, phi_on)
+            items = max(1, min(batch, int(12.0 / max(t1, 1e-3))))
+        sec = cpu_oracle_step(W, items, phi_on)
         cpu = dict(value=items * (P if phi_on else 1) / sec, unit=UNIT if phi_on else UNIT_C5, cores=blas_threads(), kind="oracle",
                    sample=f"{items} of {batch} items of {cfg['name']}, whole path, fp64 numpy, {sec:.1f} s")
 
