@@ -235,3 +235,39 @@ def test_vector_scans_any_cluster_size(L, cluster, monkeypatch):
     rl, rgu, rgx = O.adjoint(W.A, W.B, W.g)
     _check(dict(x=x.cpu().numpy(), lam=lam.cpu().numpy(), grad_u=gu.cpu().numpy(), grad_x0=gx0.cpu().numpy()),
            dict(x=O.rollout(W.A, W.B, W.c, W.x0, W.u), lam=rl, grad_u=rgu, grad_x0=rgx))
+
+
+@pytest.mark.parametrize("n,T,batch,m", [(644, 3, 2, 6),      # first size of the column-split (wide) rollout mode
+                                         (1200, 4, 3, 12),    # 4-row chunks, 16-byte state exchange
+                                         (4096, 3, 1, 6),     # 2-row chunks (4 rows exceed a ring stage)
+                                         (8192, 2, 1, 3),     # maximum n: one row per chunk
+                                         (180, 130, 2, 6),    # long horizon: many wraps of every ring / parity bit
+                                         (36, 5, 150, 6)])    # more items than resident clusters, tiny n
+def test_vector_scans_edge_sizes(L, n, T, batch, m):
+    """Rollout + adjoint only (no Phi: the oracle's n^3 products would dominate) at the extremes of n, T, batch."""
+    import torch
+
+    W = dense_random(batch, T, n, m, seed=7 * n + T, scale=0.3)
+    d = {k: torch.from_numpy(getattr(W, k)).cuda() for k in ("A", "B", "c", "x0", "u", "g")}
+    x = L.ltv_scan_rollout(d["A"], d["B"], d["c"], d["x0"], d["u"])
+    lam, gu, gx0 = L.ltv_scan_adjoint(d["A"], d["B"], d["g"])
+    torch.cuda.synchronize()
+    rl, rgu, rgx = O.adjoint(W.A, W.B, W.g)
+    _check(dict(x=x.cpu().numpy(), lam=lam.cpu().numpy(), grad_u=gu.cpu().numpy(), grad_x0=gx0.cpu().numpy()),
+           dict(x=O.rollout(W.A, W.B, W.c, W.x0, W.u), lam=rl, grad_u=rgu, grad_x0=rgx))
+
+
+@pytest.mark.parametrize("n,T,batch", [(96, 4, 2),     # smallest tensor-core size: one 96-wide n-tile
+                                       (164, 5, 1),    # two n-tiles, the second 4 columns wide
+                                       (1000, 3, 1),   # K = 31.25 k-blocks: ragged last k-block
+                                       (320, 20, 1),   # T-1 = 19: last segments ragged on every level
+                                       (128, 3, 5)])   # T = 3: a single level-1 product per item
+def test_phi_tube_shapes(L, n, T, batch):
+    import torch
+
+    W = dense_random(batch, T, n, 1, seed=3 * n + T, scale=0.4)
+    A, w = torch.from_numpy(W.A).cuda(), torch.from_numpy(W.w).cuda()
+    phi, r = L.ltv_scan_system_response_tube(A, w)
+    torch.cuda.synchronize()
+    ref = _ref_all(W)
+    _check(dict(phi=phi.cpu().numpy(), r=r.cpu().numpy()), dict(phi=ref["phi"], r=ref["r"]))
