@@ -20,6 +20,10 @@ sequential recursion - "We obtain the solution to (14) by a forward parallel ass
   tube             r_0 = 0; r_t = sum_{s<t} |Phi(t,s)| w_s           PAPER.md:147 eq.(12e) in the
                                                                      north_star (ii) form (element-wise
                                                                      abs, box disturbance |d_s| <= w_s)
+  tube_row2norm    tau_0 = 0; tau_t[i] = sum_{s<t} ||row_i(Phi(t,s) E_s)||_2    PAPER.md:147 eq.(12e) as printed
+                                                                     (row-wise two-norm, :150), with the
+                                                                     stand-in E_s = diag(w_s) (SURVEY 8f
+                                                                     NEXT-2; reading q3b)
   adjoint          lam_T = g_T; lam_t = A_t^T lam_{t+1} + g_t;       PAPER.md:106-110 eq.(10) chained
                    grad_u[t] = B_t^T lam_{t+1}; grad_x0 = A_0^T lam_1   over the horizon; north_star (iii)
 
@@ -124,6 +128,25 @@ def tube_item(A, w):
 
 def tube(A, w):
     return np.stack([tube_item(A[b], w[b]) for b in range(A.shape[0])])
+
+
+def tube_row2norm_item(A, w):
+    """tau[T,n]: tau_0 = 0, tau_t[i] = sum_{s=0}^{t-1} sqrt(sum_j (Phi(t,s)[i,j] w_s[j])^2)  -  eq.(12e),
+    PAPER.md:147, state-disturbance term with E_s = diag(w_s)."""
+    T, n, _ = A.shape
+    w = _f64(w)
+    tau = np.zeros((T, n))
+    for t, row in phi_rows_item(A):
+        acc = np.zeros(n)
+        for s in range(t):
+            PE = row[s] * w[s][None, :]                 # Phi(t,s) E_s
+            acc = acc + np.sqrt(np.sum(PE * PE, axis=1))  # row-wise two-norm
+        tau[t] = acc
+    return tau
+
+
+def tube_row2norm(A, w):
+    return np.stack([tube_row2norm_item(A[b], w[b]) for b in range(A.shape[0])])
 
 
 def system_response_tube_item(A, w):

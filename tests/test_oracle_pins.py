@@ -210,6 +210,80 @@ def test_tube_linear_monotone_in_w():
 
 
 # ------------------------------------------------------------------ rollout
+# --------------------------------------------------------------------------- row-wise two-norm tube (12e), NEXT-2
+def test_tube2_identity_A_and_rotation_closed_forms():
+    """A = I: each row of Phi E_s has one entry => tau_t = sum_{s<t} w_s.  Rotations R(th_t) with w_s = c_s (1,1):
+    rows of R(.) c_s have two-norm c_s => tau_t = sum_{s<t} c_s whatever the angles."""
+    rng = np.random.default_rng(5)
+    T, n = 7, 5
+    w = rng.uniform(0.0, 1.0, (T, n))
+    A = np.broadcast_to(np.eye(n), (T, n, n)).copy()
+    tau = O.tube_row2norm_item(A, w)
+    np.testing.assert_allclose(tau[0], 0.0)
+    np.testing.assert_allclose(tau[1:], np.cumsum(w, axis=0)[:-1], rtol=1e-13)
+    th = rng.uniform(-2.0, 2.0, T)
+    R = np.stack([np.array([[np.cos(a), -np.sin(a)], [np.sin(a), np.cos(a)]]) for a in th])
+    c = rng.uniform(0.1, 1.0, T)
+    tau = O.tube_row2norm_item(R, np.stack([c, c], axis=1))
+    np.testing.assert_allclose(tau[1:, 0], np.cumsum(c)[:-1], rtol=1e-13)
+    np.testing.assert_allclose(tau[1:, 1], np.cumsum(c)[:-1], rtol=1e-13)
+
+
+def test_tube2_bruteforce_python_loops():
+    import math
+
+    W = dense_random(1, 5, 4, 1, seed=31)
+    A, w = W.A[0].astype(np.float64), W.w[0].astype(np.float64)
+    T, n = 5, 4
+    got = O.tube_row2norm_item(W.A[0], W.w[0])
+    for t in range(1, T):
+        for i in range(n):
+            tot = 0.0
+            for s in range(t):
+                M = np.eye(n)
+                for k in range(s, t):          # Phi(t,s) = A_{t-1} ... A_s by explicit left products
+                    M = A[k] @ M
+                tot += math.sqrt(sum((M[i, j] * w[s][j]) ** 2 for j in range(n)))
+            assert abs(got[t, i] - tot) <= 1e-13 * max(1.0, abs(tot))
+
+
+def test_tube2_containment_cauchy_schwarz_and_tightness():
+    """Disturbances d_s = E_s v_s with ||v_s||_2 <= 1: |sum_s Phi(t,s) d_s|_i <= tau_t[i], with equality in row i
+    for v_s = row_i(Phi(t,s) E_s) / its norm (PAPER.md:218 containment; Cauchy-Schwarz)."""
+    rng = np.random.default_rng(9)
+    W = dense_random(1, 6, 7, 1, seed=77)
+    A, w = W.A[0], W.w[0].astype(np.float64) * 1e3
+    T, n = 6, 7
+    tau = O.tube_row2norm_item(A, w)
+    Phi = O.system_response_item(A)
+    for t in range(1, T):
+        for _ in range(20):
+            dev = np.zeros(n)
+            for s in range(t):
+                v = rng.normal(size=n)
+                v /= max(1.0, np.linalg.norm(v))
+                dev += Phi[O.packed_index(t, s)] @ (w[s] * v)
+            assert np.all(np.abs(dev) <= tau[t] * (1 + 1e-12))
+        i = t % n
+        dev = 0.0
+        for s in range(t):
+            rowE = Phi[O.packed_index(t, s)][i] * w[s]
+            dev += rowE @ (rowE / np.linalg.norm(rowE))
+        assert abs(dev - tau[t, i]) <= 1e-12 * tau[t, i]
+
+
+def test_tube2_sandwiched_by_box_tube():
+    """||v||_2 <= ||v||_1 <= sqrt(n) ||v||_2 row by row: box/sqrt(n) <= tau <= box (the box tube is pinned above)."""
+    W = generate(config(0))
+    A, w = W.A[0], W.w[0]
+    n = A.shape[-1]
+    box, tau = O.tube_item(A, w), O.tube_row2norm_item(A, w)
+    assert np.all(tau <= box * (1 + 1e-12)) and np.all(tau >= box / np.sqrt(n) * (1 - 1e-12))
+    assert np.any(tau < 0.9 * box)                       # and it is a different quantity
+    np.testing.assert_allclose(O.tube_row2norm(W.A, W.w)[0], tau, rtol=0, atol=0)
+    np.testing.assert_allclose(O.tube_row2norm_item(A, 3.0 * w.astype(np.float64)), 3.0 * tau, rtol=1e-13)   # homogeneous in w
+
+
 def test_rollout_identity_A_is_cumsum():
     T, n, m = 6, 4, 2
     _, B, c, x0, u, _, _ = _rand(T, n, m, seed=12)
