@@ -69,6 +69,9 @@ enum { LTV_OP_ROLLOUT = 0, LTV_OP_SYSTEM_RESPONSE_TUBE = 1, LTV_OP_ADJOINT = 2, 
  * divide-and-conquer combine  Phi(t,s) = Phi(t,mid) Phi(mid,s)  stream its left operand as one matrix. */
 enum { LTV_PHI_COLUMN_PACKED = 0 };
 
+/* `flags` bits of ltv_scan_system_response_tube. */
+enum { LTV_TUBE_ROW_2NORM = 1 };
+
 /* Block index q(t,s) of the COLUMN_PACKED layout; -1 if not 0 <= s < t <= T-1.  Pure host arithmetic. */
 LTV_API long long ltv_phi_block_index(int T, int t, int s);
 
@@ -95,7 +98,8 @@ LTV_API int ltv_scan_rollout(const float* A, const float* B, const float* c, con
  *   w        device [batch,T,n]       required; w_s >= 0, only s <= T-2 read
  *   phi_out  device [batch,P,n,n]     P = T(T-1)/2, layout `phi_layout`; Phi(t,t) = I is not stored
  *   r_out    device [batch,T,n]       r_0 = 0, r_t = sum_{s<t} |Phi(t,s)| w_s  (element-wise abs)
- *   flags    must be 0
+ *   flags    0, or LTV_TUBE_ROW_2NORM: r_t[i] = sum_{s<t} || row_i(Phi(t,s) diag(w_s)) ||_2, the row-wise two-norm
+ *            tube of eq.(12e) as printed with the disturbance scaling E_s = diag(w_s)
  * T == 1 is valid: no blocks, r zero-filled.  Time-parallel schedule: level 0 copies the sub-diagonal
  * blocks Phi(s+1,s) = A_s; level l = 1..ceil(log2(T-1)) forms, for every aligned segment of 2^l steps with
  * midpoint mid, all Phi(t,s) = Phi(t,mid) Phi(mid,s), s < mid < t, as one stacked GEMM (3xTF32 on tcgen05

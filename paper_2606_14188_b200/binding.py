@@ -18,6 +18,7 @@ STATUS_NAMES = {
 }
 LTV_OP_ROLLOUT, LTV_OP_SYSTEM_RESPONSE_TUBE, LTV_OP_ADJOINT, LTV_OP_PIPELINE_HOST = 0, 1, 2, 3
 LTV_OP_PIPELINE_HOST_NO_PHI = 4
+LTV_TUBE_ROW_2NORM = 1
 LTV_PHI_COLUMN_PACKED = 0
 
 EXPORTS = (
@@ -130,8 +131,9 @@ def ltv_scan_rollout(A, B, c, x0, u, x_out=None):
     return x_out
 
 
-def ltv_scan_system_response_tube(A, w, phi_out=None, r_out=None, workspace=None):
-    """Returns (phi[batch,P,n,n] COLUMN_PACKED, r[batch,T,n]).  `workspace`: optional uint8 CUDA tensor."""
+def ltv_scan_system_response_tube(A, w, phi_out=None, r_out=None, workspace=None, two_norm=False):
+    """Returns (phi[batch,P,n,n] COLUMN_PACKED, r[batch,T,n]).  `workspace`: optional uint8 CUDA tensor.
+    two_norm=True: the row-wise two-norm tube of eq.(12e) with E_s = diag(w_s) instead of the box tube."""
     batch, T, n, _ = A.shape
     P = T * (T - 1) // 2
     _dev(A, "A", (batch, T, n, n)); _dev(w, "w", (batch, T, n))
@@ -144,7 +146,8 @@ def ltv_scan_system_response_tube(A, w, phi_out=None, r_out=None, workspace=None
     if workspace is None:
         workspace = torch.empty(max(need, 16), device=A.device, dtype=torch.uint8)
     st = lib.ltv_scan_system_response_tube(_ptr(A), _ptr(w), _ptr(phi_out), _ptr(r_out), batch, T, n,
-                                           LTV_PHI_COLUMN_PACKED, 0, _ptr(workspace), workspace.numel(), _stream())
+                                           LTV_PHI_COLUMN_PACKED, LTV_TUBE_ROW_2NORM if two_norm else 0,
+                                           _ptr(workspace), workspace.numel(), _stream())
     if st != LTV_OK:
         raise LtvError(st, "ltv_scan_system_response_tube")
     return phi_out, r_out

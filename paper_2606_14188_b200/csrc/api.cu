@@ -240,7 +240,7 @@ int ltv_scan_system_response_tube(const float* A, const float* w, float* phi_out
   if (T > 1 && !phi_out) return LTV_ERR_NULL_PTR;
   int st = check_dims(batch, T, n, 0);
   if (st != LTV_OK) return st;
-  if (phi_layout != LTV_PHI_COLUMN_PACKED || flags != 0) return LTV_ERR_BAD_DIM;
+  if (phi_layout != LTV_PHI_COLUMN_PACKED || (flags & ~static_cast<unsigned>(LTV_TUBE_ROW_2NORM)) != 0) return LTV_ERR_BAD_DIM;
   if (misaligned(A) || misaligned(w) || misaligned(phi_out) || misaligned(r_out) || misaligned(workspace))
     return LTV_ERR_ALIGNMENT;
   const size_t need = phi_workspace_bytes(batch, T, n);
@@ -249,7 +249,7 @@ int ltv_scan_system_response_tube(const float* A, const float* w, float* phi_out
   int sms = 0;
   st = check_device(&sms);
   if (st != LTV_OK) return st;
-  PhiArgs a{A, w, phi_out, r_out, static_cast<float*>(workspace), batch, T, n};
+  PhiArgs a{A, w, phi_out, r_out, static_cast<float*>(workspace), batch, T, n, (flags & LTV_TUBE_ROW_2NORM) ? 1 : 0};
   unsigned long long l = 0;
   cudaError_t e = launch_phi_tube(a, static_cast<cudaStream_t>(cuda_stream), &l);
   g_launches += l;

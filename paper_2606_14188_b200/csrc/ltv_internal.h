@@ -29,6 +29,7 @@ struct PhiArgs {
   float *phi, *r;
   float* part;  // workspace: [batch, P, NT, n] per-(block, n-tile) tube partial sums
   int batch, T, n;
+  int tube_mode;  // 0: sum_j |Phi_ij| w_j (box tube); 1: sqrt(sum_j (Phi_ij w_j)^2) per block (row-wise two-norm, eq.(12e))
 };
 // n-tile width the Phi path uses for this n (decides the size of `part`) and whether it is the tcgen05 path
 int phi_tile_n(int n);

@@ -7,6 +7,13 @@
 
 namespace ltv {
 
+// one term of the fused tube reduction: |d| w (box tube) or (d w)^2 (row-wise two-norm tube, summed per block and
+// square-rooted by the finalise kernel)
+__device__ __forceinline__ float tube_term(float d, float w, int mode) {
+  const float dw = d * w;
+  return mode ? dw * dw : fabsf(dw);
+}
+
 // ------------------------------------------------------------------------------------------ level 0
 // Phi(s+1,s) = A_s, part[b][q(s+1,s)][0][i] = sum_j |A_s[i,j]| w_s[j]; part slots 1..NT-1 are zeroed.
 // HBM-bound copy.  A warp takes FOUR consecutive rows (never straddling a block: n % 4 == 0) and, per pass,
@@ -26,7 +33,7 @@ __device__ __forceinline__ float level0_reduce4(const float (&a)[4], int lane) {
 
 __global__ void __launch_bounds__(256) phi_level0_kernel(const float* __restrict__ A, const float* __restrict__ w,
                                                          float* __restrict__ phi, float* __restrict__ part,
-                                                         int batch, int T, int n, int NT) {
+                                                         int batch, int T, int n, int NT, int mode) {
   const int P = T * (T - 1) / 2;
   const long long nunits = static_cast<long long>(batch) * (T - 1) * (n >> 2);
   const int lane = threadIdx.x & 31;
@@ -59,8 +66,8 @@ __global__ void __launch_bounds__(256) phi_level0_kernel(const float* __restrict
 #pragma unroll
           for (int r = 0; r < 4; ++r) {
             st_global_f4_na(dst + static_cast<size_t>(r) * n + 4 * c, a[r][j]);
-            acc[r] = fmaf(fabsf(a[r][j].x), ww[j].x, fmaf(fabsf(a[r][j].y), ww[j].y,
-                     fmaf(fabsf(a[r][j].z), ww[j].z, fmaf(fabsf(a[r][j].w), ww[j].w, acc[r]))));
+            acc[r] += (tube_term(a[r][j].x, ww[j].x, mode) + tube_term(a[r][j].y, ww[j].y, mode)) +
+                      (tube_term(a[r][j].z, ww[j].z, mode) + tube_term(a[r][j].w, ww[j].w, mode));
           }
         }
       }
@@ -76,7 +83,7 @@ __global__ void __launch_bounds__(256) phi_level0_kernel(const float* __restrict
 // 64 x 64 output tile, 256 threads, 4 x 4 register micro-tile, K blocked by 16 through shared memory.
 constexpr int kST = 64, kSK = 16;
 __global__ void __launch_bounds__(256) phi_combine_simt_kernel(float* phi, const float* __restrict__ w,
-                                                               float* __restrict__ part, PhiGeom g) {
+                                                               float* __restrict__ part, PhiGeom g, int mode) {
   __shared__ float As[kSK][kST + 4];  // [k][m]
   __shared__ float Bs[kSK][kST + 4];  // [k][j]
   __shared__ float ws[kST];
@@ -129,7 +136,7 @@ __global__ void __launch_bounds__(256) phi_combine_simt_kernel(float* phi, const
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         const int j = j0 + tx * 4 + c;
-        tb = fmaf(fabsf(acc[r][c]), ws[tx * 4 + c], tb);
+        tb += tube_term(acc[r][c], ws[tx * 4 + c], mode);
         if (row < Mrows && j < n) Out[static_cast<size_t>(row) * n + j] = acc[r][c];
       }
       tube[ty * 4 + r][tx] = tb;
@@ -150,16 +157,19 @@ __global__ void __launch_bounds__(256) phi_combine_simt_kernel(float* phi, const
 }
 
 // ------------------------------------------------------------------------------------------ finalise
-// r[b][t][i] = sum_{s<t} sum_{nt} part[b][q(t,s)][nt][i], fixed order; r[b][0][:] = 0.
+// r[b][t][i] = sum_{s<t} f(sum_{nt} part[b][q(t,s)][nt][i]), f = identity (box tube) or sqrt (two-norm tube: the
+// partials are sums of squares over the columns of an n-tile); fixed order; r[b][0][:] = 0.
 __global__ void __launch_bounds__(128) phi_tube_finalize_kernel(const float* __restrict__ part, float* __restrict__ r,
-                                                                int batch, int T, int n, int NT) {
+                                                                int batch, int T, int n, int NT, int mode) {
   const int P = T * (T - 1) / 2;
   const int t = blockIdx.x % T, b = blockIdx.x / T;
   for (int i = blockIdx.y * blockDim.x + threadIdx.x; i < n; i += gridDim.y * blockDim.x) {
     float acc = 0.f;
     for (int s = 0; s < t; ++s) {
       const size_t q = static_cast<size_t>(b) * P + phi_colbase(T, s) + (t - s - 1);
-      for (int nt = 0; nt < NT; ++nt) acc += part[(q * NT + nt) * n + i];
+      float blk = 0.f;
+      for (int nt = 0; nt < NT; ++nt) blk += part[(q * NT + nt) * n + i];
+      acc += mode ? sqrtf(blk) : blk;
     }
     r[(static_cast<size_t>(b) * T + t) * n + i] = acc;
   }
@@ -171,7 +181,8 @@ cudaError_t launch_phi_level0(const PhiArgs& a, int NT, int num_sms, cudaStream_
   const long long cap = static_cast<long long>(num_sms) * 8;
   if (blocks > cap) blocks = cap;
   ProfScope prof(kProfPhiLevel0, stream);
-  phi_level0_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(a.A, a.w, a.phi, a.part, a.batch, a.T, a.n, NT);
+  phi_level0_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(a.A, a.w, a.phi, a.part, a.batch, a.T, a.n, NT,
+                                                                       a.tube_mode);
   return cudaGetLastError();
 }
 
@@ -182,7 +193,7 @@ cudaError_t launch_phi_combine_simt(const PhiArgs& a, int level, int num_sms, cu
   const long long cap = static_cast<long long>(num_sms) * 8;
   if (blocks > cap) blocks = cap;
   ProfScope prof(kProfPhiCombineSimt, stream);
-  phi_combine_simt_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(a.phi, a.w, a.part, g);
+  phi_combine_simt_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(a.phi, a.w, a.part, g, a.tube_mode);
   return cudaGetLastError();
 }
 
@@ -190,7 +201,7 @@ cudaError_t launch_phi_finalize(const PhiArgs& a, int NT, cudaStream_t stream) {
   dim3 grid(static_cast<unsigned>(a.batch) * a.T, static_cast<unsigned>((a.n + 127) / 128));
   if (grid.y > 64) grid.y = 64;
   ProfScope prof(kProfPhiFinalize, stream);
-  phi_tube_finalize_kernel<<<grid, 128, 0, stream>>>(a.part, a.r, a.batch, a.T, a.n, NT);
+  phi_tube_finalize_kernel<<<grid, 128, 0, stream>>>(a.part, a.r, a.batch, a.T, a.n, NT, a.tube_mode);
   return cudaGetLastError();
 }
 

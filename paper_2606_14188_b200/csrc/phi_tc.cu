@@ -57,6 +57,7 @@ struct TcParams {
   float* part;
   PhiGeom g;
   int stages;
+  int tube_mode;              // 0: |d| w, 1: (d w)^2 (row-wise two-norm tube; the finalise kernel takes the root)
   unsigned long long* trace;  // experiments only (DBG & 4096): per-role clock64 log of CTA 0
   int trace_cap;
   int dbg;                    // experiments only: selects a DBG instantiation (LTV_SCAN_TC_DBG)
@@ -302,6 +303,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
     const int wq = warp - 4;            // == warp % 4: the TMEM lane quarter this warp may read
     const int etid = threadIdx.x - 128;
     uint8_t* sbox = stage_out + wq * 4096;
+    const bool two_norm = p.tube_mode != 0;
     uint32_t lt = 0;
     for (long long idx = unit; idx < g.total; idx += nunits, ++lt) {
       if (warp == 4) { LTV_TRACE(4, lt, 0) }
@@ -336,10 +338,12 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
 #pragma unroll
           for (int e = 0; e < 8; ++e) {
             const float4 ww = w4[e];
-            tube4[0] = fmaf(fabsf(__uint_as_float(vc[4 * e + 0])), ww.x, tube4[0]);
-            tube4[1] = fmaf(fabsf(__uint_as_float(vc[4 * e + 1])), ww.y, tube4[1]);
-            tube4[2] = fmaf(fabsf(__uint_as_float(vc[4 * e + 2])), ww.z, tube4[2]);
-            tube4[3] = fmaf(fabsf(__uint_as_float(vc[4 * e + 3])), ww.w, tube4[3]);
+            const float d0 = __uint_as_float(vc[4 * e + 0]) * ww.x, d1 = __uint_as_float(vc[4 * e + 1]) * ww.y;
+            const float d2 = __uint_as_float(vc[4 * e + 2]) * ww.z, d3 = __uint_as_float(vc[4 * e + 3]) * ww.w;
+            tube4[0] += two_norm ? d0 * d0 : fabsf(d0);
+            tube4[1] += two_norm ? d1 * d1 : fabsf(d1);
+            tube4[2] += two_norm ? d2 * d2 : fabsf(d2);
+            tube4[3] += two_norm ? d3 * d3 : fabsf(d3);
           }
         }
         if (DBG & 1) continue;
@@ -493,7 +497,7 @@ cudaError_t phi_tc_make_maps(const PhiArgs& a, int nch, void* maps_out) {
 cudaError_t launch_phi_combine_tc(const PhiArgs& a, int level, int nch, const void* maps, int num_sms,
                                   cudaStream_t stream) {
   TcParams p{};
-  p.phi = a.phi; p.w = a.w; p.part = a.part;
+  p.phi = a.phi; p.w = a.w; p.part = a.part; p.tube_mode = a.tube_mode;
   p.dbg = env_int("TC_DBG", 0);
 #ifdef LTV_TC_EXPERIMENTS
   p.trace = g_trace;

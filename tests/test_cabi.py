@@ -70,7 +70,8 @@ def test_host_side_validation_needs_no_gpu(L):
     s = L.lib.ltv_scan_system_response_tube
     assert s(p, p, p, None, 1, 2, 4, 0, 0, p, 1 << 20, None) == 1                   # NULL r_out
     assert s(p, p, p, p, 1, 2, 4, 1, 0, p, 1 << 20, None) == 2                      # unknown layout
-    assert s(p, p, p, p, 1, 2, 4, 0, 1, p, 1 << 20, None) == 2                      # unknown flag
+    assert s(p, p, p, p, 1, 2, 4, 0, 2, p, 1 << 20, None) == 2                      # unknown flag
+    assert s(p, p, p, p, 1, 2, 4, 0, L.LTV_TUBE_ROW_2NORM, p, 8, None) == 5         # known flag passes on
     assert s(p, p, p, p, 1, 2, 4, 0, 0, p, 8, None) == 5                            # workspace too small
     a = L.lib.ltv_scan_adjoint
     assert a(p, None, p, p, p, None, 1, 2, 4, 2, None, 0, None) == 1                # grad_u wanted, B NULL

@@ -271,3 +271,30 @@ def test_phi_tube_shapes(L, n, T, batch):
     torch.cuda.synchronize()
     ref = _ref_all(W)
     _check(dict(phi=phi.cpu().numpy(), r=r.cpu().numpy()), dict(phi=ref["phi"], r=ref["r"]))
+
+
+@pytest.mark.parametrize("k,over", [(0, {}), (1, dict(batch=2, T=9)), (2, dict(batch=1, T=5))])
+def test_row_two_norm_tube_configs(L, k, over):
+    """flags = LTV_TUBE_ROW_2NORM: eq.(12e) as printed (row-wise two-norm, E_s = diag(w_s)); Phi itself is unchanged."""
+    import torch
+
+    W = generate(config(k, **over))
+    A, w = torch.from_numpy(W.A).cuda(), torch.from_numpy(W.w).cuda()
+    phi, r = L.ltv_scan_system_response_tube(A, w, two_norm=True)
+    phi1, r1 = L.ltv_scan_system_response_tube(A, w)
+    torch.cuda.synchronize()
+    assert torch.equal(phi, phi1)
+    ref = O.tube_row2norm(W.A, W.w)
+    assert O.rel_err(r.cpu().numpy(), ref) <= TOL
+    assert O.rel_err(r1.cpu().numpy(), O.tube(W.A, W.w)) <= TOL
+    assert O.rel_err(r.cpu().numpy(), O.tube(W.A, W.w)) > 10 * TOL      # and it is not the box tube
+
+
+@pytest.mark.parametrize("n,T,batch", [(164, 6, 2), (128, 3, 3), (420, 4, 1)])
+def test_row_two_norm_tube_dense(L, n, T, batch):
+    import torch
+
+    W = dense_random(batch, T, n, 1, seed=11 * n + T, scale=0.4)
+    phi, r = L.ltv_scan_system_response_tube(torch.from_numpy(W.A).cuda(), torch.from_numpy(W.w).cuda(), two_norm=True)
+    torch.cuda.synchronize()
+    assert O.rel_err(r.cpu().numpy(), O.tube_row2norm(W.A, W.w)) <= TOL
