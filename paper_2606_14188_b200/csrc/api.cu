@@ -155,7 +155,7 @@ size_t ltv_scan_workspace_bytes(int op, int batch, int T, int n, int m) {
     case LTV_OP_ADJOINT:
       return 0;
     case LTV_OP_SYSTEM_RESPONSE_TUBE:
-      return phi_workspace_bytes(batch, T, n);
+      return phi_workspace_bytes(batch, T, n, n);
     case LTV_OP_PIPELINE_HOST:
     case LTV_OP_PIPELINE_HOST_NO_PHI: {
       const bool with_phi = op == LTV_OP_PIPELINE_HOST;
@@ -176,7 +176,7 @@ size_t ltv_scan_workspace_bytes(int op, int batch, int T, int n, int m) {
       add(b * t * nn);       // lambda
       add(b * t * mm);       // grad_u
       add(b * nn);           // grad_x0
-      if (with_phi) tot += phi_workspace_bytes(batch, T, n);
+      if (with_phi) tot += phi_workspace_bytes(batch, T, n, n);
       return tot;
     }
     default:
@@ -243,13 +243,13 @@ int ltv_scan_system_response_tube(const float* A, const float* w, float* phi_out
   if (phi_layout != LTV_PHI_COLUMN_PACKED || (flags & ~static_cast<unsigned>(LTV_TUBE_ROW_2NORM)) != 0) return LTV_ERR_BAD_DIM;
   if (misaligned(A) || misaligned(w) || misaligned(phi_out) || misaligned(r_out) || misaligned(workspace))
     return LTV_ERR_ALIGNMENT;
-  const size_t need = phi_workspace_bytes(batch, T, n);
+  const size_t need = phi_workspace_bytes(batch, T, n, n);
   if (!workspace) return LTV_ERR_NULL_PTR;
   if (workspace_bytes < need) return LTV_ERR_WORKSPACE_TOO_SMALL;
   int sms = 0;
   st = check_device(&sms);
   if (st != LTV_OK) return st;
-  PhiArgs a{A, w, phi_out, r_out, static_cast<float*>(workspace), batch, T, n, (flags & LTV_TUBE_ROW_2NORM) ? 1 : 0};
+  PhiArgs a{A, w, phi_out, r_out, static_cast<float*>(workspace), batch, T, n, n, (flags & LTV_TUBE_ROW_2NORM) ? 1 : 0};
   unsigned long long l = 0;
   cudaError_t e = launch_phi_tube(a, static_cast<cudaStream_t>(cuda_stream), &l);
   g_launches += l;
@@ -292,7 +292,7 @@ int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float
   float* dgu = carve(b * t * mm);
   float* dgx = carve(b * nn);
   void* phi_ws = cur;
-  const size_t phi_ws_bytes = with_phi ? phi_workspace_bytes(batch, T, n) : 0;
+  const size_t phi_ws_bytes = with_phi ? phi_workspace_bytes(batch, T, n, n) : 0;
   if (phi_device_out) *phi_device_out = with_phi ? dphi : nullptr;
 
   cudaError_t e;

@@ -29,12 +29,13 @@ struct PhiArgs {
   float *phi, *r;
   float* part;  // workspace: [batch, P, NT, n] per-(block, n-tile) tube partial sums
   int batch, T, n;
+  int nc;         // columns per Phi block = its row stride: n, or n + roundup4(p) when the observer's PhiY rides along
   int tube_mode;  // 0: sum_j |Phi_ij| w_j (box tube); 1: sqrt(sum_j (Phi_ij w_j)^2) per block (row-wise two-norm, eq.(12e))
 };
 // n-tile width the Phi path uses for this n (decides the size of `part`) and whether it is the tcgen05 path
-int phi_tile_n(int n);
+int phi_tile_n(int n, int nc);
 bool phi_uses_tensor_cores(int n);
-size_t phi_workspace_bytes(int batch, int T, int n);
+size_t phi_workspace_bytes(int batch, int T, int n, int nc);
 cudaError_t launch_phi_tube(const PhiArgs& a, cudaStream_t stream, unsigned long long* launches);
 
 // Cluster size (CTAs per item, 1..16, any integer) for the two vector kernels.  max_active[C] = clusters of C CTAs

@@ -28,11 +28,11 @@ static int pick_nch(int n) {
   return best;
 }
 
-int phi_tile_n(int n) { return phi_uses_tensor_cores(n) ? 32 * pick_nch(n) : 64; }
+int phi_tile_n(int n, int nc) { return phi_uses_tensor_cores(n) ? 32 * pick_nch(nc) : 64; }
 
-size_t phi_workspace_bytes(int batch, int T, int n) {
-  const int tn = phi_tile_n(n);
-  const size_t NT = (n + tn - 1) / tn;
+size_t phi_workspace_bytes(int batch, int T, int n, int nc) {
+  const int tn = phi_tile_n(n, nc);
+  const size_t NT = (nc + tn - 1) / tn;
   const size_t P = static_cast<size_t>(T) * (T - 1) / 2;
   size_t bytes = static_cast<size_t>(batch) * P * NT * n * sizeof(float);
   if (bytes == 0) bytes = 16;
@@ -43,8 +43,8 @@ cudaError_t launch_phi_tube(const PhiArgs& a, cudaStream_t stream, unsigned long
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  const int tn = phi_tile_n(a.n);
-  const int NT = (a.n + tn - 1) / tn;
+  const int tn = phi_tile_n(a.n, a.nc);
+  const int NT = (a.nc + tn - 1) / tn;
   cudaError_t e;
   const int NS = a.T - 1;
   if (NS >= 1) {

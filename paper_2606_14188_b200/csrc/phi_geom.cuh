@@ -20,6 +20,7 @@ __host__ __device__ inline long long phi_colbase(int T, int s) {
 
 struct PhiGeom {
   int batch, T, n, P;
+  int nc;            // columns per block = row stride of Phi (n, or n + padded p with the observer's PhiY columns)
   int level, S, H;   // segment length, half length (= number of s per segment)
   int nseg;          // segments at this level
   int tm, tn;        // tile sizes
@@ -29,14 +30,14 @@ struct PhiGeom {
   long long total;
 };
 
-__host__ __device__ inline PhiGeom phi_geom(int batch, int T, int n, int level, int tm, int tn) {
+__host__ __device__ inline PhiGeom phi_geom(int batch, int T, int n, int nc, int level, int tm, int tn) {
   PhiGeom g;
-  g.batch = batch; g.T = T; g.n = n; g.P = T * (T - 1) / 2;
+  g.batch = batch; g.T = T; g.n = n; g.nc = nc; g.P = T * (T - 1) / 2;
   g.level = level; g.S = 1 << level; g.H = g.S >> 1;
   const int NS = T - 1;
   g.nseg = (NS > g.H) ? (NS - g.H + g.S - 1) / g.S : 0;
   g.tm = tm; g.tn = tn;
-  g.NT = (n + tn - 1) / tn;
+  g.NT = (nc + tn - 1) / tn;
   g.MtF = (g.H * n + tm - 1) / tm;
   int cntL = 0;
   if (g.nseg > 0) {

@@ -88,14 +88,14 @@ __global__ void __launch_bounds__(256) phi_combine_simt_kernel(float* phi, const
   __shared__ float Bs[kSK][kST + 4];  // [k][j]
   __shared__ float ws[kST];
   __shared__ float tube[kST][17];
-  const int n = g.n;
+  const int n = g.n, nc = g.nc;   // K extent / rows per block; columns per block = row stride
   const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
   for (long long idx = blockIdx.x; idx < g.total; idx += gridDim.x) {
     const PhiTile t = phi_decode(g, idx);
     const size_t item = static_cast<size_t>(t.b) * g.P;
-    const float* Aop = phi + (item + phi_colbase(g.T, t.mid)) * n * n;                       // rows (t,i)
-    const float* Bop = phi + (item + phi_colbase(g.T, t.s) + (t.mid - t.s - 1)) * n * n;    // Phi(mid,s)
-    float* Out = phi + (item + phi_colbase(g.T, t.s) + (t.mid - t.s)) * n * n;             // rows (t,i), col s
+    const float* Aop = phi + (item + phi_colbase(g.T, t.mid)) * n * nc;                       // rows (t,i)
+    const float* Bop = phi + (item + phi_colbase(g.T, t.s) + (t.mid - t.s - 1)) * n * nc;    // Phi(mid,s)
+    float* Out = phi + (item + phi_colbase(g.T, t.s) + (t.mid - t.s)) * n * nc;             // rows (t,i), col s
     const int Mrows = t.cnt_t * n;
     const int m0 = t.m_tile * kST, j0 = t.n_tile * kST;
     if (threadIdx.x < kST) {
@@ -107,12 +107,12 @@ __global__ void __launch_bounds__(256) phi_combine_simt_kernel(float* phi, const
       for (int e = threadIdx.x; e < kST * kSK; e += 256) {
         const int kk = e % kSK, mm = e / kSK;
         const int r = m0 + mm, k = k0 + kk;
-        As[kk][mm] = (r < Mrows && k < n) ? Aop[static_cast<size_t>(r) * n + k] : 0.f;
+        As[kk][mm] = (r < Mrows && k < n) ? Aop[static_cast<size_t>(r) * nc + k] : 0.f;
       }
       for (int e = threadIdx.x; e < kST * kSK; e += 256) {
         const int jj = e % kST, kk = e / kST;
         const int j = j0 + jj, k = k0 + kk;
-        Bs[kk][jj] = (j < n && k < n) ? Bop[static_cast<size_t>(k) * n + j] : 0.f;
+        Bs[kk][jj] = (j < nc && k < n) ? Bop[static_cast<size_t>(k) * nc + j] : 0.f;
       }
       __syncthreads();
 #pragma unroll
@@ -137,7 +137,7 @@ __global__ void __launch_bounds__(256) phi_combine_simt_kernel(float* phi, const
       for (int c = 0; c < 4; ++c) {
         const int j = j0 + tx * 4 + c;
         tb += tube_term(acc[r][c], ws[tx * 4 + c], mode);
-        if (row < Mrows && j < n) Out[static_cast<size_t>(row) * n + j] = acc[r][c];
+        if (row < Mrows && j < nc) Out[static_cast<size_t>(row) * nc + j] = acc[r][c];
       }
       tube[ty * 4 + r][tx] = tb;
     }
@@ -187,7 +187,7 @@ cudaError_t launch_phi_level0(const PhiArgs& a, int NT, int num_sms, cudaStream_
 }
 
 cudaError_t launch_phi_combine_simt(const PhiArgs& a, int level, int num_sms, cudaStream_t stream) {
-  const PhiGeom g = phi_geom(a.batch, a.T, a.n, level, kST, kST);
+  const PhiGeom g = phi_geom(a.batch, a.T, a.n, a.nc, level, kST, kST);
   if (g.total == 0) return cudaSuccess;
   long long blocks = g.total;
   const long long cap = static_cast<long long>(num_sms) * 8;

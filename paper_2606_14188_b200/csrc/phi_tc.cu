@@ -106,7 +106,8 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const uint32_t rank = PAIR ? cluster_ctarank() : 0u;
   const PhiGeom& g = p.g;   // decoded with tm = 128 NCTA
-  const int n = g.n;
+  const int n = g.n;     // K extent and rows per block
+  const int nc = g.nc;   // columns per block = row stride of Phi (n, or n + padded p: the observer's PhiY columns)
   const int R = p.stages;
   const int nkb = (n + kKB - 1) / kKB;
   const int ks_last = ((n - (nkb - 1) * kKB) + 7) / 8;  // k-steps of the last k-block that hold data
@@ -319,7 +320,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
       const int rbase = t.m_tile * (kTM * NCTA) + static_cast<int>(rank) * kTM + wq * 32;
       const int rho = rbase + lane;
       const int rows_valid = t.cnt_t * n - rbase;   // rows of this warp's 32 that exist (may be <= 0 or >= 32)
-      float* out = p.phi + (qcol * n + rbase) * n + j0;
+      float* out = p.phi + (qcol * n + rbase) * nc + j0;
       const int row0 = static_cast<int>(qcol * n) + rbase;
       mbar_wait(&tfull[acc], (lt >> 1) & 1);
       tc_fence_after();
@@ -348,7 +349,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
         }
         if (DBG & 1) continue;
         const int jc = j0 + cc * 32;
-        if (jc >= n || rows_valid <= 0) continue;
+        if (jc >= nc || rows_valid <= 0) continue;
         if (rows_valid >= 32) {
           // all 32 rows exist: swizzled shared-memory box + bulk tensor store (coalesced, off the LSU; columns
           // beyond n are clipped by the tensor map)
@@ -368,8 +369,8 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
           // ragged last m-tile of a stacked column: masked row-per-thread stores
 #pragma unroll
           for (int e = 0; e < 8; ++e) {
-            if (jc + 4 * e < n)
-              st_global_f4_na(out + static_cast<size_t>(lane) * n + cc * 32 + 4 * e,
+            if (jc + 4 * e < nc)
+              st_global_f4_na(out + static_cast<size_t>(lane) * nc + cc * 32 + 4 * e,
                               make_float4(__uint_as_float(vc[4 * e]), __uint_as_float(vc[4 * e + 1]),
                                           __uint_as_float(vc[4 * e + 2]), __uint_as_float(vc[4 * e + 3])));
           }
@@ -462,11 +463,11 @@ cudaError_t phi_tc_make_maps(const PhiArgs& a, int nch, void* maps_out) {
   if (!enc) return cudaErrorNotSupported;
   TcMaps* m = static_cast<TcMaps*>(maps_out);
   const cuuint64_t P = static_cast<cuuint64_t>(a.T) * (a.T - 1) / 2;
-  const cuuint64_t n = a.n;
+  const cuuint64_t n = a.n, nc = a.nc;   // rows (= K) and columns (= row stride) of a block
   const cuuint32_t estr[3] = {1, 1, 1};
   {
     const cuuint64_t dims[2] = {n, static_cast<cuuint64_t>(a.batch) * P * n};
-    const cuuint64_t strides[1] = {n * 4};
+    const cuuint64_t strides[1] = {nc * 4};
     const cuuint32_t box[2] = {kKB, kTM};
     if (enc(&m->L, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, a.phi, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -474,8 +475,8 @@ cudaError_t phi_tc_make_maps(const PhiArgs& a, int nch, void* maps_out) {
       return cudaErrorInvalidValue;
   }
   {
-    const cuuint64_t dims[3] = {n, n, static_cast<cuuint64_t>(a.batch) * P};
-    const cuuint64_t strides[2] = {n * 4, n * n * 4};
+    const cuuint64_t dims[3] = {nc, n, static_cast<cuuint64_t>(a.batch) * P};
+    const cuuint64_t strides[2] = {nc * 4, n * nc * 4};
     const cuuint32_t box[3] = {32, kKB, 1};
     if (enc(&m->R, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, a.phi, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
@@ -483,8 +484,8 @@ cudaError_t phi_tc_make_maps(const PhiArgs& a, int nch, void* maps_out) {
       return cudaErrorInvalidValue;
   }
   {
-    const cuuint64_t dims[2] = {n, static_cast<cuuint64_t>(a.batch) * P * n};
-    const cuuint64_t strides[1] = {n * 4};
+    const cuuint64_t dims[2] = {nc, static_cast<cuuint64_t>(a.batch) * P * n};
+    const cuuint64_t strides[1] = {nc * 4};
     const cuuint32_t box[2] = {32, 32};
     if (enc(&m->O, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, a.phi, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
             CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
@@ -507,8 +508,8 @@ cudaError_t launch_phi_combine_tc(const PhiArgs& a, int level, int nch, const vo
   const TcMaps& m = *static_cast<const TcMaps*>(maps);
   // CTA pairs (256-row tiles) when the level's stacked left operand is tall enough to fill them; the
   // single-CTA kernel (128-row tiles) on the low levels where 256-row tiles would be mostly padding
-  const PhiGeom g1 = phi_geom(a.batch, a.T, a.n, level, kTM, 32 * nch);
-  const PhiGeom g2 = phi_geom(a.batch, a.T, a.n, level, 2 * kTM, 32 * nch);
+  const PhiGeom g1 = phi_geom(a.batch, a.T, a.n, a.nc, level, kTM, 32 * nch);
+  const PhiGeom g2 = phi_geom(a.batch, a.T, a.n, a.nc, level, 2 * kTM, 32 * nch);
   if (g1.total == 0) return cudaSuccess;
   const int mode = env_int("TC_PAIR", -1);   // -1 auto, 0 never, 1 always
   const bool pair = (mode == 1) || (mode == -1 && 2 * g2.total * 100 <= g1.total * 108);
