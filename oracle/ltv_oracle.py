@@ -24,6 +24,9 @@ sequential recursion - "We obtain the solution to (14) by a forward parallel ass
                                                                      (row-wise two-norm, :150), with the
                                                                      stand-in E_s = diag(w_s) (SURVEY 8f
                                                                      NEXT-2; reading q3b)
+  observer_response  PhiX(k,k) = I; PhiX(k,j) = PhiX(k,j+1) (A_j + L_j^T C_j);     PAPER.md:157-160 eq.(14), read with
+                   PhiY(k,j) = PhiX(k,j) L_j^T,  0 <= j < k <= T-1                 k-independent gains L_j (:177; SURVEY
+                                                                     8f NEXT-1, reading q15)
   adjoint          lam_T = g_T; lam_t = A_t^T lam_{t+1} + g_t;       PAPER.md:106-110 eq.(10) chained
                    grad_u[t] = B_t^T lam_{t+1}; grad_x0 = A_0^T lam_1   over the horizon; north_star (iii)
 
@@ -101,6 +104,29 @@ def system_response_item(A):
 
 def system_response(A):
     return np.stack([system_response_item(A[b]) for b in range(A.shape[0])])
+
+
+def observer_response_item(A, Lt, C):
+    """Closed-loop observer propagation of one item, eq.(14) in the paper's own order: for every
+    k, PhiX(k,k) = I and, for j = k-1 down to 0, PhiX(k,j) = PhiX(k,j+1) (A_j + L_j^T C_j) (RIGHT multiplication),
+    PhiY(k,j) = PhiX(k,j) L_j^T.  Lt[j] = L_j^T [n,p], C[j] [p,n].  Returns packed PhiX[P,n,n], PhiY[P,n,p]."""
+    A, Lt, C = _f64(A), _f64(Lt), _f64(C)
+    T, n, _ = A.shape
+    p = Lt.shape[-1]
+    PhiX = np.empty((T * (T - 1) // 2, n, n))
+    PhiY = np.empty((T * (T - 1) // 2, n, p))
+    for k in range(1, T):
+        X = np.eye(n)
+        for j in range(k - 1, -1, -1):
+            X = X @ (A[j] + Lt[j] @ C[j])
+            PhiX[packed_index(k, j)] = X
+            PhiY[packed_index(k, j)] = X @ Lt[j]
+    return PhiX, PhiY
+
+
+def observer_response(A, Lt, C):
+    out = [observer_response_item(A[b], Lt[b], C[b]) for b in range(A.shape[0])]
+    return np.stack([o[0] for o in out]), np.stack([o[1] for o in out])
 
 
 def phi_block(A, t: int, s: int):

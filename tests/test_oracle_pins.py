@@ -284,6 +284,65 @@ def test_tube2_sandwiched_by_box_tube():
     np.testing.assert_allclose(O.tube_row2norm_item(A, 3.0 * w.astype(np.float64)), 3.0 * tau, rtol=1e-13)   # homogeneous in w
 
 
+# --------------------------------------------------------------------------- observer propagation (14), NEXT-1
+def _obs_inputs(T, n, p, seed):
+    rng = np.random.default_rng(seed)
+    A = np.eye(n)[None] + rng.normal(0.0, 0.4 / np.sqrt(n), (T, n, n))
+    return A, rng.normal(0.0, 0.3, (T, n, p)), rng.normal(0.0, 0.5, (T, p, n))
+
+
+def test_observer_zero_gain_and_scalar_closed_form():
+    A, Lt, C = _obs_inputs(6, 5, 2, 1)
+    X, Y = O.observer_response_item(A, 0.0 * Lt, C)
+    np.testing.assert_allclose(X, O.system_response_item(A), rtol=1e-12, atol=1e-14)   # L = 0: open loop
+    assert np.all(Y == 0.0)
+    T, n = 6, 3
+    a, l = np.linspace(0.5, 1.5, T), np.linspace(-0.4, 0.3, T)
+    I = np.eye(n)
+    X, Y = O.observer_response_item(a[:, None, None] * I, l[:, None, None] * I, np.broadcast_to(I, (T, n, n)))
+    for k in range(1, T):
+        for j in range(k):
+            pr = np.prod(a[j:k] + l[j:k])
+            np.testing.assert_allclose(X[O.packed_index(k, j)], pr * I, rtol=1e-13)
+            np.testing.assert_allclose(Y[O.packed_index(k, j)], pr * l[j] * I, rtol=1e-13)
+
+
+def test_observer_bruteforce_left_products_and_inverse_identity():
+    """PhiX(k,j) = Abar_{k-1} ... Abar_j by explicit LEFT products (the oracle multiplies on the right), and the
+    strictly-lower blocks of (I - Z blkdiag(Abar))^{-1} (the identity (12c) has for the closed loop)."""
+    T, n, p = 5, 4, 2
+    A, Lt, C = _obs_inputs(T, n, p, 2)
+    X, Y = O.observer_response_item(A, Lt, C)
+    Abar = [A[j] + Lt[j] @ C[j] for j in range(T)]
+    M = np.eye(T * n)
+    for j in range(T - 1):
+        M[(j + 1) * n:(j + 2) * n, j * n:(j + 1) * n] = -Abar[j]
+    Minv = np.linalg.inv(M)
+    for k in range(1, T):
+        for j in range(k):
+            P = np.eye(n)
+            for i in range(j, k):
+                P = Abar[i] @ P
+            np.testing.assert_allclose(X[O.packed_index(k, j)], P, rtol=1e-12, atol=1e-14)
+            np.testing.assert_allclose(X[O.packed_index(k, j)], Minv[k * n:(k + 1) * n, j * n:(j + 1) * n], rtol=1e-10, atol=1e-12)
+            np.testing.assert_allclose(Y[O.packed_index(k, j)], P @ Lt[j], rtol=1e-12, atol=1e-14)
+
+
+def test_observer_semigroup_is_what_the_scan_uses():
+    """[PhiX | PhiY](t,s) = PhiX(t,k) [PhiX | PhiY](k,s) for every s < k < t: the combine of the time-parallel scan."""
+    T, n, p = 7, 3, 2
+    A, Lt, C = _obs_inputs(T, n, p, 3)
+    X, Y = O.observer_response_item(A, Lt, C)
+    q = O.packed_index
+    for t in range(2, T):
+        for s in range(t - 1):
+            for k in range(s + 1, t):
+                np.testing.assert_allclose(X[q(t, s)], X[q(t, k)] @ X[q(k, s)], rtol=1e-11, atol=1e-13)
+                np.testing.assert_allclose(Y[q(t, s)], X[q(t, k)] @ Y[q(k, s)], rtol=1e-11, atol=1e-13)
+    Xb, Yb = O.observer_response(A[None], Lt[None], C[None])
+    assert np.array_equal(Xb[0], X) and np.array_equal(Yb[0], Y)
+
+
 def test_rollout_identity_A_is_cumsum():
     T, n, m = 6, 4, 2
     _, B, c, x0, u, _, _ = _rand(T, n, m, seed=12)
