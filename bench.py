@@ -38,6 +38,8 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (0..4)")
     ap.add_argument("--batch", type=int, default=0, help="items per GPU (0 = the config's own; config 4 sweeps 64/256/1024)")
+    ap.add_argument("--observer", type=int, default=0, metavar="P",
+                    help="also time ltv_scan_observer_response (NEXT-1, eq.(14)) with P measurement rows")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-items", type=int, default=0, help="items in the CPU-oracle sample (0 = auto)")
@@ -288,11 +290,41 @@ def main():
             extra[k] = dict(per_s=batch * world / (ms * 1e-3), ms=ms, hbm_gbs=bytes_roll / (ms * 1e-3) / 1e9,
                             hbm_frac=bytes_roll / (ms * 1e-3) / 1e9 / pk["hbm_gbs"])
 
+    # ---- NEXT-1: closed-loop observer propagation on the same A (random gains), timed alone
+    observer = None
+    if phi_on and args.observer > 0:
+        pobs = args.observer
+        gen = torch.Generator(device=dev).manual_seed(1234)
+        Lt = torch.randn((batch, T, n, pobs), device=dev, generator=gen) * (0.05 / pobs ** 0.5)
+        Cm = torch.randn((batch, T, pobs, n), device=dev, generator=gen) / n ** 0.5
+        del phi
+        torch.cuda.empty_cache()
+        nc = L.ltv_observer_row_floats(n, pobs)
+        phio = torch.empty((batch, P, n, nc), device=dev)
+        wso = torch.empty(max(16, L.ltv_scan_workspace_bytes(L.LTV_OP_OBSERVER_RESPONSE, batch, T, n, pobs)),
+                          dtype=torch.uint8, device=dev)
+        for _ in range(3):
+            L.ltv_scan_observer_response(d["A"], Lt, Cm, d["w"], phi_out=phio, r_out=r, workspace=wso)
+        o0, o1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        o0.record()
+        for _ in range(args.steps):
+            L.ltv_scan_observer_response(d["A"], Lt, Cm, d["w"], phi_out=phio, r_out=r, workspace=wso)
+        o1.record()
+        barrier()
+        oms = o0.elapsed_time(o1) / args.steps
+        observer = dict(p=pobs, ms=oms, blocks_per_s=batch * world * P / (oms * 1e-3),
+                        issued_tf32_tflops=3.0 * 2.0 * n * n * nc * ((T - 1) * (T - 2) // 2) * batch / (oms * 1e-3) / 1e12,
+                        note="ltv_scan_observer_response alone: [PhiX | PhiY] blocks of n x (n + roundup4(p)) floats")
+        del phio, wso
+        phi = None
+
     # ---- end to end through the C-ABI with host buffers
     e2e = None
     if not args.no_e2e:
         if phi_on:
-            del phi, ws
+            phi = None
+            del ws
         torch.cuda.empty_cache()
         need = L.ltv_scan_workspace_bytes(L.LTV_OP_PIPELINE_HOST if phi_on else L.LTV_OP_PIPELINE_HOST_NO_PHI, batch, T, n, m)
         wsh = torch.empty(need, dtype=torch.uint8, device=dev)
@@ -343,7 +375,7 @@ def main():
                                     f"working set (A {a_gb * 1e3:.2f} MB) fits L2: warm-cache, latency-bound case"),
                                 phi_layout="column-packed"),
                     clocks=sampler.result(), e2e=e2e, gpu_launches=int(launches), roofline=roof,
-                    cpu_baseline=cpu, kernel_ms_per_step=share, vector_scans=extra,
+                    cpu_baseline=cpu, kernel_ms_per_step=share, vector_scans=extra, observer=observer,
                     rollouts_per_s=extra.get("rollout", {}).get("per_s"),
                     adjoints_per_s=extra.get("adjoint", {}).get("per_s"))
         print(json.dumps(line), flush=True)

@@ -60,7 +60,8 @@ typedef enum {
 
 /* `op` argument of ltv_scan_workspace_bytes */
 enum { LTV_OP_ROLLOUT = 0, LTV_OP_SYSTEM_RESPONSE_TUBE = 1, LTV_OP_ADJOINT = 2, LTV_OP_PIPELINE_HOST = 3,
-       LTV_OP_PIPELINE_HOST_NO_PHI = 4 /* ltv_scan_pipeline_host with w_host == NULL: rollout + adjoint only */ };
+       LTV_OP_PIPELINE_HOST_NO_PHI = 4 /* ltv_scan_pipeline_host with w_host == NULL: rollout + adjoint only */,
+       LTV_OP_OBSERVER_RESPONSE = 5 /* ltv_scan_observer_response; pass p (rows of C) as `m` */ };
 
 /* `phi_layout` argument.  COLUMN_PACKED (the only layout of this version): the P = T(T-1)/2 blocks of one
  * item are stored column by column of the block-lower-triangular operator; block (t,s), 0 <= s < t <= T-1,
@@ -123,6 +124,25 @@ LTV_API int ltv_scan_adjoint(const float* A, const float* B, const float* g,
                      float* lambda_out, float* grad_u_out, float* grad_x0_out,
                      int batch, int T, int n, int m,
                      void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Closed-loop observer propagation (eq.(14), :177), with gains that do not
+ * depend on the injection step k (reading q15):
+ *     Abar_j = A_j + Lt_j C_j,   PhiX(t,s) = Abar_{t-1} ... Abar_s,   PhiY(t,s) = PhiX(t,s) Lt_s,   0 <= s < t <= T-1
+ *   A        device [batch,T,n,n]     required; A_0 .. A_{T-2} are read
+ *   Lt       device [batch,T,n,p]     required; Lt_j = L_j^T (the transposed Kalman gain of (13)), 1 <= p <= 32
+ *   C        device [batch,T,p,n]     required; observation Jacobians
+ *   w        device [batch,T,n]       required; tube of PhiX exactly as in ltv_scan_system_response_tube
+ *   phi_out  device [batch,P,n,nc]    nc = ltv_observer_row_floats(n,p) = n + 4*ceil(p/4); in every row, columns
+ *                                     [0,n) hold PhiX(t,s), [n,n+p) PhiY(t,s), the rest zeros; block order `phi_layout`
+ *   r_out    device [batch,T,n]       r_t = sum_{s<t} |PhiX(t,s)| w_s  (or the two-norm form with LTV_TUBE_ROW_2NORM)
+ * The same time-parallel scan as above runs over the closed-loop matrices; PhiY rides along as p extra columns of
+ * the right operand ([PhiX | PhiY](t,s) = PhiX(t,mid) [PhiX | PhiY](mid,s)), so it costs (n+p)/n of the products and
+ * no second pass over Phi.  Level 0 forms Abar_s while A_s streams through, and PhiY(s+1,s) = Abar_s Lt_s.
+ * Workspace: ltv_scan_workspace_bytes(LTV_OP_OBSERVER_RESPONSE, batch, T, n, p). */
+LTV_API int ltv_observer_row_floats(int n, int p);
+LTV_API int ltv_scan_observer_response(const float* A, const float* Lt, const float* C, const float* w,
+                                       float* phi_out, float* r_out, int batch, int T, int n, int p, int phi_layout,
+                                       unsigned flags, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* One pass of the whole hot path from HOST buffers: copies A, B, c, x0, u, w, g host->device into
  * `workspace` (device, >= ltv_scan_workspace_bytes(LTV_OP_PIPELINE_HOST, ...)), runs the three calls above

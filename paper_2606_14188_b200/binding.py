@@ -18,13 +18,15 @@ STATUS_NAMES = {
 }
 LTV_OP_ROLLOUT, LTV_OP_SYSTEM_RESPONSE_TUBE, LTV_OP_ADJOINT, LTV_OP_PIPELINE_HOST = 0, 1, 2, 3
 LTV_OP_PIPELINE_HOST_NO_PHI = 4
+LTV_OP_OBSERVER_RESPONSE = 5
 LTV_TUBE_ROW_2NORM = 1
 LTV_PHI_COLUMN_PACKED = 0
 
 EXPORTS = (
     "ltv_phi_block_index", "ltv_scan_workspace_bytes", "ltv_scan_rollout", "ltv_scan_system_response_tube",
     "ltv_scan_adjoint", "ltv_scan_pipeline_host", "ltv_status_string", "ltv_last_cuda_error", "ltv_version",
-    "ltv_launch_count", "ltv_profile_enable", "ltv_profile_collect",
+    "ltv_launch_count", "ltv_profile_enable", "ltv_profile_collect", "ltv_scan_observer_response",
+    "ltv_observer_row_floats",
 )
 
 
@@ -53,6 +55,10 @@ def _load() -> ctypes.CDLL:
     L.ltv_scan_adjoint.argtypes = [fp] * 6 + [i] * 4 + [vp, sz, vp]
     L.ltv_scan_pipeline_host.restype = i
     L.ltv_scan_pipeline_host.argtypes = [fp] * 13 + [i] * 4 + [vp, sz, vp, ctypes.POINTER(ctypes.c_void_p)]
+    L.ltv_scan_observer_response.restype = i
+    L.ltv_scan_observer_response.argtypes = [fp] * 6 + [i] * 5 + [ctypes.c_uint, vp, sz, vp]
+    L.ltv_observer_row_floats.restype = i
+    L.ltv_observer_row_floats.argtypes = [i, i]
     L.ltv_status_string.restype = ctypes.c_char_p
     L.ltv_status_string.argtypes = [i]
     L.ltv_last_cuda_error.restype = i
@@ -150,6 +156,35 @@ def ltv_scan_system_response_tube(A, w, phi_out=None, r_out=None, workspace=None
                                            _ptr(workspace), workspace.numel(), _stream())
     if st != LTV_OK:
         raise LtvError(st, "ltv_scan_system_response_tube")
+    return phi_out, r_out
+
+
+def ltv_observer_row_floats(n, p):
+    return int(lib.ltv_observer_row_floats(n, p))
+
+
+def ltv_scan_observer_response(A, Lt, C, w, phi_out=None, r_out=None, workspace=None, two_norm=False):
+    """Closed-loop observer propagation (eq.(14)): returns (phi[batch,P,n,nc] COLUMN_PACKED with PhiX in columns
+    [0,n) and PhiY in [n,n+p) of every row, r[batch,T,n]).  Lt[batch,T,n,p] = L_j^T, C[batch,T,p,n]."""
+    batch, T, n, _ = A.shape
+    p = Lt.shape[-1]
+    P = T * (T - 1) // 2
+    nc = ltv_observer_row_floats(n, p)
+    _dev(A, "A", (batch, T, n, n)); _dev(Lt, "Lt", (batch, T, n, p)); _dev(C, "C", (batch, T, p, n))
+    _dev(w, "w", (batch, T, n))
+    if phi_out is None:
+        phi_out = torch.empty((batch, P, n, nc), device=A.device, dtype=torch.float32)
+    if r_out is None:
+        r_out = torch.empty((batch, T, n), device=A.device, dtype=torch.float32)
+    _dev(phi_out, "phi_out", (batch, P, n, nc)); _dev(r_out, "r_out", (batch, T, n))
+    need = ltv_scan_workspace_bytes(LTV_OP_OBSERVER_RESPONSE, batch, T, n, p)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), device=A.device, dtype=torch.uint8)
+    st = lib.ltv_scan_observer_response(_ptr(A), _ptr(Lt), _ptr(C), _ptr(w), _ptr(phi_out), _ptr(r_out), batch, T, n, p,
+                                        LTV_PHI_COLUMN_PACKED, LTV_TUBE_ROW_2NORM if two_norm else 0,
+                                        _ptr(workspace), workspace.numel(), _stream())
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_observer_response")
     return phi_out, r_out
 
 

@@ -156,6 +156,9 @@ size_t ltv_scan_workspace_bytes(int op, int batch, int T, int n, int m) {
       return 0;
     case LTV_OP_SYSTEM_RESPONSE_TUBE:
       return phi_workspace_bytes(batch, T, n, n);
+    case LTV_OP_OBSERVER_RESPONSE:
+      if (m < 1 || m > 32) return 0;
+      return phi_workspace_bytes(batch, T, n, n + ((m + 3) & ~3));
     case LTV_OP_PIPELINE_HOST:
     case LTV_OP_PIPELINE_HOST_NO_PHI: {
       const bool with_phi = op == LTV_OP_PIPELINE_HOST;
@@ -250,6 +253,39 @@ int ltv_scan_system_response_tube(const float* A, const float* w, float* phi_out
   st = check_device(&sms);
   if (st != LTV_OK) return st;
   PhiArgs a{A, w, phi_out, r_out, static_cast<float*>(workspace), batch, T, n, n, (flags & LTV_TUBE_ROW_2NORM) ? 1 : 0};
+  unsigned long long l = 0;
+  cudaError_t e = launch_phi_tube(a, static_cast<cudaStream_t>(cuda_stream), &l);
+  g_launches += l;
+  return e == cudaSuccess ? LTV_OK : fail_cuda(e);
+}
+
+int ltv_observer_row_floats(int n, int p) { return (n < 1 || p < 1) ? 0 : n + ((p + 3) & ~3); }
+
+int ltv_scan_observer_response(const float* A, const float* Lt, const float* C, const float* w, float* phi_out,
+                               float* r_out, int batch, int T, int n, int p, int phi_layout, unsigned flags,
+                               void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!A || !Lt || !C || !w || !r_out) return LTV_ERR_NULL_PTR;
+  if (T > 1 && !phi_out) return LTV_ERR_NULL_PTR;
+  int st = check_dims(batch, T, n, 0);
+  if (st != LTV_OK) return st;
+  if (p < 1) return LTV_ERR_BAD_DIM;
+  if (p > 32) return LTV_ERR_UNSUPPORTED_SHAPE;
+  if (phi_layout != LTV_PHI_COLUMN_PACKED || (flags & ~static_cast<unsigned>(LTV_TUBE_ROW_2NORM)) != 0) return LTV_ERR_BAD_DIM;
+  const int nc = n + ((p + 3) & ~3);
+  if (static_cast<long long>(batch) * T * (T - 1) / 2 * n * nc >= (1ll << 40)) return LTV_ERR_UNSUPPORTED_SHAPE;
+  if (misaligned(A) || misaligned(Lt) || misaligned(C) || misaligned(w) || misaligned(phi_out) || misaligned(r_out) ||
+      misaligned(workspace))
+    return LTV_ERR_ALIGNMENT;
+  const size_t need = phi_workspace_bytes(batch, T, n, nc);
+  if (!workspace) return LTV_ERR_NULL_PTR;
+  if (workspace_bytes < need) return LTV_ERR_WORKSPACE_TOO_SMALL;
+  int sms = 0;
+  st = check_device(&sms);
+  if (st != LTV_OK) return st;
+  PhiArgs a{A, w, phi_out, r_out, static_cast<float*>(workspace), batch, T, n, nc, (flags & LTV_TUBE_ROW_2NORM) ? 1 : 0};
+  a.Lt = Lt;
+  a.C = C;
+  a.p = p;
   unsigned long long l = 0;
   cudaError_t e = launch_phi_tube(a, static_cast<cudaStream_t>(cuda_stream), &l);
   g_launches += l;

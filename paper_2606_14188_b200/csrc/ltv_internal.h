@@ -31,6 +31,10 @@ struct PhiArgs {
   int batch, T, n;
   int nc;         // columns per Phi block = its row stride: n, or n + roundup4(p) when the observer's PhiY rides along
   int tube_mode;  // 0: sum_j |Phi_ij| w_j (box tube); 1: sqrt(sum_j (Phi_ij w_j)^2) per block (row-wise two-norm, eq.(12e))
+  // closed-loop observer propagation (eq.(14)): level 0 forms Abar_s = A_s + Lt_s C_s and PhiY(s+1,s) = Abar_s Lt_s
+  const float* Lt = nullptr;  // [batch,T,n,p] = L_j^T, or nullptr: plain system response
+  const float* C = nullptr;   // [batch,T,p,n]
+  int p = 0;
 };
 // n-tile width the Phi path uses for this n (decides the size of `part`) and whether it is the tcgen05 path
 int phi_tile_n(int n, int nc);

@@ -48,9 +48,9 @@ cudaError_t launch_phi_tube(const PhiArgs& a, cudaStream_t stream, unsigned long
   cudaError_t e;
   const int NS = a.T - 1;
   if (NS >= 1) {
-    e = launch_phi_level0(a, NT, sms, stream);
+    e = a.Lt ? launch_phi_obs_level0(a, NT, sms, stream) : launch_phi_level0(a, NT, sms, stream);
     if (e != cudaSuccess) return e;
-    ++*launches;
+    *launches += (a.Lt && a.p > 8) ? 2 : 1;   // the observer's level 0 is two kernels beyond the fused p <= 8 path
     const bool tc = phi_uses_tensor_cores(a.n);
     alignas(64) unsigned char maps[512];
     if (tc && NS >= 2) {

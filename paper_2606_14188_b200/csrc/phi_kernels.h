@@ -5,6 +5,8 @@
 namespace ltv {
 
 cudaError_t launch_phi_level0(const PhiArgs& a, int NT, int num_sms, cudaStream_t stream);
+// observer variant (a.Lt != nullptr): two launches, Abar_s with the tube partial, then PhiY(s+1,s) = Abar_s Lt_s
+cudaError_t launch_phi_obs_level0(const PhiArgs& a, int NT, int num_sms, cudaStream_t stream);
 cudaError_t launch_phi_combine_simt(const PhiArgs& a, int level, int num_sms, cudaStream_t stream);
 cudaError_t launch_phi_finalize(const PhiArgs& a, int NT, cudaStream_t stream);
 

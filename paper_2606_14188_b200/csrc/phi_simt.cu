@@ -79,6 +79,84 @@ __global__ void __launch_bounds__(256) phi_level0_kernel(const float* __restrict
   }
 }
 
+// ------------------------------------------------------------------------------------------ observer level 0
+// Closed-loop observer propagation, eq.(14): the level-0 blocks are
+//   PhiX(s+1,s) = Abar_s = A_s + Lt_s C_s   (rank-p update while A_s streams through: HBM-bound like the copy)
+//   PhiY(s+1,s) = Abar_s Lt_s               (skinny product, second kernel; Abar_s is still in L2)
+// written side by side in rows of nc = n + roundup4(p) floats; the tube partial is taken over PhiX.
+__global__ void __launch_bounds__(256) phi_obs_level0_kernel(const float* __restrict__ A, const float* __restrict__ Lt,
+                                                             const float* __restrict__ C, const float* __restrict__ w,
+                                                             float* __restrict__ phi, float* __restrict__ part, int batch,
+                                                             int T, int n, int nc, int p, int NT, int mode) {
+  const int P = T * (T - 1) / 2;
+  const long long nrows = static_cast<long long>(batch) * (T - 1) * n;
+  const int lane = threadIdx.x & 31;
+  const int n4 = n >> 2;
+  for (long long row = static_cast<long long>(blockIdx.x) * 8 + (threadIdx.x >> 5); row < nrows;
+       row += static_cast<long long>(gridDim.x) * 8) {
+    const int i = static_cast<int>(row % n);
+    const long long bs = row / n;
+    const int s = static_cast<int>(bs % (T - 1));
+    const int b = static_cast<int>(bs / (T - 1));
+    const size_t bt = static_cast<size_t>(b) * T + s;
+    const float4* src = reinterpret_cast<const float4*>(A + (bt * n + i) * n);
+    const float4* wv = reinterpret_cast<const float4*>(w + bt * n);
+    const float* lrow = Lt + (bt * n + i) * p;
+    const float4* Cs = reinterpret_cast<const float4*>(C + bt * p * n);
+    const size_t q = static_cast<size_t>(b) * P + phi_colbase(T, s);
+    float* dst = phi + (q * n + i) * nc;
+    float acc = 0.f;
+    for (int c = lane; c < n4; c += 32) {
+      float4 a = __ldcs(src + c);
+      for (int k = 0; k < p; ++k) {
+        const float l = __ldg(lrow + k);
+        const float4 ck = __ldg(Cs + static_cast<size_t>(k) * n4 + c);
+        a.x = fmaf(l, ck.x, a.x); a.y = fmaf(l, ck.y, a.y); a.z = fmaf(l, ck.z, a.z); a.w = fmaf(l, ck.w, a.w);
+      }
+      const float4 ww = __ldg(wv + c);
+      *reinterpret_cast<float4*>(dst + 4 * c) = a;
+      acc += (tube_term(a.x, ww.x, mode) + tube_term(a.y, ww.y, mode)) + (tube_term(a.z, ww.z, mode) + tube_term(a.w, ww.w, mode));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    for (int e = lane; e < NT; e += 32) part[(q * NT + e) * n + i] = (e == 0) ? acc : 0.f;
+  }
+}
+
+// PhiY(s+1,s)[i][k] = sum_j Abar_s[i][j] Lt_s[j][k]; pad columns n+p .. nc-1 are zeroed.  One warp per row.
+__global__ void __launch_bounds__(256) phi_obs_y0_kernel(const float* __restrict__ Lt, float* __restrict__ phi, int batch,
+                                                         int T, int n, int nc, int p) {
+  const int P = T * (T - 1) / 2;
+  const long long nrows = static_cast<long long>(batch) * (T - 1) * n;
+  const int lane = threadIdx.x & 31;
+  for (long long row = static_cast<long long>(blockIdx.x) * 8 + (threadIdx.x >> 5); row < nrows;
+       row += static_cast<long long>(gridDim.x) * 8) {
+    const int i = static_cast<int>(row % n);
+    const long long bs = row / n;
+    const int s = static_cast<int>(bs % (T - 1));
+    const int b = static_cast<int>(bs / (T - 1));
+    const float* Ls = Lt + (static_cast<size_t>(b) * T + s) * n * p;
+    const size_t q = static_cast<size_t>(b) * P + phi_colbase(T, s);
+    float* prow = phi + (q * n + i) * nc;
+    for (int k0 = 0; k0 < p; k0 += 4) {       // four output columns per pass
+      float acc[4] = {0.f, 0.f, 0.f, 0.f};
+      for (int j = lane; j < n; j += 32) {
+        const float a = prow[j];
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+          if (k0 + k < p) acc[k] = fmaf(a, __ldg(Ls + static_cast<size_t>(j) * p + k0 + k), acc[k]);
+      }
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], o);
+        if (lane == 0 && k0 + k < p) prow[n + k0 + k] = acc[k];
+      }
+    }
+    for (int k = n + p + lane; k < nc; k += 32) prow[k] = 0.f;
+  }
+}
+
 // ------------------------------------------------------------------------------------------ SIMT combine
 // 64 x 64 output tile, 256 threads, 4 x 4 register micro-tile, K blocked by 16 through shared memory.
 constexpr int kST = 64, kSK = 16;
@@ -173,6 +251,137 @@ __global__ void __launch_bounds__(128) phi_tube_finalize_kernel(const float* __r
     }
     r[(static_cast<size_t>(b) * T + t) * n + i] = acc;
   }
+}
+
+// Fused fast path for p <= 8: a warp takes four rows; per column quad it loads A (4 rows), the p rows of C_s and the
+// four rows j..j+3 of Lt_s (4p contiguous floats) ONCE, forms Abar in registers, stores it, and accumulates both the
+// tube partial and the 4 x p products of PhiY(s+1,s) = Abar_s Lt_s; the 4 + 4p sums are finished by shuffles.
+template <int PP>
+__global__ void __launch_bounds__(256) phi_obs_level0_fused_kernel(const float* __restrict__ A, const float* __restrict__ Lt,
+                                                                   const float* __restrict__ C, const float* __restrict__ w,
+                                                                   float* __restrict__ phi, float* __restrict__ part,
+                                                                   int batch, int T, int n, int nc, int NT, int mode) {
+  constexpr int p = PP;   // exact number of measurement rows: every loop below unrolls, Lt is read as float4
+  const int P = T * (T - 1) / 2;
+  const int n4 = n >> 2;
+  const long long nunits = static_cast<long long>(batch) * (T - 1) * n4;
+  const int lane = threadIdx.x & 31;
+  for (long long un = static_cast<long long>(blockIdx.x) * 8 + (threadIdx.x >> 5); un < nunits;
+       un += static_cast<long long>(gridDim.x) * 8) {
+    const int i = 4 * static_cast<int>(un % n4);
+    const long long bs = un / n4;
+    const int s = static_cast<int>(bs % (T - 1));
+    const int b = static_cast<int>(bs / (T - 1));
+    const size_t bt = static_cast<size_t>(b) * T + s;
+    const float4* src = reinterpret_cast<const float4*>(A + (bt * n + i) * n);
+    const float4* wv = reinterpret_cast<const float4*>(w + bt * n);
+    const float4* Cs = reinterpret_cast<const float4*>(C + bt * p * n);
+    const float* Ls = Lt + bt * n * p;
+    const size_t q = static_cast<size_t>(b) * P + phi_colbase(T, s);
+    float* dst = phi + (q * n + i) * nc;
+    float lr[4][PP];   // Lt_s[i + r][k]: the gains of this unit's own rows
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+      for (int k = 0; k < PP; ++k) lr[r][k] = __ldg(Ls + static_cast<size_t>(i + r) * p + k);
+    float tube[4] = {0.f, 0.f, 0.f, 0.f};
+    float y[4][PP];
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+      for (int k = 0; k < PP; ++k) y[r][k] = 0.f;
+    for (int c = lane; c < n4; c += 32) {
+      float4 a[4];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) a[r] = __ldcs(src + static_cast<size_t>(r) * n4 + c);
+#pragma unroll
+      for (int k = 0; k < PP; ++k) {
+        const float4 ck = __ldg(Cs + static_cast<size_t>(k) * n4 + c);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+          a[r].x = fmaf(lr[r][k], ck.x, a[r].x); a[r].y = fmaf(lr[r][k], ck.y, a[r].y);
+          a[r].z = fmaf(lr[r][k], ck.z, a[r].z); a[r].w = fmaf(lr[r][k], ck.w, a[r].w);
+        }
+      }
+      const float4 ww = __ldg(wv + c);
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        *reinterpret_cast<float4*>(dst + static_cast<size_t>(r) * nc + 4 * c) = a[r];
+        tube[r] += (tube_term(a[r].x, ww.x, mode) + tube_term(a[r].y, ww.y, mode)) +
+                   (tube_term(a[r].z, ww.z, mode) + tube_term(a[r].w, ww.w, mode));
+      }
+      // rows 4c .. 4c+3 of Lt_s: 4p contiguous floats
+      const float4* lj4 = reinterpret_cast<const float4*>(Ls + static_cast<size_t>(4 * c) * p);
+      float lt[4 * PP];   // lt[jj * p + k] = Lt_s[4c + jj][k]
+#pragma unroll
+      for (int v = 0; v < PP; ++v) {
+        const float4 t4 = __ldg(lj4 + v);
+        lt[4 * v + 0] = t4.x; lt[4 * v + 1] = t4.y; lt[4 * v + 2] = t4.z; lt[4 * v + 3] = t4.w;
+      }
+#pragma unroll
+      for (int k = 0; k < PP; ++k)
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+          y[r][k] = fmaf(a[r].x, lt[k], fmaf(a[r].y, lt[p + k], fmaf(a[r].z, lt[2 * p + k], fmaf(a[r].w, lt[3 * p + k], y[r][k]))));
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) tube[r] += __shfl_xor_sync(0xffffffffu, tube[r], o);
+#pragma unroll
+      for (int k = 0; k < PP; ++k)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) y[r][k] += __shfl_xor_sync(0xffffffffu, y[r][k], o);
+    }
+    if (lane < 4) {
+      const int r = lane;
+      float* prow = dst + static_cast<size_t>(r) * nc + n;
+      float tr = tube[0];
+#pragma unroll
+      for (int rr = 1; rr < 4; ++rr) tr = (r == rr) ? tube[rr] : tr;
+#pragma unroll
+      for (int k = 0; k < PP; ++k) {
+        float v = y[0][k];
+#pragma unroll
+        for (int rr = 1; rr < 4; ++rr) v = (r == rr) ? y[rr][k] : v;
+        prow[k] = v;
+      }
+      for (int k = p; k < nc - n; ++k) prow[k] = 0.f;
+      for (int e = 0; e < NT; ++e) part[(q * NT + e) * n + i + r] = (e == 0) ? tr : 0.f;
+    }
+  }
+}
+
+cudaError_t launch_phi_obs_level0(const PhiArgs& a, int NT, int num_sms, cudaStream_t stream) {
+  const long long nrows = static_cast<long long>(a.batch) * (a.T - 1) * a.n;
+  long long blocks = (nrows + 7) / 8;
+  const long long cap = static_cast<long long>(num_sms) * 16;
+  if (blocks > cap) blocks = cap;
+  ProfScope prof(kProfPhiLevel0, stream);
+  if (a.p <= 8) {
+    const long long nunits = static_cast<long long>(a.batch) * (a.T - 1) * (a.n >> 2);
+    long long ub = (nunits + 7) / 8;
+    const long long ucap = static_cast<long long>(num_sms) * 8;
+    if (ub > ucap) ub = ucap;
+#define LTV_OBS_CASE(PV)                                                                                        \
+  case PV:                                                                                                     \
+    phi_obs_level0_fused_kernel<PV><<<static_cast<unsigned>(ub), 256, 0, stream>>>(a.A, a.Lt, a.C, a.w, a.phi, a.part, \
+                                                                                   a.batch, a.T, a.n, a.nc, NT,   \
+                                                                                   a.tube_mode);                \
+    break;
+    switch (a.p) {
+      LTV_OBS_CASE(1) LTV_OBS_CASE(2) LTV_OBS_CASE(3) LTV_OBS_CASE(4)
+      LTV_OBS_CASE(5) LTV_OBS_CASE(6) LTV_OBS_CASE(7) LTV_OBS_CASE(8)
+    }
+#undef LTV_OBS_CASE
+    return cudaGetLastError();
+  }
+  phi_obs_level0_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(a.A, a.Lt, a.C, a.w, a.phi, a.part, a.batch, a.T,
+                                                                           a.n, a.nc, a.p, NT, a.tube_mode);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  phi_obs_y0_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(a.Lt, a.phi, a.batch, a.T, a.n, a.nc, a.p);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_phi_level0(const PhiArgs& a, int NT, int num_sms, cudaStream_t stream) {

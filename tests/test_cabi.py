@@ -73,6 +73,13 @@ def test_host_side_validation_needs_no_gpu(L):
     assert s(p, p, p, p, 1, 2, 4, 0, 2, p, 1 << 20, None) == 2                      # unknown flag
     assert s(p, p, p, p, 1, 2, 4, 0, L.LTV_TUBE_ROW_2NORM, p, 8, None) == 5         # known flag passes on
     assert s(p, p, p, p, 1, 2, 4, 0, 0, p, 8, None) == 5                            # workspace too small
+    o = L.lib.ltv_scan_observer_response
+    assert o(p, None, p, p, p, p, 1, 2, 4, 2, 0, 0, p, 1 << 20, None) == 1              # NULL Lt
+    assert o(p, p, p, p, p, p, 1, 2, 4, 0, 0, 0, p, 1 << 20, None) == 2                 # p = 0
+    assert o(p, p, p, p, p, p, 1, 2, 4, 33, 0, 0, p, 1 << 20, None) == 3                # p > 32
+    assert o(p, p, p, p, p, p, 1, 2, 4, 2, 0, 0, p, 8, None) == 5                       # workspace too small
+    assert L.ltv_observer_row_floats(300, 6) == 308 and L.ltv_observer_row_floats(48, 4) == 52
+    assert L.ltv_scan_workspace_bytes(L.LTV_OP_OBSERVER_RESPONSE, 2, 4, 128, 6) > 0
     a = L.lib.ltv_scan_adjoint
     assert a(p, None, p, p, p, None, 1, 2, 4, 2, None, 0, None) == 1                # grad_u wanted, B NULL
     assert a(p, p, None, p, None, None, 1, 2, 4, 2, None, 0, None) == 1             # NULL g

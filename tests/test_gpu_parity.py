@@ -298,3 +298,50 @@ def test_row_two_norm_tube_dense(L, n, T, batch):
     phi, r = L.ltv_scan_system_response_tube(torch.from_numpy(W.A).cuda(), torch.from_numpy(W.w).cuda(), two_norm=True)
     torch.cuda.synchronize()
     assert O.rel_err(r.cpu().numpy(), O.tube_row2norm(W.A, W.w)) <= TOL
+
+
+def _observer_inputs(batch, T, n, p, seed):
+    rng = np.random.default_rng(seed)
+    W = dense_random(batch, T, n, 1, seed=seed, scale=0.4)
+    Lt = rng.normal(0.0, 0.3 / np.sqrt(p), (batch, T, n, p)).astype(np.float32)
+    C = rng.normal(0.0, 1.0 / np.sqrt(n), (batch, T, p, n)).astype(np.float32)
+    return W, Lt, C
+
+
+@pytest.mark.parametrize("n,T,batch,p", [(48, 6, 2, 3),      # fp32-FMA path, nc = 52
+                                         (128, 5, 2, 6),     # tensor-core path, nc = 136: second n-tile is PhiY only
+                                         (300, 9, 2, 6),     # C2 shape: nc = 308 fits the padding of two 160-wide tiles
+                                         (164, 4, 1, 32),    # widest gain block
+                                         (100, 3, 3, 1)])
+def test_observer_response(L, n, T, batch, p):
+    """NEXT-1, eq.(14): PhiX over the closed-loop matrices A + Lt C, PhiY = PhiX Lt riding along as extra columns;
+    the oracle multiplies on the RIGHT in the paper's order, the GPU runs the divide-and-conquer scan."""
+    import torch
+
+    W, Lt, C = _observer_inputs(batch, T, n, p, seed=5 * n + p)
+    d = [torch.from_numpy(a).cuda() for a in (W.A, Lt, C, W.w)]
+    phi, r = L.ltv_scan_observer_response(*d)
+    torch.cuda.synchronize()
+    nc = L.ltv_observer_row_floats(n, p)
+    assert phi.shape == (batch, T * (T - 1) // 2, n, nc)
+    phi = phi.cpu().numpy()
+    X, Y = O.observer_response(W.A, Lt, C)
+    perm = _col_perm(T)
+    assert O.rel_err(phi[..., :n], X[:, perm]) <= TOL
+    assert O.rel_err(phi[..., n:n + p], Y[:, perm]) <= TOL
+    assert np.all(phi[..., n + p:] == 0.0)
+    # tube of PhiX: the box-tube oracle applied to the closed-loop matrices (float64 Abar is not an fp32 input of
+    # the GPU, so this check carries the rounding of forming Abar in fp32: still far inside TOL)
+    Abar = W.A.astype(np.float64) + Lt.astype(np.float64) @ C.astype(np.float64)
+    assert O.rel_err(r.cpu().numpy(), O.tube(Abar, W.w)) <= TOL
+
+
+def test_observer_zero_gain_is_the_open_loop_response(L):
+    import torch
+
+    W, Lt, C = _observer_inputs(2, 6, 132, 4, seed=3)
+    A, w = torch.from_numpy(W.A).cuda(), torch.from_numpy(W.w).cuda()
+    phi, r = L.ltv_scan_observer_response(A, torch.zeros_like(torch.from_numpy(Lt)).cuda(), torch.from_numpy(C).cuda(), w)
+    phi0, r0 = L.ltv_scan_system_response_tube(A, w)
+    torch.cuda.synchronize()
+    assert torch.equal(phi[..., :132], phi0) and torch.equal(r, r0) and torch.all(phi[..., 132:] == 0)
