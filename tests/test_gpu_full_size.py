@@ -134,3 +134,36 @@ def test_c5_sweep(L, batch):
     W = generate(config(4, batch=batch))                  # n=180, T=64: rollout + adjoint only
     d = _dev(W, keys=("A", "B", "c", "x0", "u", "g"))
     _vector_outputs(L, W, d, items=[0, batch // 2, batch - 1])
+
+
+def test_c2_full_observer_and_two_norm(L):
+    """NEXT-1 / NEXT-2 at the bench size (n=300, T=32, batch=64, p=6): every block and both tubes of one item against
+    the oracle, sampled blocks of others, and the semigroup property on the GPU's own [PhiX | PhiY] blocks."""
+    import torch
+
+    W = generate(config(1))
+    batch, T, n, m = W.shape
+    p = 6
+    rng = np.random.default_rng(99)
+    Lt = rng.normal(0.0, 0.05 / np.sqrt(p), (batch, T, n, p)).astype(np.float32)
+    C = rng.normal(0.0, 1.0 / np.sqrt(n), (batch, T, p, n)).astype(np.float32)
+    A, w = torch.from_numpy(W.A).cuda(), torch.from_numpy(W.w).cuda()
+    phi, r = L.ltv_scan_observer_response(A, torch.from_numpy(Lt).cuda(), torch.from_numpy(C).cuda(), w, two_norm=True)
+    torch.cuda.synchronize()
+    nc = L.ltv_observer_row_floats(n, p)
+    assert phi.shape[-1] == nc and bool((phi[..., n + p:] == 0).all())
+    perm = [O.packed_index(t, s) for s in range(T - 1) for t in range(s + 1, T)]
+    b = 37
+    X, Y = O.observer_response_item(W.A[b], Lt[b], C[b])
+    got = phi[b].cpu().numpy()
+    assert O.rel_err(got[..., :n], X[perm]) <= TOL and O.rel_err(got[..., n:n + p], Y[perm]) <= TOL
+    Abar = W.A[b].astype(np.float64) + Lt[b].astype(np.float64) @ C[b].astype(np.float64)
+    assert O.rel_err(r[b].cpu().numpy(), O.tube_row2norm_item(Abar, W.w[b])) <= TOL
+    for (bb, t, s) in [(0, 31, 0), (63, 17, 16), (12, 9, 2)]:
+        Ab = W.A[bb].astype(np.float64) + Lt[bb].astype(np.float64) @ C[bb].astype(np.float64)
+        ref = O.phi_block(Ab, t, s)
+        blk = phi[bb, L.ltv_phi_block_index(T, t, s)].cpu().numpy()
+        assert O.rel_err(blk[:, :n], ref) <= TOL and O.rel_err(blk[:, n:n + p], ref @ Lt[bb, s].astype(np.float64)) <= TOL
+    q = lambda tt, ss: phi[50, L.ltv_phi_block_index(T, tt, ss)].double()
+    rhs = q(30, 11)[:, :n] @ q(11, 3)
+    assert float((q(30, 3) - rhs).abs().max() / rhs.abs().max()) <= TOL
