@@ -27,6 +27,15 @@ sequential recursion - "We obtain the solution to (14) by a forward parallel ass
   observer_response  PhiX(k,k) = I; PhiX(k,j) = PhiX(k,j+1) (A_j + L_j^T C_j);     PAPER.md:157-160 eq.(14), read with
                    PhiY(k,j) = PhiX(k,j) L_j^T,  0 <= j < k <= T-1                 k-independent gains L_j (:177; SURVEY
                                                                      8f NEXT-1, reading q15)
+  kalman_recursion Pi_0 = Xi Xi^T; L_{j+1} = -(F_j F_j^T + C_j Pi_j C_j^T)^{-1} C_j Pi_j A_j^T;   PAPER.md:152-155 eq.(13), with the
+                   Pi_{j+1} = E_j E_j^T + A_j Pi_j A_j^T + A_j Pi_j C_j^T L_{j+1}             k-independent reading of :177 and
+                                                                     the stand-ins E_j = diag(e_j),
+                                                                     F_j = diag(f_j) (SURVEY 8f NEXT-3;
+                                                                     DESIGN.md readings q3b, q17, q18)
+  riccati_scan     the same Pi_j by the associative combination rules (16) with the initial values   PAPER.md:166-177 eq.(16)(17); (16) is
+                   (17), folded in the order Pi_j = P~ of e_{j-1} (x) ... (x) e_0 (x) e_init          garbled in the source and
+                                                                     is re-derived from the conditional
+                                                                     value function of :166 (DESIGN.md q14)
   adjoint          lam_T = g_T; lam_t = A_t^T lam_{t+1} + g_t;       PAPER.md:106-110 eq.(10) chained
                    grad_u[t] = B_t^T lam_{t+1}; grad_x0 = A_0^T lam_1   over the horizon; north_star (iii)
 
@@ -37,7 +46,10 @@ Inputs are the fp32 arrays handed to the GPU, promoted to fp64 here (never a sep
 
 Pins (tests/test_oracle_pins.py): every function below is pinned by closed forms, the defining identity
 (12c), brute force on tiny inputs, a hand-computed worked example (tests/golden/hand_example.txt) and the
-tube-containment / adjoint dot-product invariants.  Nothing in this file is "parity unpinned".
+tube-containment / adjoint dot-product invariants.  kalman_recursion / riccati_* are pinned in
+tests/test_oracle_pins_kalman.py (brute-force Gaussian conditioning, information form, DARE fixed point from
+scipy, Lyapunov sum through Phi, Joseph form + gain optimality, scan = recursion, associativity).
+Nothing in this file is "parity unpinned".
 """
 from __future__ import annotations
 
@@ -127,6 +139,73 @@ def observer_response_item(A, Lt, C):
 def observer_response(A, Lt, C):
     out = [observer_response_item(A[b], Lt[b], C[b]) for b in range(A.shape[0])]
     return np.stack([o[0] for o in out]), np.stack([o[1] for o in out])
+
+
+# --------------------------------------------------------------------------- Kalman recursion (13), Riccati scan (16)(17)
+def kalman_recursion_item(A, C, e, f, Pi0):
+    """Backward-Kalman recursion of eq.(13), one item, written out step by step:
+        Pi_0 = Xi Xi^T (given as Pi0);   for j = 0 .. T-1:
+        L_{j+1}  = -(F_j F_j^T + C_j Pi_j C_j^T)^{-1} C_j Pi_j A_j^T                     [p,n]
+        Pi_{j+1} = E_j E_j^T + A_j Pi_j A_j^T + A_j Pi_j C_j^T L_{j+1}                   [n,n]
+    with E_j = diag(e[j]), F_j = diag(f[j]) (f > 0).  A[T,n,n], C[T,p,n], e[T,n], f[T,p], Pi0[n,n] symmetric PSD.
+    Returns Pi[T+1,n,n] (Pi[j] = Pi_j) and Lt[T,n,p] with Lt[j] = L_{j+1}^T: the gain formed from (A_j, C_j, Pi_j),
+    i.e. the one that closes the loop around A_j, A_j + Lt[j] C_j - the array `observer_response` takes (q17)."""
+    A, C, e, f, Pi0 = _f64(A), _f64(C), _f64(e), _f64(f), _f64(Pi0)
+    T, n, _ = A.shape
+    p = C.shape[1]
+    Pi = np.empty((T + 1, n, n))
+    Lt = np.empty((T, n, p))
+    Pi[0] = Pi0
+    for j in range(T):
+        E = np.diag(e[j])
+        F = np.diag(f[j])
+        S = F @ F.T + C[j] @ Pi[j] @ C[j].T
+        L = -np.linalg.solve(S, C[j] @ Pi[j] @ A[j].T)
+        Pi[j + 1] = E @ E.T + A[j] @ Pi[j] @ A[j].T + A[j] @ Pi[j] @ C[j].T @ L
+        Lt[j] = L.T
+    return Pi, Lt
+
+
+def kalman_recursion(A, C, e, f, Pi0):
+    out = [kalman_recursion_item(A[b], C[b], e[b], f[b], Pi0[b]) for b in range(A.shape[0])]
+    return np.stack([o[0] for o in out]), np.stack([o[1] for o in out])
+
+
+def riccati_combine(x, y):
+    """Combination rule (16) of two conditional value functions (:166), x = (A~,D~,P~)_{i,m} and
+    y = (A~,D~,P~)_{m,l}, giving (A~,D~,P~)_{i,l}:
+        P~_{i,l} = A~_{i,m}^T (I + P~_{m,l} D~_{i,m})^{-1} P~_{m,l} A~_{i,m} + P~_{i,m}
+        A~_{i,l} = A~_{m,l} (I + D~_{i,m} P~_{m,l})^{-1} A~_{i,m}
+        D~_{i,l} = A~_{m,l} (I + D~_{i,m} P~_{m,l})^{-1} D~_{i,m} A~_{m,l}^T + D~_{m,l}
+    (the source prints an unbalanced parenthesis in the first rule; this is the form that follows from eliminating
+    the intermediate argument of the two value functions of :166, reading q14)."""
+    A1, D1, P1 = x
+    A2, D2, P2 = y
+    I = np.eye(A1.shape[0])
+    G = I + D1 @ P2
+    P = A1.T @ np.linalg.solve(G.T, P2 @ A1) + P1
+    A = A2 @ np.linalg.solve(G, A1)
+    D = A2 @ np.linalg.solve(G, D1) @ A2.T + D2
+    return A, D, P
+
+
+def riccati_scan_item(A, C, e, f, Pi0):
+    """Pi_j of eq.(13) through the associative elements of (16)(17): step i contributes
+    e_i = (A~ = A_i^T, D~ = C_i^T (F_i F_i^T)^{-1} C_i, P~ = E_i E_i^T), the initial uncertainty contributes
+    e_init = (0, 0, Xi Xi^T) ("P~_{1,0} = Xi Xi^T, A~_{1,0} = D~_{1,0} = 0"), and
+    Pi_j = P~ part of e_{j-1} (x) e_{j-2} (x) ... (x) e_0 (x) e_init - here folded one element at a time, newest on
+    the left; any bracketing gives the same result (the operator is associative; pinned in the tests)."""
+    A, C, e, f, Pi0 = _f64(A), _f64(C), _f64(e), _f64(f), _f64(Pi0)
+    T, n, _ = A.shape
+    Z = np.zeros((n, n))
+    acc = (Z, Z, Pi0)
+    Pi = np.empty((T + 1, n, n))
+    Pi[0] = Pi0
+    for i in range(T):
+        elem = (A[i].T, C[i].T @ np.diag(1.0 / f[i] ** 2) @ C[i], np.diag(e[i] ** 2))
+        acc = riccati_combine(elem, acc)
+        Pi[i + 1] = acc[2]
+    return Pi
 
 
 def phi_block(A, t: int, s: int):

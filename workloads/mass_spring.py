@@ -223,3 +223,31 @@ def small_integer(batch: int, T: int, n: int, m: int, seed: int, density: float 
         g=f32(rng.integers(-1, 2, (batch, T, n))),
         meta=dict(name="small_integer", n=n, m=m, T=T, batch=batch, seed=seed),
     )
+
+
+def observation_model(batch: int, T: int, n: int, p: int, seed: int, kind: str = "track") -> dict:
+    """Inputs of the output-feedback stage (eq.(13)): observation Jacobians C_j, the disturbance
+    scalings E_j = diag(e_j), F_j = diag(f_j) and the initial uncertainty Pi_0 = Xi Xi^T.  The paper's C, E, F, Xi come
+    from its perception stack and calibration, which are not in the container; stand-ins:
+      kind "track"  C_j selects p position coordinates spread evenly over the first n/2 state entries (tracked points
+                    on the object, constant in j but stored per step)
+      kind "dense"  C_j ~ N(0, 1/sqrt(n)) i.i.d. per step
+      e ~ U[2e-4, 1e-3] (process), f ~ U[1e-3, 5e-3] (observation), Xi = 1e-2 (I + 0.1 N(0, 1/sqrt(n))).
+    Returns fp32 arrays C[batch,T,p,n], e[batch,T,n], f[batch,T,p], Pi0[batch,n,n] (Pi0 exactly symmetric)."""
+    rng = np.random.default_rng(seed)
+    if kind == "track":
+        half = max(p, n // 2)
+        cols = (np.arange(p) * half) // p
+        C = np.zeros((batch, T, p, n))
+        C[:, :, np.arange(p), cols] = 1.0
+    elif kind == "dense":
+        C = rng.normal(0.0, 1.0 / np.sqrt(n), (batch, T, p, n))
+    else:
+        raise ValueError(kind)
+    e = rng.uniform(2e-4, 1e-3, (batch, T, n))
+    f = rng.uniform(1e-3, 5e-3, (batch, T, p))
+    Xi = 1e-2 * (np.eye(n)[None] + 0.1 * rng.normal(0.0, 1.0 / np.sqrt(n), (batch, n, n)))
+    Pi0 = (Xi @ np.swapaxes(Xi, 1, 2)).astype(np.float32)
+    Pi0 = np.ascontiguousarray(0.5 * (Pi0 + np.swapaxes(Pi0, 1, 2)))
+    f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+    return dict(C=f32(C), e=f32(e), f=f32(f), Pi0=f32(Pi0))
