@@ -61,7 +61,8 @@ typedef enum {
 /* `op` argument of ltv_scan_workspace_bytes */
 enum { LTV_OP_ROLLOUT = 0, LTV_OP_SYSTEM_RESPONSE_TUBE = 1, LTV_OP_ADJOINT = 2, LTV_OP_PIPELINE_HOST = 3,
        LTV_OP_PIPELINE_HOST_NO_PHI = 4 /* ltv_scan_pipeline_host with w_host == NULL: rollout + adjoint only */,
-       LTV_OP_OBSERVER_RESPONSE = 5 /* ltv_scan_observer_response; pass p (rows of C) as `m` */ };
+       LTV_OP_OBSERVER_RESPONSE = 5 /* ltv_scan_observer_response; pass p (rows of C) as `m` */,
+       LTV_OP_KALMAN_GAINS = 6 /* ltv_scan_kalman_gains; pass p (rows of C) as `m` */ };
 
 /* `phi_layout` argument.  COLUMN_PACKED (the only layout of this version): the P = T(T-1)/2 blocks of one
  * item are stored column by column of the block-lower-triangular operator; block (t,s), 0 <= s < t <= T-1,
@@ -144,6 +145,30 @@ LTV_API int ltv_scan_observer_response(const float* A, const float* Lt, const fl
                                        float* phi_out, float* r_out, int batch, int T, int n, int p, int phi_layout,
                                        unsigned flags, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Backward-Kalman recursion of the output-feedback stage (eq.(13)), with the
+ * disturbance scalings taken diagonal, E_j = diag(e_j), F_j = diag(f_j) (readings q3b, q18):
+ *     Pi_0 = Xi Xi^T (given);   for j = 0 .. T-1:
+ *     L_{j+1}  = -(F_j F_j^T + C_j Pi_j C_j^T)^{-1} C_j Pi_j A_j^T
+ *     Pi_{j+1} = E_j E_j^T + A_j Pi_j A_j^T + A_j Pi_j C_j^T L_{j+1}
+ *   A        device [batch,T,n,n]      required
+ *   C        device [batch,T,p,n]      required; observation Jacobians, 1 <= p <= 32
+ *   e        device [batch,T,n]        required; process-disturbance scaling
+ *   f        device [batch,T,p]        required; observation-disturbance scaling, every entry > 0 (F_j F_j^T must be
+ *                                      positive definite; not checked)
+ *   Pi0      device [batch,n,n]        required; symmetric positive semi-definite
+ *   Lt_out   device [batch,T,n,p]      Lt_out[b,j] = L_{j+1}^T, the gain formed from (A_j, C_j, Pi_j): exactly the `Lt`
+ *                                      array of ltv_scan_observer_response (A_j + Lt_j C_j closes the loop around A_j)
+ *   Pi_out   device [batch,T+1,n,n]    Pi_out[b,j] = Pi_j (Pi_out[b,0] = Pi0)
+ *   flags    must be 0
+ * Time-sequential, batch-parallel: per step one pass forms G = C Pi, the p x p innovation covariance (Cholesky), the
+ * gain and the closed-loop matrix Abar_j = A_j + Lt_j C_j, then two batched 3xTF32 tcgen05 GEMMs form
+ * Pi_{j+1} = A_j (Abar_j Pi_j)^T + E E^T (fp32 FMA for n < 96).  The associative-scan form (16)(17) of the paper is
+ * ~10x the flops and is not used at these batch sizes.  Results are symmetric up to rounding.
+ * Workspace: ltv_scan_workspace_bytes(LTV_OP_KALMAN_GAINS, batch, T, n, p). */
+LTV_API int ltv_scan_kalman_gains(const float* A, const float* C, const float* e, const float* f, const float* Pi0,
+                                  float* Lt_out, float* Pi_out, int batch, int T, int n, int p, unsigned flags,
+                                  void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* One pass of the whole hot path from HOST buffers: copies A, B, c, x0, u, w, g host->device into
  * `workspace` (device, >= ltv_scan_workspace_bytes(LTV_OP_PIPELINE_HOST, ...)), runs the three calls above
  * on `cuda_stream`, copies x, r, lambda, grad_u, grad_x0 device->host and synchronises the stream before
@@ -180,8 +205,9 @@ LTV_API unsigned long long ltv_launch_count(void);
  * ltv_profile_collect waits for the recorded events, adds their elapsed times (milliseconds) and launch counts
  * per kernel class into the two caller arrays of LTV_PROFILE_CLASSES entries (host memory), and clears the
  * record.  Classes: 0 rollout, 1 adjoint, 2 Phi level 0 (copy + tube), 3 Phi combine (tcgen05 3xTF32),
- * 4 Phi combine (fp32 FMA, small n), 5 tube finalise. */
-#define LTV_PROFILE_CLASSES 6
+ * 4 Phi combine (fp32 FMA, small n), 5 tube finalise, 6 Kalman batched GEMMs (tcgen05 3xTF32, or fp32 FMA for
+ * small n), 7 Kalman gain / closed-loop kernels. */
+#define LTV_PROFILE_CLASSES 8
 LTV_API int ltv_profile_enable(int on);
 LTV_API int ltv_profile_collect(double* ms_by_class, unsigned long long* launches_by_class);
 

@@ -12,7 +12,8 @@ _API = (
     "LTV_OP_SYSTEM_RESPONSE_TUBE", "LTV_PHI_COLUMN_PACKED", "LTV_TUBE_ROW_2NORM", "PROFILE_CLASSES", "LtvError", "lib",
     "ltv_launch_count", "ltv_phi_block_index", "ltv_profile_collect", "ltv_profile_enable",
     "ltv_scan_adjoint", "ltv_scan_pipeline_host", "ltv_scan_rollout", "ltv_scan_system_response_tube",
-    "ltv_scan_workspace_bytes", "ltv_scan_observer_response", "ltv_observer_row_floats",
+    "ltv_scan_workspace_bytes", "ltv_scan_observer_response", "ltv_observer_row_floats", "ltv_scan_kalman_gains",
+    "LTV_OP_KALMAN_GAINS",
 )
 __all__ = list(_API)
 

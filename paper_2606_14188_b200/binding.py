@@ -19,6 +19,7 @@ STATUS_NAMES = {
 LTV_OP_ROLLOUT, LTV_OP_SYSTEM_RESPONSE_TUBE, LTV_OP_ADJOINT, LTV_OP_PIPELINE_HOST = 0, 1, 2, 3
 LTV_OP_PIPELINE_HOST_NO_PHI = 4
 LTV_OP_OBSERVER_RESPONSE = 5
+LTV_OP_KALMAN_GAINS = 6
 LTV_TUBE_ROW_2NORM = 1
 LTV_PHI_COLUMN_PACKED = 0
 
@@ -26,7 +27,7 @@ EXPORTS = (
     "ltv_phi_block_index", "ltv_scan_workspace_bytes", "ltv_scan_rollout", "ltv_scan_system_response_tube",
     "ltv_scan_adjoint", "ltv_scan_pipeline_host", "ltv_status_string", "ltv_last_cuda_error", "ltv_version",
     "ltv_launch_count", "ltv_profile_enable", "ltv_profile_collect", "ltv_scan_observer_response",
-    "ltv_observer_row_floats",
+    "ltv_observer_row_floats", "ltv_scan_kalman_gains",
 )
 
 
@@ -57,6 +58,8 @@ def _load() -> ctypes.CDLL:
     L.ltv_scan_pipeline_host.argtypes = [fp] * 13 + [i] * 4 + [vp, sz, vp, ctypes.POINTER(ctypes.c_void_p)]
     L.ltv_scan_observer_response.restype = i
     L.ltv_scan_observer_response.argtypes = [fp] * 6 + [i] * 5 + [ctypes.c_uint, vp, sz, vp]
+    L.ltv_scan_kalman_gains.restype = i
+    L.ltv_scan_kalman_gains.argtypes = [fp] * 7 + [i] * 4 + [ctypes.c_uint, vp, sz, vp]
     L.ltv_observer_row_floats.restype = i
     L.ltv_observer_row_floats.argtypes = [i, i]
     L.ltv_status_string.restype = ctypes.c_char_p
@@ -104,7 +107,8 @@ def ltv_launch_count() -> int:
     return int(lib.ltv_launch_count())
 
 
-PROFILE_CLASSES = ("rollout", "adjoint", "phi_level0", "phi_combine_tc", "phi_combine_simt", "phi_finalize")
+PROFILE_CLASSES = ("rollout", "adjoint", "phi_level0", "phi_combine_tc", "phi_combine_simt", "phi_finalize",
+                   "kalman_gemm", "kalman_simt")
 
 
 def ltv_profile_enable(on: bool) -> None:
@@ -186,6 +190,28 @@ def ltv_scan_observer_response(A, Lt, C, w, phi_out=None, r_out=None, workspace=
     if st != LTV_OK:
         raise LtvError(st, "ltv_scan_observer_response")
     return phi_out, r_out
+
+
+def ltv_scan_kalman_gains(A, C, e, f, Pi0, Lt_out=None, Pi_out=None, workspace=None):
+    """Backward-Kalman recursion (eq.(13)): returns (Lt[batch,T,n,p] with Lt[b,j] = L_{j+1}^T, Pi[batch,T+1,n,n]).
+    C[batch,T,p,n], e[batch,T,n], f[batch,T,p] (> 0), Pi0[batch,n,n] symmetric PSD."""
+    batch, T, n, _ = A.shape
+    p = C.shape[2]
+    _dev(A, "A", (batch, T, n, n)); _dev(C, "C", (batch, T, p, n)); _dev(e, "e", (batch, T, n))
+    _dev(f, "f", (batch, T, p)); _dev(Pi0, "Pi0", (batch, n, n))
+    if Lt_out is None:
+        Lt_out = torch.empty((batch, T, n, p), device=A.device, dtype=torch.float32)
+    if Pi_out is None:
+        Pi_out = torch.empty((batch, T + 1, n, n), device=A.device, dtype=torch.float32)
+    _dev(Lt_out, "Lt_out", (batch, T, n, p)); _dev(Pi_out, "Pi_out", (batch, T + 1, n, n))
+    need = ltv_scan_workspace_bytes(LTV_OP_KALMAN_GAINS, batch, T, n, p)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), device=A.device, dtype=torch.uint8)
+    st = lib.ltv_scan_kalman_gains(_ptr(A), _ptr(C), _ptr(e), _ptr(f), _ptr(Pi0), _ptr(Lt_out), _ptr(Pi_out),
+                                   batch, T, n, p, 0, _ptr(workspace), workspace.numel(), _stream())
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_kalman_gains")
+    return Lt_out, Pi_out
 
 
 def ltv_scan_adjoint(A, B, g, want_grad_x0=True, lambda_out=None, grad_u_out=None, grad_x0_out=None):

@@ -159,6 +159,9 @@ size_t ltv_scan_workspace_bytes(int op, int batch, int T, int n, int m) {
     case LTV_OP_OBSERVER_RESPONSE:
       if (m < 1 || m > 32) return 0;
       return phi_workspace_bytes(batch, T, n, n + ((m + 3) & ~3));
+    case LTV_OP_KALMAN_GAINS:
+      if (m < 1 || m > 32) return 0;
+      return kalman_workspace_bytes(batch, T, n, m);
     case LTV_OP_PIPELINE_HOST:
     case LTV_OP_PIPELINE_HOST_NO_PHI: {
       const bool with_phi = op == LTV_OP_PIPELINE_HOST;
@@ -290,6 +293,29 @@ int ltv_scan_observer_response(const float* A, const float* Lt, const float* C, 
   cudaError_t e = launch_phi_tube(a, static_cast<cudaStream_t>(cuda_stream), &l);
   g_launches += l;
   return e == cudaSuccess ? LTV_OK : fail_cuda(e);
+}
+
+int ltv_scan_kalman_gains(const float* A, const float* C, const float* e, const float* f, const float* Pi0,
+                          float* Lt_out, float* Pi_out, int batch, int T, int n, int p, unsigned flags,
+                          void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!A || !C || !e || !f || !Pi0 || !Lt_out || !Pi_out || !workspace) return LTV_ERR_NULL_PTR;
+  int st = check_dims(batch, T, n, 0);
+  if (st != LTV_OK) return st;
+  if (p < 1 || flags != 0) return LTV_ERR_BAD_DIM;
+  if (p > 32) return LTV_ERR_UNSUPPORTED_SHAPE;
+  if (static_cast<long long>(batch) * (T + 1) * n >= (1ll << 31)) return LTV_ERR_UNSUPPORTED_SHAPE;
+  if (misaligned(A) || misaligned(C) || misaligned(e) || misaligned(f) || misaligned(Pi0) || misaligned(Lt_out) ||
+      misaligned(Pi_out) || misaligned(workspace))
+    return LTV_ERR_ALIGNMENT;
+  if (workspace_bytes < kalman_workspace_bytes(batch, T, n, p)) return LTV_ERR_WORKSPACE_TOO_SMALL;
+  int sms = 0;
+  st = check_device(&sms);
+  if (st != LTV_OK) return st;
+  KalmanArgs a{A, C, e, f, Pi0, Lt_out, Pi_out, batch, T, n, p, workspace};
+  unsigned long long l = 0;
+  cudaError_t err = launch_kalman(a, static_cast<cudaStream_t>(cuda_stream), &l);
+  g_launches += l;
+  return err == cudaSuccess ? LTV_OK : fail_cuda(err);
 }
 
 int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float* c_host, const float* x0_host,

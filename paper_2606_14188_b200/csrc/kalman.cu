@@ -1,0 +1,387 @@
+// ltv_scan_kalman_gains: the backward-Kalman recursion of eq.(13), batched over
+// items and time-sequential:
+//     Pi_0 = Xi Xi^T;   L_{j+1} = -(F_j F_j^T + C_j Pi_j C_j^T)^{-1} C_j Pi_j A_j^T;
+//     Pi_{j+1} = E_j E_j^T + A_j Pi_j A_j^T + A_j Pi_j C_j^T L_{j+1}
+// computed per step j, for all items at once, as
+//     G = C_j Pi_j                     [p,n]   kalman_cpi_kernel      (split over k, fixed-order partial sums)
+//     S = F F^T + G C_j^T, K = S^{-1}G [p,n]   kalman_gain_kernel     (Cholesky of the p x p innovation covariance)
+//     Lt_j = L_{j+1}^T = -A_j K^T      [n,p]   kalman_closed_loop_kernel (A_j streams through once: the same pass
+//     Abar_j = A_j + Lt_j C_j          [n,n]                           writes the closed-loop matrix of eq.(14))
+//     Yt = (Abar_j Pi_j)^T             [n,n]   tcgen05 3xTF32 batched GEMM, transposed store
+//     Pi_{j+1} = A_j Yt + diag(e_j)^2  [n,n]   tcgen05 3xTF32 batched GEMM, E E^T added in the epilogue
+// (A_j Pi_j Abar_j^T is the right-hand side of (13) with L_{j+1} substituted.)
+//
+// Why the recursion and not the associative scan (16)(17) the paper runs: one combination of (16)
+// costs an n x n solve with 2n right-hand sides plus six n^3 products (~17 n^3 flop) against 4 n^3 for one step of
+// (13), and a scan needs (T/2) log2 T of them; at T = 32 that is ~10x the flops.  The scan buys depth log T for a
+// single item on a small GPU; here one step over the whole batch already fills all 148 SMs (C2: 384 tiles of
+// 128 x 160), so the sequential form is the faster one at every BASELINE.json size.  The scan is kept in the oracle,
+// pinned against the recursion (tests/test_oracle_pins_kalman.py).  DESIGN.md section 7.
+#include <cuda.h>
+
+#include <algorithm>
+#include <type_traits>
+
+#include "ltv_internal.h"
+#include "phi_kernels.h"
+
+namespace ltv {
+
+namespace {
+
+constexpr int kCpiCols = 128;   // columns of Pi per CTA in kalman_cpi_kernel
+constexpr int kMaxKs = 8;       // at most this many k-splits of G = C Pi
+
+// G_part[ks][b][q][j] = sum_{k in split ks} C[b][q][k] Pi[b][k][j].   grid (ceil(n/128), KS, batch), 128 threads.
+template <int PG>
+__global__ void __launch_bounds__(kCpiCols) kalman_cpi_kernel(const float* __restrict__ C, long long c_stride,
+                                                              const float* __restrict__ Pi, long long pi_stride,
+                                                              float* __restrict__ Gpart, int batch, int n, int p) {
+  constexpr int PP = 8 * PG;
+  const int b = blockIdx.z, ks = blockIdx.y, KS = gridDim.y;
+  const int j = blockIdx.x * kCpiCols + threadIdx.x;
+  const int kq = ((n / 4 + KS - 1) / KS) * 4;   // k per split, multiple of 4
+  const int k0 = ks * kq, k1 = min(n, k0 + kq);
+  const float* Cb = C + b * c_stride;
+  const float* Pb = Pi + b * pi_stride;
+  float acc[PP];
+#pragma unroll
+  for (int q = 0; q < PP; ++q) acc[q] = 0.f;
+  if (j < n) {
+    for (int k = k0; k < k1; k += 4) {
+      const float x0 = __ldg(Pb + static_cast<size_t>(k) * n + j);
+      const float x1 = __ldg(Pb + static_cast<size_t>(k + 1) * n + j);
+      const float x2 = __ldg(Pb + static_cast<size_t>(k + 2) * n + j);
+      const float x3 = __ldg(Pb + static_cast<size_t>(k + 3) * n + j);
+#pragma unroll
+      for (int q = 0; q < PP; ++q) {
+        if (q < p) {
+          const float4 c4 = __ldg(reinterpret_cast<const float4*>(Cb + static_cast<size_t>(q) * n + k));
+          acc[q] = fmaf(c4.x, x0, acc[q]);
+          acc[q] = fmaf(c4.y, x1, acc[q]);
+          acc[q] = fmaf(c4.z, x2, acc[q]);
+          acc[q] = fmaf(c4.w, x3, acc[q]);
+        }
+      }
+    }
+    float* out = Gpart + ((static_cast<size_t>(ks) * batch + b) * p) * n + j;
+#pragma unroll
+    for (int q = 0; q < PP; ++q)
+      if (q < p) out[static_cast<size_t>(q) * n] = acc[q];
+  }
+}
+
+// One CTA per item: G = sum of the k-split partials (fixed order), S = diag(f)^2 + G C^T, Cholesky S = R R^T,
+// K = S^{-1} G.  256 threads; shared memory: S [32][33].
+template <int PG>
+__global__ void __launch_bounds__(256) kalman_gain_kernel(const float* __restrict__ C, long long c_stride,
+                                                          const float* __restrict__ f, long long f_stride,
+                                                          const float* __restrict__ Gpart, int KS, float* __restrict__ G,
+                                                          float* __restrict__ K, int batch, int n, int p) {
+  constexpr int PP = 8 * PG;
+  __shared__ float S[32][33];
+  const int b = blockIdx.x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const float* Cb = C + b * c_stride;
+  float* Gb = G + static_cast<size_t>(b) * p * n;
+  float* Kb = K + static_cast<size_t>(b) * p * n;
+  for (int i = threadIdx.x; i < p * n; i += 256) {
+    float s = 0.f;
+    for (int ks = 0; ks < KS; ++ks) s += __ldg(Gpart + (static_cast<size_t>(ks) * batch + b) * p * n + i);
+    Gb[i] = s;
+  }
+  __syncthreads();
+  // S[q][r], r <= q (G C^T is symmetric because Pi is; only the lower triangle is formed and used)
+  for (int pr = warp; pr < p * p; pr += 8) {
+    const int q = pr / p, r = pr % p;
+    if (r > q) continue;
+    float s = 0.f;
+    for (int k = lane; k < n; k += 32) s = fmaf(Gb[static_cast<size_t>(q) * n + k], __ldg(Cb + static_cast<size_t>(r) * n + k), s);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) {
+      if (q == r) {
+        const float ff = __ldg(f + b * f_stride + q);
+        s = fmaf(ff, ff, s);
+      }
+      S[q][r] = s;
+    }
+  }
+  __syncthreads();
+  if (warp == 0) {
+    // right-looking Cholesky, lane = row
+    for (int k = 0; k < p; ++k) {
+      const float d = sqrtf(S[k][k]);
+      __syncwarp();
+      if (lane == k) S[k][k] = d;
+      if (lane > k && lane < p) S[lane][k] /= d;
+      __syncwarp();
+      if (lane > k && lane < p)
+        for (int c = k + 1; c <= lane; ++c) S[lane][c] -= S[lane][k] * S[c][k];
+      __syncwarp();
+    }
+  }
+  __syncthreads();
+  for (int j = threadIdx.x; j < n; j += 256) {
+    float y[PP];
+#pragma unroll
+    for (int q = 0; q < PP; ++q) y[q] = (q < p) ? Gb[static_cast<size_t>(q) * n + j] : 0.f;
+    // R y' = g (forward), R^T k = y' (backward)
+#pragma unroll
+    for (int q = 0; q < PP; ++q) {
+      if (q < p) {
+        float s = y[q];
+#pragma unroll
+        for (int r = 0; r < q; ++r) s = fmaf(-S[q][r], y[r], s);
+        y[q] = s / S[q][q];
+      }
+    }
+#pragma unroll
+    for (int q = PP - 1; q >= 0; --q) {
+      if (q < p) {
+        float s = y[q];
+#pragma unroll
+        for (int r = q + 1; r < PP; ++r)
+          if (r < p) s = fmaf(-S[r][q], y[r], s);
+        y[q] = s / S[q][q];
+      }
+    }
+#pragma unroll
+    for (int q = 0; q < PP; ++q)
+      if (q < p) Kb[static_cast<size_t>(q) * n + j] = y[q];
+  }
+}
+
+// Warp per row i of A_j: Lt[i][q] = -sum_k A[i][k] K[q][k];  Abar[i][:] = A[i][:] + sum_q Lt[i][q] C[q][:].
+// grid (ceil(n/8), batch), 256 threads.
+template <int PG>
+__global__ void __launch_bounds__(256) kalman_closed_loop_kernel(const float* __restrict__ A, long long a_stride,
+                                                                 const float* __restrict__ C, long long c_stride,
+                                                                 const float* __restrict__ K, float* __restrict__ Lt,
+                                                                 long long lt_stride, float* __restrict__ Abar, int n,
+                                                                 int p) {
+  constexpr int PP = 8 * PG;
+  const int b = blockIdx.y;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int i = blockIdx.x * 8 + warp;
+  if (i >= n) return;
+  const float4* Ar = reinterpret_cast<const float4*>(A + b * a_stride + static_cast<size_t>(i) * n);
+  const float* Kb = K + static_cast<size_t>(b) * p * n;
+  const float* Cb = C + b * c_stride;
+  const int n4 = n >> 2;
+  float acc[PP];
+#pragma unroll
+  for (int q = 0; q < PP; ++q) acc[q] = 0.f;
+  for (int k4 = lane; k4 < n4; k4 += 32) {
+    const float4 a = __ldg(Ar + k4);
+#pragma unroll
+    for (int q = 0; q < PP; ++q) {
+      if (q < p) {
+        const float4 kk = __ldg(reinterpret_cast<const float4*>(Kb + static_cast<size_t>(q) * n) + k4);
+        acc[q] = fmaf(a.x, kk.x, acc[q]);
+        acc[q] = fmaf(a.y, kk.y, acc[q]);
+        acc[q] = fmaf(a.z, kk.z, acc[q]);
+        acc[q] = fmaf(a.w, kk.w, acc[q]);
+      }
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < PP; ++q) {
+    if (q < p) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
+      acc[q] = -acc[q];
+    }
+  }
+  float* lt = Lt + b * lt_stride + static_cast<size_t>(i) * p;
+#pragma unroll
+  for (int q = 0; q < PP; ++q)
+    if (q < p && lane == (q & 31)) lt[q] = acc[q];
+  float4* Or = reinterpret_cast<float4*>(Abar + (static_cast<size_t>(b) * n + i) * n);
+  for (int k4 = lane; k4 < n4; k4 += 32) {
+    float4 a = __ldg(Ar + k4);
+#pragma unroll
+    for (int q = 0; q < PP; ++q) {
+      if (q < p) {
+        const float4 cc = __ldg(reinterpret_cast<const float4*>(Cb + static_cast<size_t>(q) * n) + k4);
+        a.x = fmaf(acc[q], cc.x, a.x);
+        a.y = fmaf(acc[q], cc.y, a.y);
+        a.z = fmaf(acc[q], cc.z, a.z);
+        a.w = fmaf(acc[q], cc.w, a.w);
+      }
+    }
+    Or[k4] = a;
+  }
+}
+
+// Pi_out[b][0] = Pi0[b]
+__global__ void kalman_copy_pi0_kernel(const float4* __restrict__ src, float4* __restrict__ dst, long long per_item4,
+                                       long long dst_stride4, long long total4) {
+  for (long long i = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; i < total4;
+       i += static_cast<long long>(gridDim.x) * blockDim.x) {
+    const long long b = i / per_item4, r = i - b * per_item4;
+    dst[b * dst_stride4 + r] = __ldg(src + i);
+  }
+}
+
+// fp32-FMA batched GEMM for n < 96 (BASELINE.json configs[0]): same operands and epilogues as the tcgen05 MODE 1
+// kernel.  16 x 16 output tile per CTA, one element per thread.
+__global__ void __launch_bounds__(256) bgemm_simt_kernel(const BatchedGemm g) {
+  __shared__ float sL[16][17], sR[16][17];
+  const int b = blockIdx.z;
+  const float* L = g.L + (static_cast<size_t>(g.l_row0) + static_cast<size_t>(b) * g.l_row_stride) * g.K;
+  const float* R = g.R + (static_cast<size_t>(g.r_blk0) + static_cast<size_t>(b) * g.r_blk_stride) * g.K * g.N;
+  float* D = g.D + (static_cast<size_t>(g.d_blk0) + static_cast<size_t>(b) * g.d_blk_stride) * g.M * g.N;
+  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+  const int row = blockIdx.y * 16 + ty, col = blockIdx.x * 16 + tx;
+  float acc = 0.f;
+  for (int k0 = 0; k0 < g.K; k0 += 16) {
+    sL[ty][tx] = (row < g.M && k0 + tx < g.K) ? L[static_cast<size_t>(row) * g.K + k0 + tx] : 0.f;
+    sR[ty][tx] = (k0 + ty < g.K && col < g.N) ? R[static_cast<size_t>(k0 + ty) * g.N + col] : 0.f;
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 16; ++k) acc = fmaf(sL[ty][k], sR[k][tx], acc);
+    __syncthreads();
+  }
+  if (row < g.M && col < g.N) {
+    if (g.diag != nullptr && row == col) {
+      const float d = g.diag[static_cast<long long>(b) * g.diag_stride + row];
+      acc += d * d;
+    }
+    if (g.transpose_out) D[static_cast<size_t>(col) * g.M + row] = acc; else D[static_cast<size_t>(row) * g.N + col] = acc;
+  }
+}
+
+template <typename F>
+cudaError_t dispatch_pg(int p, F&& fn) {
+  switch ((p + 7) / 8) {
+    case 1: return fn(std::integral_constant<int, 1>{});
+    case 2: return fn(std::integral_constant<int, 2>{});
+    case 3: return fn(std::integral_constant<int, 3>{});
+    case 4: return fn(std::integral_constant<int, 4>{});
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+struct KalmanWs {
+  float *Gpart, *G, *K, *Abar, *Yt;
+};
+
+size_t carve(size_t floats) { return align_up(floats * sizeof(float), 256); }
+
+}  // namespace
+
+size_t kalman_workspace_bytes(int batch, int T, int n, int p) {
+  (void)T;
+  const size_t b = batch, nn = n, pp = p;
+  return carve(kMaxKs * b * pp * nn) + 2 * carve(b * pp * nn) + 2 * carve(b * nn * nn);
+}
+
+cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned long long* launches) {
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int batch = a.batch, T = a.T, n = a.n, p = a.p;
+  const size_t b = batch, nn = n, pp = p;
+  KalmanWs w;
+  char* cur = static_cast<char*>(a.workspace);
+  w.Gpart = reinterpret_cast<float*>(cur); cur += carve(kMaxKs * b * pp * nn);
+  w.G = reinterpret_cast<float*>(cur); cur += carve(b * pp * nn);
+  w.K = reinterpret_cast<float*>(cur); cur += carve(b * pp * nn);
+  w.Abar = reinterpret_cast<float*>(cur); cur += carve(b * nn * nn);
+  w.Yt = reinterpret_cast<float*>(cur);
+
+  cudaError_t e;
+  {
+    const long long per4 = static_cast<long long>(nn * nn / 4), tot4 = per4 * batch;
+    const int blocks = static_cast<int>(std::min<long long>((tot4 + 255) / 256, 8ll * sms));
+    ProfScope prof(kProfKalmanSimt, stream);
+    kalman_copy_pi0_kernel<<<blocks, 256, 0, stream>>>(reinterpret_cast<const float4*>(a.Pi0),
+                                                       reinterpret_cast<float4*>(a.Pi_out), per4,
+                                                       per4 * (T + 1), tot4);
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    ++*launches;
+  }
+
+  const bool tc = phi_uses_tensor_cores(n);
+  const int nch = phi_pick_nch(n);
+  BatchedGemm g1{}, g2{};
+  // Yt[b] = (Abar[b] Pi_j[b])^T
+  g1.L = w.Abar; g1.l_rows = static_cast<long long>(b * nn); g1.l_row0 = 0; g1.l_row_stride = n;
+  g1.R = a.Pi_out; g1.r_blocks = batch * (T + 1); g1.r_blk_stride = T + 1;
+  g1.D = w.Yt; g1.d_blocks = batch; g1.d_blk0 = 0; g1.d_blk_stride = 1;
+  g1.count = batch; g1.M = n; g1.N = n; g1.K = n; g1.transpose_out = 1; g1.diag = nullptr; g1.diag_stride = 0;
+  // Pi_{j+1}[b] = A_j[b] Yt[b] + diag(e_j[b])^2
+  g2.L = a.A; g2.l_rows = static_cast<long long>(b * T * nn); g2.l_row_stride = T * n;
+  g2.R = w.Yt; g2.r_blocks = batch; g2.r_blk0 = 0; g2.r_blk_stride = 1;
+  g2.D = a.Pi_out; g2.d_blocks = batch * (T + 1); g2.d_blk_stride = T + 1;
+  g2.count = batch; g2.M = n; g2.N = n; g2.K = n; g2.transpose_out = 0; g2.diag_stride = static_cast<long long>(T) * n;
+  alignas(64) unsigned char maps1[512], maps2[512];
+  if (tc) {
+    if (phi_tc_maps_size() > sizeof(maps1)) return cudaErrorInvalidValue;
+    if ((e = bgemm_tc_make_maps(g1, maps1)) != cudaSuccess) return e;
+    if ((e = bgemm_tc_make_maps(g2, maps2)) != cudaSuccess) return e;
+  }
+
+  const int slabs = (n + kCpiCols - 1) / kCpiCols;
+  int KS = (2 * sms + slabs * batch - 1) / (slabs * batch);
+  KS = KS < 1 ? 1 : (KS > kMaxKs ? kMaxKs : KS);
+  if (KS > n / 4) KS = n / 4 > 0 ? n / 4 : 1;
+
+  const long long c_stride = static_cast<long long>(T) * p * n, a_stride = static_cast<long long>(T) * n * n;
+  const long long pi_stride = static_cast<long long>(T + 1) * n * n;
+  for (int j = 0; j < T; ++j) {
+    const float* Cj = a.C + static_cast<size_t>(j) * p * n;
+    const float* Aj = a.A + static_cast<size_t>(j) * n * n;
+    const float* Pij = a.Pi_out + static_cast<size_t>(j) * n * n;
+    e = dispatch_pg(p, [&](auto pg) {
+      constexpr int PG = decltype(pg)::value;
+      {
+        ProfScope prof(kProfKalmanSimt, stream);
+        kalman_cpi_kernel<PG><<<dim3(slabs, KS, batch), kCpiCols, 0, stream>>>(Cj, c_stride, Pij, pi_stride, w.Gpart,
+                                                                               batch, n, p);
+      }
+      cudaError_t ee = cudaGetLastError();
+      if (ee != cudaSuccess) return ee;
+      {
+        ProfScope prof(kProfKalmanSimt, stream);
+        kalman_gain_kernel<PG><<<batch, 256, 0, stream>>>(Cj, c_stride, a.f + static_cast<size_t>(j) * p,
+                                                          static_cast<long long>(T) * p, w.Gpart, KS, w.G, w.K, batch, n, p);
+      }
+      if ((ee = cudaGetLastError()) != cudaSuccess) return ee;
+      {
+        ProfScope prof(kProfKalmanSimt, stream);
+        kalman_closed_loop_kernel<PG><<<dim3((n + 7) / 8, batch), 256, 0, stream>>>(
+            Aj, a_stride, Cj, c_stride, w.K, a.Lt_out + static_cast<size_t>(j) * n * p,
+            static_cast<long long>(T) * n * p, w.Abar, n, p);
+      }
+      return cudaGetLastError();
+    });
+    if (e != cudaSuccess) return e;
+    *launches += 3;
+    g1.r_blk0 = j;
+    g2.l_row0 = j * n;
+    g2.d_blk0 = j + 1;
+    g2.diag = a.e + static_cast<size_t>(j) * n;
+    if (tc) {
+      if ((e = launch_bgemm_tc(g1, nch, maps1, sms, stream)) != cudaSuccess) return e;
+      if ((e = launch_bgemm_tc(g2, nch, maps2, sms, stream)) != cudaSuccess) return e;
+    } else {
+      const dim3 grid((n + 15) / 16, (n + 15) / 16, batch);
+      {
+        ProfScope prof(kProfKalmanGemm, stream);
+        bgemm_simt_kernel<<<grid, 256, 0, stream>>>(g1);
+      }
+      if ((e = cudaGetLastError()) != cudaSuccess) return e;
+      {
+        ProfScope prof(kProfKalmanGemm, stream);
+        bgemm_simt_kernel<<<grid, 256, 0, stream>>>(g2);
+      }
+      if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    }
+    *launches += 2;
+  }
+  return cudaSuccess;
+}
+
+}  // namespace ltv

@@ -42,6 +42,16 @@ bool phi_uses_tensor_cores(int n);
 size_t phi_workspace_bytes(int batch, int T, int n, int nc);
 cudaError_t launch_phi_tube(const PhiArgs& a, cudaStream_t stream, unsigned long long* launches);
 
+// Kalman recursion of eq.(13) (kalman.cu)
+struct KalmanArgs {
+  const float *A, *C, *e, *f, *Pi0;
+  float *Lt_out, *Pi_out;
+  int batch, T, n, p;
+  void* workspace;
+};
+size_t kalman_workspace_bytes(int batch, int T, int n, int p);
+cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned long long* launches);
+
 // Cluster size (CTAs per item, 1..16, any integer) for the two vector kernels.  max_active[C] = clusters of C CTAs
 // that can be resident at once (cudaOccupancyMaxActiveClusters; 0 = not launchable).  Minimises a simple
 // time model over the waves of clusters: an SM streams ~70 GB/s, the device ~6.5 TB/s (both measured).
@@ -53,7 +63,7 @@ int env_int(const char* name, int dflt);
 
 // optional per-kernel timing (ltv_profile_enable): CUDA events recorded on the launch stream around a kernel
 enum ProfClass { kProfRollout = 0, kProfAdjoint, kProfPhiLevel0, kProfPhiCombineTc, kProfPhiCombineSimt,
-                 kProfPhiFinalize, kProfNumClasses };
+                 kProfPhiFinalize, kProfKalmanGemm, kProfKalmanSimt, kProfNumClasses };
 struct ProfScope {
   ProfScope(int cls, cudaStream_t s);
   ~ProfScope();

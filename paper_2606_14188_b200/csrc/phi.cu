@@ -28,6 +28,8 @@ static int pick_nch(int n) {
   return best;
 }
 
+int phi_pick_nch(int n) { return pick_nch(n); }
+
 int phi_tile_n(int n, int nc) { return phi_uses_tensor_cores(n) ? 32 * pick_nch(nc) : 64; }
 
 size_t phi_workspace_bytes(int batch, int T, int n, int nc) {

@@ -17,6 +17,25 @@ cudaError_t phi_tc_make_maps(const PhiArgs& a, int nch, void* maps_out);
 cudaError_t launch_phi_combine_tc(const PhiArgs& a, int level, int nch, const void* maps, int num_sms,
                                   cudaStream_t stream);
 
+// Batched fp32 GEMM on the same tcgen05 3xTF32 kernel (its MODE 1): D[b] = L[b] R[b], b < count, all row-major.
+//   L  array viewed as [l_rows][K];       problem b reads rows [l_row0 + b l_row_stride, +M)
+//   R  array viewed as [r_blocks][K][N];  problem b reads block r_blk0 + b r_blk_stride
+//   D  array viewed as [d_blocks][M][N] (transpose_out: [d_blocks][N][M], holding D[b]^T); block d_blk0 + b d_blk_stride
+//   diag (may be null): adds diag[b diag_stride + i]^2 to D[b][i][i]
+// K, N multiples of 4, every base pointer 16-byte aligned.  The maps depend on the arrays and M, N, K only, so a
+// caller stepping l_row0 / r_blk0 / d_blk0 through time builds them once.
+struct BatchedGemm {
+  const float* L; long long l_rows; int l_row0, l_row_stride;
+  const float* R; int r_blocks, r_blk0, r_blk_stride;
+  float* D; int d_blocks, d_blk0, d_blk_stride;
+  int count, M, N, K;
+  int transpose_out;
+  const float* diag; long long diag_stride;
+};
+cudaError_t bgemm_tc_make_maps(const BatchedGemm& a, void* maps_out);
+cudaError_t launch_bgemm_tc(const BatchedGemm& a, int nch, const void* maps, int num_sms, cudaStream_t stream);
+int phi_pick_nch(int n);   // phi.cu
+
 void* get_encode_tiled();  // adjoint.cu
 
 }  // namespace ltv

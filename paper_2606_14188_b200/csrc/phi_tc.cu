@@ -51,7 +51,19 @@ constexpr int kKB = 32;         // k-block = one 128-byte swizzle row of fp32
 constexpr uint32_t kABytes = kTM * kKB * 4;  // 16 KB
 constexpr int kTcMaxStages = 6;
 
+// MODE 1 of the kernel: `count` independent products D[b] = L[b] R[b] (batched GEMM of the Kalman recursion,
+// eq.(13)); problem b reads rows [l_row0 + b l_row_stride, +M) of the L map, block r_blk0 + b r_blk_stride of the R
+// map and writes block d_blk0 + b d_blk_stride of the (3-D) O map
+struct TcGemm {
+  int count, M, Mt;
+  int l_row0, l_row_stride, r_blk0, r_blk_stride, d_blk0, d_blk_stride;
+  int transpose_out;       // store D^T (the O map then describes [blocks][N][M])
+  const float* diag;       // adds diag[b diag_stride + i]^2 to D[b][i][i] (E E^T with E = diag(e)); may be null
+  long long diag_stride;
+};
+
 struct TcParams {
+  TcGemm gm;
   float* phi;
   const float* w;
   float* part;
@@ -77,6 +89,18 @@ __device__ __forceinline__ float tf32_lo(float a) {
   return __uint_as_float(r);
 }
 
+struct GemmTile { int b, m_tile, n_tile; };
+// m_tile fastest: CTAs running at the same time share the right-operand tile out of L2
+__device__ __forceinline__ GemmTile gemm_decode(const TcGemm& gm, int NTiles, long long idx) {
+  GemmTile t;
+  int rem = static_cast<int>(idx);
+  t.m_tile = rem % gm.Mt;
+  rem /= gm.Mt;
+  t.n_tile = rem % NTiles;
+  t.b = rem / NTiles;
+  return t;
+}
+
 template <int NCH, bool PAIR>
 struct TcShape {
   static constexpr int NT = 32 * NCH;
@@ -94,7 +118,7 @@ struct TcShape {
 // DBG = compile-time knock-out mask (experiments only, -DLTV_TC_EXPERIMENTS; production is DBG = 0):
 // 1 no stores, 2 no R split, 4 no L split, 16 one MMA of three, 128 no TMEM stores, 512 no tube FMAs,
 // 1024 no proxy fence, 4096 clock traces of CTA 0.
-template <int NCH, bool PAIR, int DBG>
+template <int NCH, bool PAIR, int DBG, int MODE>
 __global__ void __launch_bounds__(kTcThreads, 1)
 phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL,
                       const __grid_constant__ CUtensorMap mapR, const __grid_constant__ CUtensorMap mapO) {
@@ -171,12 +195,20 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
     int rs = 0;
     uint32_t eph = 1;   // parity of rempty[rs] to wait for (the first pass over the ring does not block)
     for (long long idx = unit; idx < g.total; idx += nunits) {
-      const PhiTile t = phi_decode(g, idx);
-      const long long item = static_cast<long long>(t.b) * g.P;
-      const int rowL = static_cast<int>((item + phi_colbase(g.T, t.mid)) * n) + t.m_tile * (kTM * NCTA) +
-                       static_cast<int>(rank) * kTM;
-      const int blkR = static_cast<int>(item + phi_colbase(g.T, t.s) + (t.mid - t.s - 1));
-      const int j0 = t.n_tile * NT + static_cast<int>(rank) * NH;
+      int rowL, blkR, j0;
+      if (MODE == 0) {
+        const PhiTile t = phi_decode(g, idx);
+        const long long item = static_cast<long long>(t.b) * g.P;
+        rowL = static_cast<int>((item + phi_colbase(g.T, t.mid)) * n) + t.m_tile * (kTM * NCTA) +
+               static_cast<int>(rank) * kTM;
+        blkR = static_cast<int>(item + phi_colbase(g.T, t.s) + (t.mid - t.s - 1));
+        j0 = t.n_tile * NT + static_cast<int>(rank) * NH;
+      } else {
+        const GemmTile t = gemm_decode(p.gm, g.NT, idx);
+        rowL = p.gm.l_row0 + t.b * p.gm.l_row_stride + t.m_tile * (kTM * NCTA) + static_cast<int>(rank) * kTM;
+        blkR = p.gm.r_blk0 + t.b * p.gm.r_blk_stride;
+        j0 = t.n_tile * NT + static_cast<int>(rank) * NH;
+      }
       for (int kb = 0; kb < nkb; ++kb, ++it) {
         LTV_TRACE(0, it, 0)
         mbar_wait(&rempty[rs], eph);
@@ -308,8 +340,65 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
     uint32_t lt = 0;
     for (long long idx = unit; idx < g.total; idx += nunits, ++lt) {
       if (warp == 4) { LTV_TRACE(4, lt, 0) }
-      const PhiTile t = phi_decode(g, idx);
       const uint32_t acc = lt & 1;
+      if (MODE == 1) {
+        // ------------------------------------------------------------ batched GEMM epilogue (Kalman recursion)
+        const GemmTile t = gemm_decode(p.gm, g.NT, idx);
+        const int j0 = t.n_tile * NT;
+        const int rbase = t.m_tile * (kTM * NCTA) + static_cast<int>(rank) * kTM + wq * 32;
+        const int rr = rbase + lane;                 // row of D[b] held by this thread
+        const int rows_valid = p.gm.M - rbase;
+        const int oblk = p.gm.d_blk0 + t.b * p.gm.d_blk_stride;
+        const bool tr = p.gm.transpose_out != 0;
+        float dd = 0.f;
+        if (p.gm.diag != nullptr && rr < p.gm.M) {
+          const float d = __ldg(p.gm.diag + static_cast<long long>(t.b) * p.gm.diag_stride + rr);
+          dd = d * d;
+        }
+        mbar_wait(&tfull[acc], (lt >> 1) & 1);
+        tc_fence_after();
+        const uint32_t taddr = tmem_base + (static_cast<uint32_t>(wq * 32) << 16) + acc * NT;
+        uint32_t v[2][32];
+        tmem_ld_32x32(taddr, v[0]);
+#pragma unroll
+        for (int cc = 0; cc < NCH; ++cc) {
+          uint32_t (&vc)[32] = v[cc & 1];
+          tmem_ld_wait();
+          if (cc + 1 < NCH) tmem_ld_32x32(taddr + (cc + 1) * 32, v[(cc + 1) & 1]);
+          const int jc = j0 + cc * 32;
+          if (jc >= nc || rows_valid <= 0) continue;
+          if (rr >= jc && rr < jc + 32) {
+#pragma unroll
+            for (int e = 0; e < 32; ++e)
+              if (jc + e == rr) vc[e] = __float_as_uint(__uint_as_float(vc[e]) + dd);
+          }
+          if (lane == 0) tma_store_wait_read<0>();
+          __syncwarp();
+          if (!tr) {
+#pragma unroll
+            for (int e = 0; e < 8; ++e)
+              *reinterpret_cast<uint4*>(sbox + lane * 128 + ((e ^ (lane & 7)) << 4)) =
+                  make_uint4(vc[4 * e], vc[4 * e + 1], vc[4 * e + 2], vc[4 * e + 3]);
+          } else {
+            // box row e = column jc + e of D, position `lane` = row rbase + lane of D: the transposed tile
+#pragma unroll
+            for (int e = 0; e < 32; ++e)
+              *reinterpret_cast<uint32_t*>(sbox + e * 128 + ((((lane >> 2) ^ (e & 7)) << 4) | ((lane & 3) << 2))) = vc[e];
+          }
+          fence_proxy_async_smem();
+          __syncwarp();
+          if (lane == 0) {
+            // rows / columns beyond the block are clipped by the 3-D tensor map
+            if (!tr) tma_store_3d(&mapO, jc, rbase, oblk, sbox); else tma_store_3d(&mapO, rbase, jc, oblk, sbox);
+            tma_store_commit();
+          }
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) arrive_leader(&tempty[acc]);
+        continue;
+      }
+      const PhiTile t = phi_decode(g, idx);
       const int j0 = t.n_tile * NT;
       float* wb = wbuf + acc * NT;
       for (int j = etid; j < NT; j += 128)
@@ -395,7 +484,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
   }
 }
 
-template <int NCH, bool PAIR, int DBG>
+template <int NCH, bool PAIR, int DBG, int MODE = 0>
 cudaError_t launch_tc_dbg(const TcParams& p, const TcMaps& maps, int num_sms, cudaStream_t stream) {
   using S = TcShape<NCH, PAIR>;
   TcParams q = p;
@@ -404,7 +493,7 @@ cudaError_t launch_tc_dbg(const TcParams& p, const TcMaps& maps, int num_sms, cu
   if (st < 2) return cudaErrorInvalidConfiguration;
   q.stages = st;
   const uint32_t smem = 1024u + st * S::kRawBytes + kConvStages * S::kBBytes + S::kMisc;
-  auto kern = phi_combine_tc_kernel<NCH, PAIR, DBG>;
+  auto kern = phi_combine_tc_kernel<NCH, PAIR, DBG, MODE>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e != cudaSuccess) return e;
   const long long max_units = num_sms / S::NCTA;
@@ -421,7 +510,7 @@ cudaError_t launch_tc_dbg(const TcParams& p, const TcMaps& maps, int num_sms, cu
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  ProfScope prof(kProfPhiCombineTc, stream);
+  ProfScope prof(MODE == 0 ? kProfPhiCombineTc : kProfKalmanGemm, stream);
   return cudaLaunchKernelEx(&cfg, kern, q, maps.L, maps.R, maps.O);
 }
 
@@ -516,6 +605,76 @@ cudaError_t launch_phi_combine_tc(const PhiArgs& a, int level, int nch, const vo
   p.g = pair ? g2 : g1;
 #define LTV_NCH_CASE(N) \
   case N: return pair ? launch_tc<N, true>(p, m, num_sms, stream) : launch_tc<N, false>(p, m, num_sms, stream);
+  switch (nch) {
+    LTV_NCH_CASE(2) LTV_NCH_CASE(3) LTV_NCH_CASE(4) LTV_NCH_CASE(5)
+    default: return cudaErrorInvalidValue;
+  }
+#undef LTV_NCH_CASE
+}
+
+// ---------------------------------------------------------------------------------------- batched GEMM (MODE 1)
+cudaError_t bgemm_tc_make_maps(const BatchedGemm& a, void* maps_out) {
+  EncodeTiledFn enc = reinterpret_cast<EncodeTiledFn>(get_encode_tiled());
+  if (!enc) return cudaErrorNotSupported;
+  TcMaps* m = static_cast<TcMaps*>(maps_out);
+  const cuuint64_t M = a.M, N = a.N, K = a.K;
+  const cuuint32_t estr[3] = {1, 1, 1};
+  {
+    const cuuint64_t dims[2] = {K, static_cast<cuuint64_t>(a.l_rows)};
+    const cuuint64_t strides[1] = {K * 4};
+    const cuuint32_t box[2] = {kKB, kTM};
+    if (enc(&m->L, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(a.L), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+  }
+  {
+    const cuuint64_t dims[3] = {N, K, static_cast<cuuint64_t>(a.r_blocks)};
+    const cuuint64_t strides[2] = {N * 4, K * N * 4};
+    const cuuint32_t box[3] = {32, kKB, 1};
+    if (enc(&m->R, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float*>(a.R), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+  }
+  {
+    // D[b] is M x N, stored as it is or transposed (N x M); either way one block per problem, clipped per block
+    const cuuint64_t cols = a.transpose_out ? M : N, rows = a.transpose_out ? N : M;
+    const cuuint64_t dims[3] = {cols, rows, static_cast<cuuint64_t>(a.d_blocks)};
+    const cuuint64_t strides[2] = {cols * 4, rows * cols * 4};
+    const cuuint32_t box[3] = {32, 32, 1};
+    if (enc(&m->O, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, a.D, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+  }
+  return cudaSuccess;
+}
+
+cudaError_t launch_bgemm_tc(const BatchedGemm& a, int nch, const void* maps, int num_sms, cudaStream_t stream) {
+  if (a.count <= 0) return cudaSuccess;
+  TcParams p{};
+  const TcMaps& m = *static_cast<const TcMaps*>(maps);
+  const int Mt1 = (a.M + kTM - 1) / kTM, Mt2 = (a.M + 2 * kTM - 1) / (2 * kTM);
+  const int mode = env_int("TC_PAIR", -1);
+  const bool pair = (mode == 1) || (mode == -1 && 2 * Mt2 * 100 <= Mt1 * 108);
+  const int nt = 32 * nch;
+  p.g = PhiGeom{};
+  p.g.n = a.K;
+  p.g.nc = a.N;
+  p.g.tm = pair ? 2 * kTM : kTM;
+  p.g.tn = nt;
+  p.g.NT = (a.N + nt - 1) / nt;
+  p.gm.count = a.count; p.gm.M = a.M; p.gm.Mt = pair ? Mt2 : Mt1;
+  p.gm.l_row0 = a.l_row0; p.gm.l_row_stride = a.l_row_stride;
+  p.gm.r_blk0 = a.r_blk0; p.gm.r_blk_stride = a.r_blk_stride;
+  p.gm.d_blk0 = a.d_blk0; p.gm.d_blk_stride = a.d_blk_stride;
+  p.gm.transpose_out = a.transpose_out;
+  p.gm.diag = a.diag; p.gm.diag_stride = a.diag_stride;
+  p.g.total = static_cast<long long>(p.gm.Mt) * p.g.NT * a.count;
+#define LTV_NCH_CASE(N_)                                                              \
+  case N_: return pair ? launch_tc_dbg<N_, true, 0, 1>(p, m, num_sms, stream)         \
+                       : launch_tc_dbg<N_, false, 0, 1>(p, m, num_sms, stream);
   switch (nch) {
     LTV_NCH_CASE(2) LTV_NCH_CASE(3) LTV_NCH_CASE(4) LTV_NCH_CASE(5)
     default: return cudaErrorInvalidValue;

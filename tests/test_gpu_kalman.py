@@ -1,0 +1,119 @@
+"""GPU parity of ltv_scan_kalman_gains (eq.(13)) against the pinned fp64 oracle, through the C-ABI
+binding.  Tolerance: max|err| / max|ref| <= 1e-4 per output tensor (3xTF32 products, fp32 Cholesky), as north_star
+states for the rest of the path."""
+import numpy as np
+import pytest
+
+from oracle import ltv_oracle as O
+from workloads import config, dense_random, generate, observation_model
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def L():
+    import torch
+
+    assert torch.cuda.is_available(), "GPU tests need a GPU (no CPU fallback)"
+    import __graft_entry__ as G
+
+    G.build()
+    import paper_2606_14188_b200 as lib
+
+    return lib
+
+
+def _run(L, A, M):
+    import torch
+
+    d = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (A, M["C"], M["e"], M["f"], M["Pi0"])]
+    Lt, Pi = L.ltv_scan_kalman_gains(*d)
+    torch.cuda.synchronize()
+    return Lt.cpu().numpy(), Pi.cpu().numpy()
+
+
+def _check(L, A, M):
+    Lt, Pi = _run(L, A, M)
+    Pi_ref, Lt_ref = O.kalman_recursion(A, M["C"], M["e"], M["f"], M["Pi0"])
+    assert np.array_equal(Pi[:, 0], M["Pi0"])
+    assert O.rel_err(Pi, Pi_ref) <= TOL
+    assert O.rel_err(Lt, Lt_ref) <= TOL
+    # every step on its own scale too (Pi_j shrinks by orders of magnitude along the horizon once observations come in)
+    for j in range(Pi.shape[1]):
+        assert O.rel_err(Pi[:, j], Pi_ref[:, j]) <= TOL, j
+    for j in range(Lt.shape[1]):
+        assert O.rel_err(Lt[:, j], Lt_ref[:, j]) <= TOL, j
+    sym = np.max(np.abs(Pi - np.swapaxes(Pi, -1, -2))) / np.max(np.abs(Pi_ref))
+    assert sym <= TOL
+    return Lt, Pi
+
+
+@pytest.mark.parametrize("n,T,batch,p,kind", [(48, 6, 2, 3, "dense"),     # fp32-FMA products (n < 96)
+                                              (48, 16, 1, 6, "track"),    # C1 shape
+                                              (128, 5, 3, 6, "dense"),    # one 128-row tile, no ragged edge
+                                              (132, 4, 2, 1, "dense"),    # ragged m-tile and k-block, p = 1
+                                              (300, 6, 3, 6, "track"),    # C2 shape: 3 m-tiles, 2 n-tiles of 160
+                                              (164, 3, 2, 32, "dense"),   # widest observation
+                                              (500, 3, 1, 12, "dense"),   # CTA-pair tiles (256 rows), ragged second pair
+                                              (600, 3, 2, 9, "dense")])   # C3 shape
+def test_kalman_dense_random(L, n, T, batch, p, kind):
+    W = dense_random(batch, T, n, 1, seed=7 * n + p, scale=0.4)
+    M = observation_model(batch, T, n, p, seed=3 * n + p, kind=kind)
+    _check(L, W.A, M)
+
+
+@pytest.mark.parametrize("ci,T", [(0, 16), (1, 6), (2, 4)])
+def test_kalman_mass_spring(L, ci, T):
+    """BASELINE.json rope / cloth Jacobians with tracked-point observations (p = 6)."""
+    cfg = config(ci, batch=2 if ci else 1, T=T)
+    W = generate(cfg)
+    n = W.A.shape[-1]
+    M = observation_model(W.A.shape[0], T, n, 6, seed=100 + ci, kind="track")
+    _check(L, W.A, M)
+
+
+def test_kalman_without_information_is_the_lyapunov_recursion(L):
+    """C = 0: no gain, Pi_{j+1} = A Pi A^T + E E^T; Lt must come out as exact zeros."""
+    W = dense_random(2, 5, 132, 1, seed=5, scale=0.4)
+    M = observation_model(2, 5, 132, 4, seed=6, kind="dense")
+    M["C"] = np.zeros_like(M["C"])
+    Lt, Pi = _check(L, W.A, M)
+    assert np.all(Lt == 0.0)
+
+
+def test_kalman_gains_feed_the_observer_response(L):
+    """NEXT-3 -> NEXT-1 on the device: the gains of (13) go straight into the closed-loop propagation of (14)."""
+    import torch
+
+    n, T, batch, p = 132, 6, 2, 6
+    W = dense_random(batch, T, n, 1, seed=9, scale=0.4)
+    M = observation_model(batch, T, n, p, seed=10, kind="dense")
+    d = [torch.from_numpy(a).cuda() for a in (W.A, M["C"], M["e"], M["f"], M["Pi0"])]
+    Lt, Pi = L.ltv_scan_kalman_gains(*d)
+    phi, r = L.ltv_scan_observer_response(d[0], Lt, d[1], torch.from_numpy(W.w).cuda())
+    torch.cuda.synchronize()
+    _, Lt_ref = O.kalman_recursion(W.A, M["C"], M["e"], M["f"], M["Pi0"])
+    X, Y = O.observer_response(W.A, Lt_ref, M["C"])
+    perm = [O.packed_index(t, s) for s in range(T - 1) for t in range(s + 1, T)]
+    phi = phi.cpu().numpy()
+    assert O.rel_err(phi[..., :n], X[:, perm]) <= TOL
+    assert O.rel_err(phi[..., n:n + p], Y[:, perm]) <= TOL
+
+
+def test_kalman_argument_errors(L):
+    import torch
+
+    A = torch.zeros((1, 2, 48, 48), device="cuda")
+    C = torch.zeros((1, 2, 33, 48), device="cuda")
+    with pytest.raises(L.LtvError) as ei:
+        L.ltv_scan_kalman_gains(A, C, torch.ones((1, 2, 48), device="cuda"), torch.ones((1, 2, 33), device="cuda"),
+                                torch.zeros((1, 48, 48), device="cuda"),
+                                workspace=torch.empty(1 << 20, device="cuda", dtype=torch.uint8))
+    assert ei.value.status == 3   # LTV_ERR_UNSUPPORTED_SHAPE: p > 32
+    C = torch.zeros((1, 2, 4, 48), device="cuda")
+    with pytest.raises(L.LtvError) as ei:
+        L.ltv_scan_kalman_gains(A, C, torch.ones((1, 2, 48), device="cuda"), torch.ones((1, 2, 4), device="cuda"),
+                                torch.zeros((1, 48, 48), device="cuda"),
+                                workspace=torch.empty(256, device="cuda", dtype=torch.uint8))
+    assert ei.value.status == 5   # LTV_ERR_WORKSPACE_TOO_SMALL
