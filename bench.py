@@ -40,6 +40,8 @@ def parse():
     ap.add_argument("--batch", type=int, default=0, help="items per GPU (0 = the config's own; config 4 sweeps 64/256/1024)")
     ap.add_argument("--observer", type=int, default=0, metavar="P",
                     help="also time ltv_scan_observer_response (NEXT-1, eq.(14)) with P measurement rows")
+    ap.add_argument("--kalman", type=int, default=0, metavar="P",
+                    help="also time ltv_scan_kalman_gains (NEXT-3, eq.(13)) with P observation rows")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-items", type=int, default=0, help="items in the CPU-oracle sample (0 = auto)")
@@ -319,6 +321,37 @@ def main():
         del phio, wso
         phi = None
 
+    # ---- NEXT-3: Kalman recursion (13) on the same A with the tracked-point observation stand-in, timed alone
+    kalman = None
+    if args.kalman > 0:
+        from workloads import observation_model
+        pk_ = args.kalman
+        Mobs = observation_model(batch, T, n, pk_, seed=777 + rank, kind="track")
+        kd = [torch.from_numpy(Mobs[k]).to(dev) for k in ("C", "e", "f", "Pi0")]
+        if phi_on:
+            phi = None
+        torch.cuda.empty_cache()
+        Lto = torch.empty((batch, T, n, pk_), device=dev)
+        Pio = torch.empty((batch, T + 1, n, n), device=dev)
+        wsk = torch.empty(max(16, L.ltv_scan_workspace_bytes(L.LTV_OP_KALMAN_GAINS, batch, T, n, pk_)),
+                          dtype=torch.uint8, device=dev)
+        for _ in range(3):
+            L.ltv_scan_kalman_gains(d["A"], *kd, Lt_out=Lto, Pi_out=Pio, workspace=wsk)
+        k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        k0.record()
+        for _ in range(args.steps):
+            L.ltv_scan_kalman_gains(d["A"], *kd, Lt_out=Lto, Pi_out=Pio, workspace=wsk)
+        k1.record()
+        barrier()
+        kms = k0.elapsed_time(k1) / args.steps
+        kalman = dict(p=pk_, ms=kms, recursions_per_s=batch * world / (kms * 1e-3),
+                      steps_per_s=batch * world * T / (kms * 1e-3),
+                      issued_tf32_tflops=3.0 * 2.0 * 2.0 * n ** 3 * T * batch / (kms * 1e-3) / 1e12,
+                      note="ltv_scan_kalman_gains alone: T sequential steps of (13) over the whole batch, two n^3 "
+                           "products per step and item (3xTF32 on tcgen05 for n >= 96)")
+        del Lto, Pio, wsk, kd
+
     # ---- end to end through the C-ABI with host buffers
     e2e = None
     if not args.no_e2e:
@@ -375,7 +408,7 @@ def main():
                                     f"working set (A {a_gb * 1e3:.2f} MB) fits L2: warm-cache, latency-bound case"),
                                 phi_layout="column-packed"),
                     clocks=sampler.result(), e2e=e2e, gpu_launches=int(launches), roofline=roof,
-                    cpu_baseline=cpu, kernel_ms_per_step=share, vector_scans=extra, observer=observer,
+                    cpu_baseline=cpu, kernel_ms_per_step=share, vector_scans=extra, observer=observer, kalman=kalman,
                     rollouts_per_s=extra.get("rollout", {}).get("per_s"),
                     adjoints_per_s=extra.get("adjoint", {}).get("per_s"))
         print(json.dumps(line), flush=True)

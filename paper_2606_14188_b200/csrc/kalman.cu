@@ -3,7 +3,7 @@
 //     Pi_0 = Xi Xi^T;   L_{j+1} = -(F_j F_j^T + C_j Pi_j C_j^T)^{-1} C_j Pi_j A_j^T;
 //     Pi_{j+1} = E_j E_j^T + A_j Pi_j A_j^T + A_j Pi_j C_j^T L_{j+1}
 // computed per step j, for all items at once, as
-//     G = C_j Pi_j                     [p,n]   kalman_cpi_kernel      (split over k, fixed-order partial sums)
+//     G = C_j Pi_j                     [p,n]   kalman_cpi_kernel      (rows of the symmetric Pi_j against the p rows of C_j)
 //     S = F F^T + G C_j^T, K = S^{-1}G [p,n]   kalman_gain_kernel     (Cholesky of the p x p innovation covariance)
 //     Lt_j = L_{j+1}^T = -A_j K^T      [n,p]   kalman_closed_loop_kernel (A_j streams through once: the same pass
 //     Abar_j = A_j + Lt_j C_j          [n,n]                           writes the closed-loop matrix of eq.(14))
@@ -29,74 +29,125 @@ namespace ltv {
 
 namespace {
 
-constexpr int kCpiCols = 128;   // columns of Pi per CTA in kalman_cpi_kernel
-constexpr int kMaxKs = 8;       // at most this many k-splits of G = C Pi
+constexpr int kRowWarps = 8;   // warps per CTA of the row kernels
+// measured on B200 (C2 p = 6, C4 p = 12; the variants differ by < 10 %): p <= 8 runs best with two CTAs per SM and the
+// loop not unrolled, wider p with one CTA per SM and two passes in flight
+template <int PG> struct RowCfg {
+  static constexpr int kRows = PG <= 2 ? 4 : 2;
+  static constexpr int kUnroll = PG == 1 ? 1 : 2;
+  static constexpr int kMinBlocks = PG == 1 ? 2 : 1;
+};
 
-// G_part[ks][b][q][j] = sum_{k in split ks} C[b][q][k] Pi[b][k][j].   grid (ceil(n/128), KS, batch), 128 threads.
-template <int PG>
-__global__ void __launch_bounds__(kCpiCols) kalman_cpi_kernel(const float* __restrict__ C, long long c_stride,
-                                                              const float* __restrict__ Pi, long long pi_stride,
-                                                              float* __restrict__ Gpart, int batch, int n, int p) {
+// ROWS rows of a row-major matrix against p vectors V[q][0..n) (global memory, L1-resident: every warp reads the same
+// ones): acc[r][q] = sum_k row_r[k] V[q][k], complete in every lane.  Lane = float4 column, stride 32; ROWS
+// independent 128-bit loads in flight per lane and pass, the vector loads amortised over the ROWS rows.
+template <int PG, int ROWS>
+__device__ __forceinline__ void row_dots(const float4* const (&rows)[ROWS], const float* __restrict__ V, int n4, int p,
+                                         int lane, float (&acc)[ROWS][8 * PG]) {
   constexpr int PP = 8 * PG;
-  const int b = blockIdx.z, ks = blockIdx.y, KS = gridDim.y;
-  const int j = blockIdx.x * kCpiCols + threadIdx.x;
-  const int kq = ((n / 4 + KS - 1) / KS) * 4;   // k per split, multiple of 4
-  const int k0 = ks * kq, k1 = min(n, k0 + kq);
-  const float* Cb = C + b * c_stride;
-  const float* Pb = Pi + b * pi_stride;
-  float acc[PP];
 #pragma unroll
-  for (int q = 0; q < PP; ++q) acc[q] = 0.f;
-  if (j < n) {
-    for (int k = k0; k < k1; k += 4) {
-      const float x0 = __ldg(Pb + static_cast<size_t>(k) * n + j);
-      const float x1 = __ldg(Pb + static_cast<size_t>(k + 1) * n + j);
-      const float x2 = __ldg(Pb + static_cast<size_t>(k + 2) * n + j);
-      const float x3 = __ldg(Pb + static_cast<size_t>(k + 3) * n + j);
+  for (int r = 0; r < ROWS; ++r)
 #pragma unroll
-      for (int q = 0; q < PP; ++q) {
-        if (q < p) {
-          const float4 c4 = __ldg(reinterpret_cast<const float4*>(Cb + static_cast<size_t>(q) * n + k));
-          acc[q] = fmaf(c4.x, x0, acc[q]);
-          acc[q] = fmaf(c4.y, x1, acc[q]);
-          acc[q] = fmaf(c4.z, x2, acc[q]);
-          acc[q] = fmaf(c4.w, x3, acc[q]);
+    for (int q = 0; q < PP; ++q) acc[r][q] = 0.f;
+  // no branch on q < p inside the loop: behind a branch every vector load waits for the previous one's FMAs (measured:
+  // 6 serialised L2 round trips per pass).  Accumulators q >= p re-read vector p - 1 and are discarded.
+  const float4* V4 = reinterpret_cast<const float4*>(V);
+  size_t voff[PP];
+#pragma unroll
+  for (int q = 0; q < PP; ++q) voff[q] = static_cast<size_t>(min(q, p - 1)) * n4;
+#pragma unroll RowCfg<PG>::kUnroll
+  for (int k4 = lane; k4 < n4; k4 += 32) {
+    float4 a[ROWS];
+#pragma unroll
+    for (int r = 0; r < ROWS; ++r) a[r] = __ldg(rows[r] + k4);
+#pragma unroll
+    for (int qg = 0; qg < PP; qg += 8) {   // eight vector loads in flight at a time
+      float4 v[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) v[q] = __ldg(V4 + voff[qg + q] + k4);
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+#pragma unroll
+        for (int r = 0; r < ROWS; ++r) {
+          acc[r][qg + q] = fmaf(a[r].x, v[q].x, acc[r][qg + q]);
+          acc[r][qg + q] = fmaf(a[r].y, v[q].y, acc[r][qg + q]);
+          acc[r][qg + q] = fmaf(a[r].z, v[q].z, acc[r][qg + q]);
+          acc[r][qg + q] = fmaf(a[r].w, v[q].w, acc[r][qg + q]);
         }
       }
     }
-    float* out = Gpart + ((static_cast<size_t>(ks) * batch + b) * p) * n + j;
+  }
 #pragma unroll
-    for (int q = 0; q < PP; ++q)
-      if (q < p) out[static_cast<size_t>(q) * n] = acc[q];
+  for (int q = 0; q < PP; ++q) {
+    if (q < p) {
+#pragma unroll
+      for (int r = 0; r < ROWS; ++r)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc[r][q] += __shfl_xor_sync(0xffffffffu, acc[r][q], o);
+    }
   }
 }
 
-// One CTA per item: G = sum of the k-split partials (fixed order), S = diag(f)^2 + G C^T, Cholesky S = R R^T,
-// K = S^{-1} G.  256 threads; shared memory: S [32][33].
+// G[b][q][j] = sum_k Pi[b][j][k] C[b][q][k]  (= (C Pi)[q][j]: Pi is symmetric, so its ROW j serves as column j and the
+// loads are contiguous).  Warp = ROWS rows of Pi; grid (ceil(n / (8 ROWS)), batch), 256 threads.
+template <int PG, int ROWS>
+__global__ void __launch_bounds__(32 * kRowWarps, RowCfg<PG>::kMinBlocks) kalman_cpi_kernel(const float* __restrict__ C, long long c_stride,
+                                                                    const float* __restrict__ Pi, long long pi_stride,
+                                                                    float* __restrict__ G, int n, int p) {
+  const int b = blockIdx.y;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int j0 = (blockIdx.x * kRowWarps + warp) * ROWS;
+  if (j0 >= n) return;
+  const int n4 = n >> 2;
+  const float4* rows[ROWS];
+#pragma unroll
+  for (int r = 0; r < ROWS; ++r)
+    rows[r] = reinterpret_cast<const float4*>(Pi + b * pi_stride + static_cast<size_t>(min(j0 + r, n - 1)) * n);
+  float acc[ROWS][8 * PG];
+  row_dots<PG, ROWS>(rows, C + b * c_stride, n4, p, lane, acc);
+  float* Gb = G + static_cast<size_t>(b) * p * n;
+#pragma unroll
+  for (int q = 0; q < 8 * PG; ++q) {
+    if (q < p && lane == (q & 31)) {
+#pragma unroll
+      for (int r = 0; r < ROWS; ++r)
+        if (j0 + r < n) Gb[static_cast<size_t>(q) * n + j0 + r] = acc[r][q];
+    }
+  }
+}
+
+// One CTA per item: S = diag(f)^2 + G C^T (lower triangle; warp per entry), Cholesky S = R R^T (warp 0, lane = row),
+// K = S^{-1} G (thread per column).  256 threads; shared memory: S [32][33].
 template <int PG>
 __global__ void __launch_bounds__(256) kalman_gain_kernel(const float* __restrict__ C, long long c_stride,
                                                           const float* __restrict__ f, long long f_stride,
-                                                          const float* __restrict__ Gpart, int KS, float* __restrict__ G,
-                                                          float* __restrict__ K, int batch, int n, int p) {
+                                                          const float* __restrict__ G, float* __restrict__ K, int n,
+                                                          int p) {
   constexpr int PP = 8 * PG;
   __shared__ float S[32][33];
   const int b = blockIdx.x;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const float* Cb = C + b * c_stride;
-  float* Gb = G + static_cast<size_t>(b) * p * n;
+  const float4* C4 = reinterpret_cast<const float4*>(C + b * c_stride);
+  const float* Gb = G + static_cast<size_t>(b) * p * n;
+  const float4* G4 = reinterpret_cast<const float4*>(Gb);
   float* Kb = K + static_cast<size_t>(b) * p * n;
-  for (int i = threadIdx.x; i < p * n; i += 256) {
-    float s = 0.f;
-    for (int ks = 0; ks < KS; ++ks) s += __ldg(Gpart + (static_cast<size_t>(ks) * batch + b) * p * n + i);
-    Gb[i] = s;
-  }
-  __syncthreads();
-  // S[q][r], r <= q (G C^T is symmetric because Pi is; only the lower triangle is formed and used)
+  const int n4 = n >> 2;
   for (int pr = warp; pr < p * p; pr += 8) {
     const int q = pr / p, r = pr % p;
     if (r > q) continue;
-    float s = 0.f;
-    for (int k = lane; k < n; k += 32) s = fmaf(Gb[static_cast<size_t>(q) * n + k], __ldg(Cb + static_cast<size_t>(r) * n + k), s);
+    float s0 = 0.f, s1 = 0.f;
+    int k4 = lane;
+    for (; k4 + 32 < n4; k4 += 64) {
+      const float4 g0 = __ldg(G4 + static_cast<size_t>(q) * n4 + k4), c0 = __ldg(C4 + static_cast<size_t>(r) * n4 + k4);
+      const float4 g1 = __ldg(G4 + static_cast<size_t>(q) * n4 + k4 + 32), c1 = __ldg(C4 + static_cast<size_t>(r) * n4 + k4 + 32);
+      s0 = fmaf(g0.x, c0.x, fmaf(g0.y, c0.y, fmaf(g0.z, c0.z, fmaf(g0.w, c0.w, s0))));
+      s1 = fmaf(g1.x, c1.x, fmaf(g1.y, c1.y, fmaf(g1.z, c1.z, fmaf(g1.w, c1.w, s1))));
+    }
+    if (k4 < n4) {
+      const float4 g0 = __ldg(G4 + static_cast<size_t>(q) * n4 + k4), c0 = __ldg(C4 + static_cast<size_t>(r) * n4 + k4);
+      s0 = fmaf(g0.x, c0.x, fmaf(g0.y, c0.y, fmaf(g0.z, c0.z, fmaf(g0.w, c0.w, s0))));
+    }
+    float s = s0 + s1;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     if (lane == 0) {
@@ -109,7 +160,6 @@ __global__ void __launch_bounds__(256) kalman_gain_kernel(const float* __restric
   }
   __syncthreads();
   if (warp == 0) {
-    // right-looking Cholesky, lane = row
     for (int k = 0; k < p; ++k) {
       const float d = sqrtf(S[k][k]);
       __syncwarp();
@@ -125,7 +175,7 @@ __global__ void __launch_bounds__(256) kalman_gain_kernel(const float* __restric
   for (int j = threadIdx.x; j < n; j += 256) {
     float y[PP];
 #pragma unroll
-    for (int q = 0; q < PP; ++q) y[q] = (q < p) ? Gb[static_cast<size_t>(q) * n + j] : 0.f;
+    for (int q = 0; q < PP; ++q) y[q] = (q < p) ? __ldg(Gb + static_cast<size_t>(q) * n + j) : 0.f;
     // R y' = g (forward), R^T k = y' (backward)
 #pragma unroll
     for (int q = 0; q < PP; ++q) {
@@ -152,65 +202,67 @@ __global__ void __launch_bounds__(256) kalman_gain_kernel(const float* __restric
   }
 }
 
-// Warp per row i of A_j: Lt[i][q] = -sum_k A[i][k] K[q][k];  Abar[i][:] = A[i][:] + sum_q Lt[i][q] C[q][:].
-// grid (ceil(n/8), batch), 256 threads.
-template <int PG>
-__global__ void __launch_bounds__(256) kalman_closed_loop_kernel(const float* __restrict__ A, long long a_stride,
-                                                                 const float* __restrict__ C, long long c_stride,
-                                                                 const float* __restrict__ K, float* __restrict__ Lt,
-                                                                 long long lt_stride, float* __restrict__ Abar, int n,
-                                                                 int p) {
+// Warp = ROWS rows i of A_j: Lt[i][q] = -sum_k A[i][k] K[q][k];  Abar[i][:] = A[i][:] + sum_q Lt[i][q] C[q][:].
+// grid (ceil(n / (8 ROWS)), batch), 256 threads.
+template <int PG, int ROWS>
+__global__ void __launch_bounds__(32 * kRowWarps, RowCfg<PG>::kMinBlocks) kalman_closed_loop_kernel(
+    const float* __restrict__ A, long long a_stride, const float* __restrict__ C, long long c_stride,
+    const float* __restrict__ K, float* __restrict__ Lt, long long lt_stride, float* __restrict__ Abar, int n, int p) {
   constexpr int PP = 8 * PG;
   const int b = blockIdx.y;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int i = blockIdx.x * 8 + warp;
-  if (i >= n) return;
-  const float4* Ar = reinterpret_cast<const float4*>(A + b * a_stride + static_cast<size_t>(i) * n);
-  const float* Kb = K + static_cast<size_t>(b) * p * n;
-  const float* Cb = C + b * c_stride;
+  const int i0 = (blockIdx.x * kRowWarps + warp) * ROWS;
+  if (i0 >= n) return;
   const int n4 = n >> 2;
-  float acc[PP];
+  const float4* rows[ROWS];
 #pragma unroll
-  for (int q = 0; q < PP; ++q) acc[q] = 0.f;
-  for (int k4 = lane; k4 < n4; k4 += 32) {
-    const float4 a = __ldg(Ar + k4);
-#pragma unroll
-    for (int q = 0; q < PP; ++q) {
-      if (q < p) {
-        const float4 kk = __ldg(reinterpret_cast<const float4*>(Kb + static_cast<size_t>(q) * n) + k4);
-        acc[q] = fmaf(a.x, kk.x, acc[q]);
-        acc[q] = fmaf(a.y, kk.y, acc[q]);
-        acc[q] = fmaf(a.z, kk.z, acc[q]);
-        acc[q] = fmaf(a.w, kk.w, acc[q]);
-      }
-    }
-  }
+  for (int r = 0; r < ROWS; ++r)
+    rows[r] = reinterpret_cast<const float4*>(A + b * a_stride + static_cast<size_t>(min(i0 + r, n - 1)) * n);
+  float acc[ROWS][PP];
+  row_dots<PG, ROWS>(rows, K + static_cast<size_t>(b) * p * n, n4, p, lane, acc);
 #pragma unroll
   for (int q = 0; q < PP; ++q) {
     if (q < p) {
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) acc[q] += __shfl_xor_sync(0xffffffffu, acc[q], o);
-      acc[q] = -acc[q];
-    }
-  }
-  float* lt = Lt + b * lt_stride + static_cast<size_t>(i) * p;
-#pragma unroll
-  for (int q = 0; q < PP; ++q)
-    if (q < p && lane == (q & 31)) lt[q] = acc[q];
-  float4* Or = reinterpret_cast<float4*>(Abar + (static_cast<size_t>(b) * n + i) * n);
-  for (int k4 = lane; k4 < n4; k4 += 32) {
-    float4 a = __ldg(Ar + k4);
-#pragma unroll
-    for (int q = 0; q < PP; ++q) {
-      if (q < p) {
-        const float4 cc = __ldg(reinterpret_cast<const float4*>(Cb + static_cast<size_t>(q) * n) + k4);
-        a.x = fmaf(acc[q], cc.x, a.x);
-        a.y = fmaf(acc[q], cc.y, a.y);
-        a.z = fmaf(acc[q], cc.z, a.z);
-        a.w = fmaf(acc[q], cc.w, a.w);
+      for (int r = 0; r < ROWS; ++r) {
+        acc[r][q] = -acc[r][q];
+        if (lane == (q & 31) && i0 + r < n) Lt[b * lt_stride + static_cast<size_t>(i0 + r) * p + q] = acc[r][q];
       }
     }
-    Or[k4] = a;
+  }
+  const float4* C4 = reinterpret_cast<const float4*>(C + b * c_stride);
+#pragma unroll
+  for (int q = 0; q < PP; ++q)
+    if (q >= p) {
+#pragma unroll
+      for (int r = 0; r < ROWS; ++r) acc[r][q] = 0.f;   // discarded accumulators must not reach Abar
+    }
+  size_t coff[PP];
+#pragma unroll
+  for (int q = 0; q < PP; ++q) coff[q] = static_cast<size_t>(min(q, p - 1)) * n4;
+  for (int k4 = lane; k4 < n4; k4 += 32) {
+    float4 a[ROWS];
+#pragma unroll
+    for (int r = 0; r < ROWS; ++r) a[r] = __ldg(rows[r] + k4);
+#pragma unroll
+    for (int qg = 0; qg < PP; qg += 8) {
+      float4 cc[8];
+#pragma unroll
+      for (int q = 0; q < 8; ++q) cc[q] = __ldg(C4 + coff[qg + q] + k4);
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+#pragma unroll
+        for (int r = 0; r < ROWS; ++r) {
+          a[r].x = fmaf(acc[r][qg + q], cc[q].x, a[r].x);
+          a[r].y = fmaf(acc[r][qg + q], cc[q].y, a[r].y);
+          a[r].z = fmaf(acc[r][qg + q], cc[q].z, a[r].z);
+          a[r].w = fmaf(acc[r][qg + q], cc[q].w, a[r].w);
+        }
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < ROWS; ++r)
+      if (i0 + r < n) reinterpret_cast<float4*>(Abar + (static_cast<size_t>(b) * n + i0 + r) * n)[k4] = a[r];
   }
 }
 
@@ -264,7 +316,7 @@ cudaError_t dispatch_pg(int p, F&& fn) {
 }
 
 struct KalmanWs {
-  float *Gpart, *G, *K, *Abar, *Yt;
+  float *G, *K, *Abar, *Yt;
 };
 
 size_t carve(size_t floats) { return align_up(floats * sizeof(float), 256); }
@@ -274,7 +326,7 @@ size_t carve(size_t floats) { return align_up(floats * sizeof(float), 256); }
 size_t kalman_workspace_bytes(int batch, int T, int n, int p) {
   (void)T;
   const size_t b = batch, nn = n, pp = p;
-  return carve(kMaxKs * b * pp * nn) + 2 * carve(b * pp * nn) + 2 * carve(b * nn * nn);
+  return 2 * carve(b * pp * nn) + 2 * carve(b * nn * nn);
 }
 
 cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned long long* launches) {
@@ -285,7 +337,6 @@ cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned lon
   const size_t b = batch, nn = n, pp = p;
   KalmanWs w;
   char* cur = static_cast<char*>(a.workspace);
-  w.Gpart = reinterpret_cast<float*>(cur); cur += carve(kMaxKs * b * pp * nn);
   w.G = reinterpret_cast<float*>(cur); cur += carve(b * pp * nn);
   w.K = reinterpret_cast<float*>(cur); cur += carve(b * pp * nn);
   w.Abar = reinterpret_cast<float*>(cur); cur += carve(b * nn * nn);
@@ -323,11 +374,6 @@ cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned lon
     if ((e = bgemm_tc_make_maps(g2, maps2)) != cudaSuccess) return e;
   }
 
-  const int slabs = (n + kCpiCols - 1) / kCpiCols;
-  int KS = (2 * sms + slabs * batch - 1) / (slabs * batch);
-  KS = KS < 1 ? 1 : (KS > kMaxKs ? kMaxKs : KS);
-  if (KS > n / 4) KS = n / 4 > 0 ? n / 4 : 1;
-
   const long long c_stride = static_cast<long long>(T) * p * n, a_stride = static_cast<long long>(T) * n * n;
   const long long pi_stride = static_cast<long long>(T + 1) * n * n;
   for (int j = 0; j < T; ++j) {
@@ -336,22 +382,23 @@ cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned lon
     const float* Pij = a.Pi_out + static_cast<size_t>(j) * n * n;
     e = dispatch_pg(p, [&](auto pg) {
       constexpr int PG = decltype(pg)::value;
+      constexpr int ROWS = RowCfg<PG>::kRows;
+      const dim3 rgrid((n + kRowWarps * ROWS - 1) / (kRowWarps * ROWS), batch);
       {
         ProfScope prof(kProfKalmanSimt, stream);
-        kalman_cpi_kernel<PG><<<dim3(slabs, KS, batch), kCpiCols, 0, stream>>>(Cj, c_stride, Pij, pi_stride, w.Gpart,
-                                                                               batch, n, p);
+        kalman_cpi_kernel<PG, ROWS><<<rgrid, 32 * kRowWarps, 0, stream>>>(Cj, c_stride, Pij, pi_stride, w.G, n, p);
       }
       cudaError_t ee = cudaGetLastError();
       if (ee != cudaSuccess) return ee;
       {
         ProfScope prof(kProfKalmanSimt, stream);
         kalman_gain_kernel<PG><<<batch, 256, 0, stream>>>(Cj, c_stride, a.f + static_cast<size_t>(j) * p,
-                                                          static_cast<long long>(T) * p, w.Gpart, KS, w.G, w.K, batch, n, p);
+                                                          static_cast<long long>(T) * p, w.G, w.K, n, p);
       }
       if ((ee = cudaGetLastError()) != cudaSuccess) return ee;
       {
         ProfScope prof(kProfKalmanSimt, stream);
-        kalman_closed_loop_kernel<PG><<<dim3((n + 7) / 8, batch), 256, 0, stream>>>(
+        kalman_closed_loop_kernel<PG, ROWS><<<rgrid, 32 * kRowWarps, 0, stream>>>(
             Aj, a_stride, Cj, c_stride, w.K, a.Lt_out + static_cast<size_t>(j) * n * p,
             static_cast<long long>(T) * n * p, w.Abar, n, p);
       }
