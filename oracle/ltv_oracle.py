@@ -24,6 +24,10 @@ sequential recursion - "We obtain the solution to (14) by a forward parallel ass
                                                                      (row-wise two-norm, :150), with the
                                                                      stand-in E_s = diag(w_s) (SURVEY 8f
                                                                      NEXT-2; reading q3b)
+  constraint_tightening  sigma_0 = 0; sigma_k[i] = sum_{j<k} ||c_{k,i}^T Phi(k,j) E_j||_2      PAPER.md:144-145 eq.(12d), state part
+                                                                     of the constraint rows only, Phi^w = Phi,
+                                                                     E_j = diag(w_j) (DESIGN.md
+                                                                     readings q3b, q19)
   observer_response  PhiX(k,k) = I; PhiX(k,j) = PhiX(k,j+1) (A_j + L_j^T C_j);     PAPER.md:157-160 eq.(14), read with
                    PhiY(k,j) = PhiX(k,j) L_j^T,  0 <= j < k <= T-1                 k-independent gains L_j (:177; SURVEY
                                                                      8f NEXT-1, reading q15)
@@ -252,6 +256,29 @@ def tube_row2norm_item(A, w):
 
 def tube_row2norm(A, w):
     return np.stack([tube_row2norm_item(A[b], w[b]) for b in range(A.shape[0])])
+
+
+def constraint_tightening_item(A, w, Hc):
+    """Constraint-tightening margins of eq.(12d), one item, process-disturbance term:
+        sigma_0 = 0;   sigma_k[i] = sum_{j=0}^{k-1} || c_{k,i}^T Phi(k,j) E_j ||_2,   k = 1 .. T-1,
+    with c_{k,i}^T = Hc[k,i,:] (the state part of constraint row i at step k; Hc[0] is not used), Phi(k,j) the
+    system-response blocks of (12c) and E_j = diag(w[j]).  Written in the paper's order: one block, one row, one norm
+    at a time.  A[T,n,n], w[T,n], Hc[T,nc,n] -> sigma[T,nc]."""
+    A, w, Hc = _f64(A), _f64(w), _f64(Hc)
+    T, n, _ = A.shape
+    nc = Hc.shape[1]
+    Phi = system_response_item(A)
+    sigma = np.zeros((T, nc))
+    for k in range(1, T):
+        for j in range(k):
+            PE = Phi[packed_index(k, j)] @ np.diag(w[j])
+            for i in range(nc):
+                sigma[k, i] += np.sqrt(np.sum((Hc[k, i] @ PE) ** 2))
+    return sigma
+
+
+def constraint_tightening(A, w, Hc):
+    return np.stack([constraint_tightening_item(A[b], w[b], Hc[b]) for b in range(A.shape[0])])
 
 
 def system_response_tube_item(A, w):
