@@ -62,7 +62,8 @@ typedef enum {
 enum { LTV_OP_ROLLOUT = 0, LTV_OP_SYSTEM_RESPONSE_TUBE = 1, LTV_OP_ADJOINT = 2, LTV_OP_PIPELINE_HOST = 3,
        LTV_OP_PIPELINE_HOST_NO_PHI = 4 /* ltv_scan_pipeline_host with w_host == NULL: rollout + adjoint only */,
        LTV_OP_OBSERVER_RESPONSE = 5 /* ltv_scan_observer_response; pass p (rows of C) as `m` */,
-       LTV_OP_KALMAN_GAINS = 6 /* ltv_scan_kalman_gains; pass p (rows of C) as `m` */ };
+       LTV_OP_KALMAN_GAINS = 6 /* ltv_scan_kalman_gains; pass p (rows of C) as `m` */,
+       LTV_OP_CONSTRAINT_TIGHTENING = 7 /* ltv_scan_constraint_tightening; pass nc (constraint rows) as `m` */ };
 
 /* `phi_layout` argument.  COLUMN_PACKED (the only layout of this version): the P = T(T-1)/2 blocks of one
  * item are stored column by column of the block-lower-triangular operator; block (t,s), 0 <= s < t <= T-1,
@@ -145,6 +146,22 @@ LTV_API int ltv_scan_observer_response(const float* A, const float* Lt, const fl
                                        float* phi_out, float* r_out, int batch, int T, int n, int p, int phi_layout,
                                        unsigned flags, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Constraint-tightening margins (second form; eq.(12d)), process-disturbance term,
+ * state part of the constraint rows, with the system response of (12c) and E_j = diag(w_j) (DESIGN.md q3b, q19):
+ *     sigma_0 = 0;   sigma_k[i] = sum_{j=0}^{k-1} || c_{k,i}^T Phi(k,j) E_j ||_2,   k = 1 .. T-1,   c_{k,i}^T = Hc[b,k,i,:]
+ *   A          device [batch,T,n,n]     required; A_0 .. A_{T-2} are read
+ *   w          device [batch,T,n]       required; w_0 .. w_{T-2} are read
+ *   Hc         device [batch,T,nc,n]    required; constraint rows per step (Hc[b,0] is not read), nc >= 1
+ *   sigma_out  device [batch,T,nc]
+ *   flags      must be 0
+ * Phi is neither formed nor read: the rows Psi(k,j) = Hc_k Phi(k,j) obey Psi(k,j) = Psi(k,j+1) A_j, so one backward
+ * sweep over j carries the stack of all rows with k > j through one batched GEMM per step ((T-1-j) nc rows; 3xTF32 on
+ * tcgen05 for n >= 96, fp32 FMA below) and a row-norm kernel: 2 n^2 nc (T-1-j) flop per step, A read once.
+ * Deterministic.  Workspace: ltv_scan_workspace_bytes(LTV_OP_CONSTRAINT_TIGHTENING, batch, T, n, nc). */
+LTV_API int ltv_scan_constraint_tightening(const float* A, const float* w, const float* Hc, float* sigma_out,
+                                           int batch, int T, int n, int nc, unsigned flags,
+                                           void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* Backward-Kalman recursion of the output-feedback stage (eq.(13)), with the
  * disturbance scalings taken diagonal, E_j = diag(e_j), F_j = diag(f_j) (readings q3b, q18):
  *     Pi_0 = Xi Xi^T (given);   for j = 0 .. T-1:
@@ -205,8 +222,8 @@ LTV_API unsigned long long ltv_launch_count(void);
  * ltv_profile_collect waits for the recorded events, adds their elapsed times (milliseconds) and launch counts
  * per kernel class into the two caller arrays of LTV_PROFILE_CLASSES entries (host memory), and clears the
  * record.  Classes: 0 rollout, 1 adjoint, 2 Phi level 0 (copy + tube), 3 Phi combine (tcgen05 3xTF32),
- * 4 Phi combine (fp32 FMA, small n), 5 tube finalise, 6 Kalman batched GEMMs (tcgen05 3xTF32, or fp32 FMA for
- * small n), 7 Kalman gain / closed-loop kernels. */
+ * 4 Phi combine (fp32 FMA, small n), 5 tube finalise, 6 batched GEMMs of the Kalman recursion and the constraint sweep
+ * (tcgen05 3xTF32, or fp32 FMA for small n), 7 their fp32 support kernels (gain, closed loop, row norms). */
 #define LTV_PROFILE_CLASSES 8
 LTV_API int ltv_profile_enable(int on);
 LTV_API int ltv_profile_collect(double* ms_by_class, unsigned long long* launches_by_class);

@@ -20,6 +20,7 @@ LTV_OP_ROLLOUT, LTV_OP_SYSTEM_RESPONSE_TUBE, LTV_OP_ADJOINT, LTV_OP_PIPELINE_HOS
 LTV_OP_PIPELINE_HOST_NO_PHI = 4
 LTV_OP_OBSERVER_RESPONSE = 5
 LTV_OP_KALMAN_GAINS = 6
+LTV_OP_CONSTRAINT_TIGHTENING = 7
 LTV_TUBE_ROW_2NORM = 1
 LTV_PHI_COLUMN_PACKED = 0
 
@@ -28,6 +29,7 @@ EXPORTS = (
     "ltv_scan_adjoint", "ltv_scan_pipeline_host", "ltv_status_string", "ltv_last_cuda_error", "ltv_version",
     "ltv_launch_count", "ltv_profile_enable", "ltv_profile_collect", "ltv_scan_observer_response",
     "ltv_observer_row_floats", "ltv_scan_kalman_gains",
+    "ltv_scan_constraint_tightening",
 )
 
 
@@ -60,6 +62,8 @@ def _load() -> ctypes.CDLL:
     L.ltv_scan_observer_response.argtypes = [fp] * 6 + [i] * 5 + [ctypes.c_uint, vp, sz, vp]
     L.ltv_scan_kalman_gains.restype = i
     L.ltv_scan_kalman_gains.argtypes = [fp] * 7 + [i] * 4 + [ctypes.c_uint, vp, sz, vp]
+    L.ltv_scan_constraint_tightening.restype = i
+    L.ltv_scan_constraint_tightening.argtypes = [fp] * 4 + [i] * 4 + [ctypes.c_uint, vp, sz, vp]
     L.ltv_observer_row_floats.restype = i
     L.ltv_observer_row_floats.argtypes = [i, i]
     L.ltv_status_string.restype = ctypes.c_char_p
@@ -190,6 +194,24 @@ def ltv_scan_observer_response(A, Lt, C, w, phi_out=None, r_out=None, workspace=
     if st != LTV_OK:
         raise LtvError(st, "ltv_scan_observer_response")
     return phi_out, r_out
+
+
+def ltv_scan_constraint_tightening(A, w, Hc, sigma_out=None, workspace=None):
+    """Constraint-tightening margins (eq.(12d)): sigma[batch,T,nc], sigma[b,k,i] = sum_{j<k} ||Hc[b,k,i] Phi(k,j) diag(w_j)||_2."""
+    batch, T, n, _ = A.shape
+    nc = Hc.shape[2]
+    _dev(A, "A", (batch, T, n, n)); _dev(w, "w", (batch, T, n)); _dev(Hc, "Hc", (batch, T, nc, n))
+    if sigma_out is None:
+        sigma_out = torch.empty((batch, T, nc), device=A.device, dtype=torch.float32)
+    _dev(sigma_out, "sigma_out", (batch, T, nc))
+    need = ltv_scan_workspace_bytes(LTV_OP_CONSTRAINT_TIGHTENING, batch, T, n, nc)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), device=A.device, dtype=torch.uint8)
+    st = lib.ltv_scan_constraint_tightening(_ptr(A), _ptr(w), _ptr(Hc), _ptr(sigma_out), batch, T, n, nc, 0,
+                                            _ptr(workspace), workspace.numel(), _stream())
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_constraint_tightening")
+    return sigma_out
 
 
 def ltv_scan_kalman_gains(A, C, e, f, Pi0, Lt_out=None, Pi_out=None, workspace=None):

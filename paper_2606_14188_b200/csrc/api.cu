@@ -162,6 +162,9 @@ size_t ltv_scan_workspace_bytes(int op, int batch, int T, int n, int m) {
     case LTV_OP_KALMAN_GAINS:
       if (m < 1 || m > 32) return 0;
       return kalman_workspace_bytes(batch, T, n, m);
+    case LTV_OP_CONSTRAINT_TIGHTENING:
+      if (m < 1 || static_cast<long long>(batch) * T * m >= (1ll << 31) / n) return 0;
+      return constraint_workspace_bytes(batch, T, n, m);
     case LTV_OP_PIPELINE_HOST:
     case LTV_OP_PIPELINE_HOST_NO_PHI: {
       const bool with_phi = op == LTV_OP_PIPELINE_HOST;
@@ -314,6 +317,27 @@ int ltv_scan_kalman_gains(const float* A, const float* C, const float* e, const 
   KalmanArgs a{A, C, e, f, Pi0, Lt_out, Pi_out, batch, T, n, p, workspace};
   unsigned long long l = 0;
   cudaError_t err = launch_kalman(a, static_cast<cudaStream_t>(cuda_stream), &l);
+  g_launches += l;
+  return err == cudaSuccess ? LTV_OK : fail_cuda(err);
+}
+
+int ltv_scan_constraint_tightening(const float* A, const float* w, const float* Hc, float* sigma_out, int batch, int T,
+                                   int n, int nc, unsigned flags, void* workspace, size_t workspace_bytes,
+                                   void* cuda_stream) {
+  if (!A || !w || !Hc || !sigma_out || !workspace) return LTV_ERR_NULL_PTR;
+  int st = check_dims(batch, T, n, 0);
+  if (st != LTV_OK) return st;
+  if (nc < 1 || flags != 0) return LTV_ERR_BAD_DIM;
+  if (static_cast<long long>(batch) * T * nc >= (1ll << 31) / n) return LTV_ERR_UNSUPPORTED_SHAPE;
+  if (misaligned(A) || misaligned(w) || misaligned(Hc) || misaligned(sigma_out) || misaligned(workspace))
+    return LTV_ERR_ALIGNMENT;
+  if (workspace_bytes < constraint_workspace_bytes(batch, T, n, nc)) return LTV_ERR_WORKSPACE_TOO_SMALL;
+  int sms = 0;
+  st = check_device(&sms);
+  if (st != LTV_OK) return st;
+  ConstraintArgs a{A, w, Hc, sigma_out, batch, T, n, nc, workspace};
+  unsigned long long l = 0;
+  cudaError_t err = launch_constraint_tightening(a, static_cast<cudaStream_t>(cuda_stream), &l);
   g_launches += l;
   return err == cudaSuccess ? LTV_OK : fail_cuda(err);
 }

@@ -283,7 +283,7 @@ __global__ void __launch_bounds__(256) bgemm_simt_kernel(const BatchedGemm g) {
   const int b = blockIdx.z;
   const float* L = g.L + (static_cast<size_t>(g.l_row0) + static_cast<size_t>(b) * g.l_row_stride) * g.K;
   const float* R = g.R + (static_cast<size_t>(g.r_blk0) + static_cast<size_t>(b) * g.r_blk_stride) * g.K * g.N;
-  float* D = g.D + (static_cast<size_t>(g.d_blk0) + static_cast<size_t>(b) * g.d_blk_stride) * g.M * g.N;
+  float* D = g.D + (static_cast<size_t>(g.d_blk0) + static_cast<size_t>(b) * g.d_blk_stride) * (g.d_rows > 0 ? g.d_rows : g.M) * g.N;
   const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
   const int row = blockIdx.y * 16 + ty, col = blockIdx.x * 16 + tx;
   float acc = 0.f;
@@ -303,6 +303,16 @@ __global__ void __launch_bounds__(256) bgemm_simt_kernel(const BatchedGemm g) {
     if (g.transpose_out) D[static_cast<size_t>(col) * g.M + row] = acc; else D[static_cast<size_t>(row) * g.N + col] = acc;
   }
 }
+
+}  // namespace
+
+cudaError_t launch_bgemm_simt(const BatchedGemm& g, cudaStream_t stream) {
+  const dim3 grid((g.N + 15) / 16, (g.M + 15) / 16, g.count);
+  bgemm_simt_kernel<<<grid, 256, 0, stream>>>(g);
+  return cudaGetLastError();
+}
+
+namespace {
 
 template <typename F>
 cudaError_t dispatch_pg(int p, F&& fn) {

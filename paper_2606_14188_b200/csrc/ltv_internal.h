@@ -52,6 +52,16 @@ struct KalmanArgs {
 size_t kalman_workspace_bytes(int batch, int T, int n, int p);
 cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned long long* launches);
 
+// Constraint-tightening margins of eq.(12d) (constraints.cu)
+struct ConstraintArgs {
+  const float *A, *w, *Hc;
+  float* sigma_out;
+  int batch, T, n, nc;
+  void* workspace;
+};
+size_t constraint_workspace_bytes(int batch, int T, int n, int nc);
+cudaError_t launch_constraint_tightening(const ConstraintArgs& a, cudaStream_t stream, unsigned long long* launches);
+
 // Cluster size (CTAs per item, 1..16, any integer) for the two vector kernels.  max_active[C] = clusters of C CTAs
 // that can be resident at once (cudaOccupancyMaxActiveClusters; 0 = not launchable).  Minimises a simple
 // time model over the waves of clusters: an SM streams ~70 GB/s, the device ~6.5 TB/s (both measured).

@@ -29,11 +29,14 @@ struct BatchedGemm {
   const float* R; int r_blocks, r_blk0, r_blk_stride;
   float* D; int d_blocks, d_blk0, d_blk_stride;
   int count, M, N, K;
+  int d_rows;   // rows of one D block in memory; 0 = M.  (> M only without transpose_out: rows [M, d_rows) are not written;
+                // the maps are built for d_rows, so M may then change from launch to launch)
   int transpose_out;
   const float* diag; long long diag_stride;
 };
 cudaError_t bgemm_tc_make_maps(const BatchedGemm& a, void* maps_out);
 cudaError_t launch_bgemm_tc(const BatchedGemm& a, int nch, const void* maps, int num_sms, cudaStream_t stream);
+cudaError_t launch_bgemm_simt(const BatchedGemm& a, cudaStream_t stream);   // fp32 FMA, any size (kalman.cu)
 int phi_pick_nch(int n);   // phi.cu
 
 void* get_encode_tiled();  // adjoint.cu

@@ -56,6 +56,7 @@ constexpr int kTcMaxStages = 6;
 // map and writes block d_blk0 + b d_blk_stride of the (3-D) O map
 struct TcGemm {
   int count, M, Mt;
+  int d_rows;              // rows of one D block in memory (>= M; rows [M, d_rows) are never written)
   int l_row0, l_row_stride, r_blk0, r_blk_stride, d_blk0, d_blk_stride;
   int transpose_out;       // store D^T (the O map then describes [blocks][N][M])
   const float* diag;       // adds diag[b diag_stride + i]^2 to D[b][i][i] (E E^T with E = diag(e)); may be null
@@ -372,6 +373,19 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
             for (int e = 0; e < 32; ++e)
               if (jc + e == rr) vc[e] = __float_as_uint(__uint_as_float(vc[e]) + dd);
           }
+          if (!tr && rows_valid < 32) {
+            // ragged last m-tile, plain store: rows [M, d_rows) of the block belong to the caller (masked stores)
+            if (lane < rows_valid) {
+              float* out = p.phi + (static_cast<size_t>(oblk) * p.gm.d_rows + rr) * nc + jc;
+#pragma unroll
+              for (int e = 0; e < 8; ++e) {
+                if (jc + 4 * e < nc)
+                  st_global_f4_na(out + 4 * e, make_float4(__uint_as_float(vc[4 * e]), __uint_as_float(vc[4 * e + 1]),
+                                                           __uint_as_float(vc[4 * e + 2]), __uint_as_float(vc[4 * e + 3])));
+              }
+            }
+            continue;
+          }
           if (lane == 0) tma_store_wait_read<0>();
           __syncwarp();
           if (!tr) {
@@ -639,7 +653,8 @@ cudaError_t bgemm_tc_make_maps(const BatchedGemm& a, void* maps_out) {
   }
   {
     // D[b] is M x N, stored as it is or transposed (N x M); either way one block per problem, clipped per block
-    const cuuint64_t cols = a.transpose_out ? M : N, rows = a.transpose_out ? N : M;
+    const cuuint64_t cols = a.transpose_out ? M : N;
+    const cuuint64_t rows = a.transpose_out ? N : (a.d_rows > 0 ? static_cast<cuuint64_t>(a.d_rows) : M);
     const cuuint64_t dims[3] = {cols, rows, static_cast<cuuint64_t>(a.d_blocks)};
     const cuuint64_t strides[2] = {cols * 4, rows * cols * 4};
     const cuuint32_t box[3] = {32, 32, 1};
@@ -665,7 +680,9 @@ cudaError_t launch_bgemm_tc(const BatchedGemm& a, int nch, const void* maps, int
   p.g.tm = pair ? 2 * kTM : kTM;
   p.g.tn = nt;
   p.g.NT = (a.N + nt - 1) / nt;
+  p.phi = a.D;
   p.gm.count = a.count; p.gm.M = a.M; p.gm.Mt = pair ? Mt2 : Mt1;
+  p.gm.d_rows = a.d_rows > 0 ? a.d_rows : a.M;
   p.gm.l_row0 = a.l_row0; p.gm.l_row_stride = a.l_row_stride;
   p.gm.r_blk0 = a.r_blk0; p.gm.r_blk_stride = a.r_blk_stride;
   p.gm.d_blk0 = a.d_blk0; p.gm.d_blk_stride = a.d_blk_stride;
