@@ -51,8 +51,8 @@ def parse():
 
 
 def ncu_traffic(cfg_index, kernel):
-    """dram bytes per step of `kernel` from the committed ncu capture (profiles/r1_v4_traffic.csv), or None."""
-    path = os.path.join(ROOT, "profiles", "r1_v4_traffic.csv")
+    """dram bytes per step of `kernel` from the committed ncu capture (profiles/r1_v5_traffic.csv), or None."""
+    path = os.path.join(ROOT, "profiles", "r1_v5_traffic.csv")
     try:
         for ln in open(path).read().splitlines()[1:]:
             c, k, b = ln.split(",")[:3]
