@@ -42,6 +42,8 @@ def parse():
                     help="also time ltv_scan_observer_response (NEXT-1, eq.(14)) with P measurement rows")
     ap.add_argument("--kalman", type=int, default=0, metavar="P",
                     help="also time ltv_scan_kalman_gains (NEXT-3, eq.(13)) with P observation rows")
+    ap.add_argument("--constraints", type=int, default=0, metavar="NC",
+                    help="also time ltv_scan_constraint_tightening (NEXT-2, eq.(12d)) with NC constraint rows per step")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-items", type=int, default=0, help="items in the CPU-oracle sample (0 = auto)")
@@ -352,6 +354,31 @@ def main():
                            "products per step and item (3xTF32 on tcgen05 for n >= 96)")
         del Lto, Pio, wsk, kd
 
+    # ---- NEXT-2 (12d): constraint-tightening margins on the same A, w with random constraint rows, timed alone
+    constraints = None
+    if args.constraints > 0:
+        ncr = args.constraints
+        gen = torch.Generator(device=dev).manual_seed(4321 + rank)
+        Hc = torch.randn((batch, T, ncr, n), device=dev, generator=gen)
+        sig = torch.empty((batch, T, ncr), device=dev)
+        wsc = torch.empty(max(16, L.ltv_scan_workspace_bytes(L.LTV_OP_CONSTRAINT_TIGHTENING, batch, T, n, ncr)),
+                          dtype=torch.uint8, device=dev)
+        for _ in range(3):
+            L.ltv_scan_constraint_tightening(d["A"], d["w"], Hc, sigma_out=sig, workspace=wsc)
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        c0.record()
+        for _ in range(args.steps):
+            L.ltv_scan_constraint_tightening(d["A"], d["w"], Hc, sigma_out=sig, workspace=wsc)
+        c1.record()
+        barrier()
+        cms = c0.elapsed_time(c1) / args.steps
+        constraints = dict(nc=ncr, ms=cms, items_per_s=batch * world / (cms * 1e-3),
+                           hbm_gbs=batch * (T - 1) * n * n * 4 / (cms * 1e-3) / 1e9,
+                           note="ltv_scan_constraint_tightening alone: backward sweep of the stacked constraint rows, "
+                                "A read once (hbm_gbs counts those bytes), Phi never formed")
+        del Hc, sig, wsc
+
     # ---- end to end through the C-ABI with host buffers
     e2e = None
     if not args.no_e2e:
@@ -408,7 +435,7 @@ def main():
                                     f"working set (A {a_gb * 1e3:.2f} MB) fits L2: warm-cache, latency-bound case"),
                                 phi_layout="column-packed"),
                     clocks=sampler.result(), e2e=e2e, gpu_launches=int(launches), roofline=roof,
-                    cpu_baseline=cpu, kernel_ms_per_step=share, vector_scans=extra, observer=observer, kalman=kalman,
+                    cpu_baseline=cpu, kernel_ms_per_step=share, vector_scans=extra, observer=observer, kalman=kalman, constraints=constraints,
                     rollouts_per_s=extra.get("rollout", {}).get("per_s"),
                     adjoints_per_s=extra.get("adjoint", {}).get("per_s"))
         print(json.dumps(line), flush=True)

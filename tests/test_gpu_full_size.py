@@ -167,3 +167,47 @@ def test_c2_full_observer_and_two_norm(L):
     q = lambda tt, ss: phi[50, L.ltv_phi_block_index(T, tt, ss)].double()
     rhs = q(30, 11)[:, :n] @ q(11, 3)
     assert float((q(30, 3) - rhs).abs().max() / rhs.abs().max()) <= TOL
+
+
+# ------------------------------------------------------------------ NEXT rows at full size (sampled items)
+@pytest.mark.parametrize("ci,p,items", [(1, 6, (0, 37, 63)), (2, 6, (0, 15)), (3, 12, (3,))])
+def test_full_size_kalman_gains(L, ci, p, items):
+    """ltv_scan_kalman_gains at the C2 / C3 / C4 sizes with the whole batch on the device (the configuration
+    `bench.py --kalman` times); the oracle recursion (13) runs for the sampled items only.  Properties that hold at any
+    size: Pi_out[:, 0] is Pi0 bit for bit, every Pi_j is symmetric to rounding and finite."""
+    import torch
+    from workloads import observation_model
+
+    W = generate(config(ci))
+    batch, T, n, _ = W.A.shape
+    M = observation_model(batch, T, n, p, seed=900 + ci, kind="track")
+    d = [torch.from_numpy(a).cuda() for a in (W.A, M["C"], M["e"], M["f"], M["Pi0"])]
+    Lt, Pi = L.ltv_scan_kalman_gains(*d)
+    torch.cuda.synchronize()
+    assert torch.equal(Pi[:, 0], d[4]) and bool(torch.isfinite(Pi).all()) and bool(torch.isfinite(Lt).all())
+    asym = (Pi - Pi.transpose(-1, -2)).abs().amax(dim=(-1, -2)) / Pi.abs().amax(dim=(-1, -2))
+    assert float(asym.max()) <= TOL
+    for b in items:
+        Pi_ref, Lt_ref = O.kalman_recursion_item(W.A[b], M["C"][b], M["e"][b], M["f"][b], M["Pi0"][b])
+        got_Pi, got_Lt = Pi[b].cpu().numpy(), Lt[b].cpu().numpy()
+        assert O.rel_err(got_Pi, Pi_ref) <= TOL and O.rel_err(got_Lt, Lt_ref) <= TOL
+        assert O.rel_err(got_Pi[-1], Pi_ref[-1]) <= TOL and O.rel_err(got_Lt[-1], Lt_ref[-1]) <= TOL
+
+
+@pytest.mark.parametrize("ci,nc,items", [(1, 6, (0, 63)), (2, 6, (7,))])
+def test_full_size_constraint_tightening(L, ci, nc, items):
+    """ltv_scan_constraint_tightening at the C2 / C3 sizes (whole batch on the device, sampled items against the
+    oracle); sigma_0 = 0, finiteness and positivity for k >= 1 are checked on every item."""
+    import torch
+
+    W = generate(config(ci))
+    batch, T, n, _ = W.A.shape
+    Hc = np.random.default_rng(70 + ci).normal(0.0, 1.0, (batch, 1, nc, n)).astype(np.float32)
+    Hc = np.ascontiguousarray(np.broadcast_to(Hc, (batch, T, nc, n)))
+    sig = L.ltv_scan_constraint_tightening(torch.from_numpy(W.A).cuda(), torch.from_numpy(W.w).cuda(),
+                                           torch.from_numpy(Hc).cuda())
+    torch.cuda.synchronize()
+    sig = sig.cpu().numpy()
+    assert np.all(sig[:, 0] == 0.0) and np.all(np.isfinite(sig)) and np.all(sig[:, 1:] > 0.0)
+    for b in items:
+        assert O.rel_err(sig[b], O.constraint_tightening_item(W.A[b], W.w[b], Hc[b])) <= TOL
