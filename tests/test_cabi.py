@@ -80,6 +80,23 @@ def test_host_side_validation_needs_no_gpu(L):
     assert o(p, p, p, p, p, p, 1, 2, 4, 2, 0, 0, p, 8, None) == 5                       # workspace too small
     assert L.ltv_observer_row_floats(300, 6) == 308 and L.ltv_observer_row_floats(48, 4) == 52
     assert L.ltv_scan_workspace_bytes(L.LTV_OP_OBSERVER_RESPONSE, 2, 4, 128, 6) > 0
+    k = L.lib.ltv_scan_kalman_gains
+    assert k(p, p, p, p, None, p, p, 1, 2, 4, 2, 0, p, 1 << 20, None) == 1              # NULL Pi0
+    assert k(p, p, p, p, p, p, p, 1, 2, 4, 0, 0, p, 1 << 20, None) == 2                 # p = 0
+    assert k(p, p, p, p, p, p, p, 1, 2, 4, 2, 1, p, 1 << 20, None) == 2                 # unknown flag
+    assert k(p, p, p, p, p, p, p, 1, 2, 4, 33, 0, p, 1 << 20, None) == 3                # p > 32
+    assert k(p, p, p, odd, p, p, p, 1, 2, 4, 2, 0, p, 1 << 20, None) == 4               # misaligned f
+    assert k(p, p, p, p, p, p, p, 1, 2, 4, 2, 0, p, 8, None) == 5                       # workspace too small
+    n, T, b = 300, 32, 64
+    need = L.ltv_scan_workspace_bytes(L.LTV_OP_KALMAN_GAINS, b, T, n, 6)
+    assert 2 * b * n * n * 4 <= need <= 2 * b * n * n * 4 + 2 * b * 6 * n * 4 + 4096    # Abar, Yt, G, K
+    assert L.ltv_scan_workspace_bytes(L.LTV_OP_KALMAN_GAINS, b, T, n, 33) == 0
+    c = L.lib.ltv_scan_constraint_tightening
+    assert c(p, p, None, p, 1, 2, 4, 2, 0, p, 1 << 20, None) == 1                       # NULL Hc
+    assert c(p, p, p, p, 1, 2, 4, 0, 0, p, 1 << 20, None) == 2                          # nc = 0
+    assert c(p, p, p, p, 1, 2, 4, 2, 0, p, 8, None) == 5                                # workspace too small
+    need = L.ltv_scan_workspace_bytes(L.LTV_OP_CONSTRAINT_TIGHTENING, b, T, n, 6)
+    assert 2 * b * (T - 1) * 6 * n * 4 <= need <= 2 * b * (T - 1) * 6 * n * 4 + 1024   # two stacks of (T-1) nc rows
     a = L.lib.ltv_scan_adjoint
     assert a(p, None, p, p, p, None, 1, 2, 4, 2, None, 0, None) == 1                # grad_u wanted, B NULL
     assert a(p, p, None, p, None, None, 1, 2, 4, 2, None, 0, None) == 1             # NULL g

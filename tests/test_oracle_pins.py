@@ -506,3 +506,27 @@ def test_generator_free_fall_of_centre_of_mass():
 def test_rel_err_metric():
     assert O.rel_err(np.array([1.0, 2.0, 4.0]), np.array([1.0, 2.0, 5.0])) == pytest.approx(0.2)
     assert O.rel_err(np.zeros(3), np.zeros(3)) == 0.0
+
+
+def test_observer_achievability_identity_of_12c():
+    """Second identity of (12c) for the observer side, Phi_x (I - Z A) - Phi_y (Z C) = I, in blocks:
+    PhiX(k,j) - PhiX(k,j+1) A_j = PhiX(k,j+1) Lt_j C_j for j < k (PhiX(k,k) = I).  It holds for the oracle's PhiX with
+    the gain that closes the loop around A_j (DESIGN.md q17), and shows which response block that gain multiplies:
+    the observation of step j enters through PhiX(k,j+1) Lt_j, one block to the right of the PhiY(k,j) = PhiX(k,j) Lt_j
+    that (14) prints (DESIGN.md q20)."""
+    T, n, p = 6, 4, 2
+    A, Lt, C = _obs_inputs(T, n, p, 9)
+    X, _ = O.observer_response_item(A, Lt, C)
+    blk = lambda k, j: np.eye(n) if k == j else X[O.packed_index(k, j)]
+    N = T * n
+    Px, Py = np.zeros((N, N)), np.zeros((N, T * p))       # Py(k, j+1) := PhiX(k,j+1) Lt_j
+    ZA, ZC = np.zeros((N, N)), np.zeros((T * p, N))
+    for k in range(T):
+        for j in range(k + 1):
+            Px[k * n:(k + 1) * n, j * n:(j + 1) * n] = blk(k, j)
+            if j >= 1:
+                Py[k * n:(k + 1) * n, j * p:(j + 1) * p] = blk(k, j) @ Lt[j - 1]
+    for j in range(T - 1):
+        ZA[(j + 1) * n:(j + 2) * n, j * n:(j + 1) * n] = A[j]
+        ZC[(j + 1) * p:(j + 2) * p, j * n:(j + 1) * n] = C[j]
+    np.testing.assert_allclose(Px @ (np.eye(N) - ZA) - Py @ ZC, np.eye(N), rtol=0, atol=1e-12)
