@@ -176,12 +176,20 @@ LTV_API int ltv_scan_constraint_tightening(const float* A, const float* w, const
  *   Lt_out   device [batch,T,n,p]      Lt_out[b,j] = L_{j+1}^T, the gain formed from (A_j, C_j, Pi_j): exactly the `Lt`
  *                                      array of ltv_scan_observer_response (A_j + Lt_j C_j closes the loop around A_j)
  *   Pi_out   device [batch,T+1,n,n]    Pi_out[b,j] = Pi_j (Pi_out[b,0] = Pi0)
- *   flags    must be 0
- * Time-sequential, batch-parallel: per step one pass forms G = C Pi, the p x p innovation covariance (Cholesky), the
+ *   flags    0 (the library picks), LTV_KALMAN_SCAN or LTV_KALMAN_RECURSION (not both)
+ * Two device paths give the same Pi_j, L_j up to rounding:
+ *   scan       PAPER.md:166-177: the associative elements (17) combined by rule (16) (re-derived, DESIGN.md q14) in a
+ *              Sklansky prefix scan, ceil(log2(T+1)) launches with one CTA per combination (Gauss-Jordan with partial
+ *              pivoting and the five products in shared memory), then the gains of all steps in one pass.  n <= 64
+ *              (LTV_ERR_UNSUPPORTED_SHAPE beyond).  Picked for small n and batch (T+1)/2 <= 2 x SM count.
+ *   recursion  time-sequential, batch-parallel: per step one pass forms G = C Pi, the p x p innovation covariance (Cholesky), the
  * gain and the closed-loop matrix Abar_j = A_j + Lt_j C_j, then two batched 3xTF32 tcgen05 GEMMs form
- * Pi_{j+1} = A_j (Abar_j Pi_j)^T + E E^T (fp32 FMA for n < 96).  The associative-scan form (16)(17) of the paper is
- * ~10x the flops and is not used at these batch sizes.  Results are symmetric up to rounding.
+ * Pi_{j+1} = A_j (Abar_j Pi_j)^T + E E^T (fp32 FMA for n < 96).  ~10x fewer flops than the scan: the faster form
+ *              whenever one time step over the batch fills the machine.
+ * Results are symmetric up to rounding.
  * Workspace: ltv_scan_workspace_bytes(LTV_OP_KALMAN_GAINS, batch, T, n, p). */
+#define LTV_KALMAN_SCAN 1u
+#define LTV_KALMAN_RECURSION 2u
 LTV_API int ltv_scan_kalman_gains(const float* A, const float* C, const float* e, const float* f, const float* Pi0,
                                   float* Lt_out, float* Pi_out, int batch, int T, int n, int p, unsigned flags,
                                   void* workspace, size_t workspace_bytes, void* cuda_stream);

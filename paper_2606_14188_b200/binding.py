@@ -22,6 +22,7 @@ LTV_OP_OBSERVER_RESPONSE = 5
 LTV_OP_KALMAN_GAINS = 6
 LTV_OP_CONSTRAINT_TIGHTENING = 7
 LTV_TUBE_ROW_2NORM = 1
+LTV_KALMAN_SCAN, LTV_KALMAN_RECURSION = 1, 2
 LTV_PHI_COLUMN_PACKED = 0
 
 EXPORTS = (
@@ -214,9 +215,10 @@ def ltv_scan_constraint_tightening(A, w, Hc, sigma_out=None, workspace=None):
     return sigma_out
 
 
-def ltv_scan_kalman_gains(A, C, e, f, Pi0, Lt_out=None, Pi_out=None, workspace=None):
+def ltv_scan_kalman_gains(A, C, e, f, Pi0, Lt_out=None, Pi_out=None, workspace=None, mode=0):
     """Backward-Kalman recursion (eq.(13)): returns (Lt[batch,T,n,p] with Lt[b,j] = L_{j+1}^T, Pi[batch,T+1,n,n]).
-    C[batch,T,p,n], e[batch,T,n], f[batch,T,p] (> 0), Pi0[batch,n,n] symmetric PSD."""
+    C[batch,T,p,n], e[batch,T,n], f[batch,T,p] (> 0), Pi0[batch,n,n] symmetric PSD.  mode: 0 the library picks,
+    LTV_KALMAN_SCAN (associative scan (16)(17), n <= 64) or LTV_KALMAN_RECURSION."""
     batch, T, n, _ = A.shape
     p = C.shape[2]
     _dev(A, "A", (batch, T, n, n)); _dev(C, "C", (batch, T, p, n)); _dev(e, "e", (batch, T, n))
@@ -230,7 +232,7 @@ def ltv_scan_kalman_gains(A, C, e, f, Pi0, Lt_out=None, Pi_out=None, workspace=N
     if workspace is None:
         workspace = torch.empty(max(need, 16), device=A.device, dtype=torch.uint8)
     st = lib.ltv_scan_kalman_gains(_ptr(A), _ptr(C), _ptr(e), _ptr(f), _ptr(Pi0), _ptr(Lt_out), _ptr(Pi_out),
-                                   batch, T, n, p, 0, _ptr(workspace), workspace.numel(), _stream())
+                                   batch, T, n, p, mode, _ptr(workspace), workspace.numel(), _stream())
     if st != LTV_OK:
         raise LtvError(st, "ltv_scan_kalman_gains")
     return Lt_out, Pi_out

@@ -304,8 +304,9 @@ int ltv_scan_kalman_gains(const float* A, const float* C, const float* e, const 
   if (!A || !C || !e || !f || !Pi0 || !Lt_out || !Pi_out || !workspace) return LTV_ERR_NULL_PTR;
   int st = check_dims(batch, T, n, 0);
   if (st != LTV_OK) return st;
-  if (p < 1 || flags != 0) return LTV_ERR_BAD_DIM;
+  if (p < 1 || (flags & ~3u) != 0 || flags == 3u) return LTV_ERR_BAD_DIM;
   if (p > 32) return LTV_ERR_UNSUPPORTED_SHAPE;
+  if ((flags & LTV_KALMAN_SCAN) && !riccati_scan_supported(n)) return LTV_ERR_UNSUPPORTED_SHAPE;
   if (static_cast<long long>(batch) * (T + 1) * n >= (1ll << 31)) return LTV_ERR_UNSUPPORTED_SHAPE;
   if (misaligned(A) || misaligned(C) || misaligned(e) || misaligned(f) || misaligned(Pi0) || misaligned(Lt_out) ||
       misaligned(Pi_out) || misaligned(workspace))
@@ -315,6 +316,7 @@ int ltv_scan_kalman_gains(const float* A, const float* C, const float* e, const 
   st = check_device(&sms);
   if (st != LTV_OK) return st;
   KalmanArgs a{A, C, e, f, Pi0, Lt_out, Pi_out, batch, T, n, p, workspace};
+  a.mode = (flags & LTV_KALMAN_SCAN) ? 1 : ((flags & LTV_KALMAN_RECURSION) ? 2 : 0);
   unsigned long long l = 0;
   cudaError_t err = launch_kalman(a, static_cast<cudaStream_t>(cuda_stream), &l);
   g_launches += l;

@@ -11,12 +11,12 @@
 //     Pi_{j+1} = A_j Yt + diag(e_j)^2  [n,n]   tcgen05 3xTF32 batched GEMM, E E^T added in the epilogue
 // (A_j Pi_j Abar_j^T is the right-hand side of (13) with L_{j+1} substituted.)
 //
-// Why the recursion and not the associative scan (16)(17) the paper runs: one combination of (16)
-// costs an n x n solve with 2n right-hand sides plus six n^3 products (~17 n^3 flop) against 4 n^3 for one step of
-// (13), and a scan needs (T/2) log2 T of them; at T = 32 that is ~10x the flops.  The scan buys depth log T for a
-// single item on a small GPU; here one step over the whole batch already fills all 148 SMs (C2: 384 tiles of
-// 128 x 160), so the sequential form is the faster one at every BASELINE.json size.  The scan is kept in the oracle,
-// pinned against the recursion (tests/test_oracle_pins_kalman.py).  DESIGN.md section 7.
+// Recursion or associative scan (16)(17)?  One combination of (16) costs an n x n solve with 2n
+// right-hand sides plus six n^3 products (~17 n^3 flop) against 4 n^3 for one step of (13), and a scan needs
+// (T/2) log2 T of them; at T = 32 that is ~10x the flops.  The scan buys depth log T; where one step over the whole
+// batch already fills all 148 SMs (C2: 384 tiles of 128 x 160) the sequential form is the faster one.  For small n and
+// batch - the paper's own regime - the scan runs on the device too (riccati_scan.cu; kalman_use_scan picks), and the
+// gains of all steps then come out of ONE pass of the three kernels below.  DESIGN.md section 7.
 #include <cuda.h>
 
 #include <algorithm>
@@ -30,6 +30,13 @@ namespace ltv {
 namespace {
 
 constexpr int kRowWarps = 8;   // warps per CTA of the row kernels
+
+// offset of (item b, step j) in an array, for a flattened pair index it = b * nj + j
+struct Stride2 {
+  long long sb, sj;
+  int nj;
+  __device__ __forceinline__ long long at(int it) const { return (it / nj) * sb + (it % nj) * sj; }
+};
 // measured on B200 (C2 p = 6, C4 p = 12; the variants differ by < 10 %): p <= 8 runs best with two CTAs per SM and the
 // loop not unrolled, wider p with one CTA per SM and two passes in flight
 template <int PG> struct RowCfg {
@@ -91,10 +98,10 @@ __device__ __forceinline__ void row_dots(const float4* const (&rows)[ROWS], cons
 // G[b][q][j] = sum_k Pi[b][j][k] C[b][q][k]  (= (C Pi)[q][j]: Pi is symmetric, so its ROW j serves as column j and the
 // loads are contiguous).  Warp = ROWS rows of Pi; grid (ceil(n / (8 ROWS)), batch), 256 threads.
 template <int PG, int ROWS>
-__global__ void __launch_bounds__(32 * kRowWarps, RowCfg<PG>::kMinBlocks) kalman_cpi_kernel(const float* __restrict__ C, long long c_stride,
-                                                                    const float* __restrict__ Pi, long long pi_stride,
+__global__ void __launch_bounds__(32 * kRowWarps, RowCfg<PG>::kMinBlocks) kalman_cpi_kernel(const float* __restrict__ C, Stride2 c_stride,
+                                                                    const float* __restrict__ Pi, Stride2 pi_stride,
                                                                     float* __restrict__ G, int n, int p) {
-  const int b = blockIdx.y;
+  const int b = blockIdx.y;   // (item, step) pair
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int j0 = (blockIdx.x * kRowWarps + warp) * ROWS;
   if (j0 >= n) return;
@@ -102,9 +109,9 @@ __global__ void __launch_bounds__(32 * kRowWarps, RowCfg<PG>::kMinBlocks) kalman
   const float4* rows[ROWS];
 #pragma unroll
   for (int r = 0; r < ROWS; ++r)
-    rows[r] = reinterpret_cast<const float4*>(Pi + b * pi_stride + static_cast<size_t>(min(j0 + r, n - 1)) * n);
+    rows[r] = reinterpret_cast<const float4*>(Pi + pi_stride.at(b) + static_cast<size_t>(min(j0 + r, n - 1)) * n);
   float acc[ROWS][8 * PG];
-  row_dots<PG, ROWS>(rows, C + b * c_stride, n4, p, lane, acc);
+  row_dots<PG, ROWS>(rows, C + c_stride.at(b), n4, p, lane, acc);
   float* Gb = G + static_cast<size_t>(b) * p * n;
 #pragma unroll
   for (int q = 0; q < 8 * PG; ++q) {
@@ -119,15 +126,15 @@ __global__ void __launch_bounds__(32 * kRowWarps, RowCfg<PG>::kMinBlocks) kalman
 // One CTA per item: S = diag(f)^2 + G C^T (lower triangle; warp per entry), Cholesky S = R R^T (warp 0, lane = row),
 // K = S^{-1} G (thread per column).  256 threads; shared memory: S [32][33].
 template <int PG>
-__global__ void __launch_bounds__(256) kalman_gain_kernel(const float* __restrict__ C, long long c_stride,
-                                                          const float* __restrict__ f, long long f_stride,
+__global__ void __launch_bounds__(256) kalman_gain_kernel(const float* __restrict__ C, Stride2 c_stride,
+                                                          const float* __restrict__ f, Stride2 f_stride,
                                                           const float* __restrict__ G, float* __restrict__ K, int n,
                                                           int p) {
   constexpr int PP = 8 * PG;
   __shared__ float S[32][33];
   const int b = blockIdx.x;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const float4* C4 = reinterpret_cast<const float4*>(C + b * c_stride);
+  const float4* C4 = reinterpret_cast<const float4*>(C + c_stride.at(b));
   const float* Gb = G + static_cast<size_t>(b) * p * n;
   const float4* G4 = reinterpret_cast<const float4*>(Gb);
   float* Kb = K + static_cast<size_t>(b) * p * n;
@@ -152,7 +159,7 @@ __global__ void __launch_bounds__(256) kalman_gain_kernel(const float* __restric
     for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     if (lane == 0) {
       if (q == r) {
-        const float ff = __ldg(f + b * f_stride + q);
+        const float ff = __ldg(f + f_stride.at(b) + q);
         s = fmaf(ff, ff, s);
       }
       S[q][r] = s;
@@ -206,8 +213,8 @@ __global__ void __launch_bounds__(256) kalman_gain_kernel(const float* __restric
 // grid (ceil(n / (8 ROWS)), batch), 256 threads.
 template <int PG, int ROWS>
 __global__ void __launch_bounds__(32 * kRowWarps, RowCfg<PG>::kMinBlocks) kalman_closed_loop_kernel(
-    const float* __restrict__ A, long long a_stride, const float* __restrict__ C, long long c_stride,
-    const float* __restrict__ K, float* __restrict__ Lt, long long lt_stride, float* __restrict__ Abar, int n, int p) {
+    const float* __restrict__ A, Stride2 a_stride, const float* __restrict__ C, Stride2 c_stride,
+    const float* __restrict__ K, float* __restrict__ Lt, Stride2 lt_stride, float* __restrict__ Abar, int n, int p) {
   constexpr int PP = 8 * PG;
   const int b = blockIdx.y;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -217,7 +224,7 @@ __global__ void __launch_bounds__(32 * kRowWarps, RowCfg<PG>::kMinBlocks) kalman
   const float4* rows[ROWS];
 #pragma unroll
   for (int r = 0; r < ROWS; ++r)
-    rows[r] = reinterpret_cast<const float4*>(A + b * a_stride + static_cast<size_t>(min(i0 + r, n - 1)) * n);
+    rows[r] = reinterpret_cast<const float4*>(A + a_stride.at(b) + static_cast<size_t>(min(i0 + r, n - 1)) * n);
   float acc[ROWS][PP];
   row_dots<PG, ROWS>(rows, K + static_cast<size_t>(b) * p * n, n4, p, lane, acc);
 #pragma unroll
@@ -226,11 +233,12 @@ __global__ void __launch_bounds__(32 * kRowWarps, RowCfg<PG>::kMinBlocks) kalman
 #pragma unroll
       for (int r = 0; r < ROWS; ++r) {
         acc[r][q] = -acc[r][q];
-        if (lane == (q & 31) && i0 + r < n) Lt[b * lt_stride + static_cast<size_t>(i0 + r) * p + q] = acc[r][q];
+        if (lane == (q & 31) && i0 + r < n) Lt[lt_stride.at(b) + static_cast<size_t>(i0 + r) * p + q] = acc[r][q];
       }
     }
   }
-  const float4* C4 = reinterpret_cast<const float4*>(C + b * c_stride);
+  if (Abar == nullptr) return;   // gains only (the scan path has no use for the closed-loop matrix)
+  const float4* C4 = reinterpret_cast<const float4*>(C + c_stride.at(b));
 #pragma unroll
   for (int q = 0; q < PP; ++q)
     if (q >= p) {
@@ -333,10 +341,63 @@ size_t carve(size_t floats) { return align_up(floats * sizeof(float), 256); }
 
 }  // namespace
 
+// G = C Pi, K = (F F^T + G C^T)^{-1} G, Lt = -A K^T (and Abar = A + Lt C unless Abar == nullptr) for the steps
+// j0 .. j0 + nj - 1 of every item at once (three launches).  The recursion calls it with nj = 1 once Pi_j exists; the
+// scan path calls it once with j0 = 0, nj = T after all Pi_j are known.  G, K: [batch nj][p][n]; Abar: [batch][n][n]
+// (nj = 1 only).
+cudaError_t launch_kalman_gain_chain(const KalmanArgs& a, int j0, int nj, float* G, float* K, float* Abar,
+                                     cudaStream_t stream) {
+  const int batch = a.batch, T = a.T, n = a.n, p = a.p;
+  const int pairs = batch * nj;
+  const Stride2 sC{static_cast<long long>(T) * p * n, static_cast<long long>(p) * n, nj};
+  const Stride2 sA{static_cast<long long>(T) * n * n, static_cast<long long>(n) * n, nj};
+  const Stride2 sPi{static_cast<long long>(T + 1) * n * n, static_cast<long long>(n) * n, nj};
+  const Stride2 sF{static_cast<long long>(T) * p, p, nj};
+  const Stride2 sLt{static_cast<long long>(T) * n * p, static_cast<long long>(n) * p, nj};
+  const float* Cj = a.C + static_cast<size_t>(j0) * p * n;
+  const float* Aj = a.A + static_cast<size_t>(j0) * n * n;
+  const float* Pij = a.Pi_out + static_cast<size_t>(j0) * n * n;
+  return dispatch_pg(p, [&](auto pg) {
+    constexpr int PG = decltype(pg)::value;
+    constexpr int ROWS = RowCfg<PG>::kRows;
+    const dim3 rgrid((n + kRowWarps * ROWS - 1) / (kRowWarps * ROWS), pairs);
+    {
+      ProfScope prof(kProfKalmanSimt, stream);
+      kalman_cpi_kernel<PG, ROWS><<<rgrid, 32 * kRowWarps, 0, stream>>>(Cj, sC, Pij, sPi, G, n, p);
+    }
+    cudaError_t ee = cudaGetLastError();
+    if (ee != cudaSuccess) return ee;
+    {
+      ProfScope prof(kProfKalmanSimt, stream);
+      kalman_gain_kernel<PG><<<pairs, 256, 0, stream>>>(Cj, sC, a.f + static_cast<size_t>(j0) * p, sF, G, K, n, p);
+    }
+    if ((ee = cudaGetLastError()) != cudaSuccess) return ee;
+    {
+      ProfScope prof(kProfKalmanSimt, stream);
+      kalman_closed_loop_kernel<PG, ROWS><<<rgrid, 32 * kRowWarps, 0, stream>>>(
+          Aj, sA, Cj, sC, K, a.Lt_out + static_cast<size_t>(j0) * n * p, sLt, Abar, n, p);
+    }
+    return cudaGetLastError();
+  });
+}
+
 size_t kalman_workspace_bytes(int batch, int T, int n, int p) {
-  (void)T;
   const size_t b = batch, nn = n, pp = p;
-  return 2 * carve(b * pp * nn) + 2 * carve(b * nn * nn);
+  const size_t rec = 2 * carve(b * pp * nn) + 2 * carve(b * nn * nn);
+  if (!riccati_scan_supported(n)) return rec;
+  const size_t scan = riccati_scan_workspace_bytes(batch, T, n) + 2 * carve(b * T * pp * nn);
+  return rec > scan ? rec : scan;
+}
+
+// The scan (riccati_scan.cu) pays when its log2(T+1) levels of (T+1)/2 combinations per item fit the machine in about
+// one wave and the recursion's T steps would each be a handful of latency-bound launches: small n, small batch.
+static bool kalman_use_scan(const KalmanArgs& a, int sms) {
+  if (a.mode == 2 || !riccati_scan_supported(a.n)) return false;
+  if (a.mode == 1) return true;
+  const int forced = env_int("KALMAN_SCAN", -1);
+  if (forced >= 0) return forced != 0;
+  // measured on B200 (n = 48, p = 6): T = 16: 414 vs 465 us, T = 64: 578 vs 1841 us, T = 128: 665 vs 3675 us (batch 1-8)
+  return a.T >= 16 && static_cast<long long>(a.batch) * (a.T + 1) / 2 <= 2ll * sms;
 }
 
 cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned long long* launches) {
@@ -345,6 +406,18 @@ cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned lon
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   const int batch = a.batch, T = a.T, n = a.n, p = a.p;
   const size_t b = batch, nn = n, pp = p;
+  if (kalman_use_scan(a, sms)) {
+    // Pi_0 .. Pi_T by the associative scan (16)(17), then the gains of all steps in one batched pass
+    char* cur = static_cast<char*>(a.workspace);
+    float* AD = reinterpret_cast<float*>(cur); cur += riccati_scan_workspace_bytes(batch, T, n);
+    float* G = reinterpret_cast<float*>(cur); cur += carve(b * T * pp * nn);
+    float* K = reinterpret_cast<float*>(cur);
+    cudaError_t es = launch_riccati_scan(a, AD, stream, launches);
+    if (es != cudaSuccess) return es;
+    es = launch_kalman_gain_chain(a, 0, T, G, K, nullptr, stream);
+    if (es == cudaSuccess) *launches += 3;
+    return es;
+  }
   KalmanWs w;
   char* cur = static_cast<char*>(a.workspace);
   w.G = reinterpret_cast<float*>(cur); cur += carve(b * pp * nn);
@@ -384,36 +457,8 @@ cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned lon
     if ((e = bgemm_tc_make_maps(g2, maps2)) != cudaSuccess) return e;
   }
 
-  const long long c_stride = static_cast<long long>(T) * p * n, a_stride = static_cast<long long>(T) * n * n;
-  const long long pi_stride = static_cast<long long>(T + 1) * n * n;
   for (int j = 0; j < T; ++j) {
-    const float* Cj = a.C + static_cast<size_t>(j) * p * n;
-    const float* Aj = a.A + static_cast<size_t>(j) * n * n;
-    const float* Pij = a.Pi_out + static_cast<size_t>(j) * n * n;
-    e = dispatch_pg(p, [&](auto pg) {
-      constexpr int PG = decltype(pg)::value;
-      constexpr int ROWS = RowCfg<PG>::kRows;
-      const dim3 rgrid((n + kRowWarps * ROWS - 1) / (kRowWarps * ROWS), batch);
-      {
-        ProfScope prof(kProfKalmanSimt, stream);
-        kalman_cpi_kernel<PG, ROWS><<<rgrid, 32 * kRowWarps, 0, stream>>>(Cj, c_stride, Pij, pi_stride, w.G, n, p);
-      }
-      cudaError_t ee = cudaGetLastError();
-      if (ee != cudaSuccess) return ee;
-      {
-        ProfScope prof(kProfKalmanSimt, stream);
-        kalman_gain_kernel<PG><<<batch, 256, 0, stream>>>(Cj, c_stride, a.f + static_cast<size_t>(j) * p,
-                                                          static_cast<long long>(T) * p, w.G, w.K, n, p);
-      }
-      if ((ee = cudaGetLastError()) != cudaSuccess) return ee;
-      {
-        ProfScope prof(kProfKalmanSimt, stream);
-        kalman_closed_loop_kernel<PG, ROWS><<<rgrid, 32 * kRowWarps, 0, stream>>>(
-            Aj, a_stride, Cj, c_stride, w.K, a.Lt_out + static_cast<size_t>(j) * n * p,
-            static_cast<long long>(T) * n * p, w.Abar, n, p);
-      }
-      return cudaGetLastError();
-    });
+    e = launch_kalman_gain_chain(a, j, 1, w.G, w.K, w.Abar, stream);
     if (e != cudaSuccess) return e;
     *launches += 3;
     g1.r_blk0 = j;

@@ -48,7 +48,12 @@ struct KalmanArgs {
   float *Lt_out, *Pi_out;
   int batch, T, n, p;
   void* workspace;
+  int mode = 0;   // 0: pick (kalman_use_scan), 1: associative scan (16)(17) (n <= 64), 2: recursion (13)
 };
+// riccati_scan.cu
+bool riccati_scan_supported(int n);
+size_t riccati_scan_workspace_bytes(int batch, int T, int n);
+cudaError_t launch_riccati_scan(const KalmanArgs& a, float* AD, cudaStream_t stream, unsigned long long* launches);
 size_t kalman_workspace_bytes(int batch, int T, int n, int p);
 cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned long long* launches);
 

@@ -83,7 +83,9 @@ def test_host_side_validation_needs_no_gpu(L):
     k = L.lib.ltv_scan_kalman_gains
     assert k(p, p, p, p, None, p, p, 1, 2, 4, 2, 0, p, 1 << 20, None) == 1              # NULL Pi0
     assert k(p, p, p, p, p, p, p, 1, 2, 4, 0, 0, p, 1 << 20, None) == 2                 # p = 0
-    assert k(p, p, p, p, p, p, p, 1, 2, 4, 2, 1, p, 1 << 20, None) == 2                 # unknown flag
+    assert k(p, p, p, p, p, p, p, 1, 2, 4, 2, 4, p, 1 << 20, None) == 2                 # unknown flag
+    assert k(p, p, p, p, p, p, p, 1, 2, 4, 2, 3, p, 1 << 20, None) == 2                 # scan AND recursion
+    assert k(p, p, p, p, p, p, p, 1, 2, 128, 2, 1, p, 1 << 20, None) == 3               # scan path needs n <= 64
     assert k(p, p, p, p, p, p, p, 1, 2, 4, 33, 0, p, 1 << 20, None) == 3                # p > 32
     assert k(p, p, p, odd, p, p, p, 1, 2, 4, 2, 0, p, 1 << 20, None) == 4               # misaligned f
     assert k(p, p, p, p, p, p, p, 1, 2, 4, 2, 0, p, 8, None) == 5                       # workspace too small

@@ -24,17 +24,17 @@ def L():
     return lib
 
 
-def _run(L, A, M):
+def _run(L, A, M, mode=0):
     import torch
 
     d = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (A, M["C"], M["e"], M["f"], M["Pi0"])]
-    Lt, Pi = L.ltv_scan_kalman_gains(*d)
+    Lt, Pi = L.ltv_scan_kalman_gains(*d, mode=mode)
     torch.cuda.synchronize()
     return Lt.cpu().numpy(), Pi.cpu().numpy()
 
 
-def _check(L, A, M):
-    Lt, Pi = _run(L, A, M)
+def _check(L, A, M, mode=0):
+    Lt, Pi = _run(L, A, M, mode)
     Pi_ref, Lt_ref = O.kalman_recursion(A, M["C"], M["e"], M["f"], M["Pi0"])
     assert np.array_equal(Pi[:, 0], M["Pi0"])
     assert O.rel_err(Pi, Pi_ref) <= TOL
@@ -61,6 +61,33 @@ def test_kalman_dense_random(L, n, T, batch, p, kind):
     W = dense_random(batch, T, n, 1, seed=7 * n + p, scale=0.4)
     M = observation_model(batch, T, n, p, seed=3 * n + p, kind=kind)
     _check(L, W.A, M)
+
+
+@pytest.mark.parametrize("n,T,batch,p,kind", [(48, 16, 1, 6, "track"),    # C1 shape: 17 elements, 5 levels
+                                              (48, 6, 2, 3, "dense"),     # 7 elements: ragged last segment
+                                              (64, 9, 3, 8, "dense"),     # largest n of the scan path
+                                              (40, 1, 2, 2, "dense"),     # a single step: one combination
+                                              (20, 31, 2, 1, "dense")])   # 32 elements: full binary tree, p = 1
+def test_kalman_riccati_scan_path(L, n, T, batch, p, kind):
+    """The associative scan (16)(17) on the device (flags = LTV_KALMAN_SCAN) against the oracle RECURSION (13): the
+    paper's claim that the scan reaches the recursion's result, checked on the GPU; and against the recursion path of the
+    same call (flags = LTV_KALMAN_RECURSION)."""
+    W = dense_random(batch, T, n, 1, seed=17 * n + p, scale=0.4)
+    M = observation_model(batch, T, n, p, seed=5 * n + p, kind=kind)
+    Lt_s, Pi_s = _check(L, W.A, M, mode=L.LTV_KALMAN_SCAN)
+    Lt_r, Pi_r = _check(L, W.A, M, mode=L.LTV_KALMAN_RECURSION)
+    assert O.rel_err(Pi_s, Pi_r) <= TOL and O.rel_err(Lt_s, Lt_r) <= TOL
+
+
+def test_kalman_scan_rejects_large_n(L):
+    import torch
+
+    A = torch.zeros((1, 2, 128, 128), device="cuda")
+    with pytest.raises(L.LtvError) as ei:
+        L.ltv_scan_kalman_gains(A, torch.zeros((1, 2, 4, 128), device="cuda"), torch.ones((1, 2, 128), device="cuda"),
+                                torch.ones((1, 2, 4), device="cuda"), torch.zeros((1, 128, 128), device="cuda"),
+                                mode=L.LTV_KALMAN_SCAN)
+    assert ei.value.status == 3
 
 
 @pytest.mark.parametrize("ci,T", [(0, 16), (1, 6), (2, 4)])
