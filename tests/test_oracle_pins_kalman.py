@@ -171,3 +171,23 @@ def test_kalman_gains_close_the_observer_loop():
     PhiX, _ = O.observer_response_item(A, Lt, C)
     for j in range(T - 1):
         _close(Pi[j + 1], PhiX[O.packed_index(j + 1, j)] @ Pi[j] @ A[j].T + np.diag(e[j] ** 2), 1e-9)
+
+
+def test_kalman_hand_example_exact():
+    """One and two steps by hand (all values dyadic or small rationals).  A = [[1,1],[0,1]], C = [1 0], E = diag(0,1),
+    F = 1, Pi_0 = I:
+      step 0: S = 1 + 1 = 2; C Pi A^T = [1 0]; L_1 = -[1/2 0]; A Pi C^T = [1 0]^T
+              Pi_1 = diag(0,1) + A A^T + [1 0]^T L_1 = [[0,0],[0,1]] + [[2,1],[1,1]] + [[-1/2,0],[0,0]] = [[3/2,1],[1,2]]
+      step 1: S = 1 + 3/2 = 5/2; C Pi_1 A^T = [3/2 1] A^T = [5/2 1]; L_2 = -[1 2/5];
+              A Pi_1 A^T = [[11/2,3],[3,2]]; A Pi_1 C^T = [5/2 1]^T; [5/2 1]^T L_2 = -[[5/2,1],[1,2/5]]
+              Pi_2 = [[0,0],[0,1]] + [[11/2,3],[3,2]] - [[5/2,1],[1,2/5]] = [[3,2],[2,13/5]]"""
+    A = np.broadcast_to(np.array([[1.0, 1.0], [0.0, 1.0]]), (2, 2, 2))
+    C = np.broadcast_to(np.array([[1.0, 0.0]]), (2, 1, 2))
+    e = np.broadcast_to(np.array([0.0, 1.0]), (2, 2))
+    f = np.ones((2, 1))
+    Pi, Lt = O.kalman_recursion_item(A, C, e, f, np.eye(2))
+    assert np.array_equal(Pi[1], np.array([[1.5, 1.0], [1.0, 2.0]]))
+    assert np.array_equal(Lt[0], np.array([[-0.5], [0.0]]))
+    np.testing.assert_allclose(Lt[1], np.array([[-1.0], [-0.4]]), rtol=1e-15)
+    np.testing.assert_allclose(Pi[2], np.array([[3.0, 2.0], [2.0, 2.6]]), rtol=1e-15)
+    np.testing.assert_allclose(O.riccati_scan_item(A, C, e, f, np.eye(2))[2], np.array([[3.0, 2.0], [2.0, 2.6]]), rtol=1e-14)
