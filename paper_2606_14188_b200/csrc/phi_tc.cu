@@ -672,8 +672,15 @@ cudaError_t launch_bgemm_tc(const BatchedGemm& a, int nch, const void* maps, int
   const TcMaps& m = *static_cast<const TcMaps*>(maps);
   const int Mt1 = (a.M + kTM - 1) / kTM, Mt2 = (a.M + 2 * kTM - 1) / (2 * kTM);
   const int mode = env_int("TC_PAIR", -1);
-  const bool pair = (mode == 1) || (mode == -1 && 2 * Mt2 * 100 <= Mt1 * 108);
   const int nt = 32 * nch;
+  // Shape by a wave model: rounds of tiles over the CTAs (or CTA pairs) x relative time per tile.  A pair tile keeps the
+  // tensor pipe ~92 % busy against ~65 % for the single-CTA shape (profiles/r1_v5_phi_combine_tc_full.md) but pays a
+  // cluster launch and two cluster barriers (15 %, fitted: C2 384 single tiles 33.3 us vs 256 pair tiles 35.6 us;
+  // C3 320 vs 192: 49.4 vs 45.3 us).
+  const long long ntile = (a.N + nt - 1) / nt;
+  const long long r1 = (static_cast<long long>(a.count) * Mt1 * ntile + num_sms - 1) / num_sms;
+  const long long r2 = (static_cast<long long>(a.count) * Mt2 * ntile + num_sms / 2 - 1) / (num_sms / 2);
+  const bool pair = (mode == 1) || (mode == -1 && r2 * 125 < r1 * 154);
   p.g = PhiGeom{};
   p.g.n = a.K;
   p.g.nc = a.N;
