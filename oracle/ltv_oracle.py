@@ -40,6 +40,9 @@ sequential recursion - "We obtain the solution to (14) by a forward parallel ass
                    (17), folded in the order Pi_j = P~ of e_{j-1} (x) ... (x) e_0 (x) e_init          garbled in the source and
                                                                      is re-derived from the conditional
                                                                      value function of :166 (DESIGN.md q14)
+  assemble_output_feedback   Phi^xw = Phibar^x + Phihat^x - Phibar^x M Phihat^x,  Phi^uw = Phibar^u (I - M Phihat^x),      PAPER.md:162-164 eq.(15),
+                   Phi^xe = Phihat^y - Phibar^x M Phihat^y,  Phi^ue = -Phibar^u M Phihat^y,  M = I - Z A                 dense block operators
+                                                                     (DESIGN.md q20, q21)
   adjoint          lam_T = g_T; lam_t = A_t^T lam_{t+1} + g_t;       PAPER.md:106-110 eq.(10) chained
                    grad_u[t] = B_t^T lam_{t+1}; grad_x0 = A_0^T lam_1   over the horizon; north_star (iii)
 
@@ -52,7 +55,9 @@ Pins (tests/test_oracle_pins.py): every function below is pinned by closed forms
 (12c), brute force on tiny inputs, a hand-computed worked example (tests/golden/hand_example.txt) and the
 tube-containment / adjoint dot-product invariants.  kalman_recursion / riccati_* are pinned in
 tests/test_oracle_pins_kalman.py (brute-force Gaussian conditioning, information form, DARE fixed point from
-scipy, Lyapunov sum through Phi, Joseph form + gain optimality, scan = recursion, associativity).
+scipy, Lyapunov sum through Phi, Joseph form + gain optimality, scan = recursion, associativity);
+assemble_output_feedback in tests/test_oracle_pins_assembly.py (both achievability identities of (12c), a step-by-step
+simulation of plant + observer + controller, the augmented closed-loop system, the limits L = 0 and K = 0).
 Nothing in this file is "parity unpinned".
 """
 from __future__ import annotations
@@ -143,6 +148,36 @@ def observer_response_item(A, Lt, C):
 def observer_response(A, Lt, C):
     out = [observer_response_item(A[b], Lt[b], C[b]) for b in range(A.shape[0])]
     return np.stack([o[0] for o in out]), np.stack([o[1] for o in out])
+
+
+# --------------------------------------------------------------------------- assembly (15)
+def shift_operator(A):
+    """Z blkdiag(A_0 .. A_{T-1}) as a dense [T n, T n] matrix: block (t+1, t) = A_t (Z = block down-shift, PAPER.md:150;
+    A_{T-1} falls off the end).  Works for any per-step blocks A[T, r, c] (returns [T r, T c])."""
+    A = _f64(A)
+    T, r, c = A.shape
+    Z = np.zeros((T * r, T * c))
+    for t in range(T - 1):
+        Z[(t + 1) * r:(t + 2) * r, t * c:(t + 1) * c] = A[t]
+    return Z
+
+
+def assemble_output_feedback(A, PhibarX, PhibarU, PhihatX, PhihatY):
+    """Eq.(15) written out on dense block operators over the T steps of one item:
+        M = I - Z A
+        Phi^xw = Phibar^x + Phihat^x - Phibar^x M Phihat^x        Phi^uw = Phibar^u (I - M Phihat^x)
+        Phi^xe = Phihat^y - Phibar^x M Phihat^y                   Phi^ue = -Phibar^u M Phihat^y
+    A[T,n,n]; PhibarX, PhihatX [T n, T n]; PhibarU [T m, T n]; PhihatY [T n, T p], all block lower triangular.
+    Returns (Phixw, Phiuw, Phixe, Phiue)."""
+    A = _f64(A)
+    Pbx, Pbu, Phx, Phy = _f64(PhibarX), _f64(PhibarU), _f64(PhihatX), _f64(PhihatY)
+    N = Pbx.shape[0]
+    M = np.eye(N) - shift_operator(A)
+    Phixw = Pbx + Phx - Pbx @ M @ Phx
+    Phiuw = Pbu @ (np.eye(N) - M @ Phx)
+    Phixe = Phy - Pbx @ M @ Phy
+    Phiue = -Pbu @ M @ Phy
+    return Phixw, Phiuw, Phixe, Phiue
 
 
 # --------------------------------------------------------------------------- Kalman recursion (13), Riccati scan (16)(17)

@@ -1,0 +1,113 @@
+"""Pins for oracle.assemble_output_feedback (eq.(15)) against things other than
+itself.  The operators Phibar (state feedback) and Phihat (observer) are built here from gains K_k, Lt_k with the
+pinned oracles system_response / observer_response; the assembled Phi must then
+  * satisfy BOTH achievability identities of (12c),
+  * reproduce a step-by-step simulation of plant + predictor-form observer + controller u = K xhat,
+  * equal the blocks of the system response of the augmented closed loop in (x, x - xhat),
+  * reduce to the open loop for L = 0 (no information, no action) and for K = 0.
+Conventions (DESIGN.md q20, q21): the disturbance w~_k enters x_k directly (Phi(k,k) = I, w~_0 = x_0); the observation
+noise e~_k is that of the measurement of x_{k-1} (PAPER.md:125 y_{k+1} = h(q_k) + F e_k), so it enters the estimation
+error of step k through Lt_{k-1}: Phihat^y(k,j) = Phihat^x(k,j) Lt_{j-1}, j >= 1."""
+import numpy as np
+
+from oracle import ltv_oracle as O
+
+
+def _setup(T, n, m, p, seed, Kscale=0.3, Lscale=0.3):
+    rng = np.random.default_rng(seed)
+    A = np.eye(n)[None] + rng.normal(0.0, 0.4 / np.sqrt(n), (T, n, n))
+    B = rng.normal(0.0, 1.0, (T, n, m))
+    C = rng.normal(0.0, 1.0 / np.sqrt(n), (T, p, n))
+    K = Kscale * rng.normal(0.0, 1.0 / np.sqrt(n), (T, m, n))
+    Lt = Lscale * rng.normal(0.0, 1.0, (T, n, p))
+    return A, B, C, K, Lt
+
+
+def _dense(blocks, T, n, ncol=None):
+    """packed strictly-lower blocks (t,s) + identity diagonal -> dense [T n, T n]"""
+    D = np.eye(T * n)
+    for t in range(1, T):
+        for s in range(t):
+            D[t * n:(t + 1) * n, s * n:(s + 1) * n] = blocks[O.packed_index(t, s)]
+    return D
+
+
+def _operators(A, B, C, K, Lt):
+    T, n, _ = A.shape
+    m, p = B.shape[2], C.shape[1]
+    Atil = A + B @ K
+    PbX = _dense(O.system_response_item(Atil), T, n)
+    PbU = np.zeros((T * m, T * n))
+    for k in range(T):
+        PbU[k * m:(k + 1) * m] = K[k] @ PbX[k * n:(k + 1) * n]
+    PhX = _dense(O.observer_response_item(A, Lt, C)[0], T, n)
+    PhY = np.zeros((T * n, T * p))
+    for j in range(1, T):
+        PhY[:, j * p:(j + 1) * p] = PhX[:, j * n:(j + 1) * n] @ Lt[j - 1]
+    return PbX, PbU, PhX, PhY
+
+
+def test_assembly_satisfies_both_identities_of_12c():
+    T, n, m, p = 5, 4, 2, 2
+    A, B, C, K, Lt = _setup(T, n, m, p, 1)
+    Pxw, Puw, Pxe, Pue = O.assemble_output_feedback(A, *_operators(A, B, C, K, Lt))
+    N = T * n
+    M, ZB, ZC = np.eye(N) - O.shift_operator(A), O.shift_operator(B), O.shift_operator(C)
+    Phi = np.block([[Pxw, Pxe], [Puw, Pue]])
+    np.testing.assert_allclose(np.hstack([M, -ZB]) @ Phi, np.hstack([np.eye(N), np.zeros((N, T * p))]), atol=1e-12)
+    np.testing.assert_allclose(Phi @ np.vstack([M, -ZC]), np.vstack([np.eye(N), np.zeros((T * m, N))]), atol=1e-12)
+
+
+def test_assembly_reproduces_the_simulated_closed_loop():
+    T, n, m, p = 6, 4, 2, 2
+    A, B, C, K, Lt = _setup(T, n, m, p, 2)
+    Pxw, Puw, Pxe, Pue = O.assemble_output_feedback(A, *_operators(A, B, C, K, Lt))
+    rng = np.random.default_rng(3)
+    w, e = rng.normal(size=(T, n)), rng.normal(size=(T, p))
+    e[0] = 0.0                                         # no measurement precedes step 0
+    x, xh = w[0].copy(), np.zeros(n)                   # x_0 = w~_0, xhat_0 = 0
+    X, U = [], []
+    for k in range(T):
+        u = K[k] @ xh
+        X.append(x.copy()); U.append(u.copy())
+        if k + 1 < T:
+            y = C[k] @ x + e[k + 1]                    # measurement of x_k, noise e~_{k+1}
+            xh = A[k] @ xh + B[k] @ u - Lt[k] @ (y - C[k] @ xh)
+            x = A[k] @ x + B[k] @ u + w[k + 1]
+    np.testing.assert_allclose(np.concatenate(X), Pxw @ w.ravel() + Pxe @ e.ravel(), atol=1e-11)
+    np.testing.assert_allclose(np.concatenate(U), Puw @ w.ravel() + Pue @ e.ravel(), atol=1e-11)
+
+
+def test_assembly_is_the_augmented_closed_loop_response():
+    """xi = (x, eps), eps = x - xhat: xi_{k+1} = [[A + B K, -B K], [0, A + Lt C]] xi_k + [I; I] w~ + [0; Lt] e~.
+    Phi^xw(k,j) = [I 0] Phi_aug(k,j) [I; I],  Phi^xe(k,j) = [I 0] Phi_aug(k,j) [0; Lt_{j-1}] - what the existing Phi scan
+    computes when it is run on the 2n-state augmented system (the GPU test does exactly that)."""
+    T, n, m, p = 5, 3, 2, 2
+    A, B, C, K, Lt = _setup(T, n, m, p, 4)
+    Pxw, Puw, Pxe, Pue = O.assemble_output_feedback(A, *_operators(A, B, C, K, Lt))
+    Aaug = np.zeros((T, 2 * n, 2 * n))
+    Aaug[:, :n, :n] = A + B @ K
+    Aaug[:, :n, n:] = -(B @ K)
+    Aaug[:, n:, n:] = A + Lt @ C
+    Paug = O.system_response_item(Aaug)
+    for k in range(T):
+        for j in range(k + 1):
+            G = np.eye(2 * n) if k == j else Paug[O.packed_index(k, j)]
+            np.testing.assert_allclose(Pxw[k * n:(k + 1) * n, j * n:(j + 1) * n], G[:n, :n] + G[:n, n:], atol=1e-12)
+            np.testing.assert_allclose(Puw[k * m:(k + 1) * m, j * n:(j + 1) * n],
+                                       K[k] @ (G[:n, :n] + G[:n, n:] - G[n:, :n] - G[n:, n:]), atol=1e-12)
+            if j >= 1:
+                np.testing.assert_allclose(Pxe[k * n:(k + 1) * n, j * p:(j + 1) * p], G[:n, n:] @ Lt[j - 1], atol=1e-12)
+    assert np.max(np.abs(Pxe[:, :p])) == 0.0
+
+
+def test_assembly_limits_no_observer_gain_and_no_feedback_gain():
+    T, n, m, p = 5, 4, 2, 2
+    A, B, C, K, Lt = _setup(T, n, m, p, 5)
+    open_loop = _dense(O.system_response_item(A), T, n)
+    Pxw, Puw, Pxe, Pue = O.assemble_output_feedback(A, *_operators(A, B, C, K, 0.0 * Lt))
+    np.testing.assert_allclose(Pxw, open_loop, atol=1e-12)          # no information: the controller cannot act
+    assert np.max(np.abs(Puw)) < 1e-12 and np.max(np.abs(Pxe)) == 0.0 and np.max(np.abs(Pue)) == 0.0
+    Pxw, Puw, Pxe, Pue = O.assemble_output_feedback(A, *_operators(A, B, C, 0.0 * K, Lt))
+    np.testing.assert_allclose(Pxw, open_loop, atol=1e-12)          # no feedback: the estimate is never used
+    assert np.max(np.abs(Puw)) == 0.0 and np.max(np.abs(Pue)) == 0.0 and np.max(np.abs(Pxe)) < 1e-12
