@@ -1,0 +1,91 @@
+"""Eq.(15) on the device for controllers given by gains (first step): with u = K xhat and the
+predictor-form observer, the output-feedback closed loop is the LTV system xi_{k+1} = [[A + B K, -B K], [0, A + Lt C]] xi_k
+in xi = (x, x - xhat), so ONE call of ltv_scan_system_response_tube on the 2n-state augmented Jacobians yields every
+block of Phi^xw, Phi^xe (and Phi^uw, Phi^ue after the feedback gain): Phi^xw(k,j) = G11 + G12, Phi^xe(k,j) = G12 Lt_{j-1}
+with G = Phi_aug(k,j).  Checked against the pinned oracle assemble_output_feedback, which evaluates (15) as printed.
+(The block extraction below is test code; a dedicated assembly call for general Phibar is not built - DESIGN.md.)"""
+import numpy as np
+import pytest
+
+from oracle import ltv_oracle as O
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def L():
+    import torch
+
+    assert torch.cuda.is_available(), "GPU tests need a GPU (no CPU fallback)"
+    import __graft_entry__ as G
+
+    G.build()
+    import paper_2606_14188_b200 as lib
+
+    return lib
+
+
+def _gains(T, n, m, p, seed):
+    rng = np.random.default_rng(seed)
+    f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+    A = f32(np.eye(n)[None] + rng.normal(0.0, 0.4 / np.sqrt(n), (T, n, n)))
+    B = f32(rng.normal(0.0, 1.0, (T, n, m)))
+    C = f32(rng.normal(0.0, 1.0 / np.sqrt(n), (T, p, n)))
+    K = f32(0.3 * rng.normal(0.0, 1.0 / np.sqrt(n), (T, m, n)))
+    Lt = f32(0.3 * rng.normal(0.0, 1.0, (T, n, p)))
+    return A, B, C, K, Lt
+
+
+def _dense(blocks, T, n):
+    D = np.eye(T * n)
+    for t in range(1, T):
+        for s in range(t):
+            D[t * n:(t + 1) * n, s * n:(s + 1) * n] = blocks[O.packed_index(t, s)]
+    return D
+
+
+@pytest.mark.parametrize("n,T,m,p", [(24, 6, 2, 3),      # 2n = 48: fp32-FMA combine
+                                     (48, 7, 3, 4),      # 2n = 96: smallest tensor-core size
+                                     (132, 5, 6, 6)])    # 2n = 264: two n-tiles, ragged k-block
+def test_output_feedback_response_via_augmented_system(L, n, T, m, p):
+    import torch
+
+    A, B, C, K, Lt = _gains(T, n, m, p, seed=3 * n + T)
+    A64, B64, C64, K64, Lt64 = [a.astype(np.float64) for a in (A, B, C, K, Lt)]
+    # fp32 augmented Jacobians handed to the GPU (and, promoted, to the oracle operators below)
+    Aaug = np.zeros((1, T, 2 * n, 2 * n), dtype=np.float32)
+    BK = (B64 @ K64).astype(np.float32)
+    Aaug[0, :, :n, :n] = A + BK
+    Aaug[0, :, :n, n:] = -BK
+    Aaug[0, :, n:, n:] = (A64 + Lt64 @ C64).astype(np.float32)
+    w = np.ones((1, T, 2 * n), dtype=np.float32)
+    phi, _ = L.ltv_scan_system_response_tube(torch.from_numpy(Aaug).cuda(), torch.from_numpy(w).cuda())
+    torch.cuda.synchronize()
+    phi = phi[0].cpu().numpy()
+
+    # oracle: (15) as printed, on operators built from the SAME fp32 closed-loop matrices
+    Atil, Abar = Aaug[0, :, :n, :n].astype(np.float64), Aaug[0, :, n:, n:].astype(np.float64)
+    PbX = _dense(O.system_response_item(Atil), T, n)
+    PbU = np.vstack([K64[k] @ PbX[k * n:(k + 1) * n] for k in range(T)])
+    PhX = _dense(O.system_response_item(Abar), T, n)
+    PhY = np.zeros((T * n, T * p))
+    for j in range(1, T):
+        PhY[:, j * p:(j + 1) * p] = PhX[:, j * n:(j + 1) * n] @ Lt64[j - 1]
+    # M of (15) must be the open-loop I - Z A with A = Atil - B K = Abar - Lt C: use the fp32-consistent difference
+    Aopen = Atil - (-Aaug[0, :, :n, n:].astype(np.float64))
+    Pxw, Puw, Pxe, Pue = O.assemble_output_feedback(Aopen, PbX, PbU, PhX, PhY)
+
+    got_xw, ref_xw, got_xe, ref_xe, got_uw, ref_uw = [], [], [], [], [], []
+    for k in range(1, T):
+        for j in range(k):
+            G = phi[L.ltv_phi_block_index(T, k, j)].astype(np.float64)
+            got_xw.append(G[:n, :n] + G[:n, n:]); ref_xw.append(Pxw[k * n:(k + 1) * n, j * n:(j + 1) * n])
+            got_uw.append(K64[k] @ (G[:n, :n] + G[:n, n:] - G[n:, :n] - G[n:, n:]))
+            ref_uw.append(Puw[k * m:(k + 1) * m, j * n:(j + 1) * n])
+            if j >= 1:
+                got_xe.append(G[:n, n:] @ Lt64[j - 1]); ref_xe.append(Pxe[k * n:(k + 1) * n, j * p:(j + 1) * p])
+            assert np.all(G[n:, :n] == 0.0)        # block-triangular structure survives the scan exactly
+    assert O.rel_err(np.stack(got_xw), np.stack(ref_xw)) <= TOL
+    assert O.rel_err(np.stack(got_uw), np.stack(ref_uw)) <= TOL
+    assert O.rel_err(np.stack(got_xe), np.stack(ref_xe)) <= TOL
