@@ -180,6 +180,25 @@ def assemble_output_feedback(A, PhibarX, PhibarU, PhihatX, PhihatY):
     return Phixw, Phiuw, Phixe, Phiue
 
 
+def output_feedback_tube(Phixw, Phixe, w, f):
+    """Reachable-tube width of eq.(12e) as printed, both terms, for one item:
+        tau_k[i] = sum_{j=0}^{k-1} ( || row_i(Phi^xw(k,j) E_j) ||_2 + || row_i(Phi^xe(k,j) F~_j) ||_2 ),
+    E_j = diag(w[j]); F~_j = diag(f[j-1]) scales the noise of the measurement of x_{j-1} (DESIGN.md q21; no such term
+    for j = 0).  Phixw [T n, T n], Phixe [T n, T p] dense (from assemble_output_feedback); w[T,n], f[T,p] -> tau[T,n]."""
+    Pw, Pe, w, f = _f64(Phixw), _f64(Phixe), _f64(w), _f64(f)
+    T, n = w.shape
+    p = f.shape[1]
+    tau = np.zeros((T, n))
+    for k in range(1, T):
+        for j in range(k):
+            blk = Pw[k * n:(k + 1) * n, j * n:(j + 1) * n] @ np.diag(w[j])
+            tau[k] += np.sqrt(np.sum(blk ** 2, axis=1))
+            if j >= 1:
+                ble = Pe[k * n:(k + 1) * n, j * p:(j + 1) * p] @ np.diag(f[j - 1])
+                tau[k] += np.sqrt(np.sum(ble ** 2, axis=1))
+    return tau
+
+
 # --------------------------------------------------------------------------- Kalman recursion (13), Riccati scan (16)(17)
 def kalman_recursion_item(A, C, e, f, Pi0):
     """Backward-Kalman recursion of eq.(13), one item, written out step by step:

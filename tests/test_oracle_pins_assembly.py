@@ -111,3 +111,42 @@ def test_assembly_limits_no_observer_gain_and_no_feedback_gain():
     Pxw, Puw, Pxe, Pue = O.assemble_output_feedback(A, *_operators(A, B, C, 0.0 * K, Lt))
     np.testing.assert_allclose(Pxw, open_loop, atol=1e-12)          # no feedback: the estimate is never used
     assert np.max(np.abs(Puw)) == 0.0 and np.max(np.abs(Pue)) == 0.0 and np.max(np.abs(Pxe)) < 1e-12
+
+
+def test_output_feedback_tube_contains_the_simulated_loop_and_is_tight():
+    """(12e): for any ||d_j||_2 <= 1, ||g_j||_2 <= 1 the simulated state obeys |x_k[i]| <= tau_k[i] when w~_j = E_j d_j
+    (j < k; no direct term), e~_j = F~_j g_j; equality in row i for the aligned disturbances."""
+    T, n, m, p = 5, 4, 2, 2
+    A, B, C, K, Lt = _setup(T, n, m, p, 7)
+    rng = np.random.default_rng(8)
+    w, f = rng.uniform(0.1, 1.0, (T, n)), rng.uniform(0.1, 1.0, (T, p))
+    Pxw, Puw, Pxe, Pue = O.assemble_output_feedback(A, *_operators(A, B, C, K, Lt))
+    tau = O.output_feedback_tube(Pxw, Pxe, w, f)
+    assert np.all(tau[0] == 0.0)
+    k = T - 1
+    for i in range(n):
+        # aligned worst case for row i of x_k, disturbances at steps j < k only
+        wt, et = np.zeros((T, n)), np.zeros((T, p))
+        for j in range(k):
+            r = Pxw[k * n + i, j * n:(j + 1) * n] * w[j]
+            wt[j] = w[j] * r / np.linalg.norm(r)
+            if j >= 1:
+                q = Pxe[k * n + i, j * p:(j + 1) * p] * f[j - 1]
+                et[j] = f[j - 1] * q / np.linalg.norm(q)
+        xk = (Pxw @ wt.ravel() + Pxe @ et.ravel())[k * n + i]
+        assert abs(xk - tau[k, i]) <= 1e-12 * tau[k, i]
+    for _ in range(20):
+        d = rng.normal(size=(T, n)); d /= np.maximum(1.0, np.linalg.norm(d, axis=1, keepdims=True))
+        g = rng.normal(size=(T, p)); g /= np.maximum(1.0, np.linalg.norm(g, axis=1, keepdims=True))
+        wt, et = w * d, np.vstack([np.zeros((1, p)), f[:-1] * g[1:]])
+        wt[k:] = 0.0
+        x = (Pxw @ wt.ravel() + Pxe @ et.ravel()).reshape(T, n)
+        assert np.all(np.abs(x[k]) <= tau[k] * (1 + 1e-12))
+
+
+def test_output_feedback_tube_without_feedback_is_the_row2norm_tube():
+    T, n, m, p = 5, 4, 2, 2
+    A, B, C, K, Lt = _setup(T, n, m, p, 9)
+    w, f = np.random.default_rng(1).uniform(0.1, 1.0, (T, n)), np.ones((T, p))
+    Pxw, _, Pxe, _ = O.assemble_output_feedback(A, *_operators(A, B, C, 0.0 * K, Lt))
+    np.testing.assert_allclose(O.output_feedback_tube(Pxw, Pxe, w, f), O.tube_row2norm_item(A, w), rtol=1e-10, atol=1e-12)
