@@ -63,7 +63,8 @@ enum { LTV_OP_ROLLOUT = 0, LTV_OP_SYSTEM_RESPONSE_TUBE = 1, LTV_OP_ADJOINT = 2, 
        LTV_OP_PIPELINE_HOST_NO_PHI = 4 /* ltv_scan_pipeline_host with w_host == NULL: rollout + adjoint only */,
        LTV_OP_OBSERVER_RESPONSE = 5 /* ltv_scan_observer_response; pass p (rows of C) as `m` */,
        LTV_OP_KALMAN_GAINS = 6 /* ltv_scan_kalman_gains; pass p (rows of C) as `m` */,
-       LTV_OP_CONSTRAINT_TIGHTENING = 7 /* ltv_scan_constraint_tightening; pass nc (constraint rows) as `m` */ };
+       LTV_OP_CONSTRAINT_TIGHTENING = 7 /* ltv_scan_constraint_tightening; pass nc (constraint rows) as `m` */,
+       LTV_OP_OUTPUT_FEEDBACK = 8 /* ltv_scan_output_feedback_response; `m` is ignored */ };
 
 /* `phi_layout` argument.  COLUMN_PACKED (the only layout of this version): the P = T(T-1)/2 blocks of one
  * item are stored column by column of the block-lower-triangular operator; block (t,s), 0 <= s < t <= T-1,
@@ -193,6 +194,34 @@ LTV_API int ltv_scan_constraint_tightening(const float* A, const float* w, const
 LTV_API int ltv_scan_kalman_gains(const float* A, const float* C, const float* e, const float* f, const float* Pi0,
                                   float* Lt_out, float* Pi_out, int batch, int T, int n, int p, unsigned flags,
                                   void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Assembled output-feedback responses (first form; eq.(15)) and the reachable tube of
+ * eq.(12e) (:147) with both of its terms, for a controller given by GAINS: state feedback u_k = Kfb_k xhat_k on the
+ * estimate of the predictor-form observer xhat_{k+1} = A_k xhat_k + B_k u_k - Lt_k (y_k - C_k xhat_k), with Lt as
+ * ltv_scan_kalman_gains returns it.  With Phibar = (I - Z(A + B Kfb))^-1, Phihat = (I - Z(A + Lt C))^-1 (DESIGN.md q20, q21):
+ *     Phi^xw = Phibar^x + Phihat^x - Phibar^x M Phihat^x,      Phi^xe = Phihat^y - Phibar^x M Phihat^y,      M = I - Z A
+ *     tau_0 = 0;  tau_k[i] = sum_{j<k} ||row_i(Phi^xw(k,j) diag(w_j))||_2 + sum_{1<=j<k} ||row_i(Phi^xe(k,j) diag(f_{j-1}))||_2
+ *   A         device [batch,T,n,n]    required (A_0 .. A_{T-2} are read)
+ *   B         device [batch,T,n,m]    required, m >= 1
+ *   Kfb       device [batch,T,m,n]    required; state-feedback gains
+ *   Lt        device [batch,T,n,p]    required; Lt_k = L_{k+1}^T, 1 <= p <= 32
+ *   C         device [batch,T,p,n]    required
+ *   w         device [batch,T,n]      required; process-disturbance scaling E_j = diag(w_j)
+ *   f         device [batch,T,p]      required; observation-disturbance scaling; f_{j-1} scales the noise e~_j of the
+ *                                     measurement of x_{j-1}
+ *   phi_xw_out device [batch,P,n,n]   block (k,j), 0 <= j < k <= T-1, COLUMN_PACKED order (ltv_phi_block_index)
+ *   phi_xe_out device [batch,P,n,p]   same block order; blocks with j = 0 are zero; may be NULL
+ *   tau_out   device [batch,T,n]
+ *   flags     must be 0
+ * Method: the closed loop in (x, x - xhat) is the LTV system [[A + B Kfb, -B Kfb], [0, A + Lt C]]; the library forms these
+ * 2n x 2n Jacobians, runs the time-parallel scan of ltv_scan_system_response_tube on them and reads Phi^xw = G11 + G12,
+ * Phi^xe = G12 Lt_{j-1} off the blocks G of that response in one pass that also accumulates the tube (deterministic).
+ * The scan on 2n states costs 8x the n-state scan and 4x its memory (workspace); a general Phibar and the low-rank form
+ * of (15) are not built.  n <= 4096.  Workspace: ltv_scan_workspace_bytes(LTV_OP_OUTPUT_FEEDBACK, batch, T, n, 0). */
+LTV_API int ltv_scan_output_feedback_response(const float* A, const float* B, const float* Kfb, const float* Lt,
+                                              const float* C, const float* w, const float* f, float* phi_xw_out,
+                                              float* phi_xe_out, float* tau_out, int batch, int T, int n, int m, int p,
+                                              unsigned flags, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* One pass of the whole hot path from HOST buffers: copies A, B, c, x0, u, w, g host->device into
  * `workspace` (device, >= ltv_scan_workspace_bytes(LTV_OP_PIPELINE_HOST, ...)), runs the three calls above

@@ -21,6 +21,7 @@ LTV_OP_PIPELINE_HOST_NO_PHI = 4
 LTV_OP_OBSERVER_RESPONSE = 5
 LTV_OP_KALMAN_GAINS = 6
 LTV_OP_CONSTRAINT_TIGHTENING = 7
+LTV_OP_OUTPUT_FEEDBACK = 8
 LTV_TUBE_ROW_2NORM = 1
 LTV_KALMAN_SCAN, LTV_KALMAN_RECURSION = 1, 2
 LTV_PHI_COLUMN_PACKED = 0
@@ -30,7 +31,7 @@ EXPORTS = (
     "ltv_scan_adjoint", "ltv_scan_pipeline_host", "ltv_status_string", "ltv_last_cuda_error", "ltv_version",
     "ltv_launch_count", "ltv_profile_enable", "ltv_profile_collect", "ltv_scan_observer_response",
     "ltv_observer_row_floats", "ltv_scan_kalman_gains",
-    "ltv_scan_constraint_tightening",
+    "ltv_scan_constraint_tightening", "ltv_scan_output_feedback_response",
 )
 
 
@@ -65,6 +66,8 @@ def _load() -> ctypes.CDLL:
     L.ltv_scan_kalman_gains.argtypes = [fp] * 7 + [i] * 4 + [ctypes.c_uint, vp, sz, vp]
     L.ltv_scan_constraint_tightening.restype = i
     L.ltv_scan_constraint_tightening.argtypes = [fp] * 4 + [i] * 4 + [ctypes.c_uint, vp, sz, vp]
+    L.ltv_scan_output_feedback_response.restype = i
+    L.ltv_scan_output_feedback_response.argtypes = [fp] * 10 + [i] * 5 + [ctypes.c_uint, vp, sz, vp]
     L.ltv_observer_row_floats.restype = i
     L.ltv_observer_row_floats.argtypes = [i, i]
     L.ltv_status_string.restype = ctypes.c_char_p
@@ -213,6 +216,28 @@ def ltv_scan_constraint_tightening(A, w, Hc, sigma_out=None, workspace=None):
     if st != LTV_OK:
         raise LtvError(st, "ltv_scan_constraint_tightening")
     return sigma_out
+
+
+def ltv_scan_output_feedback_response(A, B, Kfb, Lt, C, w, f, want_xe=True, workspace=None):
+    """Assembled output-feedback responses (eq.(15)) for gain-defined controllers and the tube (12e): returns
+    (phi_xw[batch,P,n,n], phi_xe[batch,P,n,p] | None, tau[batch,T,n]), blocks in COLUMN_PACKED order."""
+    batch, T, n, _ = A.shape
+    m, p = B.shape[-1], C.shape[2]
+    P = T * (T - 1) // 2
+    _dev(A, "A", (batch, T, n, n)); _dev(B, "B", (batch, T, n, m)); _dev(Kfb, "Kfb", (batch, T, m, n))
+    _dev(Lt, "Lt", (batch, T, n, p)); _dev(C, "C", (batch, T, p, n)); _dev(w, "w", (batch, T, n)); _dev(f, "f", (batch, T, p))
+    phi_xw = torch.empty((batch, P, n, n), device=A.device, dtype=torch.float32)
+    phi_xe = torch.empty((batch, P, n, p), device=A.device, dtype=torch.float32) if want_xe else None
+    tau = torch.empty((batch, T, n), device=A.device, dtype=torch.float32)
+    need = ltv_scan_workspace_bytes(LTV_OP_OUTPUT_FEEDBACK, batch, T, n, 0)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), device=A.device, dtype=torch.uint8)
+    st = lib.ltv_scan_output_feedback_response(_ptr(A), _ptr(B), _ptr(Kfb), _ptr(Lt), _ptr(C), _ptr(w), _ptr(f),
+                                               _ptr(phi_xw), _ptr(phi_xe), _ptr(tau), batch, T, n, m, p, 0,
+                                               _ptr(workspace), workspace.numel(), _stream())
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_output_feedback_response")
+    return phi_xw, phi_xe, tau
 
 
 def ltv_scan_kalman_gains(A, C, e, f, Pi0, Lt_out=None, Pi_out=None, workspace=None, mode=0):

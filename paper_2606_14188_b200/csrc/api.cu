@@ -165,6 +165,9 @@ size_t ltv_scan_workspace_bytes(int op, int batch, int T, int n, int m) {
     case LTV_OP_CONSTRAINT_TIGHTENING:
       if (m < 1 || static_cast<long long>(batch) * T * m >= (1ll << 31) / n) return 0;
       return constraint_workspace_bytes(batch, T, n, m);
+    case LTV_OP_OUTPUT_FEEDBACK:
+      if (check_dims(batch, T, 2 * n, 0) != LTV_OK) return 0;
+      return ofb_workspace_bytes(batch, T, n);
     case LTV_OP_PIPELINE_HOST:
     case LTV_OP_PIPELINE_HOST_NO_PHI: {
       const bool with_phi = op == LTV_OP_PIPELINE_HOST;
@@ -340,6 +343,32 @@ int ltv_scan_constraint_tightening(const float* A, const float* w, const float* 
   ConstraintArgs a{A, w, Hc, sigma_out, batch, T, n, nc, workspace};
   unsigned long long l = 0;
   cudaError_t err = launch_constraint_tightening(a, static_cast<cudaStream_t>(cuda_stream), &l);
+  g_launches += l;
+  return err == cudaSuccess ? LTV_OK : fail_cuda(err);
+}
+
+int ltv_scan_output_feedback_response(const float* A, const float* B, const float* Kfb, const float* Lt, const float* C,
+                                      const float* w, const float* f, float* phi_xw_out, float* phi_xe_out,
+                                      float* tau_out, int batch, int T, int n, int m, int p, unsigned flags,
+                                      void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!A || !B || !Kfb || !Lt || !C || !w || !f || !tau_out || !workspace) return LTV_ERR_NULL_PTR;
+  if (T > 1 && !phi_xw_out) return LTV_ERR_NULL_PTR;
+  int st = check_dims(batch, T, n, m);
+  if (st != LTV_OK) return st;
+  if (m < 1 || p < 1 || flags != 0) return LTV_ERR_BAD_DIM;
+  if (p > 32) return LTV_ERR_UNSUPPORTED_SHAPE;
+  st = check_dims(batch, T, 2 * n, 0);   // the scan runs on 2n states
+  if (st != LTV_OK) return st;
+  if (misaligned(A) || misaligned(B) || misaligned(Kfb) || misaligned(Lt) || misaligned(C) || misaligned(w) ||
+      misaligned(f) || misaligned(phi_xw_out) || misaligned(phi_xe_out) || misaligned(tau_out) || misaligned(workspace))
+    return LTV_ERR_ALIGNMENT;
+  if (workspace_bytes < ofb_workspace_bytes(batch, T, n)) return LTV_ERR_WORKSPACE_TOO_SMALL;
+  int sms = 0;
+  st = check_device(&sms);
+  if (st != LTV_OK) return st;
+  OfbArgs a{A, B, Kfb, Lt, C, w, f, phi_xw_out, phi_xe_out, tau_out, batch, T, n, m, p, workspace};
+  unsigned long long l = 0;
+  cudaError_t err = launch_output_feedback(a, static_cast<cudaStream_t>(cuda_stream), &l);
   g_launches += l;
   return err == cudaSuccess ? LTV_OK : fail_cuda(err);
 }

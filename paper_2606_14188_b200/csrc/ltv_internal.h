@@ -67,6 +67,16 @@ struct ConstraintArgs {
 size_t constraint_workspace_bytes(int batch, int T, int n, int nc);
 cudaError_t launch_constraint_tightening(const ConstraintArgs& a, cudaStream_t stream, unsigned long long* launches);
 
+// Output-feedback responses of eq.(15) + tube (12e) for gain-defined controllers (output_feedback.cu)
+struct OfbArgs {
+  const float *A, *B, *Kfb, *Lt, *C, *w, *f;
+  float *phi_xw, *phi_xe, *tau;
+  int batch, T, n, m, p;
+  void* workspace;
+};
+size_t ofb_workspace_bytes(int batch, int T, int n);
+cudaError_t launch_output_feedback(const OfbArgs& a, cudaStream_t stream, unsigned long long* launches);
+
 // Cluster size (CTAs per item, 1..16, any integer) for the two vector kernels.  max_active[C] = clusters of C CTAs
 // that can be resident at once (cudaOccupancyMaxActiveClusters; 0 = not launchable).  Minimises a simple
 // time model over the waves of clusters: an SM streams ~70 GB/s, the device ~6.5 TB/s (both measured).

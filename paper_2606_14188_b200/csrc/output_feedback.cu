@@ -1,0 +1,176 @@
+// ltv_scan_output_feedback_response: the assembled output-feedback responses of eq.(15) and the
+// reachable tube of eq.(12e) (:147) with both terms, for controllers given by gains (first form).
+// With the predictor-form observer xhat+ = A xhat + B u - Lt (y - C xhat) and u = K xhat, the closed loop is the LTV
+// system in xi = (x, x - xhat)
+//     xi_{k+1} = [[A_k + B_k K_k, -B_k K_k], [0, A_k + Lt_k C_k]] xi_k + [I; I] w~_{k+1} + [0; Lt_k] e~_{k+1},
+// so with G = Phi_aug(k,j) = A_aug,k-1 ... A_aug,j (the system response of the augmented Jacobians):
+//     Phi^xw(k,j) = G11 + G12,        Phi^xe(k,j) = G12 Lt_{j-1}  (j >= 1),
+// which equals (15) evaluated on Phibar = (I - Z(A + BK))^-1, Phihat = (I - Z(A + LtC))^-1 (pinned in the oracle tests).
+// Three steps, all on the device: (1) form the 2n x 2n augmented Jacobians; (2) the time-parallel Phi scan of phi.cu on
+// them (tcgen05 3xTF32 for 2n >= 96); (3) one pass over Phi_aug that writes Phi^xw, Phi^xe and accumulates
+//     tau_k[i] = sum_{j<k} ||row_i(Phi^xw(k,j) diag(w_j))||_2 + ||row_i(Phi^xe(k,j) diag(f_{j-1}))||_2
+// with one warp per (k, i) walking j in order (deterministic, no partial buffers).
+// Cost: the scan on 2n states is 8x the flops of the n-state scan and ignores the block-triangular structure; the
+// structured / low-rank form for a general Phibar is the next step (NEXT-4).
+#include <cuda.h>
+
+#include "ltv_internal.h"
+#include "phi_geom.cuh"
+
+namespace ltv {
+
+namespace {
+
+// warp per row i of (b, t): top row i = [A + B K | -B K], bottom row n + i = [0 | A + Lt C].  grid (batch T, ceil(n/8))
+__global__ void __launch_bounds__(256) ofb_build_aug_kernel(const float* __restrict__ A, const float* __restrict__ B,
+                                                            const float* __restrict__ Kfb, const float* __restrict__ Lt,
+                                                            const float* __restrict__ C, float* __restrict__ Aaug, int n,
+                                                            int m, int p) {
+  const size_t bt = blockIdx.x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int i = blockIdx.y * 8 + warp;
+  if (i >= n) return;
+  const int n4 = n >> 2, n2 = 2 * n;
+  const float4* Ar = reinterpret_cast<const float4*>(A + (bt * n + i) * n);
+  const float* Bi = B + (bt * n + i) * m;
+  const float* Li = Lt + (bt * n + i) * p;
+  const float4* K4 = reinterpret_cast<const float4*>(Kfb + bt * m * n);
+  const float4* C4 = reinterpret_cast<const float4*>(C + bt * p * n);
+  float4* top = reinterpret_cast<float4*>(Aaug + (bt * n2 + i) * n2);
+  float4* bot = reinterpret_cast<float4*>(Aaug + (bt * n2 + n + i) * n2);
+  for (int c = lane; c < n4; c += 32) {
+    const float4 a = __ldg(Ar + c);
+    float4 bk = make_float4(0.f, 0.f, 0.f, 0.f), lc = bk;
+    for (int q = 0; q < m; ++q) {
+      const float s = __ldg(Bi + q);
+      const float4 k4 = __ldg(K4 + static_cast<size_t>(q) * n4 + c);
+      bk.x = fmaf(s, k4.x, bk.x); bk.y = fmaf(s, k4.y, bk.y); bk.z = fmaf(s, k4.z, bk.z); bk.w = fmaf(s, k4.w, bk.w);
+    }
+    for (int q = 0; q < p; ++q) {
+      const float s = __ldg(Li + q);
+      const float4 c4 = __ldg(C4 + static_cast<size_t>(q) * n4 + c);
+      lc.x = fmaf(s, c4.x, lc.x); lc.y = fmaf(s, c4.y, lc.y); lc.z = fmaf(s, c4.z, lc.z); lc.w = fmaf(s, c4.w, lc.w);
+    }
+    top[c] = make_float4(a.x + bk.x, a.y + bk.y, a.z + bk.z, a.w + bk.w);
+    top[n4 + c] = make_float4(-bk.x, -bk.y, -bk.z, -bk.w);
+    bot[c] = make_float4(0.f, 0.f, 0.f, 0.f);
+    bot[n4 + c] = make_float4(a.x + lc.x, a.y + lc.y, a.z + lc.z, a.w + lc.w);
+  }
+}
+
+// warp per (b, k, i): for j = 0 .. k-1 reads row i of Phi_aug(k,j) (2n floats), writes row i of Phi^xw(k,j) and of
+// Phi^xe(k,j), adds the two row norms of (12e) to tau_k[i].  Lane = column quad: it keeps 8 PG partial sums of
+// Phi^xe[i][q] = sum_c G12[i][c] Lt_{j-1}[c][q] over its own columns (accumulators q >= p re-read column p - 1 and are
+// discarded), finished by butterfly shuffles.  grid (ceil(n/8), T, batch); k = blockIdx.y (k = 0: tau_0 = 0).
+template <int PG>
+__global__ void __launch_bounds__(256) ofb_extract_kernel(const float* __restrict__ phi_aug, const float* __restrict__ Lt,
+                                                          const float* __restrict__ w, const float* __restrict__ f,
+                                                          float* __restrict__ phi_xw, float* __restrict__ phi_xe,
+                                                          float* __restrict__ tau, int T, int n, int p) {
+  constexpr int PP = 8 * PG;
+  const int b = blockIdx.z, k = blockIdx.y;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int i = blockIdx.x * 8 + warp;
+  if (i >= n) return;
+  const size_t P = static_cast<size_t>(T) * (T - 1) / 2;
+  const int n4 = n >> 2, n2 = 2 * n;
+  int qoff[PP];
+#pragma unroll
+  for (int q = 0; q < PP; ++q) qoff[q] = min(q, p - 1);
+  float acc = 0.f;
+  for (int j = 0; j < k; ++j) {
+    const size_t blk = static_cast<size_t>(b) * P + phi_colbase(T, j) + (k - j - 1);
+    const float4* g1 = reinterpret_cast<const float4*>(phi_aug + (blk * n2 + i) * n2);
+    const float4* g2 = g1 + n4;
+    const float4* w4 = reinterpret_cast<const float4*>(w + (static_cast<size_t>(b) * T + j) * n);
+    float4* out = reinterpret_cast<float4*>(phi_xw + (blk * n + i) * n);
+    const float* Lj = (j >= 1) ? Lt + (static_cast<size_t>(b) * T + (j - 1)) * n * p : nullptr;
+    float s1 = 0.f;
+    float xe[PP];
+#pragma unroll
+    for (int q = 0; q < PP; ++q) xe[q] = 0.f;
+    for (int c = lane; c < n4; c += 32) {
+      const float4 a = __ldcs(g1 + c);
+      const float4 h = __ldcs(g2 + c);
+      const float4 ww = __ldg(w4 + c);
+      const float4 x = make_float4(a.x + h.x, a.y + h.y, a.z + h.z, a.w + h.w);
+      out[c] = x;
+      const float e0 = x.x * ww.x, e1 = x.y * ww.y, e2 = x.z * ww.z, e3 = x.w * ww.w;
+      s1 = fmaf(e0, e0, fmaf(e1, e1, fmaf(e2, e2, fmaf(e3, e3, s1))));
+      if (Lj != nullptr) {
+        const float* l0 = Lj + static_cast<size_t>(4 * c) * p;   // rows 4c .. 4c+3 of Lt_{j-1}, p floats each
+#pragma unroll
+        for (int q = 0; q < PP; ++q) {
+          const int qq = qoff[q];
+          xe[q] = fmaf(h.x, __ldg(l0 + qq), fmaf(h.y, __ldg(l0 + p + qq),
+                       fmaf(h.z, __ldg(l0 + 2 * p + qq), fmaf(h.w, __ldg(l0 + 3 * p + qq), xe[q]))));
+        }
+      }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+    float s2 = 0.f;
+    if (Lj != nullptr) {
+      const float* fj = f + (static_cast<size_t>(b) * T + (j - 1)) * p;
+#pragma unroll
+      for (int q = 0; q < PP; ++q) {
+        if (q < p) {
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) xe[q] += __shfl_xor_sync(0xffffffffu, xe[q], o);
+          const float v = xe[q] * __ldg(fj + q);
+          s2 = fmaf(v, v, s2);
+          if (phi_xe != nullptr && lane == (q & 31)) phi_xe[(blk * n + i) * p + q] = xe[q];
+        }
+      }
+    } else if (phi_xe != nullptr && lane < p) {
+      phi_xe[(blk * n + i) * p + lane] = 0.f;
+    }
+    acc += sqrtf(s1) + sqrtf(s2);
+  }
+  if (lane == 0) tau[(static_cast<size_t>(b) * T + k) * n + i] = acc;
+}
+
+size_t carve(size_t floats) { return align_up(floats * sizeof(float), 256); }
+
+}  // namespace
+
+size_t ofb_workspace_bytes(int batch, int T, int n) {
+  const size_t b = batch, t = T, n2 = 2 * static_cast<size_t>(n), P = t * (t - 1) / 2;
+  return carve(b * t * n2 * n2) + carve(b * P * n2 * n2 + 4) + 2 * carve(b * t * n2) + phi_workspace_bytes(batch, T, 2 * n, 2 * n);
+}
+
+cudaError_t launch_output_feedback(const OfbArgs& a, cudaStream_t stream, unsigned long long* launches) {
+  const int batch = a.batch, T = a.T, n = a.n;
+  const size_t b = batch, t = T, n2 = 2 * static_cast<size_t>(n), P = t * (t - 1) / 2;
+  char* cur = static_cast<char*>(a.workspace);
+  float* Aaug = reinterpret_cast<float*>(cur); cur += carve(b * t * n2 * n2);
+  float* phi_aug = reinterpret_cast<float*>(cur); cur += carve(b * P * n2 * n2 + 4);
+  float* wz = reinterpret_cast<float*>(cur); cur += carve(b * t * n2);
+  float* rz = reinterpret_cast<float*>(cur); cur += carve(b * t * n2);
+  float* part = reinterpret_cast<float*>(cur);
+  cudaError_t e = cudaMemsetAsync(wz, 0, b * t * n2 * sizeof(float), stream);   // the scan's own tube is not used
+  if (e != cudaSuccess) return e;
+  {
+    ProfScope prof(kProfKalmanSimt, stream);
+    ofb_build_aug_kernel<<<dim3(batch * T, (n + 7) / 8), 256, 0, stream>>>(a.A, a.B, a.Kfb, a.Lt, a.C, Aaug, n, a.m, a.p);
+  }
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  ++*launches;
+  PhiArgs ph{Aaug, wz, phi_aug, rz, part, batch, T, 2 * n, 2 * n, 0};
+  if ((e = launch_phi_tube(ph, stream, launches)) != cudaSuccess) return e;
+  {
+    ProfScope prof(kProfKalmanSimt, stream);
+    const dim3 grid((n + 7) / 8, T, batch);
+    switch ((a.p + 7) / 8) {
+      case 1: ofb_extract_kernel<1><<<grid, 256, 0, stream>>>(phi_aug, a.Lt, a.w, a.f, a.phi_xw, a.phi_xe, a.tau, T, n, a.p); break;
+      case 2: ofb_extract_kernel<2><<<grid, 256, 0, stream>>>(phi_aug, a.Lt, a.w, a.f, a.phi_xw, a.phi_xe, a.tau, T, n, a.p); break;
+      case 3: ofb_extract_kernel<3><<<grid, 256, 0, stream>>>(phi_aug, a.Lt, a.w, a.f, a.phi_xw, a.phi_xe, a.tau, T, n, a.p); break;
+      default: ofb_extract_kernel<4><<<grid, 256, 0, stream>>>(phi_aug, a.Lt, a.w, a.f, a.phi_xw, a.phi_xe, a.tau, T, n, a.p); break;
+    }
+  }
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  ++*launches;
+  return cudaSuccess;
+}
+
+}  // namespace ltv

@@ -89,3 +89,70 @@ def test_output_feedback_response_via_augmented_system(L, n, T, m, p):
     assert O.rel_err(np.stack(got_xw), np.stack(ref_xw)) <= TOL
     assert O.rel_err(np.stack(got_uw), np.stack(ref_uw)) <= TOL
     assert O.rel_err(np.stack(got_xe), np.stack(ref_xe)) <= TOL
+
+
+def _oracle_ofb(A, B, C, K, Lt, w, f):
+    """(15) + (12e) from the oracle, on operators built from the fp32 inputs promoted to fp64 (one item)."""
+    A, B, C, K, Lt = [a.astype(np.float64) for a in (A, B, C, K, Lt)]
+    T, n, _ = A.shape
+    m, p = B.shape[2], C.shape[1]
+    PbX = _dense(O.system_response_item(A + B @ K), T, n)
+    PbU = np.vstack([K[k] @ PbX[k * n:(k + 1) * n] for k in range(T)])
+    PhX = _dense(O.observer_response_item(A, Lt, C)[0], T, n)
+    PhY = np.zeros((T * n, T * p))
+    for j in range(1, T):
+        PhY[:, j * p:(j + 1) * p] = PhX[:, j * n:(j + 1) * n] @ Lt[j - 1]
+    Pxw, Puw, Pxe, Pue = O.assemble_output_feedback(A, PbX, PbU, PhX, PhY)
+    return Pxw, Pxe, O.output_feedback_tube(Pxw, Pxe, w, f)
+
+
+@pytest.mark.parametrize("n,T,m,p,batch", [(24, 6, 2, 3, 2),      # 2n = 48: fp32-FMA combine
+                                           (48, 7, 3, 4, 1),      # 2n = 96: smallest tensor-core size
+                                           (132, 5, 6, 6, 2),     # ragged tiles
+                                           (100, 4, 1, 1, 1),     # single input, single output
+                                           (64, 3, 4, 20, 1)])    # wide observation (three groups of 8)
+def test_output_feedback_response_call(L, n, T, m, p, batch):
+    """ltv_scan_output_feedback_response (augmented Jacobians, Phi scan on 2n states, extraction + tube, all on the
+    device) against eq.(15) and (12e) evaluated by the oracle."""
+    import torch
+
+    items = [_gains(T, n, m, p, seed=7 * n + T + b) for b in range(batch)]
+    A, B, C, K, Lt = [np.stack([it[q] for it in items]) for q in range(5)]
+    rng = np.random.default_rng(n)
+    w = rng.uniform(0.1, 1.0, (batch, T, n)).astype(np.float32)
+    f = rng.uniform(0.1, 1.0, (batch, T, p)).astype(np.float32)
+    d = [torch.from_numpy(a).cuda() for a in (A, B, K, Lt, C, w, f)]
+    xw, xe, tau = L.ltv_scan_output_feedback_response(*d)
+    torch.cuda.synchronize()
+    xw, xe, tau = xw.cpu().numpy(), xe.cpu().numpy(), tau.cpu().numpy()
+    for b in range(batch):
+        Pxw, Pxe, tau_ref = _oracle_ofb(A[b], B[b], C[b], K[b], Lt[b], w[b], f[b])
+        ref_w = np.stack([Pxw[k * n:(k + 1) * n, j * n:(j + 1) * n] for j in range(T - 1) for k in range(j + 1, T)])
+        ref_e = np.stack([Pxe[k * n:(k + 1) * n, j * p:(j + 1) * p] for j in range(T - 1) for k in range(j + 1, T)])
+        assert O.rel_err(xw[b], ref_w) <= TOL
+        assert O.rel_err(xe[b], ref_e) <= TOL
+        assert O.rel_err(tau[b], tau_ref) <= TOL
+        assert np.all(tau[b, 0] == 0.0)
+        assert np.all(xe[b, :T - 1] == 0.0)      # column j = 0: no measurement precedes step 0
+
+
+def test_kalman_gains_to_output_feedback_tube_pipeline(L):
+    """Stage 3 end to end on the device: gains of (13) -> responses (15) -> tube (12e); oracle: the same chain in fp64."""
+    import torch
+    from workloads import dense_random, observation_model
+
+    n, T, batch, m, p = 64, 6, 2, 3, 4
+    W = dense_random(batch, T, n, m, seed=31, scale=0.4)
+    M = observation_model(batch, T, n, p, seed=32, kind="dense")
+    K = (0.2 * np.random.default_rng(33).normal(0.0, 1.0 / np.sqrt(n), (batch, T, m, n))).astype(np.float32)
+    w1 = (1e3 * W.w).astype(np.float32)
+    dA, dB = torch.from_numpy(W.A).cuda(), torch.from_numpy(W.B).cuda()
+    dC, de, df, dP = [torch.from_numpy(M[k]).cuda() for k in ("C", "e", "f", "Pi0")]
+    Lt, _ = L.ltv_scan_kalman_gains(dA, dC, de, df, dP)
+    xw, xe, tau = L.ltv_scan_output_feedback_response(dA, dB, torch.from_numpy(K).cuda(), Lt, dC,
+                                                      torch.from_numpy(w1).cuda(), df)
+    torch.cuda.synchronize()
+    _, Lt_ref = O.kalman_recursion(W.A, M["C"], M["e"], M["f"], M["Pi0"])
+    for b in range(batch):
+        _, _, tau_ref = _oracle_ofb(W.A[b], W.B[b], M["C"][b], K[b], Lt_ref[b], w1[b], M["f"][b])
+        assert O.rel_err(tau[b].cpu().numpy(), tau_ref) <= TOL
