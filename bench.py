@@ -44,6 +44,8 @@ def parse():
                     help="also time ltv_scan_kalman_gains (NEXT-3, eq.(13)) with P observation rows")
     ap.add_argument("--constraints", type=int, default=0, metavar="NC",
                     help="also time ltv_scan_constraint_tightening (NEXT-2, eq.(12d)) with NC constraint rows per step")
+    ap.add_argument("--output-feedback", type=int, default=0, metavar="P",
+                    help="also time ltv_scan_output_feedback_response (NEXT-4, eq.(15) + (12e)) with P observation rows")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-items", type=int, default=0, help="items in the CPU-oracle sample (0 = auto)")
@@ -379,6 +381,36 @@ def main():
                                 "A read once (hbm_gbs counts those bytes), Phi never formed")
         del Hc, sig, wsc
 
+    # ---- NEXT-4 (first form): assembled output-feedback responses + tube for gain-defined controllers, timed alone
+    ofb = None
+    if args.output_feedback > 0 and m > 0:
+        pf = args.output_feedback
+        if phi_on:
+            phi = None
+        torch.cuda.empty_cache()
+        gen = torch.Generator(device=dev).manual_seed(2468 + rank)
+        Kfb = torch.randn((batch, T, m, n), device=dev, generator=gen) * (0.2 / n ** 0.5)
+        Ltf = torch.randn((batch, T, n, pf), device=dev, generator=gen) * (0.05 / pf ** 0.5)
+        Cf = torch.randn((batch, T, pf, n), device=dev, generator=gen) / n ** 0.5
+        ff = torch.rand((batch, T, pf), device=dev, generator=gen) * 4e-3 + 1e-3
+        wsf = torch.empty(L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, batch, T, n, 0), dtype=torch.uint8, device=dev)
+        for _ in range(2):
+            out = L.ltv_scan_output_feedback_response(d["A"], d["B"], Kfb, Ltf, Cf, d["w"], ff, workspace=wsf)
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        nrep = max(1, min(args.steps, 5))
+        barrier()
+        f0.record()
+        for _ in range(nrep):
+            out = L.ltv_scan_output_feedback_response(d["A"], d["B"], Kfb, Ltf, Cf, d["w"], ff, workspace=wsf)
+        f1.record()
+        barrier()
+        fms = f0.elapsed_time(f1) / nrep
+        ofb = dict(p=pf, ms=fms, blocks_per_s=batch * world * P / (fms * 1e-3),
+                   issued_tf32_tflops=3.0 * 2.0 * (2 * n) ** 3 * ((T - 1) * (T - 2) // 2) * batch / (fms * 1e-3) / 1e12,
+                   note="ltv_scan_output_feedback_response alone: Phi scan on the 2n-state augmented closed loop "
+                        "(8x the flops of the n-state scan, counted here) + extraction / tube pass")
+        del out, wsf, Kfb, Ltf, Cf
+
     # ---- end to end through the C-ABI with host buffers
     e2e = None
     if not args.no_e2e:
@@ -435,7 +467,7 @@ def main():
                                     f"working set (A {a_gb * 1e3:.2f} MB) fits L2: warm-cache, latency-bound case"),
                                 phi_layout="column-packed"),
                     clocks=sampler.result(), e2e=e2e, gpu_launches=int(launches), roofline=roof,
-                    cpu_baseline=cpu, kernel_ms_per_step=share, vector_scans=extra, observer=observer, kalman=kalman, constraints=constraints,
+                    cpu_baseline=cpu, kernel_ms_per_step=share, vector_scans=extra, observer=observer, kalman=kalman, constraints=constraints, output_feedback=ofb,
                     rollouts_per_s=extra.get("rollout", {}).get("per_s"),
                     adjoints_per_s=extra.get("adjoint", {}).get("per_s"))
         print(json.dumps(line), flush=True)

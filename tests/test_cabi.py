@@ -99,6 +99,14 @@ def test_host_side_validation_needs_no_gpu(L):
     assert c(p, p, p, p, 1, 2, 4, 2, 0, p, 8, None) == 5                                # workspace too small
     need = L.ltv_scan_workspace_bytes(L.LTV_OP_CONSTRAINT_TIGHTENING, b, T, n, 6)
     assert 2 * b * (T - 1) * 6 * n * 4 <= need <= 2 * b * (T - 1) * 6 * n * 4 + 1024   # two stacks of (T-1) nc rows
+    o = L.lib.ltv_scan_output_feedback_response
+    assert o(p, p, None, p, p, p, p, p, None, p, 1, 2, 4, 2, 2, 0, p, 1 << 24, None) == 1   # NULL Kfb
+    assert o(p, p, p, p, p, p, p, p, None, p, 1, 2, 4, 0, 2, 0, p, 1 << 24, None) == 2      # m = 0
+    assert o(p, p, p, p, p, p, p, p, None, p, 1, 2, 4, 2, 40, 0, p, 1 << 24, None) == 3     # p > 32
+    assert o(p, p, p, p, p, p, p, p, None, p, 1, 2, 4100, 2, 2, 0, p, 1 << 24, None) == 3   # 2n beyond the scan's limit
+    assert o(p, p, p, p, p, p, p, p, None, p, 1, 2, 4, 2, 2, 0, p, 8, None) == 5            # workspace too small
+    need = L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, b, T, n, 0)
+    assert need >= 4 * b * (T * (T - 1) // 2) * n * n * 4                               # Phi of the 2n-state system
     a = L.lib.ltv_scan_adjoint
     assert a(p, None, p, p, p, None, 1, 2, 4, 2, None, 0, None) == 1                # grad_u wanted, B NULL
     assert a(p, p, None, p, None, None, 1, 2, 4, 2, None, 0, None) == 1             # NULL g
