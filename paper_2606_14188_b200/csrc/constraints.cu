@@ -89,7 +89,7 @@ cudaError_t launch_constraint_tightening(const ConstraintArgs& a, cudaStream_t s
   const bool tc = phi_uses_tensor_cores(n);
   const int nch = phi_pick_nch(n);
   BatchedGemm g[2];
-  alignas(64) unsigned char maps[2][512];
+  alignas(64) unsigned char maps[2][1024];
   for (int q = 0; q < 2; ++q) {   // q = parity of the step: left operand X[q], output X[q ^ 1]
     g[q] = BatchedGemm{};
     g[q].L = X[q]; g[q].l_rows = static_cast<long long>(batch) * rmax; g[q].l_row0 = 0; g[q].l_row_stride = rmax;

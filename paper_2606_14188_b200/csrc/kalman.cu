@@ -450,7 +450,7 @@ cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned lon
   g2.R = w.Yt; g2.r_blocks = batch; g2.r_blk0 = 0; g2.r_blk_stride = 1;
   g2.D = a.Pi_out; g2.d_blocks = batch * (T + 1); g2.d_blk_stride = T + 1;
   g2.count = batch; g2.M = n; g2.N = n; g2.K = n; g2.transpose_out = 0; g2.diag_stride = static_cast<long long>(T) * n;
-  alignas(64) unsigned char maps1[512], maps2[512];
+  alignas(64) unsigned char maps1[1024], maps2[1024];
   if (tc) {
     if (phi_tc_maps_size() > sizeof(maps1)) return cudaErrorInvalidValue;
     if ((e = bgemm_tc_make_maps(g1, maps1)) != cudaSuccess) return e;

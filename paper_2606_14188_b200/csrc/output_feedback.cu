@@ -10,12 +10,16 @@
 // them (tcgen05 3xTF32 for 2n >= 96); (3) one pass over Phi_aug that writes Phi^xw, Phi^xe and accumulates
 //     tau_k[i] = sum_{j<k} ||row_i(Phi^xw(k,j) diag(w_j))||_2 + ||row_i(Phi^xe(k,j) diag(f_{j-1}))||_2
 // with one warp per (k, i) walking j in order (deterministic, no partial buffers).
-// Cost: the scan on 2n states is 8x the flops of the n-state scan and ignores the block-triangular structure; the
-// structured / low-rank form for a general Phibar is the next step (NEXT-4).
+// The augmented matrix is block upper triangular, and so is every Phi_aug(k,j): G11 = Phibar^x, G22 = Phihat^x and the
+// cross block obeys G12(t,s) = G11(t,mid) G12(mid,s) + G12(t,mid) G22(mid,s).  For n >= 96 the call therefore runs two
+// n-state scans and one cross scan (MODE 2 of the tcgen05 kernel: one K loop over both operand pairs) - 4 instead of 8
+// n^3 products per block and 3 instead of 4 n x n blocks of storage; below that the plain 2n-state scan is used.
+// The low-rank form for a general Phibar is the next step (NEXT-4).
 #include <cuda.h>
 
 #include "ltv_internal.h"
 #include "phi_geom.cuh"
+#include "phi_kernels.h"
 
 namespace ltv {
 
@@ -24,8 +28,8 @@ namespace {
 // warp per row i of (b, t): top row i = [A + B K | -B K], bottom row n + i = [0 | A + Lt C].  grid (batch T, ceil(n/8))
 __global__ void __launch_bounds__(256) ofb_build_aug_kernel(const float* __restrict__ A, const float* __restrict__ B,
                                                             const float* __restrict__ Kfb, const float* __restrict__ Lt,
-                                                            const float* __restrict__ C, float* __restrict__ Aaug, int n,
-                                                            int m, int p) {
+                                                            const float* __restrict__ C, float* __restrict__ Aaug,
+                                                            float* __restrict__ Ltt, int n, int m, int p) {
   const size_t bt = blockIdx.x;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int i = blockIdx.y * 8 + warp;
@@ -34,6 +38,7 @@ __global__ void __launch_bounds__(256) ofb_build_aug_kernel(const float* __restr
   const float4* Ar = reinterpret_cast<const float4*>(A + (bt * n + i) * n);
   const float* Bi = B + (bt * n + i) * m;
   const float* Li = Lt + (bt * n + i) * p;
+  if (lane < p) Ltt[(bt * p + lane) * n + i] = __ldg(Li + lane);   // gains with n contiguous, for the extraction pass
   const float4* K4 = reinterpret_cast<const float4*>(Kfb + bt * m * n);
   const float4* C4 = reinterpret_cast<const float4*>(C + bt * p * n);
   float4* top = reinterpret_cast<float4*>(Aaug + (bt * n2 + i) * n2);
@@ -58,14 +63,61 @@ __global__ void __launch_bounds__(256) ofb_build_aug_kernel(const float* __restr
   }
 }
 
+// structured path: warp per row i of (b, t): Atil = A + B K, Abar = A + Lt C (n x n each), and the level-0 cross block
+// G12(t+1,t) = -B_t K_t into block (t+1, t) of the column-packed G (t <= T-2).  grid (batch T, ceil(n/8))
+__global__ void __launch_bounds__(256) ofb_build_split_kernel(const float* __restrict__ A, const float* __restrict__ B,
+                                                              const float* __restrict__ Kfb, const float* __restrict__ Lt,
+                                                              const float* __restrict__ C, float* __restrict__ Atil,
+                                                              float* __restrict__ Abar, float* __restrict__ G,
+                                                              float* __restrict__ Ltt, int T, int n, int m, int p) {
+  const size_t bt = blockIdx.x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int i = blockIdx.y * 8 + warp;
+  if (i >= n) return;
+  const int n4 = n >> 2;
+  const int t = static_cast<int>(bt % T);
+  const size_t b = bt / T;
+  const float4* Ar = reinterpret_cast<const float4*>(A + (bt * n + i) * n);
+  const float* Bi = B + (bt * n + i) * m;
+  const float* Li = Lt + (bt * n + i) * p;
+  if (lane < p) Ltt[(bt * p + lane) * n + i] = __ldg(Li + lane);   // gains with n contiguous, for the extraction pass
+  const float4* K4 = reinterpret_cast<const float4*>(Kfb + bt * m * n);
+  const float4* C4 = reinterpret_cast<const float4*>(C + bt * p * n);
+  float4* o1 = reinterpret_cast<float4*>(Atil + (bt * n + i) * n);
+  float4* o2 = reinterpret_cast<float4*>(Abar + (bt * n + i) * n);
+  float4* o3 = nullptr;
+  if (t <= T - 2) {
+    const size_t P = static_cast<size_t>(T) * (T - 1) / 2;
+    o3 = reinterpret_cast<float4*>(G + ((b * P + phi_colbase(T, t)) * n + i) * n);
+  }
+  for (int c = lane; c < n4; c += 32) {
+    const float4 a = __ldg(Ar + c);
+    float4 bk = make_float4(0.f, 0.f, 0.f, 0.f), lc = bk;
+    for (int q = 0; q < m; ++q) {
+      const float s = __ldg(Bi + q);
+      const float4 k4 = __ldg(K4 + static_cast<size_t>(q) * n4 + c);
+      bk.x = fmaf(s, k4.x, bk.x); bk.y = fmaf(s, k4.y, bk.y); bk.z = fmaf(s, k4.z, bk.z); bk.w = fmaf(s, k4.w, bk.w);
+    }
+    for (int q = 0; q < p; ++q) {
+      const float s = __ldg(Li + q);
+      const float4 c4 = __ldg(C4 + static_cast<size_t>(q) * n4 + c);
+      lc.x = fmaf(s, c4.x, lc.x); lc.y = fmaf(s, c4.y, lc.y); lc.z = fmaf(s, c4.z, lc.z); lc.w = fmaf(s, c4.w, lc.w);
+    }
+    o1[c] = make_float4(a.x + bk.x, a.y + bk.y, a.z + bk.z, a.w + bk.w);
+    o2[c] = make_float4(a.x + lc.x, a.y + lc.y, a.z + lc.z, a.w + lc.w);
+    if (o3 != nullptr) o3[c] = make_float4(-bk.x, -bk.y, -bk.z, -bk.w);
+  }
+}
+
 // warp per (b, k, i): for j = 0 .. k-1 reads row i of Phi_aug(k,j) (2n floats), writes row i of Phi^xw(k,j) and of
 // Phi^xe(k,j), adds the two row norms of (12e) to tau_k[i].  Lane = column quad: it keeps 8 PG partial sums of
 // Phi^xe[i][q] = sum_c G12[i][c] Lt_{j-1}[c][q] over its own columns (accumulators q >= p re-read column p - 1 and are
 // discarded), finished by butterfly shuffles.  grid (ceil(n/8), T, batch); k = blockIdx.y (k = 0: tau_0 = 0).
 template <int PG>
-__global__ void __launch_bounds__(256) ofb_extract_kernel(const float* __restrict__ phi_aug, const float* __restrict__ Lt,
+__global__ void __launch_bounds__(256) ofb_extract_kernel(const float* P1, const float* __restrict__ P2, int ld, int brows,
+                                                          const float* __restrict__ Lt /* transposed: [b,T,p,n] */,
                                                           const float* __restrict__ w, const float* __restrict__ f,
-                                                          float* __restrict__ phi_xw, float* __restrict__ phi_xe,
+                                                          float* phi_xw, float* __restrict__ phi_xe,
                                                           float* __restrict__ tau, int T, int n, int p) {
   constexpr int PP = 8 * PG;
   const int b = blockIdx.z, k = blockIdx.y;
@@ -73,24 +125,26 @@ __global__ void __launch_bounds__(256) ofb_extract_kernel(const float* __restric
   const int i = blockIdx.x * 8 + warp;
   if (i >= n) return;
   const size_t P = static_cast<size_t>(T) * (T - 1) / 2;
-  const int n4 = n >> 2, n2 = 2 * n;
+  const int n4 = n >> 2;
   int qoff[PP];
 #pragma unroll
   for (int q = 0; q < PP; ++q) qoff[q] = min(q, p - 1);
   float acc = 0.f;
   for (int j = 0; j < k; ++j) {
     const size_t blk = static_cast<size_t>(b) * P + phi_colbase(T, j) + (k - j - 1);
-    const float4* g1 = reinterpret_cast<const float4*>(phi_aug + (blk * n2 + i) * n2);
-    const float4* g2 = g1 + n4;
+    // G11 row from P1, G12 row from P2 (augmented scan: the two halves of one 2n-float row; structured: two arrays; P1 may
+    // be phi_xw itself - each element is read, then written, by the same thread)
+    const float4* g1 = reinterpret_cast<const float4*>(P1 + (blk * brows + i) * ld);
+    const float4* g2 = reinterpret_cast<const float4*>(P2 + (blk * brows + i) * ld);
     const float4* w4 = reinterpret_cast<const float4*>(w + (static_cast<size_t>(b) * T + j) * n);
     float4* out = reinterpret_cast<float4*>(phi_xw + (blk * n + i) * n);
-    const float* Lj = (j >= 1) ? Lt + (static_cast<size_t>(b) * T + (j - 1)) * n * p : nullptr;
+    const float4* Lj = (j >= 1) ? reinterpret_cast<const float4*>(Lt + (static_cast<size_t>(b) * T + (j - 1)) * n * p) : nullptr;
     float s1 = 0.f;
     float xe[PP];
 #pragma unroll
     for (int q = 0; q < PP; ++q) xe[q] = 0.f;
     for (int c = lane; c < n4; c += 32) {
-      const float4 a = __ldcs(g1 + c);
+      const float4 a = g1[c];
       const float4 h = __ldcs(g2 + c);
       const float4 ww = __ldg(w4 + c);
       const float4 x = make_float4(a.x + h.x, a.y + h.y, a.z + h.z, a.w + h.w);
@@ -98,12 +152,10 @@ __global__ void __launch_bounds__(256) ofb_extract_kernel(const float* __restric
       const float e0 = x.x * ww.x, e1 = x.y * ww.y, e2 = x.z * ww.z, e3 = x.w * ww.w;
       s1 = fmaf(e0, e0, fmaf(e1, e1, fmaf(e2, e2, fmaf(e3, e3, s1))));
       if (Lj != nullptr) {
-        const float* l0 = Lj + static_cast<size_t>(4 * c) * p;   // rows 4c .. 4c+3 of Lt_{j-1}, p floats each
 #pragma unroll
         for (int q = 0; q < PP; ++q) {
-          const int qq = qoff[q];
-          xe[q] = fmaf(h.x, __ldg(l0 + qq), fmaf(h.y, __ldg(l0 + p + qq),
-                       fmaf(h.z, __ldg(l0 + 2 * p + qq), fmaf(h.w, __ldg(l0 + 3 * p + qq), xe[q]))));
+          const float4 l = __ldg(Lj + static_cast<size_t>(qoff[q]) * n4 + c);   // row q of Lt_{j-1}^T, coalesced
+          xe[q] = fmaf(h.x, l.x, fmaf(h.y, l.y, fmaf(h.z, l.z, fmaf(h.w, l.w, xe[q]))));
         }
       }
     }
@@ -134,41 +186,92 @@ size_t carve(size_t floats) { return align_up(floats * sizeof(float), 256); }
 
 }  // namespace
 
+static bool ofb_structured(int n) { return phi_uses_tensor_cores(n) && env_int("OFB_AUGMENTED", 0) == 0; }
+
 size_t ofb_workspace_bytes(int batch, int T, int n) {
-  const size_t b = batch, t = T, n2 = 2 * static_cast<size_t>(n), P = t * (t - 1) / 2;
-  return carve(b * t * n2 * n2) + carve(b * P * n2 * n2 + 4) + 2 * carve(b * t * n2) + phi_workspace_bytes(batch, T, 2 * n, 2 * n);
+  const size_t b = batch, t = T, nn = n, n2 = 2 * nn, P = t * (t - 1) / 2;
+  if (ofb_structured(n))   // Atil, Abar; Phihat, G (Phibar lives in phi_xw_out); zero w, scratch r; tube partials of a scan
+    return carve(b * t * 32 * nn) + 2 * carve(b * t * nn * nn) + 2 * carve(b * P * nn * nn + 4) + 2 * carve(b * t * nn) + phi_workspace_bytes(batch, T, n, n);
+  return carve(b * t * 32 * nn) + carve(b * t * n2 * n2) + carve(b * P * n2 * n2 + 4) + 2 * carve(b * t * n2) + phi_workspace_bytes(batch, T, 2 * n, 2 * n);
+}
+
+template <typename... Args>
+static cudaError_t launch_extract(int p, dim3 grid, cudaStream_t stream, Args... args) {
+  ProfScope prof(kProfKalmanSimt, stream);
+  switch ((p + 7) / 8) {
+    case 1: ofb_extract_kernel<1><<<grid, 256, 0, stream>>>(args...); break;
+    case 2: ofb_extract_kernel<2><<<grid, 256, 0, stream>>>(args...); break;
+    case 3: ofb_extract_kernel<3><<<grid, 256, 0, stream>>>(args...); break;
+    default: ofb_extract_kernel<4><<<grid, 256, 0, stream>>>(args...); break;
+  }
+  return cudaGetLastError();
 }
 
 cudaError_t launch_output_feedback(const OfbArgs& a, cudaStream_t stream, unsigned long long* launches) {
   const int batch = a.batch, T = a.T, n = a.n;
-  const size_t b = batch, t = T, n2 = 2 * static_cast<size_t>(n), P = t * (t - 1) / 2;
+  const size_t b = batch, t = T, nn = n, n2 = 2 * nn, P = t * (t - 1) / 2;
   char* cur = static_cast<char*>(a.workspace);
+  const dim3 xgrid((n + 7) / 8, T, batch);
+  cudaError_t e;
+  float* Ltt = reinterpret_cast<float*>(cur); cur += carve(b * t * 32 * nn);   // [b,T,p,n] (sized for p = 32)
+  if (ofb_structured(n)) {
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    float* Atil = reinterpret_cast<float*>(cur); cur += carve(b * t * nn * nn);
+    float* Abar = reinterpret_cast<float*>(cur); cur += carve(b * t * nn * nn);
+    float* phat = reinterpret_cast<float*>(cur); cur += carve(b * P * nn * nn + 4);
+    float* G = reinterpret_cast<float*>(cur); cur += carve(b * P * nn * nn + 4);
+    float* wz = reinterpret_cast<float*>(cur); cur += carve(b * t * nn);
+    float* rz = reinterpret_cast<float*>(cur); cur += carve(b * t * nn);
+    float* part = reinterpret_cast<float*>(cur);
+    float* pbar = a.phi_xw;   // Phibar^x is scanned straight into the output and completed in place by the last pass
+    if ((e = cudaMemsetAsync(wz, 0, b * t * nn * sizeof(float), stream)) != cudaSuccess) return e;
+    {
+      ProfScope prof(kProfKalmanSimt, stream);
+      ofb_build_split_kernel<<<dim3(batch * T, (n + 7) / 8), 256, 0, stream>>>(a.A, a.B, a.Kfb, a.Lt, a.C, Atil, Abar, G, Ltt,
+                                                                               T, n, a.m, a.p);
+    }
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    ++*launches;
+    PhiArgs pb{Atil, wz, pbar, rz, part, batch, T, n, n, 0};
+    if ((e = launch_phi_tube(pb, stream, launches)) != cudaSuccess) return e;
+    PhiArgs ph{Abar, wz, phat, rz, part, batch, T, n, n, 0};
+    if ((e = launch_phi_tube(ph, stream, launches)) != cudaSuccess) return e;
+    if (T - 1 >= 2) {
+      PhiArgs pg{nullptr, nullptr, G, nullptr, nullptr, batch, T, n, n, 0};
+      const int nch = phi_pick_nch(n);
+      alignas(64) unsigned char maps[1024];
+      if (phi_tc_maps_size() > sizeof(maps)) return cudaErrorInvalidValue;
+      if ((e = phi_tc_make_cross_maps(pg, pbar, phat, nch, maps)) != cudaSuccess) return e;
+      for (int level = 1; (1 << (level - 1)) < T - 1; ++level) {
+        if ((e = launch_phi_cross_tc(pg, level, nch, maps, sms, stream)) != cudaSuccess) return e;
+        ++*launches;
+      }
+    }
+    if ((e = launch_extract(a.p, xgrid, stream, static_cast<const float*>(pbar), static_cast<const float*>(G), n, n,
+                            static_cast<const float*>(Ltt), a.w, a.f, a.phi_xw, a.phi_xe, a.tau, T, n, a.p)) != cudaSuccess)
+      return e;
+    ++*launches;
+    return cudaSuccess;
+  }
   float* Aaug = reinterpret_cast<float*>(cur); cur += carve(b * t * n2 * n2);
   float* phi_aug = reinterpret_cast<float*>(cur); cur += carve(b * P * n2 * n2 + 4);
   float* wz = reinterpret_cast<float*>(cur); cur += carve(b * t * n2);
   float* rz = reinterpret_cast<float*>(cur); cur += carve(b * t * n2);
   float* part = reinterpret_cast<float*>(cur);
-  cudaError_t e = cudaMemsetAsync(wz, 0, b * t * n2 * sizeof(float), stream);   // the scan's own tube is not used
-  if (e != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(wz, 0, b * t * n2 * sizeof(float), stream)) != cudaSuccess) return e;   // the scan's own tube is not used
   {
     ProfScope prof(kProfKalmanSimt, stream);
-    ofb_build_aug_kernel<<<dim3(batch * T, (n + 7) / 8), 256, 0, stream>>>(a.A, a.B, a.Kfb, a.Lt, a.C, Aaug, n, a.m, a.p);
+    ofb_build_aug_kernel<<<dim3(batch * T, (n + 7) / 8), 256, 0, stream>>>(a.A, a.B, a.Kfb, a.Lt, a.C, Aaug, Ltt, n, a.m, a.p);
   }
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   ++*launches;
   PhiArgs ph{Aaug, wz, phi_aug, rz, part, batch, T, 2 * n, 2 * n, 0};
   if ((e = launch_phi_tube(ph, stream, launches)) != cudaSuccess) return e;
-  {
-    ProfScope prof(kProfKalmanSimt, stream);
-    const dim3 grid((n + 7) / 8, T, batch);
-    switch ((a.p + 7) / 8) {
-      case 1: ofb_extract_kernel<1><<<grid, 256, 0, stream>>>(phi_aug, a.Lt, a.w, a.f, a.phi_xw, a.phi_xe, a.tau, T, n, a.p); break;
-      case 2: ofb_extract_kernel<2><<<grid, 256, 0, stream>>>(phi_aug, a.Lt, a.w, a.f, a.phi_xw, a.phi_xe, a.tau, T, n, a.p); break;
-      case 3: ofb_extract_kernel<3><<<grid, 256, 0, stream>>>(phi_aug, a.Lt, a.w, a.f, a.phi_xw, a.phi_xe, a.tau, T, n, a.p); break;
-      default: ofb_extract_kernel<4><<<grid, 256, 0, stream>>>(phi_aug, a.Lt, a.w, a.f, a.phi_xw, a.phi_xe, a.tau, T, n, a.p); break;
-    }
-  }
-  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  if ((e = launch_extract(a.p, xgrid, stream, static_cast<const float*>(phi_aug), static_cast<const float*>(phi_aug + n), 2 * n,
+                          2 * n, static_cast<const float*>(Ltt), a.w, a.f, a.phi_xw, a.phi_xe, a.tau, T, n, a.p)) != cudaSuccess)
+    return e;
   ++*launches;
   return cudaSuccess;
 }

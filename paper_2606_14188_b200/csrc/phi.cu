@@ -54,7 +54,7 @@ cudaError_t launch_phi_tube(const PhiArgs& a, cudaStream_t stream, unsigned long
     if (e != cudaSuccess) return e;
     *launches += (a.Lt && a.p > 8) ? 2 : 1;   // the observer's level 0 is two kernels beyond the fused p <= 8 path
     const bool tc = phi_uses_tensor_cores(a.n);
-    alignas(64) unsigned char maps[512];
+    alignas(64) unsigned char maps[1024];
     if (tc && NS >= 2) {
       if (phi_tc_maps_size() > sizeof(maps)) return cudaErrorInvalidValue;
       e = phi_tc_make_maps(a, tn / 32, maps);

@@ -17,6 +17,12 @@ cudaError_t phi_tc_make_maps(const PhiArgs& a, int nch, void* maps_out);
 cudaError_t launch_phi_combine_tc(const PhiArgs& a, int level, int nch, const void* maps, int num_sms,
                                   cudaStream_t stream);
 
+// Cross block of a block-triangular closed loop on the geometry of the Phi scan (MODE 2 of the kernel): at `level`, for
+// every s < mid < t of a segment, G(t,s) = Pbar(t,mid) G(mid,s) + G(t,mid) Phat(mid,s) with a.phi = G (column-packed,
+// nc = n) - one K loop over both operand pairs into one accumulator.  No tube.
+cudaError_t phi_tc_make_cross_maps(const PhiArgs& a, const float* pbar, const float* phat, int nch, void* maps_out);
+cudaError_t launch_phi_cross_tc(const PhiArgs& a, int level, int nch, const void* maps, int num_sms, cudaStream_t stream);
+
 // Batched fp32 GEMM on the same tcgen05 3xTF32 kernel (its MODE 1): D[b] = L[b] R[b], b < count, all row-major.
 //   L  array viewed as [l_rows][K];       problem b reads rows [l_row0 + b l_row_stride, +M)
 //   R  array viewed as [r_blocks][K][N];  problem b reads block r_blk0 + b r_blk_stride

@@ -80,6 +80,7 @@ struct TcMaps {
   CUtensorMap L;  // 2-D [batch*P*n rows][n]           box 32 x 128
   CUtensorMap R;  // 3-D [batch*P blocks][n][n]        box 32 x 32 x 1
   CUtensorMap O;  // 2-D [batch*P*n rows][n]           box 32 x 32 (epilogue stores)
+  CUtensorMap L2, R2;   // MODE 2: second operand pair of the K loop (same geometry, other arrays)
 };
 
 __device__ __forceinline__ float tf32_lo(float a) {
@@ -122,7 +123,8 @@ struct TcShape {
 template <int NCH, bool PAIR, int DBG, int MODE>
 __global__ void __launch_bounds__(kTcThreads, 1)
 phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL,
-                      const __grid_constant__ CUtensorMap mapR, const __grid_constant__ CUtensorMap mapO) {
+                      const __grid_constant__ CUtensorMap mapR, const __grid_constant__ CUtensorMap mapO,
+                      const __grid_constant__ CUtensorMap mapL2, const __grid_constant__ CUtensorMap mapR2) {
   using S = TcShape<NCH, PAIR>;
   constexpr int NT = S::NT, NH = S::NH, NBOX = S::NBOX, NCTA = S::NCTA;
   constexpr uint32_t kBBytes = S::kBBytes, kRawBytes = S::kRawBytes, kTmemA = S::kTmemA;
@@ -136,6 +138,8 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
   const int R = p.stages;
   const int nkb = (n + kKB - 1) / kKB;
   const int ks_last = ((n - (nkb - 1) * kKB) + 7) / 8;  // k-steps of the last k-block that hold data
+  // MODE 2 (cross block of a block-triangular system): D = L1 R1 + L2 R2, the K loop runs over both operand pairs
+  const int nkb_tot = (MODE == 2) ? 2 * nkb : nkb;
   const long long unit = PAIR ? (blockIdx.x >> 1) : blockIdx.x;
   const long long nunits = PAIR ? (gridDim.x >> 1) : gridDim.x;
 #define LTV_TRACE(role, idx, ev)                                                                  \
@@ -172,6 +176,10 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
     tma_prefetch_desc(&mapL);
     tma_prefetch_desc(&mapR);
     tma_prefetch_desc(&mapO);
+    if (MODE == 2) {
+      tma_prefetch_desc(&mapL2);
+      tma_prefetch_desc(&mapR2);
+    }
   }
   if (warp == 2) {
     if (PAIR) tmem_alloc_2cta<512>(tmem_slot); else tmem_alloc<512>(tmem_slot);
@@ -197,7 +205,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
     uint32_t eph = 1;   // parity of rempty[rs] to wait for (the first pass over the ring does not block)
     for (long long idx = unit; idx < g.total; idx += nunits) {
       int rowL, blkR, j0;
-      if (MODE == 0) {
+      if (MODE != 1) {
         const PhiTile t = phi_decode(g, idx);
         const long long item = static_cast<long long>(t.b) * g.P;
         rowL = static_cast<int>((item + phi_colbase(g.T, t.mid)) * n) + t.m_tile * (kTM * NCTA) +
@@ -210,17 +218,21 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
         blkR = p.gm.r_blk0 + t.b * p.gm.r_blk_stride;
         j0 = t.n_tile * NT + static_cast<int>(rank) * NH;
       }
-      for (int kb = 0; kb < nkb; ++kb, ++it) {
+      for (int kb = 0; kb < nkb_tot; ++kb, ++it) {
         LTV_TRACE(0, it, 0)
         mbar_wait(&rempty[rs], eph);
         LTV_TRACE(0, it, 1)
         uint8_t* sp = smem + static_cast<size_t>(rs) * kRawBytes;
+        const bool second = (MODE == 2) && kb >= nkb;
+        const int kc = (second ? kb - nkb : kb) * kKB;
+        const CUtensorMap* mL = second ? &mapL2 : &mapL;
+        const CUtensorMap* mR = second ? &mapR2 : &mapR;
         if (elect_one()) {
           mbar_arrive_expect_tx(&full[rs], kRawBytes);
-          tma_load_2d(sp, &mapL, kb * kKB, rowL, &full[rs], pol);
+          tma_load_2d(sp, mL, kc, rowL, &full[rs], pol);
 #pragma unroll
           for (int c = 0; c < NBOX; ++c)
-            tma_load_3d(sp + kABytes + c * 4096, &mapR, j0 + 32 * c, kb * kKB, blkR, &full[rs], pol);
+            tma_load_3d(sp + kABytes + c * 4096, mR, j0 + 32 * c, kc, blkR, &full[rs], pol);
         }
         __syncwarp();
         if (++rs == R) { rs = 0; eph ^= 1; }
@@ -239,7 +251,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
         if (lt >= 2) mbar_wait(&tempty[acc], ((lt >> 1) - 1) & 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + acc * NT;
-        for (int kb = 0; kb < nkb; ++kb, ++it) {
+        for (int kb = 0; kb < nkb_tot; ++kb, ++it) {
           LTV_TRACE(1, it, 0)
           mbar_wait(&conv[cs], cph);
           tc_fence_after();
@@ -248,7 +260,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
           const uint32_t sb_lo = smem_u32(lo_ring + static_cast<size_t>(cs) * kBBytes);
           const uint32_t a_hi = tmem_base + kTmemA + cs * 64;   // raw fp32 bits: the MMA keeps the top 19
           const uint32_t a_lo = a_hi + 32;
-          const int nks = (kb == nkb - 1) ? ks_last : 4;
+          const int nks = (kb == nkb - 1 || kb == nkb_tot - 1) ? ks_last : 4;
           if (elect_one()) {
 #pragma unroll
             for (int ks = 0; ks < 4; ++ks) {
@@ -264,7 +276,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
             }
             umma_commit_all<PAIR>(&rempty[rs]);
             umma_commit_all<PAIR>(&cempty[cs]);
-            if (kb == nkb - 1) umma_commit_all<PAIR>(&tfull[acc]);
+            if (kb == nkb_tot - 1) umma_commit_all<PAIR>(&tfull[acc]);
           }
           __syncwarp();
           LTV_TRACE(1, it, 2)
@@ -286,7 +298,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
     int rs = 0, cs = 0;
     uint32_t rph = 0, cph = 1;   // parity of full[rs]; parity of cempty[cs] (the first use does not block)
     for (long long idx = unit; idx < g.total; idx += nunits) {
-      for (int kb = 0; kb < nkb; ++kb, ++it) {
+      for (int kb = 0; kb < nkb_tot; ++kb, ++it) {
         if (static_cast<int>(it & 1) == grp) {
           const int trole = 2 + grp;
           if (q == 0) { LTV_TRACE(trole, it, 0) }
@@ -416,7 +428,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
       const int j0 = t.n_tile * NT;
       float* wb = wbuf + acc * NT;
       for (int j = etid; j < NT; j += 128)
-        wb[j] = (j0 + j < n) ? __ldg(p.w + (static_cast<size_t>(t.b) * g.T + t.s) * n + j0 + j) : 0.f;
+        wb[j] = (MODE == 0 && j0 + j < n) ? __ldg(p.w + (static_cast<size_t>(t.b) * g.T + t.s) * n + j0 + j) : 0.f;
       named_bar_sync(1, 128);
       const size_t item = static_cast<size_t>(t.b) * g.P;
       const size_t qcol = item + phi_colbase(g.T, t.s) + (t.mid - t.s);  // block (mid+1, s)
@@ -437,7 +449,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
         uint32_t (&vc)[32] = v[cc & 1];
         tmem_ld_wait();
         if (cc + 1 < NCH) tmem_ld_32x32(taddr + (cc + 1) * 32, v[(cc + 1) & 1]);
-        if (!(DBG & 512)) {
+        if (MODE == 0 && !(DBG & 512)) {
           const float4* w4 = reinterpret_cast<const float4*>(wb + cc * 32);
 #pragma unroll
           for (int e = 0; e < 8; ++e) {
@@ -483,7 +495,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
       __syncwarp();
       if (warp == 4) { LTV_TRACE(4, lt, 2) }
       if (lane == 0) arrive_leader(&tempty[acc]);
-      if (lane < rows_valid)
+      if (MODE == 0 && lane < rows_valid)
         p.part[((qcol + rho / n) * g.NT + t.n_tile) * n + rho % n] = (tube4[0] + tube4[1]) + (tube4[2] + tube4[3]);
     }
     if (lane == 0) tma_store_wait_all<0>();   // shared memory must outlive the last bulk store
@@ -524,8 +536,8 @@ cudaError_t launch_tc_dbg(const TcParams& p, const TcMaps& maps, int num_sms, cu
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  ProfScope prof(MODE == 0 ? kProfPhiCombineTc : kProfKalmanGemm, stream);
-  return cudaLaunchKernelEx(&cfg, kern, q, maps.L, maps.R, maps.O);
+  ProfScope prof(MODE == 1 ? kProfKalmanGemm : kProfPhiCombineTc, stream);
+  return cudaLaunchKernelEx(&cfg, kern, q, maps.L, maps.R, maps.O, MODE == 2 ? maps.L2 : maps.L, MODE == 2 ? maps.R2 : maps.R);
 }
 
 template <int NCH, bool PAIR>
@@ -619,6 +631,45 @@ cudaError_t launch_phi_combine_tc(const PhiArgs& a, int level, int nch, const vo
   p.g = pair ? g2 : g1;
 #define LTV_NCH_CASE(N) \
   case N: return pair ? launch_tc<N, true>(p, m, num_sms, stream) : launch_tc<N, false>(p, m, num_sms, stream);
+  switch (nch) {
+    LTV_NCH_CASE(2) LTV_NCH_CASE(3) LTV_NCH_CASE(4) LTV_NCH_CASE(5)
+    default: return cudaErrorInvalidValue;
+  }
+#undef LTV_NCH_CASE
+}
+
+// ---------------------------------------------------------------------------------------- cross block (MODE 2)
+// G(t,s) = Pbar(t,mid) G(mid,s) + G(t,mid) Phat(mid,s) on the geometry of the Phi scan (a.phi = G; no tube).
+cudaError_t phi_tc_make_cross_maps(const PhiArgs& a, const float* pbar, const float* phat, int nch, void* maps_out) {
+  TcMaps mg, mb, mh;
+  PhiArgs t = a;
+  cudaError_t e = phi_tc_make_maps(t, nch, &mg);
+  if (e != cudaSuccess) return e;
+  t.phi = const_cast<float*>(pbar);
+  if ((e = phi_tc_make_maps(t, nch, &mb)) != cudaSuccess) return e;
+  t.phi = const_cast<float*>(phat);
+  if ((e = phi_tc_make_maps(t, nch, &mh)) != cudaSuccess) return e;
+  TcMaps* m = static_cast<TcMaps*>(maps_out);
+  m->L = mb.L;    // Pbar(t,mid) stack
+  m->R = mg.R;    // G(mid,s)
+  m->L2 = mg.L;   // G(t,mid) stack
+  m->R2 = mh.R;   // Phat(mid,s)
+  m->O = mg.O;
+  return cudaSuccess;
+}
+
+cudaError_t launch_phi_cross_tc(const PhiArgs& a, int level, int nch, const void* maps, int num_sms, cudaStream_t stream) {
+  TcParams p{};
+  p.phi = a.phi; p.w = nullptr; p.part = nullptr; p.tube_mode = 0;
+  const TcMaps& m = *static_cast<const TcMaps*>(maps);
+  const PhiGeom g1 = phi_geom(a.batch, a.T, a.n, a.nc, level, kTM, 32 * nch);
+  const PhiGeom g2 = phi_geom(a.batch, a.T, a.n, a.nc, level, 2 * kTM, 32 * nch);
+  if (g1.total == 0) return cudaSuccess;
+  const bool pair = 2 * g2.total * 100 <= g1.total * 108;
+  p.g = pair ? g2 : g1;
+#define LTV_NCH_CASE(N_)                                                              \
+  case N_: return pair ? launch_tc_dbg<N_, true, 0, 2>(p, m, num_sms, stream)         \
+                       : launch_tc_dbg<N_, false, 0, 2>(p, m, num_sms, stream);
   switch (nch) {
     LTV_NCH_CASE(2) LTV_NCH_CASE(3) LTV_NCH_CASE(4) LTV_NCH_CASE(5)
     default: return cudaErrorInvalidValue;
