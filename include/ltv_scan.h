@@ -213,11 +213,13 @@ LTV_API int ltv_scan_kalman_gains(const float* A, const float* C, const float* e
  *   phi_xe_out device [batch,P,n,p]   same block order; blocks with j = 0 are zero; may be NULL
  *   tau_out   device [batch,T,n]
  *   flags     must be 0
- * Method: the closed loop in (x, x - xhat) is the LTV system [[A + B Kfb, -B Kfb], [0, A + Lt C]]; the library forms these
- * 2n x 2n Jacobians, runs the time-parallel scan of ltv_scan_system_response_tube on them and reads Phi^xw = G11 + G12,
- * Phi^xe = G12 Lt_{j-1} off the blocks G of that response in one pass that also accumulates the tube (deterministic).
- * The scan on 2n states costs 8x the n-state scan and 4x its memory (workspace); a general Phibar and the low-rank form
- * of (15) are not built.  n <= 4096.  Workspace: ltv_scan_workspace_bytes(LTV_OP_OUTPUT_FEEDBACK, batch, T, n, 0). */
+ * Method: the closed loop in (x, x - xhat) is the LTV system A_aug = [[A + B Kfb, -B Kfb], [0, A + Lt C]], and with
+ * G = Phi_aug(k,j): Phi^xw = G11 + G12, Phi^xe = G12 Lt_{j-1}.  G is block upper triangular (G11 = Phibar^x,
+ * G22 = Phihat^x) and G12(t,s) = G11(t,mid) G12(mid,s) + G12(t,mid) G22(mid,s), so for n >= 96 the library runs two
+ * n-state time-parallel scans and one cross scan whose combine accumulates both products in one tcgen05 K loop (4
+ * instead of 8 n^3 products per block); for n < 96 it runs the plain scan on the 2n x 2n Jacobians.  One last pass forms
+ * Phi^xw (in place over Phibar^x), Phi^xe and the tube (deterministic).  A general Phibar and the low-rank form of (15)
+ * are not built.  n <= 4096.  Workspace: ltv_scan_workspace_bytes(LTV_OP_OUTPUT_FEEDBACK, batch, T, n, 0). */
 LTV_API int ltv_scan_output_feedback_response(const float* A, const float* B, const float* Kfb, const float* Lt,
                                               const float* C, const float* w, const float* f, float* phi_xw_out,
                                               float* phi_xe_out, float* tau_out, int batch, int T, int n, int m, int p,

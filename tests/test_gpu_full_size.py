@@ -211,3 +211,44 @@ def test_full_size_constraint_tightening(L, ci, nc, items):
     assert np.all(sig[:, 0] == 0.0) and np.all(np.isfinite(sig)) and np.all(sig[:, 1:] > 0.0)
     for b in items:
         assert O.rel_err(sig[b], O.constraint_tightening_item(W.A[b], W.w[b], Hc[b])) <= TOL
+
+
+def test_full_size_output_feedback_response(L):
+    """ltv_scan_output_feedback_response at the C2 size (whole batch, structured path), sampled: for one item the whole
+    block row k = T-1 of Phi^xw, Phi^xe and tau_{T-1} against the blocks of the augmented closed loop, built here by the
+    plain ordered product in fp64 (the oracle tests pin that these blocks equal eq.(15)); tau_0 = 0 everywhere."""
+    import torch
+
+    W = generate(config(1))
+    batch, T, n, m = W.shape
+    p = 6
+    rng = np.random.default_rng(77)
+    K = (0.2 * rng.normal(0.0, 1.0 / np.sqrt(n), (batch, T, m, n))).astype(np.float32)
+    Lt = (0.05 * rng.normal(0.0, 1.0 / np.sqrt(p), (batch, T, n, p))).astype(np.float32)
+    C = rng.normal(0.0, 1.0 / np.sqrt(n), (batch, T, p, n)).astype(np.float32)
+    f = rng.uniform(1e-3, 5e-3, (batch, T, p)).astype(np.float32)
+    d = [torch.from_numpy(a).cuda() for a in (W.A, W.B, K, Lt, C, W.w, f)]
+    xw, xe, tau = L.ltv_scan_output_feedback_response(*d)
+    torch.cuda.synchronize()
+    assert bool(torch.all(tau[:, 0] == 0)) and bool(torch.isfinite(tau).all())
+    b, k = 41, T - 1
+    A64, B64, K64, Lt64, C64 = [a[b].astype(np.float64) for a in (W.A, W.B, K, Lt, C)]
+    Aaug = np.zeros((T, 2 * n, 2 * n))
+    Aaug[:, :n, :n] = A64 + B64 @ K64
+    Aaug[:, :n, n:] = -(B64 @ K64)
+    Aaug[:, n:, n:] = A64 + Lt64 @ C64
+    G = np.eye(2 * n)
+    tau_ref = np.zeros(n)
+    worst_w = worst_e = 0.0
+    for j in range(k - 1, -1, -1):          # G = Phi_aug(k, j) = Phi_aug(k, j+1) A_aug,j
+        G = G @ Aaug[j]
+        ref_w = G[:n, :n] + G[:n, n:]
+        q = L.ltv_phi_block_index(T, k, j)
+        worst_w = max(worst_w, O.rel_err(xw[b, q].cpu().numpy(), ref_w))
+        tau_ref += np.sqrt(np.sum((ref_w * W.w[b, j].astype(np.float64)[None, :]) ** 2, axis=1))
+        if j >= 1:
+            ref_e = G[:n, n:] @ Lt64[j - 1]
+            worst_e = max(worst_e, O.rel_err(xe[b, q].cpu().numpy(), ref_e))
+            tau_ref += np.sqrt(np.sum((ref_e * f[b, j - 1].astype(np.float64)[None, :]) ** 2, axis=1))
+    assert worst_w <= TOL and worst_e <= TOL
+    assert O.rel_err(tau[b, k].cpu().numpy(), tau_ref) <= TOL
