@@ -295,6 +295,7 @@ int ltv_scan_observer_response(const float* A, const float* Lt, const float* C, 
   a.Lt = Lt;
   a.C = C;
   a.p = p;
+  if (p > 8) a.Ltt = reinterpret_cast<float*>(static_cast<char*>(workspace) + phi_part_bytes(batch, T, n, nc));
   unsigned long long l = 0;
   cudaError_t e = launch_phi_tube(a, static_cast<cudaStream_t>(cuda_stream), &l);
   g_launches += l;

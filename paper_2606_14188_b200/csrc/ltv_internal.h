@@ -35,11 +35,13 @@ struct PhiArgs {
   const float* Lt = nullptr;  // [batch,T,n,p] = L_j^T, or nullptr: plain system response
   const float* C = nullptr;   // [batch,T,p,n]
   int p = 0;
+  float* Ltt = nullptr;       // workspace [batch,T,nc-n,n]: the gains transposed (p > 8 only)
 };
 // n-tile width the Phi path uses for this n (decides the size of `part`) and whether it is the tcgen05 path
 int phi_tile_n(int n, int nc);
 bool phi_uses_tensor_cores(int n);
 size_t phi_workspace_bytes(int batch, int T, int n, int nc);
+size_t phi_part_bytes(int batch, int T, int n, int nc);
 cudaError_t launch_phi_tube(const PhiArgs& a, cudaStream_t stream, unsigned long long* launches);
 
 // Kalman recursion of eq.(13) (kalman.cu)

@@ -32,13 +32,21 @@ int phi_pick_nch(int n) { return pick_nch(n); }
 
 int phi_tile_n(int n, int nc) { return phi_uses_tensor_cores(n) ? 32 * pick_nch(nc) : 64; }
 
-size_t phi_workspace_bytes(int batch, int T, int n, int nc) {
+// bytes of the tube partials `part` (the first region of the Phi workspace)
+size_t phi_part_bytes(int batch, int T, int n, int nc) {
   const int tn = phi_tile_n(n, nc);
   const size_t NT = (nc + tn - 1) / tn;
   const size_t P = static_cast<size_t>(T) * (T - 1) / 2;
   size_t bytes = static_cast<size_t>(batch) * P * NT * n * sizeof(float);
   if (bytes == 0) bytes = 16;
   return align_up(bytes, 256);
+}
+
+// observer with p > 8 (nc - n > 8): a second region holds the gains transposed, Lt^T [batch,T,nc-n,n]
+size_t phi_workspace_bytes(int batch, int T, int n, int nc) {
+  size_t bytes = phi_part_bytes(batch, T, n, nc);
+  if (nc - n > 8) bytes += align_up(static_cast<size_t>(batch) * T * (nc - n) * n * sizeof(float), 256);
+  return bytes;
 }
 
 cudaError_t launch_phi_tube(const PhiArgs& a, cudaStream_t stream, unsigned long long* launches) {

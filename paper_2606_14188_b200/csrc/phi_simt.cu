@@ -84,76 +84,109 @@ __global__ void __launch_bounds__(256) phi_level0_kernel(const float* __restrict
 //   PhiX(s+1,s) = Abar_s = A_s + Lt_s C_s   (rank-p update while A_s streams through: HBM-bound like the copy)
 //   PhiY(s+1,s) = Abar_s Lt_s               (skinny product, second kernel; Abar_s is still in L2)
 // written side by side in rows of nc = n + roundup4(p) floats; the tube partial is taken over PhiX.
-__global__ void __launch_bounds__(256) phi_obs_level0_kernel(const float* __restrict__ A, const float* __restrict__ Lt,
-                                                             const float* __restrict__ C, const float* __restrict__ w,
-                                                             float* __restrict__ phi, float* __restrict__ part, int batch,
-                                                             int T, int n, int nc, int p, int NT, int mode) {
-  const int P = T * (T - 1) / 2;
-  const long long nrows = static_cast<long long>(batch) * (T - 1) * n;
-  const int lane = threadIdx.x & 31;
-  const int n4 = n >> 2;
-  for (long long row = static_cast<long long>(blockIdx.x) * 8 + (threadIdx.x >> 5); row < nrows;
-       row += static_cast<long long>(gridDim.x) * 8) {
-    const int i = static_cast<int>(row % n);
-    const long long bs = row / n;
-    const int s = static_cast<int>(bs % (T - 1));
-    const int b = static_cast<int>(bs / (T - 1));
-    const size_t bt = static_cast<size_t>(b) * T + s;
-    const float4* src = reinterpret_cast<const float4*>(A + (bt * n + i) * n);
-    const float4* wv = reinterpret_cast<const float4*>(w + bt * n);
-    const float* lrow = Lt + (bt * n + i) * p;
-    const float4* Cs = reinterpret_cast<const float4*>(C + bt * p * n);
-    const size_t q = static_cast<size_t>(b) * P + phi_colbase(T, s);
-    float* dst = phi + (q * n + i) * nc;
-    float acc = 0.f;
-    for (int c = lane; c < n4; c += 32) {
-      float4 a = __ldcs(src + c);
-      for (int k = 0; k < p; ++k) {
-        const float l = __ldg(lrow + k);
-        const float4 ck = __ldg(Cs + static_cast<size_t>(k) * n4 + c);
-        a.x = fmaf(l, ck.x, a.x); a.y = fmaf(l, ck.y, a.y); a.z = fmaf(l, ck.z, a.z); a.w = fmaf(l, ck.w, a.w);
-      }
-      const float4 ww = __ldg(wv + c);
-      *reinterpret_cast<float4*>(dst + 4 * c) = a;
-      acc += (tube_term(a.x, ww.x, mode) + tube_term(a.y, ww.y, mode)) + (tube_term(a.z, ww.z, mode) + tube_term(a.w, ww.w, mode));
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    for (int e = lane; e < NT; e += 32) part[(q * NT + e) * n + i] = (e == 0) ? acc : 0.f;
+// p > 8: the gains are first transposed (Ltt[b,t][k][j] = Lt[b,t][j][k], columns padded to pp = nc - n with zeros) so
+// that the wide kernel reads them with coalesced 128-bit loads.  grid (batch T), 256 threads.
+__global__ void __launch_bounds__(256) phi_obs_transpose_gains_kernel(const float* __restrict__ Lt, float* __restrict__ Ltt,
+                                                                      int n, int p, int pp) {
+  const size_t bt = blockIdx.x;
+  const float* src = Lt + bt * n * p;
+  float* dst = Ltt + bt * pp * n;
+  for (int e = threadIdx.x; e < pp * n; e += 256) {
+    const int k = e / n, j = e - k * n;
+    dst[e] = (k < p) ? __ldg(src + static_cast<size_t>(j) * p + k) : 0.f;
   }
 }
 
-// PhiY(s+1,s)[i][k] = sum_j Abar_s[i][j] Lt_s[j][k]; pad columns n+p .. nc-1 are zeroed.  One warp per row.
-__global__ void __launch_bounds__(256) phi_obs_y0_kernel(const float* __restrict__ Lt, float* __restrict__ phi, int batch,
-                                                         int T, int n, int nc, int p) {
+// Wide path (8 < p <= 32): a warp takes ROWS rows; per column quad it loads A (ROWS rows), the p rows of C_s and the p rows
+// of Lt_s^T once, forms Abar in registers, stores it, and accumulates the tube partial and the ROWS x p products of
+// PhiY(s+1,s) = Abar_s Lt_s; butterfly reductions at the end.  PG = ceil(p / 8) groups of eight columns (the padded
+// columns of Ltt are zero, so they add nothing and come out as the zero padding of the row).
+template <int PG, int ROWS>
+__global__ void __launch_bounds__(256) phi_obs_level0_wide_kernel(const float* __restrict__ A, const float* __restrict__ Lt,
+                                                                  const float* __restrict__ Ltt, const float* __restrict__ C,
+                                                                  const float* __restrict__ w, float* __restrict__ phi,
+                                                                  float* __restrict__ part, int batch, int T, int n, int nc,
+                                                                  int p, int NT, int mode) {
+  constexpr int PP = 8 * PG;
+  const int pp = nc - n;
   const int P = T * (T - 1) / 2;
-  const long long nrows = static_cast<long long>(batch) * (T - 1) * n;
+  const int n4 = n >> 2;
+  const int ngrp = (n + ROWS - 1) / ROWS;
+  const long long nunits = static_cast<long long>(batch) * (T - 1) * ngrp;
   const int lane = threadIdx.x & 31;
-  for (long long row = static_cast<long long>(blockIdx.x) * 8 + (threadIdx.x >> 5); row < nrows;
-       row += static_cast<long long>(gridDim.x) * 8) {
-    const int i = static_cast<int>(row % n);
-    const long long bs = row / n;
+  for (long long un = static_cast<long long>(blockIdx.x) * 8 + (threadIdx.x >> 5); un < nunits;
+       un += static_cast<long long>(gridDim.x) * 8) {
+    const int i = ROWS * static_cast<int>(un % ngrp);
+    const long long bs = un / ngrp;
     const int s = static_cast<int>(bs % (T - 1));
     const int b = static_cast<int>(bs / (T - 1));
-    const float* Ls = Lt + (static_cast<size_t>(b) * T + s) * n * p;
+    const size_t bt = static_cast<size_t>(b) * T + s;
+    const float4* wv = reinterpret_cast<const float4*>(w + bt * n);
+    const float4* Cs = reinterpret_cast<const float4*>(C + bt * p * n);
+    const float4* Lts = reinterpret_cast<const float4*>(Ltt + bt * pp * n);
     const size_t q = static_cast<size_t>(b) * P + phi_colbase(T, s);
-    float* prow = phi + (q * n + i) * nc;
-    for (int k0 = 0; k0 < p; k0 += 4) {       // four output columns per pass
-      float acc[4] = {0.f, 0.f, 0.f, 0.f};
-      for (int j = lane; j < n; j += 32) {
-        const float a = prow[j];
+    const float4* src[ROWS];
+    const float* lrow[ROWS];
 #pragma unroll
-        for (int k = 0; k < 4; ++k)
-          if (k0 + k < p) acc[k] = fmaf(a, __ldg(Ls + static_cast<size_t>(j) * p + k0 + k), acc[k]);
+    for (int r = 0; r < ROWS; ++r) {
+      const int ir = min(i + r, n - 1);
+      src[r] = reinterpret_cast<const float4*>(A + (bt * n + ir) * n);
+      lrow[r] = Lt + (bt * n + ir) * p;
+    }
+    float tube[ROWS], y[ROWS][PP];
+#pragma unroll
+    for (int r = 0; r < ROWS; ++r) {
+      tube[r] = 0.f;
+#pragma unroll
+      for (int k = 0; k < PP; ++k) y[r][k] = 0.f;
+    }
+    for (int c = lane; c < n4; c += 32) {
+      float4 a[ROWS];
+#pragma unroll
+      for (int r = 0; r < ROWS; ++r) a[r] = __ldcs(src[r] + c);
+      for (int k = 0; k < p; ++k) {
+        const float4 ck = __ldg(Cs + static_cast<size_t>(k) * n4 + c);
+#pragma unroll
+        for (int r = 0; r < ROWS; ++r) {
+          const float l = __ldg(lrow[r] + k);
+          a[r].x = fmaf(l, ck.x, a[r].x); a[r].y = fmaf(l, ck.y, a[r].y);
+          a[r].z = fmaf(l, ck.z, a[r].z); a[r].w = fmaf(l, ck.w, a[r].w);
+        }
+      }
+      const float4 ww = __ldg(wv + c);
+#pragma unroll
+      for (int r = 0; r < ROWS; ++r) {
+        if (i + r < n) *reinterpret_cast<float4*>(phi + (q * n + i + r) * nc + 4 * c) = a[r];
+        tube[r] += (tube_term(a[r].x, ww.x, mode) + tube_term(a[r].y, ww.y, mode)) +
+                   (tube_term(a[r].z, ww.z, mode) + tube_term(a[r].w, ww.w, mode));
       }
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
+      for (int kg = 0; kg < PP; kg += 8) {
+        float4 lt[8];
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], o);
-        if (lane == 0 && k0 + k < p) prow[n + k0 + k] = acc[k];
+        for (int k = 0; k < 8; ++k) lt[k] = __ldg(Lts + static_cast<size_t>(min(kg + k, pp - 1)) * n4 + c);
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+#pragma unroll
+          for (int r = 0; r < ROWS; ++r)
+            y[r][kg + k] = fmaf(a[r].x, lt[k].x, fmaf(a[r].y, lt[k].y, fmaf(a[r].z, lt[k].z, fmaf(a[r].w, lt[k].w, y[r][kg + k]))));
       }
     }
-    for (int k = n + p + lane; k < nc; k += 32) prow[k] = 0.f;
+#pragma unroll
+    for (int r = 0; r < ROWS; ++r) {
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) tube[r] += __shfl_xor_sync(0xffffffffu, tube[r], o);
+#pragma unroll
+      for (int k = 0; k < PP; ++k) {
+        if (k < pp) {
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) y[r][k] += __shfl_xor_sync(0xffffffffu, y[r][k], o);
+          if (lane == (k & 31) && i + r < n) phi[(q * n + i + r) * nc + n + k] = y[r][k];
+        }
+      }
+      if (lane == 0 && i + r < n)
+        for (int e = 0; e < NT; ++e) part[(q * NT + e) * n + i + r] = (e == 0) ? tube[r] : 0.f;
+    }
   }
 }
 
@@ -257,7 +290,7 @@ __global__ void __launch_bounds__(128) phi_tube_finalize_kernel(const float* __r
 // four rows j..j+3 of Lt_s (4p contiguous floats) ONCE, forms Abar in registers, stores it, and accumulates both the
 // tube partial and the 4 x p products of PhiY(s+1,s) = Abar_s Lt_s; the 4 + 4p sums are finished by shuffles.
 template <int PP>
-__global__ void __launch_bounds__(256) phi_obs_level0_fused_kernel(const float* __restrict__ A, const float* __restrict__ Lt,
+__global__ void __launch_bounds__(256, 2) phi_obs_level0_fused_kernel(const float* __restrict__ A, const float* __restrict__ Lt,
                                                                    const float* __restrict__ C, const float* __restrict__ w,
                                                                    float* __restrict__ phi, float* __restrict__ part,
                                                                    int batch, int T, int n, int nc, int NT, int mode) {
@@ -376,11 +409,27 @@ cudaError_t launch_phi_obs_level0(const PhiArgs& a, int NT, int num_sms, cudaStr
 #undef LTV_OBS_CASE
     return cudaGetLastError();
   }
-  phi_obs_level0_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(a.A, a.Lt, a.C, a.w, a.phi, a.part, a.batch, a.T,
-                                                                           a.n, a.nc, a.p, NT, a.tube_mode);
+  // 8 < p <= 32: transpose the gains, then the wide fused kernel
+  const int pp = a.nc - a.n;
+  if (a.Ltt == nullptr) return cudaErrorInvalidValue;
+  phi_obs_transpose_gains_kernel<<<static_cast<unsigned>(a.batch * a.T), 256, 0, stream>>>(a.Lt, a.Ltt, a.n, a.p, pp);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
-  phi_obs_y0_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(a.Lt, a.phi, a.batch, a.T, a.n, a.nc, a.p);
+  constexpr int kRows = 2;
+  const long long nunits = static_cast<long long>(a.batch) * (a.T - 1) * ((a.n + kRows - 1) / kRows);
+  long long ub = (nunits + 7) / 8;
+  const long long ucap = static_cast<long long>(num_sms) * 8;
+  if (ub > ucap) ub = ucap;
+#define LTV_OBSW_CASE(PGV)                                                                                         \
+  case PGV:                                                                                                        \
+    phi_obs_level0_wide_kernel<PGV, kRows><<<static_cast<unsigned>(ub), 256, 0, stream>>>(                          \
+        a.A, a.Lt, a.Ltt, a.C, a.w, a.phi, a.part, a.batch, a.T, a.n, a.nc, a.p, NT, a.tube_mode);                  \
+    break;
+  switch ((pp + 7) / 8) {
+    LTV_OBSW_CASE(2) LTV_OBSW_CASE(3) LTV_OBSW_CASE(4)
+    default: return cudaErrorInvalidValue;
+  }
+#undef LTV_OBSW_CASE
   return cudaGetLastError();
 }
 

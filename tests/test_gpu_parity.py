@@ -312,6 +312,8 @@ def _observer_inputs(batch, T, n, p, seed):
                                          (128, 5, 2, 6),     # tensor-core path, nc = 136: second n-tile is PhiY only
                                          (300, 9, 2, 6),     # C2 shape: nc = 308 fits the padding of two 160-wide tiles
                                          (164, 4, 1, 32),    # widest gain block
+                                         (132, 5, 2, 12),    # wide path (p > 8): transposed gains, two column groups
+                                         (300, 4, 1, 20),    # wide path, three column groups (nc = 320)
                                          (100, 3, 3, 1)])
 def test_observer_response(L, n, T, batch, p):
     """NEXT-1, eq.(14): PhiX over the closed-loop matrices A + Lt C, PhiY = PhiX Lt riding along as extra columns;
