@@ -12,6 +12,17 @@ def shard_range(global_batch: int, rank: int, world: int) -> tuple[int, int]:
     return b0, b0 + base + (1 if rank < rem else 0)
 
 
+def shard_arrays(arrays: dict, rank: int, world: int) -> dict:
+    """The items [b0, b1) of this rank of every batch-leading array in `arrays` (None entries pass through): all calls of
+    the library - rollout, system response, adjoint, observer response, Kalman gains, constraint margins, output-feedback
+    responses - treat batch items independently, so this is the whole distribution scheme."""
+    sizes = {v.shape[0] for v in arrays.values() if v is not None}
+    if len(sizes) != 1:
+        raise ValueError("arrays disagree on the batch size")
+    b0, b1 = shard_range(sizes.pop(), rank, world)
+    return {k: (None if v is None else v[b0:b1]) for k, v in arrays.items()}
+
+
 def reduce_max(value: float, device=None) -> float:
     """max over ranks of a python float (identity when torch.distributed is not initialised)."""
     import torch

@@ -24,8 +24,8 @@ def _worker(rank, world, port, q):
     import torch.distributed as dist
 
     from oracle import ltv_oracle as O
-    from paper_2606_14188_b200.sharding import reduce_max, reduce_sum
-    from workloads import config, generate
+    from paper_2606_14188_b200.sharding import reduce_max, reduce_sum, shard_arrays
+    from workloads import config, generate, observation_model
 
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
@@ -35,9 +35,17 @@ def _worker(rank, world, port, q):
     W = generate(cfg, item_range=(b0, b1))
     X = O.rollout(W.A, W.B, W.c, W.x0, W.u)
     r = O.tube(W.A, W.w)
+    # the next rows shard the same way: observation model generated for the whole batch, sliced per rank
+    Wall = generate(cfg)
+    M = observation_model(cfg["batch"], cfg["T"], Wall.A.shape[-1], 3, seed=9, kind="track")
+    Hc = np.random.default_rng(4).normal(size=(cfg["batch"], cfg["T"], 2, Wall.A.shape[-1])).astype(np.float32)
+    mine = shard_arrays(dict(A=Wall.A, w=Wall.w, Hc=Hc, **M), rank, world)
+    assert np.array_equal(mine["A"], W.A)
+    Pi, Lt = O.kalman_recursion(mine["A"], mine["C"], mine["e"], mine["f"], mine["Pi0"])
+    sig = O.constraint_tightening(mine["A"], mine["w"], mine["Hc"])
     t_max = reduce_max(1.0 + rank)              # "time" of this rank
     units = reduce_sum(float(b1 - b0))
-    q.put((rank, b0, b1, X, r, t_max, units))
+    q.put((rank, b0, b1, X, r, t_max, units, Pi, Lt, sig))
     dist.barrier()
     dist.destroy_process_group()
 
@@ -65,5 +73,12 @@ def test_two_rank_batch_sharding_gloo():
     r = O.tube(W.A, W.w)
     assert np.array_equal(np.concatenate([g[3] for g in got]), X)
     assert np.array_equal(np.concatenate([g[4] for g in got]), r)
+    from workloads import observation_model
+    M = observation_model(5, 6, W.A.shape[-1], 3, seed=9, kind="track")
+    Hc = np.random.default_rng(4).normal(size=(5, 6, 2, W.A.shape[-1])).astype(np.float32)
+    Pi, Lt = O.kalman_recursion(W.A, M["C"], M["e"], M["f"], M["Pi0"])
+    assert np.array_equal(np.concatenate([g[7] for g in got]), Pi)
+    assert np.array_equal(np.concatenate([g[8] for g in got]), Lt)
+    assert np.array_equal(np.concatenate([g[9] for g in got]), O.constraint_tightening(W.A, W.w, Hc))
     assert all(g[5] == 2.0 for g in got)        # max over ranks
     assert all(g[6] == 5.0 for g in got)        # units of all ranks
