@@ -39,19 +39,21 @@ struct Stride2 {
 };
 // measured on B200 (C2 p = 6, C4 p = 12; the variants differ by < 10 %): p <= 8 runs best with two CTAs per SM and the
 // loop not unrolled, wider p with one CTA per SM and two passes in flight
-template <int PG> struct RowCfg {
-  static constexpr int kRows = PG <= 2 ? 4 : 2;
-  static constexpr int kUnroll = PG == 1 ? 1 : 2;
-  static constexpr int kMinBlocks = PG == 1 ? 2 : 1;
+// NP = number of accumulators per row: exactly p for p <= 8 (no padded work: the kernels are instruction-bound), else p
+// rounded up to a multiple of 8 (accumulators beyond p re-read vector p - 1 and are discarded)
+template <int NP> struct RowCfg {
+  static constexpr int kRows = NP <= 16 ? 4 : 2;
+  static constexpr int kUnroll = NP <= 8 ? 1 : 2;
+  static constexpr int kMinBlocks = NP <= 8 ? 2 : 1;
 };
 
 // ROWS rows of a row-major matrix against p vectors V[q][0..n) (global memory, L1-resident: every warp reads the same
 // ones): acc[r][q] = sum_k row_r[k] V[q][k], complete in every lane.  Lane = float4 column, stride 32; ROWS
 // independent 128-bit loads in flight per lane and pass, the vector loads amortised over the ROWS rows.
-template <int PG, int ROWS>
+template <int NP, int ROWS>
 __device__ __forceinline__ void row_dots(const float4* const (&rows)[ROWS], const float* __restrict__ V, int n4, int p,
-                                         int lane, float (&acc)[ROWS][8 * PG]) {
-  constexpr int PP = 8 * PG;
+                                         int lane, float (&acc)[ROWS][NP]) {
+  constexpr int PP = NP;
 #pragma unroll
   for (int r = 0; r < ROWS; ++r)
 #pragma unroll
@@ -62,18 +64,19 @@ __device__ __forceinline__ void row_dots(const float4* const (&rows)[ROWS], cons
   size_t voff[PP];
 #pragma unroll
   for (int q = 0; q < PP; ++q) voff[q] = static_cast<size_t>(min(q, p - 1)) * n4;
-#pragma unroll RowCfg<PG>::kUnroll
+#pragma unroll RowCfg<NP>::kUnroll
   for (int k4 = lane; k4 < n4; k4 += 32) {
     float4 a[ROWS];
 #pragma unroll
     for (int r = 0; r < ROWS; ++r) a[r] = __ldg(rows[r] + k4);
 #pragma unroll
-    for (int qg = 0; qg < PP; qg += 8) {   // eight vector loads in flight at a time
-      float4 v[8];
+    for (int qg = 0; qg < PP; qg += 8) {   // up to eight vector loads in flight at a time
+      constexpr int kGrp = PP < 8 ? PP : 8;   // PP is <= 8 or a multiple of 8
+      float4 v[kGrp];
 #pragma unroll
-      for (int q = 0; q < 8; ++q) v[q] = __ldg(V4 + voff[qg + q] + k4);
+      for (int q = 0; q < kGrp; ++q) v[q] = __ldg(V4 + voff[qg + q] + k4);
 #pragma unroll
-      for (int q = 0; q < 8; ++q) {
+      for (int q = 0; q < kGrp; ++q) {
 #pragma unroll
         for (int r = 0; r < ROWS; ++r) {
           acc[r][qg + q] = fmaf(a[r].x, v[q].x, acc[r][qg + q]);
@@ -97,8 +100,8 @@ __device__ __forceinline__ void row_dots(const float4* const (&rows)[ROWS], cons
 
 // G[b][q][j] = sum_k Pi[b][j][k] C[b][q][k]  (= (C Pi)[q][j]: Pi is symmetric, so its ROW j serves as column j and the
 // loads are contiguous).  Warp = ROWS rows of Pi; grid (ceil(n / (8 ROWS)), batch), 256 threads.
-template <int PG, int ROWS>
-__global__ void __launch_bounds__(32 * kRowWarps, RowCfg<PG>::kMinBlocks) kalman_cpi_kernel(const float* __restrict__ C, Stride2 c_stride,
+template <int NP, int ROWS>
+__global__ void __launch_bounds__(32 * kRowWarps, RowCfg<NP>::kMinBlocks) kalman_cpi_kernel(const float* __restrict__ C, Stride2 c_stride,
                                                                     const float* __restrict__ Pi, Stride2 pi_stride,
                                                                     float* __restrict__ G, int n, int p) {
   const int b = blockIdx.y;   // (item, step) pair
@@ -110,11 +113,11 @@ __global__ void __launch_bounds__(32 * kRowWarps, RowCfg<PG>::kMinBlocks) kalman
 #pragma unroll
   for (int r = 0; r < ROWS; ++r)
     rows[r] = reinterpret_cast<const float4*>(Pi + pi_stride.at(b) + static_cast<size_t>(min(j0 + r, n - 1)) * n);
-  float acc[ROWS][8 * PG];
-  row_dots<PG, ROWS>(rows, C + c_stride.at(b), n4, p, lane, acc);
+  float acc[ROWS][NP];
+  row_dots<NP, ROWS>(rows, C + c_stride.at(b), n4, p, lane, acc);
   float* Gb = G + static_cast<size_t>(b) * p * n;
 #pragma unroll
-  for (int q = 0; q < 8 * PG; ++q) {
+  for (int q = 0; q < NP; ++q) {
     if (q < p && lane == (q & 31)) {
 #pragma unroll
       for (int r = 0; r < ROWS; ++r)
@@ -211,11 +214,11 @@ __global__ void __launch_bounds__(256) kalman_gain_kernel(const float* __restric
 
 // Warp = ROWS rows i of A_j: Lt[i][q] = -sum_k A[i][k] K[q][k];  Abar[i][:] = A[i][:] + sum_q Lt[i][q] C[q][:].
 // grid (ceil(n / (8 ROWS)), batch), 256 threads.
-template <int PG, int ROWS>
-__global__ void __launch_bounds__(32 * kRowWarps, RowCfg<PG>::kMinBlocks) kalman_closed_loop_kernel(
+template <int NP, int ROWS>
+__global__ void __launch_bounds__(32 * kRowWarps, RowCfg<NP>::kMinBlocks) kalman_closed_loop_kernel(
     const float* __restrict__ A, Stride2 a_stride, const float* __restrict__ C, Stride2 c_stride,
     const float* __restrict__ K, float* __restrict__ Lt, Stride2 lt_stride, float* __restrict__ Abar, int n, int p) {
-  constexpr int PP = 8 * PG;
+  constexpr int PP = NP;
   const int b = blockIdx.y;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int i0 = (blockIdx.x * kRowWarps + warp) * ROWS;
@@ -226,7 +229,7 @@ __global__ void __launch_bounds__(32 * kRowWarps, RowCfg<PG>::kMinBlocks) kalman
   for (int r = 0; r < ROWS; ++r)
     rows[r] = reinterpret_cast<const float4*>(A + a_stride.at(b) + static_cast<size_t>(min(i0 + r, n - 1)) * n);
   float acc[ROWS][PP];
-  row_dots<PG, ROWS>(rows, K + static_cast<size_t>(b) * p * n, n4, p, lane, acc);
+  row_dots<NP, ROWS>(rows, K + static_cast<size_t>(b) * p * n, n4, p, lane, acc);
 #pragma unroll
   for (int q = 0; q < PP; ++q) {
     if (q < p) {
@@ -254,11 +257,12 @@ __global__ void __launch_bounds__(32 * kRowWarps, RowCfg<PG>::kMinBlocks) kalman
     for (int r = 0; r < ROWS; ++r) a[r] = __ldg(rows[r] + k4);
 #pragma unroll
     for (int qg = 0; qg < PP; qg += 8) {
-      float4 cc[8];
+      constexpr int kGrp = PP < 8 ? PP : 8;
+      float4 cc[kGrp];
 #pragma unroll
-      for (int q = 0; q < 8; ++q) cc[q] = __ldg(C4 + coff[qg + q] + k4);
+      for (int q = 0; q < kGrp; ++q) cc[q] = __ldg(C4 + coff[qg + q] + k4);
 #pragma unroll
-      for (int q = 0; q < 8; ++q) {
+      for (int q = 0; q < kGrp; ++q) {
 #pragma unroll
         for (int r = 0; r < ROWS; ++r) {
           a[r].x = fmaf(acc[r][qg + q], cc[q].x, a[r].x);
@@ -333,6 +337,29 @@ cudaError_t dispatch_pg(int p, F&& fn) {
   }
 }
 
+// NP (accumulators of the row kernels: p itself up to 8, else p rounded up to a multiple of 8) and PG = ceil(p / 8)
+template <typename F>
+cudaError_t dispatch_np(int p, F&& fn) {
+  using std::integral_constant;
+  switch (p) {
+    case 1: return fn(integral_constant<int, 1>{}, integral_constant<int, 1>{});
+    case 2: return fn(integral_constant<int, 2>{}, integral_constant<int, 1>{});
+    case 3: return fn(integral_constant<int, 3>{}, integral_constant<int, 1>{});
+    case 4: return fn(integral_constant<int, 4>{}, integral_constant<int, 1>{});
+    case 5: return fn(integral_constant<int, 5>{}, integral_constant<int, 1>{});
+    case 6: return fn(integral_constant<int, 6>{}, integral_constant<int, 1>{});
+    case 7: return fn(integral_constant<int, 7>{}, integral_constant<int, 1>{});
+    case 8: return fn(integral_constant<int, 8>{}, integral_constant<int, 1>{});
+    default: break;
+  }
+  switch ((p + 7) / 8) {
+    case 2: return fn(integral_constant<int, 16>{}, integral_constant<int, 2>{});
+    case 3: return fn(integral_constant<int, 24>{}, integral_constant<int, 3>{});
+    case 4: return fn(integral_constant<int, 32>{}, integral_constant<int, 4>{});
+    default: return cudaErrorInvalidValue;
+  }
+}
+
 struct KalmanWs {
   float *G, *K, *Abar, *Yt;
 };
@@ -357,13 +384,14 @@ cudaError_t launch_kalman_gain_chain(const KalmanArgs& a, int j0, int nj, float*
   const float* Cj = a.C + static_cast<size_t>(j0) * p * n;
   const float* Aj = a.A + static_cast<size_t>(j0) * n * n;
   const float* Pij = a.Pi_out + static_cast<size_t>(j0) * n * n;
-  return dispatch_pg(p, [&](auto pg) {
+  return dispatch_np(p, [&](auto np_, auto pg) {
+    constexpr int NP = decltype(np_)::value;
     constexpr int PG = decltype(pg)::value;
-    constexpr int ROWS = RowCfg<PG>::kRows;
+    constexpr int ROWS = RowCfg<NP>::kRows;
     const dim3 rgrid((n + kRowWarps * ROWS - 1) / (kRowWarps * ROWS), pairs);
     {
       ProfScope prof(kProfKalmanSimt, stream);
-      kalman_cpi_kernel<PG, ROWS><<<rgrid, 32 * kRowWarps, 0, stream>>>(Cj, sC, Pij, sPi, G, n, p);
+      kalman_cpi_kernel<NP, ROWS><<<rgrid, 32 * kRowWarps, 0, stream>>>(Cj, sC, Pij, sPi, G, n, p);
     }
     cudaError_t ee = cudaGetLastError();
     if (ee != cudaSuccess) return ee;
@@ -374,7 +402,7 @@ cudaError_t launch_kalman_gain_chain(const KalmanArgs& a, int j0, int nj, float*
     if ((ee = cudaGetLastError()) != cudaSuccess) return ee;
     {
       ProfScope prof(kProfKalmanSimt, stream);
-      kalman_closed_loop_kernel<PG, ROWS><<<rgrid, 32 * kRowWarps, 0, stream>>>(
+      kalman_closed_loop_kernel<NP, ROWS><<<rgrid, 32 * kRowWarps, 0, stream>>>(
           Aj, sA, Cj, sC, K, a.Lt_out + static_cast<size_t>(j0) * n * p, sLt, Abar, n, p);
     }
     return cudaGetLastError();
