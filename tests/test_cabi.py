@@ -106,7 +106,9 @@ def test_host_side_validation_needs_no_gpu(L):
     assert o(p, p, p, p, p, p, p, p, None, p, 1, 2, 4100, 2, 2, 0, p, 1 << 24, None) == 3   # 2n beyond the scan's limit
     assert o(p, p, p, p, p, p, p, p, None, p, 1, 2, 4, 2, 2, 0, p, 8, None) == 5            # workspace too small
     need = L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, b, T, n, 0)
-    assert need >= 4 * b * (T * (T - 1) // 2) * n * n * 4                               # Phi of the 2n-state system
+    assert need >= 2 * b * (T * (T - 1) // 2) * n * n * 4     # n >= 96: Phihat^x and the cross block (Phibar^x sits in the output)
+    need48 = L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, b, T, 48, 0)
+    assert need48 >= 4 * b * (T * (T - 1) // 2) * 48 * 48 * 4  # n < 96: Phi of the 2n-state augmented system
     a = L.lib.ltv_scan_adjoint
     assert a(p, None, p, p, p, None, 1, 2, 4, 2, None, 0, None) == 1                # grad_u wanted, B NULL
     assert a(p, p, None, p, None, None, 1, 2, 4, 2, None, 0, None) == 1             # NULL g
