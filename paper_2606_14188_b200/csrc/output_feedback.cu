@@ -25,16 +25,15 @@ namespace ltv {
 
 namespace {
 
-// warp per row i of (b, t): top row i = [A + B K | -B K], bottom row n + i = [0 | A + Lt C].  grid (batch T, ceil(n/8))
+// warp per row i of (b, t): top row i = [A + B K | -B K], bottom row n + i = [0 | A + Lt C].  grid (batch T, ceil(n/32)); four rows per warp, one after the other
 __global__ void __launch_bounds__(256) ofb_build_aug_kernel(const float* __restrict__ A, const float* __restrict__ B,
                                                             const float* __restrict__ Kfb, const float* __restrict__ Lt,
                                                             const float* __restrict__ C, float* __restrict__ Aaug,
                                                             float* __restrict__ Ltt, int n, int m, int p) {
   const size_t bt = blockIdx.x;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int i = blockIdx.y * 8 + warp;
-  if (i >= n) return;
   const int n4 = n >> 2, n2 = 2 * n;
+  for (int i = blockIdx.y * 32 + warp; i < min(n, static_cast<int>(blockIdx.y) * 32 + 32); i += 8) {
   const float4* Ar = reinterpret_cast<const float4*>(A + (bt * n + i) * n);
   const float* Bi = B + (bt * n + i) * m;
   const float* Li = Lt + (bt * n + i) * p;
@@ -61,10 +60,11 @@ __global__ void __launch_bounds__(256) ofb_build_aug_kernel(const float* __restr
     bot[c] = make_float4(0.f, 0.f, 0.f, 0.f);
     bot[n4 + c] = make_float4(a.x + lc.x, a.y + lc.y, a.z + lc.z, a.w + lc.w);
   }
+  }
 }
 
 // structured path: warp per row i of (b, t): Atil = A + B K, Abar = A + Lt C (n x n each), and the level-0 cross block
-// G12(t+1,t) = -B_t K_t into block (t+1, t) of the column-packed G (t <= T-2).  grid (batch T, ceil(n/8))
+// G12(t+1,t) = -B_t K_t into block (t+1, t) of the column-packed G (t <= T-2).  grid (batch T, ceil(n/32)); four rows per warp, one after the other
 __global__ void __launch_bounds__(256) ofb_build_split_kernel(const float* __restrict__ A, const float* __restrict__ B,
                                                               const float* __restrict__ Kfb, const float* __restrict__ Lt,
                                                               const float* __restrict__ C, float* __restrict__ Atil,
@@ -72,11 +72,10 @@ __global__ void __launch_bounds__(256) ofb_build_split_kernel(const float* __res
                                                               float* __restrict__ Ltt, int T, int n, int m, int p) {
   const size_t bt = blockIdx.x;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int i = blockIdx.y * 8 + warp;
-  if (i >= n) return;
   const int n4 = n >> 2;
   const int t = static_cast<int>(bt % T);
   const size_t b = bt / T;
+  for (int i = blockIdx.y * 32 + warp; i < min(n, static_cast<int>(blockIdx.y) * 32 + 32); i += 8) {
   const float4* Ar = reinterpret_cast<const float4*>(A + (bt * n + i) * n);
   const float* Bi = B + (bt * n + i) * m;
   const float* Li = Lt + (bt * n + i) * p;
@@ -106,6 +105,7 @@ __global__ void __launch_bounds__(256) ofb_build_split_kernel(const float* __res
     o1[c] = make_float4(a.x + bk.x, a.y + bk.y, a.z + bk.z, a.w + bk.w);
     o2[c] = make_float4(a.x + lc.x, a.y + lc.y, a.z + lc.z, a.w + lc.w);
     if (o3 != nullptr) o3[c] = make_float4(-bk.x, -bk.y, -bk.z, -bk.w);
+  }
   }
 }
 
@@ -229,7 +229,7 @@ cudaError_t launch_output_feedback(const OfbArgs& a, cudaStream_t stream, unsign
     if ((e = cudaMemsetAsync(wz, 0, b * t * nn * sizeof(float), stream)) != cudaSuccess) return e;
     {
       ProfScope prof(kProfKalmanSimt, stream);
-      ofb_build_split_kernel<<<dim3(batch * T, (n + 7) / 8), 256, 0, stream>>>(a.A, a.B, a.Kfb, a.Lt, a.C, Atil, Abar, G, Ltt,
+      ofb_build_split_kernel<<<dim3(batch * T, (n + 31) / 32), 256, 0, stream>>>(a.A, a.B, a.Kfb, a.Lt, a.C, Atil, Abar, G, Ltt,
                                                                                T, n, a.m, a.p);
     }
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
@@ -263,7 +263,7 @@ cudaError_t launch_output_feedback(const OfbArgs& a, cudaStream_t stream, unsign
   if ((e = cudaMemsetAsync(wz, 0, b * t * n2 * sizeof(float), stream)) != cudaSuccess) return e;   // the scan's own tube is not used
   {
     ProfScope prof(kProfKalmanSimt, stream);
-    ofb_build_aug_kernel<<<dim3(batch * T, (n + 7) / 8), 256, 0, stream>>>(a.A, a.B, a.Kfb, a.Lt, a.C, Aaug, Ltt, n, a.m, a.p);
+    ofb_build_aug_kernel<<<dim3(batch * T, (n + 31) / 32), 256, 0, stream>>>(a.A, a.B, a.Kfb, a.Lt, a.C, Aaug, Ltt, n, a.m, a.p);
   }
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   ++*launches;
