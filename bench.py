@@ -51,6 +51,8 @@ def parse():
     ap.add_argument("--cpu-items", type=int, default=0, help="items in the CPU-oracle sample (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--tf32-peak", action="store_true",
+                    help="only measure the TF32 library-GEMM peak (the roofline denominator) and print it")
     return ap.parse_args()
 
 
@@ -77,11 +79,15 @@ def peaks():
 
 
 class ClockSampler(threading.Thread):
-    """Samples SM clock and throttle reasons with NVML during the timed region."""
+    """Samples SM clock, power and throttle reasons with NVML in a tight loop (one query costs ~0.1-1 ms) and keeps
+    a wall-clock stamp with every sample, so that `result(window=(t0, t1))` reports the samples that fall inside
+    one timed region.  Started once, before the warm-up, so that short regions still hold several samples."""
 
-    def __init__(self, index):
+    def __init__(self, index, period=0.002):
         super().__init__(daemon=True)
-        self.index, self.samples, self.reasons, self.stop_flag, self.max_mhz = index, [], set(), False, None
+        self.index, self.period, self.samples, self.stop_flag, self.max_mhz = index, period, [], False, None
+        self.error = None
+        self.ready = threading.Event()
 
     def run(self):
         try:
@@ -90,26 +96,97 @@ class ClockSampler(threading.Thread):
             N.nvmlInit()
             h = N.nvmlDeviceGetHandleByIndex(self.index)
             self.max_mhz = N.nvmlDeviceGetMaxClockInfo(h, N.NVML_CLOCK_SM)
-            names = {
+            self.names = {
                 N.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
                 N.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
                 N.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
                 N.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
             }
+            self.ready.set()
             while not self.stop_flag:
-                self.samples.append(N.nvmlDeviceGetClockInfo(h, N.NVML_CLOCK_SM))
+                mhz = N.nvmlDeviceGetClockInfo(h, N.NVML_CLOCK_SM)
                 r = N.nvmlDeviceGetCurrentClocksThrottleReasons(h)
-                for bit, nm in names.items():
-                    if r & bit:
-                        self.reasons.add(nm)
-                time.sleep(0.02)
+                try:
+                    watts = N.nvmlDeviceGetPowerUsage(h) / 1e3
+                except Exception:
+                    watts = None
+                self.samples.append((time.time(), mhz, r, watts))
+                time.sleep(self.period)
         except Exception as e:  # NVML missing: report that, never fail the bench
-            self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+            self.error = f"nvml_unavailable:{type(e).__name__}"
+            self.ready.set()
 
-    def result(self):
-        s = sorted(self.samples)
-        return dict(sm_mhz=(s[len(s) // 2] if s else None), sm_max_mhz=self.max_mhz, reasons=sorted(self.reasons),
-                    samples=len(s))
+    def result(self, window=None):
+        """Median SM clock / reasons over the samples stamped inside `window` = (t0, t1) wall-clock seconds (all
+        samples if None).  A window shorter than the sampling period takes the nearest sample on either side."""
+        smp = list(self.samples)
+        if window is not None and smp:
+            t0, t1 = window
+            inside = [s for s in smp if t0 <= s[0] <= t1]
+            if len(inside) < 2:
+                mid = 0.5 * (t0 + t1)
+                inside = sorted(smp, key=lambda s: abs(s[0] - mid))[:2]
+            smp = inside
+        reasons = set()
+        for s in smp:
+            for bit, nm in getattr(self, "names", {}).items():
+                if s[2] & bit:
+                    reasons.add(nm)
+        if self.error:
+            reasons.add(self.error)
+        mhz = sorted(s[1] for s in smp)
+        watts = [s[3] for s in smp if s[3] is not None]
+        return dict(sm_mhz=(mhz[len(mhz) // 2] if mhz else None), sm_max_mhz=self.max_mhz, reasons=sorted(reasons),
+                    samples=len(mhz), power_w_max=(max(watts) if watts else None))
+
+
+def measure_tf32_peak(dev, index, sustained_s=4.0, size=8192):
+    """The roofline denominator of the tensor-bound kernel, measured the way MEASURED_PEAKS.json measures bf16
+    (BASELINE.md section 2): torch.matmul on fp32 size^3 with TF32 allowed (a cuBLAS library
+    GEMM - used ONLY as the yardstick, never on the path), 2 size^3 flop; best of 10 = burst, back to back for
+    `sustained_s` seconds = sustained; SM clock / throttle reasons sampled meanwhile."""
+    import torch
+
+    old = torch.backends.cuda.matmul.allow_tf32
+    torch.backends.cuda.matmul.allow_tf32 = True
+    try:
+        a = torch.randn((size, size), device=dev)
+        b = torch.randn((size, size), device=dev)
+        c = torch.empty((size, size), device=dev)
+        flop = 2.0 * size ** 3
+        for _ in range(3):
+            torch.matmul(a, b, out=c)
+        torch.cuda.synchronize()
+        best = 1e30
+        for _ in range(10):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            torch.matmul(a, b, out=c)
+            e1.record()
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        reps = max(10, int(sustained_s / (best * 1e-3)))
+        sampler = ClockSampler(index)
+        sampler.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        t0 = time.time()
+        e0.record()
+        for _ in range(reps):
+            torch.matmul(a, b, out=c)
+        e1.record()
+        torch.cuda.synchronize()
+        t1 = time.time()
+        sampler.stop_flag = True
+        sampler.join(timeout=2)
+        sus_ms = e0.elapsed_time(e1) / reps
+        del a, b, c
+        return dict(tf32_tflops=flop / (best * 1e-3) / 1e12, tf32_tflops_sustained=flop / (sus_ms * 1e-3) / 1e12,
+                    how=f"torch.matmul fp32 {size}^3, allow_tf32 (cuBLAS), 2 N^3 flop: best of 10 (burst); "
+                        f"{reps} back to back over {t1 - t0:.1f} s (sustained)",
+                    clocks_sustained=sampler.result(window=(t0, t1)))
+    finally:
+        torch.backends.cuda.matmul.allow_tf32 = old
 
 
 def workload(cfg_index, rank, world, batch_override=None):
@@ -197,6 +274,10 @@ def main():
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if args.tf32_peak:
+        if rank == 0:
+            print(json.dumps(dict(tf32_peak=measure_tf32_peak(torch.device("cuda", local), local))), flush=True)
+        return
     import __graft_entry__ as G
 
     G.build()
