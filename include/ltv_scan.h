@@ -73,8 +73,9 @@ enum { LTV_OP_ROLLOUT = 0, LTV_OP_SYSTEM_RESPONSE_TUBE = 1, LTV_OP_ADJOINT = 2, 
  * divide-and-conquer combine  Phi(t,s) = Phi(t,mid) Phi(mid,s)  stream its left operand as one matrix. */
 enum { LTV_PHI_COLUMN_PACKED = 0 };
 
-/* `flags` bits of ltv_scan_system_response_tube. */
-enum { LTV_TUBE_ROW_2NORM = 1 };
+/* `flags` bits of ltv_scan_system_response_tube / ltv_scan_observer_response. */
+enum { LTV_TUBE_ROW_2NORM = 1,
+       LTV_OBSERVER_SHIFTED_GAIN = 2 /* observer call only: PhiY(t,s) = PhiX(t,s) Lt_{s-1}, zero for s = 0 (see there) */ };
 
 /* Block index q(t,s) of the COLUMN_PACKED layout; -1 if not 0 <= s < t <= T-1.  Pure host arithmetic. */
 LTV_API long long ltv_phi_block_index(int T, int t, int s);
@@ -131,13 +132,23 @@ LTV_API int ltv_scan_adjoint(const float* A, const float* B, const float* g,
 /* Closed-loop observer propagation (eq.(14), :177), with gains that do not
  * depend on the injection step k (reading q15):
  *     Abar_j = A_j + Lt_j C_j,   PhiX(t,s) = Abar_{t-1} ... Abar_s,   PhiY(t,s) = PhiX(t,s) Lt_s,   0 <= s < t <= T-1
+ * WARNING - which PhiY: by default PhiY follows eq.(14) AS PRINTED (the gain of step s beside PhiX(t,s)).  That is NOT
+ * the Phihat^y that satisfies the second achievability identity of (12c) and that the assembly (15) needs (DESIGN.md
+ * q20, q21, demonstrated by tests/test_oracle_pins_assembly.py): there the observation of step j-1 enters through
+ * Phihat^y(k,j) = Phihat^x(k,j) Lt_{j-1}, j >= 1, and Phihat^y(k,0) = 0.  Pass LTV_OBSERVER_SHIFTED_GAIN in `flags` to
+ * get that form (PhiY(t,s) = PhiX(t,s) Lt_{s-1}, zero blocks for s = 0); chaining ltv_scan_kalman_gains ->
+ * ltv_scan_observer_response -> (15) without the flag gives a wrong Phi^xe.  ltv_scan_output_feedback_response uses
+ * the shifted form internally.
  *   A        device [batch,T,n,n]     required; A_0 .. A_{T-2} are read
- *   Lt       device [batch,T,n,p]     required; Lt_j = L_j^T (the transposed Kalman gain of (13)), 1 <= p <= 32
+ *   Lt       device [batch,T,n,p]     required; Lt_j is the gain that multiplies C_j, Abar_j = A_j + Lt_j C_j: with
+ *                                     the gains of (13) Lt_j = L_{j+1}^T, i.e. exactly the Lt_out array of
+ *                                     ltv_scan_kalman_gains (DESIGN.md q17); 1 <= p <= 32
  *   C        device [batch,T,p,n]     required; observation Jacobians
  *   w        device [batch,T,n]       required; tube of PhiX exactly as in ltv_scan_system_response_tube
  *   phi_out  device [batch,P,n,nc]    nc = ltv_observer_row_floats(n,p) = n + 4*ceil(p/4); in every row, columns
  *                                     [0,n) hold PhiX(t,s), [n,n+p) PhiY(t,s), the rest zeros; block order `phi_layout`
  *   r_out    device [batch,T,n]       r_t = sum_{s<t} |PhiX(t,s)| w_s  (or the two-norm form with LTV_TUBE_ROW_2NORM)
+ *   flags    0 or any of LTV_TUBE_ROW_2NORM, LTV_OBSERVER_SHIFTED_GAIN
  * The same time-parallel scan as above runs over the closed-loop matrices; PhiY rides along as p extra columns of
  * the right operand ([PhiX | PhiY](t,s) = PhiX(t,mid) [PhiX | PhiY](mid,s)), so it costs (n+p)/n of the products and
  * no second pass over Phi.  Level 0 forms Abar_s while A_s streams through, and PhiY(s+1,s) = Abar_s Lt_s.
@@ -245,6 +256,19 @@ LTV_API int ltv_scan_pipeline_host(const float* A_host, const float* B_host, con
                            int batch, int T, int n, int m,
                            void* workspace, size_t workspace_bytes, void* cuda_stream,
                            float** phi_device_out);
+
+/* Process-wide options: plain ints, thread-safe, each with a sound default; none changes a result beyond the order of
+ * floating-point sums.  The library reads NO environment variables (developer builds made with -DLTV_TUNING aside).
+ *   LTV_OPT_VECTOR_CLUSTER   CTAs per batch item (thread-block cluster size) of the rollout and adjoint kernels:
+ *                            0 (default) = chosen by an occupancy / bandwidth model, 1 .. 16 = forced (falls back to 1
+ *                            if that cluster cannot be placed).  Used by the tests to cover every cluster size.
+ *   LTV_OPT_PIPELINE_CHUNKS  number of batch chunks ltv_scan_pipeline_host overlaps upload and compute over:
+ *                            1 .. 16, default 4 (1 = no overlap).
+ * ltv_set_option returns LTV_ERR_BAD_DIM for an unknown option or a value out of range; ltv_get_option returns -1 for
+ * an unknown option. */
+enum { LTV_OPT_VECTOR_CLUSTER = 0, LTV_OPT_PIPELINE_CHUNKS = 1, LTV_OPT_COUNT = 2 };
+LTV_API int ltv_set_option(int option, int value);
+LTV_API int ltv_get_option(int option);
 
 /* Human-readable name of a status code (static storage). */
 LTV_API const char* ltv_status_string(int status);

@@ -127,10 +127,13 @@ def system_response(A):
     return np.stack([system_response_item(A[b]) for b in range(A.shape[0])])
 
 
-def observer_response_item(A, Lt, C):
+def observer_response_item(A, Lt, C, shifted_gain=False):
     """Closed-loop observer propagation of one item, eq.(14) in the paper's own order: for every
     k, PhiX(k,k) = I and, for j = k-1 down to 0, PhiX(k,j) = PhiX(k,j+1) (A_j + L_j^T C_j) (RIGHT multiplication),
-    PhiY(k,j) = PhiX(k,j) L_j^T.  Lt[j] = L_j^T [n,p], C[j] [p,n].  Returns packed PhiX[P,n,n], PhiY[P,n,p]."""
+    PhiY(k,j) = PhiX(k,j) L_j^T.  Lt[j] = L_j^T [n,p], C[j] [p,n].  Returns packed PhiX[P,n,n], PhiY[P,n,p].
+    shifted_gain=True returns instead the Phihat^y that satisfies the second achievability identity of (12c)
+     and enters the assembly (15): PhiY(k,j) = PhiX(k,j) Lt[j-1] for j >= 1, PhiY(k,0) = 0 (DESIGN.md
+    readings q20, q21; pinned by test_observer_achievability_identity_of_12c)."""
     A, Lt, C = _f64(A), _f64(Lt), _f64(C)
     T, n, _ = A.shape
     p = Lt.shape[-1]
@@ -141,12 +144,15 @@ def observer_response_item(A, Lt, C):
         for j in range(k - 1, -1, -1):
             X = X @ (A[j] + Lt[j] @ C[j])
             PhiX[packed_index(k, j)] = X
-            PhiY[packed_index(k, j)] = X @ Lt[j]
+            if not shifted_gain:
+                PhiY[packed_index(k, j)] = X @ Lt[j]
+            else:
+                PhiY[packed_index(k, j)] = X @ Lt[j - 1] if j >= 1 else np.zeros((n, p))
     return PhiX, PhiY
 
 
-def observer_response(A, Lt, C):
-    out = [observer_response_item(A[b], Lt[b], C[b]) for b in range(A.shape[0])]
+def observer_response(A, Lt, C, shifted_gain=False):
+    out = [observer_response_item(A[b], Lt[b], C[b], shifted_gain) for b in range(A.shape[0])]
     return np.stack([o[0] for o in out]), np.stack([o[1] for o in out])
 
 

@@ -23,15 +23,17 @@ LTV_OP_KALMAN_GAINS = 6
 LTV_OP_CONSTRAINT_TIGHTENING = 7
 LTV_OP_OUTPUT_FEEDBACK = 8
 LTV_TUBE_ROW_2NORM = 1
+LTV_OBSERVER_SHIFTED_GAIN = 2
 LTV_KALMAN_SCAN, LTV_KALMAN_RECURSION = 1, 2
 LTV_PHI_COLUMN_PACKED = 0
+LTV_OPT_VECTOR_CLUSTER, LTV_OPT_PIPELINE_CHUNKS = 0, 1
 
 EXPORTS = (
     "ltv_phi_block_index", "ltv_scan_workspace_bytes", "ltv_scan_rollout", "ltv_scan_system_response_tube",
     "ltv_scan_adjoint", "ltv_scan_pipeline_host", "ltv_status_string", "ltv_last_cuda_error", "ltv_version",
     "ltv_launch_count", "ltv_profile_enable", "ltv_profile_collect", "ltv_scan_observer_response",
     "ltv_observer_row_floats", "ltv_scan_kalman_gains",
-    "ltv_scan_constraint_tightening", "ltv_scan_output_feedback_response",
+    "ltv_scan_constraint_tightening", "ltv_scan_output_feedback_response", "ltv_set_option", "ltv_get_option",
 )
 
 
@@ -70,6 +72,10 @@ def _load() -> ctypes.CDLL:
     L.ltv_scan_output_feedback_response.argtypes = [fp] * 10 + [i] * 5 + [ctypes.c_uint, vp, sz, vp]
     L.ltv_observer_row_floats.restype = i
     L.ltv_observer_row_floats.argtypes = [i, i]
+    L.ltv_set_option.restype = i
+    L.ltv_set_option.argtypes = [i, i]
+    L.ltv_get_option.restype = i
+    L.ltv_get_option.argtypes = [i]
     L.ltv_status_string.restype = ctypes.c_char_p
     L.ltv_status_string.argtypes = [i]
     L.ltv_last_cuda_error.restype = i
@@ -109,6 +115,16 @@ def ltv_phi_block_index(T: int, t: int, s: int) -> int:
 
 def ltv_scan_workspace_bytes(op: int, batch: int, T: int, n: int, m: int) -> int:
     return int(lib.ltv_scan_workspace_bytes(op, batch, T, n, m))
+
+
+def ltv_set_option(option: int, value: int) -> None:
+    st = lib.ltv_set_option(option, value)
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_set_option")
+
+
+def ltv_get_option(option: int) -> int:
+    return int(lib.ltv_get_option(option))
 
 
 def ltv_launch_count() -> int:
@@ -175,9 +191,11 @@ def ltv_observer_row_floats(n, p):
     return int(lib.ltv_observer_row_floats(n, p))
 
 
-def ltv_scan_observer_response(A, Lt, C, w, phi_out=None, r_out=None, workspace=None, two_norm=False):
+def ltv_scan_observer_response(A, Lt, C, w, phi_out=None, r_out=None, workspace=None, two_norm=False, shifted_gain=False):
     """Closed-loop observer propagation (eq.(14)): returns (phi[batch,P,n,nc] COLUMN_PACKED with PhiX in columns
-    [0,n) and PhiY in [n,n+p) of every row, r[batch,T,n]).  Lt[batch,T,n,p] = L_j^T, C[batch,T,p,n]."""
+    [0,n) and PhiY in [n,n+p) of every row, r[batch,T,n]).  Lt[batch,T,n,p] (Lt_j closes the loop around A_j),
+    C[batch,T,p,n].  shifted_gain=True: PhiY(t,s) = PhiX(t,s) Lt_{s-1} (the Phihat^y of (12c)/(15)) instead of the
+    printed form of (14), PhiX(t,s) Lt_s."""
     batch, T, n, _ = A.shape
     p = Lt.shape[-1]
     P = T * (T - 1) // 2
@@ -193,7 +211,8 @@ def ltv_scan_observer_response(A, Lt, C, w, phi_out=None, r_out=None, workspace=
     if workspace is None:
         workspace = torch.empty(max(need, 16), device=A.device, dtype=torch.uint8)
     st = lib.ltv_scan_observer_response(_ptr(A), _ptr(Lt), _ptr(C), _ptr(w), _ptr(phi_out), _ptr(r_out), batch, T, n, p,
-                                        LTV_PHI_COLUMN_PACKED, LTV_TUBE_ROW_2NORM if two_norm else 0,
+                                        LTV_PHI_COLUMN_PACKED,
+                                        (LTV_TUBE_ROW_2NORM if two_norm else 0) | (LTV_OBSERVER_SHIFTED_GAIN if shifted_gain else 0),
                                         _ptr(workspace), workspace.numel(), _stream())
     if st != LTV_OK:
         raise LtvError(st, "ltv_scan_observer_response")

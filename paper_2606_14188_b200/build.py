@@ -26,19 +26,44 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found: libltvscan.so cannot be built (there is no CPU fallback)")
 
 
+STAMP = LIB + ".srchash"
+
+
+def source_hash() -> str:
+    """sha256 over the content of every file the library is built from (csrc/*, include/ltv_scan.h), this script, the nvcc
+    flags and the nvcc version.  Stored beside the .so at build time: a pushed binary whose sources have since changed is
+    rebuilt whatever the file times say."""
+    import hashlib
+
+    h = hashlib.sha256()
+    deps = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC))
+    deps += [os.path.normpath(os.path.join(HERE, "..", "include", "ltv_scan.h")), os.path.abspath(__file__)]
+    for d in deps:
+        h.update(os.path.basename(d).encode() + b"\0")
+        with open(d, "rb") as f:
+            h.update(f.read())
+    h.update(" ".join(NVCC_FLAGS + SOURCES).encode())
+    h.update(os.environ.get("LTV_SCAN_NVCC_EXTRA", "").encode())
+    try:
+        h.update(subprocess.run([_nvcc(), "--version"], capture_output=True, text=True).stdout.encode())
+    except Exception:
+        pass
+    return h.hexdigest()
+
+
 def _stale() -> bool:
-    if not os.path.exists(LIB):
+    if not (os.path.exists(LIB) and os.path.exists(STAMP)):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
-    deps += [os.path.join(HERE, "..", "include", "ltv_scan.h"), os.path.abspath(__file__)]
-    return any(os.path.getmtime(d) > t for d in deps)
+    with open(STAMP) as f:
+        return f.read().strip() != source_hash()
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Build the shared library if any source is newer than it; returns its path."""
+    """Build the shared library unless the one in place was built from exactly these sources and flags (content hash,
+    not file times); returns its path."""
     if not force and not _stale():
         return LIB
+    want = source_hash()
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     nvcc = _nvcc()
@@ -61,6 +86,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [nvcc, "-shared", "-cudart", "static", "-o", LIB + ".tmp", *objs, "-Xlinker", "--exclude-libs,ALL"]
     subprocess.run(cmd, check=True)
     os.replace(LIB + ".tmp", LIB)
+    with open(STAMP, "w") as f:
+        f.write(want + "\n")
     return LIB
 
 

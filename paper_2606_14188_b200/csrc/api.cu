@@ -15,15 +15,25 @@ namespace ltv {
 static thread_local int g_last_cuda_error = 0;
 static std::atomic<unsigned long long> g_launches{0};
 
+// Developer overrides LTV_SCAN_<name> exist only in builds made with -DLTV_TUNING (kernel experiments: tile shape, forced
+// code paths).  The product build ignores the environment: its only knobs are the documented ltv_set_option values.
 int env_int(const char* name, int dflt) {
+#ifdef LTV_TUNING
   char key[64] = "LTV_SCAN_";
   std::strncat(key, name, sizeof(key) - std::strlen(key) - 1);
   const char* v = std::getenv(key);
   return (v && *v) ? std::atoi(v) : dflt;
+#else
+  (void)name;
+  return dflt;
+#endif
 }
 
+static std::atomic<int> g_options[LTV_OPT_COUNT] = {{0}, {4}};
+int option(int which) { return g_options[which].load(std::memory_order_relaxed); }
+
 int pick_cluster_model(int batch, int n, const int* max_active) {
-  const int forced = env_int("CLUSTER", 0);
+  const int forced = option(LTV_OPT_VECTOR_CLUSTER);
   if (forced >= 1 && forced <= 16 && max_active[forced] > 0) return forced;
   const double sm_gbs = 70.0, dev_gbs = 6500.0;
   int best = 1;
@@ -76,7 +86,7 @@ void query_max_active_clusters(const void* kernel, int threads, size_t smem, int
 namespace {
 struct ProfState {
   std::mutex mu;
-  bool on = false;
+  std::atomic<bool> on{false};
   std::vector<cudaEvent_t> beg, end;
   std::vector<int> cls;
   size_t used = 0;
@@ -87,10 +97,11 @@ ProfState& prof() {
 }
 }  // namespace
 
-ProfScope::ProfScope(int cls_, cudaStream_t s) : slot(-1), stream(s) {
+ProfScope::ProfScope(int cls_, cudaStream_t s) : slot(-1), stream(s), end_event(nullptr) {
   ProfState& p = prof();
-  if (!p.on) return;
+  if (!p.on.load(std::memory_order_acquire)) return;
   std::lock_guard<std::mutex> lk(p.mu);
+  if (!p.on.load(std::memory_order_relaxed)) return;
   if (p.used == p.beg.size()) {
     cudaEvent_t a, b;
     if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
@@ -100,10 +111,11 @@ ProfScope::ProfScope(int cls_, cudaStream_t s) : slot(-1), stream(s) {
   }
   slot = static_cast<int>(p.used++);
   p.cls[slot] = cls_;
+  end_event = p.end[slot];   // the handle is captured under the lock: the vectors may be reallocated by other threads
   cudaEventRecord(p.beg[slot], stream);
 }
 ProfScope::~ProfScope() {
-  if (slot >= 0) cudaEventRecord(prof().end[slot], stream);
+  if (slot >= 0) cudaEventRecord(static_cast<cudaEvent_t>(end_event), stream);
 }
 
 static int fail_cuda(cudaError_t e) {
@@ -111,6 +123,9 @@ static int fail_cuda(cudaError_t e) {
   cudaGetLastError();  // clear the sticky-free error state of the runtime
   return LTV_ERR_CUDA;
 }
+
+// several kernels of the NEXT calls map the batch (or batch x steps) onto gridDim.y / gridDim.z (<= 65535)
+static bool grid_yz_overflow(long long v) { return v > 65535; }
 
 static bool misaligned(const void* p) { return p && (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 
@@ -279,7 +294,8 @@ int ltv_scan_observer_response(const float* A, const float* Lt, const float* C, 
   if (st != LTV_OK) return st;
   if (p < 1) return LTV_ERR_BAD_DIM;
   if (p > 32) return LTV_ERR_UNSUPPORTED_SHAPE;
-  if (phi_layout != LTV_PHI_COLUMN_PACKED || (flags & ~static_cast<unsigned>(LTV_TUBE_ROW_2NORM)) != 0) return LTV_ERR_BAD_DIM;
+  if (phi_layout != LTV_PHI_COLUMN_PACKED || (flags & ~static_cast<unsigned>(LTV_TUBE_ROW_2NORM | LTV_OBSERVER_SHIFTED_GAIN)) != 0)
+    return LTV_ERR_BAD_DIM;
   const int nc = n + ((p + 3) & ~3);
   if (static_cast<long long>(batch) * T * (T - 1) / 2 * n * nc >= (1ll << 40)) return LTV_ERR_UNSUPPORTED_SHAPE;
   if (misaligned(A) || misaligned(Lt) || misaligned(C) || misaligned(w) || misaligned(phi_out) || misaligned(r_out) ||
@@ -295,6 +311,7 @@ int ltv_scan_observer_response(const float* A, const float* Lt, const float* C, 
   a.Lt = Lt;
   a.C = C;
   a.p = p;
+  a.yshift = (flags & LTV_OBSERVER_SHIFTED_GAIN) ? 1 : 0;
   if (p > 8) a.Ltt = reinterpret_cast<float*>(static_cast<char*>(workspace) + phi_part_bytes(batch, T, n, nc));
   unsigned long long l = 0;
   cudaError_t e = launch_phi_tube(a, static_cast<cudaStream_t>(cuda_stream), &l);
@@ -311,6 +328,8 @@ int ltv_scan_kalman_gains(const float* A, const float* C, const float* e, const 
   if (p < 1 || (flags & ~3u) != 0 || flags == 3u) return LTV_ERR_BAD_DIM;
   if (p > 32) return LTV_ERR_UNSUPPORTED_SHAPE;
   if ((flags & LTV_KALMAN_SCAN) && !riccati_scan_supported(n)) return LTV_ERR_UNSUPPORTED_SHAPE;
+  if (grid_yz_overflow(batch) || ((flags & LTV_KALMAN_SCAN) && grid_yz_overflow(static_cast<long long>(batch) * (T + 1))))
+    return LTV_ERR_UNSUPPORTED_SHAPE;
   if (static_cast<long long>(batch) * (T + 1) * n >= (1ll << 31)) return LTV_ERR_UNSUPPORTED_SHAPE;
   if (misaligned(A) || misaligned(C) || misaligned(e) || misaligned(f) || misaligned(Pi0) || misaligned(Lt_out) ||
       misaligned(Pi_out) || misaligned(workspace))
@@ -334,7 +353,7 @@ int ltv_scan_constraint_tightening(const float* A, const float* w, const float* 
   int st = check_dims(batch, T, n, 0);
   if (st != LTV_OK) return st;
   if (nc < 1 || flags != 0) return LTV_ERR_BAD_DIM;
-  if (static_cast<long long>(batch) * T * nc >= (1ll << 31) / n) return LTV_ERR_UNSUPPORTED_SHAPE;
+  if (static_cast<long long>(batch) * T * nc >= (1ll << 31) / n || grid_yz_overflow(batch)) return LTV_ERR_UNSUPPORTED_SHAPE;
   if (misaligned(A) || misaligned(w) || misaligned(Hc) || misaligned(sigma_out) || misaligned(workspace))
     return LTV_ERR_ALIGNMENT;
   if (workspace_bytes < constraint_workspace_bytes(batch, T, n, nc)) return LTV_ERR_WORKSPACE_TOO_SMALL;
@@ -357,7 +376,7 @@ int ltv_scan_output_feedback_response(const float* A, const float* B, const floa
   int st = check_dims(batch, T, n, m);
   if (st != LTV_OK) return st;
   if (m < 1 || p < 1 || flags != 0) return LTV_ERR_BAD_DIM;
-  if (p > 32) return LTV_ERR_UNSUPPORTED_SHAPE;
+  if (p > 32 || grid_yz_overflow(batch)) return LTV_ERR_UNSUPPORTED_SHAPE;
   st = check_dims(batch, T, 2 * n, 0);   // the scan runs on 2n states
   if (st != LTV_OK) return st;
   if (misaligned(A) || misaligned(B) || misaligned(Kfb) || misaligned(Lt) || misaligned(C) || misaligned(w) ||
@@ -414,22 +433,21 @@ int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float
   if (phi_device_out) *phi_device_out = with_phi ? dphi : nullptr;
 
   cudaError_t e;
-#define LTV_H2D(dst, src, floats)                                                                   \
-  if ((src) && (floats) > 0) {                                                                      \
-    e = cudaMemcpyAsync((dst), (src), (floats) * sizeof(float), cudaMemcpyHostToDevice, s);         \
-    if (e != cudaSuccess) return fail_cuda(e);                                                      \
-  }
 #define LTV_D2H(dst, src, floats)                                                                   \
   if ((dst) && (floats) > 0) {                                                                      \
     e = cudaMemcpyAsync((dst), (src), (floats) * sizeof(float), cudaMemcpyDeviceToHost, s);         \
-    if (e != cudaSuccess) return fail_cuda(e);                                                      \
+    if (e != cudaSuccess) {                                                                         \
+      cudaStreamSynchronize(cs);                                                                    \
+      cleanup();                                                                                    \
+      return fail_cuda(e);                                                                          \
+    }                                                                                               \
   }
   // Chunks of the batch are pipelined: an internal copy stream uploads chunk i+1 while chunk i is computed on
   // the caller's stream (items are independent; the upload, 97 % of it A, is the longer leg at PCIe rates).
   // Chunks are multiples of 4 items so that every slice stays 16-byte aligned.
   int cb = batch;
-  if (batch >= 8 && env_int("E2E_CHUNKS", 4) > 1) {
-    const int want = env_int("E2E_CHUNKS", 4);
+  if (batch >= 8 && option(LTV_OPT_PIPELINE_CHUNKS) > 1) {
+    const int want = option(LTV_OPT_PIPELINE_CHUNKS);
     cb = ((batch + want - 1) / want + 3) & ~3;
   }
   const int nchunk = (batch + cb - 1) / cb;
@@ -501,7 +519,6 @@ int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float
   if (e != cudaSuccess) return fail_cuda(e);
   return LTV_OK;
 #undef LTV_TRY
-#undef LTV_H2D
 #undef LTV_D2H
 }
 
@@ -522,8 +539,8 @@ const char* ltv_status_string(int status) {
 int ltv_profile_enable(int on) {
   ProfState& p = prof();
   std::lock_guard<std::mutex> lk(p.mu);
-  p.on = on != 0;
-  p.used = 0;
+  p.on.store(on != 0, std::memory_order_release);
+  p.used = 0;   // scopes still open on other threads keep their (already captured) events; their record is dropped
   return LTV_OK;
 }
 
@@ -547,6 +564,23 @@ int ltv_profile_collect(double* ms_by_class, unsigned long long* launches_by_cla
   p.used = 0;
   return LTV_OK;
 }
+
+int ltv_set_option(int opt, int value) {
+  switch (opt) {
+    case LTV_OPT_VECTOR_CLUSTER:
+      if (value < 0 || value > 16) return LTV_ERR_BAD_DIM;
+      break;
+    case LTV_OPT_PIPELINE_CHUNKS:
+      if (value < 1 || value > 16) return LTV_ERR_BAD_DIM;
+      break;
+    default:
+      return LTV_ERR_BAD_DIM;
+  }
+  g_options[opt].store(value, std::memory_order_relaxed);
+  return LTV_OK;
+}
+
+int ltv_get_option(int opt) { return (opt >= 0 && opt < LTV_OPT_COUNT) ? option(opt) : -1; }
 
 int ltv_last_cuda_error(void) { return g_last_cuda_error; }
 int ltv_version(void) { return 100; }

@@ -36,6 +36,7 @@ struct PhiArgs {
   const float* C = nullptr;   // [batch,T,p,n]
   int p = 0;
   float* Ltt = nullptr;       // workspace [batch,T,nc-n,n]: the gains transposed (p > 8 only)
+  int yshift = 0;             // 1: PhiY(t,s) = PhiX(t,s) Lt_{s-1} (zero for s = 0): the Phihat^y of (12c)/(15)
 };
 // n-tile width the Phi path uses for this n (decides the size of `part`) and whether it is the tcgen05 path
 int phi_tile_n(int n, int nc);
@@ -85,8 +86,10 @@ cudaError_t launch_output_feedback(const OfbArgs& a, cudaStream_t stream, unsign
 int pick_cluster_model(int batch, int n, const int* max_active);
 // fills max_active[1..16] for `kernel` (any __global__ function pointer) at the given block size / dynamic smem
 void query_max_active_clusters(const void* kernel, int threads, size_t smem, int* max_active);
-// environment override for experiments: LTV_SCAN_<name>=<int>; returns `dflt` if unset
+// developer override LTV_SCAN_<name>=<int>, compiled in only with -DLTV_TUNING; the product build returns `dflt`
 int env_int(const char* name, int dflt);
+// value of a documented ltv_set_option knob (include/ltv_scan.h)
+int option(int which);
 
 // optional per-kernel timing (ltv_profile_enable): CUDA events recorded on the launch stream around a kernel
 enum ProfClass { kProfRollout = 0, kProfAdjoint, kProfPhiLevel0, kProfPhiCombineTc, kProfPhiCombineSimt,
@@ -96,6 +99,7 @@ struct ProfScope {
   ~ProfScope();
   int slot;
   cudaStream_t stream;
+  void* end_event;   // cudaEvent_t captured at construction
 };
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }

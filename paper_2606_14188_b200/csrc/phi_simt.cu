@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(256) phi_obs_level0_wide_kernel(const float* _
                                                                   const float* __restrict__ Ltt, const float* __restrict__ C,
                                                                   const float* __restrict__ w, float* __restrict__ phi,
                                                                   float* __restrict__ part, int batch, int T, int n, int nc,
-                                                                  int p, int NT, int mode) {
+                                                                  int p, int NT, int mode, int yshift) {
   constexpr int PP = 8 * PG;
   const int pp = nc - n;
   const int P = T * (T - 1) / 2;
@@ -123,7 +123,10 @@ __global__ void __launch_bounds__(256) phi_obs_level0_wide_kernel(const float* _
     const size_t bt = static_cast<size_t>(b) * T + s;
     const float4* wv = reinterpret_cast<const float4*>(w + bt * n);
     const float4* Cs = reinterpret_cast<const float4*>(C + bt * p * n);
-    const float4* Lts = reinterpret_cast<const float4*>(Ltt + bt * pp * n);
+    // PhiY columns: gain of step s (eq.(14) as printed) or, with yshift, of step s - 1 (the Phihat^y of (12c)/(15);
+    // no such term for s = 0: the products are formed on valid memory and scaled by zero)
+    const bool ynone = yshift && s == 0;
+    const float4* Lts = reinterpret_cast<const float4*>(Ltt + (bt - ((yshift && s > 0) ? 1 : 0)) * pp * n);
     const size_t q = static_cast<size_t>(b) * P + phi_colbase(T, s);
     const float4* src[ROWS];
     const float* lrow[ROWS];
@@ -181,7 +184,7 @@ __global__ void __launch_bounds__(256) phi_obs_level0_wide_kernel(const float* _
         if (k < pp) {
 #pragma unroll
           for (int o = 16; o > 0; o >>= 1) y[r][k] += __shfl_xor_sync(0xffffffffu, y[r][k], o);
-          if (lane == (k & 31) && i + r < n) phi[(q * n + i + r) * nc + n + k] = y[r][k];
+          if (lane == (k & 31) && i + r < n) phi[(q * n + i + r) * nc + n + k] = ynone ? 0.f : y[r][k];
         }
       }
       if (lane == 0 && i + r < n)
@@ -293,7 +296,8 @@ template <int PP>
 __global__ void __launch_bounds__(256, 2) phi_obs_level0_fused_kernel(const float* __restrict__ A, const float* __restrict__ Lt,
                                                                    const float* __restrict__ C, const float* __restrict__ w,
                                                                    float* __restrict__ phi, float* __restrict__ part,
-                                                                   int batch, int T, int n, int nc, int NT, int mode) {
+                                                                   int batch, int T, int n, int nc, int NT, int mode,
+                                                                   int yshift) {
   constexpr int p = PP;   // exact number of measurement rows: every loop below unrolls, Lt is read as float4
   const int P = T * (T - 1) / 2;
   const int n4 = n >> 2;
@@ -310,6 +314,9 @@ __global__ void __launch_bounds__(256, 2) phi_obs_level0_fused_kernel(const floa
     const float4* wv = reinterpret_cast<const float4*>(w + bt * n);
     const float4* Cs = reinterpret_cast<const float4*>(C + bt * p * n);
     const float* Ls = Lt + bt * n * p;
+    // gain of the PhiY columns: step s (eq.(14) as printed) or, with yshift, step s - 1 (zero block for s = 0)
+    const bool ynone = yshift && s == 0;
+    const float* Lys = Ls - ((yshift && s > 0) ? static_cast<size_t>(n) * p : 0);
     const size_t q = static_cast<size_t>(b) * P + phi_colbase(T, s);
     float* dst = phi + (q * n + i) * nc;
     float lr[4][PP];   // Lt_s[i + r][k]: the gains of this unit's own rows
@@ -344,7 +351,7 @@ __global__ void __launch_bounds__(256, 2) phi_obs_level0_fused_kernel(const floa
                    (tube_term(a[r].z, ww.z, mode) + tube_term(a[r].w, ww.w, mode));
       }
       // rows 4c .. 4c+3 of Lt_s: 4p contiguous floats
-      const float4* lj4 = reinterpret_cast<const float4*>(Ls + static_cast<size_t>(4 * c) * p);
+      const float4* lj4 = reinterpret_cast<const float4*>(Lys + static_cast<size_t>(4 * c) * p);
       float lt[4 * PP];   // lt[jj * p + k] = Lt_s[4c + jj][k]
 #pragma unroll
       for (int v = 0; v < PP; ++v) {
@@ -377,7 +384,7 @@ __global__ void __launch_bounds__(256, 2) phi_obs_level0_fused_kernel(const floa
         float v = y[0][k];
 #pragma unroll
         for (int rr = 1; rr < 4; ++rr) v = (r == rr) ? y[rr][k] : v;
-        prow[k] = v;
+        prow[k] = ynone ? 0.f : v;
       }
       for (int k = p; k < nc - n; ++k) prow[k] = 0.f;
       for (int e = 0; e < NT; ++e) part[(q * NT + e) * n + i + r] = (e == 0) ? tr : 0.f;
@@ -400,7 +407,7 @@ cudaError_t launch_phi_obs_level0(const PhiArgs& a, int NT, int num_sms, cudaStr
   case PV:                                                                                                     \
     phi_obs_level0_fused_kernel<PV><<<static_cast<unsigned>(ub), 256, 0, stream>>>(a.A, a.Lt, a.C, a.w, a.phi, a.part, \
                                                                                    a.batch, a.T, a.n, a.nc, NT,   \
-                                                                                   a.tube_mode);                \
+                                                                                   a.tube_mode, a.yshift);      \
     break;
     switch (a.p) {
       LTV_OBS_CASE(1) LTV_OBS_CASE(2) LTV_OBS_CASE(3) LTV_OBS_CASE(4)
@@ -423,7 +430,7 @@ cudaError_t launch_phi_obs_level0(const PhiArgs& a, int NT, int num_sms, cudaStr
 #define LTV_OBSW_CASE(PGV)                                                                                         \
   case PGV:                                                                                                        \
     phi_obs_level0_wide_kernel<PGV, kRows><<<static_cast<unsigned>(ub), 256, 0, stream>>>(                          \
-        a.A, a.Lt, a.Ltt, a.C, a.w, a.phi, a.part, a.batch, a.T, a.n, a.nc, a.p, NT, a.tube_mode);                  \
+        a.A, a.Lt, a.Ltt, a.C, a.w, a.phi, a.part, a.batch, a.T, a.n, a.nc, a.p, NT, a.tube_mode, a.yshift);        \
     break;
   switch ((pp + 7) / 8) {
     LTV_OBSW_CASE(2) LTV_OBSW_CASE(3) LTV_OBSW_CASE(4)

@@ -71,9 +71,6 @@ struct TcParams {
   PhiGeom g;
   int stages;
   int tube_mode;              // 0: |d| w, 1: (d w)^2 (row-wise two-norm tube; the finalise kernel takes the root)
-  unsigned long long* trace;  // experiments only (DBG & 4096): per-role clock64 log of CTA 0
-  int trace_cap;
-  int dbg;                    // experiments only: selects a DBG instantiation (LTV_SCAN_TC_DBG)
 };
 
 struct TcMaps {
@@ -117,10 +114,7 @@ struct TcShape {
   static_assert(NT % (16 * NCTA) == 0, "UMMA N granularity");
 };
 
-// DBG = compile-time knock-out mask (experiments only, -DLTV_TC_EXPERIMENTS; production is DBG = 0):
-// 1 no stores, 2 no R split, 4 no L split, 16 one MMA of three, 128 no TMEM stores, 512 no tube FMAs,
-// 1024 no proxy fence, 4096 clock traces of CTA 0.
-template <int NCH, bool PAIR, int DBG, int MODE>
+template <int NCH, bool PAIR, int MODE>
 __global__ void __launch_bounds__(kTcThreads, 1)
 phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL,
                       const __grid_constant__ CUtensorMap mapR, const __grid_constant__ CUtensorMap mapO,
@@ -142,9 +136,6 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
   const int nkb_tot = (MODE == 2) ? 2 * nkb : nkb;
   const long long unit = PAIR ? (blockIdx.x >> 1) : blockIdx.x;
   const long long nunits = PAIR ? (gridDim.x >> 1) : gridDim.x;
-#define LTV_TRACE(role, idx, ev)                                                                  \
-  if ((DBG & 4096) && blockIdx.x == 0 && lane == 0 && static_cast<int>(idx) < p.trace_cap)        \
-    p.trace[(static_cast<size_t>(role) * p.trace_cap + (idx)) * 4 + (ev)] = clock64();
 
   uint8_t* lo_ring = smem + static_cast<size_t>(R) * kRawBytes;               // [kConvStages][kBBytes]
   uint8_t* stage_out = lo_ring + kConvStages * kBBytes;                        // [4 warps][32 rows x 128 B]
@@ -219,9 +210,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
         j0 = t.n_tile * NT + static_cast<int>(rank) * NH;
       }
       for (int kb = 0; kb < nkb_tot; ++kb, ++it) {
-        LTV_TRACE(0, it, 0)
         mbar_wait(&rempty[rs], eph);
-        LTV_TRACE(0, it, 1)
         uint8_t* sp = smem + static_cast<size_t>(rs) * kRawBytes;
         const bool second = (MODE == 2) && kb >= nkb;
         const int kc = (second ? kb - nkb : kb) * kKB;
@@ -247,15 +236,12 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
       uint32_t cph = 0;
       for (long long idx = unit; idx < g.total; idx += nunits, ++lt) {
         const uint32_t acc = lt & 1;
-        LTV_TRACE(1, it, 3)
         if (lt >= 2) mbar_wait(&tempty[acc], ((lt >> 1) - 1) & 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + acc * NT;
         for (int kb = 0; kb < nkb_tot; ++kb, ++it) {
-          LTV_TRACE(1, it, 0)
           mbar_wait(&conv[cs], cph);
           tc_fence_after();
-          LTV_TRACE(1, it, 1)
           const uint32_t sb_hi = smem_u32(smem + static_cast<size_t>(rs) * kRawBytes + kABytes);
           const uint32_t sb_lo = smem_u32(lo_ring + static_cast<size_t>(cs) * kBBytes);
           const uint32_t a_hi = tmem_base + kTmemA + cs * 64;   // raw fp32 bits: the MMA keeps the top 19
@@ -267,11 +253,9 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
               if (ks < nks) {
                 const uint64_t b_hi = umma_smem_desc(sb_hi + ks * 1024, 4096, 512, kUmmaSw128Base32);
                 const uint64_t b_lo = umma_smem_desc(sb_lo + ks * 1024, 4096, 512, kUmmaSw128Base32);
-                if (!(DBG & 16)) {
-                  umma_tf32_ts<PAIR>(d_tmem, a_lo + ks * 8, b_hi, idesc, (kb | ks) != 0);
-                  umma_tf32_ts<PAIR>(d_tmem, a_hi + ks * 8, b_lo, idesc, 1);
-                }
-                umma_tf32_ts<PAIR>(d_tmem, a_hi + ks * 8, b_hi, idesc, (DBG & 16) ? ((kb | ks) != 0) : 1);
+                umma_tf32_ts<PAIR>(d_tmem, a_lo + ks * 8, b_hi, idesc, (kb | ks) != 0);
+                umma_tf32_ts<PAIR>(d_tmem, a_hi + ks * 8, b_lo, idesc, 1);
+                umma_tf32_ts<PAIR>(d_tmem, a_hi + ks * 8, b_hi, idesc, 1);
               }
             }
             umma_commit_all<PAIR>(&rempty[rs]);
@@ -279,7 +263,6 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
             if (kb == nkb_tot - 1) umma_commit_all<PAIR>(&tfull[acc]);
           }
           __syncwarp();
-          LTV_TRACE(1, it, 2)
           if (++rs == R) rs = 0;
           if (++cs == kConvStages) { cs = 0; cph ^= 1; }
         }
@@ -300,31 +283,23 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
     for (long long idx = unit; idx < g.total; idx += nunits) {
       for (int kb = 0; kb < nkb_tot; ++kb, ++it) {
         if (static_cast<int>(it & 1) == grp) {
-          const int trole = 2 + grp;
-          if (q == 0) { LTV_TRACE(trole, it, 0) }
           mbar_wait(&full[rs], rph);
           const uint8_t* sp = smem + static_cast<size_t>(rs) * kRawBytes;
           // the raw tile is only read: load the L rows before waiting for the split ring slot
           uint32_t v[32];
-          if (!(DBG & 4)) {
 #pragma unroll
-            for (int c = 0; c < 8; ++c) {
-              const uint4 f = *reinterpret_cast<const uint4*>(sp + row * 128 + ((c ^ (row & 7)) << 4));
-              v[4 * c + 0] = f.x; v[4 * c + 1] = f.y; v[4 * c + 2] = f.z; v[4 * c + 3] = f.w;
-            }
+          for (int c = 0; c < 8; ++c) {
+            const uint4 f = *reinterpret_cast<const uint4*>(sp + row * 128 + ((c ^ (row & 7)) << 4));
+            v[4 * c + 0] = f.x; v[4 * c + 1] = f.y; v[4 * c + 2] = f.z; v[4 * c + 3] = f.w;
           }
-          if (q == 0) { LTV_TRACE(trole, it, 1) }
           mbar_wait(&cempty[cs], cph);
           tc_fence_after();
-          if (q == 0) { LTV_TRACE(trole, it, 2) }
           const uint32_t ta = tmem_base + (static_cast<uint32_t>(q * 32) << 16) + kTmemA + cs * 64;
-          if (!(DBG & 4)) {
-            if (!(DBG & 128)) tmem_st_32x32(ta, v);
+          tmem_st_32x32(ta, v);
 #pragma unroll
-            for (int e = 0; e < 32; ++e) v[e] = __float_as_uint(tf32_lo(__uint_as_float(v[e])));
-            if (!(DBG & 128)) tmem_st_32x32(ta + 32, v);
-          }
-          if (!(DBG & 2)) {
+          for (int e = 0; e < 32; ++e) v[e] = __float_as_uint(tf32_lo(__uint_as_float(v[e])));
+          tmem_st_32x32(ta + 32, v);
+          {
             const float4* br = reinterpret_cast<const float4*>(sp + kABytes);
             float4* bl = reinterpret_cast<float4*>(lo_ring + static_cast<size_t>(cs) * kBBytes);
 #pragma unroll
@@ -333,12 +308,11 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
               bl[gtid + 128 * i] = make_float4(tf32_lo(a.x), tf32_lo(a.y), tf32_lo(a.z), tf32_lo(a.w));
             }
           }
-          if (!(DBG & 128)) tmem_st_wait();
-          if (!(DBG & 1024)) fence_proxy_async_smem();
+          tmem_st_wait();
+          fence_proxy_async_smem();
           tc_fence_before();
           __syncwarp();
           if (lane == 0) arrive_leader(&conv[cs]);
-          if (q == 0) { LTV_TRACE(trole, it, 3) }
         }
         if (++rs == R) { rs = 0; rph ^= 1; }
         if (++cs == kConvStages) { cs = 0; cph ^= 1; }
@@ -352,7 +326,6 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
     const bool two_norm = p.tube_mode != 0;
     uint32_t lt = 0;
     for (long long idx = unit; idx < g.total; idx += nunits, ++lt) {
-      if (warp == 4) { LTV_TRACE(4, lt, 0) }
       const uint32_t acc = lt & 1;
       if (MODE == 1) {
         // ------------------------------------------------------------ batched GEMM epilogue (Kalman recursion)
@@ -439,7 +412,6 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
       const int row0 = static_cast<int>(qcol * n) + rbase;
       mbar_wait(&tfull[acc], (lt >> 1) & 1);
       tc_fence_after();
-      if (warp == 4) { LTV_TRACE(4, lt, 1) }
       const uint32_t taddr = tmem_base + (static_cast<uint32_t>(wq * 32) << 16) + acc * NT;
       float tube4[4] = {0.f, 0.f, 0.f, 0.f};
       uint32_t v[2][32];
@@ -449,7 +421,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
         uint32_t (&vc)[32] = v[cc & 1];
         tmem_ld_wait();
         if (cc + 1 < NCH) tmem_ld_32x32(taddr + (cc + 1) * 32, v[(cc + 1) & 1]);
-        if (MODE == 0 && !(DBG & 512)) {
+        if (MODE == 0) {
           const float4* w4 = reinterpret_cast<const float4*>(wb + cc * 32);
 #pragma unroll
           for (int e = 0; e < 8; ++e) {
@@ -462,7 +434,6 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
             tube4[3] += two_norm ? d3 * d3 : fabsf(d3);
           }
         }
-        if (DBG & 1) continue;
         const int jc = j0 + cc * 32;
         if (jc >= nc || rows_valid <= 0) continue;
         if (rows_valid >= 32) {
@@ -493,14 +464,12 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
       }
       tc_fence_before();
       __syncwarp();
-      if (warp == 4) { LTV_TRACE(4, lt, 2) }
       if (lane == 0) arrive_leader(&tempty[acc]);
       if (MODE == 0 && lane < rows_valid)
         p.part[((qcol + rho / n) * g.NT + t.n_tile) * n + rho % n] = (tube4[0] + tube4[1]) + (tube4[2] + tube4[3]);
     }
     if (lane == 0) tma_store_wait_all<0>();   // shared memory must outlive the last bulk store
   }
-#undef LTV_TRACE
   tc_fence_before();
   __syncthreads();
   if (PAIR) cluster_sync_all();   // the peer may still be reading this CTA's TMEM / shared memory through the pair MMA
@@ -510,8 +479,8 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
   }
 }
 
-template <int NCH, bool PAIR, int DBG, int MODE = 0>
-cudaError_t launch_tc_dbg(const TcParams& p, const TcMaps& maps, int num_sms, cudaStream_t stream) {
+template <int NCH, bool PAIR, int MODE>
+cudaError_t launch_tc(const TcParams& p, const TcMaps& maps, int num_sms, cudaStream_t stream) {
   using S = TcShape<NCH, PAIR>;
   TcParams q = p;
   int st = static_cast<int>((227u * 1024u - 1024u - S::kMisc - kConvStages * S::kBBytes) / S::kRawBytes);
@@ -519,7 +488,7 @@ cudaError_t launch_tc_dbg(const TcParams& p, const TcMaps& maps, int num_sms, cu
   if (st < 2) return cudaErrorInvalidConfiguration;
   q.stages = st;
   const uint32_t smem = 1024u + st * S::kRawBytes + kConvStages * S::kBBytes + S::kMisc;
-  auto kern = phi_combine_tc_kernel<NCH, PAIR, DBG, MODE>;
+  auto kern = phi_combine_tc_kernel<NCH, PAIR, MODE>;
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e != cudaSuccess) return e;
   const long long max_units = num_sms / S::NCTA;
@@ -540,35 +509,11 @@ cudaError_t launch_tc_dbg(const TcParams& p, const TcMaps& maps, int num_sms, cu
   return cudaLaunchKernelEx(&cfg, kern, q, maps.L, maps.R, maps.O, MODE == 2 ? maps.L2 : maps.L, MODE == 2 ? maps.R2 : maps.R);
 }
 
-template <int NCH, bool PAIR>
-cudaError_t launch_tc(const TcParams& p, const TcMaps& maps, int num_sms, cudaStream_t stream) {
-#ifdef LTV_TC_EXPERIMENTS
-  if (NCH == 5 && PAIR) {
-    switch (p.dbg) {
-#define LTV_DBG_CASE(D) case D: return launch_tc_dbg<5, true, D>(p, maps, num_sms, stream);
-      LTV_DBG_CASE(1) LTV_DBG_CASE(16) LTV_DBG_CASE(22) LTV_DBG_CASE(23) LTV_DBG_CASE(512) LTV_DBG_CASE(4096)
-#undef LTV_DBG_CASE
-      default: break;
-    }
-  }
-#endif
-  return launch_tc_dbg<NCH, PAIR, 0>(p, maps, num_sms, stream);
-}
-
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 }  // namespace
-
-#ifdef LTV_TC_EXPERIMENTS
-static unsigned long long* g_trace = nullptr;
-static int g_trace_cap = 0;
-extern "C" __attribute__((visibility("default"))) void ltv_debug_set_trace(void* ptr, int cap) {
-  g_trace = static_cast<unsigned long long*>(ptr);
-  g_trace_cap = cap;
-}
-#endif
 
 size_t phi_tc_maps_size() { return sizeof(TcMaps); }
 
@@ -614,12 +559,6 @@ cudaError_t launch_phi_combine_tc(const PhiArgs& a, int level, int nch, const vo
                                   cudaStream_t stream) {
   TcParams p{};
   p.phi = a.phi; p.w = a.w; p.part = a.part; p.tube_mode = a.tube_mode;
-  p.dbg = env_int("TC_DBG", 0);
-#ifdef LTV_TC_EXPERIMENTS
-  p.trace = g_trace;
-  p.trace_cap = g_trace_cap;
-  if (!p.trace) p.dbg &= ~4096;
-#endif
   const TcMaps& m = *static_cast<const TcMaps*>(maps);
   // CTA pairs (256-row tiles) when the level's stacked left operand is tall enough to fill them; the
   // single-CTA kernel (128-row tiles) on the low levels where 256-row tiles would be mostly padding
@@ -630,7 +569,7 @@ cudaError_t launch_phi_combine_tc(const PhiArgs& a, int level, int nch, const vo
   const bool pair = (mode == 1) || (mode == -1 && 2 * g2.total * 100 <= g1.total * 108);
   p.g = pair ? g2 : g1;
 #define LTV_NCH_CASE(N) \
-  case N: return pair ? launch_tc<N, true>(p, m, num_sms, stream) : launch_tc<N, false>(p, m, num_sms, stream);
+  case N: return pair ? launch_tc<N, true, 0>(p, m, num_sms, stream) : launch_tc<N, false, 0>(p, m, num_sms, stream);
   switch (nch) {
     LTV_NCH_CASE(2) LTV_NCH_CASE(3) LTV_NCH_CASE(4) LTV_NCH_CASE(5)
     default: return cudaErrorInvalidValue;
@@ -668,8 +607,8 @@ cudaError_t launch_phi_cross_tc(const PhiArgs& a, int level, int nch, const void
   const bool pair = 2 * g2.total * 100 <= g1.total * 108;
   p.g = pair ? g2 : g1;
 #define LTV_NCH_CASE(N_)                                                              \
-  case N_: return pair ? launch_tc_dbg<N_, true, 0, 2>(p, m, num_sms, stream)         \
-                       : launch_tc_dbg<N_, false, 0, 2>(p, m, num_sms, stream);
+  case N_: return pair ? launch_tc<N_, true, 2>(p, m, num_sms, stream)         \
+                       : launch_tc<N_, false, 2>(p, m, num_sms, stream);
   switch (nch) {
     LTV_NCH_CASE(2) LTV_NCH_CASE(3) LTV_NCH_CASE(4) LTV_NCH_CASE(5)
     default: return cudaErrorInvalidValue;
@@ -748,8 +687,8 @@ cudaError_t launch_bgemm_tc(const BatchedGemm& a, int nch, const void* maps, int
   p.gm.diag = a.diag; p.gm.diag_stride = a.diag_stride;
   p.g.total = static_cast<long long>(p.gm.Mt) * p.g.NT * a.count;
 #define LTV_NCH_CASE(N_)                                                              \
-  case N_: return pair ? launch_tc_dbg<N_, true, 0, 1>(p, m, num_sms, stream)         \
-                       : launch_tc_dbg<N_, false, 0, 1>(p, m, num_sms, stream);
+  case N_: return pair ? launch_tc<N_, true, 1>(p, m, num_sms, stream)         \
+                       : launch_tc<N_, false, 1>(p, m, num_sms, stream);
   switch (nch) {
     LTV_NCH_CASE(2) LTV_NCH_CASE(3) LTV_NCH_CASE(4) LTV_NCH_CASE(5)
     default: return cudaErrorInvalidValue;

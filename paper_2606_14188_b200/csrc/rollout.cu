@@ -23,20 +23,6 @@
 
 namespace ltv {
 
-#ifdef LTV_ROLL_TRACE
-static unsigned long long* g_roll_trace = nullptr;
-static int g_roll_trace_cap = 0;
-extern "C" __attribute__((visibility("default"))) void ltv_debug_set_roll_trace(void* ptr, int cap) {
-  g_roll_trace = static_cast<unsigned long long*>(ptr);
-  g_roll_trace_cap = cap;
-}
-#define LTV_RT(role, idx, ev)                                                                      \
-  if (p.trace && blockIdx.x == 0 && lane == 0 && static_cast<int>(idx) < p.trace_cap)              \
-    p.trace[(static_cast<size_t>(role) * p.trace_cap + (idx)) * 4 + (ev)] = clock64();
-#else
-#define LTV_RT(role, idx, ev)
-#endif
-
 namespace {
 
 constexpr int kConsWarps = 8;    // warps of one consumer group
@@ -72,8 +58,6 @@ struct RollParams {
   float* x_out;
   int batch, T, n, m;
   RollSmemPlan sp;
-  unsigned long long* trace;   // experiments only (LTV_ROLL_TRACE)
-  int trace_cap;
 };
 
 // Four per-lane partial sums (one per row) -> every lane of lane group g = lane / 8 holds the complete sum of
@@ -177,23 +161,18 @@ __global__ void __launch_bounds__(kRollThreads, 1) rollout_kernel(const RollPara
       const uint64_t pol = l2_policy_evict_first();
       int st = 0;
       uint32_t eph = 1;   // parity of empty[st] to wait for (the first pass over the ring does not block)
-      uint32_t pit = 0;
-      (void)pit;
       for (int item = cl; item < p.batch; item += ncl) {
         const size_t itemA = static_cast<size_t>(item) * T * n * n;
         for (int t = 0; t < T; ++t) {
           const float* At = p.A + itemA + (static_cast<size_t>(t) * n + r0) * n;
           for (int k = 0; k < nchunks; ++k) {
-            LTV_RT(0, pit, 0)
             mbar_wait(&empty[st], eph);
-            LTV_RT(0, pit, 1)
             const int rk = min(rc, rows - k * rc);
             const uint32_t bytes = static_cast<uint32_t>(rk) * n * 4u;
             mbar_arrive_expect_tx(&full[st], bytes);
             bulk_g2s(reinterpret_cast<uint8_t*>(ring) + static_cast<size_t>(st) * p.sp.stage_bytes,
                      At + static_cast<size_t>(k) * rc * n, bytes, &full[st], pol);
             if (++st == stages) { st = 0; eph ^= 1; }
-            ++pit;
           }
         }
       }
@@ -292,7 +271,6 @@ __global__ void __launch_bounds__(kRollThreads, 1) rollout_kernel(const RollPara
     for (int t = 0; t < T; ++t) {
       const uint32_t ht = h + t;
       const bool exch = t + 1 < T;   // x_T only goes to global memory
-      if (warp == 0) { LTV_RT(1, ht, 0) }
       float4 xq[QLMAX];
       if (t == 0) {
         const float4* x4 = reinterpret_cast<const float4*>(p.x0 + static_cast<size_t>(item) * n);
@@ -313,18 +291,14 @@ __global__ void __launch_bounds__(kRollThreads, 1) rollout_kernel(const RollPara
       }
       // every warp of every CTA has finished step t-1, so nobody reads xbuf[(ht+1) % 3] (= x_{t-2}) any more
       if (exch && threadIdx.x == 0) mbar_arrive_expect_tx(&xfull[(ht + 1) % 3], static_cast<uint32_t>(n) * 4u);
-      if (warp == 0) { LTV_RT(1, ht, 1) }
       mbar_wait(&bfull[bs], bph);
-      if (warp == 0) { LTV_RT(1, ht, 2) }
       float* xn = xbuf + ((ht + 1) % 3) * n;
       const float* bv = bvec + bs * p.sp.rows_max;
       uint64_t* xbar = &xfull[(ht + 1) % 3];
       float* xg = p.x_out + (static_cast<size_t>(item) * T + t) * n + r0;   // x_{t+1}, this CTA's rows
       for (int k = 0; k < nchunks; ++k, ++cidx) {
         if (static_cast<int>(cidx % kGroups) == grpid) {
-        if (warp == 0) { LTV_RT(2, cidx, 0) }
         mbar_wait(&full[st], fph);
-        if (warp == 0) { LTV_RT(2, cidx, 1) }
         const float* tile = reinterpret_cast<const float*>(reinterpret_cast<uint8_t*>(ring) +
                                                             static_cast<size_t>(st) * p.sp.stage_bytes);
         const int rk = min(rc, rows - k * rc);
@@ -336,9 +310,7 @@ __global__ void __launch_bounds__(kRollThreads, 1) rollout_kernel(const RollPara
             const int nval = min(4, rk - base);
             float acc[4] = {0.f, 0.f, 0.f, 0.f};
             rows_dot_n<QLMAX>(nval, tile, n, base, q0, q_end, ql, xq, acc);
-            if (warp == 0 && un == 0) { LTV_RT(3, cidx, 0) }
             const float v = reduce4_rows(acc, lane);
-            if (warp == 0 && un == 0) { LTV_RT(3, cidx, 1) }
             const int li0 = k * rc + base;
             if (nval == 4) {
               // all four sums into every lane: one 16-byte remote store per destination CTA, one 16-byte global store
@@ -356,7 +328,6 @@ __global__ void __launch_bounds__(kRollThreads, 1) rollout_kernel(const RollPara
                 for (int cta = sub; cta < C; cta += 8) st_async_remote_f32(xn + r0 + li, y, xbar, cta);
               if (sub == 0) xg[li] = y;
             }
-            if (warp == 0 && un == 0) { LTV_RT(3, cidx, 2) }
           }
         } else {
           // warp gw: its eighth of the columns of all (<= 4) rows of the chunk; partial sums meet in shared memory
@@ -388,13 +359,11 @@ __global__ void __launch_bounds__(kRollThreads, 1) rollout_kernel(const RollPara
           }
         }
         __syncwarp();
-        if (warp == 0) { LTV_RT(2, cidx, 2) }
         if (lane == 0) mbar_arrive(&empty[st]);
         }
         if (++st == stages) { st = 0; fph ^= 1; }
       }
       __syncwarp();
-      if (warp == 0) { LTV_RT(1, ht, 3) }
       if (lane == 0) mbar_arrive(&bempty[bs]);
       if (++bs == kBStages) { bs = 0; bph ^= 1; }
     }
@@ -463,10 +432,6 @@ cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t strea
   p.A = a.A; p.B = (a.m > 0) ? a.B : nullptr; p.c = a.c; p.x0 = a.x0; p.u = a.u; p.x_out = a.x_out;
   p.batch = a.batch; p.T = a.T; p.n = a.n; p.m = a.m;
   p.sp = plan_rollout(a.n, cluster, 1);
-#ifdef LTV_ROLL_TRACE
-  p.trace = g_roll_trace;
-  p.trace_cap = g_roll_trace_cap;
-#endif
   if (p.sp.stages < 2) return cudaErrorInvalidConfiguration;
 
   auto kern = p.sp.wide ? rollout_kernel<true> : rollout_kernel<false>;

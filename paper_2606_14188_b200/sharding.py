@@ -20,7 +20,18 @@ def shard_arrays(arrays: dict, rank: int, world: int) -> dict:
     if len(sizes) != 1:
         raise ValueError("arrays disagree on the batch size")
     b0, b1 = shard_range(sizes.pop(), rank, world)
-    return {k: (None if v is None else v[b0:b1]) for k, v in arrays.items()}
+    return {k: (None if v is None else _aligned(v[b0:b1])) for k, v in arrays.items()}
+
+
+def _aligned(view):
+    """The library wants 16-byte aligned device pointers (LTV_ERR_ALIGNMENT otherwise).  A slice that starts at an
+    arbitrary item of an array whose per-item size is not a multiple of 4 floats (u[T,m], f[T,p], grad_u with odd T m)
+    is not: such views are returned as fresh contiguous copies, all others as views."""
+    if hasattr(view, "data_ptr"):                      # torch tensor
+        return view if (view.data_ptr() % 16 == 0 and view.is_contiguous()) else view.clone(
+            memory_format=__import__("torch").contiguous_format)
+    ptr = view.__array_interface__["data"][0]          # numpy array
+    return view if (ptr % 16 == 0 and view.flags["C_CONTIGUOUS"]) else view.copy()
 
 
 def reduce_max(value: float, device=None) -> float:

@@ -221,17 +221,21 @@ def test_pipeline_host_chunked_and_without_phi(L):
 
 
 @pytest.mark.parametrize("cluster", [1, 2, 3, 5, 6, 7, 9, 10, 16])
-def test_vector_scans_any_cluster_size(L, cluster, monkeypatch):
-    """Rollout and adjoint give the same answer for every cluster size the model may pick (LTV_SCAN_CLUSTER
-    forces it): bands of 4-row multiples, last band blocks with fewer rows than m, clusters wider than 8."""
+def test_vector_scans_any_cluster_size(L, cluster):
+    """Rollout and adjoint give the same answer for every cluster size the model may pick (ltv_set_option
+    LTV_OPT_VECTOR_CLUSTER forces it): bands of 4-row multiples, last band blocks with fewer rows than m, clusters wider than 8."""
     import torch
 
     W = dense_random(2, 7, 640 if cluster == 16 else 300, 6, seed=40 + cluster)
     d = {k: torch.from_numpy(getattr(W, k)).cuda() for k in ("A", "B", "c", "x0", "u", "g")}
-    monkeypatch.setenv("LTV_SCAN_CLUSTER", str(cluster))
-    x = L.ltv_scan_rollout(d["A"], d["B"], d["c"], d["x0"], d["u"])
-    lam, gu, gx0 = L.ltv_scan_adjoint(d["A"], d["B"], d["g"])
-    torch.cuda.synchronize()
+    L.ltv_set_option(L.LTV_OPT_VECTOR_CLUSTER, cluster)
+    try:
+        assert L.ltv_get_option(L.LTV_OPT_VECTOR_CLUSTER) == cluster
+        x = L.ltv_scan_rollout(d["A"], d["B"], d["c"], d["x0"], d["u"])
+        lam, gu, gx0 = L.ltv_scan_adjoint(d["A"], d["B"], d["g"])
+        torch.cuda.synchronize()
+    finally:
+        L.ltv_set_option(L.LTV_OPT_VECTOR_CLUSTER, 0)
     rl, rgu, rgx = O.adjoint(W.A, W.B, W.g)
     _check(dict(x=x.cpu().numpy(), lam=lam.cpu().numpy(), grad_u=gu.cpu().numpy(), grad_x0=gx0.cpu().numpy()),
            dict(x=O.rollout(W.A, W.B, W.c, W.x0, W.u), lam=rl, grad_u=rgu, grad_x0=rgx))
@@ -338,6 +342,27 @@ def test_observer_response(L, n, T, batch, p):
     assert O.rel_err(r.cpu().numpy(), O.tube(Abar, W.w)) <= TOL
 
 
+@pytest.mark.parametrize("n,T,batch,p", [(48, 6, 2, 3), (300, 9, 2, 6), (132, 5, 2, 12)])
+def test_observer_response_shifted_gain(L, n, T, batch, p):
+    """LTV_OBSERVER_SHIFTED_GAIN: PhiY(t,s) = PhiX(t,s) Lt_{s-1} (zero for s = 0), the Phihat^y of (12c)/(15) (DESIGN.md
+    q20, q21); PhiX and the tube are unchanged.  SIMT, fused (p <= 8) and wide (p > 8) level-0 kernels."""
+    import torch
+
+    W, Lt, C = _observer_inputs(batch, T, n, p, seed=7 * n + p)
+    d = [torch.from_numpy(a).cuda() for a in (W.A, Lt, C, W.w)]
+    phi, r = L.ltv_scan_observer_response(*d, shifted_gain=True)
+    phi_p, r_p = L.ltv_scan_observer_response(*d)
+    torch.cuda.synchronize()
+    assert torch.equal(phi[..., :n], phi_p[..., :n]) and torch.equal(r, r_p)
+    phi = phi.cpu().numpy()
+    X, Y = O.observer_response(W.A, Lt, C, shifted_gain=True)
+    perm = _col_perm(T)
+    assert O.rel_err(phi[..., :n], X[:, perm]) <= TOL
+    assert O.rel_err(phi[..., n:n + p], Y[:, perm]) <= TOL
+    assert np.all(phi[..., n + p:] == 0.0)
+    assert np.all(phi[:, :T - 1, :, n:] == 0.0)          # column s = 0: blocks q = 0 .. T-2 of the column-packed order
+
+
 def test_observer_zero_gain_is_the_open_loop_response(L):
     import torch
 
@@ -347,3 +372,24 @@ def test_observer_zero_gain_is_the_open_loop_response(L):
     phi0, r0 = L.ltv_scan_system_response_tube(A, w)
     torch.cuda.synchronize()
     assert torch.equal(phi[..., :132], phi0) and torch.equal(r, r0) and torch.all(phi[..., 132:] == 0)
+
+
+def test_sharded_device_views_with_odd_item_size(L):
+    """Device shards of a batch whose per-item sizes are not multiples of 4 floats (T m = 15, T p = 9): shard_arrays must
+    hand the library 16-byte aligned tensors, and the shards must reproduce the whole batch bit for bit."""
+    import torch
+
+    from paper_2606_14188_b200.sharding import shard_arrays
+
+    W = dense_random(5, 3, 36, 5, seed=91)
+    d = {k: torch.from_numpy(getattr(W, k)).cuda() for k in ("A", "B", "c", "x0", "u", "g")}
+    x = L.ltv_scan_rollout(d["A"], d["B"], d["c"], d["x0"], d["u"])
+    lam, gu, _ = L.ltv_scan_adjoint(d["A"], d["B"], d["g"])
+    xs, gus = [], []
+    for rank in range(2):
+        m = shard_arrays(d, rank, 2)
+        assert all(v.data_ptr() % 16 == 0 for v in m.values())
+        xs.append(L.ltv_scan_rollout(m["A"], m["B"], m["c"], m["x0"], m["u"]))
+        gus.append(L.ltv_scan_adjoint(m["A"], m["B"], m["g"])[1])
+    torch.cuda.synchronize()
+    assert torch.equal(torch.cat(xs), x) and torch.equal(torch.cat(gus), gu)

@@ -530,3 +530,18 @@ def test_observer_achievability_identity_of_12c():
         ZA[(j + 1) * n:(j + 2) * n, j * n:(j + 1) * n] = A[j]
         ZC[(j + 1) * p:(j + 2) * p, j * n:(j + 1) * n] = C[j]
     np.testing.assert_allclose(Px @ (np.eye(N) - ZA) - Py @ ZC, np.eye(N), rtol=0, atol=1e-12)
+    # the oracle's own shifted-gain output is exactly that Py (strictly-lower blocks; the diagonal block of Py is
+    # PhiX(k,k) Lt_{k-1} = Lt_{k-1}), and the printed form of (14) is NOT: it breaks the identity
+    _, Ys = O.observer_response_item(A, Lt, C, shifted_gain=True)
+    _, Yp = O.observer_response_item(A, Lt, C)
+    Py2, Py3 = np.zeros_like(Py), np.zeros_like(Py)
+    for k in range(T):
+        if k >= 1:
+            Py2[k * n:(k + 1) * n, k * p:(k + 1) * p] = Lt[k - 1]
+            Py3[k * n:(k + 1) * n, k * p:(k + 1) * p] = Lt[k - 1]
+        for j in range(k):
+            Py2[k * n:(k + 1) * n, j * p:(j + 1) * p] = Ys[O.packed_index(k, j)]
+            Py3[k * n:(k + 1) * n, j * p:(j + 1) * p] = Yp[O.packed_index(k, j)]
+    np.testing.assert_allclose(Py2, Py, rtol=0, atol=1e-13)
+    assert np.all(Py2[:, :p] == 0.0)
+    assert np.max(np.abs(Px @ (np.eye(N) - ZA) - Py3 @ ZC - np.eye(N))) > 1e-3

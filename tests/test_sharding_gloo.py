@@ -20,6 +20,29 @@ def test_shard_range_partitions():
             assert max(sizes) - min(sizes) <= 1
 
 
+def test_shard_arrays_returns_16_byte_aligned_slices():
+    """A slice starting at an odd item of an array with T*m (or T*p) not a multiple of 4 floats is not 16-byte aligned
+    (the library would answer LTV_ERR_ALIGNMENT): shard_arrays hands out an aligned copy with the same content."""
+    import torch
+
+    from paper_2606_14188_b200.sharding import shard_arrays
+
+    batch, T, p, n = 5, 6, 3, 8
+    base = np.zeros(batch * T * p + 4, dtype=np.float32)
+    off = (-base.ctypes.data // 4) % 4                       # make f itself 16-byte aligned
+    f = base[off:off + batch * T * p].reshape(batch, T, p)
+    f[:] = np.arange(f.size, dtype=np.float32).reshape(f.shape)
+    A = np.zeros((batch, T, n, n), dtype=np.float32)
+    for world in (2, 3):
+        for rank in range(world):
+            b0, b1 = shard_range(batch, rank, world)
+            mine = shard_arrays(dict(A=A, f=f, none=None), rank, world)
+            assert mine["none"] is None and np.array_equal(mine["f"], f[b0:b1])
+            assert mine["f"].ctypes.data % 16 == 0 and mine["A"].ctypes.data % 16 == 0
+            tm = shard_arrays(dict(f=torch.from_numpy(f)), rank, world)["f"]
+            assert tm.data_ptr() % 16 == 0 and torch.equal(tm, torch.from_numpy(f)[b0:b1])
+
+
 def _worker(rank, world, port, q):
     import torch.distributed as dist
 
