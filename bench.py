@@ -38,14 +38,13 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (0..4)")
     ap.add_argument("--batch", type=int, default=0, help="items per GPU (0 = the config's own; config 4 sweeps 64/256/1024)")
-    ap.add_argument("--observer", type=int, default=0, metavar="P",
-                    help="also time ltv_scan_observer_response (NEXT-1, eq.(14)) with P measurement rows")
-    ap.add_argument("--kalman", type=int, default=0, metavar="P",
-                    help="also time ltv_scan_kalman_gains (NEXT-3, eq.(13)) with P observation rows")
-    ap.add_argument("--constraints", type=int, default=0, metavar="NC",
-                    help="also time ltv_scan_constraint_tightening (NEXT-2, eq.(12d)) with NC constraint rows per step")
-    ap.add_argument("--output-feedback", type=int, default=0, metavar="P",
-                    help="also time ltv_scan_output_feedback_response (NEXT-4, eq.(15) + (12e)) with P observation rows")
+    ap.add_argument("--quick", action="store_true",
+                    help="only the headline workload: no sustained / dense legs, no other configs, no NEXT rows")
+    ap.add_argument("--sustained", action="store_true", help="add the >= 2 s sustained leg (always on in the default run)")
+    ap.add_argument("--next-rows", action="store_true",
+                    help="add the SURVEY 8(f) calls timed alone (observer, Kalman, constraints, output feedback; p = 6)")
+    ap.add_argument("--no-tf32-peak", action="store_true",
+                    help="skip the live TF32 library-GEMM peak measurement (the committed figure is used instead)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-items", type=int, default=0, help="items in the CPU-oracle sample (0 = auto)")
@@ -56,17 +55,23 @@ def parse():
     return ap.parse_args()
 
 
+TRAFFIC_FILE = "profiles/r1_v5_traffic.csv"
+
+
 def ncu_traffic(cfg_index, kernel):
-    """dram bytes per step of `kernel` from the committed ncu capture (profiles/r1_v5_traffic.csv), or None."""
-    path = os.path.join(ROOT, "profiles", "r1_v5_traffic.csv")
+    """(dram bytes per step of `kernel`, where the figure comes from).  NOT measured in this run: ncu cannot be attached
+    to a timed run, so the figure is read from the committed `ncu --set full` capture of the same kernel and workload
+    (dram__bytes_read.sum + dram__bytes_write.sum summed over the launches of one step); (None, None) if that capture
+    has no row for this config."""
+    path = os.path.join(ROOT, TRAFFIC_FILE)
     try:
         for ln in open(path).read().splitlines()[1:]:
             c, k, b = ln.split(",")[:3]
             if int(c) == cfg_index and k == kernel:
-                return float(b)
+                return float(b), f"{TRAFFIC_FILE} (committed ncu --set full capture, not measured in this run)"
     except Exception:
         pass
-    return None
+    return None, None
 
 
 def peaks():
@@ -257,37 +262,57 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
-def main():
-    args = parse()
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
-        run_reference(args, rank, world)
-        return
+def _events(torch):
+    return torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
 
-    import numpy as np
-    import torch
-    import torch.distributed as dist
 
-    assert torch.cuda.is_available(), "bench.py needs a GPU (there is no CPU fallback)"
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    if args.tf32_peak:
-        if rank == 0:
-            print(json.dumps(dict(tf32_peak=measure_tf32_peak(torch.device("cuda", local), local))), flush=True)
-        return
-    import __graft_entry__ as G
+class Bench:
+    """Shared state of one bench.py process: device, distributed world, NVML sampler, measured peaks."""
 
-    G.build()
-    import paper_2606_14188_b200 as L
+    def __init__(self, args, rank, world, local):
+        import torch
+        import torch.distributed as dist
 
-    cfg, W = workload(args.config, rank, world, batch_override=args.batch or None)
+        self.args, self.rank, self.world, self.local = args, rank, world, local
+        self.torch, self.dist = torch, dist
+        self.dev = torch.device("cuda", local)
+        self.sampler = ClockSampler(local)
+        self.sampler.start()                      # before any warm-up: short regions still get several samples
+        self.sampler.ready.wait(timeout=10)
+        self.pk = peaks()
+        self.tf32 = None
+
+    def barrier(self):
+        if self.world > 1:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
+
+    def max_over_ranks(self, v):
+        if self.world > 1:
+            t = self.torch.tensor([v], device=self.dev, dtype=self.torch.float64)
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
+            return float(t.item())
+        return float(v)
+
+    def tensor_peak(self, region_s):
+        """(peak TFLOP/s, source): the MEASURED TF32 library-GEMM peak of this run - the burst figure for a timed region
+        under one second, the sustained one otherwise; without a live measurement, the committed one of
+        profiles/tf32_peak.md."""
+        t = self.tf32 or dict(tf32_tflops=746.0, tf32_tflops_sustained=606.8, committed=True)
+        which = "burst" if region_s < 1.0 else "sustained"
+        val = t["tf32_tflops"] if which == "burst" else t["tf32_tflops_sustained"]
+        src = ("profiles/tf32_peak.md (committed measurement)" if t.get("committed") else
+               "measured in this run (torch.matmul fp32 8192^3, allow_tf32)")
+        return val, f"TF32 library GEMM, {which} figure ({region_s:.2f} s timed region), {src}"
+
+
+def run_workload(B, L, W, name, cfg_index, steps, warmup, phi_on, min_seconds=0.0, label=None):
+    """Times `steps` passes of the whole hot path (rollout, Phi + tube, adjoint) over the device-resident workload W
+    (or as many as fill `min_seconds`); returns the measurement block (value, per-kernel times, rooflines, clocks)."""
+    torch = B.torch
+    dev = B.dev
     batch, T, n, m = W.shape
     P = T * (T - 1) // 2
-    phi_on = args.config != 4
-    dev = torch.device("cuda", local)
     d = {k: torch.from_numpy(getattr(W, k)).to(dev) for k in ("A", "B", "c", "x0", "u", "w", "g")}
     x = torch.empty((batch, T, n), device=dev)
     lam = torch.empty((batch, T, n), device=dev)
@@ -305,223 +330,220 @@ def main():
             L.ltv_scan_system_response_tube(d["A"], d["w"], phi_out=phi, r_out=r, workspace=ws)
         L.ltv_scan_adjoint(d["A"], d["B"], d["g"], lambda_out=lam, grad_u_out=gu, grad_x0_out=gx0)
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
-    L.ltv_profile_enable(True)
-    l0 = L.ltv_launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
+    warm = max(warmup, 3)
+    e0, e1 = _events(torch)
+    B.barrier()
     e0.record()
-    for _ in range(args.steps):
+    for _ in range(warm):
         step()
     e1.record()
-    barrier()
+    B.barrier()
+    if min_seconds > 0:
+        est = max(e0.elapsed_time(e1) / warm * 1e-3, 1e-6)
+        steps = max(steps, int(min_seconds / est) + 1)
+    L.ltv_profile_enable(True)
+    l0 = L.ltv_launch_count()
+    e0, e1 = _events(torch)
+    B.barrier()
+    t0 = time.time()
+    e0.record()
+    for _ in range(steps):
+        step()
+    e1.record()
+    B.barrier()
+    t1 = time.time()
     launches = L.ltv_launch_count() - l0
     prof = L.ltv_profile_collect()
     L.ltv_profile_enable(False)
-    sampler.stop_flag = True
-    sampler.join(timeout=2)
-    ms_total = e0.elapsed_time(e1)
-    if world > 1:
-        tt = torch.tensor([ms_total], device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms_total = float(tt.item())
-    ms_step = ms_total / args.steps
-    units = (P if phi_on else 1) * batch * world            # Phi blocks (or rollouts at config 5) per step
-    value = units / (ms_step * 1e-3)
+    ms_total = B.max_over_ranks(e0.elapsed_time(e1))
+    ms_step = ms_total / steps
+    units = (P if phi_on else 1) * batch * B.world
+    clocks = B.sampler.result(window=(t0, t1))
+    out = dict(workload=label or name, n=n, m=m, T=T, batch_per_gpu=batch, steps=steps, warmup=warm,
+               ms_per_step=ms_step, timed_region_s=ms_total * 1e-3,
+               value=units / (ms_step * 1e-3), unit=UNIT if phi_on else UNIT_C5, gpu_launches=int(launches),
+               kernel_ms_per_step={k: round(v[0] / steps, 5) for k, v in prof.items() if v[1]}, clocks=clocks)
 
-    # ---- roofline of the dominant kernel
-    pk = peaks()
-    k_ms = {k: (v[0] / max(v[1], 1), v[1]) for k, v in prof.items()}       # avg ms per launch, launches
-    if phi_on and prof["phi_combine_tc"][1] > 0:
-        G_blocks = (T - 1) * (T - 2) // 2                                   # GEMM blocks per item
-        flops_issued = 3.0 * 2.0 * n ** 3 * G_blocks * batch                # 3xTF32, per step (all levels)
-        ms_kernel = prof["phi_combine_tc"][0] / args.steps                  # all level launches of one step
-        ach = flops_issued / (ms_kernel * 1e-3) / 1e12
-        peak = pk["bf16_sustained"] * NOMINAL_TF32_OVER_BF16
-        clk = sampler.result()["sm_mhz"] or 1965
-        ceiling = 148 * 4096 * clk * 1e6 / 1e12            # 4096 dense tf32 flop / clk / SM at the sampled SM clock
-        roof = dict(bound="tensor", kernel="phi_combine_tc_kernel (3xTF32 tcgen05, all levels of one step)",
-                    achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak,
-                    traffic=ncu_traffic(args.config, "phi_combine_tc"),
-                    algorithmic="issued tf32 flop = 3 x 2 n^3 x (T-1)(T-2)/2 x batch per step (no padding, no split work)",
-                    frac_of_unit_ceiling=ach / ceiling,
-                    unit_ceiling=f"{ceiling:.0f} TFLOP/s = 148 SM x 4096 flop/clk x {clk} MHz (median SM clock sampled during the run)",
-                    peak_source=f"{pk['source']} bf16 sustained x {NOMINAL_TF32_OVER_BF16} (nominal tf32/bf16)",
-                    logical_fp32_tflops=ach / 3.0, kernel_ms_per_step=ms_kernel,
-                    launches_per_step=prof["phi_combine_tc"][1] / args.steps)
-    else:
-        bytes_roll = batch * (T * (n * n + n * m + n + m) + n + T * n) * 4.0
-        ms_kernel = prof["rollout"][0] / max(prof["rollout"][1], 1)
-        ach = bytes_roll / (ms_kernel * 1e-3) / 1e9
-        roof = dict(bound="hbm", kernel="rollout_kernel", achieved=ach, peak=pk["hbm_gbs"], unit="GB/s",
-                    frac=ach / pk["hbm_gbs"], traffic=ncu_traffic(args.config, "rollout"),
-                    algorithmic="bytes = batch x (T(n^2 + nm + n + m) + n + Tn) x 4 per launch",
-                    peak_source=pk["source"] + " copy bandwidth", kernel_ms_per_step=ms_kernel)
-    share = {k: round(v[0] / args.steps, 4) for k, v in prof.items() if v[1]}
-
-    # ---- secondary HBM rooflines (rollout / adjoint), reported beside the headline
     bytes_roll = batch * (T * (n * n + n * m + n + m) + n + T * n) * 4.0
-    extra = {}
+    vec = {}
     for k in ("rollout", "adjoint"):
         if prof[k][1]:
             ms = prof[k][0] / prof[k][1]
-            extra[k] = dict(per_s=batch * world / (ms * 1e-3), ms=ms, hbm_gbs=bytes_roll / (ms * 1e-3) / 1e9,
-                            hbm_frac=bytes_roll / (ms * 1e-3) / 1e9 / pk["hbm_gbs"])
+            gbs = bytes_roll / (ms * 1e-3) / 1e9
+            vec[k] = dict(per_s=batch * B.world / (ms * 1e-3), ms=ms, hbm_gbs=gbs, hbm_frac=gbs / B.pk["hbm_gbs"])
+    out["vector_scans"] = vec
+    out["rollouts_per_s"] = vec.get("rollout", {}).get("per_s")
+    out["adjoints_per_s"] = vec.get("adjoint", {}).get("per_s")
 
-    # ---- NEXT-1: closed-loop observer propagation on the same A (random gains), timed alone
-    observer = None
-    if phi_on and args.observer > 0:
-        pobs = args.observer
-        gen = torch.Generator(device=dev).manual_seed(1234)
-        Lt = torch.randn((batch, T, n, pobs), device=dev, generator=gen) * (0.05 / pobs ** 0.5)
-        Cm = torch.randn((batch, T, pobs, n), device=dev, generator=gen) / n ** 0.5
-        del phi
-        torch.cuda.empty_cache()
-        nc = L.ltv_observer_row_floats(n, pobs)
-        phio = torch.empty((batch, P, n, nc), device=dev)
-        wso = torch.empty(max(16, L.ltv_scan_workspace_bytes(L.LTV_OP_OBSERVER_RESPONSE, batch, T, n, pobs)),
-                          dtype=torch.uint8, device=dev)
-        for _ in range(3):
-            L.ltv_scan_observer_response(d["A"], Lt, Cm, d["w"], phi_out=phio, r_out=r, workspace=wso)
-        o0, o1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        barrier()
-        o0.record()
-        for _ in range(args.steps):
-            L.ltv_scan_observer_response(d["A"], Lt, Cm, d["w"], phi_out=phio, r_out=r, workspace=wso)
-        o1.record()
-        barrier()
-        oms = o0.elapsed_time(o1) / args.steps
-        observer = dict(p=pobs, ms=oms, blocks_per_s=batch * world * P / (oms * 1e-3),
-                        issued_tf32_tflops=3.0 * 2.0 * n * n * nc * ((T - 1) * (T - 2) // 2) * batch / (oms * 1e-3) / 1e12,
-                        note="ltv_scan_observer_response alone: [PhiX | PhiY] blocks of n x (n + roundup4(p)) floats")
-        del phio, wso
-        phi = None
+    if phi_on and prof["phi_combine_tc"][1] > 0:
+        G_blocks = (T - 1) * (T - 2) // 2                                   # GEMM blocks per item
+        flops_issued = 3.0 * 2.0 * n ** 3 * G_blocks * batch                # 3xTF32, per step (all levels)
+        ms_kernel = prof["phi_combine_tc"][0] / steps                       # all level launches of one step
+        ach = flops_issued / (ms_kernel * 1e-3) / 1e12
+        peak, src = B.tensor_peak(ms_total * 1e-3)
+        clk = clocks["sm_mhz"] or 1965
+        ceiling = 148 * 4096 * clk * 1e6 / 1e12            # 4096 dense tf32 flop / clk / SM at the sampled SM clock
+        tr, tr_src = ncu_traffic(cfg_index, "phi_combine_tc") if label is None else (None, None)
+        out["roofline"] = dict(
+            bound="tensor", kernel="phi_combine_tc_kernel (3xTF32 tcgen05, all levels of one step)",
+            achieved=ach, peak=peak, unit="TFLOP/s", frac=ach / peak, traffic=tr, traffic_source=tr_src,
+            algorithmic="issued tf32 flop = 3 x 2 n^3 x (T-1)(T-2)/2 x batch per step (no padding, no split work)",
+            peak_source=src, frac_of_unit_ceiling=ach / ceiling,
+            unit_ceiling=f"{ceiling:.0f} TFLOP/s = 148 SM x 4096 flop/clk x {clk} MHz (median SM clock sampled in the timed region)",
+            logical_fp32_tflops=ach / 3.0, kernel_ms_per_step=ms_kernel,
+            launches_per_step=prof["phi_combine_tc"][1] / steps,
+            share_of_step=ms_kernel / ms_step)
+    elif "rollout" in vec:
+        tr, tr_src = ncu_traffic(cfg_index, "rollout") if label is None else (None, None)
+        out["roofline"] = dict(bound="hbm", kernel="rollout_kernel", achieved=vec["rollout"]["hbm_gbs"],
+                               peak=B.pk["hbm_gbs"], unit="GB/s", frac=vec["rollout"]["hbm_frac"], traffic=tr,
+                               traffic_source=tr_src,
+                               algorithmic="bytes = batch x (T(n^2 + nm + n + m) + n + Tn) x 4 per launch",
+                               peak_source=B.pk["source"] + " copy bandwidth (MEASURED_PEAKS.json hbm_gbs)",
+                               kernel_ms_per_step=vec["rollout"]["ms"], share_of_step=vec["rollout"]["ms"] / ms_step)
+    return out
 
-    # ---- NEXT-3: Kalman recursion (13) on the same A with the tracked-point observation stand-in, timed alone
-    kalman = None
-    if args.kalman > 0:
-        from workloads import observation_model
-        pk_ = args.kalman
-        Mobs = observation_model(batch, T, n, pk_, seed=777 + rank, kind="track")
-        kd = [torch.from_numpy(Mobs[k]).to(dev) for k in ("C", "e", "f", "Pi0")]
-        if phi_on:
-            phi = None
-        torch.cuda.empty_cache()
-        Lto = torch.empty((batch, T, n, pk_), device=dev)
-        Pio = torch.empty((batch, T + 1, n, n), device=dev)
-        wsk = torch.empty(max(16, L.ltv_scan_workspace_bytes(L.LTV_OP_KALMAN_GAINS, batch, T, n, pk_)),
-                          dtype=torch.uint8, device=dev)
-        for _ in range(3):
-            L.ltv_scan_kalman_gains(d["A"], *kd, Lt_out=Lto, Pi_out=Pio, workspace=wsk)
-        k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        barrier()
-        k0.record()
-        for _ in range(args.steps):
-            L.ltv_scan_kalman_gains(d["A"], *kd, Lt_out=Lto, Pi_out=Pio, workspace=wsk)
-        k1.record()
-        barrier()
-        kms = k0.elapsed_time(k1) / args.steps
-        kalman = dict(p=pk_, ms=kms, recursions_per_s=batch * world / (kms * 1e-3),
-                      steps_per_s=batch * world * T / (kms * 1e-3),
-                      issued_tf32_tflops=3.0 * 2.0 * 2.0 * n ** 3 * T * batch / (kms * 1e-3) / 1e12,
-                      note="ltv_scan_kalman_gains alone: T sequential steps of (13) over the whole batch, two n^3 "
-                           "products per step and item (3xTF32 on tcgen05 for n >= 96)")
-        del Lto, Pio, wsk, kd
 
-    # ---- NEXT-2 (12d): constraint-tightening margins on the same A, w with random constraint rows, timed alone
-    constraints = None
-    if args.constraints > 0:
-        ncr = args.constraints
-        gen = torch.Generator(device=dev).manual_seed(4321 + rank)
-        Hc = torch.randn((batch, T, ncr, n), device=dev, generator=gen)
-        sig = torch.empty((batch, T, ncr), device=dev)
-        wsc = torch.empty(max(16, L.ltv_scan_workspace_bytes(L.LTV_OP_CONSTRAINT_TIGHTENING, batch, T, n, ncr)),
-                          dtype=torch.uint8, device=dev)
-        for _ in range(3):
-            L.ltv_scan_constraint_tightening(d["A"], d["w"], Hc, sigma_out=sig, workspace=wsc)
-        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        barrier()
-        c0.record()
-        for _ in range(args.steps):
-            L.ltv_scan_constraint_tightening(d["A"], d["w"], Hc, sigma_out=sig, workspace=wsc)
-        c1.record()
-        barrier()
-        cms = c0.elapsed_time(c1) / args.steps
-        constraints = dict(nc=ncr, ms=cms, items_per_s=batch * world / (cms * 1e-3),
-                           hbm_gbs=batch * (T - 1) * n * n * 4 / (cms * 1e-3) / 1e9,
-                           note="ltv_scan_constraint_tightening alone: backward sweep of the stacked constraint rows, "
-                                "A read once (hbm_gbs counts those bytes), Phi never formed")
-        del Hc, sig, wsc
+def next_rows(B, L, W, steps):
+    """SURVEY 8(f) rows, each timed alone on the device-resident C2 inputs (a few repetitions)."""
+    torch, dev = B.torch, B.dev
+    from workloads import observation_model
 
-    # ---- NEXT-4 (first form): assembled output-feedback responses + tube for gain-defined controllers, timed alone
-    ofb = None
-    if args.output_feedback > 0 and m > 0:
-        pf = args.output_feedback
-        if phi_on:
-            phi = None
-        torch.cuda.empty_cache()
-        gen = torch.Generator(device=dev).manual_seed(2468 + rank)
-        Kfb = torch.randn((batch, T, m, n), device=dev, generator=gen) * (0.2 / n ** 0.5)
-        Ltf = torch.randn((batch, T, n, pf), device=dev, generator=gen) * (0.05 / pf ** 0.5)
-        Cf = torch.randn((batch, T, pf, n), device=dev, generator=gen) / n ** 0.5
-        ff = torch.rand((batch, T, pf), device=dev, generator=gen) * 4e-3 + 1e-3
-        wsf = torch.empty(L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, batch, T, n, 0), dtype=torch.uint8, device=dev)
+    batch, T, n, m = W.shape
+    P = T * (T - 1) // 2
+    p = 6
+    d = {k: torch.from_numpy(getattr(W, k)).to(dev) for k in ("A", "B", "w")}
+    out = {}
+
+    def timed(fn, reps):
         for _ in range(2):
-            out = L.ltv_scan_output_feedback_response(d["A"], d["B"], Kfb, Ltf, Cf, d["w"], ff, workspace=wsf)
-        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        nrep = max(1, min(args.steps, 5))
-        barrier()
-        f0.record()
-        for _ in range(nrep):
-            out = L.ltv_scan_output_feedback_response(d["A"], d["B"], Kfb, Ltf, Cf, d["w"], ff, workspace=wsf)
-        f1.record()
-        barrier()
-        fms = f0.elapsed_time(f1) / nrep
-        ofb = dict(p=pf, ms=fms, blocks_per_s=batch * world * P / (fms * 1e-3),
-                   issued_tf32_tflops=3.0 * 2.0 * (2 * n) ** 3 * ((T - 1) * (T - 2) // 2) * batch / (fms * 1e-3) / 1e12,
-                   note="ltv_scan_output_feedback_response alone: Phi scan on the 2n-state augmented closed loop "
-                        "(8x the flops of the n-state scan, counted here) + extraction / tube pass")
-        del out, wsf, Kfb, Ltf, Cf
+            fn()
+        e0, e1 = _events(torch)
+        B.barrier()
+        e0.record()
+        for _ in range(reps):
+            fn()
+        e1.record()
+        B.barrier()
+        return B.max_over_ranks(e0.elapsed_time(e1)) / reps
 
-    # ---- end to end through the C-ABI with host buffers
-    e2e = None
-    if not args.no_e2e:
-        if phi_on:
-            phi = None
-            del ws
-        torch.cuda.empty_cache()
-        need = L.ltv_scan_workspace_bytes(L.LTV_OP_PIPELINE_HOST if phi_on else L.LTV_OP_PIPELINE_HOST_NO_PHI, batch, T, n, m)
-        wsh = torch.empty(need, dtype=torch.uint8, device=dev)
-        h = {k: torch.from_numpy(getattr(W, k)).pin_memory() for k in ("A", "B", "c", "x0", "u", "w", "g")}
-        if not phi_on:
-            h.pop("w")
-        outs = None
-        h2d = sum(v.numel() * 4 for v in h.values())
-        for i in range(1 + args.e2e_steps):
-            if i == 1:
-                barrier()
-                t0 = time.perf_counter()
-            outs = L.ltv_scan_pipeline_host(h["A"], h["B"], h["c"], h["x0"], h["u"], h["w"] if phi_on else None, h["g"],
-                                            wsh, outs=outs)
-        barrier()
-        sec = (time.perf_counter() - t0) / args.e2e_steps
-        if world > 1:
-            tt = torch.tensor([sec], device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            sec = float(tt.item())
-        d2h = sum(outs[k].numel() * 4 for k in ("x", "r", "lam", "grad_u", "grad_x0") if outs[k] is not None)
-        e2e = dict(value=units / sec, unit=UNIT if phi_on else UNIT_C5, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
-                   ms_per_step=sec * 1e3, note="ltv_scan_pipeline_host, pinned host buffers, upload of chunk i+1 overlapped with the compute of chunk i" +
-                        ("; Phi stays in HBM" if phi_on else "; rollout + adjoint only"))
+    gen = torch.Generator(device=dev).manual_seed(1234 + B.rank)
+    Lt = torch.randn((batch, T, n, p), device=dev, generator=gen) * (0.05 / p ** 0.5)
+    Cm = torch.randn((batch, T, p, n), device=dev, generator=gen) / n ** 0.5
+    Kfb = torch.randn((batch, T, m, n), device=dev, generator=gen) * (0.2 / n ** 0.5)
+    ff = torch.rand((batch, T, p), device=dev, generator=gen) * 4e-3 + 1e-3
+    # NEXT-1: closed-loop observer propagation (14)
+    nc = L.ltv_observer_row_floats(n, p)
+    phio = torch.empty((batch, P, n, nc), device=dev)
+    ro = torch.empty((batch, T, n), device=dev)
+    wso = torch.empty(max(16, L.ltv_scan_workspace_bytes(L.LTV_OP_OBSERVER_RESPONSE, batch, T, n, p)), dtype=torch.uint8, device=dev)
+    ms = timed(lambda: L.ltv_scan_observer_response(d["A"], Lt, Cm, d["w"], phi_out=phio, r_out=ro, workspace=wso), steps)
+    out["observer"] = dict(p=p, ms=ms, blocks_per_s=batch * B.world * P / (ms * 1e-3),
+                           issued_tf32_tflops=6.0 * n * n * nc * ((T - 1) * (T - 2) // 2) * batch / (ms * 1e-3) / 1e12)
+    del phio, wso
+    torch.cuda.empty_cache()
+    # NEXT-3: Kalman recursion (13)
+    Mobs = observation_model(batch, T, n, p, seed=777 + B.rank, kind="track")
+    kd = [torch.from_numpy(Mobs[k]).to(dev) for k in ("C", "e", "f", "Pi0")]
+    Lto = torch.empty((batch, T, n, p), device=dev)
+    Pio = torch.empty((batch, T + 1, n, n), device=dev)
+    wsk = torch.empty(max(16, L.ltv_scan_workspace_bytes(L.LTV_OP_KALMAN_GAINS, batch, T, n, p)), dtype=torch.uint8, device=dev)
+    ms = timed(lambda: L.ltv_scan_kalman_gains(d["A"], *kd, Lt_out=Lto, Pi_out=Pio, workspace=wsk), steps)
+    out["kalman"] = dict(p=p, ms=ms, recursions_per_s=batch * B.world / (ms * 1e-3),
+                         issued_tf32_tflops=12.0 * n ** 3 * T * batch / (ms * 1e-3) / 1e12)
+    del Pio, wsk, kd
+    # NEXT-2: constraint margins (12d), open-loop form
+    Hc = torch.randn((batch, T, 6, n), device=dev, generator=gen)
+    sig = torch.empty((batch, T, 6), device=dev)
+    wsc = torch.empty(max(16, L.ltv_scan_workspace_bytes(L.LTV_OP_CONSTRAINT_TIGHTENING, batch, T, n, 6)), dtype=torch.uint8, device=dev)
+    ms = timed(lambda: L.ltv_scan_constraint_tightening(d["A"], d["w"], Hc, sigma_out=sig, workspace=wsc), steps)
+    out["constraints"] = dict(nc=6, ms=ms, items_per_s=batch * B.world / (ms * 1e-3))
+    del wsc
+    # NEXT-4: assembled output-feedback responses (15) + tube (12e)
+    wsf = torch.empty(L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, batch, T, n, 0), dtype=torch.uint8, device=dev)
+    ms = timed(lambda: L.ltv_scan_output_feedback_response(d["A"], d["B"], Kfb, Lt, Cm, d["w"], ff, workspace=wsf), min(steps, 3))
+    out["output_feedback"] = dict(p=p, ms=ms, blocks_per_s=batch * B.world * P / (ms * 1e-3))
+    del wsf
+    torch.cuda.empty_cache()
+    return out
+
+
+def e2e_leg(B, L, W, phi_on, reps):
+    """The same metric through ltv_scan_pipeline_host: pinned HOST buffers in, host results out, copies timed."""
+    torch, dev = B.torch, B.dev
+    batch, T, n, m = W.shape
+    P = T * (T - 1) // 2
+    units = (P if phi_on else 1) * batch * B.world
+    need = L.ltv_scan_workspace_bytes(L.LTV_OP_PIPELINE_HOST if phi_on else L.LTV_OP_PIPELINE_HOST_NO_PHI, batch, T, n, m)
+    wsh = torch.empty(need, dtype=torch.uint8, device=dev)
+    h = {k: torch.from_numpy(getattr(W, k)).pin_memory() for k in ("A", "B", "c", "x0", "u", "w", "g")}
+    if not phi_on:
+        h.pop("w")
+    h2d = sum(v.numel() * 4 for v in h.values())
+    outs = None
+    for i in range(1 + reps):
+        if i == 1:
+            B.barrier()
+            t0 = time.perf_counter()
+        outs = L.ltv_scan_pipeline_host(h["A"], h["B"], h["c"], h["x0"], h["u"], h["w"] if phi_on else None, h["g"],
+                                        wsh, outs=outs)
+    B.barrier()
+    sec = B.max_over_ranks((time.perf_counter() - t0) / reps)
+    d2h = sum(outs[k].numel() * 4 for k in ("x", "r", "lam", "grad_u", "grad_x0") if outs[k] is not None)
+    del wsh
+    torch.cuda.empty_cache()
+    return dict(value=units / sec, unit=UNIT if phi_on else UNIT_C5, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
+                ms_per_step=sec * 1e3, steps=reps,
+                note="ltv_scan_pipeline_host, pinned host buffers, upload of chunk i+1 overlapped with the compute of chunk i"
+                     + ("; Phi (the largest result) stays in HBM where its consumers run: value counts x, r, lambda, "
+                        "grad_u, grad_x0 back on the host" if phi_on else "; rollout + adjoint only"))
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    assert torch.cuda.is_available(), "bench.py needs a GPU (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if args.tf32_peak:
+        if rank == 0:
+            print(json.dumps(dict(tf32_peak=measure_tf32_peak(torch.device("cuda", local), local))), flush=True)
+        return
+    import __graft_entry__ as G
+
+    G.build()
+    import paper_2606_14188_b200 as L
+    from workloads import dense_random
+
+    B = Bench(args, rank, world, local)
+    full = args.config == 1 and not args.batch and not args.quick     # the default line carries every config
+    if not args.no_tf32_peak:
+        B.tf32 = measure_tf32_peak(B.dev, local, sustained_s=2.5)
+        B.barrier()
+
+    cfg, W = workload(args.config, rank, world, batch_override=args.batch or None)
+    batch, T, n, m = W.shape
+    P = T * (T - 1) // 2
+    phi_on = args.config != 4
+    head = run_workload(B, L, W, cfg["name"], args.config, args.steps, args.warmup, phi_on)
+
+    sustained = dense = nxt = None
+    others = {}
+    if full or args.sustained:
+        sustained = run_workload(B, L, W, cfg["name"], args.config, args.steps, args.warmup, phi_on, min_seconds=2.0)
+    if full or args.next_rows:
+        nxt = next_rows(B, L, W, max(3, min(args.steps, 10))) if phi_on else None
+    e2e = None if args.no_e2e else e2e_leg(B, L, W, phi_on, args.e2e_steps)
 
     # ---- CPU oracle beside it (rank 0, N = 1 only)
     cpu = None
@@ -535,22 +557,37 @@ def main():
         cpu = dict(value=items * (P if phi_on else 1) / sec, unit=UNIT if phi_on else UNIT_C5, cores=blas_threads(), kind="oracle",
                    sample=f"{items} of {batch} items of {cfg['name']}, whole path, fp64 numpy, {sec:.1f} s")
 
+    if full:
+        # the same shape on DENSE Jacobians (what PAPER.md:166 calls "dense matrix multiplications"): the like-for-like
+        # figure against the library-GEMM peak, which is itself measured on dense random operands
+        Wd = dense_random(batch, T, n, m, seed=4242 + rank)
+        dense = run_workload(B, L, Wd, "dense_random", 1, args.steps, args.warmup, True, min_seconds=2.0,
+                             label=f"dense random A_t = I + N(0, 0.5/sqrt(n)) at the C2 shape (n={n} T={T} batch={batch})")
+        del Wd, W
+        for ci, bo, st in ((0, None, 200), (2, None, 20), (3, None, 8), (4, 64, 40), (4, 256, 20), (4, 1024, 8)):
+            c2, W2 = workload(ci, rank, world, batch_override=bo)
+            key = f"C{ci + 1}" + (f"_b{bo}" if bo else "")
+            others[key] = run_workload(B, L, W2, c2["name"], ci, st, 3, ci != 4)
+            del W2
+
+    B.sampler.stop_flag = True
     if rank == 0:
         a_gb = batch * T * n * n * 4 / 1e9
         phi_gb = batch * P * n * n * 4 / 1e9 if phi_on else 0.0
-        line = dict(metric=METRIC, value=value, unit=UNIT if phi_on else UNIT_C5, n_gpus=world,
-                    steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=ms_step, higher_is_better=True,
+        line = dict(metric=METRIC, value=head["value"], unit=head["unit"], n_gpus=world,
+                    steps=head["steps"], warmup=head["warmup"], ms_per_step=head["ms_per_step"], higher_is_better=True,
                     scaling="weak", vs_baseline=None, dtype="tf32x3/f32", data="synthetic",
                     config=dict(workload=f"{cfg['name']}: n={n} m={m} T={T} batch={batch} per GPU, "
                                          f"{P if phi_on else 0} Phi blocks/item (BASELINE.json configs[{args.config}])",
                                 l2=(f"inputs (A {a_gb:.2f} GB) and outputs (Phi {phi_gb:.1f} GB) larger than the 126 MB L2; "
                                     "no flush" if a_gb > 0.3 else
                                     f"working set (A {a_gb * 1e3:.2f} MB) fits L2: warm-cache, latency-bound case"),
-                                phi_layout="column-packed"),
-                    clocks=sampler.result(), e2e=e2e, gpu_launches=int(launches), roofline=roof,
-                    cpu_baseline=cpu, kernel_ms_per_step=share, vector_scans=extra, observer=observer, kalman=kalman, constraints=constraints, output_feedback=ofb,
-                    rollouts_per_s=extra.get("rollout", {}).get("per_s"),
-                    adjoints_per_s=extra.get("adjoint", {}).get("per_s"))
+                                phi_layout="column-packed (LTV_PHI_COLUMN_PACKED, the scan's native order)"),
+                    clocks=head["clocks"], e2e=e2e, gpu_launches=head["gpu_launches"], roofline=head.get("roofline"),
+                    cpu_baseline=cpu, kernel_ms_per_step=head["kernel_ms_per_step"], vector_scans=head["vector_scans"],
+                    rollouts_per_s=head["rollouts_per_s"], adjoints_per_s=head["adjoints_per_s"],
+                    timed_region_s=head["timed_region_s"], tf32_peak=B.tf32, hbm_peak_gbs=B.pk["hbm_gbs"],
+                    sustained=sustained, dense=dense, configs=others or None, next=nxt)
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -64,14 +64,26 @@ enum { LTV_OP_ROLLOUT = 0, LTV_OP_SYSTEM_RESPONSE_TUBE = 1, LTV_OP_ADJOINT = 2, 
        LTV_OP_OBSERVER_RESPONSE = 5 /* ltv_scan_observer_response; pass p (rows of C) as `m` */,
        LTV_OP_KALMAN_GAINS = 6 /* ltv_scan_kalman_gains; pass p (rows of C) as `m` */,
        LTV_OP_CONSTRAINT_TIGHTENING = 7 /* ltv_scan_constraint_tightening; pass nc (constraint rows) as `m` */,
-       LTV_OP_OUTPUT_FEEDBACK = 8 /* ltv_scan_output_feedback_response; `m` is ignored */ };
+       LTV_OP_OUTPUT_FEEDBACK = 8 /* ltv_scan_output_feedback_response; `m` is ignored */,
+       LTV_OP_SYSTEM_RESPONSE_TUBE_RELAYOUT = 9 /* ltv_scan_system_response_tube with LTV_PHI_ROW_PACKED / _SQUARE_GRID */ };
 
-/* `phi_layout` argument.  COLUMN_PACKED (the only layout of this version): the P = T(T-1)/2 blocks of one
- * item are stored column by column of the block-lower-triangular operator; block (t,s), 0 <= s < t <= T-1,
- * sits at block index  q(t,s) = s(T-1) - s(s-1)/2 + (t-s-1)  in phi_out[batch, P, n, n].  All blocks with
- * the same s are therefore one contiguous tall (T-1-s)n x n row-major matrix, which is what lets the
- * divide-and-conquer combine  Phi(t,s) = Phi(t,mid) Phi(mid,s)  stream its left operand as one matrix. */
-enum { LTV_PHI_COLUMN_PACKED = 0 };
+/* `phi_layout` argument: where block (t,s), 0 <= s < t <= T-1, of one item sits in phi_out.  Blocks are contiguous
+ * n x n row-major matrices in every layout; P = T(T-1)/2.
+ *   LTV_PHI_ROW_PACKED (0)     phi_out[batch, P, n, n], block index p(t,s) = t(t-1)/2 + s: the block rows of the lower-
+ *                              triangular operator one after the other, the order (12c)-(12e) index it in.
+ *   LTV_PHI_SQUARE_GRID (1)    phi_out[batch, T, T, n, n], block (t,s) at grid cell t T + s; only cells with s < t are
+ *                              written, the others are left untouched.
+ *   LTV_PHI_COLUMN_PACKED (2)  phi_out[batch, P, n, n], block index q(t,s) = s(T-1) - s(s-1)/2 + (t-s-1)
+ *                              (ltv_phi_block_index): column by column, so all blocks with the same s are one contiguous
+ *                              tall (T-1-s)n x n row-major matrix.  This is the order the scan COMPUTES in - the
+ *                              divide-and-conquer combine Phi(t,s) = Phi(t,mid) Phi(mid,s) streams its stacked left
+ *                              operand and each output column as one matrix (128-row tiles run across block boundaries:
+ *                              97-99 % tile fill instead of 78 % at n = 300) - and the FAST PATH: no extra pass.
+ * With ROW_PACKED or SQUARE_GRID the scan runs column-packed inside the workspace (which must then also hold a
+ * column-packed copy of Phi: op LTV_OP_SYSTEM_RESPONSE_TUBE_RELAYOUT) and one streaming block copy re-orders it into
+ * phi_out at the end: + 8 n^2 bytes of HBM traffic per block (about + 3.5 ms on the 6 ms call at n = 300, T = 32,
+ * batch 64).  ltv_scan_observer_response and ltv_scan_output_feedback_response accept LTV_PHI_COLUMN_PACKED only. */
+enum { LTV_PHI_ROW_PACKED = 0, LTV_PHI_SQUARE_GRID = 1, LTV_PHI_COLUMN_PACKED = 2 };
 
 /* `flags` bits of ltv_scan_system_response_tube / ltv_scan_observer_response. */
 enum { LTV_TUBE_ROW_2NORM = 1,
@@ -79,6 +91,8 @@ enum { LTV_TUBE_ROW_2NORM = 1,
 
 /* Block index q(t,s) of the COLUMN_PACKED layout; -1 if not 0 <= s < t <= T-1.  Pure host arithmetic. */
 LTV_API long long ltv_phi_block_index(int T, int t, int s);
+/* The same for any layout (ROW_PACKED: t(t-1)/2 + s; SQUARE_GRID: t T + s); -1 for a bad layout or index. */
+LTV_API long long ltv_phi_block_index_layout(int T, int t, int s, int phi_layout);
 
 /* Bytes of device workspace the given op needs for these sizes (0 is a valid answer; a NULL workspace is
  * then accepted).  Returns 0 for invalid arguments.  For LTV_OP_PIPELINE_HOST the figure covers device
@@ -101,7 +115,8 @@ LTV_API int ltv_scan_rollout(const float* A, const float* B, const float* c, con
 /* System response + reachable tube (north_star (ii); eq.(12c), :147 eq.(12e)).
  *   A        device [batch,T,n,n]     required; only A_0 .. A_{T-2} are read
  *   w        device [batch,T,n]       required; w_s >= 0, only s <= T-2 read
- *   phi_out  device [batch,P,n,n]     P = T(T-1)/2, layout `phi_layout`; Phi(t,t) = I is not stored
+ *   phi_out  device [batch,P,n,n]     P = T(T-1)/2, or [batch,T,T,n,n] for LTV_PHI_SQUARE_GRID: layout `phi_layout`;
+ *                                     Phi(t,t) = I is not stored
  *   r_out    device [batch,T,n]       r_0 = 0, r_t = sum_{s<t} |Phi(t,s)| w_s  (element-wise abs)
  *   flags    0, or LTV_TUBE_ROW_2NORM: r_t[i] = sum_{s<t} || row_i(Phi(t,s) diag(w_s)) ||_2, the row-wise two-norm
  *            tube of eq.(12e) as printed with the disturbance scaling E_s = diag(w_s)
@@ -286,9 +301,12 @@ LTV_API unsigned long long ltv_launch_count(void);
  * per kernel class into the two caller arrays of LTV_PROFILE_CLASSES entries (host memory), and clears the
  * record.  Classes: 0 rollout, 1 adjoint, 2 Phi level 0 (copy + tube), 3 Phi combine (tcgen05 3xTF32),
  * 4 Phi combine (fp32 FMA, small n), 5 tube finalise, 6 batched GEMMs of the Kalman recursion and the constraint sweep
- * (tcgen05 3xTF32, or fp32 FMA for small n), 7 their fp32 support kernels (gain, closed loop, row norms). */
-#define LTV_PROFILE_CLASSES 8
+ * (tcgen05 3xTF32, or fp32 FMA for small n), 7 their fp32 support kernels (gain, closed loop, row norms), 8 the block
+ * re-ordering copy of the non-native Phi layouts, 9-11 see ltv_profile_class_name. */
+#define LTV_PROFILE_CLASSES 12
 LTV_API int ltv_profile_enable(int on);
+/* Short name of a profile class (static storage), NULL if cls is out of range. */
+LTV_API const char* ltv_profile_class_name(int cls);
 LTV_API int ltv_profile_collect(double* ms_by_class, unsigned long long* launches_by_class);
 
 #ifdef __cplusplus

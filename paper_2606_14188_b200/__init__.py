@@ -9,7 +9,8 @@ import importlib
 _API = (
     "EXPORTS", "LIB_PATH", "LTV_OP_ADJOINT", "LTV_OP_PIPELINE_HOST", "LTV_OP_PIPELINE_HOST_NO_PHI", "LTV_OP_OBSERVER_RESPONSE",
     "LTV_OP_ROLLOUT",
-    "LTV_OP_SYSTEM_RESPONSE_TUBE", "LTV_PHI_COLUMN_PACKED", "LTV_TUBE_ROW_2NORM", "LTV_OBSERVER_SHIFTED_GAIN", "PROFILE_CLASSES", "LtvError", "lib",
+    "LTV_OP_SYSTEM_RESPONSE_TUBE", "LTV_PHI_COLUMN_PACKED", "LTV_PHI_ROW_PACKED", "LTV_PHI_SQUARE_GRID", "LTV_OP_SYSTEM_RESPONSE_TUBE_RELAYOUT",
+    "ltv_phi_block_index_layout", "LTV_TUBE_ROW_2NORM", "LTV_OBSERVER_SHIFTED_GAIN", "PROFILE_CLASSES", "LtvError", "lib",
     "ltv_launch_count", "ltv_phi_block_index", "ltv_profile_collect", "ltv_profile_enable",
     "ltv_scan_adjoint", "ltv_scan_pipeline_host", "ltv_scan_rollout", "ltv_scan_system_response_tube",
     "ltv_scan_workspace_bytes", "ltv_scan_observer_response", "ltv_observer_row_floats", "ltv_scan_kalman_gains",

@@ -25,15 +25,17 @@ LTV_OP_OUTPUT_FEEDBACK = 8
 LTV_TUBE_ROW_2NORM = 1
 LTV_OBSERVER_SHIFTED_GAIN = 2
 LTV_KALMAN_SCAN, LTV_KALMAN_RECURSION = 1, 2
-LTV_PHI_COLUMN_PACKED = 0
+LTV_PHI_ROW_PACKED, LTV_PHI_SQUARE_GRID, LTV_PHI_COLUMN_PACKED = 0, 1, 2
+LTV_OP_SYSTEM_RESPONSE_TUBE_RELAYOUT = 9
 LTV_OPT_VECTOR_CLUSTER, LTV_OPT_PIPELINE_CHUNKS = 0, 1
 
 EXPORTS = (
-    "ltv_phi_block_index", "ltv_scan_workspace_bytes", "ltv_scan_rollout", "ltv_scan_system_response_tube",
+    "ltv_phi_block_index", "ltv_phi_block_index_layout", "ltv_scan_workspace_bytes", "ltv_scan_rollout", "ltv_scan_system_response_tube",
     "ltv_scan_adjoint", "ltv_scan_pipeline_host", "ltv_status_string", "ltv_last_cuda_error", "ltv_version",
     "ltv_launch_count", "ltv_profile_enable", "ltv_profile_collect", "ltv_scan_observer_response",
     "ltv_observer_row_floats", "ltv_scan_kalman_gains",
     "ltv_scan_constraint_tightening", "ltv_scan_output_feedback_response", "ltv_set_option", "ltv_get_option",
+    "ltv_profile_class_name",
 )
 
 
@@ -52,6 +54,8 @@ def _load() -> ctypes.CDLL:
     vp, sz, i, fp = ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int, ctypes.c_void_p
     L.ltv_phi_block_index.restype = ctypes.c_longlong
     L.ltv_phi_block_index.argtypes = [i, i, i]
+    L.ltv_phi_block_index_layout.restype = ctypes.c_longlong
+    L.ltv_phi_block_index_layout.argtypes = [i, i, i, i]
     L.ltv_scan_workspace_bytes.restype = sz
     L.ltv_scan_workspace_bytes.argtypes = [i, i, i, i, i]
     L.ltv_scan_rollout.restype = i
@@ -131,8 +135,9 @@ def ltv_launch_count() -> int:
     return int(lib.ltv_launch_count())
 
 
-PROFILE_CLASSES = ("rollout", "adjoint", "phi_level0", "phi_combine_tc", "phi_combine_simt", "phi_finalize",
-                   "kalman_gemm", "kalman_simt")
+lib.ltv_profile_class_name.restype = ctypes.c_char_p
+lib.ltv_profile_class_name.argtypes = [ctypes.c_int]
+PROFILE_CLASSES = tuple(lib.ltv_profile_class_name(i).decode() for i in range(12))
 
 
 def ltv_profile_enable(on: bool) -> None:
@@ -165,22 +170,30 @@ def ltv_scan_rollout(A, B, c, x0, u, x_out=None):
     return x_out
 
 
-def ltv_scan_system_response_tube(A, w, phi_out=None, r_out=None, workspace=None, two_norm=False):
-    """Returns (phi[batch,P,n,n] COLUMN_PACKED, r[batch,T,n]).  `workspace`: optional uint8 CUDA tensor.
+def ltv_phi_block_index_layout(T: int, t: int, s: int, layout: int) -> int:
+    return int(lib.ltv_phi_block_index_layout(T, t, s, layout))
+
+
+def ltv_scan_system_response_tube(A, w, phi_out=None, r_out=None, workspace=None, two_norm=False,
+                                  layout=LTV_PHI_COLUMN_PACKED):
+    """Returns (phi, r[batch,T,n]); phi[batch,P,n,n] in COLUMN_PACKED (default, the fast path) or ROW_PACKED order, or
+    phi[batch,T,T,n,n] for LTV_PHI_SQUARE_GRID (cells with s >= t untouched).  `workspace`: optional uint8 CUDA tensor.
     two_norm=True: the row-wise two-norm tube of eq.(12e) with E_s = diag(w_s) instead of the box tube."""
     batch, T, n, _ = A.shape
     P = T * (T - 1) // 2
+    shape = (batch, T, T, n, n) if layout == LTV_PHI_SQUARE_GRID else (batch, P, n, n)
     _dev(A, "A", (batch, T, n, n)); _dev(w, "w", (batch, T, n))
     if phi_out is None:
-        phi_out = torch.empty((batch, P, n, n), device=A.device, dtype=torch.float32)
+        phi_out = torch.empty(shape, device=A.device, dtype=torch.float32)
     if r_out is None:
         r_out = torch.empty((batch, T, n), device=A.device, dtype=torch.float32)
-    _dev(phi_out, "phi_out", (batch, P, n, n)); _dev(r_out, "r_out", (batch, T, n))
-    need = ltv_scan_workspace_bytes(LTV_OP_SYSTEM_RESPONSE_TUBE, batch, T, n, 0)
+    _dev(phi_out, "phi_out", shape); _dev(r_out, "r_out", (batch, T, n))
+    need = ltv_scan_workspace_bytes(LTV_OP_SYSTEM_RESPONSE_TUBE if layout == LTV_PHI_COLUMN_PACKED
+                                    else LTV_OP_SYSTEM_RESPONSE_TUBE_RELAYOUT, batch, T, n, 0)
     if workspace is None:
         workspace = torch.empty(max(need, 16), device=A.device, dtype=torch.uint8)
     st = lib.ltv_scan_system_response_tube(_ptr(A), _ptr(w), _ptr(phi_out), _ptr(r_out), batch, T, n,
-                                           LTV_PHI_COLUMN_PACKED, LTV_TUBE_ROW_2NORM if two_norm else 0,
+                                           layout, LTV_TUBE_ROW_2NORM if two_norm else 0,
                                            _ptr(workspace), workspace.numel(), _stream())
     if st != LTV_OK:
         raise LtvError(st, "ltv_scan_system_response_tube")

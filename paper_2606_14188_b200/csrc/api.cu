@@ -163,6 +163,16 @@ long long ltv_phi_block_index(int T, int t, int s) {
   return phi_colbase(T, s) + (t - s - 1);
 }
 
+long long ltv_phi_block_index_layout(int T, int t, int s, int phi_layout) {
+  if (T < 1 || s < 0 || t <= s || t > T - 1) return -1;
+  switch (phi_layout) {
+    case LTV_PHI_ROW_PACKED: return static_cast<long long>(t) * (t - 1) / 2 + s;
+    case LTV_PHI_SQUARE_GRID: return static_cast<long long>(t) * T + s;
+    case LTV_PHI_COLUMN_PACKED: return phi_colbase(T, s) + (t - s - 1);
+    default: return -1;
+  }
+}
+
 size_t ltv_scan_workspace_bytes(int op, int batch, int T, int n, int m) {
   if (check_dims(batch, T, n, m) != LTV_OK) return 0;
   switch (op) {
@@ -171,6 +181,8 @@ size_t ltv_scan_workspace_bytes(int op, int batch, int T, int n, int m) {
       return 0;
     case LTV_OP_SYSTEM_RESPONSE_TUBE:
       return phi_workspace_bytes(batch, T, n, n);
+    case LTV_OP_SYSTEM_RESPONSE_TUBE_RELAYOUT:
+      return phi_workspace_bytes(batch, T, n, n) + phi_colpacked_bytes(batch, T, n, n);
     case LTV_OP_OBSERVER_RESPONSE:
       if (m < 1 || m > 32) return 0;
       return phi_workspace_bytes(batch, T, n, n + ((m + 3) & ~3));
@@ -267,18 +279,28 @@ int ltv_scan_system_response_tube(const float* A, const float* w, float* phi_out
   if (T > 1 && !phi_out) return LTV_ERR_NULL_PTR;
   int st = check_dims(batch, T, n, 0);
   if (st != LTV_OK) return st;
-  if (phi_layout != LTV_PHI_COLUMN_PACKED || (flags & ~static_cast<unsigned>(LTV_TUBE_ROW_2NORM)) != 0) return LTV_ERR_BAD_DIM;
+  const bool native = phi_layout == LTV_PHI_COLUMN_PACKED;
+  if ((!native && phi_layout != LTV_PHI_ROW_PACKED && phi_layout != LTV_PHI_SQUARE_GRID) ||
+      (flags & ~static_cast<unsigned>(LTV_TUBE_ROW_2NORM)) != 0)
+    return LTV_ERR_BAD_DIM;
   if (misaligned(A) || misaligned(w) || misaligned(phi_out) || misaligned(r_out) || misaligned(workspace))
     return LTV_ERR_ALIGNMENT;
-  const size_t need = phi_workspace_bytes(batch, T, n, n);
+  const size_t need = phi_workspace_bytes(batch, T, n, n) + (native ? 0 : phi_colpacked_bytes(batch, T, n, n));
   if (!workspace) return LTV_ERR_NULL_PTR;
   if (workspace_bytes < need) return LTV_ERR_WORKSPACE_TOO_SMALL;
   int sms = 0;
   st = check_device(&sms);
   if (st != LTV_OK) return st;
-  PhiArgs a{A, w, phi_out, r_out, static_cast<float*>(workspace), batch, T, n, n, (flags & LTV_TUBE_ROW_2NORM) ? 1 : 0};
+  // the scan computes column-packed: straight into phi_out, or into the workspace followed by one block re-ordering copy
+  float* phi_cp = native ? phi_out
+                         : reinterpret_cast<float*>(static_cast<char*>(workspace) + phi_workspace_bytes(batch, T, n, n));
+  PhiArgs a{A, w, phi_cp, r_out, static_cast<float*>(workspace), batch, T, n, n, (flags & LTV_TUBE_ROW_2NORM) ? 1 : 0};
   unsigned long long l = 0;
   cudaError_t e = launch_phi_tube(a, static_cast<cudaStream_t>(cuda_stream), &l);
+  if (e == cudaSuccess && !native && T > 1) {
+    e = launch_phi_relayout(phi_cp, phi_out, batch, T, n, n, phi_layout, sms, static_cast<cudaStream_t>(cuda_stream));
+    if (e == cudaSuccess) ++l;
+  }
   g_launches += l;
   return e == cudaSuccess ? LTV_OK : fail_cuda(e);
 }
@@ -542,6 +564,13 @@ int ltv_profile_enable(int on) {
   p.on.store(on != 0, std::memory_order_release);
   p.used = 0;   // scopes still open on other threads keep their (already captured) events; their record is dropped
   return LTV_OK;
+}
+
+const char* ltv_profile_class_name(int cls) {
+  static const char* const names[LTV_PROFILE_CLASSES] = {
+      "rollout", "adjoint", "phi_level0", "phi_combine_tc", "phi_combine_simt", "phi_finalize", "kalman_gemm",
+      "kalman_simt", "phi_relayout", "vector_pair", "ofb_support", "fused_small"};
+  return (cls >= 0 && cls < LTV_PROFILE_CLASSES) ? names[cls] : nullptr;
 }
 
 int ltv_profile_collect(double* ms_by_class, unsigned long long* launches_by_class) {

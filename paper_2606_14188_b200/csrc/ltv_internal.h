@@ -44,6 +44,11 @@ bool phi_uses_tensor_cores(int n);
 size_t phi_workspace_bytes(int batch, int T, int n, int nc);
 size_t phi_part_bytes(int batch, int T, int n, int nc);
 cudaError_t launch_phi_tube(const PhiArgs& a, cudaStream_t stream, unsigned long long* launches);
+// bytes of a COLUMN_PACKED Phi staging buffer (the scan's native order) and the block re-ordering copy into
+// LTV_PHI_ROW_PACKED / LTV_PHI_SQUARE_GRID
+size_t phi_colpacked_bytes(int batch, int T, int n, int nc);
+cudaError_t launch_phi_relayout(const float* src, float* dst, int batch, int T, int n, int nc, int layout, int num_sms,
+                                cudaStream_t stream);
 
 // Kalman recursion of eq.(13) (kalman.cu)
 struct KalmanArgs {
@@ -93,7 +98,7 @@ int option(int which);
 
 // optional per-kernel timing (ltv_profile_enable): CUDA events recorded on the launch stream around a kernel
 enum ProfClass { kProfRollout = 0, kProfAdjoint, kProfPhiLevel0, kProfPhiCombineTc, kProfPhiCombineSimt,
-                 kProfPhiFinalize, kProfKalmanGemm, kProfKalmanSimt, kProfNumClasses };
+                 kProfPhiFinalize, kProfKalmanGemm, kProfKalmanSimt, kProfPhiRelayout, kProfVectorPair, kProfOfbSupport, kProfFusedSmall, kProfNumClasses };
 struct ProfScope {
   ProfScope(int cls, cudaStream_t s);
   ~ProfScope();

@@ -2,6 +2,7 @@
 // All launches go to one stream in level order; no host synchronisation.
 #include <cuda.h>
 
+#include "../../include/ltv_scan.h"
 #include "ltv_internal.h"
 #include "phi_geom.cuh"
 #include "phi_kernels.h"
@@ -47,6 +48,61 @@ size_t phi_workspace_bytes(int batch, int T, int n, int nc) {
   size_t bytes = phi_part_bytes(batch, T, n, nc);
   if (nc - n > 8) bytes += align_up(static_cast<size_t>(batch) * T * (nc - n) * n * sizeof(float), 256);
   return bytes;
+}
+
+// ------------------------------------------------------------------------------------------ block re-ordering
+// COLUMN_PACKED -> ROW_PACKED (block (t,s) at t(t-1)/2 + s) or SQUARE_GRID (block (t,s) at t T + s of a T x T grid; blocks
+// with s >= t are not touched).  Blocks are contiguous n x n matrices in every layout, so this is a streaming copy of
+// whole blocks: unit = (block, 32 KB chunk), 128-bit loads / stores, read-once / write-once cache hints.
+namespace {
+constexpr int kRelayoutVecs = 2048;   // float4 per unit
+__global__ void __launch_bounds__(256) phi_relayout_kernel(const float4* __restrict__ src, float4* __restrict__ dst,
+                                                           int batch, int T, long long vecs_per_block, int layout) {
+  const int P = T * (T - 1) / 2;
+  const long long cpb = (vecs_per_block + kRelayoutVecs - 1) / kRelayoutVecs;   // chunks per block
+  const long long nunits = static_cast<long long>(batch) * P * cpb;
+  for (long long un = blockIdx.x; un < nunits; un += gridDim.x) {
+    const long long blk = un / cpb;
+    const long long ch = un - blk * cpb;
+    const int b = static_cast<int>(blk / P);
+    const int q = static_cast<int>(blk - static_cast<long long>(b) * P);
+    // invert q = colbase(s) + (t - s - 1): s is the largest column with colbase(s) <= q
+    int s = 0;
+    while (s + 1 < T - 1 && phi_colbase(T, s + 1) <= q) ++s;
+    const int t = s + 1 + (q - static_cast<int>(phi_colbase(T, s)));
+    const long long dblk = (layout == LTV_PHI_ROW_PACKED)
+                               ? static_cast<long long>(b) * P + static_cast<long long>(t) * (t - 1) / 2 + s
+                               : (static_cast<long long>(b) * T + t) * T + s;
+    const float4* sp = src + blk * vecs_per_block + ch * kRelayoutVecs;
+    float4* dp = dst + dblk * vecs_per_block + ch * kRelayoutVecs;
+    const long long lim = vecs_per_block - ch * kRelayoutVecs;
+    const int cnt = lim < kRelayoutVecs ? static_cast<int>(lim) : kRelayoutVecs;
+    float4 v[kRelayoutVecs / 256];
+#pragma unroll
+    for (int j = 0; j < kRelayoutVecs / 256; ++j)
+      if (threadIdx.x + 256 * j < cnt) v[j] = __ldcs(sp + threadIdx.x + 256 * j);
+#pragma unroll
+    for (int j = 0; j < kRelayoutVecs / 256; ++j)
+      if (threadIdx.x + 256 * j < cnt) __stcs(dp + threadIdx.x + 256 * j, v[j]);
+  }
+}
+}  // namespace
+
+size_t phi_colpacked_bytes(int batch, int T, int n, int nc) {
+  const size_t P = static_cast<size_t>(T) * (T - 1) / 2;
+  return align_up(static_cast<size_t>(batch) * P * n * nc * sizeof(float) + 16, 256);
+}
+
+cudaError_t launch_phi_relayout(const float* src, float* dst, int batch, int T, int n, int nc, int layout, int num_sms,
+                                cudaStream_t stream) {
+  if (T < 2) return cudaSuccess;
+  const long long vecs = static_cast<long long>(n) * nc / 4;
+  const long long nunits = static_cast<long long>(batch) * (T * (T - 1) / 2) * ((vecs + kRelayoutVecs - 1) / kRelayoutVecs);
+  long long blocks = nunits < static_cast<long long>(num_sms) * 8 ? nunits : static_cast<long long>(num_sms) * 8;
+  ProfScope prof(kProfPhiRelayout, stream);
+  phi_relayout_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(reinterpret_cast<const float4*>(src),
+                                                                        reinterpret_cast<float4*>(dst), batch, T, vecs, layout);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_phi_tube(const PhiArgs& a, cudaStream_t stream, unsigned long long* launches) {

@@ -69,15 +69,29 @@ def test_host_side_validation_needs_no_gpu(L):
     assert r(odd, None, None, p, None, p, 1, 1, 4, 0, None, 0, None) == 4           # alignment
     s = L.lib.ltv_scan_system_response_tube
     assert s(p, p, p, None, 1, 2, 4, 0, 0, p, 1 << 20, None) == 1                   # NULL r_out
-    assert s(p, p, p, p, 1, 2, 4, 1, 0, p, 1 << 20, None) == 2                      # unknown layout
+    assert s(p, p, p, p, 1, 2, 4, 3, 0, p, 1 << 20, None) == 2                      # unknown layout
     assert s(p, p, p, p, 1, 2, 4, 0, 2, p, 1 << 20, None) == 2                      # unknown flag
     assert s(p, p, p, p, 1, 2, 4, 0, L.LTV_TUBE_ROW_2NORM, p, 8, None) == 5         # known flag passes on
-    assert s(p, p, p, p, 1, 2, 4, 0, 0, p, 8, None) == 5                            # workspace too small
+    for layout in (L.LTV_PHI_ROW_PACKED, L.LTV_PHI_SQUARE_GRID, L.LTV_PHI_COLUMN_PACKED):
+        assert s(p, p, p, p, 1, 2, 4, layout, 0, p, 8, None) == 5                   # workspace too small
+    assert (L.LTV_PHI_ROW_PACKED, L.LTV_PHI_SQUARE_GRID, L.LTV_PHI_COLUMN_PACKED) == (0, 1, 2)   # 0, 1
+    nat = L.ltv_scan_workspace_bytes(L.LTV_OP_SYSTEM_RESPONSE_TUBE, 2, 5, 48, 0)
+    rel = L.ltv_scan_workspace_bytes(L.LTV_OP_SYSTEM_RESPONSE_TUBE_RELAYOUT, 2, 5, 48, 0)
+    assert rel - nat >= 2 * 10 * 48 * 48 * 4                                        # + a column-packed copy of Phi
+    assert L.ltv_phi_block_index_layout(5, 3, 1, L.LTV_PHI_ROW_PACKED) == 4
+    assert L.ltv_phi_block_index_layout(5, 3, 1, L.LTV_PHI_SQUARE_GRID) == 16
+    assert L.ltv_phi_block_index_layout(5, 3, 1, L.LTV_PHI_COLUMN_PACKED) == L.ltv_phi_block_index(5, 3, 1) == 5
+    assert L.ltv_set_option(L.LTV_OPT_PIPELINE_CHUNKS, 2) is None and L.ltv_get_option(L.LTV_OPT_PIPELINE_CHUNKS) == 2
+    L.ltv_set_option(L.LTV_OPT_PIPELINE_CHUNKS, 4)
+    assert L.lib.ltv_set_option(L.LTV_OPT_VECTOR_CLUSTER, 17) == 2 and L.lib.ltv_set_option(9, 1) == 2
+    assert L.ltv_get_option(L.LTV_OPT_VECTOR_CLUSTER) == 0 and L.lib.ltv_get_option(9) == -1
     o = L.lib.ltv_scan_observer_response
     assert o(p, None, p, p, p, p, 1, 2, 4, 2, 0, 0, p, 1 << 20, None) == 1              # NULL Lt
     assert o(p, p, p, p, p, p, 1, 2, 4, 0, 0, 0, p, 1 << 20, None) == 2                 # p = 0
     assert o(p, p, p, p, p, p, 1, 2, 4, 33, 0, 0, p, 1 << 20, None) == 3                # p > 32
-    assert o(p, p, p, p, p, p, 1, 2, 4, 2, 0, 0, p, 8, None) == 5                       # workspace too small
+    assert o(p, p, p, p, p, p, 1, 2, 4, 2, L.LTV_PHI_COLUMN_PACKED, 0, p, 8, None) == 5 # workspace too small
+    assert o(p, p, p, p, p, p, 1, 2, 4, 2, L.LTV_PHI_ROW_PACKED, 0, p, 1 << 20, None) == 2   # observer: native layout only
+    assert o(p, p, p, p, p, p, 1, 2, 4, 2, L.LTV_PHI_COLUMN_PACKED, 4, p, 1 << 20, None) == 2  # unknown flag
     assert L.ltv_observer_row_floats(300, 6) == 308 and L.ltv_observer_row_floats(48, 4) == 52
     assert L.ltv_scan_workspace_bytes(L.LTV_OP_OBSERVER_RESPONSE, 2, 4, 128, 6) > 0
     k = L.lib.ltv_scan_kalman_gains

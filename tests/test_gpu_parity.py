@@ -393,3 +393,53 @@ def test_sharded_device_views_with_odd_item_size(L):
         gus.append(L.ltv_scan_adjoint(m["A"], m["B"], m["g"])[1])
     torch.cuda.synchronize()
     assert torch.equal(torch.cat(xs), x) and torch.equal(torch.cat(gus), gu)
+
+
+@pytest.mark.parametrize("n,T,batch", [(48, 6, 2),       # fp32-FMA combine
+                                       (132, 7, 3),      # tcgen05 combine, ragged k-block and m-tile
+                                       (300, 4, 1)])
+def test_phi_layouts_of_the_survey_boundary(L, n, T, batch):
+    """phi_layout = ROW_PACKED (block index t(t-1)/2 + s, the oracle's own order: no permutation in the
+    test) and SQUARE_GRID ([batch,T,T,n,n], only s < t written).  Both must hold exactly the COLUMN_PACKED result
+    (the re-ordering is a copy) and match the oracle; r is the same in every layout."""
+    import torch
+
+    W = dense_random(batch, T, n, 1, seed=13 * n + T, scale=0.4)
+    A, w = torch.from_numpy(W.A).cuda(), torch.from_numpy(W.w).cuda()
+    P = T * (T - 1) // 2
+    phi_c, r_c = L.ltv_scan_system_response_tube(A, w)
+    phi_r, r_r = L.ltv_scan_system_response_tube(A, w, layout=L.LTV_PHI_ROW_PACKED)
+    grid = torch.full((batch, T, T, n, n), 777.0, device="cuda")
+    phi_g, r_g = L.ltv_scan_system_response_tube(A, w, phi_out=grid, layout=L.LTV_PHI_SQUARE_GRID)
+    torch.cuda.synchronize()
+    ref = O.system_response(W.A)                                # row-packed
+    assert O.rel_err(phi_r.cpu().numpy(), ref) <= TOL
+    assert torch.equal(r_c, r_r) and torch.equal(r_c, r_g)
+    assert O.rel_err(r_c.cpu().numpy(), O.tube(W.A, W.w)) <= TOL
+    g = phi_g.cpu().numpy()
+    for t in range(T):
+        for s in range(T):
+            if s < t:
+                assert L.ltv_phi_block_index_layout(T, t, s, L.LTV_PHI_SQUARE_GRID) == t * T + s
+                assert L.ltv_phi_block_index_layout(T, t, s, L.LTV_PHI_ROW_PACKED) == O.packed_index(t, s)
+                assert L.ltv_phi_block_index_layout(T, t, s, L.LTV_PHI_COLUMN_PACKED) == L.ltv_phi_block_index(T, t, s)
+                assert np.array_equal(g[:, t, s], phi_c[:, L.ltv_phi_block_index(T, t, s)].cpu().numpy())
+                assert np.array_equal(g[:, t, s], phi_r[:, O.packed_index(t, s)].cpu().numpy())
+            else:
+                assert np.all(g[:, t, s] == 777.0)               # untouched
+    assert L.ltv_phi_block_index_layout(T, 0, 0, L.LTV_PHI_ROW_PACKED) == -1
+    assert L.ltv_phi_block_index_layout(T, 1, 0, 7) == -1
+
+
+def test_phi_layout_validation(L):
+    import torch
+
+    W = dense_random(1, 3, 48, 1, seed=5)
+    A, w = torch.from_numpy(W.A).cuda(), torch.from_numpy(W.w).cuda()
+    with pytest.raises(L.LtvError) as e:
+        L.ltv_scan_system_response_tube(A, w, layout=3)
+    assert e.value.status == 2
+    ws = torch.empty(max(16, L.ltv_scan_workspace_bytes(L.LTV_OP_SYSTEM_RESPONSE_TUBE, 1, 3, 48, 0)), dtype=torch.uint8, device="cuda")
+    with pytest.raises(L.LtvError) as e:      # the native workspace is too small for a re-ordered layout
+        L.ltv_scan_system_response_tube(A, w, workspace=ws, layout=L.LTV_PHI_ROW_PACKED)
+    assert e.value.status == 5
