@@ -43,6 +43,8 @@ sequential recursion - "We obtain the solution to (14) by a forward parallel ass
   assemble_output_feedback   Phi^xw = Phibar^x + Phihat^x - Phibar^x M Phihat^x,  Phi^uw = Phibar^u (I - M Phihat^x),      PAPER.md:162-164 eq.(15),
                    Phi^xe = Phihat^y - Phibar^x M Phihat^y,  Phi^ue = -Phibar^u M Phihat^y,  M = I - Z A                 dense block operators
                                                                      (DESIGN.md q20, q21)
+  output_feedback_constraint_tightening   sigma_k[i] = sum_{j<k} ||c_{k,i}^T Phi^w(k,j) E_j||_2 + ||c_{k,i}^T Phi^e(k,j) F~_j||_2,     PAPER.md:144-145 eq.(12d) as
+                   c on [z_k; v_k], Phi^w = [Phi^xw; Phi^uw], Phi^e = [Phi^xe; Phi^ue] of (15)                    printed, both terms (NEXT-4)
   adjoint          lam_T = g_T; lam_t = A_t^T lam_{t+1} + g_t;       PAPER.md:106-110 eq.(10) chained
                    grad_u[t] = B_t^T lam_{t+1}; grad_x0 = A_0^T lam_1   over the horizon; north_star (iii)
 
@@ -57,7 +59,9 @@ tube-containment / adjoint dot-product invariants.  kalman_recursion / riccati_*
 tests/test_oracle_pins_kalman.py (brute-force Gaussian conditioning, information form, DARE fixed point from
 scipy, Lyapunov sum through Phi, Joseph form + gain optimality, scan = recursion, associativity);
 assemble_output_feedback in tests/test_oracle_pins_assembly.py (both achievability identities of (12c), a step-by-step
-simulation of plant + observer + controller, the augmented closed-loop system, the limits L = 0 and K = 0).
+simulation of plant + observer + controller, the augmented closed-loop system, the limits L = 0 and K = 0);
+output_feedback_constraint_tightening there too (worst-case containment with tightness on the simulated loop for state
+AND input rows, identity state rows = the output-feedback tube, K = 0 = the open-loop margins).
 Nothing in this file is "parity unpinned".
 """
 from __future__ import annotations
@@ -203,6 +207,33 @@ def output_feedback_tube(Phixw, Phixe, w, f):
                 ble = Pe[k * n:(k + 1) * n, j * p:(j + 1) * p] @ np.diag(f[j - 1])
                 tau[k] += np.sqrt(np.sum(ble ** 2, axis=1))
     return tau
+
+
+def output_feedback_constraint_tightening(Phixw, Phiuw, Phixe, Phiue, w, f, Hx, Hu):
+    """Constraint-tightening margins of eq.(12d) as printed, BOTH terms, constraint rows acting on
+    the stacked (state, input) pair [z_k; v_k], for one item:
+        sigma_0 = 0;   sigma_k[i] = sum_{j=0}^{k-1} ( || c_{k,i}^T Phi^w(k,j) E_j ||_2 + || c_{k,i}^T Phi^e(k,j) F~_j ||_2 ),
+    c_{k,i}^T = [Hx[k,i,:], Hu[k,i,:]] (n + m entries),  Phi^w(k,j) = [Phi^xw(k,j); Phi^uw(k,j)] ((n+m) x n),
+    Phi^e(k,j) = [Phi^xe(k,j); Phi^ue(k,j)] ((n+m) x p), E_j = diag(w[j]); F~_j = diag(f[j-1]) scales the noise of the
+    measurement of x_{j-1} (DESIGN.md q21: no such term for j = 0).  The dense operators are those of
+    assemble_output_feedback: Phixw [T n, T n], Phiuw [T m, T n], Phixe [T n, T p], Phiue [T m, T p].
+    w[T,n], f[T,p], Hx[T,nc,n], Hu[T,nc,m] -> sigma[T,nc].  One block, one row, one norm at a time."""
+    Pxw, Puw, Pxe, Pue = _f64(Phixw), _f64(Phiuw), _f64(Phixe), _f64(Phiue)
+    w, f, Hx, Hu = _f64(w), _f64(f), _f64(Hx), _f64(Hu)
+    T, n = w.shape
+    p = f.shape[1]
+    nc, m = Hu.shape[1], Hu.shape[2]
+    sigma = np.zeros((T, nc))
+    for k in range(1, T):
+        for j in range(k):
+            Pw = np.vstack([Pxw[k * n:(k + 1) * n, j * n:(j + 1) * n], Puw[k * m:(k + 1) * m, j * n:(j + 1) * n]])
+            Pe = np.vstack([Pxe[k * n:(k + 1) * n, j * p:(j + 1) * p], Pue[k * m:(k + 1) * m, j * p:(j + 1) * p]])
+            for i in range(nc):
+                c = np.concatenate([Hx[k, i], Hu[k, i]])
+                sigma[k, i] += np.sqrt(np.sum((c @ Pw @ np.diag(w[j])) ** 2))
+                if j >= 1:
+                    sigma[k, i] += np.sqrt(np.sum((c @ Pe @ np.diag(f[j - 1])) ** 2))
+    return sigma
 
 
 # --------------------------------------------------------------------------- Kalman recursion (13), Riccati scan (16)(17)

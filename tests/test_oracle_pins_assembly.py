@@ -150,3 +150,82 @@ def test_output_feedback_tube_without_feedback_is_the_row2norm_tube():
     w, f = np.random.default_rng(1).uniform(0.1, 1.0, (T, n)), np.ones((T, p))
     Pxw, _, Pxe, _ = O.assemble_output_feedback(A, *_operators(A, B, C, 0.0 * K, Lt))
     np.testing.assert_allclose(O.output_feedback_tube(Pxw, Pxe, w, f), O.tube_row2norm_item(A, w), rtol=1e-10, atol=1e-12)
+
+
+# ------------------------------------------------------------------ (12d), both terms, rows on [z; v]
+def _simulate(A, B, C, K, Lt, wt, et):
+    """plant + predictor-form observer + controller u = K xhat, step by step (q21 conventions); returns X[T,n], U[T,m]"""
+    T, n = wt.shape
+    x, xh = wt[0].copy(), np.zeros(n)
+    X, U = [], []
+    for k in range(T):
+        u = K[k] @ xh
+        X.append(x.copy()); U.append(u.copy())
+        if k + 1 < T:
+            y = C[k] @ x + et[k + 1]
+            xh = A[k] @ xh + B[k] @ u - Lt[k] @ (y - C[k] @ xh)
+            x = A[k] @ x + B[k] @ u + wt[k + 1]
+    return np.array(X), np.array(U)
+
+
+def test_closed_loop_constraint_margins_contain_the_simulated_loop_and_are_tight():
+    """(12d): with w~_j = E_j d_j, e~_j = F~_j g_j, ||d_j||_2, ||g_j||_2 <= 1 injected at steps j < k only, the SIMULATED
+    closed loop obeys c^T [x_k; u_k] <= sigma_k[i]; the aligned disturbances reach it.  Rows mix state and input."""
+    T, n, m, p, nc = 6, 4, 2, 2, 3
+    A, B, C, K, Lt = _setup(T, n, m, p, 21)
+    rng = np.random.default_rng(22)
+    w, f = rng.uniform(0.1, 1.0, (T, n)), rng.uniform(0.1, 1.0, (T, p))
+    Hx, Hu = rng.normal(size=(T, nc, n)), rng.normal(size=(T, nc, m))
+    Pxw, Puw, Pxe, Pue = O.assemble_output_feedback(A, *_operators(A, B, C, K, Lt))
+    sig = O.output_feedback_constraint_tightening(Pxw, Puw, Pxe, Pue, w, f, Hx, Hu)
+    assert np.all(sig[0] == 0.0) and np.all(sig[1:] > 0.0)
+    for k in (2, T - 1):
+        for i in range(nc):
+            wt, et = np.zeros((T, n)), np.zeros((T, p))
+            for j in range(k):
+                rw = (Hx[k, i] @ Pxw[k * n:(k + 1) * n, j * n:(j + 1) * n] + Hu[k, i] @ Puw[k * m:(k + 1) * m, j * n:(j + 1) * n]) * w[j]
+                wt[j] = w[j] * rw / np.linalg.norm(rw)
+                if j >= 1:
+                    re = (Hx[k, i] @ Pxe[k * n:(k + 1) * n, j * p:(j + 1) * p] + Hu[k, i] @ Pue[k * m:(k + 1) * m, j * p:(j + 1) * p]) * f[j - 1]
+                    et[j] = f[j - 1] * re / np.linalg.norm(re)
+            X, U = _simulate(A, B, C, K, Lt, wt, et)
+            val = Hx[k, i] @ X[k] + Hu[k, i] @ U[k]
+            assert abs(val - sig[k, i]) <= 1e-11 * sig[k, i]
+        for _ in range(20):
+            d = rng.normal(size=(T, n)); d /= np.maximum(1.0, np.linalg.norm(d, axis=1, keepdims=True))
+            g = rng.normal(size=(T, p)); g /= np.maximum(1.0, np.linalg.norm(g, axis=1, keepdims=True))
+            wt, et = w * d, np.vstack([np.zeros((1, p)), f[:-1] * g[1:]])
+            wt[k:] = 0.0
+            et[k:] = 0.0
+            X, U = _simulate(A, B, C, K, Lt, wt, et)
+            assert np.all(np.abs(Hx[k] @ X[k] + Hu[k] @ U[k]) <= sig[k] * (1 + 1e-12))
+
+
+def test_closed_loop_constraint_margins_special_cases():
+    T, n, m, p = 5, 4, 2, 2
+    A, B, C, K, Lt = _setup(T, n, m, p, 23)
+    rng = np.random.default_rng(24)
+    w, f = rng.uniform(0.1, 1.0, (T, n)), rng.uniform(0.1, 1.0, (T, p))
+    ops = O.assemble_output_feedback(A, *_operators(A, B, C, K, Lt))
+    # identity state rows, no input part: the output-feedback tube (12e)
+    Hx = np.broadcast_to(np.eye(n), (T, n, n))
+    sig = O.output_feedback_constraint_tightening(*ops, w, f, Hx, np.zeros((T, n, m)))
+    np.testing.assert_allclose(sig, O.output_feedback_tube(ops[0], ops[2], w, f), rtol=1e-12, atol=0)
+    # input rows only: scalar loops over the blocks of Phi^uw, Phi^ue
+    Hu = rng.normal(size=(T, 3, m))
+    sig = O.output_feedback_constraint_tightening(*ops, w, f, np.zeros((T, 3, n)), Hu)
+    for k in range(T):
+        for i in range(3):
+            acc = 0.0
+            for j in range(k):
+                s1 = sum((sum(Hu[k, i, a] * ops[1][k * m + a, j * n + c] for a in range(m)) * w[j, c]) ** 2 for c in range(n))
+                acc += np.sqrt(s1)
+                if j >= 1:
+                    s2 = sum((sum(Hu[k, i, a] * ops[3][k * m + a, j * p + q] for a in range(m)) * f[j - 1, q]) ** 2 for q in range(p))
+                    acc += np.sqrt(s2)
+            assert abs(acc - sig[k, i]) <= 1e-12 * max(1.0, acc)
+    # no feedback (K = 0): Phi^u = 0, Phi^xe = 0, Phi^xw = open loop -> the open-loop margins of constraint_tightening
+    ops0 = O.assemble_output_feedback(A, *_operators(A, B, C, 0.0 * K, Lt))
+    Hx = rng.normal(size=(T, 3, n))
+    sig0 = O.output_feedback_constraint_tightening(*ops0, w, f, Hx, Hu)
+    np.testing.assert_allclose(sig0, O.constraint_tightening_item(A, w, Hx), rtol=1e-10, atol=1e-12)
