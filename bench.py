@@ -465,6 +465,14 @@ def next_rows(B, L, W, steps):
     out["output_feedback"] = dict(p=p, ms=ms, blocks_per_s=batch * B.world * P / (ms * 1e-3))
     del wsf
     torch.cuda.empty_cache()
+    # NEXT-4 / NEXT-2: input-side responses of (15) + closed-loop margins (12d), both terms, rows on [z; v]
+    Hu = torch.randn((batch, T, 6, m), device=dev, generator=gen)
+    wsq = torch.empty(L.lib.ltv_scan_output_feedback_constraints_workspace_bytes(batch, T, n, m, 6), dtype=torch.uint8, device=dev)
+    ms = timed(lambda: L.ltv_scan_output_feedback_constraints(d["A"], d["B"], Kfb, Lt, Cm, d["w"], ff, Hc, Hu, workspace=wsq), steps)
+    out["output_feedback_constraints"] = dict(p=p, nc=6, ms=ms, items_per_s=batch * B.world / (ms * 1e-3),
+                                              note="Phi^uw, Phi^ue of (15) + sigma of (12d): backward sweep on the 2n-state closed loop")
+    del wsq
+    torch.cuda.empty_cache()
     return out
 
 

@@ -244,12 +244,39 @@ LTV_API int ltv_scan_kalman_gains(const float* A, const float* C, const float* e
  * G22 = Phihat^x) and G12(t,s) = G11(t,mid) G12(mid,s) + G12(t,mid) G22(mid,s), so for n >= 96 the library runs two
  * n-state time-parallel scans and one cross scan whose combine accumulates both products in one tcgen05 K loop (4
  * instead of 8 n^3 products per block); for n < 96 it runs the plain scan on the 2n x 2n Jacobians.  One last pass forms
- * Phi^xw (in place over Phibar^x), Phi^xe and the tube (deterministic).  A general Phibar and the low-rank form of (15)
- * are not built.  n <= 4096.  Workspace: ltv_scan_workspace_bytes(LTV_OP_OUTPUT_FEEDBACK, batch, T, n, 0). */
+ * Phi^xw (in place over Phibar^x), Phi^xe and the tube (deterministic).  The input-side operators Phi^uw, Phi^ue of (15)
+ * come from ltv_scan_output_feedback_constraints (below).  n <= 4096.  Workspace: ltv_scan_workspace_bytes(LTV_OP_OUTPUT_FEEDBACK, batch, T, n, 0). */
 LTV_API int ltv_scan_output_feedback_response(const float* A, const float* B, const float* Kfb, const float* Lt,
                                               const float* C, const float* w, const float* f, float* phi_xw_out,
                                               float* phi_xe_out, float* tau_out, int batch, int T, int n, int m, int p,
                                               unsigned flags, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Input-side output-feedback responses of eq.(15) and the constraint-tightening margins of eq.(12d) with BOTH terms and
+ * constraint rows on the stacked pair [z_k; v_k], for the same
+ * gain-defined controller as ltv_scan_output_feedback_response (u_k = Kfb_k xhat_k, predictor-form observer):
+ *     Phi^uw(k,j) = Kfb_k (Phi^xw(k,j) - Phihat^x(k,j)),    Phi^ue(k,j) = Kfb_k (Phi^xe(k,j) - Phihat^x(k,j) Lt_{j-1}),
+ *     sigma_0 = 0;  sigma_k[i] = sum_{j<k} || c_{k,i}^T [Phi^xw; Phi^uw](k,j) diag(w_j) ||_2
+ *                              + sum_{1<=j<k} || c_{k,i}^T [Phi^xe; Phi^ue](k,j) diag(f_{j-1}) ||_2,   c_{k,i}^T = [Hx[b,k,i,:], Hu[b,k,i,:]]
+ * (0 <= j < k <= T-1; the blocks equal Phibar^u (I - M Phihat^x) and -Phibar^u M Phihat^y of (15): pinned in the oracle tests).
+ *   A, B, Kfb, Lt, C, w, f   as in ltv_scan_output_feedback_response (all required, m >= 1, 1 <= p <= 32)
+ *   Hx         device [batch,T,nc,n]   state part of the constraint rows (Hx[b,0] is not read); required iff nc > 0
+ *   Hu         device [batch,T,nc,m]   input part of the constraint rows; required iff nc > 0
+ *   phi_uw_out device [batch,P,m,n]    block (k,j) in COLUMN_PACKED order (ltv_phi_block_index); may be NULL
+ *   phi_ue_out device [batch,P,m,p]    same order; blocks with j = 0 are zero; may be NULL
+ *   sigma_out  device [batch,T,nc]     required iff nc > 0
+ *   flags      must be 0
+ * Method: a row s^T on xi = (x, x - xhat) propagates backwards as psi(k,j) = psi(k,j+1) A_aug,j with the augmented closed-
+ * loop Jacobian A_aug = [[A + B Kfb, -B Kfb], [0, A + Lt C]]; constraint row i of step k starts from
+ * [Hx + Hu Kfb_k | -Hu Kfb_k], row a of the input response from [Kfb_k[a] | -Kfb_k[a]]; then c^T Phi^w(k,j) = psi1 + psi2 and
+ * c^T Phi^e(k,j) = psi2 Lt_{j-1}.  One backward sweep over j carries the stack of the rows of all k > j through one batched
+ * GEMM per step ((T-1-j)(nc + m) rows of 2n floats; tcgen05 3xTF32 for 2n >= 96) - no Phi is formed or read.  Deterministic.
+ * 2n <= 8192, batch <= 65535.  Workspace: ltv_scan_output_feedback_constraints_workspace_bytes(batch, T, n, m, nc). */
+LTV_API size_t ltv_scan_output_feedback_constraints_workspace_bytes(int batch, int T, int n, int m, int nc);
+LTV_API int ltv_scan_output_feedback_constraints(const float* A, const float* B, const float* Kfb, const float* Lt,
+                                                 const float* C, const float* w, const float* f, const float* Hx,
+                                                 const float* Hu, float* phi_uw_out, float* phi_ue_out, float* sigma_out,
+                                                 int batch, int T, int n, int m, int p, int nc, unsigned flags,
+                                                 void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* One pass of the whole hot path from HOST buffers: copies A, B, c, x0, u, w, g host->device into
  * `workspace` (device, >= ltv_scan_workspace_bytes(LTV_OP_PIPELINE_HOST, ...)), runs the three calls above

@@ -35,7 +35,7 @@ EXPORTS = (
     "ltv_launch_count", "ltv_profile_enable", "ltv_profile_collect", "ltv_scan_observer_response",
     "ltv_observer_row_floats", "ltv_scan_kalman_gains",
     "ltv_scan_constraint_tightening", "ltv_scan_output_feedback_response", "ltv_set_option", "ltv_get_option",
-    "ltv_profile_class_name",
+    "ltv_profile_class_name", "ltv_scan_output_feedback_constraints", "ltv_scan_output_feedback_constraints_workspace_bytes",
 )
 
 
@@ -74,6 +74,10 @@ def _load() -> ctypes.CDLL:
     L.ltv_scan_constraint_tightening.argtypes = [fp] * 4 + [i] * 4 + [ctypes.c_uint, vp, sz, vp]
     L.ltv_scan_output_feedback_response.restype = i
     L.ltv_scan_output_feedback_response.argtypes = [fp] * 10 + [i] * 5 + [ctypes.c_uint, vp, sz, vp]
+    L.ltv_scan_output_feedback_constraints.restype = i
+    L.ltv_scan_output_feedback_constraints.argtypes = [fp] * 12 + [i] * 6 + [ctypes.c_uint, vp, sz, vp]
+    L.ltv_scan_output_feedback_constraints_workspace_bytes.restype = sz
+    L.ltv_scan_output_feedback_constraints_workspace_bytes.argtypes = [i] * 5
     L.ltv_observer_row_floats.restype = i
     L.ltv_observer_row_floats.argtypes = [i, i]
     L.ltv_set_option.restype = i
@@ -270,6 +274,31 @@ def ltv_scan_output_feedback_response(A, B, Kfb, Lt, C, w, f, want_xe=True, work
     if st != LTV_OK:
         raise LtvError(st, "ltv_scan_output_feedback_response")
     return phi_xw, phi_xe, tau
+
+
+def ltv_scan_output_feedback_constraints(A, B, Kfb, Lt, C, w, f, Hx=None, Hu=None, want_inputs=True, workspace=None):
+    """Input-side responses of eq.(15) and the closed-loop margins of eq.(12d), both terms, rows on [z; v]: returns
+    (phi_uw[batch,P,m,n] | None, phi_ue[batch,P,m,p] | None, sigma[batch,T,nc] | None), blocks in COLUMN_PACKED order.
+    Hx[batch,T,nc,n], Hu[batch,T,nc,m] (both or neither)."""
+    batch, T, n, _ = A.shape
+    m, p = B.shape[-1], C.shape[2]
+    P = T * (T - 1) // 2
+    nc = 0 if Hx is None else Hx.shape[2]
+    _dev(A, "A", (batch, T, n, n)); _dev(B, "B", (batch, T, n, m)); _dev(Kfb, "Kfb", (batch, T, m, n))
+    _dev(Lt, "Lt", (batch, T, n, p)); _dev(C, "C", (batch, T, p, n)); _dev(w, "w", (batch, T, n)); _dev(f, "f", (batch, T, p))
+    _dev(Hx, "Hx", (batch, T, nc, n)); _dev(Hu, "Hu", (batch, T, nc, m))
+    phi_uw = torch.empty((batch, P, m, n), device=A.device, dtype=torch.float32) if want_inputs else None
+    phi_ue = torch.empty((batch, P, m, p), device=A.device, dtype=torch.float32) if want_inputs else None
+    sigma = torch.empty((batch, T, nc), device=A.device, dtype=torch.float32) if nc > 0 else None
+    need = int(lib.ltv_scan_output_feedback_constraints_workspace_bytes(batch, T, n, m, nc))
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), device=A.device, dtype=torch.uint8)
+    st = lib.ltv_scan_output_feedback_constraints(_ptr(A), _ptr(B), _ptr(Kfb), _ptr(Lt), _ptr(C), _ptr(w), _ptr(f), _ptr(Hx),
+                                                  _ptr(Hu), _ptr(phi_uw), _ptr(phi_ue), _ptr(sigma), batch, T, n, m, p, nc, 0,
+                                                  _ptr(workspace), workspace.numel(), _stream())
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_output_feedback_constraints")
+    return phi_uw, phi_ue, sigma
 
 
 def ltv_scan_kalman_gains(A, C, e, f, Pi0, Lt_out=None, Pi_out=None, workspace=None, mode=0):

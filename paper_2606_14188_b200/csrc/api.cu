@@ -415,6 +415,41 @@ int ltv_scan_output_feedback_response(const float* A, const float* B, const floa
   return err == cudaSuccess ? LTV_OK : fail_cuda(err);
 }
 
+size_t ltv_scan_output_feedback_constraints_workspace_bytes(int batch, int T, int n, int m, int nc) {
+  if (check_dims(batch, T, n, m) != LTV_OK || check_dims(batch, T, 2 * n, 0) != LTV_OK || m < 1 || nc < 0) return 0;
+  if (static_cast<long long>(batch) * T * (nc + m) >= (1ll << 31) / (2 * n)) return 0;
+  return ofb_constraints_workspace_bytes(batch, T, n, nc, m);
+}
+
+int ltv_scan_output_feedback_constraints(const float* A, const float* B, const float* Kfb, const float* Lt, const float* C,
+                                         const float* w, const float* f, const float* Hx, const float* Hu,
+                                         float* phi_uw_out, float* phi_ue_out, float* sigma_out, int batch, int T, int n,
+                                         int m, int p, int nc, unsigned flags, void* workspace, size_t workspace_bytes,
+                                         void* cuda_stream) {
+  if (!A || !B || !Kfb || !Lt || !C || !w || !f || !workspace) return LTV_ERR_NULL_PTR;
+  if (nc > 0 && (!Hx || !Hu || !sigma_out)) return LTV_ERR_NULL_PTR;
+  int st = check_dims(batch, T, n, m);
+  if (st != LTV_OK) return st;
+  if (m < 1 || p < 1 || nc < 0 || flags != 0) return LTV_ERR_BAD_DIM;
+  if (p > 32 || grid_yz_overflow(batch)) return LTV_ERR_UNSUPPORTED_SHAPE;
+  st = check_dims(batch, T, 2 * n, 0);   // the sweep runs on 2n states
+  if (st != LTV_OK) return st;
+  if (static_cast<long long>(batch) * T * (nc + m) >= (1ll << 31) / (2 * n)) return LTV_ERR_UNSUPPORTED_SHAPE;
+  if (misaligned(A) || misaligned(B) || misaligned(Kfb) || misaligned(Lt) || misaligned(C) || misaligned(w) ||
+      misaligned(f) || misaligned(Hx) || misaligned(Hu) || misaligned(phi_uw_out) || misaligned(phi_ue_out) ||
+      misaligned(sigma_out) || misaligned(workspace))
+    return LTV_ERR_ALIGNMENT;
+  if (workspace_bytes < ofb_constraints_workspace_bytes(batch, T, n, nc, m)) return LTV_ERR_WORKSPACE_TOO_SMALL;
+  int sms = 0;
+  st = check_device(&sms);
+  if (st != LTV_OK) return st;
+  OfbConArgs a{A, B, Kfb, Lt, C, w, f, Hx, Hu, phi_uw_out, phi_ue_out, nc > 0 ? sigma_out : nullptr, batch, T, n, m, p, nc, workspace};
+  unsigned long long l = 0;
+  cudaError_t err = launch_ofb_constraints(a, static_cast<cudaStream_t>(cuda_stream), &l);
+  g_launches += l;
+  return err == cudaSuccess ? LTV_OK : fail_cuda(err);
+}
+
 int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float* c_host, const float* x0_host,
                            const float* u_host, const float* w_host, const float* g_host, float* x_host,
                            float* phi_host, float* r_host, float* lambda_host, float* grad_u_host,

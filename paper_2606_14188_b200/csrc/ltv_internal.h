@@ -85,6 +85,16 @@ struct OfbArgs {
 size_t ofb_workspace_bytes(int batch, int T, int n);
 cudaError_t launch_output_feedback(const OfbArgs& a, cudaStream_t stream, unsigned long long* launches);
 
+// Input-side responses of eq.(15) and closed-loop margins of eq.(12d) (output_feedback.cu)
+struct OfbConArgs {
+  const float *A, *B, *Kfb, *Lt, *C, *w, *f, *Hx, *Hu;   // Hx, Hu null iff nc == 0
+  float *phi_uw, *phi_ue, *sigma;                        // each may be null
+  int batch, T, n, m, p, nc;
+  void* workspace;
+};
+size_t ofb_constraints_workspace_bytes(int batch, int T, int n, int nc, int m);
+cudaError_t launch_ofb_constraints(const OfbConArgs& a, cudaStream_t stream, unsigned long long* launches);
+
 // Cluster size (CTAs per item, 1..16, any integer) for the two vector kernels.  max_active[C] = clusters of C CTAs
 // that can be resident at once (cudaOccupancyMaxActiveClusters; 0 = not launchable).  Minimises a simple
 // time model over the waves of clusters: an SM streams ~70 GB/s, the device ~6.5 TB/s (both measured).

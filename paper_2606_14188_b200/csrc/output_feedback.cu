@@ -184,6 +184,109 @@ __global__ void __launch_bounds__(256) ofb_extract_kernel(const float* P1, const
 
 size_t carve(size_t floats) { return align_up(floats * sizeof(float), 256); }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Closed-loop backward sweep (ltv_scan_output_feedback_constraints): input-side responses of eq.(15) and both terms of
+// the margins (12d).  A row s^T acting on xi_k = (x_k, x_k - xhat_k) propagates as psi(k,j) = psi(k,j+1) A_aug,j with
+// psi(k,k) = s^T.  For a constraint row c = [hx, hu] on [z_k; v_k] (u = K xhat = K [I -I] xi): s = [hx + hu K_k | -hu K_k];
+// for row a of the input response: s = [K_k[a] | -K_k[a]].  With psi = [psi1 | psi2] (n floats each):
+//     c^T Phi^w(k,j) = psi1 + psi2  (= psi(k,j) [I; I]),       c^T Phi^e(k,j) = psi2 Lt_{j-1}  (j >= 1),
+// and the same two expressions are rows of Phi^uw(k,j), Phi^ue(k,j) for the K rows.
+
+// start rows: X[(k-1)&1][b][(T-1-k) nr + i][0 .. 2n), k = 1 .. T-1, i < nr = nc + mu (mu = m if the input responses are
+// wanted, else 0); sigma[b][k][:] = 0.  grid (T, batch), 256 threads.
+__global__ void __launch_bounds__(256) cls_prefill_kernel(const float* __restrict__ Hx, const float* __restrict__ Hu,
+                                                          const float* __restrict__ Kfb, float* __restrict__ X0,
+                                                          float* __restrict__ X1, float* __restrict__ sigma, int T, int n,
+                                                          int m, int nc, int mu, int rmax) {
+  const int k = blockIdx.x, b = blockIdx.y;
+  const int nr = nc + mu, n2 = 2 * n;
+  if (sigma != nullptr)
+    for (int i = threadIdx.x; i < nc; i += 256) sigma[(static_cast<size_t>(b) * T + k) * nc + i] = 0.f;
+  if (k == 0) return;
+  float* X = ((k - 1) & 1) ? X1 : X0;
+  float* dst = X + (static_cast<size_t>(b) * rmax + static_cast<size_t>(T - 1 - k) * nr) * n2;
+  const size_t bk = static_cast<size_t>(b) * T + k;
+  const float* Kk = Kfb + bk * m * n;
+  for (int e = threadIdx.x; e < nr * n; e += 256) {
+    const int i = e / n, c = e - i * n;
+    float s1, s2;
+    if (i < nc) {
+      const float* hu = Hu + (bk * nc + i) * m;
+      float hk = 0.f;
+      for (int a = 0; a < m; ++a) hk = fmaf(__ldg(hu + a), __ldg(Kk + static_cast<size_t>(a) * n + c), hk);
+      s1 = __ldg(Hx + (bk * nc + i) * n + c) + hk;
+      s2 = -hk;
+    } else {
+      s1 = __ldg(Kk + static_cast<size_t>(i - nc) * n + c);
+      s2 = -s1;
+    }
+    dst[static_cast<size_t>(i) * n2 + c] = s1;
+    dst[static_cast<size_t>(i) * n2 + n + c] = s2;
+  }
+}
+
+// after the GEMM of step j: warp per stacked row (k, i) of X = [psi(T-1,j); ..; psi(j+1,j)].  Constraint rows add the two
+// norms of (12d) to sigma[b][k][i] (one owner per entry and launch, launches stream-ordered: deterministic); K rows are
+// written out as rows of Phi^uw(k,j) (n floats) and Phi^ue(k,j) (p floats).  grid (ceil(rows/8), batch).
+__global__ void __launch_bounds__(256) cls_post_kernel(const float* __restrict__ X, const float* __restrict__ Ltt,
+                                                       const float* __restrict__ w, const float* __restrict__ f,
+                                                       float* __restrict__ sigma, float* __restrict__ phi_uw,
+                                                       float* __restrict__ phi_ue, int T, int n, int m, int p, int nc,
+                                                       int mu, int rmax, int rows, int j) {
+  const int b = blockIdx.y;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int row = blockIdx.x * 8 + warp;
+  if (row >= rows) return;
+  const int nr = nc + mu, n4 = n >> 2;
+  const int k = T - 1 - row / nr, i = row % nr;
+  const float4* p1 = reinterpret_cast<const float4*>(X + (static_cast<size_t>(b) * rmax + row) * 2 * n);
+  const float4* p2 = p1 + n4;
+  const size_t P = static_cast<size_t>(T) * (T - 1) / 2;
+  const size_t blk = static_cast<size_t>(b) * P + phi_colbase(T, j) + (k - j - 1);
+  const bool krow = i >= nc;
+  const float4* w4 = reinterpret_cast<const float4*>(w + (static_cast<size_t>(b) * T + j) * n);
+  float4* uw = (krow && phi_uw != nullptr) ? reinterpret_cast<float4*>(phi_uw + (blk * m + (i - nc)) * n) : nullptr;
+  float s1 = 0.f;
+  for (int c = lane; c < n4; c += 32) {
+    const float4 a = p1[c], h = p2[c];
+    const float4 x = make_float4(a.x + h.x, a.y + h.y, a.z + h.z, a.w + h.w);
+    if (uw != nullptr) uw[c] = x;
+    if (!krow) {
+      const float4 ww = __ldg(w4 + c);
+      const float e0 = x.x * ww.x, e1 = x.y * ww.y, e2 = x.z * ww.z, e3 = x.w * ww.w;
+      s1 = fmaf(e0, e0, fmaf(e1, e1, fmaf(e2, e2, fmaf(e3, e3, s1))));
+    }
+  }
+  float s2 = 0.f;
+  if (j >= 1) {
+    const float4* L4 = reinterpret_cast<const float4*>(Ltt + (static_cast<size_t>(b) * T + (j - 1)) * p * n);
+    const float* fj = f + (static_cast<size_t>(b) * T + (j - 1)) * p;
+    for (int q = 0; q < p; ++q) {
+      float y = 0.f;
+      for (int c = lane; c < n4; c += 32) {
+        const float4 h = p2[c];
+        const float4 l = __ldg(L4 + static_cast<size_t>(q) * n4 + c);
+        y = fmaf(h.x, l.x, fmaf(h.y, l.y, fmaf(h.z, l.z, fmaf(h.w, l.w, y))));
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) y += __shfl_xor_sync(0xffffffffu, y, o);
+      if (krow) {
+        if (phi_ue != nullptr && lane == 0) phi_ue[(blk * m + (i - nc)) * p + q] = y;
+      } else {
+        const float v = y * __ldg(fj + q);
+        s2 = fmaf(v, v, s2);
+      }
+    }
+  } else if (krow && phi_ue != nullptr && lane < p) {
+    phi_ue[(blk * m + (i - nc)) * p + lane] = 0.f;
+  }
+  if (!krow) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+    if (lane == 0) sigma[(static_cast<size_t>(b) * T + k) * nc + i] += sqrtf(s1) + sqrtf(s2);
+  }
+}
+
 }  // namespace
 
 static bool ofb_structured(int n) { return phi_uses_tensor_cores(n) && env_int("OFB_AUGMENTED", 0) == 0; }
@@ -273,6 +376,86 @@ cudaError_t launch_output_feedback(const OfbArgs& a, cudaStream_t stream, unsign
                           2 * n, static_cast<const float*>(Ltt), a.w, a.f, a.phi_xw, a.phi_xe, a.tau, T, n, a.p)) != cudaSuccess)
     return e;
   ++*launches;
+  return cudaSuccess;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// ltv_scan_output_feedback_constraints: Phi^uw, Phi^ue of eq.(15) and the closed-loop margins of eq.(12d), both terms.
+// One backward sweep over j on the 2n-state augmented closed loop carries the stack of all start rows with k > j,
+//     X_j = [X_{j+1}; S_{j+1}] A_aug,j        ((T-1-j) nr rows of 2n floats, nr = nc + m),
+// as one batched GEMM per step (MODE 1 of the tcgen05 3xTF32 kernel for 2n >= 96, fp32 FMA below), followed by
+// cls_post_kernel.  Phi_aug is never formed: 2 (2n)^2 nr (T-1-j) flop per step.
+size_t ofb_constraints_workspace_bytes(int batch, int T, int n, int nc, int m) {
+  const size_t b = batch, t = T, nn = n, n2 = 2 * nn;
+  const size_t rmax = static_cast<size_t>(T > 1 ? T - 1 : 1) * (nc + m);
+  return carve(b * t * 32 * nn) + carve(b * t * n2 * n2) + 2 * carve(b * rmax * n2);
+}
+
+cudaError_t launch_ofb_constraints(const OfbConArgs& a, cudaStream_t stream, unsigned long long* launches) {
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int batch = a.batch, T = a.T, n = a.n, n2 = 2 * a.n, nc = a.nc;
+  const int mu = (a.phi_uw != nullptr || a.phi_ue != nullptr) ? a.m : 0;
+  const int nr = nc + mu;
+  const int rmax = (T > 1 ? T - 1 : 1) * (nc + a.m);   // sized as the workspace query (which does not know mu)
+  const size_t b = batch, t = T, nn = n;
+  char* cur = static_cast<char*>(a.workspace);
+  float* Ltt = reinterpret_cast<float*>(cur); cur += carve(b * t * 32 * nn);
+  float* Aaug = reinterpret_cast<float*>(cur); cur += carve(b * t * n2 * static_cast<size_t>(n2));
+  float* X[2];
+  X[0] = reinterpret_cast<float*>(cur); cur += carve(b * rmax * n2);
+  X[1] = reinterpret_cast<float*>(cur);
+  cudaError_t e;
+  {
+    ProfScope prof(kProfOfbSupport, stream);
+    ofb_build_aug_kernel<<<dim3(batch * T, (n + 31) / 32), 256, 0, stream>>>(a.A, a.B, a.Kfb, a.Lt, a.C, Aaug, Ltt, n, a.m, a.p);
+  }
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  {
+    ProfScope prof(kProfOfbSupport, stream);
+    cls_prefill_kernel<<<dim3(T, batch), 256, 0, stream>>>(a.Hx, a.Hu, a.Kfb, X[0], X[1], a.sigma, T, n, a.m, nc, mu, rmax);
+  }
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  *launches += 2;
+  if (T < 2 || nr == 0) return cudaSuccess;
+
+  const bool tc = phi_uses_tensor_cores(n2);
+  const int nch = phi_pick_nch(n2);
+  BatchedGemm g[2];
+  alignas(64) unsigned char maps[2][1024];
+  for (int q = 0; q < 2; ++q) {   // q = parity of the step: left operand X[q], output X[q ^ 1]
+    g[q] = BatchedGemm{};
+    g[q].L = X[q]; g[q].l_rows = static_cast<long long>(batch) * rmax; g[q].l_row0 = 0; g[q].l_row_stride = rmax;
+    g[q].R = Aaug; g[q].r_blocks = batch * T; g[q].r_blk_stride = T;
+    g[q].D = X[q ^ 1]; g[q].d_blocks = batch; g[q].d_blk0 = 0; g[q].d_blk_stride = 1;
+    g[q].count = batch; g[q].M = rmax; g[q].N = n2; g[q].K = n2; g[q].d_rows = rmax;
+    g[q].transpose_out = 0; g[q].diag = nullptr; g[q].diag_stride = 0;
+    if (tc) {
+      if (phi_tc_maps_size() > sizeof(maps[q])) return cudaErrorInvalidValue;
+      if ((e = bgemm_tc_make_maps(g[q], maps[q])) != cudaSuccess) return e;
+    }
+  }
+  for (int j = T - 2; j >= 0; --j) {
+    const int q = j & 1;
+    const int rows = (T - 1 - j) * nr;
+    g[q].M = rows;
+    g[q].r_blk0 = j;
+    if (tc) {
+      e = launch_bgemm_tc(g[q], nch, maps[q], sms, stream);
+    } else {
+      ProfScope prof(kProfKalmanGemm, stream);
+      e = launch_bgemm_simt(g[q], stream);
+    }
+    if (e != cudaSuccess) return e;
+    {
+      ProfScope prof(kProfOfbSupport, stream);
+      cls_post_kernel<<<dim3((rows + 7) / 8, batch), 256, 0, stream>>>(X[q ^ 1], Ltt, a.w, a.f, a.sigma, a.phi_uw, a.phi_ue, T, n,
+                                                                     a.m, a.p, nc, mu, rmax, rows, j);
+    }
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    *launches += 2;
+  }
   return cudaSuccess;
 }
 

@@ -123,6 +123,17 @@ def test_host_side_validation_needs_no_gpu(L):
     assert need >= 2 * b * (T * (T - 1) // 2) * n * n * 4     # n >= 96: Phihat^x and the cross block (Phibar^x sits in the output)
     need48 = L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, b, T, 48, 0)
     assert need48 >= 4 * b * (T * (T - 1) // 2) * 48 * 48 * 4  # n < 96: Phi of the 2n-state augmented system
+    oc = L.lib.ltv_scan_output_feedback_constraints
+    args7 = (p, p, p, p, p, p, p)
+    assert oc(*args7, p, p, p, p, p, 1, 2, 4, 2, 2, 3, 0, None, 1 << 24, None) == 1         # NULL workspace
+    assert oc(*args7, None, p, p, p, p, 1, 2, 4, 2, 2, 3, 0, p, 1 << 24, None) == 1         # nc > 0 but Hx NULL
+    assert oc(*args7, p, p, p, p, p, 1, 2, 4, 0, 2, 3, 0, p, 1 << 24, None) == 2            # m = 0
+    assert oc(*args7, p, p, p, p, p, 1, 2, 4, 2, 2, 3, 1, p, 1 << 24, None) == 2            # flags
+    assert oc(*args7, p, p, p, p, p, 1, 2, 4, 2, 33, 3, 0, p, 1 << 24, None) == 3           # p > 32
+    assert oc(*args7, p, p, p, p, p, 1, 2, 4, 2, 2, 3, 0, p, 8, None) == 5                  # workspace too small
+    wsb = L.lib.ltv_scan_output_feedback_constraints_workspace_bytes
+    assert wsb(b, T, n, 6, 6) >= b * T * 4 * n * n * 4 + 2 * b * (T - 1) * 12 * 2 * n * 4    # A_aug + two stacks
+    assert wsb(b, T, n, 0, 6) == 0 and wsb(b, T, 4100, 6, 6) == 0
     a = L.lib.ltv_scan_adjoint
     assert a(p, None, p, p, p, None, 1, 2, 4, 2, None, 0, None) == 1                # grad_u wanted, B NULL
     assert a(p, p, None, p, None, None, 1, 2, 4, 2, None, 0, None) == 1             # NULL g

@@ -156,3 +156,73 @@ def test_kalman_gains_to_output_feedback_tube_pipeline(L):
     for b in range(batch):
         _, _, tau_ref = _oracle_ofb(W.A[b], W.B[b], M["C"][b], K[b], Lt_ref[b], w1[b], M["f"][b])
         assert O.rel_err(tau[b].cpu().numpy(), tau_ref) <= TOL
+
+
+def _oracle_all_four(A, B, C, K, Lt):
+    A, B, C, K, Lt = [a.astype(np.float64) for a in (A, B, C, K, Lt)]
+    T, n, _ = A.shape
+    p = C.shape[1]
+    PbX = _dense(O.system_response_item(A + B @ K), T, n)
+    PbU = np.vstack([K[k] @ PbX[k * n:(k + 1) * n] for k in range(T)])
+    PhX = _dense(O.observer_response_item(A, Lt, C)[0], T, n)
+    PhY = np.zeros((T * n, T * p))
+    for j in range(1, T):
+        PhY[:, j * p:(j + 1) * p] = PhX[:, j * n:(j + 1) * n] @ Lt[j - 1]
+    return O.assemble_output_feedback(A, PbX, PbU, PhX, PhY)
+
+
+@pytest.mark.parametrize("n,T,m,p,nc,batch", [(24, 6, 2, 3, 3, 2),     # 2n = 48: fp32-FMA GEMMs
+                                              (48, 7, 3, 4, 5, 1),     # 2n = 96: smallest tensor-core size
+                                              (132, 5, 6, 6, 4, 2),    # ragged tiles
+                                              (100, 4, 1, 1, 1, 1),    # single input / output / constraint
+                                              (64, 9, 4, 20, 2, 1),    # wide observation, longer horizon (parity of the ping-pong)
+                                              (300, 4, 6, 6, 6, 1)])   # C2 state size
+def test_output_feedback_constraints_call(L, n, T, m, p, nc, batch):
+    """ltv_scan_output_feedback_constraints: Phi^uw, Phi^ue of eq.(15) and the margins of eq.(12d) with both terms and
+    rows on [z; v], against the oracle (assemble_output_feedback as printed + output_feedback_constraint_tightening)."""
+    import torch
+
+    items = [_gains(T, n, m, p, seed=11 * n + T + b) for b in range(batch)]
+    A, B, C, K, Lt = [np.stack([it[q] for it in items]) for q in range(5)]
+    rng = np.random.default_rng(n + 1)
+    w = rng.uniform(0.1, 1.0, (batch, T, n)).astype(np.float32)
+    f = rng.uniform(0.1, 1.0, (batch, T, p)).astype(np.float32)
+    Hx = rng.normal(0.0, 1.0, (batch, T, nc, n)).astype(np.float32)
+    Hu = rng.normal(0.0, 1.0, (batch, T, nc, m)).astype(np.float32)
+    d = [torch.from_numpy(a).cuda() for a in (A, B, K, Lt, C, w, f, Hx, Hu)]
+    uw, ue, sig = L.ltv_scan_output_feedback_constraints(*d)
+    _, _, sig_only = L.ltv_scan_output_feedback_constraints(*d, want_inputs=False)
+    uw2, ue2, none = L.ltv_scan_output_feedback_constraints(*d[:7])
+    torch.cuda.synchronize()
+    assert none is None and torch.equal(uw, uw2) and torch.equal(ue, ue2) and torch.equal(sig, sig_only)
+    uw, ue, sig = uw.cpu().numpy(), ue.cpu().numpy(), sig.cpu().numpy()
+    for b in range(batch):
+        Pxw, Puw, Pxe, Pue = _oracle_all_four(A[b], B[b], C[b], K[b], Lt[b])
+        ref_uw = np.stack([Puw[k * m:(k + 1) * m, j * n:(j + 1) * n] for j in range(T - 1) for k in range(j + 1, T)])
+        ref_ue = np.stack([Pue[k * m:(k + 1) * m, j * p:(j + 1) * p] for j in range(T - 1) for k in range(j + 1, T)])
+        assert O.rel_err(uw[b], ref_uw) <= TOL
+        assert O.rel_err(ue[b], ref_ue) <= TOL
+        assert np.all(ue[b, :T - 1] == 0.0)      # column j = 0: no measurement precedes step 0
+        ref_sig = O.output_feedback_constraint_tightening(Pxw, Puw, Pxe, Pue, w[b], f[b], Hx[b], Hu[b])
+        assert O.rel_err(sig[b], ref_sig) <= TOL
+        assert np.all(sig[b, 0] == 0.0)
+
+
+def test_output_feedback_constraints_identity_rows_equal_the_tube_call(L):
+    """Identity state rows, no input part: the margins are the output-feedback tube of (12e) - the two device calls
+    (forward structured scan + extraction vs backward sweep) must agree to rounding."""
+    import torch
+
+    n, T, m, p = 96, 6, 3, 4
+    A, B, C, K, Lt = [a[None] for a in _gains(T, n, m, p, seed=5)]
+    rng = np.random.default_rng(6)
+    w = rng.uniform(0.1, 1.0, (1, T, n)).astype(np.float32)
+    f = rng.uniform(0.1, 1.0, (1, T, p)).astype(np.float32)
+    Hx = np.ascontiguousarray(np.broadcast_to(np.eye(n, dtype=np.float32), (1, T, n, n)))
+    Hu = np.zeros((1, T, n, m), dtype=np.float32)
+    d = [torch.from_numpy(a).cuda() for a in (A, B, K, Lt, C, w, f)]
+    _, _, tau = L.ltv_scan_output_feedback_response(*d)
+    _, _, sig = L.ltv_scan_output_feedback_constraints(*d, torch.from_numpy(Hx).cuda(), torch.from_numpy(Hu).cuda(),
+                                                       want_inputs=False)
+    torch.cuda.synchronize()
+    assert O.rel_err(sig.cpu().numpy(), tau.cpu().numpy()) <= TOL

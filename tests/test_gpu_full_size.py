@@ -280,6 +280,39 @@ def test_full_size_output_feedback_response_vs_oracle(L):
         assert O.rel_err(tau[b].cpu().numpy(), O.output_feedback_tube(Pxw, Pxe, W.w[b], f[b])) <= TOL
 
 
+def test_full_size_output_feedback_constraints_vs_oracle(L):
+    """ltv_scan_output_feedback_constraints on C2-size items (n=300, m=6, p=6, nc=6, whole batch of 64) at T=8, where the
+    oracle's dense operators of (15) fit: every block of Phi^uw, Phi^ue and all margins of (12d) of sampled items."""
+    import torch
+
+    W = generate(config(1, T=8))
+    batch, T, n, m = W.shape
+    p, nc = 6, 6
+    K, Lt, C, f = _ofb_inputs(W, p, seed=79)
+    rng = np.random.default_rng(80)
+    Hx = rng.normal(0.0, 1.0, (batch, T, nc, n)).astype(np.float32)
+    Hu = rng.normal(0.0, 1.0, (batch, T, nc, m)).astype(np.float32)
+    d = [torch.from_numpy(a).cuda() for a in (W.A, W.B, K, Lt, C, W.w, f, Hx, Hu)]
+    uw, ue, sig = L.ltv_scan_output_feedback_constraints(*d)
+    torch.cuda.synchronize()
+    assert bool(torch.all(sig[:, 0] == 0)) and bool(torch.isfinite(sig).all())
+    for b in (0, 45):
+        A64, B64, K64, Lt64, C64 = [a[b].astype(np.float64) for a in (W.A, W.B, K, Lt, C)]
+        PbX = _dense_lower(O.system_response_item(A64 + B64 @ K64), T, n)
+        PbU = np.vstack([K64[k] @ PbX[k * n:(k + 1) * n] for k in range(T)])
+        PhX = _dense_lower(O.system_response_item(A64 + Lt64 @ C64), T, n)
+        PhY = np.zeros((T * n, T * p))
+        for j in range(1, T):
+            PhY[:, j * p:(j + 1) * p] = PhX[:, j * n:(j + 1) * n] @ Lt64[j - 1]
+        Pxw, Puw, Pxe, Pue = O.assemble_output_feedback(A64, PbX, PbU, PhX, PhY)
+        ref_uw = np.stack([Puw[k * m:(k + 1) * m, j * n:(j + 1) * n] for j in range(T - 1) for k in range(j + 1, T)])
+        ref_ue = np.stack([Pue[k * m:(k + 1) * m, j * p:(j + 1) * p] for j in range(T - 1) for k in range(j + 1, T)])
+        assert O.rel_err(uw[b].cpu().numpy(), ref_uw) <= TOL
+        assert O.rel_err(ue[b].cpu().numpy(), ref_ue) <= TOL
+        ref = O.output_feedback_constraint_tightening(Pxw, Puw, Pxe, Pue, W.w[b], f[b], Hx[b], Hu[b])
+        assert O.rel_err(sig[b].cpu().numpy(), ref) <= TOL
+
+
 def test_full_size_output_feedback_response(L):
     """The same call at the full C2 horizon (T=32, whole batch), where the oracle's dense operators of (15) would be
     [9600 x 9600]: a SECOND check only (the oracle-routed test is the one above) - the block row k = T-1 of one item
