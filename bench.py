@@ -324,11 +324,16 @@ def run_workload(B, L, W, name, cfg_index, steps, warmup, phi_on, min_seconds=0.
         ws = torch.empty(max(16, L.ltv_scan_workspace_bytes(L.LTV_OP_SYSTEM_RESPONSE_TUBE, batch, T, n, 0)),
                          dtype=torch.uint8, device=dev)
 
+    outs = dict(x=x, phi=phi, r=r, lam=lam, grad_u=gu, grad_x0=gx0) if phi_on else None
+    fused = bool(phi_on and L.ltv_scan_all_is_fused(batch, T, n, m))
+
     def step():
-        L.ltv_scan_rollout(d["A"], d["B"], d["c"], d["x0"], d["u"], x_out=x)
+        # the whole path in one call: ONE launch for small problems, else rollout + adjoint, then Phi + tube
         if phi_on:
-            L.ltv_scan_system_response_tube(d["A"], d["w"], phi_out=phi, r_out=r, workspace=ws)
-        L.ltv_scan_adjoint(d["A"], d["B"], d["g"], lambda_out=lam, grad_u_out=gu, grad_x0_out=gx0)
+            L.ltv_scan_all(d["A"], d["B"], d["c"], d["x0"], d["u"], d["w"], d["g"], outs=outs, workspace=ws)
+        else:
+            L.ltv_scan_rollout_adjoint(d["A"], d["B"], d["c"], d["x0"], d["u"], d["g"], x_out=x, lambda_out=lam,
+                                       grad_u_out=gu, grad_x0_out=gx0)
 
     warm = max(warmup, 3)
     e0, e1 = _events(torch)
@@ -360,6 +365,9 @@ def run_workload(B, L, W, name, cfg_index, steps, warmup, phi_on, min_seconds=0.
     units = (P if phi_on else 1) * batch * B.world
     clocks = B.sampler.result(window=(t0, t1))
     out = dict(workload=label or name, n=n, m=m, T=T, batch_per_gpu=batch, steps=steps, warmup=warm,
+               route=("ltv_scan_all: ONE fused launch per step (fused_small_kernel)" if fused else
+                      "ltv_scan_all: rollout + adjoint, then Phi levels + tube" if phi_on else "ltv_scan_rollout_adjoint"),
+               us_per_step=ms_step * 1e3,
                ms_per_step=ms_step, timed_region_s=ms_total * 1e-3,
                value=units / (ms_step * 1e-3), unit=UNIT if phi_on else UNIT_C5, gpu_launches=int(launches),
                kernel_ms_per_step={k: round(v[0] / steps, 5) for k, v in prof.items() if v[1]}, clocks=clocks)
@@ -370,10 +378,34 @@ def run_workload(B, L, W, name, cfg_index, steps, warmup, phi_on, min_seconds=0.
         if prof[k][1]:
             ms = prof[k][0] / prof[k][1]
             gbs = bytes_roll / (ms * 1e-3) / 1e9
-            vec[k] = dict(per_s=batch * B.world / (ms * 1e-3), ms=ms, hbm_gbs=gbs, hbm_frac=gbs / B.pk["hbm_gbs"])
+            vec[k] = dict(per_s=batch * B.world / (ms * 1e-3), ms=ms, hbm_gbs=gbs, hbm_frac=gbs / B.pk["hbm_gbs"],
+                          note="inside the concurrent pair: shares the SMs and HBM with the other scan")
+    if prof["vector_pair"][1]:
+        ms = prof["vector_pair"][0] / prof["vector_pair"][1]
+        gbs = 2.0 * bytes_roll / (ms * 1e-3) / 1e9
+        vec["pair"] = dict(per_s=batch * B.world / (ms * 1e-3), ms=ms, hbm_gbs=gbs, hbm_frac=gbs / B.pk["hbm_gbs"],
+                           note="ltv_scan_rollout_adjoint: both scans side by side; bytes = rollout + adjoint (A read twice)")
+    # each scan ALONE on the whole machine (the stand-alone calls), a few launches outside the timed step loop
+    alone = {}
+    for k, fn in (("rollout", lambda: L.ltv_scan_rollout(d["A"], d["B"], d["c"], d["x0"], d["u"], x_out=x)),
+                  ("adjoint", lambda: L.ltv_scan_adjoint(d["A"], d["B"], d["g"], lambda_out=lam, grad_u_out=gu, grad_x0_out=gx0))):
+        for _ in range(2):
+            fn()
+        a0, a1 = _events(torch)
+        reps = 5
+        B.barrier()
+        a0.record()
+        for _ in range(reps):
+            fn()
+        a1.record()
+        B.barrier()
+        ms = B.max_over_ranks(a0.elapsed_time(a1)) / reps
+        gbs = bytes_roll / (ms * 1e-3) / 1e9
+        alone[k] = dict(per_s=batch * B.world / (ms * 1e-3), ms=ms, hbm_gbs=gbs, hbm_frac=gbs / B.pk["hbm_gbs"])
+    vec["alone"] = alone
     out["vector_scans"] = vec
-    out["rollouts_per_s"] = vec.get("rollout", {}).get("per_s")
-    out["adjoints_per_s"] = vec.get("adjoint", {}).get("per_s")
+    out["rollouts_per_s"] = vec.get("pair", {}).get("per_s")
+    out["adjoints_per_s"] = vec.get("pair", {}).get("per_s")
 
     if phi_on and prof["phi_combine_tc"][1] > 0:
         G_blocks = (T - 1) * (T - 2) // 2                                   # GEMM blocks per item
@@ -393,14 +425,26 @@ def run_workload(B, L, W, name, cfg_index, steps, warmup, phi_on, min_seconds=0.
             logical_fp32_tflops=ach / 3.0, kernel_ms_per_step=ms_kernel,
             launches_per_step=prof["phi_combine_tc"][1] / steps,
             share_of_step=ms_kernel / ms_step)
-    elif "rollout" in vec:
-        tr, tr_src = ncu_traffic(cfg_index, "rollout") if label is None else (None, None)
-        out["roofline"] = dict(bound="hbm", kernel="rollout_kernel", achieved=vec["rollout"]["hbm_gbs"],
-                               peak=B.pk["hbm_gbs"], unit="GB/s", frac=vec["rollout"]["hbm_frac"], traffic=tr,
+    elif fused:
+        ms_f = prof["fused_small"][0] / max(prof["fused_small"][1], 1)
+        # latency-bound by construction: the critical path is the chain of T-2 dependent n^3 products of column s = 0 on ONE SM
+        chain_flop = 2.0 * n ** 3 * (T - 2)
+        sm_peak = 128 * 2 * (clocks["sm_mhz"] or 1965) * 1e6          # fp32 FMA lanes of one SM
+        out["roofline"] = dict(bound="alu", kernel="fused_small_kernel (critical path: column s = 0, one SM, fp32 FMA)",
+                               achieved=chain_flop / (ms_f * 1e-3) / 1e9, peak=sm_peak / 1e9, unit="GFLOP/s (one SM)",
+                               frac=chain_flop / (ms_f * 1e-3) / sm_peak, traffic=None, traffic_source=None,
+                               algorithmic="2 n^3 (T-2) flop of the longest column chain over the kernel time; working set fits L2 / shared memory",
+                               peak_source="128 fp32 FMA lanes x 2 flop x sampled SM clock (B300_MICROARCH.md unit counts)",
+                               kernel_ms_per_step=ms_f, share_of_step=ms_f / ms_step)
+    elif "pair" in vec:
+        tr, tr_src = ncu_traffic(cfg_index, "vector_pair") if label is None else (None, None)
+        out["roofline"] = dict(bound="hbm", kernel="rollout_kernel + adjoint_kernel running concurrently (ltv_scan_rollout_adjoint)",
+                               achieved=vec["pair"]["hbm_gbs"],
+                               peak=B.pk["hbm_gbs"], unit="GB/s", frac=vec["pair"]["hbm_frac"], traffic=tr,
                                traffic_source=tr_src,
-                               algorithmic="bytes = batch x (T(n^2 + nm + n + m) + n + Tn) x 4 per launch",
+                               algorithmic="bytes = 2 x batch x (T(n^2 + nm + n + m) + n + Tn) x 4 per step (each scan reads A once)",
                                peak_source=B.pk["source"] + " copy bandwidth (MEASURED_PEAKS.json hbm_gbs)",
-                               kernel_ms_per_step=vec["rollout"]["ms"], share_of_step=vec["rollout"]["ms"] / ms_step)
+                               kernel_ms_per_step=vec["pair"]["ms"], share_of_step=vec["pair"]["ms"] / ms_step)
     return out
 
 

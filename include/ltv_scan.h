@@ -144,6 +144,37 @@ LTV_API int ltv_scan_adjoint(const float* A, const float* B, const float* g,
                      int batch, int T, int n, int m,
                      void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Rollout and adjoint scan of the same batch in ONE call (north_star (i) + (iii)): same arguments, results and
+ * conventions as ltv_scan_rollout and ltv_scan_adjoint (the same kernels).  The two scans are independent - g is an
+ * input - and each is a chain of T dependent steps per item.  When each of them, in the configuration it would choose
+ * alone, leaves at least half of the SMs idle (one small problem such as BASELINE.json configs[0]; few items, whose
+ * clusters cannot be wider than 16 CTAs), the adjoint is enqueued on an internal side stream forked from and joined back
+ * into `cuda_stream` with events, and the two run CONCURRENTLY; otherwise they run back to back on `cuda_stream`
+ * (measured: once either saturates HBM alone, running both at once is slower).  Either way the call is stream-ordered
+ * like any other and capturable in a CUDA graph.  The side stream and its two events are created once per host thread
+ * and device and kept. */
+LTV_API int ltv_scan_rollout_adjoint(const float* A, const float* B, const float* c, const float* x0, const float* u,
+                                     const float* g, float* x_out, float* lambda_out, float* grad_u_out,
+                                     float* grad_x0_out, int batch, int T, int n, int m,
+                                     void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* The whole hot path - north_star (i), (ii), (iii) - in one call on device buffers: every argument as in
+ * ltv_scan_rollout, ltv_scan_system_response_tube and ltv_scan_adjoint (B, c, u, grad_u_out, grad_x0_out may be NULL as
+ * there; flags: 0 or LTV_TUBE_ROW_2NORM; workspace: ltv_scan_workspace_bytes(LTV_OP_SYSTEM_RESPONSE_TUBE or
+ * _RELAYOUT, ...)).  Two routes, same results up to the order of floating-point sums:
+ *   small problems  n <= 64, T >= 2, phi_layout = LTV_PHI_COLUMN_PACKED and all of A_0 .. A_{T-1} fitting one SM's shared
+ *                   memory (T n (n + 4) 4 bytes + ~40 KB <= 227 KB; BASELINE.json configs[0]: n = 48, T = 16): ONE
+ *                   launch, one thread-block cluster per item - CTA r owns the block columns s = r, r + 15, .. of Phi as
+ *                   chains Phi(t,s) = A_{t-1} Phi(t-1,s) that never leave its shared memory (fp32 FMA), the last CTA
+ *                   runs rollout and adjoint side by side, one cluster barrier, tube rows summed over the columns
+ *                   through distributed shared memory in fixed order (deterministic).  ltv_scan_all_is_fused tells.
+ *   otherwise       ltv_scan_rollout_adjoint followed by ltv_scan_system_response_tube on `cuda_stream`. */
+LTV_API int ltv_scan_all_is_fused(int batch, int T, int n, int m, int phi_layout);
+LTV_API int ltv_scan_all(const float* A, const float* B, const float* c, const float* x0, const float* u, const float* w,
+                         const float* g, float* x_out, float* phi_out, float* r_out, float* lambda_out,
+                         float* grad_u_out, float* grad_x0_out, int batch, int T, int n, int m, int phi_layout,
+                         unsigned flags, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* Closed-loop observer propagation (eq.(14), :177), with gains that do not
  * depend on the injection step k (reading q15):
  *     Abar_j = A_j + Lt_j C_j,   PhiX(t,s) = Abar_{t-1} ... Abar_s,   PhiY(t,s) = PhiX(t,s) Lt_s,   0 <= s < t <= T-1
@@ -279,7 +310,8 @@ LTV_API int ltv_scan_output_feedback_constraints(const float* A, const float* B,
                                                  void* workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* One pass of the whole hot path from HOST buffers: copies A, B, c, x0, u, w, g host->device into
- * `workspace` (device, >= ltv_scan_workspace_bytes(LTV_OP_PIPELINE_HOST, ...)), runs the three calls above
+ * `workspace` (device, >= ltv_scan_workspace_bytes(LTV_OP_PIPELINE_HOST, ...)), runs the path (ltv_scan_rollout_adjoint, then
+ * ltv_scan_system_response_tube)
  * on `cuda_stream`, copies x, r, lambda, grad_u, grad_x0 device->host and synchronises the stream before
  * returning.  Phi (11 GB at the benchmark sizes) stays in the workspace on the device, where its consumer
  * (the tube / constraint tightening) lives, unless phi_host != NULL, in which case it is copied back too.

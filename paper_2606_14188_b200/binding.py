@@ -35,7 +35,7 @@ EXPORTS = (
     "ltv_launch_count", "ltv_profile_enable", "ltv_profile_collect", "ltv_scan_observer_response",
     "ltv_observer_row_floats", "ltv_scan_kalman_gains",
     "ltv_scan_constraint_tightening", "ltv_scan_output_feedback_response", "ltv_set_option", "ltv_get_option",
-    "ltv_profile_class_name", "ltv_scan_output_feedback_constraints", "ltv_scan_output_feedback_constraints_workspace_bytes",
+    "ltv_profile_class_name", "ltv_scan_rollout_adjoint", "ltv_scan_all", "ltv_scan_all_is_fused", "ltv_scan_output_feedback_constraints", "ltv_scan_output_feedback_constraints_workspace_bytes",
 )
 
 
@@ -64,6 +64,12 @@ def _load() -> ctypes.CDLL:
     L.ltv_scan_system_response_tube.argtypes = [fp] * 4 + [i] * 4 + [ctypes.c_uint, vp, sz, vp]
     L.ltv_scan_adjoint.restype = i
     L.ltv_scan_adjoint.argtypes = [fp] * 6 + [i] * 4 + [vp, sz, vp]
+    L.ltv_scan_rollout_adjoint.restype = i
+    L.ltv_scan_rollout_adjoint.argtypes = [fp] * 10 + [i] * 4 + [vp, sz, vp]
+    L.ltv_scan_all.restype = i
+    L.ltv_scan_all.argtypes = [fp] * 13 + [i] * 5 + [ctypes.c_uint, vp, sz, vp]
+    L.ltv_scan_all_is_fused.restype = i
+    L.ltv_scan_all_is_fused.argtypes = [i] * 5
     L.ltv_scan_pipeline_host.restype = i
     L.ltv_scan_pipeline_host.argtypes = [fp] * 13 + [i] * 4 + [vp, sz, vp, ctypes.POINTER(ctypes.c_void_p)]
     L.ltv_scan_observer_response.restype = i
@@ -340,6 +346,60 @@ def ltv_scan_adjoint(A, B, g, want_grad_x0=True, lambda_out=None, grad_u_out=Non
     if st != LTV_OK:
         raise LtvError(st, "ltv_scan_adjoint")
     return lambda_out, grad_u_out, grad_x0_out
+
+
+def ltv_scan_rollout_adjoint(A, B, c, x0, u, g, want_grad_x0=True, x_out=None, lambda_out=None, grad_u_out=None,
+                             grad_x0_out=None):
+    """Rollout and adjoint of the same batch, concurrently (one call): returns (x, lam, grad_u | None, grad_x0 | None)
+    with the conventions of ltv_scan_rollout / ltv_scan_adjoint."""
+    batch, T, n, _ = A.shape
+    m = 0 if B is None else B.shape[-1]
+    _dev(A, "A", (batch, T, n, n)); _dev(B, "B", (batch, T, n, m)); _dev(c, "c", (batch, T, n))
+    _dev(x0, "x0", (batch, n)); _dev(u, "u", (batch, T, m)); _dev(g, "g", (batch, T, n))
+    mk = lambda *s: torch.empty(s, device=A.device, dtype=torch.float32)
+    if x_out is None:
+        x_out = mk(batch, T, n)
+    if lambda_out is None:
+        lambda_out = mk(batch, T, n)
+    if grad_u_out is None and B is not None and m > 0:
+        grad_u_out = mk(batch, T, m)
+    if grad_x0_out is None and want_grad_x0:
+        grad_x0_out = mk(batch, n)
+    st = lib.ltv_scan_rollout_adjoint(_ptr(A), _ptr(B), _ptr(c), _ptr(x0), _ptr(u), _ptr(g), _ptr(x_out), _ptr(lambda_out),
+                                      _ptr(grad_u_out), _ptr(grad_x0_out), batch, T, n, m, None, 0, _stream())
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_rollout_adjoint")
+    return x_out, lambda_out, grad_u_out, grad_x0_out
+
+
+def ltv_scan_all_is_fused(batch, T, n, m, layout=LTV_PHI_COLUMN_PACKED) -> bool:
+    return bool(lib.ltv_scan_all_is_fused(batch, T, n, m, layout))
+
+
+def ltv_scan_all(A, B, c, x0, u, w, g, want_grad_x0=True, two_norm=False, layout=LTV_PHI_COLUMN_PACKED, outs=None,
+                 workspace=None):
+    """The whole hot path in one call: returns dict(x, phi, r, lam, grad_u, grad_x0) of device tensors (conventions of the
+    three single calls).  Small problems (ltv_scan_all_is_fused) run as ONE kernel launch."""
+    batch, T, n, _ = A.shape
+    m = 0 if B is None else B.shape[-1]
+    P = T * (T - 1) // 2
+    _dev(A, "A", (batch, T, n, n)); _dev(B, "B", (batch, T, n, m)); _dev(c, "c", (batch, T, n))
+    _dev(x0, "x0", (batch, n)); _dev(u, "u", (batch, T, m)); _dev(w, "w", (batch, T, n)); _dev(g, "g", (batch, T, n))
+    mk = lambda *s: torch.empty(s, device=A.device, dtype=torch.float32)
+    if outs is None:
+        outs = dict(x=mk(batch, T, n), phi=mk(*((batch, T, T, n, n) if layout == LTV_PHI_SQUARE_GRID else (batch, P, n, n))),
+                    r=mk(batch, T, n), lam=mk(batch, T, n), grad_u=mk(batch, T, m) if (B is not None and m > 0) else None,
+                    grad_x0=mk(batch, n) if want_grad_x0 else None)
+    need = ltv_scan_workspace_bytes(LTV_OP_SYSTEM_RESPONSE_TUBE if layout == LTV_PHI_COLUMN_PACKED
+                                    else LTV_OP_SYSTEM_RESPONSE_TUBE_RELAYOUT, batch, T, n, 0)
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), device=A.device, dtype=torch.uint8)
+    st = lib.ltv_scan_all(_ptr(A), _ptr(B), _ptr(c), _ptr(x0), _ptr(u), _ptr(w), _ptr(g), _ptr(outs["x"]), _ptr(outs["phi"]),
+                          _ptr(outs["r"]), _ptr(outs["lam"]), _ptr(outs["grad_u"]), _ptr(outs["grad_x0"]), batch, T, n, m,
+                          layout, LTV_TUBE_ROW_2NORM if two_norm else 0, _ptr(workspace), workspace.numel(), _stream())
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_all")
+    return outs
 
 
 def ltv_scan_pipeline_host(A, B, c, x0, u, w, g, workspace, want_grad_x0=True, phi_host=None, outs=None):

@@ -304,18 +304,24 @@ void* get_encode_tiled() {
   return fn;
 }
 
-cudaError_t launch_adjoint(const AdjointArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches) {
-  AdjParams p{};
-  p.A = a.A; p.B = a.B; p.g = a.g;
-  p.lam_out = a.lambda_out; p.gu_out = (a.m > 0) ? a.grad_u_out : nullptr; p.gx0_out = a.grad_x0_out;
-  p.batch = a.batch; p.T = a.T; p.n = a.n; p.m = a.m;
+static const int* adjoint_max_active() {
   static int max_active[17];
   static bool have = false;
   if (!have) {
     query_max_active_clusters(reinterpret_cast<const void*>(adjoint_kernel), kAdjThreads, 200 * 1024, max_active);
     have = true;
   }
-  if (cluster <= 0) cluster = pick_cluster_model(a.batch, a.n, max_active);
+  return max_active;
+}
+
+int adjoint_cluster_choice(const AdjointArgs& a) { return pick_cluster_model(a.batch, a.n, adjoint_max_active(), a.sm_budget); }
+
+cudaError_t launch_adjoint(const AdjointArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches) {
+  AdjParams p{};
+  p.A = a.A; p.B = a.B; p.g = a.g;
+  p.lam_out = a.lambda_out; p.gu_out = (a.m > 0) ? a.grad_u_out : nullptr; p.gx0_out = a.grad_x0_out;
+  p.batch = a.batch; p.T = a.T; p.n = a.n; p.m = a.m;
+  if (cluster <= 0) cluster = pick_cluster_model(a.batch, a.n, adjoint_max_active(), a.sm_budget);
   p.ap = plan_adjoint(a.n, cluster);
   if (p.ap.stages < 2) return cudaErrorInvalidConfiguration;
 

@@ -32,7 +32,7 @@ int env_int(const char* name, int dflt) {
 static std::atomic<int> g_options[LTV_OPT_COUNT] = {{0}, {4}};
 int option(int which) { return g_options[which].load(std::memory_order_relaxed); }
 
-int pick_cluster_model(int batch, int n, const int* max_active) {
+int pick_cluster_model(int batch, int n, const int* max_active, int sm_budget) {
   const int forced = option(LTV_OPT_VECTOR_CLUSTER);
   if (forced >= 1 && forced <= 16 && max_active[forced] > 0) return forced;
   const double sm_gbs = 70.0, dev_gbs = 6500.0;
@@ -41,9 +41,11 @@ int pick_cluster_model(int batch, int n, const int* max_active) {
   for (int c = 1; c <= 16; ++c) {
     if (max_active[c] <= 0) continue;
     if (c > 1 && (n / c < 32 || (n >> 2) < c)) continue;   // keep at least ~32 rows / columns per CTA
+    int cap = max_active[c];
+    if (sm_budget > 0 && cap > sm_budget / c) cap = sm_budget / c > 0 ? sm_budget / c : 1;
     double t = 0.0;
     for (int rem = batch; rem > 0;) {
-      const int w = rem < max_active[c] ? rem : max_active[c];
+      const int w = rem < cap ? rem : cap;
       const double rate = (w * c * sm_gbs < dev_gbs) ? w * c * sm_gbs : dev_gbs;
       t += w / rate;
       rem -= w;
@@ -272,6 +274,91 @@ int ltv_scan_adjoint(const float* A, const float* B, const float* g, float* lamb
   return e == cudaSuccess ? LTV_OK : fail_cuda(e);
 }
 
+namespace {
+// side stream + fork / join events of ltv_scan_rollout_adjoint: created once per host thread and device (the only
+// state the library keeps besides cached function attributes); never destroyed (a handful of handles per thread)
+struct PairCtx {
+  int dev = -1;
+  cudaStream_t side = nullptr;
+  cudaEvent_t fork = nullptr, join = nullptr;
+};
+cudaError_t pair_ctx(PairCtx** out) {
+  static thread_local PairCtx ctx[16];
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  PairCtx& c = ctx[dev & 15];
+  if (c.dev != dev) {
+    if ((e = cudaStreamCreateWithFlags(&c.side, cudaStreamNonBlocking)) != cudaSuccess) return e;
+    if ((e = cudaEventCreateWithFlags(&c.fork, cudaEventDisableTiming)) != cudaSuccess) return e;
+    if ((e = cudaEventCreateWithFlags(&c.join, cudaEventDisableTiming)) != cudaSuccess) return e;
+    c.dev = dev;
+  }
+  *out = &c;
+  return cudaSuccess;
+}
+}  // namespace
+
+int ltv_scan_rollout_adjoint(const float* A, const float* B, const float* c, const float* x0, const float* u,
+                             const float* g, float* x_out, float* lambda_out, float* grad_u_out, float* grad_x0_out,
+                             int batch, int T, int n, int m, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  (void)workspace; (void)workspace_bytes;
+  if (!A || !x0 || !x_out || !g || !lambda_out) return LTV_ERR_NULL_PTR;
+  if (grad_u_out && m > 0 && !B) return LTV_ERR_NULL_PTR;
+  int st = check_dims(batch, T, n, m);
+  if (st != LTV_OK) return st;
+  if (misaligned(A) || misaligned(B) || misaligned(c) || misaligned(x0) || misaligned(u) || misaligned(x_out) ||
+      misaligned(g) || misaligned(lambda_out) || misaligned(grad_u_out) || misaligned(grad_x0_out))
+    return LTV_ERR_ALIGNMENT;
+  int sms = 0;
+  st = check_device(&sms);
+  if (st != LTV_OK) return st;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  PairCtx* pc = nullptr;
+  cudaError_t e = pair_ctx(&pc);
+  if (e != cudaSuccess) return fail_cuda(e);
+  // The two scans are independent (g is an input).  Measured on B200: running them side by side pays
+  // only when each one, in the configuration it would choose alone, leaves at least half of the SMs idle (one small
+  // problem, or few items whose clusters cannot be wider than 16 CTAs); once either saturates HBM on its own the two only
+  // get in each other's way (C2: 0.55 ms side by side on 64 + 64 SMs against 0.25 ms back to back).  So: concurrent when
+  // both fit into half the machine, back to back on the caller's stream otherwise.
+  RolloutArgs ra{A, B, c, x0, u, x_out, batch, T, n, m};
+  AdjointArgs aa{A, B, g, lambda_out, grad_u_out, grad_x0_out, batch, T, n, m};
+  const long long ctas_r = static_cast<long long>(batch) * rollout_cluster_choice(ra);
+  const long long ctas_a = static_cast<long long>(batch) * adjoint_cluster_choice(aa);
+  const bool side_by_side = ctas_r <= sms / 2 && ctas_a <= sms / 2;
+  unsigned long long l = 0;
+  {
+    ProfScope prof(kProfVectorPair, s);
+    cudaStream_t sa = s;
+    if (side_by_side) {
+      if ((e = cudaEventRecord(pc->fork, s)) != cudaSuccess) return fail_cuda(e);
+      if ((e = cudaStreamWaitEvent(pc->side, pc->fork, 0)) != cudaSuccess) return fail_cuda(e);
+      sa = pc->side;
+    }
+    e = launch_adjoint(aa, 0, sa, &l);
+    if (e != cudaSuccess) {
+      cudaGetLastError();
+      e = launch_adjoint(aa, 1, sa, &l);
+    }
+    cudaError_t e2 = launch_rollout(ra, 0, s, &l);
+    if (e2 != cudaSuccess) {
+      cudaGetLastError();
+      e2 = launch_rollout(ra, 1, s, &l);
+    }
+    cudaError_t e3 = cudaSuccess;
+    if (side_by_side) {
+      // always join, so that the caller's stream is ordered after whatever did get enqueued on the side stream
+      e3 = cudaEventRecord(pc->join, pc->side);
+      if (e3 == cudaSuccess) e3 = cudaStreamWaitEvent(s, pc->join, 0);
+    }
+    if (e == cudaSuccess) e = e2;
+    if (e == cudaSuccess) e = e3;
+  }
+  g_launches += l;
+  return e == cudaSuccess ? LTV_OK : fail_cuda(e);
+}
+
 int ltv_scan_system_response_tube(const float* A, const float* w, float* phi_out, float* r_out, int batch, int T,
                                   int n, int phi_layout, unsigned flags, void* workspace, size_t workspace_bytes,
                                   void* cuda_stream) {
@@ -301,6 +388,42 @@ int ltv_scan_system_response_tube(const float* A, const float* w, float* phi_out
     e = launch_phi_relayout(phi_cp, phi_out, batch, T, n, n, phi_layout, sms, static_cast<cudaStream_t>(cuda_stream));
     if (e == cudaSuccess) ++l;
   }
+  g_launches += l;
+  return e == cudaSuccess ? LTV_OK : fail_cuda(e);
+}
+
+int ltv_scan_all_is_fused(int batch, int T, int n, int m, int phi_layout) {
+  return (check_dims(batch, T, n, m) == LTV_OK && phi_layout == LTV_PHI_COLUMN_PACKED && fused_small_supported(batch, T, n, m)) ? 1 : 0;
+}
+
+int ltv_scan_all(const float* A, const float* B, const float* c, const float* x0, const float* u, const float* w,
+                 const float* g, float* x_out, float* phi_out, float* r_out, float* lambda_out, float* grad_u_out,
+                 float* grad_x0_out, int batch, int T, int n, int m, int phi_layout, unsigned flags, void* workspace,
+                 size_t workspace_bytes, void* cuda_stream) {
+  if (!A || !x0 || !w || !g || !x_out || !r_out || !lambda_out) return LTV_ERR_NULL_PTR;
+  if (T > 1 && !phi_out) return LTV_ERR_NULL_PTR;
+  if (grad_u_out && m > 0 && !B) return LTV_ERR_NULL_PTR;
+  int st = check_dims(batch, T, n, m);
+  if (st != LTV_OK) return st;
+  if ((flags & ~static_cast<unsigned>(LTV_TUBE_ROW_2NORM)) != 0) return LTV_ERR_BAD_DIM;
+  if (!ltv_scan_all_is_fused(batch, T, n, m, phi_layout)) {
+    st = ltv_scan_rollout_adjoint(A, B, c, x0, u, g, x_out, lambda_out, grad_u_out, grad_x0_out, batch, T, n, m, nullptr, 0,
+                                  cuda_stream);
+    if (st != LTV_OK) return st;
+    return ltv_scan_system_response_tube(A, w, phi_out, r_out, batch, T, n, phi_layout, flags, workspace, workspace_bytes,
+                                         cuda_stream);
+  }
+  if (misaligned(A) || misaligned(B) || misaligned(c) || misaligned(x0) || misaligned(u) || misaligned(w) || misaligned(g) ||
+      misaligned(x_out) || misaligned(phi_out) || misaligned(r_out) || misaligned(lambda_out) || misaligned(grad_u_out) ||
+      misaligned(grad_x0_out))
+    return LTV_ERR_ALIGNMENT;
+  int sms = 0;
+  st = check_device(&sms);
+  if (st != LTV_OK) return st;
+  FusedSmallArgs a{A, B, c, x0, u, w, g, x_out, phi_out, r_out, lambda_out, grad_u_out, grad_x0_out, batch, T, n, m,
+                   (flags & LTV_TUBE_ROW_2NORM) ? 1 : 0};
+  unsigned long long l = 0;
+  cudaError_t e = launch_fused_small(a, static_cast<cudaStream_t>(cuda_stream), &l);
   g_launches += l;
   return e == cudaSuccess ? LTV_OK : fail_cuda(e);
 }
@@ -547,17 +670,15 @@ int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float
     const size_t c0 = static_cast<size_t>(ci) * cb;
     const int cn = (c0 + cb <= b) ? cb : static_cast<int>(b - c0);
     LTV_TRY(cudaStreamWaitEvent(s, ev_up[ci], 0));
-    st = ltv_scan_rollout(dA + c0 * t * nn * nn, B_host ? dB + c0 * t * nn * mm : nullptr,
-                          c_host ? dc + c0 * t * nn : nullptr, dx0 + c0 * nn, u_host ? du + c0 * t * mm : nullptr,
-                          dx + c0 * t * nn, cn, T, n, m, nullptr, 0, cuda_stream);
+    st = ltv_scan_rollout_adjoint(dA + c0 * t * nn * nn, B_host ? dB + c0 * t * nn * mm : nullptr,
+                                  c_host ? dc + c0 * t * nn : nullptr, dx0 + c0 * nn, u_host ? du + c0 * t * mm : nullptr,
+                                  dg + c0 * t * nn, dx + c0 * t * nn, dl + c0 * t * nn,
+                                  (grad_u_host && B_host) ? dgu + c0 * t * mm : nullptr,
+                                  grad_x0_host ? dgx + c0 * nn : nullptr, cn, T, n, m, nullptr, 0, cuda_stream);
     if (st == LTV_OK && with_phi)
       st = ltv_scan_system_response_tube(dA + c0 * t * nn * nn, dw + c0 * t * nn, dphi + c0 * P * nn * nn,
                                          dr + c0 * t * nn, cn, T, n, LTV_PHI_COLUMN_PACKED, 0, phi_ws, phi_ws_bytes,
                                          cuda_stream);
-    if (st == LTV_OK)
-      st = ltv_scan_adjoint(dA + c0 * t * nn * nn, B_host ? dB + c0 * t * nn * mm : nullptr, dg + c0 * t * nn,
-                            dl + c0 * t * nn, (grad_u_host && B_host) ? dgu + c0 * t * mm : nullptr,
-                            grad_x0_host ? dgx + c0 * nn : nullptr, cn, T, n, m, nullptr, 0, cuda_stream);
     if (st != LTV_OK) {
       cudaStreamSynchronize(cs);
       cleanup();

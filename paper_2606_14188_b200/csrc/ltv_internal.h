@@ -13,16 +13,20 @@ struct RolloutArgs {
   const float *A, *B, *c, *x0, *u;
   float* x_out;
   int batch, T, n, m;
+  int sm_budget = 0;   // > 0: use at most this many SMs (the rollout / adjoint pair shares the machine); 0 = all
 };
 // cluster = 0: chosen by pick_cluster_model
 cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches);
+int rollout_cluster_choice(const RolloutArgs& a);   // the cluster size `cluster = 0` would pick
 
 struct AdjointArgs {
   const float *A, *B, *g;
   float *lambda_out, *grad_u_out, *grad_x0_out;
   int batch, T, n, m;
+  int sm_budget = 0;   // as RolloutArgs (cluster choice only: the adjoint grid is one cluster per item)
 };
 cudaError_t launch_adjoint(const AdjointArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches);
+int adjoint_cluster_choice(const AdjointArgs& a);
 
 struct PhiArgs {
   const float *A, *w;
@@ -95,10 +99,19 @@ struct OfbConArgs {
 size_t ofb_constraints_workspace_bytes(int batch, int T, int n, int nc, int m);
 cudaError_t launch_ofb_constraints(const OfbConArgs& a, cudaStream_t stream, unsigned long long* launches);
 
+// Whole hot path of a small problem in one launch (fused_small.cu): n <= 64 and all of A in one SM's shared memory
+struct FusedSmallArgs {
+  const float *A, *B, *c, *x0, *u, *w, *g;
+  float *x_out, *phi_out, *r_out, *lambda_out, *grad_u_out, *grad_x0_out;
+  int batch, T, n, m, tube_mode;
+};
+bool fused_small_supported(int batch, int T, int n, int m);
+cudaError_t launch_fused_small(const FusedSmallArgs& a, cudaStream_t stream, unsigned long long* launches);
+
 // Cluster size (CTAs per item, 1..16, any integer) for the two vector kernels.  max_active[C] = clusters of C CTAs
 // that can be resident at once (cudaOccupancyMaxActiveClusters; 0 = not launchable).  Minimises a simple
 // time model over the waves of clusters: an SM streams ~70 GB/s, the device ~6.5 TB/s (both measured).
-int pick_cluster_model(int batch, int n, const int* max_active);
+int pick_cluster_model(int batch, int n, const int* max_active, int sm_budget = 0);
 // fills max_active[1..16] for `kernel` (any __global__ function pointer) at the given block size / dynamic smem
 void query_max_active_clusters(const void* kernel, int threads, size_t smem, int* max_active);
 // developer override LTV_SCAN_<name>=<int>, compiled in only with -DLTV_TUNING; the product build returns `dflt`

@@ -417,17 +417,26 @@ RollSmemPlan plan_rollout(int n, int C, int occ) {
 
 // `cluster` CTAs per item (0 = modelled); the grid is as many clusters as can be resident at once (at most one
 // per item), each looping over items
-cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches) {
+static const int* rollout_max_active(int wide) {
   static int max_active[2][17];
   static bool have[2] = {false, false};
-  const int wide = a.n > kModeAMaxN ? 1 : 0;
   if (!have[wide]) {
     query_max_active_clusters(wide ? reinterpret_cast<const void*>(rollout_kernel<true>)
                                    : reinterpret_cast<const void*>(rollout_kernel<false>),
                               kRollThreads, 200 * 1024, max_active[wide]);
     have[wide] = true;
   }
-  if (cluster <= 0) cluster = pick_cluster_model(a.batch, a.n, max_active[wide]);
+  return max_active[wide];
+}
+
+int rollout_cluster_choice(const RolloutArgs& a) {
+  return pick_cluster_model(a.batch, a.n, rollout_max_active(a.n > kModeAMaxN ? 1 : 0), a.sm_budget);
+}
+
+cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches) {
+  const int wide = a.n > kModeAMaxN ? 1 : 0;
+  const int* max_active = rollout_max_active(wide);
+  if (cluster <= 0) cluster = pick_cluster_model(a.batch, a.n, max_active, a.sm_budget);
   RollParams p{};
   p.A = a.A; p.B = (a.m > 0) ? a.B : nullptr; p.c = a.c; p.x0 = a.x0; p.u = a.u; p.x_out = a.x_out;
   p.batch = a.batch; p.T = a.T; p.n = a.n; p.m = a.m;
@@ -442,8 +451,9 @@ cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t strea
     if (e != cudaSuccess) return e;
   }
   cudaLaunchConfig_t cfg{};
-  int ncl = max_active[wide][cluster];
+  int ncl = max_active[cluster];
   if (ncl > a.batch) ncl = a.batch;
+  if (a.sm_budget > 0 && ncl > a.sm_budget / cluster) ncl = a.sm_budget / cluster;
   if (ncl < 1) ncl = 1;
   cfg.gridDim = dim3(static_cast<unsigned>(ncl) * cluster);
   cfg.blockDim = dim3(kRollThreads);

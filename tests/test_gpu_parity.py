@@ -443,3 +443,89 @@ def test_phi_layout_validation(L):
     with pytest.raises(L.LtvError) as e:      # the native workspace is too small for a re-ordered layout
         L.ltv_scan_system_response_tube(A, w, workspace=ws, layout=L.LTV_PHI_ROW_PACKED)
     assert e.value.status == 5
+
+
+@pytest.mark.parametrize("n,T,batch,m", [(48, 16, 1, 6), (300, 9, 5, 6), (180, 20, 70, 6), (644, 3, 2, 4), (1200, 4, 3, 12)])
+def test_rollout_adjoint_pair(L, n, T, batch, m):
+    """ltv_scan_rollout_adjoint (both scans concurrently, half of the SMs each) against the oracle and the single calls."""
+    import torch
+
+    W = dense_random(batch, T, n, m, seed=3 * n + batch, scale=0.3)
+    d = {k: torch.from_numpy(getattr(W, k)).cuda() for k in ("A", "B", "c", "x0", "u", "g")}
+    for rep in range(2):                                   # twice: the cached side stream / events are reused
+        x, lam, gu, gx0 = L.ltv_scan_rollout_adjoint(d["A"], d["B"], d["c"], d["x0"], d["u"], d["g"])
+    x1 = L.ltv_scan_rollout(d["A"], d["B"], d["c"], d["x0"], d["u"])
+    torch.cuda.synchronize()
+    assert torch.equal(x, x1)
+    rl, rgu, rgx = O.adjoint(W.A, W.B, W.g)
+    _check(dict(x=x.cpu().numpy(), lam=lam.cpu().numpy(), grad_u=gu.cpu().numpy(), grad_x0=gx0.cpu().numpy()),
+           dict(x=O.rollout(W.A, W.B, W.c, W.x0, W.u), lam=rl, grad_u=rgu, grad_x0=rgx))
+    # optional outputs absent
+    x2, lam2, gu2, gx2 = L.ltv_scan_rollout_adjoint(d["A"], None, d["c"], d["x0"], None, d["g"], want_grad_x0=False)
+    torch.cuda.synchronize()
+    assert gu2 is None and gx2 is None
+    assert O.rel_err(x2.cpu().numpy(), O.rollout(W.A, None, W.c, W.x0, None)) <= TOL
+    assert O.rel_err(lam2.cpu().numpy(), rl) <= TOL
+
+
+def _all_vs_oracle(L, W, two_norm=False, exact=False, layout=None):
+    import torch
+
+    d = {k: torch.from_numpy(getattr(W, k)).cuda() for k in ("A", "B", "c", "x0", "u", "w", "g")}
+    kw = {} if layout is None else dict(layout=layout)
+    o = L.ltv_scan_all(d["A"], d["B"], d["c"], d["x0"], d["u"], d["w"], d["g"], two_norm=two_norm, **kw)
+    torch.cuda.synchronize()
+    T = W.A.shape[1]
+    rl, rgu, rgx = O.adjoint(W.A, W.B, W.g)
+    phi_ref = O.system_response(W.A)
+    if layout is None:
+        phi_ref = phi_ref[:, _col_perm(T)]
+    ref = dict(x=O.rollout(W.A, W.B, W.c, W.x0, W.u), phi=phi_ref,
+               r=(O.tube_row2norm(W.A, W.w) if two_norm else O.tube(W.A, W.w)), lam=rl, grad_u=rgu, grad_x0=rgx)
+    return _check({k: v.cpu().numpy() for k, v in o.items() if v is not None}, ref, exact=exact)
+
+
+@pytest.mark.parametrize("n,T,batch,m", [(48, 16, 1, 6),      # C1 exactly (shape)
+                                         (48, 16, 20, 6),     # more clusters than fit at once
+                                         (64, 8, 3, 5),       # largest n, two k groups
+                                         (32, 20, 2, 3),      # T - 1 = 19 columns over 15 column CTAs (two slots)
+                                         (4, 3, 2, 1), (16, 2, 1, 2), (36, 5, 4, 0), (60, 9, 2, 12)])
+def test_scan_all_fused_small(L, n, T, batch, m):
+    """ltv_scan_all on shapes that take the single-launch route, against the oracle (both tube forms)."""
+    assert L.ltv_scan_all_is_fused(batch, T, n, m)
+    W = dense_random(batch, T, n, max(m, 1), seed=17 * n + T, scale=0.4)
+    if m == 0:
+        import torch
+
+        d = {k: torch.from_numpy(getattr(W, k)).cuda() for k in ("A", "c", "x0", "w", "g")}
+        o = L.ltv_scan_all(d["A"], None, d["c"], d["x0"], None, d["w"], d["g"])
+        torch.cuda.synchronize()
+        assert o["grad_u"] is None
+        assert O.rel_err(o["x"].cpu().numpy(), O.rollout(W.A, None, W.c, W.x0, None)) <= TOL
+        assert O.rel_err(o["r"].cpu().numpy(), O.tube(W.A, W.w)) <= TOL
+        assert O.rel_err(o["phi"].cpu().numpy(), O.system_response(W.A)[:, _col_perm(T)]) <= TOL
+        rl, _, rgx = O.adjoint(W.A, None, W.g)
+        assert O.rel_err(o["lam"].cpu().numpy(), rl) <= TOL and O.rel_err(o["grad_x0"].cpu().numpy(), rgx) <= TOL
+        return
+    _all_vs_oracle(L, W)
+    _all_vs_oracle(L, W, two_norm=True)
+
+
+def test_scan_all_config1_and_integer_exact(L):
+    """BASELINE.json configs[0] through the single launch; small-integer inputs must come out bit-exact."""
+    from workloads import small_integer
+
+    W = generate(config(0))
+    assert L.ltv_scan_all_is_fused(*W.shape)
+    print("C1 fused", _all_vs_oracle(L, W))
+    _all_vs_oracle(L, small_integer(2, 9, 48, 3, seed=12), exact=True)
+
+
+def test_scan_all_generic_route_and_layouts(L):
+    """Shapes that do not fit the single launch go through ltv_scan_rollout_adjoint + ltv_scan_system_response_tube;
+    a non-native layout forces the generic route even for a small problem."""
+    assert not L.ltv_scan_all_is_fused(2, 5, 132, 3)
+    assert not L.ltv_scan_all_is_fused(1, 64, 64, 3)          # A does not fit one SM's shared memory
+    _all_vs_oracle(L, dense_random(2, 5, 132, 3, seed=77, scale=0.4))
+    assert not L.ltv_scan_all_is_fused(2, 6, 48, 3, L.LTV_PHI_ROW_PACKED)
+    _all_vs_oracle(L, dense_random(2, 6, 48, 3, seed=78, scale=0.4), layout=L.LTV_PHI_ROW_PACKED)
