@@ -262,6 +262,11 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def _log(msg):
+    """Progress on stderr (the JSON line on stdout stays alone)."""
+    print(f"[bench {time.strftime('%H:%M:%S')}] {msg}", file=sys.stderr, flush=True)
+
+
 def _events(torch):
     return torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
 
@@ -313,6 +318,7 @@ def run_workload(B, L, W, name, cfg_index, steps, warmup, phi_on, min_seconds=0.
     dev = B.dev
     batch, T, n, m = W.shape
     P = T * (T - 1) // 2
+    _log(f"run_workload {label or name}: n={n} T={T} batch={batch} steps={steps} min_seconds={min_seconds}")
     d = {k: torch.from_numpy(getattr(W, k)).to(dev) for k in ("A", "B", "c", "x0", "u", "w", "g")}
     x = torch.empty((batch, T, n), device=dev)
     lam = torch.empty((batch, T, n), device=dev)
@@ -471,6 +477,7 @@ def next_rows(B, L, W, steps):
         B.barrier()
         return B.max_over_ranks(e0.elapsed_time(e1)) / reps
 
+    _log("next_rows: observer, kalman, constraints, output_feedback, output_feedback_constraints")
     gen = torch.Generator(device=dev).manual_seed(1234 + B.rank)
     Lt = torch.randn((batch, T, n, p), device=dev, generator=gen) * (0.05 / p ** 0.5)
     Cm = torch.randn((batch, T, p, n), device=dev, generator=gen) / n ** 0.5
@@ -526,6 +533,7 @@ def e2e_leg(B, L, W, phi_on, reps):
     batch, T, n, m = W.shape
     P = T * (T - 1) // 2
     units = (P if phi_on else 1) * batch * B.world
+    _log("e2e leg (ltv_scan_pipeline_host)")
     need = L.ltv_scan_workspace_bytes(L.LTV_OP_PIPELINE_HOST if phi_on else L.LTV_OP_PIPELINE_HOST_NO_PHI, batch, T, n, m)
     wsh = torch.empty(need, dtype=torch.uint8, device=dev)
     h = {k: torch.from_numpy(getattr(W, k)).pin_memory() for k in ("A", "B", "c", "x0", "u", "w", "g")}

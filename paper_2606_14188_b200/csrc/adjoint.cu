@@ -46,7 +46,11 @@ __host__ __device__ inline void col_band(int n, int C, int rank, int& j0, int& j
   j1 = 4 * static_cast<int>((static_cast<long long>(nq) * (rank + 1)) / C);
 }
 
-__device__ __forceinline__ uint32_t lam_parity(int k) { return static_cast<uint32_t>(k / 3 - (k % 3 == 0 ? 1 : 0)) & 1u; }
+constexpr int kLamBufs = 4;   // costate buffers / barriers: a remote CTA can be two steps ahead of this CTA's helper warp, which
+                              // still reads lam_{t+1} of its step for grad_u, so the buffer written two steps ahead must differ
+__device__ __forceinline__ uint32_t lam_parity(int k) {
+  return static_cast<uint32_t>(k / kLamBufs - (k % kLamBufs == 0 ? 1 : 0)) & 1u;
+}
 
 __global__ void __launch_bounds__(kAdjThreads, 1)
 adjoint_kernel(const AdjParams p, const __grid_constant__ CUtensorMap tmapA) {
@@ -64,21 +68,19 @@ adjoint_kernel(const AdjParams p, const __grid_constant__ CUtensorMap tmapA) {
   const int nrb = (n + ap.rcb - 1) / ap.rcb;
   const int nstep = (T - 1) + (p.gx0_out ? 1 : 0);  // GEMV steps: A_{T-1} .. A_1 (, A_0)
 
-  float* lambuf = reinterpret_cast<float*>(smem + ap.off_lam);  // [3][n] (three: the helper may lag a step)
+  float* lambuf = reinterpret_cast<float*>(smem + ap.off_lam);  // [kLamBufs][n]
   float* red = reinterpret_cast<float*>(smem + ap.off_red);     // [rg][bw]
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + ap.off_bar);
   uint64_t* full = bars;
   uint64_t* empty = bars + kAdjMaxStages;   // kAdjConsThreads/32 arrivals
-  uint64_t* lfull = bars + 2 * kAdjMaxStages;  // [3] input costate of step k complete in lambuf[k%3]
+  uint64_t* lfull = bars + 2 * kAdjMaxStages;  // [kLamBufs] input costate of step k complete in lambuf[k % kLamBufs]
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < ap.stages; ++s) {
       mbar_init(&full[s], 1);
       mbar_init(&empty[s], kAdjConsThreads / 32);
     }
-    mbar_init(&lfull[0], 1);
-    mbar_init(&lfull[1], 1);
-    mbar_init(&lfull[2], 1);
+    for (int s = 0; s < kLamBufs; ++s) mbar_init(&lfull[s], 1);
     fence_mbar_init();
     tma_prefetch_desc(&tmapA);
   }
@@ -92,8 +94,8 @@ adjoint_kernel(const AdjParams p, const __grid_constant__ CUtensorMap tmapA) {
   __syncthreads();
   cluster_sync_all();
 
-  // step k = 0 .. nstep-1 multiplies by A_t^T with t = T-1-k; its input costate lam_{t+1} is lambuf[k%3];
-  // barrier lfull[k%3] is used for k = j, j+3, .. except k = 0 (local init): phase index k/3 - (k%3==0)
+  // step k = 0 .. nstep-1 multiplies by A_t^T with t = T-1-k; its input costate lam_{t+1} is lambuf[k % kLamBufs];
+  // barrier lfull[j] is used for k = j, j + kLamBufs, .. except k = 0 (local init): phase index k / kLamBufs - (k % kLamBufs == 0)
   if (warp == kAdjAllCons / 32) {
     // ------------------------------------------------------------------ producer
     if (lane == 0 && W > 0) {
@@ -137,9 +139,9 @@ adjoint_kernel(const AdjParams p, const __grid_constant__ CUtensorMap tmapA) {
         for (int j = 0; j < kVB; ++j) vb[j] = (lane + 32 * j < nv) ? __ldg(src + lane + 32 * j) : make_float4(0.f, 0.f, 0.f, 0.f);
       };
       if (fast) issue(0);
-      if (k >= 1) mbar_wait_cluster(&lfull[k % 3], lam_parity(k));
-      if (k + 1 < T && lane == 0) mbar_arrive_expect_tx(&lfull[(k + 1) % 3], static_cast<uint32_t>(n) * 4u);
-      const float* lam = lambuf + (k % 3) * n;
+      if (k >= 1) mbar_wait_cluster(&lfull[k % kLamBufs], lam_parity(k));
+      if (k + 1 < T && lane == 0) mbar_arrive_expect_tx(&lfull[(k + 1) % kLamBufs], static_cast<uint32_t>(n) * 4u);
+      const float* lam = lambuf + (k % kLamBufs) * n;
       if (fast) {
         float acc[kMaxL];
 #pragma unroll
@@ -194,10 +196,10 @@ adjoint_kernel(const AdjParams p, const __grid_constant__ CUtensorMap tmapA) {
     uint32_t fph = 0;
     for (int k = 0; k < nstep; ++k) {
       const int t = T - 1 - k;
-      if (k >= 1) mbar_wait_cluster(&lfull[k % 3], lam_parity(k));
-      const float* lam = lambuf + (k % 3) * n;
-      float* lnext = lambuf + ((k + 1) % 3) * n;
-      uint64_t* lbar = &lfull[(k + 1) % 3];
+      if (k >= 1) mbar_wait_cluster(&lfull[k % kLamBufs], lam_parity(k));
+      const float* lam = lambuf + (k % kLamBufs) * n;
+      float* lnext = lambuf + ((k + 1) % kLamBufs) * n;
+      uint64_t* lbar = &lfull[(k + 1) % kLamBufs];
       const float* gt = (t >= 1) ? p.g + (static_cast<size_t>(item) * T + (t - 1)) * n : nullptr;
       for (int sl = 0; sl < nslab; ++sl) {
         float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -265,23 +267,39 @@ AdjPlan plan_adjoint(int n, int C) {
   ap.qt = ap.bw / 4;
   ap.rg = kAdjConsThreads / ap.qt;
   if (ap.rg > 32) ap.rg = 32;
-  int rcb = (32 * 1024) / (ap.bw * 4);
+  const uint32_t lam_bytes = static_cast<uint32_t>(align_up(static_cast<size_t>(kLamBufs) * n * 4u, 128));
+  const uint32_t red_bytes = static_cast<uint32_t>(align_up(static_cast<size_t>(kAdjGroups) * ap.rg * ap.bw * 4, 128));
+  const uint32_t budget = 227u * 1024u - lam_bytes - red_bytes - kStageVecs * 16u - 256u;
+  // The ring must have an EVEN number of stages.  The two consumer groups take alternate boxes and never look at the other
+  // group's: with an odd ring a stage changes hands every pass, so a group sees only every other phase of that stage's `full`
+  // barrier and its parity test cannot tell "my box has landed" from "the other group's box of the pass before is still in
+  // flight" (bulk copies of different boxes may complete out of order).  A group that runs into this reads a stale box and
+  // arrives on `empty` out of turn - an mbarrier arrival-count underflow, i.e. the sporadic "unspecified launch failure"s
+  // (and, rarely, dead locks) that matrices of n >= 1536 on >= ~100 CTAs raised in round 2 with a ring of 5.  With an even ring
+  // every stage belongs to one group, which then observes every phase.
+  // Boxes of ~32 KB, shrunk so that an even number of them fills the budget, the row blocks of a step equal.
+  int st = static_cast<int>(budget / (32u * 1024u));
+  if (st > kAdjMaxStages) st = kAdjMaxStages;
+  if (st & 1) st += 1;                     // e.g. 5 boxes of 32 KB -> 6 of ~27 KB
+  if (st < 2) st = 2;
+  uint32_t box = budget / static_cast<uint32_t>(st);
+  if (box > 32u * 1024u) box = 32u * 1024u;
+  int rcb = static_cast<int>(box / (ap.bw * 4u));
   if (rcb > 256) rcb = 256;
   if (rcb > n) rcb = n;
   if (rcb < 1) rcb = 1;
+  rcb = (n + (n + rcb - 1) / rcb - 1) / ((n + rcb - 1) / rcb);   // equal row blocks: no rows of the next matrix are fetched
   ap.rcb = rcb;
   ap.stage_bytes = static_cast<uint32_t>(align_up(static_cast<size_t>(ap.bw) * rcb * 4, 128));
-  const uint32_t lam_bytes = static_cast<uint32_t>(align_up(3u * n * 4u, 128));
-  const uint32_t red_bytes = static_cast<uint32_t>(align_up(static_cast<size_t>(kAdjGroups) * ap.rg * ap.bw * 4, 128));
-  const uint32_t budget = 227u * 1024u - lam_bytes - red_bytes - kStageVecs * 16u - 256u;
-  int st = static_cast<int>(budget / ap.stage_bytes);
+  st = static_cast<int>(budget / ap.stage_bytes);
   if (st > kAdjMaxStages) st = kAdjMaxStages;
+  st &= ~1;
   ap.stages = st;
   ap.off_lam = ap.stage_bytes * st;
   ap.off_red = ap.off_lam + lam_bytes;
   ap.off_stage = ap.off_red + red_bytes;
   ap.off_bar = ap.off_stage + kStageVecs * 16u;
-  ap.total = ap.off_bar + (2 * kAdjMaxStages + 3) * 8;
+  ap.total = ap.off_bar + (2 * kAdjMaxStages + kLamBufs) * 8;
   return ap;
 }
 
@@ -355,6 +373,7 @@ cudaError_t launch_adjoint(const AdjointArgs& a, int cluster, cudaStream_t strea
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
+  LTV_DBG_INSTALL();
   {
     ProfScope prof(kProfAdjoint, stream);
     e = cudaLaunchKernelEx(&cfg, adjoint_kernel, p, tmap);

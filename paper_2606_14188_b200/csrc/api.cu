@@ -29,6 +29,20 @@ int env_int(const char* name, int dflt) {
 #endif
 }
 
+#ifdef LTV_TUNING
+static unsigned int* g_dbg_host = nullptr;
+unsigned int* dbg_buffer_device() {
+  static unsigned int* dptr = nullptr;
+  if (!dptr) {
+    if (cudaHostAlloc(reinterpret_cast<void**>(&g_dbg_host), 65536, cudaHostAllocMapped) != cudaSuccess) return nullptr;
+    std::memset(g_dbg_host, 0, 65536);
+    if (cudaHostGetDevicePointer(reinterpret_cast<void**>(&dptr), g_dbg_host, 0) != cudaSuccess) return nullptr;
+  }
+  return dptr;
+}
+extern "C" LTV_API unsigned int* ltv_debug_buffer(void) { return g_dbg_host; }
+#endif
+
 static std::atomic<int> g_options[LTV_OPT_COUNT] = {{0}, {4}};
 int option(int which) { return g_options[which].load(std::memory_order_relaxed); }
 

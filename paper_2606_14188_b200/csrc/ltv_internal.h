@@ -130,6 +130,18 @@ struct ProfScope {
   void* end_event;   // cudaEvent_t captured at construction
 };
 
+#ifdef LTV_TUNING
+// developer builds: host-mapped record buffer of the spin-limit traps (ptx.cuh); device alias of the same memory
+unsigned int* dbg_buffer_device();
+#define LTV_DBG_INSTALL()                                                        \
+  do {                                                                           \
+    unsigned int* dbgp_ = dbg_buffer_device();                                   \
+    cudaMemcpyToSymbolAsync(g_ltv_dbg, &dbgp_, sizeof(dbgp_), 0, cudaMemcpyHostToDevice, stream); \
+  } while (0)
+#else
+#define LTV_DBG_INSTALL() do {} while (0)
+#endif
+
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 }  // namespace ltv

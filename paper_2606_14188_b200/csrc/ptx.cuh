@@ -73,16 +73,57 @@ __device__ __forceinline__ bool mbar_try_wait_cluster(uint64_t* bar, uint32_t pa
       : "memory");
   return ok != 0;
 }
+#ifdef LTV_TUNING
+// Developer builds only: before a spin-limit trap the waiting thread leaves a record {blockDim.x, blockIdx.x, threadIdx.x,
+// barrier address, parity, kind} in a host-mapped buffer (it survives the dead context); each translation unit has its
+// own copy of the pointer, installed by its launcher through ltv_dbg_install.
+static __device__ unsigned int* g_ltv_dbg = nullptr;
+static __device__ __noinline__ void ltv_dbg_record(uint64_t* bar, uint32_t parity, uint32_t kind) {
+  unsigned int* d = g_ltv_dbg;
+  if (d != nullptr) {
+    const unsigned slot = atomicAdd_system(d, 1u);
+    if (slot < 2000) {
+      volatile unsigned int* r = d + 8 + slot * 8;
+      r[0] = blockDim.x; r[1] = blockIdx.x; r[2] = threadIdx.x;
+      r[3] = static_cast<uint32_t>(__cvta_generic_to_shared(bar)); r[4] = parity; r[5] = kind; r[6] = gridDim.x;
+    }
+    __threadfence_system();
+    for (int i = 0; i < 2000; ++i) __nanosleep(1000);   // let other stuck threads leave their records too
+  }
+}
+#define LTV_DBG_RECORD(bar, parity, kind) ltv_dbg_record(bar, parity, kind)
+#else
+#define LTV_DBG_RECORD(bar, parity, kind)
+#endif
+
+#ifdef LTV_TUNING
+// once one thread has hit the spin limit (count in word 0 of the record buffer), every other waiting thread records itself too
+#define LTV_DBG_PEER_CHECK(bar, parity, kind)                                                         \
+  if ((spins & 0x3ffu) == 0 && g_ltv_dbg != nullptr && *reinterpret_cast<volatile unsigned int*>(g_ltv_dbg) != 0) { \
+    LTV_DBG_RECORD(bar, parity, kind);                                                                \
+    __trap();                                                                                         \
+  }
+#else
+#define LTV_DBG_PEER_CHECK(bar, parity, kind)
+#endif
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   uint32_t spins = 0;
   while (!mbar_try_wait(bar, parity)) {
-    if (++spins > LTV_SPIN_LIMIT) __trap();
+    if (++spins > LTV_SPIN_LIMIT) {
+      LTV_DBG_RECORD(bar, parity, 1u);
+      __trap();
+    }
+    LTV_DBG_PEER_CHECK(bar, parity, 1u)
   }
 }
 __device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity) {
   uint32_t spins = 0;
   while (!mbar_try_wait_cluster(bar, parity)) {
-    if (++spins > LTV_SPIN_LIMIT) __trap();
+    if (++spins > LTV_SPIN_LIMIT) {
+      LTV_DBG_RECORD(bar, parity, 2u);
+      __trap();
+    }
+    LTV_DBG_PEER_CHECK(bar, parity, 2u)
   }
 }
 

@@ -403,6 +403,10 @@ RollSmemPlan plan_rollout(int n, int C, int occ) {
   sp.stage_bytes = static_cast<uint32_t>(align_up(static_cast<size_t>(rc) * row_bytes, 128));
   int st = static_cast<int>(budget / sp.stage_bytes);
   if (st > kMaxStages) st = kMaxStages;
+  // An EVEN number of stages: the two consumer groups take alternate chunks, so with an odd ring a stage would change
+  // hands every pass and a group would see only every other phase of its `full` barrier - the parity test then cannot
+  // tell its own chunk from the other group's chunk of the pass before, still in flight (adjoint.cu has the story).
+  st &= ~1;
   sp.stages = st;
   sp.off_x = sp.stage_bytes * st;
   sp.off_b = sp.off_x + static_cast<uint32_t>(align_up(3 * row_bytes, 128));
@@ -466,6 +470,7 @@ cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t strea
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
+  LTV_DBG_INSTALL();
   {
     ProfScope prof(kProfRollout, stream);
     e = cudaLaunchKernelEx(&cfg, kern, p);
