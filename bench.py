@@ -55,7 +55,7 @@ def parse():
     return ap.parse_args()
 
 
-TRAFFIC_FILE = "profiles/r1_v5_traffic.csv"
+TRAFFIC_FILE = "profiles/r2_traffic.csv"
 
 
 def ncu_traffic(cfg_index, kernel):
