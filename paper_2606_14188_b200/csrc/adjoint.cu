@@ -294,6 +294,7 @@ AdjPlan plan_adjoint(int n, int C) {
   st = static_cast<int>(budget / ap.stage_bytes);
   if (st > kAdjMaxStages) st = kAdjMaxStages;
   st &= ~1;
+  if (env_int("ADJ_ODD_RING", 0) && st > 3) st -= 1;   // developer builds: bring the ring bug back (to check the regression test)
   ap.stages = st;
   ap.off_lam = ap.stage_bytes * st;
   ap.off_red = ap.off_lam + lam_bytes;
@@ -333,6 +334,10 @@ static const int* adjoint_max_active() {
 }
 
 int adjoint_cluster_choice(const AdjointArgs& a) { return pick_cluster_model(a.batch, a.n, adjoint_max_active(), a.sm_budget); }
+
+int adjoint_cluster_fit(const AdjointArgs& a, int max_ctas) {
+  return fit_cluster_single_wave(a.batch, a.n, adjoint_max_active(), max_ctas);
+}
 
 cudaError_t launch_adjoint(const AdjointArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches) {
   AdjParams p{};

@@ -1,6 +1,7 @@
 // extern "C" boundary of libltvscan.so (include/ltv_scan.h): argument validation, workspace sizing,
 // device check, dispatch to the launchers.  No torch types, no exceptions across the ABI.
 #include <atomic>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <mutex>
@@ -69,6 +70,16 @@ int pick_cluster_model(int batch, int n, const int* max_active, int sm_budget) {
       best_t = t;
       best = c;
     }
+  }
+  return best;
+}
+
+int fit_cluster_single_wave(int batch, int n, const int* max_active, int max_ctas) {
+  int best = 0;
+  for (int c = 1; c <= 16; ++c) {
+    if (max_active[c] < batch || static_cast<long long>(batch) * c > max_ctas) continue;
+    if (c > 1 && (n / c < 32 || (n >> 2) < c)) continue;
+    best = c;
   }
   return best;
 }
@@ -340,7 +351,21 @@ int ltv_scan_rollout_adjoint(const float* A, const float* B, const float* c, con
   AdjointArgs aa{A, B, g, lambda_out, grad_u_out, grad_x0_out, batch, T, n, m};
   const long long ctas_r = static_cast<long long>(batch) * rollout_cluster_choice(ra);
   const long long ctas_a = static_cast<long long>(batch) * adjoint_cluster_choice(aa);
-  const bool side_by_side = ctas_r <= sms / 2 && ctas_a <= sms / 2;
+  bool side_by_side = ctas_r <= sms / 2 && ctas_a <= sms / 2;
+  int cl_r = 0, cl_a = 0;   // CTAs per item of the two scans; 0 = each kernel's own model
+  if (!side_by_side) {
+    // Second case (measured, round 2): few items of a SMALL system.  Alone, each scan spreads an item over more CTAs than
+    // its short steps can feed (n = 180, batch 64: two CTAs per item exchange the state every 1.3 us and reach 0.55-0.7 of
+    // the HBM peak); restricted to half the machine each (one wave of the widest clusters that fit there), with <= 192 rows (columns) per CTA, the two scans together move
+    // more: 0.263 -> 0.200 ms at n = 180 x 64 items, 0.185 -> 0.127 ms at n = 300 x 32.  With more rows per CTA a CTA
+    // cannot keep up with its share (n = 300 x 64 items, one CTA per item: 0.280 against 0.239 ms), so the rule stops there.
+    const int cr = rollout_cluster_fit(ra, sms / 2), ca = adjoint_cluster_fit(aa, sms / 2);   // widest single-wave clusters
+    if (cr > 0 && ca > 0 && n / cr <= 192 && n / ca <= 192 && option(LTV_OPT_VECTOR_CLUSTER) == 0) {
+      side_by_side = true;
+      cl_r = cr;
+      cl_a = ca;
+    }
+  }
   unsigned long long l = 0;
   {
     ProfScope prof(kProfVectorPair, s);
@@ -350,12 +375,12 @@ int ltv_scan_rollout_adjoint(const float* A, const float* B, const float* c, con
       if ((e = cudaStreamWaitEvent(pc->side, pc->fork, 0)) != cudaSuccess) return fail_cuda(e);
       sa = pc->side;
     }
-    e = launch_adjoint(aa, 0, sa, &l);
+    e = launch_adjoint(aa, cl_a, sa, &l);
     if (e != cudaSuccess) {
       cudaGetLastError();
       e = launch_adjoint(aa, 1, sa, &l);
     }
-    cudaError_t e2 = launch_rollout(ra, 0, s, &l);
+    cudaError_t e2 = launch_rollout(ra, cl_r, s, &l);
     if (e2 != cudaSuccess) {
       cudaGetLastError();
       e2 = launch_rollout(ra, 1, s, &l);

@@ -437,6 +437,10 @@ int rollout_cluster_choice(const RolloutArgs& a) {
   return pick_cluster_model(a.batch, a.n, rollout_max_active(a.n > kModeAMaxN ? 1 : 0), a.sm_budget);
 }
 
+int rollout_cluster_fit(const RolloutArgs& a, int max_ctas) {
+  return fit_cluster_single_wave(a.batch, a.n, rollout_max_active(a.n > kModeAMaxN ? 1 : 0), max_ctas);
+}
+
 cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches) {
   const int wide = a.n > kModeAMaxN ? 1 : 0;
   const int* max_active = rollout_max_active(wide);

@@ -445,8 +445,10 @@ def test_phi_layout_validation(L):
     assert e.value.status == 5
 
 
-@pytest.mark.parametrize("n,T,batch,m", [(48, 16, 1, 6), (300, 9, 5, 6), (180, 20, 70, 6), (644, 3, 2, 4), (1200, 4, 3, 12)])
-def test_rollout_adjoint_pair(L, n, T, batch, m):
+@pytest.mark.parametrize("n,T,batch,m", [(48, 16, 1, 6), (300, 9, 5, 6), (180, 20, 70, 6), (644, 3, 2, 4), (1200, 4, 3, 12),
+                                         (180, 12, 64, 6), (300, 6, 32, 6), (180, 8, 32, 6)])   # the last three: few items of a
+def test_rollout_adjoint_pair(L, n, T, batch, m):                                                # small system, side by side on half
+                                                                                                 # the machine each (second rule)
     """ltv_scan_rollout_adjoint (both scans concurrently, half of the SMs each) against the oracle and the single calls."""
     import torch
 
@@ -466,6 +468,50 @@ def test_rollout_adjoint_pair(L, n, T, batch, m):
     assert gu2 is None and gx2 is None
     assert O.rel_err(x2.cpu().numpy(), O.rollout(W.A, None, W.c, W.x0, None)) <= TOL
     assert O.rel_err(lam2.cpu().numpy(), rl) <= TOL
+
+
+@pytest.mark.parametrize("n,batch,cluster", [(1536, 48, 4), (2400, 16, 8), (2432, 8, 16)])
+def test_vector_scans_many_ctas_large_n_repeatable(L, n, batch, cluster):
+    """Regression test of the ring bug of round 2: big matrices on >= ~100 CTAs, more clusters than fit
+    at once, both scans also on two streams at the same time.  With an odd shared-memory ring these shapes died with
+    'unspecified launch failure' within 1-30 launches; now every repeat must reproduce the first result bit for bit and
+    item 0 must match the oracle."""
+    import torch
+
+    T, m = 6, 12
+    g = torch.Generator(device="cuda").manual_seed(n + batch)
+    A = torch.randn((batch, T, n, n), device="cuda", generator=g) * (0.3 / n ** 0.5)
+    A += torch.eye(n, device="cuda")
+    B = torch.randn((batch, T, n, m), device="cuda", generator=g) * 0.1
+    c = torch.randn((batch, T, n), device="cuda", generator=g) * 0.01
+    x0 = torch.randn((batch, n), device="cuda", generator=g)
+    u = torch.randn((batch, T, m), device="cuda", generator=g) * 0.1
+    gg = torch.randn((batch, T, n), device="cuda", generator=g)
+    side = torch.cuda.Stream()
+    L.ltv_set_option(L.LTV_OPT_VECTOR_CLUSTER, cluster)
+    try:
+        first = None
+        for rep in range(25):
+            x = L.ltv_scan_rollout(A, B, c, x0, u)
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                lam, gu, gx0 = L.ltv_scan_adjoint(A, B, gg)
+                lam_b, _, _ = L.ltv_scan_adjoint(A, B, gg)       # a second adjoint right behind: clusters of two launches overlap
+            torch.cuda.current_stream().wait_stream(side)
+            torch.cuda.synchronize()
+            got = (x, lam, gu, gx0)
+            assert torch.equal(lam, lam_b)
+            if first is None:
+                first = [t.clone() for t in got]
+            else:
+                for a, b in zip(first, got):
+                    assert torch.equal(a, b)
+    finally:
+        L.ltv_set_option(L.LTV_OPT_VECTOR_CLUSTER, 0)
+    A0, B0 = A[0].cpu().numpy(), B[0].cpu().numpy()
+    rl, rgu, rgx = O.adjoint_item(A0, B0, gg[0].cpu().numpy())
+    _check(dict(x=first[0][0].cpu().numpy(), lam=first[1][0].cpu().numpy(), grad_u=first[2][0].cpu().numpy(), grad_x0=first[3][0].cpu().numpy()),
+           dict(x=O.rollout_item(A0, B0, c[0].cpu().numpy(), x0[0].cpu().numpy(), u[0].cpu().numpy()), lam=rl, grad_u=rgu, grad_x0=rgx))
 
 
 def _all_vs_oracle(L, W, two_norm=False, exact=False, layout=None):
