@@ -335,8 +335,8 @@ static const int* adjoint_max_active() {
 
 int adjoint_cluster_choice(const AdjointArgs& a) { return pick_cluster_model(a.batch, a.n, adjoint_max_active(), a.sm_budget); }
 
-int adjoint_cluster_fit(const AdjointArgs& a, int max_ctas) {
-  return fit_cluster_single_wave(a.batch, a.n, adjoint_max_active(), max_ctas);
+int adjoint_clusters_resident(const AdjointArgs& a, int cluster) {
+  return (cluster >= 1 && cluster <= 16) ? adjoint_max_active()[cluster] : 0;
 }
 
 cudaError_t launch_adjoint(const AdjointArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches) {

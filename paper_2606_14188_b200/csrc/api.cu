@@ -1,5 +1,6 @@
 // extern "C" boundary of libltvscan.so (include/ltv_scan.h): argument validation, workspace sizing,
 // device check, dispatch to the launchers.  No torch types, no exceptions across the ABI.
+#include <algorithm>
 #include <atomic>
 #include <cstdio>
 #include <cstdlib>
@@ -70,16 +71,6 @@ int pick_cluster_model(int batch, int n, const int* max_active, int sm_budget) {
       best_t = t;
       best = c;
     }
-  }
-  return best;
-}
-
-int fit_cluster_single_wave(int batch, int n, const int* max_active, int max_ctas) {
-  int best = 0;
-  for (int c = 1; c <= 16; ++c) {
-    if (max_active[c] < batch || static_cast<long long>(batch) * c > max_ctas) continue;
-    if (c > 1 && (n / c < 32 || (n >> 2) < c)) continue;
-    best = c;
   }
   return best;
 }
@@ -349,21 +340,29 @@ int ltv_scan_rollout_adjoint(const float* A, const float* B, const float* c, con
   // both fit into half the machine, back to back on the caller's stream otherwise.
   RolloutArgs ra{A, B, c, x0, u, x_out, batch, T, n, m};
   AdjointArgs aa{A, B, g, lambda_out, grad_u_out, grad_x0_out, batch, T, n, m};
-  const long long ctas_r = static_cast<long long>(batch) * rollout_cluster_choice(ra);
-  const long long ctas_a = static_cast<long long>(batch) * adjoint_cluster_choice(aa);
-  bool side_by_side = ctas_r <= sms / 2 && ctas_a <= sms / 2;
+  const int cfr = rollout_cluster_choice(ra), cfa = adjoint_cluster_choice(aa);
+  // Side by side or back to back?  Measured on B200 ("the pair"):
+  //  - a scan that ALONE runs on >= 80 % of the SMs with >= 128 rows (columns) per CTA streams at 0.8-1.0 of the HBM peak
+  //    (n = 300 x 64 items): nothing to gain, the two would only get in each other's way -> back to back;
+  //  - otherwise each scan alone is short of CTAs (few items: 4 x 16-CTA clusters = 64 SMs) or of work per step (n = 180: two
+  //    CTAs per item exchange the state every 1.3 us), and both at once on half the machine each move more, PROVIDED every
+  //    cluster of both kernels is resident at the same time - else the last cluster waits for a slot and the pair is slower
+  //    than back to back (n = 2400 x 4 items: 4 + 4 clusters of 16 on 7 slots 0.665 ms, back to back 0.631, 4 + 4 clusters of
+  //    10 side by side 0.536).  So: the widest cluster size c with batch c <= SMs / 2 and 2 batch clusters resident.
+  auto slots = [&](int c) { return std::min(rollout_clusters_resident(ra, c), adjoint_clusters_resident(aa, c)); };
+  const bool alone_good = std::min(batch * cfr, batch * cfa) * 10 >= sms * 8 && n / std::max(cfr, cfa) >= 128;
   int cl_r = 0, cl_a = 0;   // CTAs per item of the two scans; 0 = each kernel's own model
-  if (!side_by_side) {
-    // Second case (measured, round 2): few items of a SMALL system.  Alone, each scan spreads an item over more CTAs than
-    // its short steps can feed (n = 180, batch 64: two CTAs per item exchange the state every 1.3 us and reach 0.55-0.7 of
-    // the HBM peak); restricted to half the machine each (one wave of the widest clusters that fit there), with <= 192 rows (columns) per CTA, the two scans together move
-    // more: 0.263 -> 0.200 ms at n = 180 x 64 items, 0.185 -> 0.127 ms at n = 300 x 32.  With more rows per CTA a CTA
-    // cannot keep up with its share (n = 300 x 64 items, one CTA per item: 0.280 against 0.239 ms), so the rule stops there.
-    const int cr = rollout_cluster_fit(ra, sms / 2), ca = adjoint_cluster_fit(aa, sms / 2);   // widest single-wave clusters
-    if (cr > 0 && ca > 0 && n / cr <= 192 && n / ca <= 192 && option(LTV_OPT_VECTOR_CLUSTER) == 0) {
+  bool side_by_side = false;
+  if (!alone_good && option(LTV_OPT_VECTOR_CLUSTER) == 0) {
+    int c = 0;
+    for (int cc = 1; cc <= 16; ++cc) {
+      if (static_cast<long long>(batch) * cc > sms / 2 || 2 * batch > slots(cc)) continue;
+      if (cc > 1 && (n / cc < 32 || (n >> 2) < cc)) continue;
+      c = cc;
+    }
+    if (c > 0) {
       side_by_side = true;
-      cl_r = cr;
-      cl_a = ca;
+      cl_r = cl_a = c;
     }
   }
   unsigned long long l = 0;

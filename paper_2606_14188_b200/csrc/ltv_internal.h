@@ -18,8 +18,7 @@ struct RolloutArgs {
 // cluster = 0: chosen by pick_cluster_model
 cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches);
 int rollout_cluster_choice(const RolloutArgs& a);   // the cluster size `cluster = 0` would pick
-// widest cluster with which ALL items run at once on at most max_ctas CTAs (>= 32 rows per CTA); 0 if none
-int rollout_cluster_fit(const RolloutArgs& a, int max_ctas);
+int rollout_clusters_resident(const RolloutArgs& a, int cluster);   // clusters of that size that can be resident at once
 
 struct AdjointArgs {
   const float *A, *B, *g;
@@ -29,7 +28,7 @@ struct AdjointArgs {
 };
 cudaError_t launch_adjoint(const AdjointArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches);
 int adjoint_cluster_choice(const AdjointArgs& a);
-int adjoint_cluster_fit(const AdjointArgs& a, int max_ctas);
+int adjoint_clusters_resident(const AdjointArgs& a, int cluster);
 
 struct PhiArgs {
   const float *A, *w;
@@ -115,7 +114,6 @@ cudaError_t launch_fused_small(const FusedSmallArgs& a, cudaStream_t stream, uns
 // that can be resident at once (cudaOccupancyMaxActiveClusters; 0 = not launchable).  Minimises a simple
 // time model over the waves of clusters: an SM streams ~70 GB/s, the device ~6.5 TB/s (both measured).
 int pick_cluster_model(int batch, int n, const int* max_active, int sm_budget = 0);
-int fit_cluster_single_wave(int batch, int n, const int* max_active, int max_ctas);
 // fills max_active[1..16] for `kernel` (any __global__ function pointer) at the given block size / dynamic smem
 void query_max_active_clusters(const void* kernel, int threads, size_t smem, int* max_active);
 // developer override LTV_SCAN_<name>=<int>, compiled in only with -DLTV_TUNING; the product build returns `dflt`

@@ -437,8 +437,8 @@ int rollout_cluster_choice(const RolloutArgs& a) {
   return pick_cluster_model(a.batch, a.n, rollout_max_active(a.n > kModeAMaxN ? 1 : 0), a.sm_budget);
 }
 
-int rollout_cluster_fit(const RolloutArgs& a, int max_ctas) {
-  return fit_cluster_single_wave(a.batch, a.n, rollout_max_active(a.n > kModeAMaxN ? 1 : 0), max_ctas);
+int rollout_clusters_resident(const RolloutArgs& a, int cluster) {
+  return (cluster >= 1 && cluster <= 16) ? rollout_max_active(a.n > kModeAMaxN ? 1 : 0)[cluster] : 0;
 }
 
 cudaError_t launch_rollout(const RolloutArgs& a, int cluster, cudaStream_t stream, unsigned long long* launches) {
