@@ -241,6 +241,11 @@ LTV_API int ltv_scan_constraint_tightening(const float* A, const float* w, const
  *              Sklansky prefix scan, ceil(log2(T+1)) launches with one CTA per combination (Gauss-Jordan with partial
  *              pivoting and the five products in shared memory), then the gains of all steps in one pass.  n <= 64
  *              (LTV_ERR_UNSUPPORTED_SHAPE beyond).  Picked for small n and batch (T+1)/2 <= 2 x SM count.
+ *              ACCURACY: the combination solves (I + D~ P~) X = [A~ | D~] in fp32, D~ = C^T (F F^T)^-1 C; its condition number
+ *              grows like max(C^2 / f^2) ||Pi||, so with very small observation noise against a large prior (say f ~ 1e-5,
+ *              Pi0 ~ 1) the scan loses digits where the recursion - whose only inverse is the p x p innovation covariance -
+ *              does not (tests/test_gpu_kalman.py has the case).  The library cannot look at device data when it picks:
+ *              pass LTV_KALMAN_RECURSION for such models.
  *   recursion  time-sequential, batch-parallel: per step one pass forms G = C Pi, the p x p innovation covariance (Cholesky), the
  * gain and the closed-loop matrix Abar_j = A_j + Lt_j C_j, then two batched 3xTF32 tcgen05 GEMMs form
  * Pi_{j+1} = A_j (Abar_j Pi_j)^T + E E^T (fp32 FMA for n < 96).  ~10x fewer flops than the scan: the faster form

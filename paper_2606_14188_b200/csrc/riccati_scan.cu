@@ -203,9 +203,11 @@ __global__ void __launch_bounds__(kRicThreads, 1) riccati_combine_kernel(const R
             wv[u] = W[(i0 + u) * ldw + c];
           }
 #pragma unroll
-          for (int u = 0; u < 8; ++u) W[(i0 + u) * ldw + c] = fmaf(-fac[u], wkc, wv[u]);
+          for (int u = 0; u < 8; ++u)
+            if (i0 + u != k) W[(i0 + u) * ldw + c] = fmaf(-fac[u], wkc, wv[u]);   // row k is read by the other half: leave it alone
         }
-        for (; i0 < r1; ++i0) W[i0 * ldw + c] = fmaf(-s_fac[i0], wkc, W[i0 * ldw + c]);
+        for (; i0 < r1; ++i0)
+          if (i0 != k) W[i0 * ldw + c] = fmaf(-s_fac[i0], wkc, W[i0 * ldw + c]);
       }
     }
     __syncthreads();
