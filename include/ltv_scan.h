@@ -235,17 +235,18 @@ LTV_API int ltv_scan_constraint_tightening(const float* A, const float* w, const
  *   Lt_out   device [batch,T,n,p]      Lt_out[b,j] = L_{j+1}^T, the gain formed from (A_j, C_j, Pi_j): exactly the `Lt`
  *                                      array of ltv_scan_observer_response (A_j + Lt_j C_j closes the loop around A_j)
  *   Pi_out   device [batch,T+1,n,n]    Pi_out[b,j] = Pi_j (Pi_out[b,0] = Pi0)
- *   flags    0 (the library picks), LTV_KALMAN_SCAN or LTV_KALMAN_RECURSION (not both)
- * Two device paths give the same Pi_j, L_j up to rounding:
+ *   flags    0 or LTV_KALMAN_RECURSION: the recursion; LTV_KALMAN_SCAN: the paper's associative scan (not both)
+ * Two device paths give the same Pi_j, L_j up to rounding on well-conditioned models:
  *   scan       PAPER.md:166-177: the associative elements (17) combined by rule (16) (re-derived, DESIGN.md q14) in a
  *              Sklansky prefix scan, ceil(log2(T+1)) launches with one CTA per combination (Gauss-Jordan with partial
  *              pivoting and the five products in shared memory), then the gains of all steps in one pass.  n <= 64
- *              (LTV_ERR_UNSUPPORTED_SHAPE beyond).  Picked for small n and batch (T+1)/2 <= 2 x SM count.
+ *              (LTV_ERR_UNSUPPORTED_SHAPE beyond).  Logarithmic depth: the faster form for ONE small problem (n = 40, batch 1:
+ *              417 vs 927 us at T = 32, 550 vs 3677 us at T = 128).  Runs only on request, because of its
  *              ACCURACY: the combination solves (I + D~ P~) X = [A~ | D~] in fp32, D~ = C^T (F F^T)^-1 C; its condition number
- *              grows like max(C^2 / f^2) ||Pi||, so with very small observation noise against a large prior (say f ~ 1e-5,
- *              Pi0 ~ 1) the scan loses digits where the recursion - whose only inverse is the p x p innovation covariance -
- *              does not (tests/test_gpu_kalman.py has the case).  The library cannot look at device data when it picks:
- *              pass LTV_KALMAN_RECURSION for such models.
+ *              grows like max(C^2 / f^2) ||Pi||.  Measured at n = 48 against the fp64 oracle: within 1e-4 for f >= 1e-3 with
+ *              Pi0 ~ 1e-4 (the library's test models) and for f = 1e-2 with Pi0 = 0.01 I; gains off by 7.5e-3 at Pi0 = 0.01 I,
+ *              f = 1e-3, by 2.5e-2 at Pi0 = I, f = 1e-2, NaN beyond - where the recursion, whose only inverse is the p x p
+ *              innovation covariance, stays at 1e-5 .. 5e-4 (tests/test_gpu_kalman.py has the case).
  *   recursion  time-sequential, batch-parallel: per step one pass forms G = C Pi, the p x p innovation covariance (Cholesky), the
  * gain and the closed-loop matrix Abar_j = A_j + Lt_j C_j, then two batched 3xTF32 tcgen05 GEMMs form
  * Pi_{j+1} = A_j (Abar_j Pi_j)^T + E E^T (fp32 FMA for n < 96).  ~10x fewer flops than the scan: the faster form

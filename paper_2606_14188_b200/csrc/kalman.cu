@@ -424,8 +424,12 @@ static bool kalman_use_scan(const KalmanArgs& a, int sms) {
   if (a.mode == 1) return true;
   const int forced = env_int("KALMAN_SCAN", -1);
   if (forced >= 0) return forced != 0;
-  // measured on B200 (n = 48, p = 6): T = 16: 414 vs 465 us, T = 64: 578 vs 1841 us, T = 128: 665 vs 3675 us (batch 1-8)
-  return a.T >= 16 && static_cast<long long>(a.batch) * (a.T + 1) / 2 <= 2ll * sms;
+  // The scan is faster for one small problem (n = 40, batch 1: 417 vs 927 us at T = 32, 550 vs 3677 us at T = 128), but its
+  // fp32 n x n solves lose digits as max(C^2 / f^2) ||Pi|| grows (measured, n = 48: Pi0 = 0.01 I, f = 1e-3: gains off by 7.5e-3;
+  // Pi0 = I, f = 1e-2: 2.5e-2; NaN beyond) where the recursion stays at 1e-5 .. 5e-4.  The library cannot look at device data when
+  // it picks, so the scan runs only when the caller asks for it (LTV_KALMAN_SCAN).
+  (void)sms;
+  return false;
 }
 
 cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned long long* launches) {
