@@ -247,7 +247,8 @@ LTV_API int ltv_scan_constraint_tightening(const float* A, const float* w, const
  *              Pi0 ~ 1e-4 (the library's test models) and for f = 1e-2 with Pi0 = 0.01 I; gains off by 7.5e-3 at Pi0 = 0.01 I,
  *              f = 1e-3, by 2.5e-2 at Pi0 = I, f = 1e-2, NaN beyond - where the recursion, whose only inverse is the p x p
  *              innovation covariance, stays at 1e-5 .. 5e-4 (tests/test_gpu_kalman.py has the case).
- *   recursion  time-sequential, batch-parallel: per step one pass forms G = C Pi, the p x p innovation covariance (Cholesky), the
+ *   recursion  n <= 64: the whole recursion of an item in ONE CTA, one launch for the batch (Pi_j stays in shared memory, fp32 FMA;
+ *              n = 40, batch 1: 363 us at T = 32 against 927 us for the batched form below).  Larger n: time-sequential, batch-parallel: per step one pass forms G = C Pi, the p x p innovation covariance (Cholesky), the
  * gain and the closed-loop matrix Abar_j = A_j + Lt_j C_j, then two batched 3xTF32 tcgen05 GEMMs form
  * Pi_{j+1} = A_j (Abar_j Pi_j)^T + E E^T (fp32 FMA for n < 96).  ~10x fewer flops than the scan: the faster form
  *              whenever one time step over the batch fills the machine.

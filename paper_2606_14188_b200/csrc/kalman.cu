@@ -450,6 +450,7 @@ cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned lon
     if (es == cudaSuccess) *launches += 3;
     return es;
   }
+  if (kalman_small_supported(n, p)) return launch_kalman_small(a, stream, launches);   // one launch, Pi_j in shared memory
   KalmanWs w;
   char* cur = static_cast<char*>(a.workspace);
   w.G = reinterpret_cast<float*>(cur); cur += carve(b * pp * nn);

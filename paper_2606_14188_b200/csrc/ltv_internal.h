@@ -69,6 +69,9 @@ bool riccati_scan_supported(int n);
 size_t riccati_scan_workspace_bytes(int batch, int T, int n);
 cudaError_t launch_riccati_scan(const KalmanArgs& a, float* AD, cudaStream_t stream, unsigned long long* launches);
 size_t kalman_workspace_bytes(int batch, int T, int n, int p);
+// kalman_small.cu: the whole recursion of an item in one CTA (n <= 64)
+bool kalman_small_supported(int n, int p);
+cudaError_t launch_kalman_small(const KalmanArgs& a, cudaStream_t stream, unsigned long long* launches);
 cudaError_t launch_kalman(const KalmanArgs& a, cudaStream_t stream, unsigned long long* launches);
 
 // Constraint-tightening margins of eq.(12d) (constraints.cu)
