@@ -63,6 +63,17 @@ def test_kalman_dense_random(L, n, T, batch, p, kind):
     _check(L, W.A, M)
 
 
+@pytest.mark.parametrize("n,T,batch,p", [(4, 1, 2, 1), (4, 5, 1, 3), (8, 2, 3, 8), (12, 9, 2, 5), (40, 7, 70, 6),
+                                         (64, 4, 3, 32), (60, 3, 2, 17), (64, 33, 1, 1)])
+def test_kalman_small_single_launch_edges(L, n, T, batch, p):
+    """The single-launch recursion of small systems (csrc/kalman_small.cu, n <= 64: one CTA per item): smallest and largest n and
+    p, a single step, more items than SMs would hold at once, odd p, a horizon longer than a warp."""
+    W = dense_random(batch, T, n, 1, seed=11 * n + p + T, scale=0.4)
+    M = observation_model(batch, T, n, p, seed=13 * n + p, kind="dense")
+    _check(L, W.A, M)
+    _check(L, W.A, M, mode=L.LTV_KALMAN_RECURSION)
+
+
 @pytest.mark.parametrize("n,T,batch,p,kind", [(48, 16, 1, 6, "track"),    # C1 shape: 17 elements, 5 levels
                                               (48, 6, 2, 3, "dense"),     # 7 elements: ragged last segment
                                               (64, 9, 3, 8, "dense"),     # largest n of the scan path
