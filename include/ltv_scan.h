@@ -327,7 +327,7 @@ LTV_API int ltv_scan_output_feedback_constraints(const float* A, const float* B,
  * phi_host may be NULL.  *phi_device_out (if not NULL) receives the device address of Phi inside workspace.
  * w_host == NULL skips the system-response / tube stage (rollout + adjoint only, BASELINE.json configs[4]): r_host
  * is then not written and may be NULL, and the workspace need is LTV_OP_PIPELINE_HOST_NO_PHI.
- * The batch is processed in up to four chunks (multiples of 4 items): an internal non-blocking copy stream,
+ * The batch is processed in up to eight chunks (LTV_OPT_PIPELINE_CHUNKS; multiples of 4 items): an internal non-blocking copy stream,
  * created and destroyed inside the call, uploads chunk i+1 while chunk i is computed on `cuda_stream` (items
  * are independent, so this changes no result); host buffers should be pinned for the copies to overlap. */
 LTV_API int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float* c_host,
@@ -345,7 +345,7 @@ LTV_API int ltv_scan_pipeline_host(const float* A_host, const float* B_host, con
  *                            0 (default) = chosen by an occupancy / bandwidth model, 1 .. 16 = forced (falls back to 1
  *                            if that cluster cannot be placed).  Used by the tests to cover every cluster size.
  *   LTV_OPT_PIPELINE_CHUNKS  number of batch chunks ltv_scan_pipeline_host overlaps upload and compute over:
- *                            1 .. 16, default 4 (1 = no overlap).
+ *                            1 .. 16, default 8 (1 = no overlap; C2: 16.0 ms with 4, 15.2 ms with 8 - the upload at PCIe rates is the long leg, more chunks shorten the exposed last compute).
  * ltv_set_option returns LTV_ERR_BAD_DIM for an unknown option or a value out of range; ltv_get_option returns -1 for
  * an unknown option. */
 enum { LTV_OPT_VECTOR_CLUSTER = 0, LTV_OPT_PIPELINE_CHUNKS = 1, LTV_OPT_COUNT = 2 };
