@@ -55,7 +55,9 @@ typedef enum {
   LTV_ERR_ALIGNMENT = 4,           /* a device pointer is not 16-byte aligned                         */
   LTV_ERR_WORKSPACE_TOO_SMALL = 5, /* workspace_bytes < ltv_scan_workspace_bytes(...)                 */
   LTV_ERR_ARCH = 6,                /* current device is not compute capability 10.x                   */
-  LTV_ERR_CUDA = 7                 /* a CUDA runtime / driver call failed: see ltv_last_cuda_error()  */
+  LTV_ERR_CUDA = 7,                /* a CUDA runtime / driver call failed: see ltv_last_cuda_error()  */
+  LTV_ERR_STATIC_SCRATCH_LIMIT = 8 /* ltv_scan_system_response_tube_static: the problem needs more scratch than the
+                                      library's fixed device array holds (ltv_static_scratch_bytes())      */
 } ltv_status;
 
 /* `op` argument of ltv_scan_workspace_bytes */
@@ -128,6 +130,21 @@ LTV_API int ltv_scan_rollout(const float* A, const float* B, const float* c, con
 LTV_API int ltv_scan_system_response_tube(const float* A, const float* w, float* phi_out, float* r_out,
                                   int batch, int T, int n, int phi_layout, unsigned flags,
                                   void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* The same call for callers that cannot allocate device memory at all (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): no workspace argument.  The scratch the call needs - the tube partial sums, exactly
+ * ltv_scan_workspace_bytes(LTV_OP_SYSTEM_RESPONSE_TUBE, batch, T, n, 0) bytes - lives in a device array of FIXED size inside
+ * the library: ltv_static_scratch_bytes() = 32 MiB, held by every GPU that loads the library until the process exits (enough
+ * for BASELINE.json configs[0] whole, ~27 items of configs[1], 6 of configs[2], one of configs[3]).  Problems that need more
+ * return LTV_ERR_STATIC_SCRATCH_LIMIT before anything is enqueued: split the batch, or use the regular call with a workspace.
+ * The library calls no cudaMalloc, cudaFree or other allocating routine in this call.  Arguments, results and kernels are those
+ * of ltv_scan_system_response_tube with phi_layout = LTV_PHI_COLUMN_PACKED (the only layout here: the others need a second
+ * Phi-sized buffer).  SHARING: every call on a device uses the same array.  It keeps the previous call's contents, which is
+ * harmless - each call writes every partial sum before it reads it, nothing needs to start at zero - but two calls that
+ * overlap on the GPU (different streams without ordering between them) race on it; calls on one stream are safe. */
+LTV_API size_t ltv_static_scratch_bytes(void);
+LTV_API int ltv_scan_system_response_tube_static(const float* A, const float* w, float* phi_out, float* r_out,
+                                                 int batch, int T, int n, unsigned flags, void* cuda_stream);
 
 /* Adjoint scan (north_star (iii); eq.(10) chained over the horizon) for
  * L = sum_{t=1}^{T} l_t(x_t), g_t = dl_t/dx_t, lam_{T+1} = 0:

@@ -15,7 +15,9 @@ LTV_OK = 0
 STATUS_NAMES = {
     0: "LTV_OK", 1: "LTV_ERR_NULL_PTR", 2: "LTV_ERR_BAD_DIM", 3: "LTV_ERR_UNSUPPORTED_SHAPE",
     4: "LTV_ERR_ALIGNMENT", 5: "LTV_ERR_WORKSPACE_TOO_SMALL", 6: "LTV_ERR_ARCH", 7: "LTV_ERR_CUDA",
+    8: "LTV_ERR_STATIC_SCRATCH_LIMIT",
 }
+LTV_ERR_STATIC_SCRATCH_LIMIT = 8
 LTV_OP_ROLLOUT, LTV_OP_SYSTEM_RESPONSE_TUBE, LTV_OP_ADJOINT, LTV_OP_PIPELINE_HOST = 0, 1, 2, 3
 LTV_OP_PIPELINE_HOST_NO_PHI = 4
 LTV_OP_OBSERVER_RESPONSE = 5
@@ -36,6 +38,7 @@ EXPORTS = (
     "ltv_observer_row_floats", "ltv_scan_kalman_gains",
     "ltv_scan_constraint_tightening", "ltv_scan_output_feedback_response", "ltv_set_option", "ltv_get_option",
     "ltv_profile_class_name", "ltv_scan_rollout_adjoint", "ltv_scan_all", "ltv_scan_all_is_fused", "ltv_scan_output_feedback_constraints", "ltv_scan_output_feedback_constraints_workspace_bytes",
+    "ltv_static_scratch_bytes", "ltv_scan_system_response_tube_static",
 )
 
 
@@ -62,6 +65,10 @@ def _load() -> ctypes.CDLL:
     L.ltv_scan_rollout.argtypes = [fp] * 6 + [i] * 4 + [vp, sz, vp]
     L.ltv_scan_system_response_tube.restype = i
     L.ltv_scan_system_response_tube.argtypes = [fp] * 4 + [i] * 4 + [ctypes.c_uint, vp, sz, vp]
+    L.ltv_static_scratch_bytes.restype = sz
+    L.ltv_static_scratch_bytes.argtypes = []
+    L.ltv_scan_system_response_tube_static.restype = i
+    L.ltv_scan_system_response_tube_static.argtypes = [fp] * 4 + [i] * 3 + [ctypes.c_uint, vp]
     L.ltv_scan_adjoint.restype = i
     L.ltv_scan_adjoint.argtypes = [fp] * 6 + [i] * 4 + [vp, sz, vp]
     L.ltv_scan_rollout_adjoint.restype = i
@@ -207,6 +214,28 @@ def ltv_scan_system_response_tube(A, w, phi_out=None, r_out=None, workspace=None
                                            _ptr(workspace), workspace.numel(), _stream())
     if st != LTV_OK:
         raise LtvError(st, "ltv_scan_system_response_tube")
+    return phi_out, r_out
+
+
+def ltv_static_scratch_bytes():
+    return int(lib.ltv_static_scratch_bytes())
+
+
+def ltv_scan_system_response_tube_static(A, w, phi_out, r_out, two_norm=False):
+    """ltv_scan_system_response_tube without any workspace: the library's fixed 32 MiB device array is the scratch, nothing is
+    allocated by the library or by this binding (phi_out[batch,P,n,n] COLUMN_PACKED and r_out[batch,T,n] must be given).
+    Raises LtvError(LTV_ERR_STATIC_SCRATCH_LIMIT) if the problem needs more scratch.  Calls that overlap on the GPU race on
+    the shared array; calls on one stream are safe."""
+    batch, T, n, _ = A.shape
+    P = T * (T - 1) // 2
+    _dev(A, "A", (batch, T, n, n)); _dev(w, "w", (batch, T, n))
+    if phi_out is None or r_out is None:
+        raise ValueError("ltv_scan_system_response_tube_static allocates nothing: pass phi_out and r_out")
+    _dev(phi_out, "phi_out", (batch, P, n, n)); _dev(r_out, "r_out", (batch, T, n))
+    st = lib.ltv_scan_system_response_tube_static(_ptr(A), _ptr(w), _ptr(phi_out), _ptr(r_out), batch, T, n,
+                                                  LTV_TUBE_ROW_2NORM if two_norm else 0, _stream())
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_system_response_tube_static")
     return phi_out, r_out
 
 

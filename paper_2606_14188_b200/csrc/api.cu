@@ -142,6 +142,9 @@ static int fail_cuda(cudaError_t e) {
   return LTV_ERR_CUDA;
 }
 
+void count_launches(unsigned long long n) { g_launches += n; }
+int report_cuda_error(cudaError_t e) { return fail_cuda(e); }
+
 // several kernels of the NEXT calls map the batch (or batch x steps) onto gridDim.y / gridDim.z (<= 65535)
 static bool grid_yz_overflow(long long v) { return v > 65535; }
 
@@ -748,6 +751,7 @@ const char* ltv_status_string(int status) {
     case LTV_ERR_WORKSPACE_TOO_SMALL: return "LTV_ERR_WORKSPACE_TOO_SMALL";
     case LTV_ERR_ARCH: return "LTV_ERR_ARCH";
     case LTV_ERR_CUDA: return "LTV_ERR_CUDA";
+    case LTV_ERR_STATIC_SCRATCH_LIMIT: return "LTV_ERR_STATIC_SCRATCH_LIMIT";
     default: return "LTV_ERR_UNKNOWN";
   }
 }

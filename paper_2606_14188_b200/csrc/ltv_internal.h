@@ -123,6 +123,10 @@ void query_max_active_clusters(const void* kernel, int threads, size_t smem, int
 int env_int(const char* name, int dflt);
 // value of a documented ltv_set_option knob (include/ltv_scan.h)
 int option(int which);
+// for entry points that live outside api.cu: add to the library's launch counter; record a failed CUDA call for
+// ltv_last_cuda_error (clears the runtime's error state) and return LTV_ERR_CUDA
+void count_launches(unsigned long long n);
+int report_cuda_error(cudaError_t e);
 
 // optional per-kernel timing (ltv_profile_enable): CUDA events recorded on the launch stream around a kernel
 enum ProfClass { kProfRollout = 0, kProfAdjoint, kProfPhiLevel0, kProfPhiCombineTc, kProfPhiCombineSimt,
