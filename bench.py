@@ -524,6 +524,20 @@ def next_rows(B, L, W, steps):
                                               note="Phi^uw, Phi^ue of (15) + sigma of (12d): backward sweep on the 2n-state closed loop")
     del wsq
     torch.cuda.empty_cache()
+    # NEXT-4, general Phibar: eq.(15) + tube (12e) for a state-feedback response given as block operators (here: the
+    # response of A + B Kfb and Kfb Phibar^x, produced on the device by the library's own Phi scan - input preparation,
+    # outside the timed calls)
+    Atil = d["A"] + torch.matmul(d["B"], Kfb)
+    pbx, _ = L.ltv_scan_system_response_tube(Atil, d["w"])
+    del Atil
+    pbu = torch.zeros((batch, P + T, m, n), device=dev)
+    wsa = torch.empty(L.lib.ltv_scan_output_feedback_assemble_workspace_bytes(batch, T, n, m, p), dtype=torch.uint8, device=dev)
+    ms = timed(lambda: L.ltv_scan_output_feedback_assemble(d["A"], Lt, Cm, d["w"], ff, pbx, pbu, workspace=wsa), min(steps, 3))
+    out["output_feedback_assemble"] = dict(p=p, ms=ms, blocks_per_s=batch * B.world * P / (ms * 1e-3),
+                                           note="general Phibar: all four operators of (15) + tube, backward recursion over the columns "
+                                                "(one n^3 product per block, T-1 batched tcgen05 GEMMs + fused row kernels)")
+    del pbx, pbu, wsa
+    torch.cuda.empty_cache()
     return out
 
 

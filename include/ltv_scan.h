@@ -334,6 +334,40 @@ LTV_API int ltv_scan_output_feedback_constraints(const float* A, const float* B,
                                                  int batch, int T, int n, int m, int p, int nc, unsigned flags,
                                                  void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Eq.(15) for a GENERAL state-feedback response: Phibar = (Phibar^x, Phibar^u) is given
+ * as block operators - e.g. the solution of the state-feedback SLS problem - instead of being generated from gains; the
+ * observer response Phihat is that of the gains of (13)/(14) as in ltv_scan_output_feedback_response (Phihat^x(k,j) =
+ * Abar_{k-1} .. Abar_j, Abar_j = A_j + Lt_j C_j, Phihat^y(k,j) = Phihat^x(k,j) Lt_{j-1}; DESIGN.md q20, q21).  With M = I - Z A:
+ *     Phi^xw = Phibar^x + Phihat^x - Phibar^x M Phihat^x,    Phi^uw = Phibar^u (I - M Phihat^x),
+ *     Phi^xe = Phihat^y - Phibar^x M Phihat^y,               Phi^ue = -Phibar^u M Phihat^y,
+ *     tau_0 = 0;  tau_k[i] = sum_{j<k} ||row_i(Phi^xw(k,j) diag(w_j))||_2 + sum_{1<=j<k} ||row_i(Phi^xe(k,j) diag(f_{j-1}))||_2
+ *   A, Lt, C, w, f  as in ltv_scan_output_feedback_response (all required; 1 <= p <= 32)
+ *   phibar_x   device [batch,P,n,n]     blocks (k,j), 0 <= j < k <= T-1, COLUMN_PACKED (ltv_phi_block_index); the diagonal
+ *                                       blocks are NOT passed: Phibar^x(k,k) = I for every achievable response
+ *   phibar_u   device [batch,P+T,m,n]   blocks (k,j), 0 <= j <= k <= T-1, INCLUDING the diagonal: column j holds its T - j
+ *                                       blocks k = j .. T-1 one after the other, block index j T - j(j-1)/2 + (k - j);
+ *                                       required iff phi_uw_out != NULL
+ *   phi_xw_out device [batch,P,n,n]     COLUMN_PACKED, strictly-lower blocks (Phi^xw(k,k) = I)
+ *   phi_xe_out device [batch,P,n,p]     same order; blocks with j = 0 are zero; may be NULL
+ *   phi_uw_out device [batch,P,m,n]     same order (Phi^uw(k,k) = 0); may be NULL
+ *   phi_ue_out device [batch,P,m,p]     same order, j = 0 zero (the diagonal blocks Phi^ue(k,k) = -Phibar^u(k,k) Lt_{k-1} are
+ *                                       not part of the output); may be NULL; needs phi_uw_out
+ *   tau_out    device [batch,T,n]       may be NULL
+ *   flags      must be 0
+ * Method: no block-operator product is formed.  M is block bidiagonal and Phihat^x(i,j) = Phihat^x(i,j+1) Abar_j, so
+ *     Phi^xw(k,j) = Phi^xw(k,j+1) Abar_j - [Phibar^x(k,j+1) Lt_j] C_j  (Phi^xw(k,k) = I),   same for Phi^uw with Phibar^u (start 0),
+ *     Phi^xe(k,j) = (Phi^xw - Phibar^x)(k,j) Lt_{j-1},   Phi^ue(k,j) = (Phi^uw - Phibar^u)(k,j) Lt_{j-1}
+ * (pinned against the oracle's dense evaluation of (15)): one n^3 product per block - as many as the Phi scan - in T-1
+ * backward steps, each one batched GEMM of the stacked column j+1 with Abar_j (tcgen05 3xTF32 for n >= 96) plus a fused row
+ * kernel (rank-p correction, Phi^xe / Phi^ue, tube).  Deterministic.  batch <= 65535.
+ * Workspace: ltv_scan_output_feedback_assemble_workspace_bytes(batch, T, n, m, p). */
+LTV_API size_t ltv_scan_output_feedback_assemble_workspace_bytes(int batch, int T, int n, int m, int p);
+LTV_API int ltv_scan_output_feedback_assemble(const float* A, const float* Lt, const float* C, const float* w,
+                                              const float* f, const float* phibar_x, const float* phibar_u,
+                                              float* phi_xw_out, float* phi_xe_out, float* phi_uw_out, float* phi_ue_out,
+                                              float* tau_out, int batch, int T, int n, int m, int p, unsigned flags,
+                                              void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* One pass of the whole hot path from HOST buffers: copies A, B, c, x0, u, w, g host->device into
  * `workspace` (device, >= ltv_scan_workspace_bytes(LTV_OP_PIPELINE_HOST, ...)), runs the path (ltv_scan_rollout_adjoint, then
  * ltv_scan_system_response_tube)

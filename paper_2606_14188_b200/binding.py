@@ -39,6 +39,7 @@ EXPORTS = (
     "ltv_scan_constraint_tightening", "ltv_scan_output_feedback_response", "ltv_set_option", "ltv_get_option",
     "ltv_profile_class_name", "ltv_scan_rollout_adjoint", "ltv_scan_all", "ltv_scan_all_is_fused", "ltv_scan_output_feedback_constraints", "ltv_scan_output_feedback_constraints_workspace_bytes",
     "ltv_static_scratch_bytes", "ltv_scan_system_response_tube_static",
+    "ltv_scan_output_feedback_assemble", "ltv_scan_output_feedback_assemble_workspace_bytes",
 )
 
 
@@ -65,6 +66,10 @@ def _load() -> ctypes.CDLL:
     L.ltv_scan_rollout.argtypes = [fp] * 6 + [i] * 4 + [vp, sz, vp]
     L.ltv_scan_system_response_tube.restype = i
     L.ltv_scan_system_response_tube.argtypes = [fp] * 4 + [i] * 4 + [ctypes.c_uint, vp, sz, vp]
+    L.ltv_scan_output_feedback_assemble.restype = i
+    L.ltv_scan_output_feedback_assemble.argtypes = [fp] * 12 + [i] * 5 + [ctypes.c_uint, vp, sz, vp]
+    L.ltv_scan_output_feedback_assemble_workspace_bytes.restype = sz
+    L.ltv_scan_output_feedback_assemble_workspace_bytes.argtypes = [i] * 5
     L.ltv_static_scratch_bytes.restype = sz
     L.ltv_static_scratch_bytes.argtypes = []
     L.ltv_scan_system_response_tube_static.restype = i
@@ -215,6 +220,35 @@ def ltv_scan_system_response_tube(A, w, phi_out=None, r_out=None, workspace=None
     if st != LTV_OK:
         raise LtvError(st, "ltv_scan_system_response_tube")
     return phi_out, r_out
+
+
+def ltv_scan_output_feedback_assemble(A, Lt, C, w, f, phibar_x, phibar_u=None, want_xe=True, want_ue=True, want_tau=True,
+                                      workspace=None):
+    """Eq.(15) for a general Phibar: phibar_x[batch,P,n,n] (COLUMN_PACKED strictly-lower blocks, diagonal = I implied),
+    phibar_u[batch,P+T,m,n] (blocks j <= k incl. the diagonal, column by column) or None.  Returns a dict with phi_xw
+    [batch,P,n,n], phi_xe [batch,P,n,p] | None, phi_uw [batch,P,m,n] | None, phi_ue [batch,P,m,p] | None, tau [batch,T,n] | None."""
+    batch, T, n, _ = A.shape
+    p = C.shape[2]
+    P = T * (T - 1) // 2
+    m = 0 if phibar_u is None else phibar_u.shape[2]
+    _dev(A, "A", (batch, T, n, n)); _dev(Lt, "Lt", (batch, T, n, p)); _dev(C, "C", (batch, T, p, n))
+    _dev(w, "w", (batch, T, n)); _dev(f, "f", (batch, T, p)); _dev(phibar_x, "phibar_x", (batch, P, n, n))
+    _dev(phibar_u, "phibar_u", (batch, P + T, m, n))
+    mk = lambda *shape: torch.empty(shape, device=A.device, dtype=torch.float32)
+    out = dict(phi_xw=mk(batch, P, n, n), phi_xe=mk(batch, P, n, p) if want_xe else None,
+               phi_uw=mk(batch, P, m, n) if phibar_u is not None else None,
+               phi_ue=mk(batch, P, m, p) if (phibar_u is not None and want_ue) else None,
+               tau=mk(batch, T, n) if want_tau else None)
+    need = int(lib.ltv_scan_output_feedback_assemble_workspace_bytes(batch, T, n, m, p))
+    if workspace is None:
+        workspace = torch.empty(max(need, 16), device=A.device, dtype=torch.uint8)
+    st = lib.ltv_scan_output_feedback_assemble(_ptr(A), _ptr(Lt), _ptr(C), _ptr(w), _ptr(f), _ptr(phibar_x), _ptr(phibar_u),
+                                               _ptr(out["phi_xw"]), _ptr(out["phi_xe"]), _ptr(out["phi_uw"]),
+                                               _ptr(out["phi_ue"]), _ptr(out["tau"]), batch, T, n, m, p, 0,
+                                               _ptr(workspace), workspace.numel(), _stream())
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_output_feedback_assemble")
+    return out
 
 
 def ltv_static_scratch_bytes():

@@ -614,6 +614,39 @@ int ltv_scan_output_feedback_constraints(const float* A, const float* B, const f
   return err == cudaSuccess ? LTV_OK : fail_cuda(err);
 }
 
+size_t ltv_scan_output_feedback_assemble_workspace_bytes(int batch, int T, int n, int m, int p) {
+  if (check_dims(batch, T, n, m) != LTV_OK || p < 1 || p > 32) return 0;
+  return asm_workspace_bytes(batch, T, n, p);
+}
+
+int ltv_scan_output_feedback_assemble(const float* A, const float* Lt, const float* C, const float* w, const float* f,
+                                      const float* phibar_x, const float* phibar_u, float* phi_xw_out, float* phi_xe_out,
+                                      float* phi_uw_out, float* phi_ue_out, float* tau_out, int batch, int T, int n, int m,
+                                      int p, unsigned flags, void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!A || !Lt || !C || !w || !f || !workspace) return LTV_ERR_NULL_PTR;
+  if (T > 1 && (!phibar_x || !phi_xw_out)) return LTV_ERR_NULL_PTR;
+  if ((phi_uw_out || phi_ue_out) && !phibar_u) return LTV_ERR_NULL_PTR;
+  if (phi_ue_out && !phi_uw_out) return LTV_ERR_NULL_PTR;   // Phi^ue is derived from Phi^uw
+  int st = check_dims(batch, T, n, m);
+  if (st != LTV_OK) return st;
+  if (p < 1 || flags != 0 || (phi_uw_out && m < 1)) return LTV_ERR_BAD_DIM;
+  if (p > 32 || grid_yz_overflow(batch)) return LTV_ERR_UNSUPPORTED_SHAPE;
+  if (misaligned(A) || misaligned(Lt) || misaligned(C) || misaligned(w) || misaligned(f) || misaligned(phibar_x) ||
+      misaligned(phibar_u) || misaligned(phi_xw_out) || misaligned(phi_xe_out) || misaligned(phi_uw_out) ||
+      misaligned(phi_ue_out) || misaligned(tau_out) || misaligned(workspace))
+    return LTV_ERR_ALIGNMENT;
+  if (workspace_bytes < asm_workspace_bytes(batch, T, n, p)) return LTV_ERR_WORKSPACE_TOO_SMALL;
+  int sms = 0;
+  st = check_device(&sms);
+  if (st != LTV_OK) return st;
+  AsmArgs a{A, Lt, C, w, f, phibar_x, phi_uw_out ? phibar_u : nullptr, phi_xw_out, phi_xe_out, phi_uw_out, phi_ue_out,
+            tau_out, batch, T, n, m, p, workspace};
+  unsigned long long l = 0;
+  cudaError_t err = launch_ofb_assemble(a, static_cast<cudaStream_t>(cuda_stream), &l);
+  g_launches += l;
+  return err == cudaSuccess ? LTV_OK : fail_cuda(err);
+}
+
 int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float* c_host, const float* x0_host,
                            const float* u_host, const float* w_host, const float* g_host, float* x_host,
                            float* phi_host, float* r_host, float* lambda_host, float* grad_u_host,

@@ -295,7 +295,8 @@ __global__ void __launch_bounds__(256) bgemm_simt_kernel(const BatchedGemm g) {
   const int b = blockIdx.z;
   const float* L = g.L + (static_cast<size_t>(g.l_row0) + static_cast<size_t>(b) * g.l_row_stride) * g.K;
   const float* R = g.R + (static_cast<size_t>(g.r_blk0) + static_cast<size_t>(b) * g.r_blk_stride) * g.K * g.N;
-  float* D = g.D + (static_cast<size_t>(g.d_blk0) + static_cast<size_t>(b) * g.d_blk_stride) * (g.d_rows > 0 ? g.d_rows : g.M) * g.N;
+  float* D = g.D + (static_cast<size_t>(g.d_blk0) + static_cast<size_t>(b) * g.d_blk_stride) * (g.d_rows > 0 ? g.d_rows : g.M) * g.N +
+             (static_cast<size_t>(g.d_row0) + static_cast<size_t>(b) * g.d_row_stride) * g.N;
   const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
   const int row = blockIdx.y * 16 + ty, col = blockIdx.x * 16 + tx;
   float acc = 0.f;

@@ -104,6 +104,17 @@ struct OfbConArgs {
 size_t ofb_constraints_workspace_bytes(int batch, int T, int n, int nc, int m);
 cudaError_t launch_ofb_constraints(const OfbConArgs& a, cudaStream_t stream, unsigned long long* launches);
 
+// Eq.(15) for a general Phibar (assemble.cu)
+struct AsmArgs {
+  const float *A, *Lt, *C, *w, *f;
+  const float *phibar_x, *phibar_u;            // phibar_u null iff phi_uw null
+  float *phi_xw, *phi_xe, *phi_uw, *phi_ue, *tau;   // phi_xe, phi_uw, phi_ue, tau may be null
+  int batch, T, n, m, p;
+  void* workspace;
+};
+size_t asm_workspace_bytes(int batch, int T, int n, int p);
+cudaError_t launch_ofb_assemble(const AsmArgs& a, cudaStream_t stream, unsigned long long* launches);
+
 // Whole hot path of a small problem in one launch (fused_small.cu): n <= 64 and all of A in one SM's shared memory
 struct FusedSmallArgs {
   const float *A, *B, *c, *x0, *u, *w, *g;

@@ -39,6 +39,8 @@ struct BatchedGemm {
                 // the maps are built for d_rows, so M may then change from launch to launch)
   int transpose_out;
   const float* diag; long long diag_stride;
+  int d_row0 = 0, d_row_stride = 0;   // extra row offset d_row0 + b d_row_stride of problem b inside its D block (plain stores only:
+                                      // several problems may then share one big block, e.g. a whole column-packed Phi array)
 };
 cudaError_t bgemm_tc_make_maps(const BatchedGemm& a, void* maps_out);
 cudaError_t launch_bgemm_tc(const BatchedGemm& a, int nch, const void* maps, int num_sms, cudaStream_t stream);

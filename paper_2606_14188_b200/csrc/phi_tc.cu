@@ -61,6 +61,7 @@ struct TcGemm {
   int transpose_out;       // store D^T (the O map then describes [blocks][N][M])
   const float* diag;       // adds diag[b diag_stride + i]^2 to D[b][i][i] (E E^T with E = diag(e)); may be null
   long long diag_stride;
+  int d_row0, d_row_stride;   // row offset of problem b inside its D block: d_row0 + b d_row_stride (plain stores only)
 };
 
 struct TcParams {
@@ -335,6 +336,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
         const int rr = rbase + lane;                 // row of D[b] held by this thread
         const int rows_valid = p.gm.M - rbase;
         const int oblk = p.gm.d_blk0 + t.b * p.gm.d_blk_stride;
+        const int roff = p.gm.d_row0 + t.b * p.gm.d_row_stride;
         const bool tr = p.gm.transpose_out != 0;
         float dd = 0.f;
         if (p.gm.diag != nullptr && rr < p.gm.M) {
@@ -361,7 +363,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
           if (!tr && rows_valid < 32) {
             // ragged last m-tile, plain store: rows [M, d_rows) of the block belong to the caller (masked stores)
             if (lane < rows_valid) {
-              float* out = p.phi + (static_cast<size_t>(oblk) * p.gm.d_rows + rr) * nc + jc;
+              float* out = p.phi + (static_cast<size_t>(oblk) * p.gm.d_rows + rr + roff) * nc + jc;
 #pragma unroll
               for (int e = 0; e < 8; ++e) {
                 if (jc + 4 * e < nc)
@@ -388,7 +390,7 @@ phi_combine_tc_kernel(const TcParams p, const __grid_constant__ CUtensorMap mapL
           __syncwarp();
           if (lane == 0) {
             // rows / columns beyond the block are clipped by the 3-D tensor map
-            if (!tr) tma_store_3d(&mapO, jc, rbase, oblk, sbox); else tma_store_3d(&mapO, rbase, jc, oblk, sbox);
+            if (!tr) tma_store_3d(&mapO, jc, rbase + roff, oblk, sbox); else tma_store_3d(&mapO, rbase, jc, oblk, sbox);
             tma_store_commit();
           }
         }
@@ -685,6 +687,8 @@ cudaError_t launch_bgemm_tc(const BatchedGemm& a, int nch, const void* maps, int
   p.gm.d_blk0 = a.d_blk0; p.gm.d_blk_stride = a.d_blk_stride;
   p.gm.transpose_out = a.transpose_out;
   p.gm.diag = a.diag; p.gm.diag_stride = a.diag_stride;
+  p.gm.d_row0 = a.d_row0; p.gm.d_row_stride = a.d_row_stride;
+  if (a.transpose_out && (a.d_row0 != 0 || a.d_row_stride != 0)) return cudaErrorInvalidValue;
   p.g.total = static_cast<long long>(p.gm.Mt) * p.g.NT * a.count;
 #define LTV_NCH_CASE(N_)                                                              \
   case N_: return pair ? launch_tc<N_, true, 1>(p, m, num_sms, stream)         \

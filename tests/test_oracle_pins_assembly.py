@@ -229,3 +229,44 @@ def test_closed_loop_constraint_margins_special_cases():
     Hx = rng.normal(size=(T, 3, n))
     sig0 = O.output_feedback_constraint_tightening(*ops0, w, f, Hx, Hu)
     np.testing.assert_allclose(sig0, O.constraint_tightening_item(A, w, Hx), rtol=1e-10, atol=1e-12)
+
+
+def test_backward_recursion_of_the_general_assembly_equals_eq15():
+    """The identity the device call ltv_scan_output_feedback_assemble is built on, checked against (15) AS EVALUATED BY THE
+    ORACLE on dense operators, for a general achievable Phibar (not generated from gains):
+        Phi^xw(k,j) = Phi^xw(k,j+1) Abar_j - Phibar^x(k,j+1) Lt_j C_j,  Phi^xw(k,k) = I;   same for Phi^uw with Phibar^u, start 0;
+        Phi^xe(k,j) = (Phi^xw - Phibar^x)(k,j) Lt_{j-1},   Phi^ue(k,j) = (Phi^uw - Phibar^u)(k,j) Lt_{j-1}   (j >= 1)."""
+    from assembly_inputs import blk, general_phibar, observer_operators
+
+    rng = np.random.default_rng(77)
+    T, n, m, p = 7, 6, 2, 3
+    A = np.eye(n)[None] + rng.normal(0.0, 0.4 / np.sqrt(n), (T, n, n))
+    B = rng.normal(0.0, 1.0, (T, n, m))
+    C = rng.normal(0.0, 1.0 / np.sqrt(n), (T, p, n))
+    Lt = 0.3 * rng.normal(0.0, 1.0, (T, n, p))
+    PbX, PbU = general_phibar(A, B, seed=5)
+    for k in range(T):
+        assert np.allclose(blk(PbX, k, k, n, n), np.eye(n), atol=1e-12)          # what the call takes for granted
+    # the state-feedback achievability constraint holds (so this IS a response the first SLS stage could return)
+    ZB = np.zeros((T * n, T * m))
+    for t in range(T - 1):
+        ZB[(t + 1) * n:(t + 2) * n, t * m:(t + 1) * m] = B[t]
+    assert np.allclose((np.eye(T * n) - O.shift_operator(A)) @ PbX - ZB @ PbU, np.eye(T * n), atol=1e-10)
+    PhX, PhY = observer_operators(A, Lt, C)
+    Pxw, Puw, Pxe, Pue = O.assemble_output_feedback(A, PbX, PbU, PhX, PhY)
+    Abar = A + Lt @ C
+    err = 0.0
+    for k in range(1, T):
+        X, U = np.eye(n), np.zeros((m, n))
+        for j in range(k - 1, -1, -1):
+            X = X @ Abar[j] - blk(PbX, k, j + 1, n, n) @ Lt[j] @ C[j]
+            U = U @ Abar[j] - blk(PbU, k, j + 1, m, n) @ Lt[j] @ C[j]
+            err = max(err, np.abs(X - blk(Pxw, k, j, n, n)).max(), np.abs(U - blk(Puw, k, j, m, n)).max())
+            if j >= 1:
+                err = max(err, np.abs((X - blk(PbX, k, j, n, n)) @ Lt[j - 1] - blk(Pxe, k, j, n, p)).max())
+                err = max(err, np.abs((U - blk(PbU, k, j, m, n)) @ Lt[j - 1] - blk(Pue, k, j, m, p)).max())
+            else:
+                assert np.abs(blk(Pxe, k, 0, n, p)).max() == 0.0 and np.abs(blk(Pue, k, 0, m, p)).max() == 0.0
+    assert err < 1e-12
+    # the gain-defined controller is the special case Phibar^u(k,j) = K_k Phibar^x(k,j)
+    assert np.abs(blk(Puw, 3, 3, m, n)).max() < 1e-12 and np.allclose(blk(Pxw, 3, 3, n, n), np.eye(n))
