@@ -18,9 +18,12 @@
 // stream-ordered: deterministic.  T-1 steps, sequential in j, parallel over k and the batch.
 #include <cuda.h>
 
+#include <algorithm>
+
 #include "ltv_internal.h"
 #include "phi_geom.cuh"
 #include "phi_kernels.h"
+#include "ptx.cuh"
 
 namespace ltv {
 
@@ -68,109 +71,361 @@ __device__ __forceinline__ float warp_sum(float v) {
   return v;
 }
 
-// Step j of the backward recursion for the rows of column j: warp per row (b, k, i), k = j+1 .. T-1, i < R.
+// Step j of the backward recursion for the rows of column j: a warp takes kAsmRows consecutive rows i of one block (b, k),
+// k = j+1 .. T-1 (the p gain / measurement vectors are then loaded once per kAsmRows rows, and kAsmRows independent row loads
+// are in flight per lane).
 //   k = j+1:  x: row = A_j[i]                                   u: row = -(Phibar^u(j+1,j+1)[i] Lt_j) C_j
 //   k > j+1:  row = (GEMM result already in out) - (Phibar(k,j+1)[i] Lt_j) C_j
 // then e = (row - Phibar(k,j)[i]) Lt_{j-1} (j >= 1) and, x side, tau_k[i] += ||row o w_j|| + ||e o f_{j-1}||.
-// grid (ceil(rows / 8), batch), rows = (T-1-j) R.
+// NP = p exactly for p <= 8 (every loop over the measurements unrolls, the sums stay in registers); NP = 0: any p <= 32
+// (32 guarded accumulators, one row per warp).  grid (ceil(groups / 8), batch), groups = (T-1-j) ceil(R / ROWS).
+template <int NP, int ROWS>
 __global__ void __launch_bounds__(256) asm_step_kernel(const AsmStep s) {
-  const int T = s.T, n = s.n, p = s.p, R = s.R, j = s.j;
+  constexpr int PMAX = NP > 0 ? NP : 32;
+  const int T = s.T, n = s.n, R = s.R, j = s.j;
+  const int p = NP > 0 ? NP : s.p;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int row = blockIdx.x * 8 + warp;
-  if (row >= (T - 1 - j) * R) return;
+  const int gpb = (R + ROWS - 1) / ROWS;   // row groups per block
+  const int grp = blockIdx.x * 8 + warp;
+  if (grp >= (T - 1 - j) * gpb) return;
   const int b = blockIdx.y;
-  const int kk = row / R, i = row - kk * R;
+  const int kk = grp / gpb, i0 = (grp - kk * gpb) * ROWS;
+  const int nr = min(ROWS, R - i0);        // rows of this group that exist
   const int k = j + 1 + kk;
   const int n4 = n >> 2;
   const size_t P = static_cast<size_t>(T) * (T - 1) / 2;
   const size_t bT = static_cast<size_t>(b) * T;
-  // Phibar blocks (k, j+1) and (k, j)
+  // Phibar blocks (k, j+1) and (k, j), row i0
   const float4 *pb_next = nullptr, *pb_cur;
   if (s.is_u) {
     const size_t item = static_cast<size_t>(b) * (P + T);
     auto qd = [&](int kq, int jq) { return static_cast<size_t>(jq) * T - static_cast<size_t>(jq) * (jq - 1) / 2 + (kq - jq); };
-    pb_next = reinterpret_cast<const float4*>(s.pbar + ((item + qd(k, j + 1)) * R + i) * n);
-    pb_cur = reinterpret_cast<const float4*>(s.pbar + ((item + qd(k, j)) * R + i) * n);
+    pb_next = reinterpret_cast<const float4*>(s.pbar + ((item + qd(k, j + 1)) * R + i0) * n);
+    pb_cur = reinterpret_cast<const float4*>(s.pbar + ((item + qd(k, j)) * R + i0) * n);
   } else {
     const size_t item = static_cast<size_t>(b) * P;
-    if (kk > 0) pb_next = reinterpret_cast<const float4*>(s.pbar + ((item + phi_colbase(T, j + 1) + (k - j - 2)) * R + i) * n);
-    pb_cur = reinterpret_cast<const float4*>(s.pbar + ((item + phi_colbase(T, j) + (k - j - 1)) * R + i) * n);
+    if (kk > 0) pb_next = reinterpret_cast<const float4*>(s.pbar + ((item + phi_colbase(T, j + 1) + (k - j - 2)) * R + i0) * n);
+    pb_cur = reinterpret_cast<const float4*>(s.pbar + ((item + phi_colbase(T, j) + (k - j - 1)) * R + i0) * n);
   }
   const size_t oblk = static_cast<size_t>(b) * P + phi_colbase(T, j) + (k - j - 1);
-  float4* orow = reinterpret_cast<float4*>(s.out + (oblk * R + i) * n);
+  float4* orow = reinterpret_cast<float4*>(s.out + (oblk * R + i0) * n);
   const float4* Lj = reinterpret_cast<const float4*>(s.Ltt + (bT + j) * p * n);
   const float4* Cj = reinterpret_cast<const float4*>(s.C + (bT + j) * p * n);
   const float4* Ljm = (j >= 1) ? reinterpret_cast<const float4*>(s.Ltt + (bT + j - 1) * p * n) : nullptr;
   const float4* wj = reinterpret_cast<const float4*>(s.w + (bT + j) * n);
+  const float4* arow = (!s.is_u && kk == 0) ? reinterpret_cast<const float4*>(s.A + ((bT + j) * n + i0) * n) : nullptr;
+  const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
 
-  // u[q] = Phibar(k,j+1)[i] . Lt_j[:,q]
-  float u[32];
-  if (pb_next != nullptr) {
-    for (int q0 = 0; q0 < p; q0 += 8) {
-      float acc[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-      for (int c = lane; c < n4; c += 32) {
-        const float4 a = __ldg(pb_next + c);
+  // u[r][q] = Phibar(k,j+1)[i0 + r] . Lt_j[:,q]
+  float u[ROWS][PMAX];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) {
-          if (q0 + q < p) {
-            const float4 l = __ldg(Lj + static_cast<size_t>(q0 + q) * n4 + c);
-            acc[q] = fmaf(a.x, l.x, fmaf(a.y, l.y, fmaf(a.z, l.z, fmaf(a.w, l.w, acc[q]))));
+  for (int r = 0; r < ROWS; ++r)
+#pragma unroll
+    for (int q = 0; q < PMAX; ++q) u[r][q] = 0.f;
+  if (pb_next != nullptr) {
+    for (int c = lane; c < n4; c += 32) {
+      float4 a[ROWS];
+#pragma unroll
+      for (int r = 0; r < ROWS; ++r) a[r] = (r < nr) ? __ldg(pb_next + static_cast<size_t>(r) * n4 + c) : z4;
+#pragma unroll
+      for (int q = 0; q < PMAX; ++q) {
+        if (NP > 0 || q < p) {
+          const float4 l = __ldg(Lj + static_cast<size_t>(q) * n4 + c);
+#pragma unroll
+          for (int r = 0; r < ROWS; ++r)
+            u[r][q] = fmaf(a[r].x, l.x, fmaf(a[r].y, l.y, fmaf(a[r].z, l.z, fmaf(a[r].w, l.w, u[r][q]))));
+        }
+      }
+    }
+#pragma unroll
+    for (int r = 0; r < ROWS; ++r)
+#pragma unroll
+      for (int q = 0; q < PMAX; ++q)
+        if (NP > 0 || q < p) u[r][q] = warp_sum(u[r][q]);
+  }
+  // the rows, their tube terms and e = (row - Phibar(k,j)[i]) Lt_{j-1}
+  float s1[ROWS];
+  float e[ROWS][PMAX];
+#pragma unroll
+  for (int r = 0; r < ROWS; ++r) {
+    s1[r] = 0.f;
+#pragma unroll
+    for (int q = 0; q < PMAX; ++q) e[r][q] = 0.f;
+  }
+  for (int c = lane; c < n4; c += 32) {
+    float4 x[ROWS], pc[ROWS];
+#pragma unroll
+    for (int r = 0; r < ROWS; ++r) {
+      if (r < nr) {
+        if (kk == 0) x[r] = s.is_u ? z4 : __ldg(arow + static_cast<size_t>(r) * n4 + c); else x[r] = orow[static_cast<size_t>(r) * n4 + c];
+        pc[r] = (Ljm != nullptr) ? __ldg(pb_cur + static_cast<size_t>(r) * n4 + c) : z4;
+      } else {
+        x[r] = z4; pc[r] = z4;
+      }
+    }
+    if (pb_next != nullptr) {
+#pragma unroll
+      for (int q = 0; q < PMAX; ++q) {
+        if (NP > 0 || q < p) {
+          const float4 cq = __ldg(Cj + static_cast<size_t>(q) * n4 + c);
+#pragma unroll
+          for (int r = 0; r < ROWS; ++r) {
+            x[r].x = fmaf(-u[r][q], cq.x, x[r].x); x[r].y = fmaf(-u[r][q], cq.y, x[r].y);
+            x[r].z = fmaf(-u[r][q], cq.z, x[r].z); x[r].w = fmaf(-u[r][q], cq.w, x[r].w);
           }
         }
       }
+    }
 #pragma unroll
-      for (int q = 0; q < 8; ++q) u[(q0 + q) & 31] = warp_sum(acc[q]);
-    }
-  }
-  // the row, its tube term and e = (row - Phibar(k,j)[i]) Lt_{j-1}
-  float s1 = 0.f;
-  float e[32];
-#pragma unroll
-  for (int q = 0; q < 32; ++q) e[q] = 0.f;
-  for (int c = lane; c < n4; c += 32) {
-    float4 x;
-    if (kk == 0) {
-      x = s.is_u ? make_float4(0.f, 0.f, 0.f, 0.f) : __ldg(reinterpret_cast<const float4*>(s.A + ((bT + j) * n + i) * n) + c);
-    } else {
-      x = orow[c];
-    }
-    if (pb_next != nullptr) {
-      for (int q = 0; q < p; ++q) {
-        const float4 cq = __ldg(Cj + static_cast<size_t>(q) * n4 + c);
-        const float uq = u[q];
-        x.x = fmaf(-uq, cq.x, x.x); x.y = fmaf(-uq, cq.y, x.y); x.z = fmaf(-uq, cq.z, x.z); x.w = fmaf(-uq, cq.w, x.w);
-      }
-    }
-    orow[c] = x;
+    for (int r = 0; r < ROWS; ++r)
+      if (r < nr) orow[static_cast<size_t>(r) * n4 + c] = x[r];
     if (!s.is_u) {
       const float4 ww = __ldg(wj + c);
-      const float e0 = x.x * ww.x, e1 = x.y * ww.y, e2 = x.z * ww.z, e3 = x.w * ww.w;
-      s1 = fmaf(e0, e0, fmaf(e1, e1, fmaf(e2, e2, fmaf(e3, e3, s1))));
+#pragma unroll
+      for (int r = 0; r < ROWS; ++r) {
+        const float e0 = x[r].x * ww.x, e1 = x[r].y * ww.y, e2 = x[r].z * ww.z, e3 = x[r].w * ww.w;
+        s1[r] = fmaf(e0, e0, fmaf(e1, e1, fmaf(e2, e2, fmaf(e3, e3, s1[r]))));
+      }
     }
     if (Ljm != nullptr) {
-      const float4 pc = __ldg(pb_cur + c);
-      const float4 v = make_float4(x.x - pc.x, x.y - pc.y, x.z - pc.z, x.w - pc.w);
-      for (int q = 0; q < p; ++q) {
-        const float4 l = __ldg(Ljm + static_cast<size_t>(q) * n4 + c);
-        e[q] = fmaf(v.x, l.x, fmaf(v.y, l.y, fmaf(v.z, l.z, fmaf(v.w, l.w, e[q]))));
+#pragma unroll
+      for (int r = 0; r < ROWS; ++r) {
+        pc[r].x = x[r].x - pc[r].x; pc[r].y = x[r].y - pc[r].y; pc[r].z = x[r].z - pc[r].z; pc[r].w = x[r].w - pc[r].w;
+      }
+#pragma unroll
+      for (int q = 0; q < PMAX; ++q) {
+        if (NP > 0 || q < p) {
+          const float4 l = __ldg(Ljm + static_cast<size_t>(q) * n4 + c);
+#pragma unroll
+          for (int r = 0; r < ROWS; ++r)
+            e[r][q] = fmaf(pc[r].x, l.x, fmaf(pc[r].y, l.y, fmaf(pc[r].z, l.z, fmaf(pc[r].w, l.w, e[r][q]))));
+        }
       }
     }
   }
-  float s2 = 0.f;
-  if (Ljm != nullptr) {
-    const float* fj = s.f + (bT + j - 1) * p;
-    for (int q = 0; q < p; ++q) {
-      const float eq = warp_sum(e[q]);
-      const float t = eq * __ldg(fj + q);
-      s2 = fmaf(t, t, s2);
-      if (s.oute != nullptr && lane == (q & 31)) s.oute[(oblk * R + i) * p + q] = eq;
+  const float* fj = (Ljm != nullptr) ? s.f + (bT + j - 1) * p : nullptr;
+#pragma unroll
+  for (int r = 0; r < ROWS; ++r) {
+    if (r >= nr) continue;   // warp-uniform
+    float s2 = 0.f;
+    float* er = s.oute ? s.oute + (oblk * R + i0 + r) * p : nullptr;
+    if (Ljm != nullptr) {
+#pragma unroll
+      for (int q = 0; q < PMAX; ++q) {
+        if (NP > 0 || q < p) {
+          const float eq = warp_sum(e[r][q]);
+          const float t = eq * __ldg(fj + q);
+          s2 = fmaf(t, t, s2);
+          if (er != nullptr && lane == q) er[q] = eq;
+        }
+      }
+    } else if (er != nullptr && lane < p) {
+      er[lane] = 0.f;   // j = 0: no measurement noise has entered yet
     }
-  } else if (s.oute != nullptr && lane < p) {
-    s.oute[(oblk * R + i) * p + lane] = 0.f;   // j = 0: no measurement noise has entered yet
+    if (!s.is_u && s.tau != nullptr) {
+      const float t1 = warp_sum(s1[r]);
+      if (lane == 0) s.tau[(bT + k) * n + i0 + r] += sqrtf(t1) + sqrtf(s2);
+    }
   }
-  if (!s.is_u && s.tau != nullptr) {
-    s1 = warp_sum(s1);
-    if (lane == 0) s.tau[(bT + k) * n + i] += sqrtf(s1) + sqrtf(s2);
+}
+
+// The same step as a small persistent pipeline (p <= 8 and the buffers below fit shared memory; C2: 80 KB, C3: 160 KB).
+// ncu on the register version: 24 % dram throughput, long-scoreboard stalls 7 per issue - a warp lived for one row, waited
+// out a DRAM latency per pass, and every CTA re-fetched the 3 p gain / measurement vectors of its (b, j) through L1.  Here a
+// CTA stays on one item, stages Lt_j^T, C_j, Lt_{j-1}^T and w_j in shared memory ONCE, and each warp walks its rows with a
+// two-stage cp.async ring: the (up to) three rows of row r+1 - Phibar(k,j+1)[i], the GEMM result, Phibar(k,j)[i] - are in
+// flight while row r is reduced out of shared memory.
+template <int NP>
+__global__ void __launch_bounds__(256) asm_step_pipe_kernel(const AsmStep s) {
+  extern __shared__ float4 asm_sm[];
+  const int T = s.T, n = s.n, R = s.R, j = s.j;
+  constexpr int p = NP;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int b = blockIdx.y;
+  const int n4 = n >> 2;
+  const int rtot = (T - 1 - j) * R;
+  const size_t P = static_cast<size_t>(T) * (T - 1) / 2;
+  const size_t bT = static_cast<size_t>(b) * T;
+  float4* vL = asm_sm;                 // [p][n4] Lt_j^T
+  float4* vC = vL + p * n4;            // [p][n4] C_j
+  float4* vLm = vC + p * n4;           // [p][n4] Lt_{j-1}^T (j >= 1)
+  float4* vw = vLm + p * n4;           // [n4]    w_j
+  float4* ring = vw + n4 + static_cast<size_t>(warp) * 6 * n4;   // [2 stages][3 rows][n4] of this warp
+  {
+    const float4* Lj = reinterpret_cast<const float4*>(s.Ltt + (bT + j) * p * n);
+    const float4* Cj = reinterpret_cast<const float4*>(s.C + (bT + j) * p * n);
+    const float4* wj = reinterpret_cast<const float4*>(s.w + (bT + j) * n);
+    for (int e = threadIdx.x; e < p * n4; e += 256) {
+      vL[e] = __ldg(Lj + e);
+      vC[e] = __ldg(Cj + e);
+      if (j >= 1) vLm[e] = __ldg(reinterpret_cast<const float4*>(s.Ltt + (bT + j - 1) * p * n) + e);
+    }
+    for (int e = threadIdx.x; e < n4; e += 256) vw[e] = __ldg(wj + e);
+  }
+  __syncthreads();
+  const bool has_e = j >= 1;
+  const size_t item_x = static_cast<size_t>(b) * P, item_u = static_cast<size_t>(b) * (P + T);
+  auto qd = [&](int kq, int jq) { return static_cast<size_t>(jq) * T - static_cast<size_t>(jq) * (jq - 1) / 2 + (kq - jq); };
+  // global rows of row index `row` of this step: Phibar(k,j+1)[i] (or null), base row (or null = zero), Phibar(k,j)[i], out row
+  auto rows_of = [&](int row, const float4*& nx, const float4*& bs, const float4*& cu, float4*& orow, size_t& oidx, int& k) {
+    const int kk = row / R, i = row - kk * R;
+    k = j + 1 + kk;
+    oidx = (item_x + phi_colbase(T, j) + (k - j - 1)) * R + i;
+    orow = reinterpret_cast<float4*>(s.out + oidx * n);
+    if (s.is_u) {
+      nx = reinterpret_cast<const float4*>(s.pbar + ((item_u + qd(k, j + 1)) * R + i) * n);
+      cu = reinterpret_cast<const float4*>(s.pbar + ((item_u + qd(k, j)) * R + i) * n);
+      bs = kk == 0 ? nullptr : orow;
+    } else {
+      nx = kk > 0 ? reinterpret_cast<const float4*>(s.pbar + ((item_x + phi_colbase(T, j + 1) + (k - j - 2)) * R + i) * n) : nullptr;
+      cu = reinterpret_cast<const float4*>(s.pbar + ((item_x + phi_colbase(T, j) + (k - j - 1)) * R + i) * n);
+      bs = kk == 0 ? reinterpret_cast<const float4*>(s.A + ((bT + j) * n + i) * n) : orow;
+    }
+  };
+  auto prefetch = [&](int row, int stage) {
+    if (row < rtot) {
+      const float4 *nx, *bs, *cu; float4* orow; size_t oidx; int k;
+      rows_of(row, nx, bs, cu, orow, oidx, k);
+      float4* dst = ring + static_cast<size_t>(stage) * 3 * n4;
+      for (int c = lane; c < n4; c += 32) {
+        if (nx != nullptr) cp_async16(dst + c, nx + c);
+        if (bs != nullptr) cp_async16(dst + n4 + c, bs + c);
+        if (has_e) cp_async16(dst + 2 * n4 + c, cu + c);
+      }
+    }
+    cp_async_commit();
+  };
+  float fq[NP];   // f_{j-1}: the scaling of the measurement noise that enters through Lt_{j-1}
+#pragma unroll
+  for (int q = 0; q < NP; ++q) fq[q] = has_e ? __ldg(s.f + (bT + j - 1) * p + q) : 0.f;
+  const int stride = gridDim.x * 8;
+  int row = blockIdx.x * 8 + warp;
+  prefetch(row, 0);
+  for (int it = 0; row < rtot; row += stride, ++it) {
+    const int stage = it & 1;
+    prefetch(row + stride, stage ^ 1);
+    cp_async_wait<1>();
+    __syncwarp();
+    const float4 *nx, *bs, *cu; float4* orow; size_t oidx; int k;
+    rows_of(row, nx, bs, cu, orow, oidx, k);
+    // tau_k[i] so far: loaded now, needed only at the end of the row (one owner per entry and step: no race)
+    float* tau_p = (!s.is_u && s.tau != nullptr) ? s.tau + (bT + k) * n + row % R : nullptr;
+    const float tau_old = (tau_p != nullptr && lane == 0) ? *tau_p : 0.f;
+    const float4* s_next = ring + static_cast<size_t>(stage) * 3 * n4;
+    const float4* s_base = s_next + n4;
+    const float4* s_cur = s_base + n4;
+    float u[NP];
+#pragma unroll
+    for (int q = 0; q < NP; ++q) u[q] = 0.f;
+    if (nx != nullptr) {
+      for (int c = lane; c < n4; c += 32) {
+        const float4 a = s_next[c];
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+          const float4 l = vL[q * n4 + c];
+          u[q] = fmaf(a.x, l.x, fmaf(a.y, l.y, fmaf(a.z, l.z, fmaf(a.w, l.w, u[q]))));
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < NP; ++q) u[q] = warp_sum(u[q]);
+    }
+    float s1 = 0.f;
+    float e[NP];
+#pragma unroll
+    for (int q = 0; q < NP; ++q) e[q] = 0.f;
+    for (int c = lane; c < n4; c += 32) {
+      float4 x = (bs != nullptr) ? s_base[c] : make_float4(0.f, 0.f, 0.f, 0.f);
+      if (nx != nullptr) {
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+          const float4 cq = vC[q * n4 + c];
+          x.x = fmaf(-u[q], cq.x, x.x); x.y = fmaf(-u[q], cq.y, x.y); x.z = fmaf(-u[q], cq.z, x.z); x.w = fmaf(-u[q], cq.w, x.w);
+        }
+      }
+      orow[c] = x;
+      if (!s.is_u) {
+        const float4 ww = vw[c];
+        const float e0 = x.x * ww.x, e1 = x.y * ww.y, e2 = x.z * ww.z, e3 = x.w * ww.w;
+        s1 = fmaf(e0, e0, fmaf(e1, e1, fmaf(e2, e2, fmaf(e3, e3, s1))));
+      }
+      if (has_e) {
+        const float4 pc = s_cur[c];
+        const float4 v = make_float4(x.x - pc.x, x.y - pc.y, x.z - pc.z, x.w - pc.w);
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+          const float4 l = vLm[q * n4 + c];
+          e[q] = fmaf(v.x, l.x, fmaf(v.y, l.y, fmaf(v.z, l.z, fmaf(v.w, l.w, e[q]))));
+        }
+      }
+    }
+    float s2 = 0.f;
+    if (has_e) {
+#pragma unroll
+      for (int q = 0; q < NP; ++q) {
+        const float eq = warp_sum(e[q]);
+        const float t = eq * fq[q];
+        s2 = fmaf(t, t, s2);
+        if (s.oute != nullptr && lane == q) s.oute[oidx * p + q] = eq;
+      }
+    } else if (s.oute != nullptr && lane < p) {
+      s.oute[oidx * p + lane] = 0.f;   // j = 0: no measurement noise has entered yet
+    }
+    if (tau_p != nullptr) {
+      s1 = warp_sum(s1);
+      if (lane == 0) *tau_p = tau_old + (sqrtf(s1) + sqrtf(s2));
+    }
+    __syncwarp();   // every lane is done with this stage before the next iteration's prefetch overwrites the other one's successor
+  }
+  cp_async_wait<0>();
+}
+
+size_t asm_pipe_smem_bytes(int n, int p) { return (static_cast<size_t>(3) * p * n + n + static_cast<size_t>(8) * 6 * n) * sizeof(float); }
+
+template <int NP>
+cudaError_t launch_asm_step_pipe(const AsmStep& s, int batch, int sms, cudaStream_t stream) {
+  const size_t smem = asm_pipe_smem_bytes(s.n, NP);
+  static size_t attr_set = 0;   // largest dynamic shared-memory size the attribute was raised to (per instantiation)
+  if (smem > 48 * 1024 && smem > attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(asm_step_pipe_kernel<NP>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    if (e != cudaSuccess) return e;
+    attr_set = smem;
+  }
+  const int rtot = (s.T - 1 - s.j) * s.R;
+  const int per_sm = static_cast<int>(std::max<size_t>(1, std::min<size_t>(4, (200u * 1024u) / smem)));
+  int cx = (per_sm * sms) / batch;   // CTAs per item: one resident wave (rounding UP would leave a second, nearly empty wave)
+  cx = std::max(1, std::min(cx, (rtot + 7) / 8));
+  asm_step_pipe_kernel<NP><<<dim3(cx, batch), 256, smem, stream>>>(s);
+  return cudaSuccess;
+}
+
+constexpr int kAsmRows = 2;
+
+void launch_asm_step(const AsmStep& s, int batch, int sms, cudaStream_t stream) {
+  if (s.p <= 8 && asm_pipe_smem_bytes(s.n, s.p) <= 200u * 1024u) {
+    switch (s.p) {
+      case 1: launch_asm_step_pipe<1>(s, batch, sms, stream); return;
+      case 2: launch_asm_step_pipe<2>(s, batch, sms, stream); return;
+      case 3: launch_asm_step_pipe<3>(s, batch, sms, stream); return;
+      case 4: launch_asm_step_pipe<4>(s, batch, sms, stream); return;
+      case 5: launch_asm_step_pipe<5>(s, batch, sms, stream); return;
+      case 6: launch_asm_step_pipe<6>(s, batch, sms, stream); return;
+      case 7: launch_asm_step_pipe<7>(s, batch, sms, stream); return;
+      default: launch_asm_step_pipe<8>(s, batch, sms, stream); return;
+    }
+  }
+  const int rows = s.p <= 8 ? kAsmRows : 1;
+  const int groups = (s.T - 1 - s.j) * ((s.R + rows - 1) / rows);
+  const dim3 grid((groups + 7) / 8, batch);
+  switch (s.p <= 8 ? s.p : 0) {
+    case 1: asm_step_kernel<1, kAsmRows><<<grid, 256, 0, stream>>>(s); break;
+    case 2: asm_step_kernel<2, kAsmRows><<<grid, 256, 0, stream>>>(s); break;
+    case 3: asm_step_kernel<3, kAsmRows><<<grid, 256, 0, stream>>>(s); break;
+    case 4: asm_step_kernel<4, kAsmRows><<<grid, 256, 0, stream>>>(s); break;
+    case 5: asm_step_kernel<5, kAsmRows><<<grid, 256, 0, stream>>>(s); break;
+    case 6: asm_step_kernel<6, kAsmRows><<<grid, 256, 0, stream>>>(s); break;
+    case 7: asm_step_kernel<7, kAsmRows><<<grid, 256, 0, stream>>>(s); break;
+    case 8: asm_step_kernel<8, kAsmRows><<<grid, 256, 0, stream>>>(s); break;
+    default: asm_step_kernel<0, 1><<<grid, 256, 0, stream>>>(s); break;
   }
 }
 
@@ -245,10 +500,9 @@ cudaError_t launch_ofb_assemble(const AsmArgs& a, cudaStream_t stream, unsigned 
       s.out = sd ? a.phi_uw : a.phi_xw; s.oute = sd ? a.phi_ue : a.phi_xe; s.pbar = sd ? a.phibar_u : a.phibar_x;
       s.A = a.A; s.Ltt = Ltt; s.C = a.C; s.w = a.w; s.f = a.f; s.tau = sd ? nullptr : a.tau;
       s.T = T; s.n = n; s.p = p; s.R = R; s.is_u = sd; s.j = j;
-      const int rows = (T - 1 - j) * R;
       {
         ProfScope prof(kProfOfbSupport, stream);
-        asm_step_kernel<<<dim3((rows + 7) / 8, batch), 256, 0, stream>>>(s);
+        launch_asm_step(s, batch, sms, stream);
       }
       if ((e = cudaGetLastError()) != cudaSuccess) return e;
       ++*launches;
