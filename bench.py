@@ -538,6 +538,21 @@ def next_rows(B, L, W, steps):
                                                 "(one n^3 product per block, T-1 batched tcgen05 GEMMs + fused row kernels)")
     del pbx, pbu, wsa
     torch.cuda.empty_cache()
+    # the paper's own regime - ONE small problem (tens of states): the single-launch paths, in microseconds
+    from workloads import dense_random
+    small = {}
+    for (ns, Ts) in ((40, 32), (64, 64)):
+        Ws = dense_random(1, Ts, ns, 6, seed=ns + Ts, scale=0.3)
+        Ms = observation_model(1, Ts, ns, p, seed=11, kind="track")
+        As = torch.from_numpy(Ws.A).to(dev)
+        ks = [torch.from_numpy(Ms[k]).to(dev) for k in ("C", "e", "f", "Pi0")]
+        wsk = torch.empty(max(16, L.ltv_scan_workspace_bytes(L.LTV_OP_KALMAN_GAINS, 1, Ts, ns, p)), dtype=torch.uint8, device=dev)
+        Lts = torch.empty((1, Ts, ns, p), device=dev)
+        Pis = torch.empty((1, Ts + 1, ns, ns), device=dev)
+        rec = timed(lambda: L.ltv_scan_kalman_gains(As, *ks, Lt_out=Lts, Pi_out=Pis, workspace=wsk), 20)
+        scan = timed(lambda: L.ltv_scan_kalman_gains(As, *ks, Lt_out=Lts, Pi_out=Pis, workspace=wsk, mode=L.LTV_KALMAN_SCAN), 20)
+        small[f"kalman_n{ns}_T{Ts}_batch1"] = dict(recursion_single_launch_us=rec * 1e3, riccati_scan_on_request_us=scan * 1e3)
+    out["small_problem"] = small
     return out
 
 
