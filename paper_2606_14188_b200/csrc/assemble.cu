@@ -381,6 +381,8 @@ __global__ void __launch_bounds__(256) asm_step_pipe_kernel(const AsmStep s) {
 
 size_t asm_pipe_smem_bytes(int n, int p) { return (static_cast<size_t>(3) * p * n + n + static_cast<size_t>(8) * 6 * n) * sizeof(float); }
 
+constexpr int kAsmWaves = 8;
+
 template <int NP>
 cudaError_t launch_asm_step_pipe(const AsmStep& s, int batch, int sms, cudaStream_t stream) {
   const size_t smem = asm_pipe_smem_bytes(s.n, NP);
@@ -392,7 +394,10 @@ cudaError_t launch_asm_step_pipe(const AsmStep& s, int batch, int sms, cudaStrea
   }
   const int rtot = (s.T - 1 - s.j) * s.R;
   const int per_sm = static_cast<int>(std::max<size_t>(1, std::min<size_t>(4, (200u * 1024u) / smem)));
-  int cx = (per_sm * sms) / batch;   // CTAs per item: one resident wave (rounding UP would leave a second, nearly empty wave)
+  // CTAs per item: about kAsmWaves waves of resident CTAs (a single wave wants batch to divide the slots - 64 items on 296
+  // slots left 14 % of them empty -, two or three waves end in a long tail; with eight the tail is <= 1/8 of a wave and the
+  // staging of the vectors is still amortised over >= 30 rows per warp on the long steps)
+  int cx = (env_int("ASM_WAVES", kAsmWaves) * per_sm * sms + batch - 1) / batch;
   cx = std::max(1, std::min(cx, (rtot + 7) / 8));
   asm_step_pipe_kernel<NP><<<dim3(cx, batch), 256, smem, stream>>>(s);
   return cudaSuccess;
