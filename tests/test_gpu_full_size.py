@@ -45,6 +45,19 @@ def _vector_outputs(L, W, d, items):
         assert O.rel_err(gu[b].cpu().numpy(), rgu) <= TOL
         assert O.rel_err(gx0[b].cpu().numpy(), rgx) <= TOL
     assert bool(torch.isfinite(x).all()) and bool(torch.isfinite(lam).all())
+    # the same through ltv_scan_rollout_adjoint - the call bench.py's step makes (ltv_scan_all): at these sizes it may run the two
+    # scans side by side on half of the SMs each with cluster sizes of its own (C3: 4 CTAs per item, C4: 10, C5 batch 64: 1)
+    x2, lam2, gu2, gx2 = L.ltv_scan_rollout_adjoint(d["A"], d["B"], d["c"], d["x0"], d["u"], d["g"])
+    torch.cuda.synchronize()
+    for b in items:
+        assert O.rel_err(x2[b].cpu().numpy(), O.rollout_item(W.A[b], W.B[b], W.c[b], W.x0[b], W.u[b])) <= TOL
+        rl, rgu, rgx = O.adjoint_item(W.A[b], W.B[b], W.g[b])
+        assert O.rel_err(lam2[b].cpu().numpy(), rl) <= TOL
+        assert O.rel_err(gu2[b].cpu().numpy(), rgu) <= TOL
+        assert O.rel_err(gx2[b].cpu().numpy(), rgx) <= TOL
+    assert bool(torch.isfinite(x2).all()) and bool(torch.isfinite(lam2).all())
+    # every item, not only the sampled ones: the two routes agree (different summation orders: tolerance, not bit equality)
+    assert float((x2 - x).abs().max() / x.abs().max()) <= TOL and float((lam2 - lam).abs().max() / lam.abs().max()) <= TOL
 
 
 def _phi_samples(L, W, phi, samples):
