@@ -536,7 +536,15 @@ def next_rows(B, L, W, steps):
     out["output_feedback_assemble"] = dict(p=p, ms=ms, blocks_per_s=batch * B.world * P / (ms * 1e-3),
                                            note="general Phibar: all four operators of (15) + tube, backward recursion over the columns "
                                                 "(one n^3 product per block, T-1 batched tcgen05 GEMMs + fused row kernels)")
-    del pbx, pbu, wsa
+    # margins (12d), both terms, rows on [z; v], from the assembled operators of the general call
+    asm = L.ltv_scan_output_feedback_assemble(d["A"], Lt, Cm, d["w"], ff, pbx, pbu, workspace=wsa)
+    ms = timed(lambda: L.ltv_scan_operator_constraint_margins(asm["phi_xw"], Hc, d["w"], phi_uw=asm["phi_uw"], Hu=Hu,
+                                                              phi_xe=asm["phi_xe"], phi_ue=asm["phi_ue"], f=ff), min(steps, 3))
+    read_gb = batch * P * (n * n + m * n + n * p + m * p) * 4 / 1e9
+    out["operator_constraint_margins"] = dict(nc=6, ms=ms, items_per_s=batch * B.world / (ms * 1e-3),
+                                              hbm_gbs=read_gb / (ms * 1e-3), hbm_frac=read_gb / (ms * 1e-3) / B.pk["hbm_gbs"],
+                                              note="eq.(12d) on assembled operators: every block read once")
+    del asm, pbx, pbu, wsa
     torch.cuda.empty_cache()
     # the paper's own regime - ONE small problem (tens of states): the single-launch paths, in microseconds
     from workloads import dense_random

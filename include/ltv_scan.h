@@ -368,6 +368,26 @@ LTV_API int ltv_scan_output_feedback_assemble(const float* A, const float* Lt, c
                                               float* tau_out, int batch, int T, int n, int m, int p, unsigned flags,
                                               void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Constraint-tightening margins of eq.(12d), both terms, constraint rows on [z_k; v_k], evaluated on
+ * ASSEMBLED output-feedback operators - those of ltv_scan_output_feedback_assemble (general Phibar) or of the gain-defined calls:
+ *     sigma_0 = 0;  sigma_k[i] = sum_{j<k}    || (Hx[b,k,i,:] Phi^xw(k,j) + Hu[b,k,i,:] Phi^uw(k,j)) diag(w_j) ||_2
+ *                              + sum_{1<=j<k} || (Hx[b,k,i,:] Phi^xe(k,j) + Hu[b,k,i,:] Phi^ue(k,j)) diag(f_{j-1}) ||_2
+ *   phi_xw   device [batch,P,n,n]   COLUMN_PACKED strictly-lower blocks; required
+ *   phi_uw   device [batch,P,m,n]   may be NULL together with Hu (constraints on the state only)
+ *   phi_xe   device [batch,P,n,p]   may be NULL (no observation term; f is then not read)
+ *   phi_ue   device [batch,P,m,p]   may be NULL; needs phi_uw
+ *   Hx       device [batch,T,nc,n]  required (Hx[b,0] is not read);   Hu  device [batch,T,nc,m]
+ *   w        device [batch,T,n];    f  device [batch,T,p]
+ *   sigma_out device [batch,T,nc]
+ *   flags    must be 0
+ * One CTA per (item, step k) walks j in order and keeps the nc sums: deterministic, no workspace, every operator block is
+ * read once (HBM-bound).  n <= 512, p <= 32, batch <= 65535 (LTV_ERR_UNSUPPORTED_SHAPE beyond); any nc (8 rows per pass
+ * over the operators). */
+LTV_API int ltv_scan_operator_constraint_margins(const float* phi_xw, const float* phi_uw, const float* phi_xe,
+                                                 const float* phi_ue, const float* Hx, const float* Hu, const float* w,
+                                                 const float* f, float* sigma_out, int batch, int T, int n, int m, int p,
+                                                 int nc, unsigned flags, void* cuda_stream);
+
 /* One pass of the whole hot path from HOST buffers: copies A, B, c, x0, u, w, g host->device into
  * `workspace` (device, >= ltv_scan_workspace_bytes(LTV_OP_PIPELINE_HOST, ...)), runs the path (ltv_scan_rollout_adjoint, then
  * ltv_scan_system_response_tube)

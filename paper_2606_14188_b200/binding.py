@@ -40,6 +40,7 @@ EXPORTS = (
     "ltv_profile_class_name", "ltv_scan_rollout_adjoint", "ltv_scan_all", "ltv_scan_all_is_fused", "ltv_scan_output_feedback_constraints", "ltv_scan_output_feedback_constraints_workspace_bytes",
     "ltv_static_scratch_bytes", "ltv_scan_system_response_tube_static",
     "ltv_scan_output_feedback_assemble", "ltv_scan_output_feedback_assemble_workspace_bytes",
+    "ltv_scan_operator_constraint_margins",
 )
 
 
@@ -70,6 +71,8 @@ def _load() -> ctypes.CDLL:
     L.ltv_scan_output_feedback_assemble.argtypes = [fp] * 12 + [i] * 5 + [ctypes.c_uint, vp, sz, vp]
     L.ltv_scan_output_feedback_assemble_workspace_bytes.restype = sz
     L.ltv_scan_output_feedback_assemble_workspace_bytes.argtypes = [i] * 5
+    L.ltv_scan_operator_constraint_margins.restype = i
+    L.ltv_scan_operator_constraint_margins.argtypes = [fp] * 9 + [i] * 6 + [ctypes.c_uint, vp]
     L.ltv_static_scratch_bytes.restype = sz
     L.ltv_static_scratch_bytes.argtypes = []
     L.ltv_scan_system_response_tube_static.restype = i
@@ -249,6 +252,24 @@ def ltv_scan_output_feedback_assemble(A, Lt, C, w, f, phibar_x, phibar_u=None, w
     if st != LTV_OK:
         raise LtvError(st, "ltv_scan_output_feedback_assemble")
     return out
+
+
+def ltv_scan_operator_constraint_margins(phi_xw, Hx, w, phi_uw=None, Hu=None, phi_xe=None, phi_ue=None, f=None):
+    """sigma[batch,T,nc] of eq.(12d), both terms, from assembled operators (COLUMN_PACKED strictly-lower blocks)."""
+    batch, P, n, _ = phi_xw.shape
+    T = w.shape[1]
+    nc = Hx.shape[2]
+    m = 0 if phi_uw is None else phi_uw.shape[2]
+    p = 0 if phi_xe is None else phi_xe.shape[3]
+    _dev(phi_xw, "phi_xw", (batch, P, n, n)); _dev(Hx, "Hx", (batch, T, nc, n)); _dev(w, "w", (batch, T, n))
+    _dev(phi_uw, "phi_uw", (batch, P, m, n)); _dev(Hu, "Hu", (batch, T, nc, m))
+    _dev(phi_xe, "phi_xe", (batch, P, n, p)); _dev(phi_ue, "phi_ue", (batch, P, m, p)); _dev(f, "f", (batch, T, p))
+    sigma = torch.empty((batch, T, nc), device=phi_xw.device, dtype=torch.float32)
+    st = lib.ltv_scan_operator_constraint_margins(_ptr(phi_xw), _ptr(phi_uw), _ptr(phi_xe), _ptr(phi_ue), _ptr(Hx), _ptr(Hu),
+                                                  _ptr(w), _ptr(f), _ptr(sigma), batch, T, n, m, p, nc, 0, _stream())
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_operator_constraint_margins")
+    return sigma
 
 
 def ltv_static_scratch_bytes():

@@ -647,6 +647,32 @@ int ltv_scan_output_feedback_assemble(const float* A, const float* Lt, const flo
   return err == cudaSuccess ? LTV_OK : fail_cuda(err);
 }
 
+int ltv_scan_operator_constraint_margins(const float* phi_xw, const float* phi_uw, const float* phi_xe, const float* phi_ue,
+                                         const float* Hx, const float* Hu, const float* w, const float* f, float* sigma_out,
+                                         int batch, int T, int n, int m, int p, int nc, unsigned flags, void* cuda_stream) {
+  if (!Hx || !w || !sigma_out) return LTV_ERR_NULL_PTR;
+  if (T > 1 && !phi_xw) return LTV_ERR_NULL_PTR;
+  if ((phi_uw != nullptr) != (Hu != nullptr)) return LTV_ERR_NULL_PTR;   // input part of the rows and of the operators go together
+  if (phi_ue && !phi_uw) return LTV_ERR_NULL_PTR;
+  if (phi_xe && !f) return LTV_ERR_NULL_PTR;
+  int st = check_dims(batch, T, n, m);
+  if (st != LTV_OK) return st;
+  if (nc < 1 || flags != 0 || (phi_uw && m < 1) || (phi_xe && p < 1)) return LTV_ERR_BAD_DIM;
+  if (p > 32 || grid_yz_overflow(batch) || !margins_supported(n, phi_uw ? m : 0, T)) return LTV_ERR_UNSUPPORTED_SHAPE;
+  if (misaligned(phi_xw) || misaligned(phi_uw) || misaligned(phi_xe) || misaligned(phi_ue) || misaligned(Hx) || misaligned(Hu) ||
+      misaligned(w) || misaligned(f) || misaligned(sigma_out))
+    return LTV_ERR_ALIGNMENT;
+  int sms = 0;
+  st = check_device(&sms);
+  if (st != LTV_OK) return st;
+  MarginArgs a{phi_xw, phi_uw, phi_xe, phi_xe ? phi_ue : nullptr, Hx, Hu, w, f, sigma_out, batch, T, n, phi_uw ? m : 0,
+               phi_xe ? p : 0, nc};
+  unsigned long long l = 0;
+  cudaError_t err = launch_operator_margins(a, static_cast<cudaStream_t>(cuda_stream), &l);
+  g_launches += l;
+  return err == cudaSuccess ? LTV_OK : fail_cuda(err);
+}
+
 int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float* c_host, const float* x0_host,
                            const float* u_host, const float* w_host, const float* g_host, float* x_host,
                            float* phi_host, float* r_host, float* lambda_host, float* grad_u_host,

@@ -115,6 +115,15 @@ struct AsmArgs {
 size_t asm_workspace_bytes(int batch, int T, int n, int p);
 cudaError_t launch_ofb_assemble(const AsmArgs& a, cudaStream_t stream, unsigned long long* launches);
 
+// Margins (12d) on assembled operators (margins.cu)
+struct MarginArgs {
+  const float *phi_xw, *phi_uw, *phi_xe, *phi_ue, *Hx, *Hu, *w, *f;   // phi_uw / Hu and phi_xe / phi_ue may be null
+  float* sigma;
+  int batch, T, n, m, p, nc;
+};
+bool margins_supported(int n, int m, int T);
+cudaError_t launch_operator_margins(const MarginArgs& a, cudaStream_t stream, unsigned long long* launches);
+
 // Whole hot path of a small problem in one launch (fused_small.cu): n <= 64 and all of A in one SM's shared memory
 struct FusedSmallArgs {
   const float *A, *B, *c, *x0, *u, *w, *g;

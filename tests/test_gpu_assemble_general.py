@@ -183,3 +183,77 @@ def test_general_assembly_full_batch_c2_shape_sampled_items(L):
                 ref["phi_uw"][q] = blk(Puw, k, j, m, n); ref["phi_ue"][q] = blk(Pue, k, j, m, p)
         for key in ref:
             assert O.rel_err(out[key][b].cpu().numpy(), ref[key]) <= TOL, (b, key)
+
+
+@pytest.mark.parametrize("n,T,m,p,nc,batch", [(24, 6, 2, 3, 4, 2),      # fp32-FMA path of the assembly
+                                              (132, 5, 6, 6, 3, 2),     # two column quads per lane, ragged
+                                              (300, 6, 6, 6, 6, 2),     # C2-size blocks
+                                              (96, 4, 3, 4, 11, 1),     # more than 8 constraint rows: two passes
+                                              (48, 2, 1, 1, 1, 1)])     # T = 2: one block
+def test_margins_on_assembled_operators_general_phibar(L, n, T, m, p, nc, batch):
+    """Chain general assembly -> ltv_scan_operator_constraint_margins against the oracle's eq.(12d) (both terms, rows on
+    [z; v]) evaluated on the oracle's own dense operators of eq.(15)."""
+    import torch
+
+    items = [_item(T, n, m, p, seed=13 * n + T + 100 * b) for b in range(batch)]
+    A, C, Lt, w, f = [np.stack([it[q] for it in items]) for q in range(5)]
+    packed = [_pack(L, T, n, m, it[5], it[6]) for it in items]
+    px = np.stack([q[0] for q in packed]); pu = np.stack([q[1] for q in packed])
+    rng = np.random.default_rng(n + nc)
+    Hx = rng.normal(0.0, 1.0, (batch, T, nc, n)).astype(np.float32)
+    Hu = rng.normal(0.0, 1.0, (batch, T, nc, m)).astype(np.float32)
+    cu = lambda a: torch.from_numpy(a).cuda()
+    out = L.ltv_scan_output_feedback_assemble(cu(A), cu(Lt), cu(C), cu(w), cu(f), cu(px), cu(pu))
+    sig = L.ltv_scan_operator_constraint_margins(out["phi_xw"], cu(Hx), cu(w), phi_uw=out["phi_uw"], Hu=cu(Hu),
+                                                 phi_xe=out["phi_xe"], phi_ue=out["phi_ue"], f=cu(f))
+    sig_x = L.ltv_scan_operator_constraint_margins(out["phi_xw"], cu(Hx), cu(w))          # state rows, w term only
+    torch.cuda.synchronize()
+    ref = np.zeros((batch, T, nc)); ref_x = np.zeros((batch, T, nc))
+    for b, it in enumerate(items):
+        A64 = it[0].astype(np.float64)
+        PbX, PbU = it[5].astype(np.float64), it[6].astype(np.float64)
+        for k in range(T):
+            PbX[k * n:(k + 1) * n, k * n:(k + 1) * n] = np.eye(n)
+            PbX[k * n:(k + 1) * n, (k + 1) * n:] = 0.0
+        PhX, PhY = observer_operators(A64, it[2], it[1])
+        Pxw, Puw, Pxe, Pue = O.assemble_output_feedback(A64, PbX, PbU, PhX, PhY)
+        ref[b] = O.output_feedback_constraint_tightening(Pxw, Puw, Pxe, Pue, it[3], it[4], Hx[b], Hu[b])
+        ref_x[b] = O.output_feedback_constraint_tightening(Pxw, np.zeros_like(Puw), np.zeros_like(Pxe), np.zeros_like(Pue),
+                                                           it[3], it[4], Hx[b], np.zeros_like(Hu[b]))
+    assert np.all(sig.cpu().numpy()[:, 0] == 0.0)
+    assert O.rel_err(sig.cpu().numpy(), ref) <= TOL, O.rel_err(sig.cpu().numpy(), ref)
+    assert O.rel_err(sig_x.cpu().numpy(), ref_x) <= TOL
+
+
+def test_margins_on_operators_equal_the_gain_defined_sweep(L):
+    """For a gain-defined controller the margins computed from the assembled operators must equal those of
+    ltv_scan_output_feedback_constraints (which never forms an operator block)."""
+    import torch
+
+    n, T, m, p, nc, batch = 132, 6, 3, 4, 5, 2
+    rng = np.random.default_rng(19)
+    f32 = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+    A = f32(np.eye(n)[None, None] + rng.normal(0.0, 0.4 / np.sqrt(n), (batch, T, n, n)))
+    B = f32(rng.normal(0.0, 1.0, (batch, T, n, m)))
+    K = f32(0.3 * rng.normal(0.0, 1.0 / np.sqrt(n), (batch, T, m, n)))
+    C = f32(rng.normal(0.0, 1.0 / np.sqrt(n), (batch, T, p, n)))
+    Lt = f32(0.3 * rng.normal(0.0, 1.0, (batch, T, n, p)))
+    w = f32(rng.uniform(0.0, 1e-3, (batch, T, n))); f = f32(rng.uniform(1e-3, 5e-3, (batch, T, p)))
+    Hx = f32(rng.normal(0.0, 1.0, (batch, T, nc, n))); Hu = f32(rng.normal(0.0, 1.0, (batch, T, nc, m)))
+    cu = lambda a: torch.from_numpy(a).cuda()
+    xw, xe, _ = L.ltv_scan_output_feedback_response(cu(A), cu(B), cu(K), cu(Lt), cu(C), cu(w), cu(f))
+    uw, ue, sig_ref = L.ltv_scan_output_feedback_constraints(cu(A), cu(B), cu(K), cu(Lt), cu(C), cu(w), cu(f), cu(Hx), cu(Hu))
+    sig = L.ltv_scan_operator_constraint_margins(xw, cu(Hx), cu(w), phi_uw=uw, Hu=cu(Hu), phi_xe=xe, phi_ue=ue, f=cu(f))
+    torch.cuda.synchronize()
+    assert float((sig - sig_ref).abs().max() / sig_ref.abs().max()) <= TOL
+
+
+def test_margins_validation(L):
+    import ctypes
+    g = L.lib.ltv_scan_operator_constraint_margins
+    buf = (ctypes.c_float * 64)()
+    q = ctypes.cast(buf, ctypes.c_void_p)
+    assert g(q, None, None, None, None, None, q, None, q, 1, 2, 4, 0, 0, 1, 0, None) == 1      # NULL Hx
+    assert g(q, q, None, None, q, None, q, None, q, 1, 2, 4, 1, 0, 1, 0, None) == 1            # phi_uw without Hu
+    assert g(q, None, None, None, q, None, q, None, q, 1, 2, 4, 0, 0, 0, 0, None) == 2         # nc = 0
+    assert g(q, None, None, None, q, None, q, None, q, 1, 2, 1028, 0, 0, 1, 0, None) == 3      # n > 512
