@@ -46,7 +46,7 @@ def parse():
     ap.add_argument("--no-tf32-peak", action="store_true",
                     help="skip the live TF32 library-GEMM peak measurement (the committed figure is used instead)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--cpu-items", type=int, default=0, help="items in the CPU-oracle sample (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -578,19 +578,24 @@ def e2e_leg(B, L, W, phi_on, reps):
         h.pop("w")
     h2d = sum(v.numel() * 4 for v in h.values())
     outs = None
-    for i in range(1 + reps):
-        if i == 1:
-            B.barrier()
-            t0 = time.perf_counter()
+    warm = 2                                   # the first calls also pay for page-locking effects and the copy stream's set-up
+    times = []
+    for i in range(warm + reps):
+        B.barrier()
+        t0 = time.perf_counter()
         outs = L.ltv_scan_pipeline_host(h["A"], h["B"], h["c"], h["x0"], h["u"], h["w"] if phi_on else None, h["g"],
-                                        wsh, outs=outs)
+                                        wsh, outs=outs)            # returns after the results are on the host (stream synchronised)
+        if i >= warm:
+            times.append(time.perf_counter() - t0)
     B.barrier()
-    sec = B.max_over_ranks((time.perf_counter() - t0) / reps)
+    mean_sec = sum(times) / len(times)
+    sec = B.max_over_ranks(sorted(times)[len(times) // 2])   # median step: a fresh box shows single outliers of 2x (mean / min / max beside it)
     d2h = sum(outs[k].numel() * 4 for k in ("x", "r", "lam", "grad_u", "grad_x0") if outs[k] is not None)
     del wsh
     torch.cuda.empty_cache()
     return dict(value=units / sec, unit=UNIT if phi_on else UNIT_C5, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
-                ms_per_step=sec * 1e3, steps=reps,
+                ms_per_step=sec * 1e3, steps=reps, statistic="median of the timed steps", ms_mean=mean_sec * 1e3,
+                ms_min=min(times) * 1e3, ms_max=max(times) * 1e3,
                 note="ltv_scan_pipeline_host, pinned host buffers, upload of chunk i+1 overlapped with the compute of chunk i"
                      + ("; Phi (the largest result) stays in HBM where its consumers run: value counts x, r, lambda, "
                         "grad_u, grad_x0 back on the host" if phi_on else "; rollout + adjoint only"))
