@@ -30,7 +30,7 @@
 //                -> swizzled 32x32 shared-memory box -> bulk tensor store (masked row-per-thread stores on the
 //                ragged last m-tile of a column)
 // Why L goes through TMEM: with both operands in shared memory a k-block moves 216 KB through the shared-
-// memory port against 960 cycles of MMA issue (measured 47 % tensor-pipe activity, profiles/r1_v1_*).
+// memory port against 960 cycles of MMA issue (measured 47 % tensor-pipe activity with the first version of round 1).
 // The accumulator is double-buffered in TMEM (2 * NT columns) so the epilogue of tile i overlaps the MMAs of
 // tile i+1; TMEM columns: [0, 2NT) accumulators, [2NT, 2NT + 192) L-operand ring.
 #include <cuda.h>
@@ -666,7 +666,7 @@ cudaError_t launch_bgemm_tc(const BatchedGemm& a, int nch, const void* maps, int
   const int mode = env_int("TC_PAIR", -1);
   const int nt = 32 * nch;
   // Shape by a wave model: rounds of tiles over the CTAs (or CTA pairs) x relative time per tile.  A pair tile keeps the
-  // tensor pipe ~92 % busy against ~65 % for the single-CTA shape (profiles/r1_v5_phi_combine_tc_full.md) but pays a
+  // tensor pipe ~92 % busy against ~65 % for the single-CTA shape (profiles/r2_kernels_full.md) but pays a
   // cluster launch and two cluster barriers (15 %, fitted: C2 384 single tiles 33.3 us vs 256 pair tiles 35.6 us;
   // C3 320 vs 192: 49.4 vs 45.3 us).
   const long long ntile = (a.N + nt - 1) / nt;
