@@ -146,6 +146,27 @@ LTV_API size_t ltv_static_scratch_bytes(void);
 LTV_API int ltv_scan_system_response_tube_static(const float* A, const float* w, float* phi_out, float* r_out,
                                                  int batch, int T, int n, unsigned flags, void* cuda_stream);
 
+/* One SHARD of the system response of the same items: the block ROWS k_lo <= k < k_hi (1 <= k_lo < k_hi <= T) and their tube
+ * rows - what one GPU computes when single large items are split over several GPUs (optional; sharding.py has the
+ * partition).  The split is by rows because a block row needs nothing outside itself, Phi(k,j) = Phi(k,j+1) A_j with
+ * Phi(k,k) = I: every GPU holds A (replicated), no GPU reads another one's blocks, and r_k is COMPLETE on the GPU that owns row
+ * k - no reduction over GPUs (summing the zero-initialised r of all shards, or gathering the rows, assembles r).
+ *   A, w       as in ltv_scan_system_response_tube
+ *   phi_rows_out device [batch,Ps,n,n]  Ps = ltv_phi_row_shard_blocks(T,k_lo,k_hi) = sum_{k=k_lo}^{k_hi-1} k; block (k,j), 0 <= j < k,
+ *                                       at ltv_phi_row_shard_block_index(T,k_lo,k_hi,k,j): column by column (the shard's own
+ *                                       column-packed order: column j holds k = max(k_lo, j+1) .. k_hi-1)
+ *   r_out      device [batch,T,n]       rows k_lo .. k_hi-1 are written (and r_0 = 0 if k_lo == 1), the others left untouched
+ *   flags      0 or LTV_TUBE_ROW_2NORM
+ * k_hi - 1 backward steps over the columns, each one batched GEMM of the shard's stacked column j+1 with A_j (tcgen05 3xTF32
+ * for n >= 96) plus a row kernel (block (j+1,j) = A_j, tube terms): one n^3 product per block as in the time-parallel scan, but
+ * sequential in j - the price of a split with no communication.  k_lo = 1, k_hi = T is the whole response.  Deterministic.
+ * No workspace.  batch <= 65535. */
+LTV_API long long ltv_phi_row_shard_blocks(int T, int k_lo, int k_hi);
+LTV_API long long ltv_phi_row_shard_block_index(int T, int k_lo, int k_hi, int k, int j);
+LTV_API int ltv_scan_system_response_tube_rows(const float* A, const float* w, float* phi_rows_out, float* r_out,
+                                               int batch, int T, int n, int k_lo, int k_hi, unsigned flags,
+                                               void* cuda_stream);
+
 /* Adjoint scan (north_star (iii); eq.(10) chained over the horizon) for
  * L = sum_{t=1}^{T} l_t(x_t), g_t = dl_t/dx_t, lam_{T+1} = 0:
  *     lam_T = g_T;  lam_t = A_t^T lam_{t+1} + g_t (t = T-1 .. 1);  grad_u[t] = B_t^T lam_{t+1} (t = 0 .. T-1);

@@ -18,6 +18,7 @@ _API = (
     "LTV_OP_KALMAN_GAINS", "LTV_OP_OUTPUT_FEEDBACK", "ltv_scan_output_feedback_response", "LTV_KALMAN_SCAN", "LTV_KALMAN_RECURSION", "LTV_OP_CONSTRAINT_TIGHTENING", "ltv_scan_constraint_tightening",
     "ltv_static_scratch_bytes", "ltv_scan_system_response_tube_static", "LTV_ERR_STATIC_SCRATCH_LIMIT",
     "ltv_scan_output_feedback_assemble", "ltv_scan_operator_constraint_margins",
+    "ltv_phi_row_shard_blocks", "ltv_phi_row_shard_block_index", "ltv_scan_system_response_tube_rows",
 )
 __all__ = list(_API)
 

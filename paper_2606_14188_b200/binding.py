@@ -41,6 +41,7 @@ EXPORTS = (
     "ltv_static_scratch_bytes", "ltv_scan_system_response_tube_static",
     "ltv_scan_output_feedback_assemble", "ltv_scan_output_feedback_assemble_workspace_bytes",
     "ltv_scan_operator_constraint_margins",
+    "ltv_phi_row_shard_blocks", "ltv_phi_row_shard_block_index", "ltv_scan_system_response_tube_rows",
 )
 
 
@@ -73,6 +74,12 @@ def _load() -> ctypes.CDLL:
     L.ltv_scan_output_feedback_assemble_workspace_bytes.argtypes = [i] * 5
     L.ltv_scan_operator_constraint_margins.restype = i
     L.ltv_scan_operator_constraint_margins.argtypes = [fp] * 9 + [i] * 6 + [ctypes.c_uint, vp]
+    L.ltv_phi_row_shard_blocks.restype = ctypes.c_longlong
+    L.ltv_phi_row_shard_blocks.argtypes = [i, i, i]
+    L.ltv_phi_row_shard_block_index.restype = ctypes.c_longlong
+    L.ltv_phi_row_shard_block_index.argtypes = [i] * 5
+    L.ltv_scan_system_response_tube_rows.restype = i
+    L.ltv_scan_system_response_tube_rows.argtypes = [fp] * 4 + [i] * 5 + [ctypes.c_uint, vp]
     L.ltv_static_scratch_bytes.restype = sz
     L.ltv_static_scratch_bytes.argtypes = []
     L.ltv_scan_system_response_tube_static.restype = i
@@ -270,6 +277,35 @@ def ltv_scan_operator_constraint_margins(phi_xw, Hx, w, phi_uw=None, Hu=None, ph
     if st != LTV_OK:
         raise LtvError(st, "ltv_scan_operator_constraint_margins")
     return sigma
+
+
+def ltv_phi_row_shard_blocks(T, k_lo, k_hi):
+    return int(lib.ltv_phi_row_shard_blocks(T, k_lo, k_hi))
+
+
+def ltv_phi_row_shard_block_index(T, k_lo, k_hi, k, j):
+    return int(lib.ltv_phi_row_shard_block_index(T, k_lo, k_hi, k, j))
+
+
+def ltv_scan_system_response_tube_rows(A, w, k_lo, k_hi, phi_rows_out=None, r_out=None, two_norm=False):
+    """Block rows k_lo <= k < k_hi of the system response (one shard of items split over GPUs): returns (phi_rows
+    [batch,Ps,n,n] in the shard's column-packed order, r[batch,T,n] with the shard's rows filled, zeros elsewhere if r_out
+    is not given)."""
+    batch, T, n, _ = A.shape
+    Ps = ltv_phi_row_shard_blocks(T, k_lo, k_hi)
+    if Ps < 0:
+        raise ValueError("need 1 <= k_lo < k_hi <= T")
+    _dev(A, "A", (batch, T, n, n)); _dev(w, "w", (batch, T, n))
+    if phi_rows_out is None:
+        phi_rows_out = torch.empty((batch, Ps, n, n), device=A.device, dtype=torch.float32)
+    if r_out is None:
+        r_out = torch.zeros((batch, T, n), device=A.device, dtype=torch.float32)
+    _dev(phi_rows_out, "phi_rows_out", (batch, Ps, n, n)); _dev(r_out, "r_out", (batch, T, n))
+    st = lib.ltv_scan_system_response_tube_rows(_ptr(A), _ptr(w), _ptr(phi_rows_out), _ptr(r_out), batch, T, n, k_lo, k_hi,
+                                                LTV_TUBE_ROW_2NORM if two_norm else 0, _stream())
+    if st != LTV_OK:
+        raise LtvError(st, "ltv_scan_system_response_tube_rows")
+    return phi_rows_out, r_out
 
 
 def ltv_static_scratch_bytes():

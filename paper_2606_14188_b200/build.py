@@ -9,7 +9,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libltvscan.so")
-SOURCES = ["api.cu", "rollout.cu", "adjoint.cu", "phi.cu", "phi_simt.cu", "phi_tc.cu", "kalman.cu", "constraints.cu", "riccati_scan.cu", "output_feedback.cu", "fused_small.cu", "kalman_small.cu", "no_alloc.cu", "assemble.cu", "margins.cu"]
+SOURCES = ["api.cu", "rollout.cu", "adjoint.cu", "phi.cu", "phi_simt.cu", "phi_tc.cu", "kalman.cu", "constraints.cu", "riccati_scan.cu", "output_feedback.cu", "fused_small.cu", "kalman_small.cu", "no_alloc.cu", "assemble.cu", "margins.cu", "phi_rows.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",

@@ -673,6 +673,31 @@ int ltv_scan_operator_constraint_margins(const float* phi_xw, const float* phi_u
   return err == cudaSuccess ? LTV_OK : fail_cuda(err);
 }
 
+long long ltv_phi_row_shard_blocks(int T, int k_lo, int k_hi) {
+  if (T < 1 || k_lo < 1 || k_hi > T || k_lo >= k_hi) return -1;
+  return phi_row_shard_blocks(T, k_lo, k_hi);
+}
+
+long long ltv_phi_row_shard_block_index(int T, int k_lo, int k_hi, int k, int j) { return phi_row_shard_index(T, k_lo, k_hi, k, j); }
+
+int ltv_scan_system_response_tube_rows(const float* A, const float* w, float* phi_rows_out, float* r_out, int batch, int T,
+                                       int n, int k_lo, int k_hi, unsigned flags, void* cuda_stream) {
+  if (!A || !w || !phi_rows_out || !r_out) return LTV_ERR_NULL_PTR;
+  int st = check_dims(batch, T, n, 0);
+  if (st != LTV_OK) return st;
+  if (k_lo < 1 || k_hi > T || k_lo >= k_hi || (flags & ~static_cast<unsigned>(LTV_TUBE_ROW_2NORM)) != 0) return LTV_ERR_BAD_DIM;
+  if (grid_yz_overflow(batch)) return LTV_ERR_UNSUPPORTED_SHAPE;
+  if (misaligned(A) || misaligned(w) || misaligned(phi_rows_out) || misaligned(r_out)) return LTV_ERR_ALIGNMENT;
+  int sms = 0;
+  st = check_device(&sms);
+  if (st != LTV_OK) return st;
+  PhiRowsArgs a{A, w, phi_rows_out, r_out, batch, T, n, k_lo, k_hi, (flags & LTV_TUBE_ROW_2NORM) ? 1 : 0};
+  unsigned long long l = 0;
+  cudaError_t err = launch_phi_rows(a, static_cast<cudaStream_t>(cuda_stream), &l);
+  g_launches += l;
+  return err == cudaSuccess ? LTV_OK : fail_cuda(err);
+}
+
 int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float* c_host, const float* x0_host,
                            const float* u_host, const float* w_host, const float* g_host, float* x_host,
                            float* phi_host, float* r_host, float* lambda_host, float* grad_u_host,

@@ -115,6 +115,16 @@ struct AsmArgs {
 size_t asm_workspace_bytes(int batch, int T, int n, int p);
 cudaError_t launch_ofb_assemble(const AsmArgs& a, cudaStream_t stream, unsigned long long* launches);
 
+// Block rows of the system response of one shard (phi_rows.cu)
+struct PhiRowsArgs {
+  const float *A, *w;
+  float *phi, *r;      // phi [batch, Ps, n, n] (the shard's column-packed order), r [batch, T, n] (rows k_lo .. k_hi-1 written)
+  int batch, T, n, k_lo, k_hi, tube_mode;
+};
+long long phi_row_shard_blocks(int T, int k_lo, int k_hi);
+long long phi_row_shard_index(int T, int k_lo, int k_hi, int k, int j);
+cudaError_t launch_phi_rows(const PhiRowsArgs& a, cudaStream_t stream, unsigned long long* launches);
+
 // Margins (12d) on assembled operators (margins.cu)
 struct MarginArgs {
   const float *phi_xw, *phi_uw, *phi_xe, *phi_ue, *Hx, *Hu, *w, *f;   // phi_uw / Hu and phi_xe / phi_ue may be null

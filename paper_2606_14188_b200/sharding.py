@@ -12,6 +12,39 @@ def shard_range(global_batch: int, rank: int, world: int) -> tuple[int, int]:
     return b0, b0 + base + (1 if rank < rem else 0)
 
 
+def row_shard_range(T: int, rank: int, world: int) -> tuple[int, int]:
+    """Block rows [k_lo, k_hi) of the system response Phi(k,j), 1 <= k <= T-1, for `rank` of `world` when ONE item (or a
+    batch too small to shard) is split over the GPUs (ltv_scan_system_response_tube_rows, optional).  Row k has
+    k blocks, so the ranges are balanced by block count, not by row count: contiguous, disjoint, covering 1 .. T-1; a rank
+    may get an empty range (k_lo == k_hi) when there are more ranks than rows.  Nothing is exchanged on the data path: every
+    rank holds A, computes its rows alone, and owns the complete tube rows r_k of its range."""
+    if not (0 <= rank < world) or T < 1:
+        raise ValueError("bad rank/world/T")
+    total = T * (T - 1) // 2                       # blocks of all rows
+    bounds = [1]
+    k = 1
+    acc = 0
+    for r in range(1, world):
+        target = total * r / world
+        while k < T and abs(acc + k - target) <= abs(acc - target):  # take row k while that brings the block count closer to the target
+            acc += k
+            k += 1
+        bounds.append(k)
+    bounds.append(T)
+    return bounds[rank], bounds[rank + 1]
+
+
+def assemble_tube_rows(r_local, device=None):
+    """Sum over ranks of the zero-initialised r[batch,T,n] arrays of the row shards = the complete tube (every row is
+    non-zero on exactly one rank; identity without torch.distributed).  The only exchange of the row-sharded path, and not
+    on its data path: T n floats per item."""
+    import torch.distributed as dist
+
+    if dist.is_available() and dist.is_initialized():
+        dist.all_reduce(r_local, op=dist.ReduceOp.SUM)
+    return r_local
+
+
 def shard_arrays(arrays: dict, rank: int, world: int) -> dict:
     """The items [b0, b1) of this rank of every batch-leading array in `arrays` (None entries pass through): all calls of
     the library - rollout, system response, adjoint, observer response, Kalman gains, constraint margins, output-feedback

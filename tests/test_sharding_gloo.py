@@ -105,3 +105,81 @@ def test_two_rank_batch_sharding_gloo():
     assert np.array_equal(np.concatenate([g[9] for g in got]), O.constraint_tightening(W.A, W.w, Hc))
     assert all(g[5] == 2.0 for g in got)        # max over ranks
     assert all(g[6] == 5.0 for g in got)        # units of all ranks
+
+
+def test_row_shard_range_partitions_the_block_rows():
+    from paper_2606_14188_b200.sharding import row_shard_range
+
+    for T in (1, 2, 3, 16, 32, 65):
+        for world in (1, 2, 3, 8):
+            r = [row_shard_range(T, k, world) for k in range(world)]
+            assert r[0][0] == 1 and r[-1][1] == max(T, 1)
+            assert all(r[k][1] == r[k + 1][0] for k in range(world - 1))        # contiguous, disjoint, covering 1 .. T-1
+            assert all(a <= b for a, b in r)
+            blocks = [sum(range(a, b)) for a, b in r]
+            assert sum(blocks) == T * (T - 1) // 2
+            if T >= 16:                                                        # balanced by BLOCKS up to one row (<= T-1 blocks)
+                assert max(blocks) - T * (T - 1) / 2 / world <= T
+
+
+def _row_worker(rank, world, port, q):
+    """One item split over the ranks by block rows: each rank computes ITS rows with the oracle's row recursion (what
+    ltv_scan_system_response_tube_rows does on a GPU), the tube is assembled by the one all-reduce of the row-sharded path."""
+    import torch
+    import torch.distributed as dist
+
+    from oracle import ltv_oracle as O
+    from paper_2606_14188_b200.sharding import assemble_tube_rows, row_shard_range
+    from workloads import config, generate
+
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    W = generate(config(0, batch=2, T=9))                    # A is replicated: every rank generates the same items
+    batch, T, n, _ = W.shape
+    k_lo, k_hi = row_shard_range(T, rank, world)
+    r_local = torch.zeros((batch, T, n), dtype=torch.float64)
+    mine = {}
+    for b in range(batch):
+        for t, row in O.phi_rows_item(W.A[b]):               # block rows of the oracle, in order
+            if k_lo <= t < k_hi:
+                acc = np.zeros(n)
+                for s in range(t):
+                    acc = acc + np.abs(row[s]) @ W.w[b, s].astype(np.float64)
+                    mine[(b, t, s)] = row[s].copy()
+                r_local[b, t] = torch.from_numpy(acc)
+    own = r_local.clone()
+    r_all = assemble_tube_rows(r_local)
+    q.put((rank, k_lo, k_hi, own.numpy(), r_all.numpy(), sorted(mine.keys())))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_row_sharding_of_single_items_gloo():
+    from oracle import ltv_oracle as O
+    from workloads import config, generate
+
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    world = 2
+    procs = [ctx.Process(target=_row_worker, args=(k, world, port, q)) for k in range(world)]
+    for p in procs:
+        p.start()
+    got = sorted([q.get(timeout=120) for _ in range(world)], key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    W = generate(config(0, batch=2, T=9))
+    T = W.A.shape[1]
+    r = O.tube(W.A, W.w)
+    assert got[0][1] == 1 and got[0][2] == got[1][1] and got[1][2] == T
+    for g in got:
+        assert np.allclose(g[4], r, rtol=1e-12, atol=0.0)                     # every rank ends up with the complete tube
+        mask = np.zeros(T, dtype=bool); mask[g[1]:g[2]] = True
+        assert np.all(g[3][:, ~mask] == 0.0) and np.allclose(g[3][:, mask], r[:, mask], rtol=1e-12)   # its own rows were complete
+    keys = got[0][5] + got[1][5]
+    assert len(keys) == len(set(keys)) == 2 * T * (T - 1) // 2                # every block on exactly one rank
