@@ -511,9 +511,21 @@ def next_rows(B, L, W, steps):
     out["constraints"] = dict(nc=6, ms=ms, items_per_s=batch * B.world / (ms * 1e-3))
     del wsc
     # NEXT-4: assembled output-feedback responses (15) + tube (12e)
-    wsf = torch.empty(L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, batch, T, n, 0), dtype=torch.uint8, device=dev)
+    #   default route (column recursion on D = Phi^xw - Phibar^x at this size) and the log-depth cross-scan route
+    need = L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, batch, T, n, max(m, p))
+    wsf = torch.empty(need, dtype=torch.uint8, device=dev)
     ms = timed(lambda: L.ltv_scan_output_feedback_response(d["A"], d["B"], Kfb, Lt, Cm, d["w"], ff, workspace=wsf), min(steps, 3))
-    out["output_feedback"] = dict(p=p, ms=ms, blocks_per_s=batch * B.world * P / (ms * 1e-3))
+    out["output_feedback"] = dict(p=p, ms=ms, blocks_per_s=batch * B.world * P / (ms * 1e-3), workspace_gb=need / 1e9)
+    del wsf
+    torch.cuda.empty_cache()
+    L.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, 1)
+    try:
+        need = L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, batch, T, n, max(m, p))
+        wsf = torch.empty(need, dtype=torch.uint8, device=dev)
+        ms1 = timed(lambda: L.ltv_scan_output_feedback_response(d["A"], d["B"], Kfb, Lt, Cm, d["w"], ff, workspace=wsf), min(steps, 3))
+        out["output_feedback"].update(cross_scan_route_ms=ms1, cross_scan_route_workspace_gb=need / 1e9)
+    finally:
+        L.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, 0)
     del wsf
     torch.cuda.empty_cache()
     # NEXT-4 / NEXT-2: input-side responses of (15) + closed-loop margins (12d), both terms, rows on [z; v]

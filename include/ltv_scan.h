@@ -438,9 +438,14 @@ LTV_API int ltv_scan_pipeline_host(const float* A_host, const float* B_host, con
  *                            if that cluster cannot be placed).  Used by the tests to cover every cluster size.
  *   LTV_OPT_PIPELINE_CHUNKS  number of batch chunks ltv_scan_pipeline_host overlaps upload and compute over:
  *                            1 .. 16, default 8 (1 = no overlap; C2: 16.0 ms with 4, 15.2 ms with 8 - the upload at PCIe rates is the long leg, more chunks shorten the exposed last compute).
+ *   LTV_OPT_OUTPUT_FEEDBACK_ROUTE  how ltv_scan_output_feedback_response evaluates (15) for n >= 96: 1 = cross scan (log depth,
+ *                            4 n^3 products per block), 2 = column recursion (one scan for Phibar^x + the backward recursion
+ *                            of ltv_scan_output_feedback_assemble: 2 n^3 products per block, T-1 sequential steps), 0
+ *                            (default) = by size (2 once a step's GEMM fills the GPU).  Read by the call AND by
+ *                            ltv_scan_workspace_bytes(LTV_OP_OUTPUT_FEEDBACK, ..): size the workspace after setting it.
  * ltv_set_option returns LTV_ERR_BAD_DIM for an unknown option or a value out of range; ltv_get_option returns -1 for
  * an unknown option. */
-enum { LTV_OPT_VECTOR_CLUSTER = 0, LTV_OPT_PIPELINE_CHUNKS = 1, LTV_OPT_COUNT = 2 };
+enum { LTV_OPT_VECTOR_CLUSTER = 0, LTV_OPT_PIPELINE_CHUNKS = 1, LTV_OPT_OUTPUT_FEEDBACK_ROUTE = 2, LTV_OPT_COUNT = 3 };
 LTV_API int ltv_set_option(int option, int value);
 LTV_API int ltv_get_option(int option);
 

@@ -14,7 +14,7 @@ _API = (
     "ltv_launch_count", "ltv_phi_block_index", "ltv_profile_collect", "ltv_profile_enable",
     "ltv_scan_adjoint", "ltv_scan_pipeline_host", "ltv_scan_rollout", "ltv_scan_system_response_tube",
     "ltv_scan_workspace_bytes", "ltv_scan_observer_response", "ltv_observer_row_floats", "ltv_scan_kalman_gains",
-    "ltv_set_option", "ltv_get_option", "ltv_scan_all", "ltv_scan_all_is_fused", "ltv_scan_rollout_adjoint", "ltv_scan_output_feedback_constraints", "LTV_OPT_VECTOR_CLUSTER", "LTV_OPT_PIPELINE_CHUNKS",
+    "ltv_set_option", "ltv_get_option", "ltv_scan_all", "ltv_scan_all_is_fused", "ltv_scan_rollout_adjoint", "ltv_scan_output_feedback_constraints", "LTV_OPT_VECTOR_CLUSTER", "LTV_OPT_PIPELINE_CHUNKS", "LTV_OPT_OUTPUT_FEEDBACK_ROUTE",
     "LTV_OP_KALMAN_GAINS", "LTV_OP_OUTPUT_FEEDBACK", "ltv_scan_output_feedback_response", "LTV_KALMAN_SCAN", "LTV_KALMAN_RECURSION", "LTV_OP_CONSTRAINT_TIGHTENING", "ltv_scan_constraint_tightening",
     "ltv_static_scratch_bytes", "ltv_scan_system_response_tube_static", "LTV_ERR_STATIC_SCRATCH_LIMIT",
     "ltv_scan_output_feedback_assemble", "ltv_scan_operator_constraint_margins",

@@ -29,7 +29,7 @@ LTV_OBSERVER_SHIFTED_GAIN = 2
 LTV_KALMAN_SCAN, LTV_KALMAN_RECURSION = 1, 2
 LTV_PHI_ROW_PACKED, LTV_PHI_SQUARE_GRID, LTV_PHI_COLUMN_PACKED = 0, 1, 2
 LTV_OP_SYSTEM_RESPONSE_TUBE_RELAYOUT = 9
-LTV_OPT_VECTOR_CLUSTER, LTV_OPT_PIPELINE_CHUNKS = 0, 1
+LTV_OPT_VECTOR_CLUSTER, LTV_OPT_PIPELINE_CHUNKS, LTV_OPT_OUTPUT_FEEDBACK_ROUTE = 0, 1, 2
 
 EXPORTS = (
     "ltv_phi_block_index", "ltv_phi_block_index_layout", "ltv_scan_workspace_bytes", "ltv_scan_rollout", "ltv_scan_system_response_tube",
@@ -391,7 +391,7 @@ def ltv_scan_output_feedback_response(A, B, Kfb, Lt, C, w, f, want_xe=True, work
     phi_xw = torch.empty((batch, P, n, n), device=A.device, dtype=torch.float32)
     phi_xe = torch.empty((batch, P, n, p), device=A.device, dtype=torch.float32) if want_xe else None
     tau = torch.empty((batch, T, n), device=A.device, dtype=torch.float32)
-    need = ltv_scan_workspace_bytes(LTV_OP_OUTPUT_FEEDBACK, batch, T, n, 0)
+    need = ltv_scan_workspace_bytes(LTV_OP_OUTPUT_FEEDBACK, batch, T, n, max(m, p))
     if workspace is None:
         workspace = torch.empty(max(need, 16), device=A.device, dtype=torch.uint8)
     st = lib.ltv_scan_output_feedback_response(_ptr(A), _ptr(B), _ptr(Kfb), _ptr(Lt), _ptr(C), _ptr(w), _ptr(f),

@@ -45,7 +45,7 @@ unsigned int* dbg_buffer_device() {
 extern "C" LTV_API unsigned int* ltv_debug_buffer(void) { return g_dbg_host; }
 #endif
 
-static std::atomic<int> g_options[LTV_OPT_COUNT] = {{0}, {8}};
+static std::atomic<int> g_options[LTV_OPT_COUNT] = {{0}, {8}, {0}};
 int option(int which) { return g_options[which].load(std::memory_order_relaxed); }
 
 int pick_cluster_model(int batch, int n, const int* max_active, int sm_budget) {
@@ -215,7 +215,7 @@ size_t ltv_scan_workspace_bytes(int op, int batch, int T, int n, int m) {
       return constraint_workspace_bytes(batch, T, n, m);
     case LTV_OP_OUTPUT_FEEDBACK:
       if (check_dims(batch, T, 2 * n, 0) != LTV_OK) return 0;
-      return ofb_workspace_bytes(batch, T, n);
+      return ofb_workspace_bytes(batch, T, n, m, m);   // m = max(m, p) of the call, or 0 = unknown
     case LTV_OP_PIPELINE_HOST:
     case LTV_OP_PIPELINE_HOST_NO_PHI: {
       const bool with_phi = op == LTV_OP_PIPELINE_HOST;
@@ -568,7 +568,7 @@ int ltv_scan_output_feedback_response(const float* A, const float* B, const floa
   if (misaligned(A) || misaligned(B) || misaligned(Kfb) || misaligned(Lt) || misaligned(C) || misaligned(w) ||
       misaligned(f) || misaligned(phi_xw_out) || misaligned(phi_xe_out) || misaligned(tau_out) || misaligned(workspace))
     return LTV_ERR_ALIGNMENT;
-  if (workspace_bytes < ofb_workspace_bytes(batch, T, n)) return LTV_ERR_WORKSPACE_TOO_SMALL;
+  if (workspace_bytes < ofb_workspace_bytes(batch, T, n, m, p)) return LTV_ERR_WORKSPACE_TOO_SMALL;
   int sms = 0;
   st = check_device(&sms);
   if (st != LTV_OK) return st;
@@ -883,6 +883,9 @@ int ltv_set_option(int opt, int value) {
       break;
     case LTV_OPT_PIPELINE_CHUNKS:
       if (value < 1 || value > 16) return LTV_ERR_BAD_DIM;
+      break;
+    case LTV_OPT_OUTPUT_FEEDBACK_ROUTE:
+      if (value < 0 || value > 2) return LTV_ERR_BAD_DIM;
       break;
     default:
       return LTV_ERR_BAD_DIM;

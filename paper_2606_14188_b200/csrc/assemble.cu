@@ -63,6 +63,13 @@ struct AsmStep {
   const float *Ltt, *C, *w, *f;
   float* tau;            // [batch, T, n], x side only, or null
   int T, n, p, R, is_u, j;
+  // DIFFERENCE mode (gain-defined controllers, x side only; see launch_ofb_response_columns): the recursion carries
+  // D = Phi^xw - Phibar^x.  Ltt / C above are replaced by Gt = B^T [batch,T,pc,n] and Cm = Kfb [batch,T,pc,n] for the rank-pc
+  // correction, Lte = Lt^T [batch,T,p,n] gives e = D Lt_{j-1}; dcol = the D blocks (k, j), k = j+1 .. T-1, of this column
+  // ([batch, T-1, n, n], block k-j-1), read (GEMM result) and written in place; out receives Phi^xw = D + Phibar^x.
+  const float *Gt, *Cm, *Lte;
+  float* dcol;
+  int pc;
 };
 
 __device__ __forceinline__ float warp_sum(float v) {
@@ -79,11 +86,12 @@ __device__ __forceinline__ float warp_sum(float v) {
 // then e = (row - Phibar(k,j)[i]) Lt_{j-1} (j >= 1) and, x side, tau_k[i] += ||row o w_j|| + ||e o f_{j-1}||.
 // NP = p exactly for p <= 8 (every loop over the measurements unrolls, the sums stay in registers); NP = 0: any p <= 32
 // (32 guarded accumulators, one row per warp).  grid (ceil(groups / 8), batch), groups = (T-1-j) ceil(R / ROWS).
-template <int NP, int ROWS>
+template <int NP, int ROWS, bool DIFF = false>
 __global__ void __launch_bounds__(256) asm_step_kernel(const AsmStep s) {
   constexpr int PMAX = NP > 0 ? NP : 32;
   const int T = s.T, n = s.n, R = s.R, j = s.j;
-  const int p = NP > 0 ? NP : s.p;
+  const int p = (NP > 0 && !DIFF) ? NP : s.p;   // rank of the noise term (DIFF: p <= NP, the rest of the accumulators idle)
+  const int pcr = DIFF ? s.pc : p;             // rank of the correction
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int gpb = (R + ROWS - 1) / ROWS;   // row groups per block
   const int grp = blockIdx.x * 8 + warp;
@@ -108,13 +116,16 @@ __global__ void __launch_bounds__(256) asm_step_kernel(const AsmStep s) {
     pb_cur = reinterpret_cast<const float4*>(s.pbar + ((item + phi_colbase(T, j) + (k - j - 1)) * R + i0) * n);
   }
   const size_t oblk = static_cast<size_t>(b) * P + phi_colbase(T, j) + (k - j - 1);
-  float4* orow = reinterpret_cast<float4*>(s.out + (oblk * R + i0) * n);
-  const float4* Lj = reinterpret_cast<const float4*>(s.Ltt + (bT + j) * p * n);
-  const float4* Cj = reinterpret_cast<const float4*>(s.C + (bT + j) * p * n);
-  const float4* Ljm = (j >= 1) ? reinterpret_cast<const float4*>(s.Ltt + (bT + j - 1) * p * n) : nullptr;
+  float4* orow = DIFF ? reinterpret_cast<float4*>(s.dcol + ((static_cast<size_t>(b) * (T - 1) + kk) * n + i0) * n)
+                      : reinterpret_cast<float4*>(s.out + (oblk * R + i0) * n);
+  float4* xrow = DIFF ? reinterpret_cast<float4*>(s.out + (oblk * R + i0) * n) : nullptr;   // Phi^xw = D + Phibar^x
+  const float4* Lj = reinterpret_cast<const float4*>((DIFF ? s.Gt : s.Ltt) + (bT + j) * pcr * n);
+  const float4* Cj = reinterpret_cast<const float4*>((DIFF ? s.Cm : s.C) + (bT + j) * pcr * n);
+  const float4* Ljm = (j >= 1) ? reinterpret_cast<const float4*>((DIFF ? s.Lte : s.Ltt) + (bT + j - 1) * p * n) : nullptr;
   const float4* wj = reinterpret_cast<const float4*>(s.w + (bT + j) * n);
-  const float4* arow = (!s.is_u && kk == 0) ? reinterpret_cast<const float4*>(s.A + ((bT + j) * n + i0) * n) : nullptr;
+  const float4* arow = (!DIFF && !s.is_u && kk == 0) ? reinterpret_cast<const float4*>(s.A + ((bT + j) * n + i0) * n) : nullptr;
   const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+  const bool corr = pb_next != nullptr || (DIFF && kk == 0);   // DIFF, k = j+1: Phibar^x(j+1,j+1) = I, the gain row is B_j[i]
 
   // u[r][q] = Phibar(k,j+1)[i0 + r] . Lt_j[:,q]
   float u[ROWS][PMAX];
@@ -129,7 +140,7 @@ __global__ void __launch_bounds__(256) asm_step_kernel(const AsmStep s) {
       for (int r = 0; r < ROWS; ++r) a[r] = (r < nr) ? __ldg(pb_next + static_cast<size_t>(r) * n4 + c) : z4;
 #pragma unroll
       for (int q = 0; q < PMAX; ++q) {
-        if (NP > 0 || q < p) {
+        if ((NP > 0 && !DIFF) || q < pcr) {
           const float4 l = __ldg(Lj + static_cast<size_t>(q) * n4 + c);
 #pragma unroll
           for (int r = 0; r < ROWS; ++r)
@@ -141,7 +152,14 @@ __global__ void __launch_bounds__(256) asm_step_kernel(const AsmStep s) {
     for (int r = 0; r < ROWS; ++r)
 #pragma unroll
       for (int q = 0; q < PMAX; ++q)
-        if (NP > 0 || q < p) u[r][q] = warp_sum(u[r][q]);
+        if ((NP > 0 && !DIFF) || q < pcr) u[r][q] = warp_sum(u[r][q]);
+  } else if (DIFF && kk == 0) {
+    const float* Bt = s.Gt + (bT + j) * pcr * n;
+#pragma unroll
+    for (int r = 0; r < ROWS; ++r)
+#pragma unroll
+      for (int q = 0; q < PMAX; ++q)
+        if (q < pcr && r < nr) u[r][q] = __ldg(Bt + static_cast<size_t>(q) * n + i0 + r);
   }
   // the rows, their tube terms and e = (row - Phibar(k,j)[i]) Lt_{j-1}
   float s1[ROWS];
@@ -157,16 +175,16 @@ __global__ void __launch_bounds__(256) asm_step_kernel(const AsmStep s) {
 #pragma unroll
     for (int r = 0; r < ROWS; ++r) {
       if (r < nr) {
-        if (kk == 0) x[r] = s.is_u ? z4 : __ldg(arow + static_cast<size_t>(r) * n4 + c); else x[r] = orow[static_cast<size_t>(r) * n4 + c];
-        pc[r] = (Ljm != nullptr) ? __ldg(pb_cur + static_cast<size_t>(r) * n4 + c) : z4;
+        if (kk == 0) x[r] = (s.is_u || DIFF) ? z4 : __ldg(arow + static_cast<size_t>(r) * n4 + c); else x[r] = orow[static_cast<size_t>(r) * n4 + c];
+        pc[r] = (DIFF || Ljm != nullptr) ? __ldg(pb_cur + static_cast<size_t>(r) * n4 + c) : z4;
       } else {
         x[r] = z4; pc[r] = z4;
       }
     }
-    if (pb_next != nullptr) {
+    if (corr) {
 #pragma unroll
       for (int q = 0; q < PMAX; ++q) {
-        if (NP > 0 || q < p) {
+        if ((NP > 0 && !DIFF) || q < pcr) {
           const float4 cq = __ldg(Cj + static_cast<size_t>(q) * n4 + c);
 #pragma unroll
           for (int r = 0; r < ROWS; ++r) {
@@ -178,7 +196,17 @@ __global__ void __launch_bounds__(256) asm_step_kernel(const AsmStep s) {
     }
 #pragma unroll
     for (int r = 0; r < ROWS; ++r)
-      if (r < nr) orow[static_cast<size_t>(r) * n4 + c] = x[r];
+      if (r < nr && (!DIFF || j > 0)) orow[static_cast<size_t>(r) * n4 + c] = x[r];   // DIFF: column 0 feeds no further product
+    if (DIFF) {
+      // x = row of D: the response row is D + Phibar^x, and e = D Lt_{j-1} runs over D itself (no subtraction)
+#pragma unroll
+      for (int r = 0; r < ROWS; ++r) {
+        const float4 d = x[r];
+        x[r].x += pc[r].x; x[r].y += pc[r].y; x[r].z += pc[r].z; x[r].w += pc[r].w;
+        if (r < nr) xrow[static_cast<size_t>(r) * n4 + c] = x[r];
+        pc[r] = d;
+      }
+    }
     if (!s.is_u) {
       const float4 ww = __ldg(wj + c);
 #pragma unroll
@@ -188,13 +216,15 @@ __global__ void __launch_bounds__(256) asm_step_kernel(const AsmStep s) {
       }
     }
     if (Ljm != nullptr) {
+      if (!DIFF) {
 #pragma unroll
-      for (int r = 0; r < ROWS; ++r) {
-        pc[r].x = x[r].x - pc[r].x; pc[r].y = x[r].y - pc[r].y; pc[r].z = x[r].z - pc[r].z; pc[r].w = x[r].w - pc[r].w;
+        for (int r = 0; r < ROWS; ++r) {
+          pc[r].x = x[r].x - pc[r].x; pc[r].y = x[r].y - pc[r].y; pc[r].z = x[r].z - pc[r].z; pc[r].w = x[r].w - pc[r].w;
+        }
       }
 #pragma unroll
       for (int q = 0; q < PMAX; ++q) {
-        if (NP > 0 || q < p) {
+        if ((NP > 0 && !DIFF) || q < p) {
           const float4 l = __ldg(Ljm + static_cast<size_t>(q) * n4 + c);
 #pragma unroll
           for (int r = 0; r < ROWS; ++r)
@@ -212,7 +242,7 @@ __global__ void __launch_bounds__(256) asm_step_kernel(const AsmStep s) {
     if (Ljm != nullptr) {
 #pragma unroll
       for (int q = 0; q < PMAX; ++q) {
-        if (NP > 0 || q < p) {
+        if ((NP > 0 && !DIFF) || q < p) {
           const float eq = warp_sum(e[r][q]);
           const float t = eq * __ldg(fj + q);
           s2 = fmaf(t, t, s2);
@@ -235,11 +265,14 @@ __global__ void __launch_bounds__(256) asm_step_kernel(const AsmStep s) {
 // CTA stays on one item, stages Lt_j^T, C_j, Lt_{j-1}^T and w_j in shared memory ONCE, and each warp walks its rows with a
 // two-stage cp.async ring: the (up to) three rows of row r+1 - Phibar(k,j+1)[i], the GEMM result, Phibar(k,j)[i] - are in
 // flight while row r is reduced out of shared memory.
-template <int NP>
+// DIFF (difference mode, see AsmStep): NP = max(pc, p); the vectors beyond a rank are staged as zeros.
+template <int NP, bool DIFF = false>
 __global__ void __launch_bounds__(256) asm_step_pipe_kernel(const AsmStep s) {
   extern __shared__ float4 asm_sm[];
   const int T = s.T, n = s.n, R = s.R, j = s.j;
   constexpr int p = NP;
+  const int pe = DIFF ? s.p : NP;     // rank of the noise term = row length of oute and f
+  const int pcr = DIFF ? s.pc : NP;   // rank of the correction
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int b = blockIdx.y;
   const int n4 = n >> 2;
@@ -252,13 +285,15 @@ __global__ void __launch_bounds__(256) asm_step_pipe_kernel(const AsmStep s) {
   float4* vw = vLm + p * n4;           // [n4]    w_j
   float4* ring = vw + n4 + static_cast<size_t>(warp) * 6 * n4;   // [2 stages][3 rows][n4] of this warp
   {
-    const float4* Lj = reinterpret_cast<const float4*>(s.Ltt + (bT + j) * p * n);
-    const float4* Cj = reinterpret_cast<const float4*>(s.C + (bT + j) * p * n);
+    const float4* Lj = reinterpret_cast<const float4*>((DIFF ? s.Gt : s.Ltt) + (bT + j) * pcr * n);
+    const float4* Cj = reinterpret_cast<const float4*>((DIFF ? s.Cm : s.C) + (bT + j) * pcr * n);
     const float4* wj = reinterpret_cast<const float4*>(s.w + (bT + j) * n);
+    const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int e = threadIdx.x; e < p * n4; e += 256) {
-      vL[e] = __ldg(Lj + e);
-      vC[e] = __ldg(Cj + e);
-      if (j >= 1) vLm[e] = __ldg(reinterpret_cast<const float4*>(s.Ltt + (bT + j - 1) * p * n) + e);
+      const bool in_c = !DIFF || e < pcr * n4, in_e = !DIFF || e < pe * n4;
+      vL[e] = in_c ? __ldg(Lj + e) : z4;
+      vC[e] = in_c ? __ldg(Cj + e) : z4;
+      if (j >= 1) vLm[e] = in_e ? __ldg(reinterpret_cast<const float4*>((DIFF ? s.Lte : s.Ltt) + (bT + j - 1) * pe * n) + e) : z4;
     }
     for (int e = threadIdx.x; e < n4; e += 256) vw[e] = __ldg(wj + e);
   }
@@ -272,7 +307,12 @@ __global__ void __launch_bounds__(256) asm_step_pipe_kernel(const AsmStep s) {
     k = j + 1 + kk;
     oidx = (item_x + phi_colbase(T, j) + (k - j - 1)) * R + i;
     orow = reinterpret_cast<float4*>(s.out + oidx * n);
-    if (s.is_u) {
+    if (DIFF) {
+      orow = reinterpret_cast<float4*>(s.dcol + ((static_cast<size_t>(b) * (T - 1) + kk) * n + i) * n);   // row of D(k,j)
+      nx = kk > 0 ? reinterpret_cast<const float4*>(s.pbar + ((item_x + phi_colbase(T, j + 1) + (k - j - 2)) * R + i) * n) : nullptr;
+      cu = reinterpret_cast<const float4*>(s.pbar + ((item_x + phi_colbase(T, j) + (k - j - 1)) * R + i) * n);
+      bs = kk == 0 ? nullptr : orow;
+    } else if (s.is_u) {
       nx = reinterpret_cast<const float4*>(s.pbar + ((item_u + qd(k, j + 1)) * R + i) * n);
       cu = reinterpret_cast<const float4*>(s.pbar + ((item_u + qd(k, j)) * R + i) * n);
       bs = kk == 0 ? nullptr : orow;
@@ -290,14 +330,14 @@ __global__ void __launch_bounds__(256) asm_step_pipe_kernel(const AsmStep s) {
       for (int c = lane; c < n4; c += 32) {
         if (nx != nullptr) cp_async16(dst + c, nx + c);
         if (bs != nullptr) cp_async16(dst + n4 + c, bs + c);
-        if (has_e) cp_async16(dst + 2 * n4 + c, cu + c);
+        if (has_e || DIFF) cp_async16(dst + 2 * n4 + c, cu + c);
       }
     }
     cp_async_commit();
   };
   float fq[NP];   // f_{j-1}: the scaling of the measurement noise that enters through Lt_{j-1}
 #pragma unroll
-  for (int q = 0; q < NP; ++q) fq[q] = has_e ? __ldg(s.f + (bT + j - 1) * p + q) : 0.f;
+  for (int q = 0; q < NP; ++q) fq[q] = (has_e && q < pe) ? __ldg(s.f + (bT + j - 1) * pe + q) : 0.f;
   const int stride = gridDim.x * 8;
   int row = blockIdx.x * 8 + warp;
   prefetch(row, 0);
@@ -328,29 +368,45 @@ __global__ void __launch_bounds__(256) asm_step_pipe_kernel(const AsmStep s) {
       }
 #pragma unroll
       for (int q = 0; q < NP; ++q) u[q] = warp_sum(u[q]);
+    } else if (DIFF) {
+      // k = j+1: Phibar^x(j+1,j+1) = I, so the gain row is row i of B_j = column i of the staged B_j^T (zeros beyond pc)
+      const float* vLf = reinterpret_cast<const float*>(vL);
+#pragma unroll
+      for (int q = 0; q < NP; ++q) u[q] = vLf[static_cast<size_t>(q) * n + row % R];
     }
+    const bool corr = nx != nullptr || DIFF;
+    float4* xrow = DIFF ? reinterpret_cast<float4*>(s.out + oidx * n) : nullptr;   // Phi^xw = D + Phibar^x
     float s1 = 0.f;
     float e[NP];
 #pragma unroll
     for (int q = 0; q < NP; ++q) e[q] = 0.f;
     for (int c = lane; c < n4; c += 32) {
       float4 x = (bs != nullptr) ? s_base[c] : make_float4(0.f, 0.f, 0.f, 0.f);
-      if (nx != nullptr) {
+      if (corr) {
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
           const float4 cq = vC[q * n4 + c];
           x.x = fmaf(-u[q], cq.x, x.x); x.y = fmaf(-u[q], cq.y, x.y); x.z = fmaf(-u[q], cq.z, x.z); x.w = fmaf(-u[q], cq.w, x.w);
         }
       }
-      orow[c] = x;
+      if (!DIFF || j > 0) orow[c] = x;   // DIFF: column 0 of D feeds no further product
+      const float4 d = x;
+      if (DIFF) {
+        const float4 pc = s_cur[c];
+        x.x += pc.x; x.y += pc.y; x.z += pc.z; x.w += pc.w;
+        xrow[c] = x;
+      }
       if (!s.is_u) {
         const float4 ww = vw[c];
         const float e0 = x.x * ww.x, e1 = x.y * ww.y, e2 = x.z * ww.z, e3 = x.w * ww.w;
         s1 = fmaf(e0, e0, fmaf(e1, e1, fmaf(e2, e2, fmaf(e3, e3, s1))));
       }
       if (has_e) {
-        const float4 pc = s_cur[c];
-        const float4 v = make_float4(x.x - pc.x, x.y - pc.y, x.z - pc.z, x.w - pc.w);
+        float4 v = d;   // DIFF: e = D Lt_{j-1}
+        if (!DIFF) {
+          const float4 pc = s_cur[c];
+          v = make_float4(x.x - pc.x, x.y - pc.y, x.z - pc.z, x.w - pc.w);
+        }
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
           const float4 l = vLm[q * n4 + c];
@@ -365,10 +421,10 @@ __global__ void __launch_bounds__(256) asm_step_pipe_kernel(const AsmStep s) {
         const float eq = warp_sum(e[q]);
         const float t = eq * fq[q];
         s2 = fmaf(t, t, s2);
-        if (s.oute != nullptr && lane == q) s.oute[oidx * p + q] = eq;
+        if (s.oute != nullptr && lane == q && q < pe) s.oute[oidx * pe + q] = eq;
       }
-    } else if (s.oute != nullptr && lane < p) {
-      s.oute[oidx * p + lane] = 0.f;   // j = 0: no measurement noise has entered yet
+    } else if (s.oute != nullptr && lane < pe) {
+      s.oute[oidx * pe + lane] = 0.f;   // j = 0: no measurement noise has entered yet
     }
     if (tau_p != nullptr) {
       s1 = warp_sum(s1);
@@ -383,12 +439,12 @@ size_t asm_pipe_smem_bytes(int n, int p) { return (static_cast<size_t>(3) * p * 
 
 constexpr int kAsmWaves = 8;
 
-template <int NP>
+template <int NP, bool DIFF = false>
 cudaError_t launch_asm_step_pipe(const AsmStep& s, int batch, int sms, cudaStream_t stream) {
   const size_t smem = asm_pipe_smem_bytes(s.n, NP);
   static size_t attr_set = 0;   // largest dynamic shared-memory size the attribute was raised to (per instantiation)
   if (smem > 48 * 1024 && smem > attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(asm_step_pipe_kernel<NP>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    cudaError_t e = cudaFuncSetAttribute(asm_step_pipe_kernel<NP, DIFF>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     if (e != cudaSuccess) return e;
     attr_set = smem;
   }
@@ -399,7 +455,7 @@ cudaError_t launch_asm_step_pipe(const AsmStep& s, int batch, int sms, cudaStrea
   // staging of the vectors is still amortised over >= 30 rows per warp on the long steps)
   int cx = (env_int("ASM_WAVES", kAsmWaves) * per_sm * sms + batch - 1) / batch;
   cx = std::max(1, std::min(cx, (rtot + 7) / 8));
-  asm_step_pipe_kernel<NP><<<dim3(cx, batch), 256, smem, stream>>>(s);
+  asm_step_pipe_kernel<NP, DIFF><<<dim3(cx, batch), 256, smem, stream>>>(s);
   return cudaSuccess;
 }
 
@@ -434,9 +490,164 @@ void launch_asm_step(const AsmStep& s, int batch, int sms, cudaStream_t stream) 
   }
 }
 
+// difference mode: NP = max(pc, p) <= 8
+void launch_asm_step_diff(const AsmStep& s, int batch, int sms, cudaStream_t stream) {
+  const int np = std::max(s.pc, s.p);
+  if (asm_pipe_smem_bytes(s.n, np) <= 200u * 1024u) {
+    switch (np) {
+      case 1: launch_asm_step_pipe<1, true>(s, batch, sms, stream); return;
+      case 2: launch_asm_step_pipe<2, true>(s, batch, sms, stream); return;
+      case 3: launch_asm_step_pipe<3, true>(s, batch, sms, stream); return;
+      case 4: launch_asm_step_pipe<4, true>(s, batch, sms, stream); return;
+      case 5: launch_asm_step_pipe<5, true>(s, batch, sms, stream); return;
+      case 6: launch_asm_step_pipe<6, true>(s, batch, sms, stream); return;
+      case 7: launch_asm_step_pipe<7, true>(s, batch, sms, stream); return;
+      default: launch_asm_step_pipe<8, true>(s, batch, sms, stream); return;
+    }
+  }
+  const int groups = (s.T - 1 - s.j) * ((s.R + kAsmRows - 1) / kAsmRows);
+  const dim3 grid((groups + 7) / 8, batch);
+  switch (np) {
+    case 1: asm_step_kernel<1, kAsmRows, true><<<grid, 256, 0, stream>>>(s); break;
+    case 2: asm_step_kernel<2, kAsmRows, true><<<grid, 256, 0, stream>>>(s); break;
+    case 3: asm_step_kernel<3, kAsmRows, true><<<grid, 256, 0, stream>>>(s); break;
+    case 4: asm_step_kernel<4, kAsmRows, true><<<grid, 256, 0, stream>>>(s); break;
+    case 5: asm_step_kernel<5, kAsmRows, true><<<grid, 256, 0, stream>>>(s); break;
+    case 6: asm_step_kernel<6, kAsmRows, true><<<grid, 256, 0, stream>>>(s); break;
+    case 7: asm_step_kernel<7, kAsmRows, true><<<grid, 256, 0, stream>>>(s); break;
+    default: asm_step_kernel<8, kAsmRows, true><<<grid, 256, 0, stream>>>(s); break;
+  }
+}
+
+// Gain-defined controllers: Atil = A + B K, Abar = A + Lt C and both gains transposed, Btt[b,t,q,:] = B[b,t,:,q],
+// Ltt[b,t,q,:] = Lt[b,t,:,q], in one pass over A.  Warp per row; grid (batch T, ceil(n / 32)).
+__global__ void __launch_bounds__(256) asm_prep_gains_kernel(const float* __restrict__ A, const float* __restrict__ B,
+                                                             const float* __restrict__ Kfb, const float* __restrict__ Lt,
+                                                             const float* __restrict__ C, float* __restrict__ Atil,
+                                                             float* __restrict__ Abar, float* __restrict__ Btt,
+                                                             float* __restrict__ Ltt, int n, int m, int p) {
+  const size_t bt = blockIdx.x;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int n4 = n >> 2;
+  const float4* K4 = reinterpret_cast<const float4*>(Kfb + bt * m * n);
+  const float4* C4 = reinterpret_cast<const float4*>(C + bt * p * n);
+  for (int i = blockIdx.y * 32 + warp; i < min(n, static_cast<int>(blockIdx.y) * 32 + 32); i += 8) {
+    const float4* Ar = reinterpret_cast<const float4*>(A + (bt * n + i) * n);
+    const float* Bi = B + (bt * n + i) * m;
+    const float* Li = Lt + (bt * n + i) * p;
+    if (lane < m) Btt[(bt * m + lane) * n + i] = __ldg(Bi + lane);
+    if (lane < p) Ltt[(bt * p + lane) * n + i] = __ldg(Li + lane);
+    float4* o1 = reinterpret_cast<float4*>(Atil + (bt * n + i) * n);
+    float4* o2 = reinterpret_cast<float4*>(Abar + (bt * n + i) * n);
+    for (int c = lane; c < n4; c += 32) {
+      const float4 a = __ldg(Ar + c);
+      float4 bk = a, lc = a;
+      for (int q = 0; q < m; ++q) {
+        const float sc = __ldg(Bi + q);
+        const float4 k4 = __ldg(K4 + static_cast<size_t>(q) * n4 + c);
+        bk.x = fmaf(sc, k4.x, bk.x); bk.y = fmaf(sc, k4.y, bk.y); bk.z = fmaf(sc, k4.z, bk.z); bk.w = fmaf(sc, k4.w, bk.w);
+      }
+      for (int q = 0; q < p; ++q) {
+        const float sc = __ldg(Li + q);
+        const float4 c4 = __ldg(C4 + static_cast<size_t>(q) * n4 + c);
+        lc.x = fmaf(sc, c4.x, lc.x); lc.y = fmaf(sc, c4.y, lc.y); lc.z = fmaf(sc, c4.z, lc.z); lc.w = fmaf(sc, c4.w, lc.w);
+      }
+      o1[c] = bk;
+      o2[c] = lc;
+    }
+  }
+}
+
 size_t carve(size_t floats) { return align_up(floats * sizeof(float), 256); }
 
 }  // namespace
+
+// ------------------------------------------------------------------------------------------------------------------
+// ltv_scan_output_feedback_response, COLUMN route (gain-defined controller u = Kfb xhat; n >= 96, m, p <= 8): eq.(15) by the
+// backward column recursion above, carried on the DIFFERENCE D = Phi^xw - Phibar^x.  With Atil = A + B Kfb (Phibar^x(k,j) =
+// Phibar^x(k,j+1) Atil_j) the recursion of Phi^xw turns into
+//     D(k,j) = D(k,j+1) Abar_j - [Phibar^x(k,j+1) B_j] Kfb_j,    D(k,k) = 0,    Phibar^x(j+1,j+1) = I,
+//     Phi^xw(k,j) = Phibar^x(k,j) + D(k,j),    Phi^xe(k,j) = D(k,j) Lt_{j-1}
+// (D = the cross block G12 of the augmented closed loop): no subtraction of nearly equal operators - for small gains
+// D << Phi^xw and (Phi^xw - Phibar^x) Lt computed in fp32 loses the digits the cross-scan route keeps (measured 7e-4 at C2-size
+// items) - and D only ever needs TWO column buffers (the column being read and the one being written: 2 (T-1) n^2 floats per
+// item instead of a third T(T-1)/2 n^2 array).  Work: one scan (Phibar^x, into the workspace) + one n^3 product per block.
+size_t ofb_columns_workspace_bytes(int batch, int T, int n) {
+  const size_t b = batch, t = T, nn = n, P = t * (t - 1) / 2;
+  return 2 * carve(b * t * nn * nn) + 2 * carve(b * t * 8 * nn) + carve(b * P * nn * nn + 4) + 2 * carve(b * t * nn) +
+         align_up(phi_workspace_bytes(batch, T, n, n), 256) + 2 * carve(b * (t - 1) * nn * nn + 4);
+}
+
+bool ofb_columns_supported(int n, int m, int p) { return phi_uses_tensor_cores(n) && m >= 1 && m <= 8 && p >= 1 && p <= 8; }
+
+cudaError_t launch_ofb_response_columns(const OfbArgs& a, cudaStream_t stream, unsigned long long* launches) {
+  int dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int batch = a.batch, T = a.T, n = a.n, m = a.m, p = a.p;
+  const size_t b = batch, t = T, nn = n, P = t * (t - 1) / 2;
+  char* cur = static_cast<char*>(a.workspace);
+  float* Atil = reinterpret_cast<float*>(cur); cur += carve(b * t * nn * nn);
+  float* Abar = reinterpret_cast<float*>(cur); cur += carve(b * t * nn * nn);
+  float* Btt = reinterpret_cast<float*>(cur); cur += carve(b * t * 8 * nn);
+  float* Ltt = reinterpret_cast<float*>(cur); cur += carve(b * t * 8 * nn);
+  float* pbar = reinterpret_cast<float*>(cur); cur += carve(b * P * nn * nn + 4);
+  float* wz = reinterpret_cast<float*>(cur); cur += carve(b * t * nn);
+  float* rz = reinterpret_cast<float*>(cur); cur += carve(b * t * nn);
+  float* part = reinterpret_cast<float*>(cur); cur += align_up(phi_workspace_bytes(batch, T, n, n), 256);
+  float* dbuf[2];
+  dbuf[0] = reinterpret_cast<float*>(cur); cur += carve(b * (t - 1) * nn * nn + 4);
+  dbuf[1] = reinterpret_cast<float*>(cur);
+  cudaError_t e;
+  if ((e = cudaMemsetAsync(wz, 0, b * t * nn * sizeof(float), stream)) != cudaSuccess) return e;   // the scan's own tube is not used
+  if ((e = cudaMemsetAsync(a.tau, 0, b * t * nn * sizeof(float), stream)) != cudaSuccess) return e;
+  {
+    ProfScope prof(kProfOfbSupport, stream);
+    asm_prep_gains_kernel<<<dim3(batch * T, (n + 31) / 32), 256, 0, stream>>>(a.A, a.B, a.Kfb, a.Lt, a.C, Atil, Abar, Btt, Ltt, n, m, p);
+  }
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  ++*launches;
+  if (T < 2) return cudaSuccess;
+  PhiArgs pb{Atil, wz, pbar, rz, part, batch, T, n, n, 0};
+  if ((e = launch_phi_tube(pb, stream, launches)) != cudaSuccess) return e;
+  // step j: [D blocks (k, j+1), k = j+2 .. T-1: the first T-2-j blocks of the buffer of column j+1] x Abar_j -> blocks 1 .. of
+  // the buffer of column j; buffers alternate with the parity of the column
+  const int nch = phi_pick_nch(n);
+  const int rows_item = (T - 1) * n;
+  BatchedGemm g[2];
+  alignas(64) unsigned char maps[2][1024];
+  for (int q = 0; q < 2; ++q) {   // q = parity of the column being WRITTEN
+    g[q] = BatchedGemm{};
+    g[q].L = dbuf[q ^ 1]; g[q].l_rows = static_cast<long long>(b) * rows_item; g[q].l_row_stride = rows_item; g[q].l_row0 = 0;
+    g[q].R = Abar; g[q].r_blocks = batch * T; g[q].r_blk_stride = T;
+    g[q].D = dbuf[q]; g[q].d_blocks = 1; g[q].d_blk0 = 0; g[q].d_blk_stride = 0;
+    g[q].d_rows = static_cast<int>(b * rows_item); g[q].d_row_stride = rows_item; g[q].d_row0 = n;
+    g[q].count = batch; g[q].N = n; g[q].K = n; g[q].M = n;
+    if (phi_tc_maps_size() > sizeof(maps[q])) return cudaErrorInvalidValue;
+    if ((e = bgemm_tc_make_maps(g[q], maps[q])) != cudaSuccess) return e;
+  }
+  for (int j = T - 2; j >= 0; --j) {
+    const int q = j & 1;
+    const int mrows = (T - 2 - j) * n;
+    if (mrows > 0) {
+      g[q].M = mrows;
+      g[q].r_blk0 = j;
+      if ((e = launch_bgemm_tc(g[q], nch, maps[q], sms, stream)) != cudaSuccess) return e;
+      ++*launches;
+    }
+    AsmStep s{};
+    s.out = a.phi_xw; s.oute = a.phi_xe; s.pbar = pbar; s.A = a.A; s.w = a.w; s.f = a.f; s.tau = a.tau;
+    s.Gt = Btt; s.Cm = a.Kfb; s.Lte = Ltt; s.dcol = dbuf[q]; s.pc = m;
+    s.T = T; s.n = n; s.p = p; s.R = n; s.is_u = 0; s.j = j;
+    {
+      ProfScope prof(kProfOfbSupport, stream);
+      launch_asm_step_diff(s, batch, sms, stream);
+    }
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    ++*launches;
+  }
+  return cudaSuccess;
+}
 
 size_t asm_workspace_bytes(int batch, int T, int n, int p) {
   const size_t b = batch, t = T;

@@ -91,8 +91,12 @@ struct OfbArgs {
   int batch, T, n, m, p;
   void* workspace;
 };
-size_t ofb_workspace_bytes(int batch, int T, int n);
+size_t ofb_workspace_bytes(int batch, int T, int n, int m, int p);   // m = p = 0: sizes of the gains unknown
 cudaError_t launch_output_feedback(const OfbArgs& a, cudaStream_t stream, unsigned long long* launches);
+// column route of the same call (assemble.cu): one scan + the backward column recursion on D = Phi^xw - Phibar^x
+size_t ofb_columns_workspace_bytes(int batch, int T, int n);
+bool ofb_columns_supported(int n, int m, int p);
+cudaError_t launch_ofb_response_columns(const OfbArgs& a, cudaStream_t stream, unsigned long long* launches);
 
 // Input-side responses of eq.(15) and closed-loop margins of eq.(12d) (output_feedback.cu)
 struct OfbConArgs {

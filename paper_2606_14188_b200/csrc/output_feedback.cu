@@ -17,6 +17,9 @@
 // The low-rank form for a general Phibar is the next step (NEXT-4).
 #include <cuda.h>
 
+#include <algorithm>
+
+#include "../../include/ltv_scan.h"
 #include "ltv_internal.h"
 #include "phi_geom.cuh"
 #include "phi_kernels.h"
@@ -291,10 +294,29 @@ __global__ void __launch_bounds__(256) cls_post_kernel(const float* __restrict__
 
 static bool ofb_structured(int n) { return phi_uses_tensor_cores(n) && env_int("OFB_AUGMENTED", 0) == 0; }
 
-size_t ofb_workspace_bytes(int batch, int T, int n) {
+// Route of the structured path (n >= 96), LTV_OPT_OUTPUT_FEEDBACK_ROUTE: 1 = CROSS SCAN (two n-state scans + the cross scan with
+// the two-source K loop: 4 n^3 products per block, log depth), 2 = COLUMN RECURSION (assemble.cu: one scan for Phibar^x, then
+// the backward recursion over the columns on D = Phi^xw - Phibar^x: 2 n^3 products per block, half the passes over the
+// blocks, but a chain of 2 (T - 1) launches; needs m, p <= 8), 0 = by size: the column recursion wins once the GEMM of a
+// middle step is worth about four waves of tiles (C2 batch 64: 1.33x, one n = 1200 or 2400 item: 1.75x; C2 batch 4: 0.95x).
+static int ofb_route(int batch, int T, int n, int m, int p) {
+  if (!ofb_columns_supported(n, m, p)) return 1;
+  const int forced = option(LTV_OPT_OUTPUT_FEEDBACK_ROUTE);
+  if (forced == 1 || forced == 2) return forced;
+  const long long rows = static_cast<long long>(batch) * (T / 2) * n;   // column T/2 holds T/2 blocks per item
+  const long long tiles = (rows / 128) * ((n + 159) / 160);
+  return tiles >= 4 * 148 ? 2 : 1;
+}
+
+// m = p = 0: the gains' sizes are not known to the caller of ltv_scan_workspace_bytes - room for either route
+size_t ofb_workspace_bytes(int batch, int T, int n, int m, int p) {
   const size_t b = batch, t = T, nn = n, n2 = 2 * nn, P = t * (t - 1) / 2;
-  if (ofb_structured(n))   // Atil, Abar; Phihat, G (Phibar lives in phi_xw_out); zero w, scratch r; tube partials of a scan
-    return carve(b * t * 32 * nn) + 2 * carve(b * t * nn * nn) + 2 * carve(b * P * nn * nn + 4) + 2 * carve(b * t * nn) + phi_workspace_bytes(batch, T, n, n);
+  if (ofb_structured(n)) {
+    // Atil, Abar; Phihat, G (Phibar lives in phi_xw_out); zero w, scratch r; tube partials of a scan
+    const size_t cross = carve(b * t * 32 * nn) + 2 * carve(b * t * nn * nn) + 2 * carve(b * P * nn * nn + 4) + 2 * carve(b * t * nn) + phi_workspace_bytes(batch, T, n, n);
+    if (m < 1 || p < 1) return std::max(cross, ofb_columns_workspace_bytes(batch, T, n));
+    return ofb_route(batch, T, n, m, p) == 2 ? ofb_columns_workspace_bytes(batch, T, n) : cross;
+  }
   return carve(b * t * 32 * nn) + carve(b * t * n2 * n2) + carve(b * P * n2 * n2 + 4) + 2 * carve(b * t * n2) + phi_workspace_bytes(batch, T, 2 * n, 2 * n);
 }
 
@@ -316,6 +338,7 @@ cudaError_t launch_output_feedback(const OfbArgs& a, cudaStream_t stream, unsign
   char* cur = static_cast<char*>(a.workspace);
   const dim3 xgrid((n + 7) / 8, T, batch);
   cudaError_t e;
+  if (ofb_structured(n) && ofb_route(batch, T, n, a.m, a.p) == 2) return launch_ofb_response_columns(a, stream, launches);
   float* Ltt = reinterpret_cast<float*>(cur); cur += carve(b * t * 32 * nn);   // [b,T,p,n] (sized for p = 32)
   if (ofb_structured(n)) {
     int dev = 0, sms = 148;

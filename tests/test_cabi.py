@@ -119,8 +119,19 @@ def test_host_side_validation_needs_no_gpu(L):
     assert o(p, p, p, p, p, p, p, p, None, p, 1, 2, 4, 2, 40, 0, p, 1 << 24, None) == 3     # p > 32
     assert o(p, p, p, p, p, p, p, p, None, p, 1, 2, 4100, 2, 2, 0, p, 1 << 24, None) == 3   # 2n beyond the scan's limit
     assert o(p, p, p, p, p, p, p, p, None, p, 1, 2, 4, 2, 2, 0, p, 8, None) == 5            # workspace too small
-    need = L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, b, T, n, 0)
-    assert need >= 2 * b * (T * (T - 1) // 2) * n * n * 4     # n >= 96: Phihat^x and the cross block (Phibar^x sits in the output)
+    blk = b * (T * (T - 1) // 2) * n * n * 4
+    try:
+        L.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, 1)
+        need = L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, b, T, n, 0)
+        assert need >= 2 * blk                                 # cross scan: Phihat^x and the cross block (Phibar^x sits in the output)
+        L.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, 2)
+        assert L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, b, T, n, 0) >= need   # gains' sizes unknown: room for either route
+        assert L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, b, T, n, 9) == need   # m or p > 8: cross scan only
+        need = L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, b, T, n, 6)
+        assert blk <= need < 2 * blk                           # column recursion: Phibar^x + two column buffers of D
+    finally:
+        L.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, 0)
+    assert L.lib.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, 3) == 2
     need48 = L.ltv_scan_workspace_bytes(L.LTV_OP_OUTPUT_FEEDBACK, b, T, 48, 0)
     assert need48 >= 4 * b * (T * (T - 1) // 2) * 48 * 48 * 4  # n < 96: Phi of the 2n-state augmented system
     oc = L.lib.ltv_scan_output_feedback_constraints

@@ -111,9 +111,22 @@ def _oracle_ofb(A, B, C, K, Lt, w, f):
                                            (132, 5, 6, 6, 2),     # ragged tiles
                                            (100, 4, 1, 1, 1),     # single input, single output
                                            (64, 3, 4, 20, 1)])    # wide observation (three groups of 8)
-def test_output_feedback_response_call(L, n, T, m, p, batch):
-    """ltv_scan_output_feedback_response (augmented Jacobians, Phi scan on 2n states, extraction + tube, all on the
-    device) against eq.(15) and (12e) evaluated by the oracle."""
+@pytest.mark.parametrize("route", [1, 2])                         # n >= 96: cross scan / column recursion (LTV_OPT_OUTPUT_FEEDBACK_ROUTE)
+def test_output_feedback_response_call(L, n, T, m, p, batch, route):
+    """ltv_scan_output_feedback_response (n < 96: augmented Jacobians, Phi scan on 2n states, extraction + tube; n >= 96: both
+    structured routes; all on the device) against eq.(15) and (12e) evaluated by the oracle."""
+    import torch
+
+    if n < 96 and route == 2:
+        pytest.skip("one route below n = 96")
+    L.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, route)
+    try:
+        _response_call_case(L, n, T, m, p, batch)
+    finally:
+        L.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, 0)
+
+
+def _response_call_case(L, n, T, m, p, batch):
     import torch
 
     items = [_gains(T, n, m, p, seed=7 * n + T + b) for b in range(batch)]

@@ -259,7 +259,16 @@ def _dense_lower(blocks, T, n, cols=None):
     return D
 
 
-def test_full_size_output_feedback_response_vs_oracle(L):
+@pytest.mark.parametrize("route", [0, 1, 2])     # default (column recursion at this size), cross scan, column recursion
+def test_full_size_output_feedback_response_vs_oracle(L, route):
+    L.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, route)
+    try:
+        _full_size_output_feedback_response_vs_oracle(L)
+    finally:
+        L.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, 0)
+
+
+def _full_size_output_feedback_response_vs_oracle(L):
     """ltv_scan_output_feedback_response on C2-size items (n=300, m=6, p=6, whole batch of 64, structured tcgen05 path)
     at a horizon the oracle's dense block operators can hold (T=8: [2400 x 2400] operators): every block of Phi^xw,
     Phi^xe and the whole tube of a sampled item against oracle/ - eq.(15) as printed (O.assemble_output_feedback) on
