@@ -66,7 +66,7 @@ enum { LTV_OP_ROLLOUT = 0, LTV_OP_SYSTEM_RESPONSE_TUBE = 1, LTV_OP_ADJOINT = 2, 
        LTV_OP_OBSERVER_RESPONSE = 5 /* ltv_scan_observer_response; pass p (rows of C) as `m` */,
        LTV_OP_KALMAN_GAINS = 6 /* ltv_scan_kalman_gains; pass p (rows of C) as `m` */,
        LTV_OP_CONSTRAINT_TIGHTENING = 7 /* ltv_scan_constraint_tightening; pass nc (constraint rows) as `m` */,
-       LTV_OP_OUTPUT_FEEDBACK = 8 /* ltv_scan_output_feedback_response; `m` is ignored */,
+       LTV_OP_OUTPUT_FEEDBACK = 8 /* ltv_scan_output_feedback_response; `m` = max(m, p) of the call, or 0 = unknown */,
        LTV_OP_SYSTEM_RESPONSE_TUBE_RELAYOUT = 9 /* ltv_scan_system_response_tube with LTV_PHI_ROW_PACKED / _SQUARE_GRID */ };
 
 /* `phi_layout` argument: where block (t,s), 0 <= s < t <= T-1, of one item sits in phi_out.  Blocks are contiguous
@@ -318,11 +318,22 @@ LTV_API int ltv_scan_kalman_gains(const float* A, const float* C, const float* e
  *   flags     must be 0
  * Method: the closed loop in (x, x - xhat) is the LTV system A_aug = [[A + B Kfb, -B Kfb], [0, A + Lt C]], and with
  * G = Phi_aug(k,j): Phi^xw = G11 + G12, Phi^xe = G12 Lt_{j-1}.  G is block upper triangular (G11 = Phibar^x,
- * G22 = Phihat^x) and G12(t,s) = G11(t,mid) G12(mid,s) + G12(t,mid) G22(mid,s), so for n >= 96 the library runs two
- * n-state time-parallel scans and one cross scan whose combine accumulates both products in one tcgen05 K loop (4
- * instead of 8 n^3 products per block); for n < 96 it runs the plain scan on the 2n x 2n Jacobians.  One last pass forms
- * Phi^xw (in place over Phibar^x), Phi^xe and the tube (deterministic).  The input-side operators Phi^uw, Phi^ue of (15)
- * come from ltv_scan_output_feedback_constraints (below).  n <= 4096.  Workspace: ltv_scan_workspace_bytes(LTV_OP_OUTPUT_FEEDBACK, batch, T, n, 0). */
+ * G22 = Phihat^x).  For n < 96 the library runs the plain scan on the 2n x 2n Jacobians and one extraction pass.  For
+ * n >= 96 one of two routes (LTV_OPT_OUTPUT_FEEDBACK_ROUTE; default: chosen by size):
+ *   cross scan   G12(t,s) = G11(t,mid) G12(mid,s) + G12(t,mid) G22(mid,s): two n-state time-parallel scans and one cross scan
+ *                whose combine accumulates both products in one tcgen05 K loop (4 n^3 products per block, log depth), then one
+ *                pass that forms Phi^xw (in place over Phibar^x), Phi^xe and the tube;
+ *   columns      (m, p <= 8) one scan for Phibar^x, then the backward recursion over the columns of
+ *                ltv_scan_output_feedback_assemble carried on the difference D = G12 = Phi^xw - Phibar^x,
+ *                    D(k,j) = D(k,j+1) Abar_j - [Phibar^x(k,j+1) B_j] Kfb_j,   D(k,k) = 0,   Abar_j = A_j + Lt_j C_j,
+ *                    Phi^xw = Phibar^x + D,   Phi^xe(k,j) = D(k,j) Lt_{j-1}
+ *                (2 n^3 products per block, T-1 sequential steps of one batched GEMM + one fused row kernel; no difference of
+ *                nearly equal operators is formed, so small gains lose no digits; D lives in two column buffers).  C2 (batch
+ *                64): 26 ms against 38 ms for the cross scan, workspace 14.5 against 24.5 GB; single large items 1.65x;
+ *                small problems (a GEMM step below ~4 waves of tiles) stay on the log-depth route.
+ * Both are deterministic.  The input-side operators Phi^uw, Phi^ue of (15) come from ltv_scan_output_feedback_constraints
+ * (below).  n <= 4096.  Workspace: ltv_scan_workspace_bytes(LTV_OP_OUTPUT_FEEDBACK, batch, T, n, max(m, p)) - the last
+ * argument may be 0 ("not known yet": room for either route); it must be asked AFTER LTV_OPT_OUTPUT_FEEDBACK_ROUTE is set. */
 LTV_API int ltv_scan_output_feedback_response(const float* A, const float* B, const float* Kfb, const float* Lt,
                                               const float* C, const float* w, const float* f, float* phi_xw_out,
                                               float* phi_xe_out, float* tau_out, int batch, int T, int n, int m, int p,

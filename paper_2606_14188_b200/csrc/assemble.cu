@@ -490,9 +490,194 @@ void launch_asm_step(const AsmStep& s, int batch, int sms, cudaStream_t stream) 
   }
 }
 
+// Difference mode, second form: TWO rows per warp and the gain products stashed one step ahead.
+// ncu on the one-row pipeline: 38 % of the HBM copy peak at 56 % issue-slot use - ~1060 warp instructions per 1.2 KB row, most of
+// them the 3 NP shared-memory vector loads per column quad and the 5-step butterflies of 2 NP + 1 sums.  Here
+//   * a warp reduces rows i, i+1 of a block together: every staged vector is loaded once for both rows, and the butterflies
+//     start with an exchange between the two rows (lanes 0-15 end with row i's sums, lanes 16-31 with row i+1's): half the shuffles;
+//   * the skinny product S(k,j+1)[i] = Phibar^x(k,j+1)[i] B_j that the correction of step j needs is formed at step j+1, when the
+//     row of Phibar^x(k,j+1) is in shared memory anyway (for Phi^xw = D + Phibar^x), and stashed in sbuf[b,k,i,0..7]: the row of
+//     Phibar^x(k,j+1) is not read a second time (4 instead of 5 row passes per step, two rows instead of three in the ring).
+// Shared memory: K_j, B_{j-1}^T, Lt_{j-1}^T, w_j + per warp 2 stages x (2 rows of D + 2 rows of Phibar^x + 16 floats of S).
+template <int NP>
+__global__ void __launch_bounds__(256) asm_diff2_kernel(const AsmStep s, float* __restrict__ sbuf) {
+  extern __shared__ float4 asm_sm[];
+  const int T = s.T, n = s.n, j = s.j;
+  const int pe = s.p, pcr = s.pc;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int half = lane >> 4;   // which row of the pair this lane ends up owning
+  const int b = blockIdx.y;
+  const int n4 = n >> 2;
+  const int ptot = (T - 1 - j) * (n >> 1);   // row pairs of this column (n is even)
+  const size_t P = static_cast<size_t>(T) * (T - 1) / 2;
+  const size_t bT = static_cast<size_t>(b) * T;
+  const bool has_e = j >= 1;
+  float4* vK = asm_sm;                  // [NP][n4] Kfb_j          (zeros beyond pc)
+  float4* vB = vK + NP * n4;            // [NP][n4] B_{j-1}^T      (zeros beyond pc; j >= 1)
+  float4* vLm = vB + NP * n4;           // [NP][n4] Lt_{j-1}^T     (zeros beyond p;  j >= 1)
+  float4* vw = vLm + NP * n4;           // [n4]     w_j
+  const int stage_f4 = 4 * n4 + 4;      // 2 rows of D, 2 rows of Phibar^x, 2 x 8 floats of S
+  float4* ring = vw + n4 + static_cast<size_t>(warp) * 2 * stage_f4;
+  {
+    const float4* Kj = reinterpret_cast<const float4*>(s.Cm + (bT + j) * pcr * n);
+    const float4* wj = reinterpret_cast<const float4*>(s.w + (bT + j) * n);
+    const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int e = threadIdx.x; e < NP * n4; e += 256) {
+      vK[e] = e < pcr * n4 ? __ldg(Kj + e) : z4;
+      if (has_e) {
+        vB[e] = e < pcr * n4 ? __ldg(reinterpret_cast<const float4*>(s.Gt + (bT + j - 1) * pcr * n) + e) : z4;
+        vLm[e] = e < pe * n4 ? __ldg(reinterpret_cast<const float4*>(s.Lte + (bT + j - 1) * pe * n) + e) : z4;
+      }
+    }
+    for (int e = threadIdx.x; e < n4; e += 256) vw[e] = __ldg(wj + e);
+  }
+  __syncthreads();
+  const size_t item_x = static_cast<size_t>(b) * P;
+  const float* Btj = s.Gt + (bT + j) * pcr * n;   // B_j^T: the gain rows of the blocks (j+1, j)
+  auto prefetch = [&](int pr, int stage) {
+    if (pr < ptot) {
+      const int row = pr * 2, kk = row / n, i = row - kk * n, k = j + 1 + kk;
+      float4* dst = ring + static_cast<size_t>(stage) * stage_f4;
+      const float4* bs = reinterpret_cast<const float4*>(s.dcol + ((static_cast<size_t>(b) * (T - 1) + kk) * n + i) * n);
+      const float4* cu = reinterpret_cast<const float4*>(s.pbar + ((item_x + phi_colbase(T, j) + kk) * n + i) * n);
+      for (int c = lane; c < 2 * n4; c += 32) {   // rows i and i+1 are contiguous in both arrays
+        if (kk > 0) cp_async16(dst + c, bs + c);
+        cp_async16(dst + 2 * n4 + c, cu + c);
+      }
+      float* su = reinterpret_cast<float*>(dst + 4 * n4);   // [2][8]
+      if (kk > 0) {
+        if (lane < 4) cp_async16(dst + 4 * n4 + lane, reinterpret_cast<const float4*>(sbuf + ((bT + k) * n + i) * 8) + lane);
+      } else if (lane < 16) {
+        const int r = lane >> 3, q = lane & 7;
+        if (q < pcr) cp_async4(su + lane, Btj + static_cast<size_t>(q) * n + i + r); else su[lane] = 0.f;
+      }
+    }
+    cp_async_commit();
+  };
+  float fq[NP];
+#pragma unroll
+  for (int q = 0; q < NP; ++q) fq[q] = (has_e && q < pe) ? __ldg(s.f + (bT + j - 1) * pe + q) : 0.f;
+  const int stride = gridDim.x * 8;
+  int pr = blockIdx.x * 8 + warp;
+  prefetch(pr, 0);
+  for (int it = 0; pr < ptot; pr += stride, ++it) {
+    const int stage = it & 1;
+    prefetch(pr + stride, stage ^ 1);
+    cp_async_wait<1>();
+    __syncwarp();
+    const int row = pr * 2, kk = row / n, i = row - kk * n, k = j + 1 + kk;
+    const size_t oidx = (item_x + phi_colbase(T, j) + kk) * n + i;   // row i of block (k, j) in COLUMN_PACKED order
+    float* tau_p = s.tau + (bT + k) * n + i + half;
+    const float tau_old = (lane & 15) == 0 ? *tau_p : 0.f;
+    const float4* sD = ring + static_cast<size_t>(stage) * stage_f4;
+    const float4* sP = sD + 2 * n4;
+    const float* su = reinterpret_cast<const float*>(sD + 4 * n4);
+    float4* drow = reinterpret_cast<float4*>(s.dcol + ((static_cast<size_t>(b) * (T - 1) + kk) * n + i) * n);
+    float4* xrow = reinterpret_cast<float4*>(s.out + oidx * n);
+    float u0[NP], u1[NP], e0[NP], e1[NP], g0[NP], g1[NP];
+#pragma unroll
+    for (int q = 0; q < NP; ++q) { u0[q] = su[q]; u1[q] = su[8 + q]; e0[q] = e1[q] = g0[q] = g1[q] = 0.f; }
+    float t0 = 0.f, t1 = 0.f;
+    for (int c = lane; c < n4; c += 32) {
+      float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0;
+      if (kk > 0) { x0 = sD[c]; x1 = sD[n4 + c]; }
+#pragma unroll
+      for (int q = 0; q < NP; ++q) {
+        const float4 kq = vK[q * n4 + c];
+        x0.x = fmaf(-u0[q], kq.x, x0.x); x0.y = fmaf(-u0[q], kq.y, x0.y); x0.z = fmaf(-u0[q], kq.z, x0.z); x0.w = fmaf(-u0[q], kq.w, x0.w);
+        x1.x = fmaf(-u1[q], kq.x, x1.x); x1.y = fmaf(-u1[q], kq.y, x1.y); x1.z = fmaf(-u1[q], kq.z, x1.z); x1.w = fmaf(-u1[q], kq.w, x1.w);
+      }
+      const float4 p0 = sP[c], p1 = sP[n4 + c];
+      if (has_e) {   // column 0 of D feeds no further product
+        drow[c] = x0; drow[n4 + c] = x1;
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+          const float4 l = vLm[q * n4 + c];
+          e0[q] = fmaf(x0.x, l.x, fmaf(x0.y, l.y, fmaf(x0.z, l.z, fmaf(x0.w, l.w, e0[q]))));
+          e1[q] = fmaf(x1.x, l.x, fmaf(x1.y, l.y, fmaf(x1.z, l.z, fmaf(x1.w, l.w, e1[q]))));
+          const float4 bq = vB[q * n4 + c];
+          g0[q] = fmaf(p0.x, bq.x, fmaf(p0.y, bq.y, fmaf(p0.z, bq.z, fmaf(p0.w, bq.w, g0[q]))));
+          g1[q] = fmaf(p1.x, bq.x, fmaf(p1.y, bq.y, fmaf(p1.z, bq.z, fmaf(p1.w, bq.w, g1[q]))));
+        }
+      }
+      x0.x += p0.x; x0.y += p0.y; x0.z += p0.z; x0.w += p0.w;
+      x1.x += p1.x; x1.y += p1.y; x1.z += p1.z; x1.w += p1.w;
+      xrow[c] = x0; xrow[n4 + c] = x1;
+      const float4 ww = vw[c];
+      {
+        const float a0 = x0.x * ww.x, a1 = x0.y * ww.y, a2 = x0.z * ww.z, a3 = x0.w * ww.w;
+        t0 = fmaf(a0, a0, fmaf(a1, a1, fmaf(a2, a2, fmaf(a3, a3, t0))));
+        const float b0 = x1.x * ww.x, b1 = x1.y * ww.y, b2 = x1.z * ww.z, b3 = x1.w * ww.w;
+        t1 = fmaf(b0, b0, fmaf(b1, b1, fmaf(b2, b2, fmaf(b3, b3, t1))));
+      }
+    }
+    // pair reduction: lanes 0-15 keep row i's partial and take the partner's, lanes 16-31 the same for row i+1; then four
+    // butterfly steps inside each half
+    auto pair_sum = [&](float a0, float a1) {
+      float v = (half ? a1 : a0) + __shfl_xor_sync(0xffffffffu, half ? a0 : a1, 16);
+#pragma unroll
+      for (int o = 8; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+      return v;
+    };
+    const float s1 = pair_sum(t0, t1);
+    float s2 = 0.f;
+    if (has_e) {
+      float* er = s.oute != nullptr ? s.oute + (oidx + half) * pe : nullptr;
+      float* sn = sbuf + ((bT + k) * n + i + half) * 8;
+#pragma unroll
+      for (int q = 0; q < NP; ++q) {
+        const float eq = pair_sum(e0[q], e1[q]);
+        const float gq = pair_sum(g0[q], g1[q]);
+        const float t = eq * fq[q];
+        s2 = fmaf(t, t, s2);
+        if ((lane & 15) == q) {
+          if (er != nullptr && q < pe) er[q] = eq;
+          sn[q] = gq;   // S(k,j)[i] = Phibar^x(k,j)[i] B_{j-1}: the gain row of step j-1
+        }
+      }
+    } else if (s.oute != nullptr && (lane & 15) < pe) {
+      s.oute[(oidx + half) * pe + (lane & 15)] = 0.f;   // j = 0: no measurement noise has entered yet
+    }
+    if ((lane & 15) == 0) *tau_p = tau_old + (sqrtf(s1) + sqrtf(s2));
+    __syncwarp();
+  }
+  cp_async_wait<0>();
+}
+
+size_t asm_diff2_smem_bytes(int n, int np) { return (static_cast<size_t>(3) * np * n + n + static_cast<size_t>(8) * 2 * (4 * n + 16)) * sizeof(float); }
+
+template <int NP>
+cudaError_t launch_asm_diff2(const AsmStep& s, float* sbuf, int batch, int sms, cudaStream_t stream) {
+  const size_t smem = asm_diff2_smem_bytes(s.n, NP);
+  static size_t attr_set = 0;
+  if (smem > 48 * 1024 && smem > attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(asm_diff2_kernel<NP>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    if (e != cudaSuccess) return e;
+    attr_set = smem;
+  }
+  const int ptot = (s.T - 1 - s.j) * (s.n / 2);
+  const int per_sm = static_cast<int>(std::max<size_t>(1, std::min<size_t>(4, (200u * 1024u) / smem)));
+  int cx = (env_int("ASM_WAVES", kAsmWaves) * per_sm * sms + batch - 1) / batch;
+  cx = std::max(1, std::min(cx, (ptot + 7) / 8));
+  asm_diff2_kernel<NP><<<dim3(cx, batch), 256, smem, stream>>>(s, sbuf);
+  return cudaSuccess;
+}
+
 // difference mode: NP = max(pc, p) <= 8
-void launch_asm_step_diff(const AsmStep& s, int batch, int sms, cudaStream_t stream) {
+void launch_asm_step_diff(const AsmStep& s, float* sbuf, bool two_rows, int batch, int sms, cudaStream_t stream) {
   const int np = std::max(s.pc, s.p);
+  if (two_rows) {
+    switch (np) {
+      case 1: launch_asm_diff2<1>(s, sbuf, batch, sms, stream); return;
+      case 2: launch_asm_diff2<2>(s, sbuf, batch, sms, stream); return;
+      case 3: launch_asm_diff2<3>(s, sbuf, batch, sms, stream); return;
+      case 4: launch_asm_diff2<4>(s, sbuf, batch, sms, stream); return;
+      case 5: launch_asm_diff2<5>(s, sbuf, batch, sms, stream); return;
+      case 6: launch_asm_diff2<6>(s, sbuf, batch, sms, stream); return;
+      case 7: launch_asm_diff2<7>(s, sbuf, batch, sms, stream); return;
+      default: launch_asm_diff2<8>(s, sbuf, batch, sms, stream); return;
+    }
+  }
   if (asm_pipe_smem_bytes(s.n, np) <= 200u * 1024u) {
     switch (np) {
       case 1: launch_asm_step_pipe<1, true>(s, batch, sms, stream); return;
@@ -575,7 +760,7 @@ size_t carve(size_t floats) { return align_up(floats * sizeof(float), 256); }
 size_t ofb_columns_workspace_bytes(int batch, int T, int n) {
   const size_t b = batch, t = T, nn = n, P = t * (t - 1) / 2;
   return 2 * carve(b * t * nn * nn) + 2 * carve(b * t * 8 * nn) + carve(b * P * nn * nn + 4) + 2 * carve(b * t * nn) +
-         align_up(phi_workspace_bytes(batch, T, n, n), 256) + 2 * carve(b * (t - 1) * nn * nn + 4);
+         align_up(phi_workspace_bytes(batch, T, n, n), 256) + 2 * carve(b * (t - 1) * nn * nn + 4) + carve(b * t * nn * 8);
 }
 
 bool ofb_columns_supported(int n, int m, int p) { return phi_uses_tensor_cores(n) && m >= 1 && m <= 8 && p >= 1 && p <= 8; }
@@ -597,7 +782,10 @@ cudaError_t launch_ofb_response_columns(const OfbArgs& a, cudaStream_t stream, u
   float* part = reinterpret_cast<float*>(cur); cur += align_up(phi_workspace_bytes(batch, T, n, n), 256);
   float* dbuf[2];
   dbuf[0] = reinterpret_cast<float*>(cur); cur += carve(b * (t - 1) * nn * nn + 4);
-  dbuf[1] = reinterpret_cast<float*>(cur);
+  dbuf[1] = reinterpret_cast<float*>(cur); cur += carve(b * (t - 1) * nn * nn + 4);
+  float* sbuf = reinterpret_cast<float*>(cur);   // [b, T, n, 8] stashed gain rows S(k, .)[i] of the two-row kernel
+  // the two-row kernel while its buffers fit shared memory (every step of a call takes the same kernel: the stash links the steps)
+  const bool two_rows = env_int("ASM_DIFF2", 1) != 0 && asm_diff2_smem_bytes(n, std::max(m, p)) <= 200u * 1024u;
   cudaError_t e;
   if ((e = cudaMemsetAsync(wz, 0, b * t * nn * sizeof(float), stream)) != cudaSuccess) return e;   // the scan's own tube is not used
   if ((e = cudaMemsetAsync(a.tau, 0, b * t * nn * sizeof(float), stream)) != cudaSuccess) return e;
@@ -641,7 +829,7 @@ cudaError_t launch_ofb_response_columns(const OfbArgs& a, cudaStream_t stream, u
     s.T = T; s.n = n; s.p = p; s.R = n; s.is_u = 0; s.j = j;
     {
       ProfScope prof(kProfOfbSupport, stream);
-      launch_asm_step_diff(s, batch, sms, stream);
+      launch_asm_step_diff(s, sbuf, two_rows, batch, sms, stream);
     }
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     ++*launches;
