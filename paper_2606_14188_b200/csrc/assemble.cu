@@ -499,7 +499,11 @@ void launch_asm_step(const AsmStep& s, int batch, int sms, cudaStream_t stream) 
 //     row of Phibar^x(k,j+1) is in shared memory anyway (for Phi^xw = D + Phibar^x), and stashed in sbuf[b,k,i,0..7]: the row of
 //     Phibar^x(k,j+1) is not read a second time (4 instead of 5 row passes per step, two rows instead of three in the ring).
 // Shared memory: K_j, B_{j-1}^T, Lt_{j-1}^T, w_j + per warp 2 stages x (2 rows of D + 2 rows of Phibar^x + 16 floats of S).
-template <int NP>
+// GEN = true: the same pipeline for the x side of the GENERAL assembly (Phibar given as operators): the recursion runs on
+// Phi^xw itself (rows of column j in `out`: GEMM result, or A_j for k = j+1), correction vectors C_j, gain rows
+// S(k,j+1) = Phibar^x(k,j+1) Lt_j stashed the same way (Lt_{j-1}^T serves both e = (row - Phibar^x(k,j)) Lt_{j-1} and the stash),
+// three row passes per step (read GEMM result, read Phibar^x(k,j), write Phi^xw(k,j)).
+template <int NP, bool GEN>
 __global__ void __launch_bounds__(256) asm_diff2_kernel(const AsmStep s, float* __restrict__ sbuf) {
   extern __shared__ float4 asm_sm[];
   const int T = s.T, n = s.n, j = s.j;
@@ -525,7 +529,7 @@ __global__ void __launch_bounds__(256) asm_diff2_kernel(const AsmStep s, float* 
     for (int e = threadIdx.x; e < NP * n4; e += 256) {
       vK[e] = e < pcr * n4 ? __ldg(Kj + e) : z4;
       if (has_e) {
-        vB[e] = e < pcr * n4 ? __ldg(reinterpret_cast<const float4*>(s.Gt + (bT + j - 1) * pcr * n) + e) : z4;
+        if (!GEN) vB[e] = e < pcr * n4 ? __ldg(reinterpret_cast<const float4*>(s.Gt + (bT + j - 1) * pcr * n) + e) : z4;
         vLm[e] = e < pe * n4 ? __ldg(reinterpret_cast<const float4*>(s.Lte + (bT + j - 1) * pe * n) + e) : z4;
       }
     }
@@ -538,18 +542,20 @@ __global__ void __launch_bounds__(256) asm_diff2_kernel(const AsmStep s, float* 
     if (pr < ptot) {
       const int row = pr * 2, kk = row / n, i = row - kk * n, k = j + 1 + kk;
       float4* dst = ring + static_cast<size_t>(stage) * stage_f4;
-      const float4* bs = reinterpret_cast<const float4*>(s.dcol + ((static_cast<size_t>(b) * (T - 1) + kk) * n + i) * n);
-      const float4* cu = reinterpret_cast<const float4*>(s.pbar + ((item_x + phi_colbase(T, j) + kk) * n + i) * n);
-      for (int c = lane; c < 2 * n4; c += 32) {   // rows i and i+1 are contiguous in both arrays
-        if (kk > 0) cp_async16(dst + c, bs + c);
-        cp_async16(dst + 2 * n4 + c, cu + c);
+      const size_t orow = ((item_x + phi_colbase(T, j) + kk) * n + i) * n;   // row i of block (k, j), COLUMN_PACKED
+      const float4* bs = GEN ? reinterpret_cast<const float4*>(kk > 0 ? s.out + orow : s.A + ((bT + j) * n + i) * n)
+                             : reinterpret_cast<const float4*>(s.dcol + ((static_cast<size_t>(b) * (T - 1) + kk) * n + i) * n);
+      const float4* cu = reinterpret_cast<const float4*>(s.pbar + orow);
+      for (int c = lane; c < 2 * n4; c += 32) {   // rows i and i+1 are contiguous in every array
+        if (GEN || kk > 0) cp_async16(dst + c, bs + c);
+        if (!GEN || has_e) cp_async16(dst + 2 * n4 + c, cu + c);
       }
       float* su = reinterpret_cast<float*>(dst + 4 * n4);   // [2][8]
       if (kk > 0) {
         if (lane < 4) cp_async16(dst + 4 * n4 + lane, reinterpret_cast<const float4*>(sbuf + ((bT + k) * n + i) * 8) + lane);
       } else if (lane < 16) {
         const int r = lane >> 3, q = lane & 7;
-        if (q < pcr) cp_async4(su + lane, Btj + static_cast<size_t>(q) * n + i + r); else su[lane] = 0.f;
+        if (!GEN && q < pcr) cp_async4(su + lane, Btj + static_cast<size_t>(q) * n + i + r); else su[lane] = 0.f;
       }
     }
     cp_async_commit();
@@ -567,8 +573,8 @@ __global__ void __launch_bounds__(256) asm_diff2_kernel(const AsmStep s, float* 
     __syncwarp();
     const int row = pr * 2, kk = row / n, i = row - kk * n, k = j + 1 + kk;
     const size_t oidx = (item_x + phi_colbase(T, j) + kk) * n + i;   // row i of block (k, j) in COLUMN_PACKED order
-    float* tau_p = s.tau + (bT + k) * n + i + half;
-    const float tau_old = (lane & 15) == 0 ? *tau_p : 0.f;
+    float* tau_p = s.tau != nullptr ? s.tau + (bT + k) * n + i + half : nullptr;
+    const float tau_old = (tau_p != nullptr && (lane & 15) == 0) ? *tau_p : 0.f;
     const float4* sD = ring + static_cast<size_t>(stage) * stage_f4;
     const float4* sP = sD + 2 * n4;
     const float* su = reinterpret_cast<const float*>(sD + 4 * n4);
@@ -580,28 +586,46 @@ __global__ void __launch_bounds__(256) asm_diff2_kernel(const AsmStep s, float* 
     float t0 = 0.f, t1 = 0.f;
     for (int c = lane; c < n4; c += 32) {
       float4 x0 = make_float4(0.f, 0.f, 0.f, 0.f), x1 = x0;
-      if (kk > 0) { x0 = sD[c]; x1 = sD[n4 + c]; }
-#pragma unroll
-      for (int q = 0; q < NP; ++q) {
-        const float4 kq = vK[q * n4 + c];
-        x0.x = fmaf(-u0[q], kq.x, x0.x); x0.y = fmaf(-u0[q], kq.y, x0.y); x0.z = fmaf(-u0[q], kq.z, x0.z); x0.w = fmaf(-u0[q], kq.w, x0.w);
-        x1.x = fmaf(-u1[q], kq.x, x1.x); x1.y = fmaf(-u1[q], kq.y, x1.y); x1.z = fmaf(-u1[q], kq.z, x1.z); x1.w = fmaf(-u1[q], kq.w, x1.w);
-      }
-      const float4 p0 = sP[c], p1 = sP[n4 + c];
-      if (has_e) {   // column 0 of D feeds no further product
-        drow[c] = x0; drow[n4 + c] = x1;
+      if (GEN || kk > 0) { x0 = sD[c]; x1 = sD[n4 + c]; }
+      if (!GEN || kk > 0) {   // GEN, k = j+1: the row is A_j[i] as it stands
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
-          const float4 l = vLm[q * n4 + c];
-          e0[q] = fmaf(x0.x, l.x, fmaf(x0.y, l.y, fmaf(x0.z, l.z, fmaf(x0.w, l.w, e0[q]))));
-          e1[q] = fmaf(x1.x, l.x, fmaf(x1.y, l.y, fmaf(x1.z, l.z, fmaf(x1.w, l.w, e1[q]))));
-          const float4 bq = vB[q * n4 + c];
-          g0[q] = fmaf(p0.x, bq.x, fmaf(p0.y, bq.y, fmaf(p0.z, bq.z, fmaf(p0.w, bq.w, g0[q]))));
-          g1[q] = fmaf(p1.x, bq.x, fmaf(p1.y, bq.y, fmaf(p1.z, bq.z, fmaf(p1.w, bq.w, g1[q]))));
+          const float4 kq = vK[q * n4 + c];
+          x0.x = fmaf(-u0[q], kq.x, x0.x); x0.y = fmaf(-u0[q], kq.y, x0.y); x0.z = fmaf(-u0[q], kq.z, x0.z); x0.w = fmaf(-u0[q], kq.w, x0.w);
+          x1.x = fmaf(-u1[q], kq.x, x1.x); x1.y = fmaf(-u1[q], kq.y, x1.y); x1.z = fmaf(-u1[q], kq.z, x1.z); x1.w = fmaf(-u1[q], kq.w, x1.w);
         }
       }
-      x0.x += p0.x; x0.y += p0.y; x0.z += p0.z; x0.w += p0.w;
-      x1.x += p1.x; x1.y += p1.y; x1.z += p1.z; x1.w += p1.w;
+      if (GEN) {
+        if (has_e) {
+          const float4 p0 = sP[c], p1 = sP[n4 + c];
+          const float4 v0 = make_float4(x0.x - p0.x, x0.y - p0.y, x0.z - p0.z, x0.w - p0.w);
+          const float4 v1 = make_float4(x1.x - p1.x, x1.y - p1.y, x1.z - p1.z, x1.w - p1.w);
+#pragma unroll
+          for (int q = 0; q < NP; ++q) {
+            const float4 l = vLm[q * n4 + c];
+            e0[q] = fmaf(v0.x, l.x, fmaf(v0.y, l.y, fmaf(v0.z, l.z, fmaf(v0.w, l.w, e0[q]))));
+            e1[q] = fmaf(v1.x, l.x, fmaf(v1.y, l.y, fmaf(v1.z, l.z, fmaf(v1.w, l.w, e1[q]))));
+            g0[q] = fmaf(p0.x, l.x, fmaf(p0.y, l.y, fmaf(p0.z, l.z, fmaf(p0.w, l.w, g0[q]))));
+            g1[q] = fmaf(p1.x, l.x, fmaf(p1.y, l.y, fmaf(p1.z, l.z, fmaf(p1.w, l.w, g1[q]))));
+          }
+        }
+      } else {
+        const float4 p0 = sP[c], p1 = sP[n4 + c];
+        if (has_e) {   // column 0 of D feeds no further product
+          drow[c] = x0; drow[n4 + c] = x1;
+#pragma unroll
+          for (int q = 0; q < NP; ++q) {
+            const float4 l = vLm[q * n4 + c];
+            e0[q] = fmaf(x0.x, l.x, fmaf(x0.y, l.y, fmaf(x0.z, l.z, fmaf(x0.w, l.w, e0[q]))));
+            e1[q] = fmaf(x1.x, l.x, fmaf(x1.y, l.y, fmaf(x1.z, l.z, fmaf(x1.w, l.w, e1[q]))));
+            const float4 bq = vB[q * n4 + c];
+            g0[q] = fmaf(p0.x, bq.x, fmaf(p0.y, bq.y, fmaf(p0.z, bq.z, fmaf(p0.w, bq.w, g0[q]))));
+            g1[q] = fmaf(p1.x, bq.x, fmaf(p1.y, bq.y, fmaf(p1.z, bq.z, fmaf(p1.w, bq.w, g1[q]))));
+          }
+        }
+        x0.x += p0.x; x0.y += p0.y; x0.z += p0.z; x0.w += p0.w;
+        x1.x += p1.x; x1.y += p1.y; x1.z += p1.z; x1.w += p1.w;
+      }
       xrow[c] = x0; xrow[n4 + c] = x1;
       const float4 ww = vw[c];
       {
@@ -638,7 +662,7 @@ __global__ void __launch_bounds__(256) asm_diff2_kernel(const AsmStep s, float* 
     } else if (s.oute != nullptr && (lane & 15) < pe) {
       s.oute[(oidx + half) * pe + (lane & 15)] = 0.f;   // j = 0: no measurement noise has entered yet
     }
-    if ((lane & 15) == 0) *tau_p = tau_old + (sqrtf(s1) + sqrtf(s2));
+    if (tau_p != nullptr && (lane & 15) == 0) *tau_p = tau_old + (sqrtf(s1) + sqrtf(s2));
     __syncwarp();
   }
   cp_async_wait<0>();
@@ -646,12 +670,12 @@ __global__ void __launch_bounds__(256) asm_diff2_kernel(const AsmStep s, float* 
 
 size_t asm_diff2_smem_bytes(int n, int np) { return (static_cast<size_t>(3) * np * n + n + static_cast<size_t>(8) * 2 * (4 * n + 16)) * sizeof(float); }
 
-template <int NP>
+template <int NP, bool GEN = false>
 cudaError_t launch_asm_diff2(const AsmStep& s, float* sbuf, int batch, int sms, cudaStream_t stream) {
   const size_t smem = asm_diff2_smem_bytes(s.n, NP);
   static size_t attr_set = 0;
   if (smem > 48 * 1024 && smem > attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(asm_diff2_kernel<NP>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
+    cudaError_t e = cudaFuncSetAttribute(asm_diff2_kernel<NP, GEN>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     if (e != cudaSuccess) return e;
     attr_set = smem;
   }
@@ -659,7 +683,7 @@ cudaError_t launch_asm_diff2(const AsmStep& s, float* sbuf, int batch, int sms, 
   const int per_sm = static_cast<int>(std::max<size_t>(1, std::min<size_t>(4, (200u * 1024u) / smem)));
   int cx = (env_int("ASM_WAVES", kAsmWaves) * per_sm * sms + batch - 1) / batch;
   cx = std::max(1, std::min(cx, (ptot + 7) / 8));
-  asm_diff2_kernel<NP><<<dim3(cx, batch), 256, smem, stream>>>(s, sbuf);
+  asm_diff2_kernel<NP, GEN><<<dim3(cx, batch), 256, smem, stream>>>(s, sbuf);
   return cudaSuccess;
 }
 
@@ -839,7 +863,21 @@ cudaError_t launch_ofb_response_columns(const OfbArgs& a, cudaStream_t stream, u
 
 size_t asm_workspace_bytes(int batch, int T, int n, int p) {
   const size_t b = batch, t = T;
-  return carve(b * t * n * n) + carve(b * t * p * n);
+  return carve(b * t * n * n) + carve(b * t * p * n) + carve(b * t * n * 8);   // Abar, Lt^T, stashed gain rows of the two-row kernel
+}
+
+// x side of the general assembly through the two-row kernel (p <= 8, buffers fit shared memory)
+static void launch_asm_gen2(const AsmStep& s, float* sbuf, int batch, int sms, cudaStream_t stream) {
+  switch (s.p) {
+    case 1: launch_asm_diff2<1, true>(s, sbuf, batch, sms, stream); return;
+    case 2: launch_asm_diff2<2, true>(s, sbuf, batch, sms, stream); return;
+    case 3: launch_asm_diff2<3, true>(s, sbuf, batch, sms, stream); return;
+    case 4: launch_asm_diff2<4, true>(s, sbuf, batch, sms, stream); return;
+    case 5: launch_asm_diff2<5, true>(s, sbuf, batch, sms, stream); return;
+    case 6: launch_asm_diff2<6, true>(s, sbuf, batch, sms, stream); return;
+    case 7: launch_asm_diff2<7, true>(s, sbuf, batch, sms, stream); return;
+    default: launch_asm_diff2<8, true>(s, sbuf, batch, sms, stream); return;
+  }
 }
 
 cudaError_t launch_ofb_assemble(const AsmArgs& a, cudaStream_t stream, unsigned long long* launches) {
@@ -851,7 +889,9 @@ cudaError_t launch_ofb_assemble(const AsmArgs& a, cudaStream_t stream, unsigned 
   const int P = T * (T - 1) / 2;
   char* cur = static_cast<char*>(a.workspace);
   float* Abar = reinterpret_cast<float*>(cur); cur += carve(b * t * n * n);
-  float* Ltt = reinterpret_cast<float*>(cur);
+  float* Ltt = reinterpret_cast<float*>(cur); cur += carve(b * t * p * n);
+  float* sbuf = reinterpret_cast<float*>(cur);
+  const bool two_rows = p <= 8 && env_int("ASM_GEN2", 1) != 0 && asm_diff2_smem_bytes(n, p) <= 200u * 1024u;
   cudaError_t e;
   if (a.tau != nullptr && (e = cudaMemsetAsync(a.tau, 0, b * t * n * sizeof(float), stream)) != cudaSuccess) return e;
   {
@@ -904,9 +944,10 @@ cudaError_t launch_ofb_assemble(const AsmArgs& a, cudaStream_t stream, unsigned 
       s.out = sd ? a.phi_uw : a.phi_xw; s.oute = sd ? a.phi_ue : a.phi_xe; s.pbar = sd ? a.phibar_u : a.phibar_x;
       s.A = a.A; s.Ltt = Ltt; s.C = a.C; s.w = a.w; s.f = a.f; s.tau = sd ? nullptr : a.tau;
       s.T = T; s.n = n; s.p = p; s.R = R; s.is_u = sd; s.j = j;
+      s.Cm = a.C; s.Lte = Ltt; s.pc = p;
       {
         ProfScope prof(kProfOfbSupport, stream);
-        launch_asm_step(s, batch, sms, stream);
+        if (sd == 0 && two_rows) launch_asm_gen2(s, sbuf, batch, sms, stream); else launch_asm_step(s, batch, sms, stream);
       }
       if ((e = cudaGetLastError()) != cudaSuccess) return e;
       ++*launches;

@@ -57,6 +57,7 @@ def _pack(L, T, n, m, PbX, PbU):
                                            (100, 4, 1, 1, 1),     # single input, single output
                                            (64, 3, 4, 20, 1),     # wide observation
                                            (300, 6, 6, 6, 2),     # C2-size blocks: two n-tiles of 160, stacks across blocks
+                                           (640, 3, 2, 6, 1),     # one-row shared-memory pipeline on the x side (two-row buffers do not fit)
                                            (1200, 3, 2, 6, 1)])   # rows too long for the shared-memory pipeline: register kernel
 def test_general_assembly_against_the_oracle(L, n, T, m, p, batch):
     import torch

@@ -110,7 +110,11 @@ def _oracle_ofb(A, B, C, K, Lt, w, f):
                                            (48, 7, 3, 4, 1),      # 2n = 96: smallest tensor-core size
                                            (132, 5, 6, 6, 2),     # ragged tiles
                                            (100, 4, 1, 1, 1),     # single input, single output
-                                           (64, 3, 4, 20, 1)])    # wide observation (three groups of 8)
+                                           (64, 3, 4, 20, 1),     # wide observation (three groups of 8)
+                                           (300, 5, 3, 5, 2),     # column route: two-row kernel, m != p (zero-padded vectors)
+                                           (640, 4, 3, 5, 1),     # column route: one-row shared-memory pipeline in difference mode
+                                           (800, 3, 2, 2, 1),     # column route: register kernel in difference mode
+                                           (132, 4, 12, 3, 1)])   # m > 8: the column route is not available, both settings take the cross scan
 @pytest.mark.parametrize("route", [1, 2])                         # n >= 96: cross scan / column recursion (LTV_OPT_OUTPUT_FEEDBACK_ROUTE)
 def test_output_feedback_response_call(L, n, T, m, p, batch, route):
     """ltv_scan_output_feedback_response (n < 96: augmented Jacobians, Phi scan on 2n states, extraction + tube; n >= 96: both
