@@ -122,6 +122,23 @@ def test_row_shard_range_partitions_the_block_rows():
                 assert max(blocks) - T * (T - 1) / 2 / world <= T
 
 
+def test_row_shard_range_balanced_by_the_time_model():
+    """With the state dimension given the partition is balanced by modelled time, not block count: still contiguous, disjoint
+    and covering, the same on every rank, and its slowest shard is modelled no slower than the block-count partition's."""
+    from paper_2606_14188_b200.sharding import row_shard_cost, row_shard_range
+
+    for n, T in ((2400, 16), (1200, 32), (300, 32), (132, 9)):
+        for world in (2, 3, 8):
+            r = [row_shard_range(T, k, world, n=n) for k in range(world)]
+            assert r[0][0] == 1 and r[-1][1] == T
+            assert all(r[k][1] == r[k + 1][0] for k in range(world - 1)) and all(a <= b for a, b in r)
+            assert sum(sum(range(a, b)) for a, b in r) == T * (T - 1) // 2
+            old = [row_shard_range(T, k, world) for k in range(world)]
+            worst = lambda part: max(row_shard_cost(T, a, b, n) for a, b in part)
+            assert worst(r) <= worst(old) * (1 + 1e-9)
+    assert row_shard_range(16, 1, 2, n=48) == row_shard_range(16, 1, 2)      # below the tensor-core path: block count
+
+
 def _row_worker(rank, world, port, q):
     """One item split over the ranks by block rows: each rank computes ITS rows with the oracle's row recursion (what
     ltv_scan_system_response_tube_rows does on a GPU), the tube is assembled by the one all-reduce of the row-sharded path."""
