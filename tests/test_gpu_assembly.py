@@ -114,6 +114,8 @@ def _oracle_ofb(A, B, C, K, Lt, w, f):
                                            (300, 5, 3, 5, 2),     # column route: two-row kernel, m != p (zero-padded vectors)
                                            (640, 4, 3, 5, 1),     # column route: one-row shared-memory pipeline in difference mode
                                            (800, 3, 2, 2, 1),     # column route: register kernel in difference mode
+                                           (96, 2, 2, 2, 1),      # T = 2: a single block, no product in either route
+                                           (100, 3, 2, 3, 2),     # T = 3: one product step
                                            (132, 4, 12, 3, 1)])   # m > 8: the column route is not available, both settings take the cross scan
 @pytest.mark.parametrize("route", [1, 2])                         # n >= 96: cross scan / column recursion (LTV_OPT_OUTPUT_FEEDBACK_ROUTE)
 def test_output_feedback_response_call(L, n, T, m, p, batch, route):
@@ -243,3 +245,20 @@ def test_output_feedback_constraints_identity_rows_equal_the_tube_call(L):
                                                        want_inputs=False)
     torch.cuda.synchronize()
     assert O.rel_err(sig.cpu().numpy(), tau.cpu().numpy()) <= TOL
+
+
+@pytest.mark.parametrize("route", [1, 2])
+def test_output_feedback_response_single_step_horizon(L, route):
+    """T = 1: no block exists, tau_0 = 0, nothing is written to the (empty) operator arrays - on both routes."""
+    import torch
+
+    n, m, p, batch = 96, 2, 3, 2
+    A, B, C, K, Lt = [np.stack([q for q in x]) for x in zip(*[_gains(1, n, m, p, seed=5 + b) for b in range(batch)])]
+    w = np.ones((batch, 1, n), np.float32); f = np.ones((batch, 1, p), np.float32)
+    L.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, route)
+    try:
+        xw, xe, tau = L.ltv_scan_output_feedback_response(*[torch.from_numpy(a).cuda() for a in (A, B, K, Lt, C, w, f)])
+        torch.cuda.synchronize()
+    finally:
+        L.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, 0)
+    assert xw.shape[1] == 0 and bool(torch.all(tau == 0))
