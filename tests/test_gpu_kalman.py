@@ -64,9 +64,11 @@ def test_kalman_dense_random(L, n, T, batch, p, kind):
 
 
 @pytest.mark.parametrize("n,T,batch,p", [(4, 1, 2, 1), (4, 5, 1, 3), (8, 2, 3, 8), (12, 9, 2, 5), (40, 7, 70, 6),
-                                         (64, 4, 3, 32), (60, 3, 2, 17), (64, 33, 1, 1)])
+                                         (64, 4, 3, 32), (60, 3, 2, 17), (64, 33, 1, 1),
+                                         (68, 12, 2, 6),      # just above the single launch (the paper's 66 states padded to a multiple of 4): batched fp32-FMA path
+                                         (92, 5, 150, 8)])    # largest n below the tensor-core path, more items than SMs
 def test_kalman_small_single_launch_edges(L, n, T, batch, p):
-    """The single-launch recursion of small systems (csrc/kalman_small.cu, n <= 64: one CTA per item): smallest and largest n and
+    """The single-launch recursion of small systems (csrc/kalman_small.cu, n <= 64: one CTA per item; measured: beyond n = 72 a step of the one-CTA form - 27 us at n = 68, 49 us at n = 96 - is no faster than the five launches of the batched path, 29-38 us): smallest and largest n and
     p, a single step, more items than SMs would hold at once, odd p, a horizon longer than a warp."""
     W = dense_random(batch, T, n, 1, seed=11 * n + p + T, scale=0.4)
     M = observation_model(batch, T, n, p, seed=13 * n + p, kind="dense")
