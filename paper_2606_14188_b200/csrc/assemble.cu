@@ -442,11 +442,9 @@ constexpr int kAsmWaves = 8;
 template <int NP, bool DIFF = false>
 cudaError_t launch_asm_step_pipe(const AsmStep& s, int batch, int sms, cudaStream_t stream) {
   const size_t smem = asm_pipe_smem_bytes(s.n, NP);
-  static size_t attr_set = 0;   // largest dynamic shared-memory size the attribute was raised to (per instantiation)
-  if (smem > 48 * 1024 && smem > attr_set) {
+  if (smem > 48 * 1024) {   // every launch: the attribute belongs to the current device's copy of the function
     cudaError_t e = cudaFuncSetAttribute(asm_step_pipe_kernel<NP, DIFF>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     if (e != cudaSuccess) return e;
-    attr_set = smem;
   }
   const int rtot = (s.T - 1 - s.j) * s.R;
   const int per_sm = static_cast<int>(std::max<size_t>(1, std::min<size_t>(4, (200u * 1024u) / smem)));
@@ -456,22 +454,22 @@ cudaError_t launch_asm_step_pipe(const AsmStep& s, int batch, int sms, cudaStrea
   int cx = (env_int("ASM_WAVES", kAsmWaves) * per_sm * sms + batch - 1) / batch;
   cx = std::max(1, std::min(cx, (rtot + 7) / 8));
   asm_step_pipe_kernel<NP, DIFF><<<dim3(cx, batch), 256, smem, stream>>>(s);
-  return cudaSuccess;
+  return cudaGetLastError();
 }
 
 constexpr int kAsmRows = 2;
 
-void launch_asm_step(const AsmStep& s, int batch, int sms, cudaStream_t stream) {
+cudaError_t launch_asm_step(const AsmStep& s, int batch, int sms, cudaStream_t stream) {
   if (s.p <= 8 && asm_pipe_smem_bytes(s.n, s.p) <= 200u * 1024u) {
     switch (s.p) {
-      case 1: launch_asm_step_pipe<1>(s, batch, sms, stream); return;
-      case 2: launch_asm_step_pipe<2>(s, batch, sms, stream); return;
-      case 3: launch_asm_step_pipe<3>(s, batch, sms, stream); return;
-      case 4: launch_asm_step_pipe<4>(s, batch, sms, stream); return;
-      case 5: launch_asm_step_pipe<5>(s, batch, sms, stream); return;
-      case 6: launch_asm_step_pipe<6>(s, batch, sms, stream); return;
-      case 7: launch_asm_step_pipe<7>(s, batch, sms, stream); return;
-      default: launch_asm_step_pipe<8>(s, batch, sms, stream); return;
+      case 1: return launch_asm_step_pipe<1>(s, batch, sms, stream);
+      case 2: return launch_asm_step_pipe<2>(s, batch, sms, stream);
+      case 3: return launch_asm_step_pipe<3>(s, batch, sms, stream);
+      case 4: return launch_asm_step_pipe<4>(s, batch, sms, stream);
+      case 5: return launch_asm_step_pipe<5>(s, batch, sms, stream);
+      case 6: return launch_asm_step_pipe<6>(s, batch, sms, stream);
+      case 7: return launch_asm_step_pipe<7>(s, batch, sms, stream);
+      default: return launch_asm_step_pipe<8>(s, batch, sms, stream);
     }
   }
   const int rows = s.p <= 8 ? kAsmRows : 1;
@@ -488,6 +486,7 @@ void launch_asm_step(const AsmStep& s, int batch, int sms, cudaStream_t stream) 
     case 8: asm_step_kernel<8, kAsmRows><<<grid, 256, 0, stream>>>(s); break;
     default: asm_step_kernel<0, 1><<<grid, 256, 0, stream>>>(s); break;
   }
+  return cudaGetLastError();
 }
 
 // Difference mode, second form: TWO rows per warp and the gain products stashed one step ahead.
@@ -673,45 +672,43 @@ size_t asm_diff2_smem_bytes(int n, int np) { return (static_cast<size_t>(3) * np
 template <int NP, bool GEN = false>
 cudaError_t launch_asm_diff2(const AsmStep& s, float* sbuf, int batch, int sms, cudaStream_t stream) {
   const size_t smem = asm_diff2_smem_bytes(s.n, NP);
-  static size_t attr_set = 0;
-  if (smem > 48 * 1024 && smem > attr_set) {
+  if (smem > 48 * 1024) {   // every launch: the attribute belongs to the current device's copy of the function
     cudaError_t e = cudaFuncSetAttribute(asm_diff2_kernel<NP, GEN>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     if (e != cudaSuccess) return e;
-    attr_set = smem;
   }
   const int ptot = (s.T - 1 - s.j) * (s.n / 2);
   const int per_sm = static_cast<int>(std::max<size_t>(1, std::min<size_t>(4, (200u * 1024u) / smem)));
   int cx = (env_int("ASM_WAVES", kAsmWaves) * per_sm * sms + batch - 1) / batch;
   cx = std::max(1, std::min(cx, (ptot + 7) / 8));
   asm_diff2_kernel<NP, GEN><<<dim3(cx, batch), 256, smem, stream>>>(s, sbuf);
-  return cudaSuccess;
+  return cudaGetLastError();
 }
 
 // difference mode: NP = max(pc, p) <= 8
-void launch_asm_step_diff(const AsmStep& s, float* sbuf, bool two_rows, int batch, int sms, cudaStream_t stream) {
+cudaError_t launch_asm_step_diff(const AsmStep& s, float* sbuf, bool two_rows, int batch, int sms, cudaStream_t stream) {
   const int np = std::max(s.pc, s.p);
   if (two_rows) {
     switch (np) {
-      case 1: launch_asm_diff2<1>(s, sbuf, batch, sms, stream); return;
-      case 2: launch_asm_diff2<2>(s, sbuf, batch, sms, stream); return;
-      case 3: launch_asm_diff2<3>(s, sbuf, batch, sms, stream); return;
-      case 4: launch_asm_diff2<4>(s, sbuf, batch, sms, stream); return;
-      case 5: launch_asm_diff2<5>(s, sbuf, batch, sms, stream); return;
-      case 6: launch_asm_diff2<6>(s, sbuf, batch, sms, stream); return;
-      case 7: launch_asm_diff2<7>(s, sbuf, batch, sms, stream); return;
-      default: launch_asm_diff2<8>(s, sbuf, batch, sms, stream); return;
+      case 1: return launch_asm_diff2<1>(s, sbuf, batch, sms, stream);
+      case 2: return launch_asm_diff2<2>(s, sbuf, batch, sms, stream);
+      case 3: return launch_asm_diff2<3>(s, sbuf, batch, sms, stream);
+      case 4: return launch_asm_diff2<4>(s, sbuf, batch, sms, stream);
+      case 5: return launch_asm_diff2<5>(s, sbuf, batch, sms, stream);
+      case 6: return launch_asm_diff2<6>(s, sbuf, batch, sms, stream);
+      case 7: return launch_asm_diff2<7>(s, sbuf, batch, sms, stream);
+      default: return launch_asm_diff2<8>(s, sbuf, batch, sms, stream);
     }
   }
   if (asm_pipe_smem_bytes(s.n, np) <= 200u * 1024u) {
     switch (np) {
-      case 1: launch_asm_step_pipe<1, true>(s, batch, sms, stream); return;
-      case 2: launch_asm_step_pipe<2, true>(s, batch, sms, stream); return;
-      case 3: launch_asm_step_pipe<3, true>(s, batch, sms, stream); return;
-      case 4: launch_asm_step_pipe<4, true>(s, batch, sms, stream); return;
-      case 5: launch_asm_step_pipe<5, true>(s, batch, sms, stream); return;
-      case 6: launch_asm_step_pipe<6, true>(s, batch, sms, stream); return;
-      case 7: launch_asm_step_pipe<7, true>(s, batch, sms, stream); return;
-      default: launch_asm_step_pipe<8, true>(s, batch, sms, stream); return;
+      case 1: return launch_asm_step_pipe<1, true>(s, batch, sms, stream);
+      case 2: return launch_asm_step_pipe<2, true>(s, batch, sms, stream);
+      case 3: return launch_asm_step_pipe<3, true>(s, batch, sms, stream);
+      case 4: return launch_asm_step_pipe<4, true>(s, batch, sms, stream);
+      case 5: return launch_asm_step_pipe<5, true>(s, batch, sms, stream);
+      case 6: return launch_asm_step_pipe<6, true>(s, batch, sms, stream);
+      case 7: return launch_asm_step_pipe<7, true>(s, batch, sms, stream);
+      default: return launch_asm_step_pipe<8, true>(s, batch, sms, stream);
     }
   }
   const int groups = (s.T - 1 - s.j) * ((s.R + kAsmRows - 1) / kAsmRows);
@@ -726,6 +723,7 @@ void launch_asm_step_diff(const AsmStep& s, float* sbuf, bool two_rows, int batc
     case 7: asm_step_kernel<7, kAsmRows, true><<<grid, 256, 0, stream>>>(s); break;
     default: asm_step_kernel<8, kAsmRows, true><<<grid, 256, 0, stream>>>(s); break;
   }
+  return cudaGetLastError();
 }
 
 // Gain-defined controllers: Atil = A + B K, Abar = A + Lt C and both gains transposed, Btt[b,t,q,:] = B[b,t,:,q],
@@ -853,9 +851,9 @@ cudaError_t launch_ofb_response_columns(const OfbArgs& a, cudaStream_t stream, u
     s.T = T; s.n = n; s.p = p; s.R = n; s.is_u = 0; s.j = j;
     {
       ProfScope prof(kProfOfbSupport, stream);
-      launch_asm_step_diff(s, sbuf, two_rows, batch, sms, stream);
+      e = launch_asm_step_diff(s, sbuf, two_rows, batch, sms, stream);
     }
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    if (e != cudaSuccess) return e;
     ++*launches;
   }
   return cudaSuccess;
@@ -867,16 +865,16 @@ size_t asm_workspace_bytes(int batch, int T, int n, int p) {
 }
 
 // x side of the general assembly through the two-row kernel (p <= 8, buffers fit shared memory)
-static void launch_asm_gen2(const AsmStep& s, float* sbuf, int batch, int sms, cudaStream_t stream) {
+static cudaError_t launch_asm_gen2(const AsmStep& s, float* sbuf, int batch, int sms, cudaStream_t stream) {
   switch (s.p) {
-    case 1: launch_asm_diff2<1, true>(s, sbuf, batch, sms, stream); return;
-    case 2: launch_asm_diff2<2, true>(s, sbuf, batch, sms, stream); return;
-    case 3: launch_asm_diff2<3, true>(s, sbuf, batch, sms, stream); return;
-    case 4: launch_asm_diff2<4, true>(s, sbuf, batch, sms, stream); return;
-    case 5: launch_asm_diff2<5, true>(s, sbuf, batch, sms, stream); return;
-    case 6: launch_asm_diff2<6, true>(s, sbuf, batch, sms, stream); return;
-    case 7: launch_asm_diff2<7, true>(s, sbuf, batch, sms, stream); return;
-    default: launch_asm_diff2<8, true>(s, sbuf, batch, sms, stream); return;
+    case 1: return launch_asm_diff2<1, true>(s, sbuf, batch, sms, stream);
+    case 2: return launch_asm_diff2<2, true>(s, sbuf, batch, sms, stream);
+    case 3: return launch_asm_diff2<3, true>(s, sbuf, batch, sms, stream);
+    case 4: return launch_asm_diff2<4, true>(s, sbuf, batch, sms, stream);
+    case 5: return launch_asm_diff2<5, true>(s, sbuf, batch, sms, stream);
+    case 6: return launch_asm_diff2<6, true>(s, sbuf, batch, sms, stream);
+    case 7: return launch_asm_diff2<7, true>(s, sbuf, batch, sms, stream);
+    default: return launch_asm_diff2<8, true>(s, sbuf, batch, sms, stream);
   }
 }
 
@@ -947,9 +945,9 @@ cudaError_t launch_ofb_assemble(const AsmArgs& a, cudaStream_t stream, unsigned 
       s.Cm = a.C; s.Lte = Ltt; s.pc = p;
       {
         ProfScope prof(kProfOfbSupport, stream);
-        if (sd == 0 && two_rows) launch_asm_gen2(s, sbuf, batch, sms, stream); else launch_asm_step(s, batch, sms, stream);
+        e = (sd == 0 && two_rows) ? launch_asm_gen2(s, sbuf, batch, sms, stream) : launch_asm_step(s, batch, sms, stream);
       }
-      if ((e = cudaGetLastError()) != cudaSuccess) return e;
+      if (e != cudaSuccess) return e;
       ++*launches;
     }
   }
