@@ -111,7 +111,8 @@ def _oracle_ofb(A, B, C, K, Lt, w, f):
                                            (132, 5, 6, 6, 2),     # ragged tiles
                                            (100, 4, 1, 1, 1),     # single input, single output
                                            (64, 3, 4, 20, 1),     # wide observation (three groups of 8)
-                                           (300, 5, 3, 5, 2),     # column route: two-row kernel, m != p (zero-padded vectors)
+                                           (300, 5, 3, 5, 2),     # column route: two-row kernel, m < p (zero-padded vectors)
+                                           (164, 4, 7, 2, 1),     # column route: two-row kernel, m > p, ragged tiles
                                            (640, 4, 3, 5, 1),     # column route: one-row shared-memory pipeline in difference mode
                                            (800, 3, 2, 2, 1),     # column route: register kernel in difference mode
                                            (96, 2, 2, 2, 1),      # T = 2: a single block, no product in either route
