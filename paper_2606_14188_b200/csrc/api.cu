@@ -339,14 +339,14 @@ int ltv_scan_rollout_adjoint(const float* A, const float* B, const float* c, con
   // The two scans are independent (g is an input).  Measured on B200: running them side by side pays
   // only when each one, in the configuration it would choose alone, leaves at least half of the SMs idle (one small
   // problem, or few items whose clusters cannot be wider than 16 CTAs); once either saturates HBM on its own the two only
-  // get in each other's way (C2: 0.55 ms side by side on 64 + 64 SMs against 0.25 ms back to back).  So: concurrent when
-  // both fit into half the machine, back to back on the caller's stream otherwise.
+  // get in each other's way (C2: 0.55 ms side by side on 64 + 64 SMs against 0.25 ms back to back).  So: on half the machine
+  // each when both fit there, else each in its own configuration on two streams (the second fills the SMs the first leaves idle).
   RolloutArgs ra{A, B, c, x0, u, x_out, batch, T, n, m};
   AdjointArgs aa{A, B, g, lambda_out, grad_u_out, grad_x0_out, batch, T, n, m};
   const int cfr = rollout_cluster_choice(ra), cfa = adjoint_cluster_choice(aa);
   // Side by side or back to back?  Measured on B200 ("the pair"):
   //  - a scan that ALONE runs on >= 80 % of the SMs with >= 128 rows (columns) per CTA streams at 0.8-1.0 of the HBM peak
-  //    (n = 300 x 64 items): nothing to gain, the two would only get in each other's way -> back to back;
+  //    (n = 300 x 64 items): splitting the SMs would only get the two in each other's way -> each keeps its configuration;
   //  - otherwise each scan alone is short of CTAs (few items: 4 x 16-CTA clusters = 64 SMs) or of work per step (n = 180: two
   //    CTAs per item exchange the state every 1.3 us), and both at once on half the machine each move more, PROVIDED every
   //    cluster of both kernels is resident at the same time - else the last cluster waits for a slot and the pair is slower
@@ -368,6 +368,9 @@ int ltv_scan_rollout_adjoint(const float* A, const float* B, const float* c, con
       cl_r = cl_a = c;
     }
   }
+  // back to back, but on two streams: the second scan's clusters take the SMs the first leaves idle (64 items x 2 CTAs = 128
+  // of 148) and fill in as its clusters finish - clusters are independent, so any interleaving is correct
+  if (!side_by_side && alone_good && option(LTV_OPT_VECTOR_CLUSTER) == 0 && env_int("PAIR_OVERLAP", 1) != 0) side_by_side = true;
   unsigned long long l = 0;
   {
     ProfScope prof(kProfVectorPair, s);
