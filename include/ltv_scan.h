@@ -146,8 +146,8 @@ LTV_API size_t ltv_static_scratch_bytes(void);
 LTV_API int ltv_scan_system_response_tube_static(const float* A, const float* w, float* phi_out, float* r_out,
                                                  int batch, int T, int n, unsigned flags, void* cuda_stream);
 
-/* One SHARD of the system response of the same items: the block ROWS k_lo <= k < k_hi (1 <= k_lo < k_hi <= T) and their tube
- * rows - what one GPU computes when single large items are split over several GPUs (optional; sharding.py has the
+/* One SHARD of the system response of the same items (eq.(12c): the blocks of (I - Z A)^-1; tube rows :147
+ * eq.(12e)): the block ROWS k_lo <= k < k_hi (1 <= k_lo < k_hi <= T) and their tube rows - what one GPU computes when single large items are split over several GPUs (optional; sharding.py has the
  * partition).  The split is by rows because a block row needs nothing outside itself, Phi(k,j) = Phi(k,j+1) A_j with
  * Phi(k,k) = I: every GPU holds A (replicated), no GPU reads another one's blocks, and r_k is COMPLETE on the GPU that owns row
  * k - no reduction over GPUs (summing the zero-initialised r of all shards, or gathering the rows, assembles r).
