@@ -270,3 +270,43 @@ def test_backward_recursion_of_the_general_assembly_equals_eq15():
     assert err < 1e-12
     # the gain-defined controller is the special case Phibar^u(k,j) = K_k Phibar^x(k,j)
     assert np.abs(blk(Puw, 3, 3, m, n)).max() < 1e-12 and np.allclose(blk(Pxw, 3, 3, n, n), np.eye(n))
+
+
+def test_difference_recursion_of_the_gain_defined_response_equals_eq15():
+    """The identity the COLUMN route of ltv_scan_output_feedback_response is built on, against (15) as evaluated by the oracle
+    on dense operators, for a controller given by gains (u = K xhat, Phibar = (I - Z(A + B K))^-1): the difference
+    D = Phi^xw - Phibar^x obeys
+        D(k,j) = D(k,j+1) Abar_j - [Phibar^x(k,j+1) B_j] K_j,   D(k,k) = 0,   Abar_j = A_j + Lt_j C_j,
+    (the general recursion minus Phibar^x(k,j) = Phibar^x(k,j+1)(A_j + B_j K_j)), and Phi^xe(k,j) = D(k,j) Lt_{j-1}: no
+    difference of nearly equal operators appears - which is why the device carries D and not Phi^xw when the gains are small."""
+    from assembly_inputs import blk, observer_operators
+
+    rng = np.random.default_rng(91)
+    T, n, m, p = 7, 6, 2, 3
+    A = np.eye(n)[None] + rng.normal(0.0, 0.4 / np.sqrt(n), (T, n, n))
+    B = rng.normal(0.0, 1.0, (T, n, m))
+    C = rng.normal(0.0, 1.0 / np.sqrt(n), (T, p, n))
+    K = 0.3 * rng.normal(0.0, 1.0 / np.sqrt(n), (T, m, n))
+    Lt = 0.3 * rng.normal(0.0, 1.0, (T, n, p))
+    Atil = A + B @ K
+    PbX = np.eye(T * n)
+    for t, row in O.phi_rows_item(Atil):
+        for s_ in range(t):
+            PbX[t * n:(t + 1) * n, s_ * n:(s_ + 1) * n] = row[s_]
+    PbU = np.vstack([K[k] @ PbX[k * n:(k + 1) * n] for k in range(T)])
+    PhX, PhY = observer_operators(A, Lt, C)
+    Pxw, _, Pxe, _ = O.assemble_output_feedback(A, PbX, PbU, PhX, PhY)
+    Abar = A + Lt @ C
+    err = 0.0
+    for k in range(1, T):
+        D = np.zeros((n, n))
+        for j in range(k - 1, -1, -1):
+            D = D @ Abar[j] - blk(PbX, k, j + 1, n, n) @ B[j] @ K[j]
+            err = max(err, np.abs(D + blk(PbX, k, j, n, n) - blk(Pxw, k, j, n, n)).max())
+            if j >= 1:
+                err = max(err, np.abs(D @ Lt[j - 1] - blk(Pxe, k, j, n, p)).max())
+    assert err < 1e-12
+    # small gains: D is small against Phi^xw, the case in which (Phi^xw - Phibar^x) Lt computed in fp32 loses digits
+    Ks = 1e-4 * K
+    Ds = -(B[0] @ Ks[0])                                   # D(1,0)
+    assert np.abs(Ds).max() < 1e-3 * np.abs(A[0]).max()
