@@ -573,6 +573,35 @@ def next_rows(B, L, W, steps):
         scan = timed(lambda: L.ltv_scan_kalman_gains(As, *ks, Lt_out=Lts, Pi_out=Pis, workspace=wsk, mode=L.LTV_KALMAN_SCAN), 20)
         small[f"kalman_n{ns}_T{Ts}_batch1"] = dict(recursion_single_launch_us=rec * 1e3, riccati_scan_on_request_us=scan * 1e3)
     out["small_problem"] = small
+    # SURVEY 8(e), optional: ONE large item split over GPUs by block rows (no data-path collective).  Measured on this one GPU
+    # shard by shard (a rank's time is its own shard's; the multi-GPU time is the slowest shard), against the whole-item scan.
+    from paper_2606_14188_b200.sharding import row_shard_range
+    from workloads import config, generate
+    del d
+    torch.cuda.empty_cache()
+    n4, T4 = 2400, 16                                       # one item of BASELINE.json configs[3]
+    W4 = generate(config(3, batch=1))
+    A4 = torch.from_numpy(W4.A).to(dev); w4 = torch.from_numpy(W4.w).to(dev)
+    P4 = T4 * (T4 - 1) // 2
+    phi4 = torch.empty((1, P4, n4, n4), device=dev); r4 = torch.empty((1, T4, n4), device=dev)
+    ws4 = torch.empty(max(16, L.ltv_scan_workspace_bytes(L.LTV_OP_SYSTEM_RESPONSE_TUBE, 1, T4, n4, 0)), dtype=torch.uint8, device=dev)
+    shards = dict(item="C4 item: n=2400 T=16 batch=1",
+                  scan_whole_ms=timed(lambda: L.ltv_scan_system_response_tube(A4, w4, phi_out=phi4, r_out=r4, workspace=ws4), 3))
+    del phi4
+    for world in (1, 2, 4, 8):
+        ts = []
+        for rank in range(world):
+            k_lo, k_hi = row_shard_range(T4, rank, world, n=n4)
+            if k_hi <= k_lo:
+                ts.append(0.0)
+                continue
+            po = torch.empty((1, L.ltv_phi_row_shard_blocks(T4, k_lo, k_hi), n4, n4), device=dev)
+            ro = torch.zeros((1, T4, n4), device=dev)
+            ts.append(timed(lambda: L.ltv_scan_system_response_tube_rows(A4, w4, k_lo, k_hi, phi_rows_out=po, r_out=ro), 3))
+            del po
+        shards[f"rows_{world}_shards_ms"] = [round(t, 3) for t in ts]
+    shards["note"] = "each shard timed alone on this GPU; with one GPU per shard the item takes the slowest shard's time"
+    out["row_shards"] = shards
     return out
 
 

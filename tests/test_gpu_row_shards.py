@@ -25,7 +25,7 @@ def L():
     return lib
 
 
-def _check_partition(L, W, world, two_norm=False):
+def _check_partition(L, W, world, two_norm=False, by_time_model=False):
     import torch
 
     batch, T, n, _ = W.shape
@@ -35,7 +35,7 @@ def _check_partition(L, W, world, two_norm=False):
     r_sum = torch.zeros((batch, T, n), device="cuda")
     seen = set()
     for rank in range(world):
-        k_lo, k_hi = row_shard_range(T, rank, world)
+        k_lo, k_hi = row_shard_range(T, rank, world, n=n if by_time_model else None)
         if k_lo == k_hi:
             continue
         phi, r = L.ltv_scan_system_response_tube_rows(A, w, k_lo, k_hi, two_norm=two_norm)
@@ -69,6 +69,12 @@ def _check_partition(L, W, world, two_norm=False):
                                              (96, 3, 1, 4)])      # more ranks than rows: empty shards
 def test_row_shards_assemble_to_the_oracle_response(L, n, T, batch, world):
     _check_partition(L, dense_random(batch, T, n, 2, seed=n + T + world), world)
+
+
+def test_row_shards_of_the_time_model_partition(L):
+    """The partition balanced by modelled time (row_shard_range with the state dimension given) assembles to the same response."""
+    _check_partition(L, dense_random(1, 12, 164, 2, seed=31), 3, by_time_model=True)
+    _check_partition(L, dense_random(2, 7, 300, 2, seed=32), 4, by_time_model=True)
 
 
 def test_row_shards_two_norm_tube_and_config1(L):
