@@ -432,7 +432,7 @@ LTV_API int ltv_scan_operator_constraint_margins(const float* phi_xw, const floa
  * phi_host may be NULL.  *phi_device_out (if not NULL) receives the device address of Phi inside workspace.
  * w_host == NULL skips the system-response / tube stage (rollout + adjoint only, BASELINE.json configs[4]): r_host
  * is then not written and may be NULL, and the workspace need is LTV_OP_PIPELINE_HOST_NO_PHI.
- * The batch is processed in up to eight chunks (LTV_OPT_PIPELINE_CHUNKS; multiples of 4 items): an internal non-blocking copy stream,
+ * The batch is processed in up to sixteen chunks (LTV_OPT_PIPELINE_CHUNKS; multiples of 4 items): an internal non-blocking copy stream,
  * created and destroyed inside the call, uploads chunk i+1 while chunk i is computed on `cuda_stream` (items
  * are independent, so this changes no result); host buffers should be pinned for the copies to overlap. */
 LTV_API int ltv_scan_pipeline_host(const float* A_host, const float* B_host, const float* c_host,
@@ -450,7 +450,7 @@ LTV_API int ltv_scan_pipeline_host(const float* A_host, const float* B_host, con
  *                            0 (default) = chosen by an occupancy / bandwidth model, 1 .. 16 = forced (falls back to 1
  *                            if that cluster cannot be placed).  Used by the tests to cover every cluster size.
  *   LTV_OPT_PIPELINE_CHUNKS  number of batch chunks ltv_scan_pipeline_host overlaps upload and compute over:
- *                            1 .. 16, default 8 (1 = no overlap; C2: 16.0 ms with 4, 15.2 ms with 8 - the upload at PCIe rates is the long leg, more chunks shorten the exposed last compute).
+ *                            1 .. 16, default 16 (1 = no overlap; C2: 16.0 ms with 4, 15.3 ms with 8, 15.1 ms with 16 - the upload at PCIe rates is the long leg, more chunks shorten the exposed last compute).
  *   LTV_OPT_OUTPUT_FEEDBACK_ROUTE  how ltv_scan_output_feedback_response evaluates (15) for n >= 96: 1 = cross scan (log depth,
  *                            4 n^3 products per block), 2 = column recursion (one scan for Phibar^x + the backward recursion
  *                            of ltv_scan_output_feedback_assemble: 2 n^3 products per block, T-1 sequential steps), 0

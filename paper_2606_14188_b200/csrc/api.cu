@@ -45,7 +45,7 @@ unsigned int* dbg_buffer_device() {
 extern "C" LTV_API unsigned int* ltv_debug_buffer(void) { return g_dbg_host; }
 #endif
 
-static std::atomic<int> g_options[LTV_OPT_COUNT] = {{0}, {8}, {0}};
+static std::atomic<int> g_options[LTV_OPT_COUNT] = {{0}, {16}, {0}};
 int option(int which) { return g_options[which].load(std::memory_order_relaxed); }
 
 int pick_cluster_model(int batch, int n, const int* max_active, int sm_budget) {

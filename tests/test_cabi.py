@@ -81,8 +81,10 @@ def test_host_side_validation_needs_no_gpu(L):
     assert L.ltv_phi_block_index_layout(5, 3, 1, L.LTV_PHI_ROW_PACKED) == 4
     assert L.ltv_phi_block_index_layout(5, 3, 1, L.LTV_PHI_SQUARE_GRID) == 16
     assert L.ltv_phi_block_index_layout(5, 3, 1, L.LTV_PHI_COLUMN_PACKED) == L.ltv_phi_block_index(5, 3, 1) == 5
+    chunks0 = L.ltv_get_option(L.LTV_OPT_PIPELINE_CHUNKS)
+    assert chunks0 == 16                                                           # the documented default
     assert L.ltv_set_option(L.LTV_OPT_PIPELINE_CHUNKS, 2) is None and L.ltv_get_option(L.LTV_OPT_PIPELINE_CHUNKS) == 2
-    L.ltv_set_option(L.LTV_OPT_PIPELINE_CHUNKS, 4)
+    L.ltv_set_option(L.LTV_OPT_PIPELINE_CHUNKS, chunks0)
     assert L.lib.ltv_set_option(L.LTV_OPT_VECTOR_CLUSTER, 17) == 2 and L.lib.ltv_set_option(9, 1) == 2
     assert L.ltv_get_option(L.LTV_OPT_VECTOR_CLUSTER) == 0 and L.lib.ltv_get_option(9) == -1
     o = L.lib.ltv_scan_observer_response
