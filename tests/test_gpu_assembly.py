@@ -263,3 +263,26 @@ def test_output_feedback_response_single_step_horizon(L, route):
     finally:
         L.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, 0)
     assert xw.shape[1] == 0 and bool(torch.all(tau == 0))
+
+
+@pytest.mark.parametrize("route", [1, 2])
+def test_output_feedback_response_without_phi_xe(L, route):
+    """phi_xe_out = NULL: Phi^xw and the tube (which still contains the observation term) are unchanged - on both routes."""
+    import torch
+
+    n, T, m, p, batch = 132, 5, 3, 4, 2
+    items = [_gains(T, n, m, p, seed=40 + b) for b in range(batch)]
+    A, B, C, K, Lt = [np.stack([it[q] for it in items]) for q in range(5)]
+    rng = np.random.default_rng(8)
+    w = rng.uniform(0.1, 1.0, (batch, T, n)).astype(np.float32)
+    f = rng.uniform(0.1, 1.0, (batch, T, p)).astype(np.float32)
+    d = [torch.from_numpy(a).cuda() for a in (A, B, K, Lt, C, w, f)]
+    L.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, route)
+    try:
+        xw, xe, tau = L.ltv_scan_output_feedback_response(*d)
+        xw2, xe2, tau2 = L.ltv_scan_output_feedback_response(*d, want_xe=False)
+        torch.cuda.synchronize()
+    finally:
+        L.ltv_set_option(L.LTV_OPT_OUTPUT_FEEDBACK_ROUTE, 0)
+    assert xe is not None and xe2 is None
+    assert torch.equal(xw, xw2) and torch.equal(tau, tau2)      # deterministic: bitwise the same
